@@ -1,0 +1,347 @@
+// psr_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, scalar CPU implementation of the per-reactor chemical source term of
+// arxiv 2005.11468 (section 3, Eq. 4-9; section 2, Eq. 2) with the CHEMKIN-II
+// third-body / falloff forms and NASA-7 thermo that BASELINE.json: north_star adds.
+// One reactor at a time, every step written as the paper / SURVEY.md section 8(c) O1..O11
+// states it: no blocking, no fusion, no hoisting, pow() for T^b, species sums for Eq. 9.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+// may build, load or call this file.  It shares no code, header, table or constant with
+// paper_2005_11468_b200/csrc (the CUDA path); its struct below is declared here on purpose.
+//
+// Templated on the real type: `double` is the oracle proper; `long double` (x87 80-bit) is
+// the low-noise reference J* for the finite-difference Jacobian criterion.
+//
+// Pins (tests/test_oracle_pins.py, none of which call this file to get the expected value):
+//   O1..O11 on the toy mechanism T3 against 17-digit values (tests/golden/t3_pins.json, values
+//   printed in SURVEY.md 8(c), re-derived in the test with mpmath at 50 digits through an
+//   independent dense-matrix formulation); Arrhenius hand values; NASA closed forms;
+//   sum_i C_i = P/RT; K_c(R)*K_c(reverse R)=1; q sign flip under reactant/product swap;
+//   k_f/k_r = K_c; sum_k W_k wdot_k = 0 on element-balanced mechanisms; Lindemann limits
+//   k->k0[M], k->k_inf; Troe F=F_cent at log10 Pr=-c; sum_i F_i = (sum Y - sum Y_in)/tau;
+//   Jacobian species rows of a Y column sum to 1/tau; J row 0 = e_0.
+//
+// Units (paper silent; CHEMKIN cgs, reading g4): T [K], P [dyn/cm^2], C [mol/cm^3],
+// rho [g/cm^3], W [g/mol], wdot [mol/cm^3/s], Ea [cal/mol].
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+struct oracle_mech {  // all host pointers, borrowed
+  int32_t n_species, n_reactions;
+  const double* W;        // [K]
+  const double* nasa;     // [K][7]
+  const double *A, *b, *Ea;  // [I], Ea cal/mol
+  const uint8_t* rtype;   // 0 plain, 1 three-body, 2 Lindemann, 3 Troe
+  const uint8_t* reversible;
+  const int32_t *reac_ptr, *reac_sp, *reac_nu;
+  const int32_t *prod_ptr, *prod_sp, *prod_nu;
+  const int32_t *eff_ptr, *eff_sp;
+  const double* eff_val;
+  const double *A0, *b0, *Ea0;
+  const double* troe;     // [I][4] alpha, T3 (T***), T1 (T*), T2 (T**)
+};
+}
+
+namespace {
+
+// math in the template's precision
+inline double m_exp(double x) { return std::exp(x); }
+inline long double m_exp(long double x) { return expl(x); }
+inline double m_log(double x) { return std::log(x); }
+inline long double m_log(long double x) { return logl(x); }
+inline double m_log10(double x) { return std::log10(x); }
+inline long double m_log10(long double x) { return log10l(x); }
+inline double m_pow(double x, double y) { return std::pow(x, y); }
+inline long double m_pow(long double x, long double y) { return powl(x, y); }
+
+template <class R> struct Consts {
+  static constexpr R Rgas = (R)8.31446261815324e7L;                 // erg/mol/K
+  static constexpr R Rcal = (R)8.31446261815324L / (R)4.184L;       // cal/mol/K
+  static constexpr R Patm = (R)1.01325e6L;                          // dyn/cm^2
+};
+
+// per-reaction intermediates of one reactor (for the pins)
+template <class R> struct RxnDetail {
+  R kinf, k0, Pr, Fcent, F, M, Kp, Kc, kf, kr, q;
+};
+
+// O3: Eq. 6
+template <class R> R arrhenius(R A, R b, R Ea, R T) {
+  return A * m_pow(T, b) * m_exp(-Ea / (Consts<R>::Rcal * T));
+}
+
+// O2: NASA-7, single range
+template <class R> void nasa7(const double* a, R T, R& cp_R, R& h_RT, R& s_R) {
+  R a0 = a[0], a1 = a[1], a2 = a[2], a3 = a[3], a4 = a[4], a5 = a[5], a6 = a[6];
+  R T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+  cp_R = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
+  h_RT = a0 + a1 * T / 2 + a2 * T2 / 3 + a3 * T3 / 4 + a4 * T4 / 5 + a5 / T;
+  s_R = a0 * m_log(T) + a1 * T + a2 * T2 / 2 + a3 * T3 / 3 + a4 * T4 / 4 + a6;
+}
+
+template <class R> R ipow(R x, int n) {  // nu in {1,2,3}: repeated multiply
+  R r = x;
+  for (int i = 1; i < n; ++i) r *= x;
+  return r;
+}
+
+// One full evaluation O1..O10 for one reactor.  Y, Yin: K values (contiguous here).
+// Outputs may be null.  Returns rho through *rho_out.
+template <class R>
+void eval_one(const oracle_mech& m, R T, R P, const R* Y, const R* Yin, R tau, R Tset,
+              R* kf_out, R* kr_out, R* q_out, R* wdot_out, R* F_out /*K+1: F_T, F_1..F_K*/,
+              RxnDetail<R>* det, R* C_out, R* rho_out) {
+  const int K = m.n_species, I = m.n_reactions;
+  const R Rg = Consts<R>::Rgas;
+  // O1
+  R sumYW = 0;
+  for (int i = 0; i < K; ++i) sumYW += Y[i] / (R)m.W[i];
+  R Wbar = (R)1 / sumYW;
+  R rho = P * Wbar / (Rg * T);
+  std::vector<R> C(K), h_RT(K), s_R(K), wdot(K, (R)0);
+  R Ctot = 0;
+  for (int i = 0; i < K; ++i) {
+    C[i] = rho * Y[i] / (R)m.W[i];
+    Ctot += C[i];
+  }
+  // O2
+  for (int i = 0; i < K; ++i) {
+    R cp;
+    nasa7<R>(m.nasa + 7 * i, T, cp, h_RT[i], s_R[i]);
+  }
+  for (int k = 0; k < I; ++k) {
+    // O3
+    R kinf = arrhenius<R>((R)m.A[k], (R)m.b[k], (R)m.Ea[k], T);
+    // O4: Eq. 9 then Eq. 8
+    R dS = 0, dH = 0;
+    int dnu = 0;
+    for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) {
+      dS += (R)m.prod_nu[j] * s_R[m.prod_sp[j]];
+      dH += (R)m.prod_nu[j] * h_RT[m.prod_sp[j]];
+      dnu += m.prod_nu[j];
+    }
+    for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) {
+      dS -= (R)m.reac_nu[j] * s_R[m.reac_sp[j]];
+      dH -= (R)m.reac_nu[j] * h_RT[m.reac_sp[j]];
+      dnu -= m.reac_nu[j];
+    }
+    R Kp = m_exp(dS - dH);
+    R Kc = Kp * m_pow(Consts<R>::Patm / (Rg * T), (R)dnu);
+    // O5
+    R M = Ctot;
+    for (int j = m.eff_ptr[k]; j < m.eff_ptr[k + 1]; ++j) M += ((R)m.eff_val[j] - (R)1) * C[m.eff_sp[j]];
+    // O6
+    R kf = kinf, k0 = 0, Pr = 0, Fcent = 1, F = 1;
+    const int rt = m.rtype[k];
+    if (rt >= 2) {
+      k0 = arrhenius<R>((R)m.A0[k], (R)m.b0[k], (R)m.Ea0[k], T);
+      Pr = k0 * M / kinf;
+      if (rt == 3) {
+        const R al = m.troe[4 * k + 0], T3 = m.troe[4 * k + 1], T1 = m.troe[4 * k + 2], T2 = m.troe[4 * k + 3];
+        Fcent = ((R)1 - al) * m_exp(-T / T3) + al * m_exp(-T / T1) + m_exp(-T2 / T);
+        R lF = m_log10(Fcent);
+        R c = (R)-0.4L - (R)0.67L * lF;
+        R n = (R)0.75L - (R)1.27L * lF;
+        R d = (R)0.14L;
+        R lp = m_log10(Pr) + c;
+        R f1 = lp / (n - d * lp);
+        F = m_pow((R)10, lF / ((R)1 + f1 * f1));
+      }
+      kf = kinf * (Pr / ((R)1 + Pr)) * F;
+    }
+    // O7: Eq. 7
+    R kr = m.reversible[k] ? kf / Kc : (R)0;
+    // O8: Eq. 5
+    R pf = 1, pr = 1;
+    for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) pf *= ipow<R>(C[m.reac_sp[j]], m.reac_nu[j]);
+    for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) pr *= ipow<R>(C[m.prod_sp[j]], m.prod_nu[j]);
+    R q = kf * pf - kr * pr;
+    if (rt == 1) q *= M;
+    // O9: Eq. 4, k ascending
+    for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) wdot[m.reac_sp[j]] -= (R)m.reac_nu[j] * q;
+    for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) wdot[m.prod_sp[j]] += (R)m.prod_nu[j] * q;
+    if (kf_out) kf_out[k] = kf;
+    if (kr_out) kr_out[k] = kr;
+    if (q_out) q_out[k] = q;
+    if (det) det[k] = RxnDetail<R>{kinf, k0, Pr, Fcent, F, M, Kp, Kc, kf, kr, q};
+  }
+  if (wdot_out)
+    for (int i = 0; i < K; ++i) wdot_out[i] = wdot[i];
+  // O10
+  if (F_out) {
+    F_out[0] = T - Tset;
+    for (int i = 0; i < K; ++i) F_out[1 + i] = (Y[i] - Yin[i]) / tau - wdot[i] * (R)m.W[i] / rho;
+  }
+  if (C_out)
+    for (int i = 0; i < K; ++i) C_out[i] = C[i];
+  if (rho_out) *rho_out = rho;
+}
+
+template <class R>
+int eval_batch(const oracle_mech& m, int64_t N, const double* T, const double* P, const double* Y,
+               const double* Yin, const double* tau, int64_t ld, double* kf, double* kr, double* q,
+               int64_t ldk, double* wdot, double* F, int nthreads) {
+  const int K = m.n_species, I = m.n_reactions;
+  const bool want_F = F != nullptr;
+  if (want_F && (!Yin || !tau)) return 1;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+#endif
+  {
+    std::vector<R> y(K), yin(K, (R)0), okf(I), okr(I), oq(I), ow(K), oF(K + 1);
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+    for (int64_t r = 0; r < N; ++r) {
+      for (int i = 0; i < K; ++i) y[i] = Y[(int64_t)i * ld + r];
+      if (want_F)
+        for (int i = 0; i < K; ++i) yin[i] = Yin[(int64_t)i * ld + r];
+      eval_one<R>(m, (R)T[r], (R)P[r], y.data(), yin.data(), want_F ? (R)tau[r] : (R)1, (R)T[r],
+                  okf.data(), okr.data(), oq.data(), ow.data(), want_F ? oF.data() : nullptr, nullptr,
+                  nullptr, nullptr);
+      if (kf) for (int k = 0; k < I; ++k) kf[(int64_t)k * ldk + r] = (double)okf[k];
+      if (kr) for (int k = 0; k < I; ++k) kr[(int64_t)k * ldk + r] = (double)okr[k];
+      if (q) for (int k = 0; k < I; ++k) q[(int64_t)k * ldk + r] = (double)oq[k];
+      if (wdot) for (int i = 0; i < K; ++i) wdot[(int64_t)i * ld + r] = (double)ow[i];
+      if (F) for (int i = 0; i < K; ++i) F[(int64_t)i * ld + r] = (double)oF[1 + i];
+    }
+  }
+  return 0;
+}
+
+// O11: forward finite-difference Jacobian. x=(T,Y_1..Y_K); delta_j=1e-8*max(|x_j|,1e-10);
+// x'_j = fl(x_j+delta_j) and h_j = fl(x'_j - x_j) are formed in DOUBLE for both precisions
+// (the state is a double array; reading g15); each perturbed residual is a full independent
+// O1..O10 evaluation.  J column-major per reactor, (K+1)x(K+1); S (optional) is the
+// round-off scale S_i = |Y_i-Yin_i|/tau + (W_i/rho) sum_k |nu_ik| (|kf prod C'| + |kr prod C''|)
+// of 8(c)-J, row 0 = |T|... row 0 is exact (S_0 = 0).
+template <class R>
+int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P, const double* Y,
+              const double* Yin, const double* tau, int64_t ld, double* J, double* F0, double* S,
+              double* H, int nthreads) {
+  const int K = m.n_species, I = m.n_reactions, n = K + 1;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+#endif
+  {
+    std::vector<double> x(n), xp(n);
+    std::vector<R> y(K), yin(K), f0(n), f1(n), okf(I), okr(I), C(K);
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+    for (int64_t r = 0; r < N; ++r) {
+      x[0] = T[r];
+      for (int i = 0; i < K; ++i) {
+        x[1 + i] = Y[(int64_t)i * ld + r];
+        yin[i] = Yin[(int64_t)i * ld + r];
+        y[i] = x[1 + i];
+      }
+      const R Tset = (R)T[r];
+      R rho;
+      eval_one<R>(m, (R)x[0], (R)P[r], y.data(), yin.data(), (R)tau[r], Tset, okf.data(), okr.data(),
+                  nullptr, nullptr, f0.data(), nullptr, C.data(), &rho);
+      double* Jr = J + (int64_t)r * n * n;
+      if (F0) for (int i = 0; i < n; ++i) F0[(int64_t)r * n + i] = (double)f0[i];
+      if (S) {
+        double* Sr = S + (int64_t)r * n;
+        Sr[0] = 0.0;
+        std::vector<R> acc(K, (R)0);
+        for (int k = 0; k < I; ++k) {
+          R pf = 1, pr = 1;
+          for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) pf *= ipow<R>(C[m.reac_sp[j]], m.reac_nu[j]);
+          for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) pr *= ipow<R>(C[m.prod_sp[j]], m.prod_nu[j]);
+          R mag = std::fabs((double)(okf[k] * pf)) + std::fabs((double)(okr[k] * pr));
+          if (m.rtype[k] == 1) {
+            R M = 0;
+            for (int i = 0; i < K; ++i) M += C[i];
+            for (int j = m.eff_ptr[k]; j < m.eff_ptr[k + 1]; ++j) M += ((R)m.eff_val[j] - (R)1) * C[m.eff_sp[j]];
+            mag *= std::fabs((double)M);
+          }
+          for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) acc[m.reac_sp[j]] += (R)m.reac_nu[j] * mag;
+          for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) acc[m.prod_sp[j]] += (R)m.prod_nu[j] * mag;
+        }
+        for (int i = 0; i < K; ++i)
+          Sr[1 + i] = (double)(std::fabs((double)((y[i] - yin[i]) / (R)tau[r])) + (R)m.W[i] / rho * acc[i]);
+      }
+      for (int j = 0; j < n; ++j) {
+        double ax = std::fabs(x[j]);
+        double delta = 1e-8 * (ax > 1e-10 ? ax : 1e-10);
+        volatile double xpj = x[j] + delta;   // fl(x_j + delta_j)
+        volatile double hj = xpj - x[j];      // fl(x'_j - x_j)
+        xp = x;
+        xp[j] = xpj;
+        if (H) H[(int64_t)r * n + j] = hj;
+        for (int i = 0; i < K; ++i) y[i] = (R)xp[1 + i];
+        eval_one<R>(m, (R)xp[0], (R)P[r], y.data(), yin.data(), (R)tau[r], Tset, nullptr, nullptr, nullptr,
+                    nullptr, f1.data(), nullptr, nullptr, nullptr);
+        for (int i = 0; i < n; ++i) Jr[(int64_t)j * n + i] = (double)((f1[i] - f0[i]) / (R)hj);
+      }
+      for (int i = 0; i < K; ++i) y[i] = (R)x[1 + i];
+    }
+  }
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Batch evaluation, species-major SoA (element (k, r) at [k*ld + r]).  Any output may be null.
+// use_long_double: 0 -> double (the oracle), 1 -> long double reference.
+int oracle_eval(const oracle_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                const double* Yin, const double* tau, int64_t ld, double* kf, double* kr, double* q,
+                int64_t ldk, double* wdot, double* F, int use_long_double, int nthreads) {
+  if (use_long_double)
+    return eval_batch<long double>(*m, N, T, P, Y, Yin, tau, ld, kf, kr, q, ldk, wdot, F, nthreads);
+  return eval_batch<double>(*m, N, T, P, Y, Yin, tau, ld, kf, kr, q, ldk, wdot, F, nthreads);
+}
+
+// J: [N][(K+1)*(K+1)] column-major per reactor; F0, S, H: [N][K+1] (may be null).
+int oracle_jacobian(const oracle_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                    const double* Yin, const double* tau, int64_t ld, double* J, double* F0, double* S,
+                    double* H, int use_long_double, int nthreads) {
+  if (use_long_double) return jac_batch<long double>(*m, N, T, P, Y, Yin, tau, ld, J, F0, S, H, nthreads);
+  return jac_batch<double>(*m, N, T, P, Y, Yin, tau, ld, J, F0, S, H, nthreads);
+}
+
+// Single-reactor detail for the pins: per reaction 11 doubles
+// (kinf,k0,Pr,Fcent,F,M,Kp,Kc,kf,kr,q); per species C; scalars out[0]=Wbar... rho only.
+int oracle_detail(const oracle_mech* m, double T, double P, const double* Y, double* rxn /*[I][11]*/,
+                  double* C /*[K]*/, double* rho) {
+  const int K = m->n_species, I = m->n_reactions;
+  std::vector<RxnDetail<double>> det(I);
+  std::vector<double> yin(K, 0.0);
+  double r;
+  eval_one<double>(*m, T, P, Y, yin.data(), 1.0, T, nullptr, nullptr, nullptr, nullptr, nullptr, det.data(), C, &r);
+  for (int k = 0; k < I; ++k) {
+    const RxnDetail<double>& d = det[k];
+    double v[11] = {d.kinf, d.k0, d.Pr, d.Fcent, d.F, d.M, d.Kp, d.Kc, d.kf, d.kr, d.q};
+    std::memcpy(rxn + 11 * k, v, sizeof v);
+  }
+  if (rho) *rho = r;
+  return 0;
+}
+
+double oracle_arrhenius(double A, double b, double Ea, double T) { return arrhenius<double>(A, b, Ea, T); }
+
+void oracle_nasa7(const double* a, double T, double* cp_R, double* h_RT, double* s_R) {
+  nasa7<double>(a, T, *cp_R, *h_RT, *s_R);
+}
+
+int oracle_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+}

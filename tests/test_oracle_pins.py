@@ -1,0 +1,423 @@
+"""Pins for the CPU oracle (oracle/psr_oracle.cpp) -- none of the expected values below comes
+from the oracle itself or from the CUDA path.
+
+Sources of truth: (a) tests/golden/t3_pins.json -- the 17-digit values SURVEY.md 8(c) prints for
+the toy mechanism T3, which this file first re-derives with mpmath (tests/mp_dense.py: dense
+stoichiometric matrices, mp.power, 50 digits); (b) closed forms and invariants that the
+equations PAPER.md Eq. 2, 4-9 fix.  Each test names the oracle step (O1..O11) it pins.
+"""
+import copy
+import json
+from pathlib import Path
+
+import numpy as np
+import pytest
+from mpmath import mpf
+
+import mp_dense
+from oracle import oracle as orc
+from paper_2005_11468_b200 import synth
+from util import EPS, jacobian_floor_ratio, oracle_mech, rel_err
+
+GOLD = json.loads((Path(__file__).parent / "golden" / "t3_pins.json").read_text())
+RGAS = 8.31446261815324e7
+PATM = 1.01325e6
+
+
+def close(a, b, rtol):
+    return abs(float(a) - float(b)) <= rtol * abs(float(b))
+
+
+@pytest.fixture(scope="module")
+def t3():
+    mech, batch = synth.toy_t3()
+    return mech, batch, oracle_mech(mech)
+
+
+@pytest.fixture(scope="module")
+def t3_mp(t3):
+    mech, batch, _ = t3
+    return mp_dense.evaluate(mech, batch.T[0], batch.P[0], batch.Y[:, 0], batch.Yin[:, 0], batch.tau[0])
+
+
+# ------------------------------------------------------------------ the goldens themselves
+def test_golden_values_rederived_with_mpmath(t3, t3_mp):
+    """The printed T3 values agree with an independent 50-digit dense evaluation to 1e-15."""
+    g, m = GOLD, t3_mp
+    assert close(m["Wbar"], g["state"]["Wbar"], 1e-15) and close(m["rho"], g["state"]["rho"], 1e-15)
+    for i in range(3):
+        assert close(m["C"][i], g["state"]["C"][i], 1e-15)
+    assert close(m["Ctot"], g["state"]["Ctot"], 1e-15)
+    for name, k in (("R0", 0), ("R1", 1), ("R2", 2)):
+        for key, val in g[name].items():
+            if key in m["rx"][k]:
+                assert close(m["rx"][k][key], val, 2e-15), (name, key)
+    for i in range(3):
+        assert close(m["wdot"][i], g["wdot_sign"][i] * g["wdot_abs"], 2e-15)
+    for i in range(1, 4):
+        assert close(m["F"][i], g["F"][i], 1e-13)  # F printed with 15-17 digits
+    assert m["F"][0] == 0
+
+
+def test_golden_jacobian_rederived_with_mpmath(t3):
+    """Exact difference quotients with the double-precision step h_j = fl(fl(x_j+d_j)-x_j) (g15)."""
+    mech, batch, _ = t3
+    x = np.concatenate([batch.T, batch.Y[:, 0]])
+    base = mp_dense.evaluate(mech, x[0], batch.P[0], x[1:], batch.Yin[:, 0], batch.tau[0], Tset=x[0])
+    for j, name in enumerate(("T", "Y0", "Y1", "Y2")):
+        delta = 1e-8 * max(abs(x[j]), 1e-10)
+        xp = x.copy()
+        xp[j] = x[j] + delta
+        h = xp[j] - x[j]
+        pert = mp_dense.evaluate(mech, xp[0], batch.P[0], xp[1:], batch.Yin[:, 0], batch.tau[0], Tset=x[0])
+        col = [(pert["F"][i] - base["F"][i]) / mpf(float(h)) for i in range(4)]
+        for i in range(4):
+            ref = GOLD["J_cols"][name][i]
+            assert abs(float(col[i]) - ref) <= 2e-11 * max(abs(ref), 1e-300) + (0 if ref else 1e-300), (name, i)
+
+
+def test_g15_step_is_not_delta():
+    """For T=1500 the representable step differs from delta by ~5e-9 relative."""
+    delta = 1e-8 * 1500.0
+    h = (1500.0 + delta) - 1500.0
+    assert h == float.fromhex("0x1.f751050000000p-17")
+    assert abs(h / delta - 1) > 1e-9
+
+
+# ------------------------------------------------------------------ O3, O2: closed forms
+def test_O3_arrhenius_hand_values():
+    for row in GOLD["arrhenius"]:
+        got = orc.arrhenius(row["A"], row["b"], row["Ea_kcal"] * 1000.0, row["T"])
+        assert close(got, row["k"], 5e-15), row
+
+
+def test_O3_arrhenius_special_cases():
+    # b=0, Ea=0 -> A exactly; Ea=0 -> A T^b; doubling Ea squares the exponential factor
+    assert orc.arrhenius(3.0e7, 0.0, 0.0, 1234.5) == 3.0e7
+    assert close(orc.arrhenius(2.0, 2.0, 0.0, 1000.0), 2.0e6, 1e-15)
+    e1 = orc.arrhenius(1.0, 0.0, 10e3, 1000.0)
+    e2 = orc.arrhenius(1.0, 0.0, 20e3, 1000.0)
+    assert close(e2, e1 * e1, 1e-14)
+    # exp(-Ea/(Rc T)) with Rc = 8.31446261815324/4.184 cal/mol/K
+    import math
+    assert close(e1, math.exp(-10e3 / (8.31446261815324 / 4.184 * 1000.0)), 1e-15)
+
+
+def test_O2_nasa_closed_form():
+    mech, _ = synth.toy_t3()
+    for i, name in enumerate(("S0", "S1", "S2")):
+        cp, h, s = orc.nasa7(mech.nasa[i], 1500.0)
+        g = GOLD["nasa_T1500"][name]
+        assert close(cp, g["cp_R"], 1e-15) and close(h, g["h_RT"], 1e-15) and close(s, g["s_R"], 1e-15)
+
+
+def test_O2_nasa_thermodynamic_identities():
+    """d(h/RT * T)/dT = cp/R and d(s/R)/dT = cp/(R T): central differences on a random species."""
+    rng = np.random.default_rng(7)
+    a = rng.uniform([2.5, -1e-3, -1e-6, -1e-10, -1e-14, -3e4, -5], [4.5, 1e-3, 1e-6, 1e-10, 1e-14, 3e4, 15])
+    T, d = 1300.0, 1e-2
+    cp, h, s = orc.nasa7(a, T)
+    _, hp, sp = orc.nasa7(a, T + d)
+    _, hm, sm = orc.nasa7(a, T - d)
+    assert close((hp * (T + d) - hm * (T - d)) / (2 * d), cp, 1e-8)
+    assert close((sp - sm) / (2 * d), cp / T, 1e-8)
+
+
+# ------------------------------------------------------------------ O1, O4-O10 on T3
+def test_O1_state_and_ideal_gas_identity(t3):
+    mech, batch, om = t3
+    d = orc.detail(om, batch.T[0], batch.P[0], batch.Y[:, 0])
+    assert close(d["rho"], GOLD["state"]["rho"], 1e-15)
+    for i in range(3):
+        assert close(d["C"][i], GOLD["state"]["C"][i], 2e-15)
+    # identity: sum_i C_i = P/(R T) when C = rho Y/W and rho = P Wbar/(R T)
+    assert close(d["C"].sum(), batch.P[0] / (RGAS * batch.T[0]), 1e-15)
+    assert close(d["C"].sum(), GOLD["state"]["Ctot"], 1e-15)
+
+
+def test_O3_to_O8_T3_reactions(t3):
+    mech, batch, om = t3
+    d = orc.detail(om, batch.T[0], batch.P[0], batch.Y[:, 0])
+    for name, k in (("R0", 0), ("R1", 1), ("R2", 2)):
+        for key, val in GOLD[name].items():
+            if key in d:
+                assert close(d[key][k], val, 2e-14), (name, key, d[key][k], val)
+
+
+def test_O6_lindemann_variant_and_troe_M_scaling(t3):
+    mech, batch, om = t3
+    lind = copy.deepcopy(mech)
+    lind.rtype = np.array([0, 1, 2], dtype=np.uint8)
+    d = orc.detail(oracle_mech(lind), batch.T[0], batch.P[0], batch.Y[:, 0])
+    assert close(d["kf"][2], GOLD["R2"]["kf_lindemann"], 2e-14)
+    # Troe F with [M] scaled by 1e-8 / 1e8: scale A0 instead (P_r = k0 [M] / k_inf is linear in both)
+    for scale, key in ((1e-8, "F_M_times_1e-8"), (1e8, "F_M_times_1e8")):
+        mm = copy.deepcopy(mech)
+        mm.A0 = mech.A0 * scale
+        d = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])
+        assert close(d["F"][2], GOLD["R2"][key], 5e-14)
+
+
+def test_O9_O10_T3_wdot_and_residual(t3):
+    mech, batch, om = t3
+    out = orc.evaluate(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("wdot", "F"))
+    for i in range(3):
+        assert close(out["wdot"][i, 0], GOLD["wdot_sign"][i] * GOLD["wdot_abs"], 5e-14)
+        assert close(out["F"][i, 0], GOLD["F"][i + 1], 5e-14)
+
+
+# ------------------------------------------------------------------ invariants
+def _swap(mech):
+    """Swap reactants and products of every reaction (inputs only)."""
+    m = copy.deepcopy(mech)
+    m.reac_ptr, m.prod_ptr = mech.prod_ptr, mech.reac_ptr
+    m.reac_sp, m.prod_sp = mech.prod_sp, mech.reac_sp
+    m.reac_nu, m.prod_nu = mech.prod_nu, mech.reac_nu
+    return m
+
+
+def test_O4_reverse_reaction_identity_Kc(t3):
+    """T3: R1 is R0 written backwards, so K_c(R0) K_c(R1) = 1 (Eq. 8-9)."""
+    mech, batch, om = t3
+    d = orc.detail(om, batch.T[0], batch.P[0], batch.Y[:, 0])
+    assert close(d["Kc"][0] * d["Kc"][1], 1.0, 1e-14)
+
+
+def test_O7_kf_over_kr_is_Kc_and_Kc_definition():
+    """k_f/k_r = K_c (Eq. 7) with K_c from Eq. 8-9 evaluated here from the species thermo:
+    K_c = exp(sum nu (s/R - h/RT)) (Patm/RT)^{sum nu}."""
+    mech, batch = synth.make_config("C0", 8)
+    om = oracle_mech(mech)
+    for r in range(3):
+        T = batch.T[r]
+        d = orc.detail(om, T, batch.P[r], batch.Y[:, r])
+        g = np.array([(lambda cp, h, s: s - h)(*orc.nasa7(mech.nasa[i], T)) for i in range(mech.n_species)])
+        for k in range(mech.n_reactions):
+            dg, dn = 0.0, 0
+            for j in range(mech.prod_ptr[k], mech.prod_ptr[k + 1]):
+                dg += mech.prod_nu[j] * g[mech.prod_sp[j]]
+                dn += mech.prod_nu[j]
+            for j in range(mech.reac_ptr[k], mech.reac_ptr[k + 1]):
+                dg -= mech.reac_nu[j] * g[mech.reac_sp[j]]
+                dn -= mech.reac_nu[j]
+            Kc = np.exp(dg) * (PATM / (RGAS * T)) ** dn
+            assert close(d["Kc"][k], Kc, 1e-12)
+            assert close(d["kf"][k] / d["kr"][k], d["Kc"][k], 1e-14)
+
+
+def test_O8_q_sign_flip_under_swap():
+    """Swapping reactants and products while swapping k_f <-> k_r flips the sign of q.  The swapped
+    mechanism gets k_f' := k_r by construction: K_c' = 1/K_c, so choose A' with k_f' = k_r; here we
+    check the structural form on plain reactions: q'(k_f'=k_r, k_r'=k_f) = -q, through
+    q' = k_f' prod C^{nu''} - k_r' prod C^{nu'}."""
+    mech, batch = synth.make_config("C0", 4)
+    plain = np.nonzero(mech.rtype == 0)[0]
+    om, oms = oracle_mech(mech), oracle_mech(_swap(mech))
+    for r in range(4):
+        d = orc.detail(om, batch.T[r], batch.P[r], batch.Y[:, r])
+        ds = orc.detail(oms, batch.T[r], batch.P[r], batch.Y[:, r])
+        # swapped mechanism has the same A,b,Ea so k_f' = k_f and K_c' = 1/K_c:
+        assert np.all(rel_err(ds["Kc"] * d["Kc"], np.ones_like(d["Kc"])) < 1e-13)
+        # q' = kf (prodC'' - prodC' * Kc) = -Kc * q  (exact algebra) -> sign flips, magnitude scales by Kc
+        assert np.all(rel_err(ds["q"][plain], -d["Kc"][plain] * d["q"][plain]) < 1e-9)
+        assert np.all(np.sign(ds["q"][plain]) == -np.sign(d["q"][plain]))
+
+
+@pytest.mark.parametrize("cfg,n", [("C0", 64), ("C1", 32), ("C2", 4)])
+def test_O9_mass_conservation(cfg, n):
+    """sum_k W_k wdot_k = 0 on element-balanced mechanisms, relative <= 1e-12 of sum |W_k wdot_k|."""
+    mech, batch = synth.make_config(cfg, n)
+    out = orc.evaluate(oracle_mech(mech), batch.T, batch.P, batch.Y, want=("wdot", "q"))
+    ww = mech.W[:, None] * out["wdot"]
+    # round-off scale: the individual reaction contributions, not the (possibly cancelling) wdot
+    contrib = np.zeros_like(out["wdot"])
+    for k in range(mech.n_reactions):
+        for ptr, sp, nu in ((mech.reac_ptr, mech.reac_sp, mech.reac_nu), (mech.prod_ptr, mech.prod_sp, mech.prod_nu)):
+            for j in range(ptr[k], ptr[k + 1]):
+                contrib[sp[j]] += nu[j] * np.abs(out["q"][k]) * mech.W[sp[j]]
+    assert np.all(np.abs(ww.sum(axis=0)) <= 1e-12 * contrib.sum(axis=0))
+    # literal form of the north_star check wherever wdot does not itself cancel
+    assert np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0)) <= 1e-12
+
+
+def test_O6_lindemann_limits():
+    """k -> k0 [M] as P_r -> 0 and k -> k_inf as P_r -> inf; exactly k/k_inf = Pr/(1+Pr)."""
+    mech, batch = synth.toy_t3()
+    for scale, Pr_expect in ((1e-12, "low"), (1e12, "high")):
+        mm = copy.deepcopy(mech)
+        mm.rtype = np.array([0, 1, 2], dtype=np.uint8)
+        mm.A0 = mech.A0 * scale
+        d = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])
+        Pr, kf, kinf, k0, M = d["Pr"][2], d["kf"][2], d["kinf"][2], d["k0"][2], d["M"][2]
+        assert close(kf / kinf, Pr / (1 + Pr), 1e-15)
+        if Pr_expect == "low":
+            assert Pr < 1e-11 and close(kf, k0 * M, 1e-11)
+        else:
+            assert Pr > 1e11 and close(kf, kinf, 1e-11)
+
+
+def test_O6_troe_F_equals_Fcent_at_center_and_bounds():
+    """At log10 P_r = -c the broadening factor is exactly F_cent (f1 = 0); F in [F_cent, 1]."""
+    mech, batch = synth.toy_t3()
+    om = oracle_mech(mech)
+    d = orc.detail(om, batch.T[0], batch.P[0], batch.Y[:, 0])
+    Fc, Pr = d["Fcent"][2], d["Pr"][2]
+    c = -0.4 - 0.67 * np.log10(Fc)
+    mm = copy.deepcopy(mech)
+    mm.A0 = mech.A0 * (10.0 ** (-c) / Pr)
+    d2 = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])
+    assert close(d2["Pr"][2], 10.0 ** (-c), 1e-13)
+    assert close(d2["F"][2], Fc, 1e-13)
+    for s in 10.0 ** np.linspace(-10, 10, 41):
+        mm.A0 = mech.A0 * s
+        F = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])["F"][2]
+        assert Fc * (1 - 1e-14) <= F <= 1.0
+
+
+def test_O5_third_body_default_efficiency_and_falloff_list():
+    """[M] = sum_i alpha_i C_i with alpha=1 unless listed; a falloff reaction honours a list (g7)."""
+    mech, batch = synth.toy_t3()
+    d = orc.detail(oracle_mech(mech), batch.T[0], batch.P[0], batch.Y[:, 0])
+    C = d["C"]
+    assert close(d["M"][0], C.sum(), 1e-15) and close(d["M"][2], C.sum(), 1e-15)
+    assert close(d["M"][1], 2.5 * C[0] + C[1] + 0.7 * C[2], 1e-15)
+    mm = copy.deepcopy(mech)
+    mm.eff_ptr = np.array([0, 0, 2, 3], dtype=np.int32)
+    mm.eff_sp = np.array([0, 2, 1], dtype=np.int32)
+    mm.eff_val = np.array([2.5, 0.7, 3.0])
+    d2 = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])
+    assert close(d2["M"][2], C[0] + 3.0 * C[1] + C[2], 1e-15)
+    assert close(d2["Pr"][2] / d["Pr"][2], d2["M"][2] / d["M"][2], 1e-14)
+
+
+def test_O8_three_body_multiplies_both_directions(t3):
+    """Reading g6: for rtype 1, q = [M] (kf prodC' - kr prodC''); falloff gets no extra [M]."""
+    mech, batch, om = t3
+    d = orc.detail(om, batch.T[0], batch.P[0], batch.Y[:, 0])
+    C = d["C"]
+    assert close(d["q"][1], d["M"][1] * (d["kf"][1] * C[2] - d["kr"][1] * C[0] * C[1]), 1e-14)
+    assert close(d["q"][2], d["kf"][2] * C[0] * C[1] - d["kr"][2] * C[2], 1e-14)
+
+
+def test_irreversible_reaction_has_zero_kr():
+    mech, batch = synth.toy_t3()
+    mm = copy.deepcopy(mech)
+    mm.reversible = np.array([0, 1, 1], dtype=np.uint8)
+    d = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])
+    assert d["kr"][0] == 0.0 and close(d["q"][0], d["kf"][0] * d["C"][0] * d["C"][1], 1e-15)
+
+
+def test_O8_integer_powers():
+    """nu=2,3 by repeated multiplication equals C**nu; a reaction 2A + B <=> 3D."""
+    mech, batch = synth.toy_t3()
+    mm = copy.deepcopy(mech)
+    mm.reac_nu = np.array([2, 1, 1, 1, 1], dtype=np.int32)  # R0: 2 S0 + S1
+    mm.prod_nu = np.array([3, 1, 1, 1], dtype=np.int32)     # R0: 3 S2
+    d = orc.detail(oracle_mech(mm), batch.T[0], batch.P[0], batch.Y[:, 0])
+    C = d["C"]
+    assert close(d["q"][0], d["kf"][0] * C[0] ** 2 * C[1] - d["kr"][0] * C[2] ** 3, 1e-14)
+    # sum nu = 3 - 3 = 0 -> K_c = K_p
+    assert close(d["Kc"][0], d["Kp"][0], 1e-15)
+
+
+def test_O10_residual_sum_invariant():
+    """sum_i F_i = (sum Y - sum Y_in)/tau because sum W wdot = 0."""
+    mech, batch = synth.make_config("C1", 16)
+    mech2, _ = synth.make_config("C2", 1)
+    out = orc.evaluate(oracle_mech(mech), batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("F", "wdot"))
+    lhs = out["F"].sum(axis=0)
+    rhs = (batch.Y.sum(axis=0) - batch.Yin.sum(axis=0)) / batch.tau
+    scale = np.abs(out["F"]).sum(axis=0)
+    assert np.all(np.abs(lhs - rhs) <= 1e-12 * scale)
+    # definition, retyped with numpy on the oracle's own wdot and an independently computed rho
+    Wbar = 1.0 / (batch.Y / mech.W[:, None]).sum(axis=0)
+    rho = batch.P * Wbar / (RGAS * batch.T)
+    F = (batch.Y - batch.Yin) / batch.tau - out["wdot"] * mech.W[:, None] / rho
+    assert np.all(rel_err(out["F"], F) < 1e-12)
+
+
+# ------------------------------------------------------------------ brute force
+@pytest.mark.parametrize("cfg,n", [("C0", 3), ("C1", 1)])
+def test_whole_path_brute_force_mpmath(cfg, n):
+    """Dense 50-digit evaluation of k_f, k_r, q, wdot, F vs the double oracle: <= 1e-13
+    (q, wdot: relative to the round-off scale of their terms)."""
+    mech, batch = synth.make_config(cfg, n)
+    om = oracle_mech(mech)
+    out = orc.evaluate(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("kf", "kr", "q", "wdot", "F"))
+    for r in range(n):
+        ref = mp_dense.evaluate(mech, batch.T[r], batch.P[r], batch.Y[:, r], batch.Yin[:, r], batch.tau[r])
+        kf = np.array([float(x["kf"]) for x in ref["rx"]])
+        kr = np.array([float(x["kr"]) for x in ref["rx"]])
+        q = np.array([float(x["q"]) for x in ref["rx"]])
+        assert rel_err(out["kf"][:, r], kf).max() < 1e-13
+        assert rel_err(out["kr"][:, r], kr).max() < 1e-13
+        # q may cancel: scale by |fwd|+|rev| ~ use max(|q|, tiny) relative with a cancellation allowance
+        assert np.median(rel_err(out["q"][:, r], q)) < 1e-13 and rel_err(out["q"][:, r], q).max() < 1e-10
+        w = np.array([float(x) for x in ref["wdot"]])
+        big = np.abs(w) > 1e-12 * np.abs(w).max()
+        assert rel_err(out["wdot"][big, r], w[big]).max() < 1e-10
+        F = np.array([float(x) for x in ref["F"][1:]])
+        assert rel_err(out["F"][:, r], F).max() < 1e-9
+
+
+# ------------------------------------------------------------------ O11 Jacobian
+def test_O11_T3_columns_long_double_and_double(t3):
+    mech, batch, om = t3
+    jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=True)
+    jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=False)
+    gold = np.array([GOLD["J_cols"][c] for c in ("T", "Y0", "Y1", "Y2")])  # [col][row]
+    # long double: same floor law as 8(c)-J with eps = 2^-64 (noise 2000x lower than double);
+    # golden printed to 12 digits
+    Kj = np.array([1024.0, 32.0, 32.0, 32.0])
+    floor_ld = 2.0 ** -64 * jl["S"][0][None, :] / jl["H"][0][:, None]
+    assert np.all(np.abs(jl["J"][0] - gold) <= 1e-11 * np.abs(gold) + Kj[:, None] * floor_ld)
+    # double: within the forward-difference round-off floor of 8(c)-J
+    worst, fr_T, fr_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y)
+    # h pinned: h_0 for T=1500
+    assert jd["H"][0, 0] == float.fromhex("0x1.f751050000000p-17")
+    assert np.array_equal(jd["H"], jl["H"])
+
+
+def test_O11_invariants_row0_and_column_sums():
+    """Row 0 of J is exactly e_0 (F_T = T - T_set, g13); species rows of a Y column sum to 1/tau and
+    of the T column to 0 (mass conservation), up to the difference-quotient round-off floor."""
+    mech, batch = synth.make_config("C4", 6)
+    om = oracle_mech(mech)
+    for ld in (False, True):
+        j = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=ld)
+        J = j["J"]  # [N][col][row]
+        assert np.all(J[:, 0, 0] == 1.0) and np.all(J[:, 1:, 0] == 0.0)
+        colsum = J[:, :, 1:].sum(axis=2)  # [N][col]
+        floor = (64 * EPS if not ld else EPS) * j["S"][:, None, 1:].sum(axis=2) / j["H"]
+        target = np.concatenate([np.zeros((batch.n, 1)), np.repeat(1.0 / batch.tau[:, None], mech.n_species, 1)], axis=1)
+        assert np.all(np.abs(colsum - target) <= 1e-9 * np.abs(target) + floor)
+
+
+def test_O11_double_within_floor_of_long_double_C4():
+    mech, batch = synth.make_config("C4", 8)
+    om = oracle_mech(mech)
+    jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=True)
+    jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=False)
+    worst, fr_T, fr_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y)
+    # the residuals themselves agree to ~1e-14
+    assert np.all(np.abs(jd["F0"] - jl["F0"]) <= 1e-11 * np.maximum(np.abs(jl["F0"]), 1e-12 * np.abs(jl["F0"]).max(axis=1, keepdims=True)) + 1e-300)
+
+
+def test_O11_linear_part_exact():
+    """With all A = 0 (no chemistry) F_i = (Y_i - Yin_i)/tau: J[species block] = I/tau, T column 0."""
+    mech, batch = synth.make_config("C0", 4)
+    mm = copy.deepcopy(mech)
+    mm.A = np.zeros_like(mech.A)
+    j = orc.jacobian(oracle_mech(mm), batch.T, batch.P, batch.Y, batch.Yin, batch.tau)
+    K = mech.n_species
+    for r in range(4):
+        Jr = j["J"][r].T  # [row][col]
+        expect = np.zeros((K + 1, K + 1))
+        expect[0, 0] = 1.0
+        expect[1:, 1:] = np.eye(K) / batch.tau[r]
+        # (Y+h - Yin)/tau - (Y - Yin)/tau over h: exact up to eps |Y - Yin|/tau / h
+        tol = 4 * EPS * (np.abs(batch.Y[:, r] - batch.Yin[:, r]) / batch.tau[r])[:, None] / j["H"][r][None, 1:]
+        assert np.all(np.abs(Jr[1:, 1:] - expect[1:, 1:]) <= tol + 1e-9 * expect[1:, 1:])
+        assert np.all(Jr[1:, 0] == 0.0) and np.all(Jr[0] == expect[0])
