@@ -1,0 +1,129 @@
+/* psr.h -- C ABI of the B200 (sm_100a) batched perfectly-stirred-reactor chemistry library.
+ *
+ * The hot path of arxiv 2005.11468 ("Towards using GPGPU units for accelerating the batched PSR
+ * calculations"): for N independent reactors that share one reaction mechanism, evaluate in FP64
+ *   k_f (Eq. 6), K_p/K_c/k_r (Eq. 7-9), the rate of progress q
+ *   (Eq. 5), the net production rate wdot (Eq. 4), the steady
+ *   species residual of PAPER.md:33-35 Eq. 2, and the forward finite-difference Jacobian the Newton
+ *   solver builds from it,
+ * with NASA-7 thermo, third-body concentrations and Lindemann/Troe falloff in their CHEMKIN-II form
+ * (BASELINE.json: north_star; DESIGN.md lists every reading of the paper).
+ * Unlike the paper's three kernels + host loop, every step runs on the device and
+ * nothing returns to the host between them.
+ *
+ * Units (CHEMKIN cgs): T [K], P [dyn/cm^2], Y mass fraction, tau [s], W [g/mol], Ea [cal/mol],
+ * A in (mol/cm^3)^(1-order)/s, C [mol/cm^3], wdot and q [mol/cm^3/s], F [1/s].
+ * Constants: R = 8.31446261815324e7 erg/mol/K, R_c = R/4.184e7 cal/mol/K, P_atm = 1.01325e6.
+ *
+ * Memory: mechanism descriptions are HOST pointers, borrowed for the call.  Reactor state and
+ * outputs are DEVICE pointers owned by the caller, species-major struct-of-arrays: element
+ * (species or reaction k, reactor r) is at base[k*ld + r] with ld >= N, 8-byte aligned.  The
+ * library never frees or keeps caller arrays; inputs and outputs must not alias.
+ *
+ * Execution: every psr_eval_* / psr_fd_jacobian call enqueues kernels on `stream` (a cudaStream_t
+ * cast to void*, NULL = legacy default stream) of the current device and returns without
+ * synchronising.  Calls on one psr_mech from several host threads must be serialised by the caller.
+ *
+ * Errors: every call returns a psr_status; on failure nothing was launched and psr_last_error()
+ * describes why.  N == 0 is PSR_OK.  Non-finite or negative T/Y are not checked and propagate by
+ * IEEE rules.  There is no CPU fallback: without a CUDA device the calls return PSR_ECUDA.
+ */
+#ifndef PSR_H_
+#define PSR_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psr_mech psr_mech; /* opaque; owns the device-side mechanism tables */
+
+typedef enum {
+  PSR_OK = 0,
+  PSR_EINVAL = 1,       /* bad argument or malformed mechanism */
+  PSR_EUNSUPPORTED = 2, /* valid but outside what the kernels handle (see psr_mech_load) */
+  PSR_ENOMEM = 3,
+  PSR_ECUDA = 4,        /* CUDA runtime error or no device */
+  PSR_EIO = 5
+} psr_status;
+
+/* Reaction types (rtype) */
+enum { PSR_RX_PLAIN = 0, PSR_RX_THREE_BODY = 1, PSR_RX_LINDEMANN = 2, PSR_RX_TROE = 3 };
+
+/* Mechanism description: K species, I reactions.  All HOST pointers. */
+typedef struct {
+  int32_t n_species, n_reactions;
+  const double* W;           /* [K]   molar mass, > 0 */
+  const double* nasa;        /* [K][7] NASA-7 a0..a6, one temperature range:
+                                cp/R = a0+a1 T+a2 T^2+a3 T^3+a4 T^4
+                                h/RT = a0+a1 T/2+a2 T^2/3+a3 T^3/4+a4 T^4/5+a5/T
+                                s/R  = a0 ln T+a1 T+a2 T^2/2+a3 T^3/3+a4 T^4/4+a6 */
+  const double *A, *b, *Ea;  /* [I]   k = A T^b exp(-Ea/(R_c T)) (Eq. 6); the high-pressure limit for falloff */
+  const uint8_t* rtype;      /* [I]   PSR_RX_* */
+  const uint8_t* reversible; /* [I]   1: k_r = k_f/K_c (Eq. 7); 0: k_r = 0 */
+  const int32_t *reac_ptr, *reac_sp, *reac_nu; /* CSR over reactions: reactant species and nu' in {1,2,3} */
+  const int32_t *prod_ptr, *prod_sp, *prod_nu; /* products and nu'' in {1,2,3} */
+  const int32_t *eff_ptr, *eff_sp;             /* CSR over reactions: third-body efficiencies (default 1) */
+  const double* eff_val;
+  const double *A0, *b0, *Ea0; /* [I]   low-pressure limit, read when rtype >= 2 */
+  const double* troe;          /* [I][4] alpha, T***, T*, T**, read when rtype == 3 */
+} psr_mech_desc;
+
+/* psr_mech_load: validate the description, build the device tables (per-reaction log-linear rate and
+ * equilibrium coefficients, factor lists, per-chunk CSR of nu^T) and upload them once.
+ * PSR_EINVAL: null pointers, K or I < 1, species index out of range, nu outside 1..3, W <= 0,
+ *   non-monotone CSR pointers, unknown rtype, A <= 0 (A0 <= 0 for falloff).
+ * PSR_EUNSUPPORTED: K > 512, more than 15 concentration factors on one side of a reaction, more
+ *   than 65535 efficiency entries.  *out is set only on PSR_OK.  Synchronous. */
+psr_status psr_mech_load(const psr_mech_desc* desc, psr_mech** out);
+void psr_mech_free(psr_mech* mech);
+
+/* Effective forward and reverse rate constants (reading g18): kf has falloff
+ * applied but no [M] factor; kr = kf/K_c, 0 if irreversible.  kf, kr: [I][ldk], either may be NULL. */
+psr_status psr_eval_kf_kr(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                          const double* Y, int64_t ld, double* kf, double* kr, int64_t ldk, void* stream);
+
+/* Net production rates wdot [K][ld] (Eq. 4) and, if q != NULL, rates of progress q [I][ldq] (Eq. 5). */
+psr_status psr_eval_wdot(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                         const double* Y, int64_t ld, double* wdot, double* q, int64_t ldq, void* stream);
+
+/* PSR species residual F_i = (Y_i - Yin_i)/tau - wdot_i W_i/rho (steady Eq. 2 with tau = rho V/mdot),
+ * F [K][ld]; wdot [K][ld] may be NULL. */
+psr_status psr_eval_residual(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                             const double* Y, const double* Yin, const double* tau, int64_t ld,
+                             double* F, double* wdot, void* stream);
+
+/* Forward finite-difference Jacobian of the residual in x = (T, Y_1..Y_K) (
+ * BASELINE.json configs[4]): delta_j = 1e-8 max(|x_j|, 1e-10), x'_j = fl(x_j + delta_j),
+ * h_j = fl(x'_j - x_j), J_ij = (F_i(x') - F_i(x))/h_j.  Row 0 is the fixed-temperature equation
+ * F_T = T - T_set with T_set the input T, so row 0 of J is e_0.
+ * J: [N][(K+1)*(K+1)], column-major per reactor (entry (i,j) of reactor r at J[r*n*n + j*n + i],
+ * n = K+1), directly usable by a batched LU.  F0: [N][K+1] residual at x (row 0 = 0), may be NULL. */
+psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                           const double* Y, const double* Yin, const double* tau, int64_t ld,
+                           double* J, double* F0, void* stream);
+
+/* Thread-local description of the last failure on this thread; valid until its next psr_* call. */
+const char* psr_last_error(void);
+
+/* Introspection: n_species, n_reactions, reactors per tile, warps per CTA, reactions per chunk,
+ * number of chunks, dynamic shared memory bytes, CTAs per SM the launch is sized for. */
+typedef struct {
+  int32_t n_species, n_reactions, tile, warps, chunk_reactions, n_chunks, smem_bytes, ctas_per_sm;
+  int32_t n_sm, n_falloff, n_third_body, nnz_nu;
+} psr_mech_info_t;
+psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);
+
+/* FP64 pipe probes used for the roofline denominator: run `iters` dependent-
+ * chain iterations of (kind 0) DFMA, (kind 1) exp, (kind 2) log on every SM and return the device
+ * time in milliseconds and the number of operations executed per thread-lane in total.
+ * Synchronous; returns PSR_ECUDA without a device. */
+psr_status psr_probe_fp64(int kind, int iters, double* elapsed_ms, double* ops);
+
+const char* psr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSR_H_ */

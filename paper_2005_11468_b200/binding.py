@@ -1,0 +1,221 @@
+"""Thin ctypes binding over libpsr_b200.so (include/psr.h).  Argument marshalling only: every step
+of the hot path runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and the
+current stream.  There is no CPU fallback: a missing library or device raises."""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from . import build as _build
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libpsr_b200.so"
+
+PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
+_STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
+
+EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
+           "psr_fd_jacobian", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_version")
+
+_DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
+                ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
+                ("reac_nu", np.int32), ("prod_ptr", np.int32), ("prod_sp", np.int32), ("prod_nu", np.int32),
+                ("eff_ptr", np.int32), ("eff_sp", np.int32), ("eff_val", np.float64), ("A0", np.float64),
+                ("b0", np.float64), ("Ea0", np.float64), ("troe", np.float64))
+
+
+class PsrMechDesc(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("n_reactions", C.c_int32)] + [(n, C.c_void_p) for n, _ in _DESC_ARRAYS]
+
+
+class PsrMechInfo(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("n_species", "n_reactions", "tile", "warps", "chunk_reactions", "n_chunks",
+                                         "smem_bytes", "ctas_per_sm", "n_sm", "n_falloff", "n_third_body", "nnz_nu")]
+
+
+class PsrError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load (building first if the sources are newer) the C-ABI library.  Raises if it cannot be had."""
+    global _lib
+    if _lib is None:
+        if _build.needs_build():
+            _build.build()
+        if not _LIB_PATH.exists():
+            raise RuntimeError(f"{_LIB_PATH} is missing: the CUDA extension must be built (python -m paper_2005_11468_b200.build)")
+        L = C.CDLL(str(_LIB_PATH))
+        vp, i64, dp = C.c_void_p, C.c_int64, C.c_void_p
+        L.psr_mech_load.argtypes = [C.POINTER(PsrMechDesc), C.POINTER(vp)]
+        L.psr_mech_load.restype = C.c_int
+        L.psr_mech_free.argtypes = [vp]
+        L.psr_mech_free.restype = None
+        L.psr_eval_kf_kr.argtypes = [vp, i64, dp, dp, dp, i64, dp, dp, i64, vp]
+        L.psr_eval_kf_kr.restype = C.c_int
+        L.psr_eval_wdot.argtypes = [vp, i64, dp, dp, dp, i64, dp, dp, i64, vp]
+        L.psr_eval_wdot.restype = C.c_int
+        L.psr_eval_residual.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
+        L.psr_eval_residual.restype = C.c_int
+        L.psr_fd_jacobian.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
+        L.psr_fd_jacobian.restype = C.c_int
+        L.psr_last_error.argtypes = []
+        L.psr_last_error.restype = C.c_char_p
+        L.psr_mech_info.argtypes = [vp, C.POINTER(PsrMechInfo)]
+        L.psr_mech_info.restype = C.c_int
+        L.psr_probe_fp64.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.psr_probe_fp64.restype = C.c_int
+        L.psr_version.argtypes = []
+        L.psr_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != PSR_OK:
+        raise PsrError(status, lib().psr_last_error().decode())
+
+
+def make_desc(n_species: int, n_reactions: int, arrays: dict):
+    """Build a psr_mech_desc from numpy arrays; returns (desc, keepalive list)."""
+    desc = PsrMechDesc()
+    desc.n_species, desc.n_reactions = int(n_species), int(n_reactions)
+    keep = []
+    for name, dt in _DESC_ARRAYS:
+        a = arrays.get(name)
+        if a is None:
+            setattr(desc, name, None)
+            continue
+        a = np.ascontiguousarray(a, dtype=dt)
+        if a.size == 0:
+            a = np.zeros(1, dtype=dt)
+        keep.append(a)
+        setattr(desc, name, a.ctypes.data)
+    return desc, keep
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _chk_dev(name, t, rows=None, N=None):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
+        raise TypeError(f"{name}: expected a CUDA float64 tensor")
+    if t.dim() == 2 and t.stride(1) != 1:
+        raise ValueError(f"{name}: rows must be contiguous (species-major [K][ld])")
+
+
+class Mechanism:
+    """Device-resident mechanism (psr_mech).  Methods mirror the C ABI one-to-one."""
+
+    def __init__(self, n_species: int, n_reactions: int, arrays: dict):
+        desc, keep = make_desc(n_species, n_reactions, arrays)
+        h = C.c_void_p()
+        _check(lib().psr_mech_load(C.byref(desc), C.byref(h)))
+        self._h = h
+        self.K, self.I = int(n_species), int(n_reactions)
+
+    @classmethod
+    def from_synth(cls, mech):
+        return cls(mech.n_species, mech.n_reactions, mech.arrays())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().psr_mech_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> dict:
+        inf = PsrMechInfo()
+        _check(lib().psr_mech_info(self._h, C.byref(inf)))
+        return {n: getattr(inf, n) for n, _ in PsrMechInfo._fields_}
+
+    # --- psr_eval_kf_kr
+    def eval_kf_kr(self, T, P, Y, kf=None, kr=None):
+        import torch
+        N, ld = T.shape[0], Y.stride(0) if Y.dim() == 2 else T.shape[0]
+        for nm, t in (("T", T), ("P", P), ("Y", Y)):
+            _chk_dev(nm, t)
+        if kf is None:
+            kf = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
+        if kr is None:
+            kr = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
+        _check(lib().psr_eval_kf_kr(self._h, N, _ptr(T), _ptr(P), _ptr(Y), ld, _ptr(kf), _ptr(kr), kf.stride(0), _stream()))
+        return kf, kr
+
+    # --- psr_eval_wdot
+    def eval_wdot(self, T, P, Y, wdot=None, q=None, want_q=False):
+        import torch
+        N, ld = T.shape[0], Y.stride(0)
+        for nm, t in (("T", T), ("P", P), ("Y", Y)):
+            _chk_dev(nm, t)
+        if wdot is None:
+            wdot = torch.empty((self.K, ld), dtype=torch.float64, device=T.device)[:, :N] if ld != N else \
+                torch.empty((self.K, N), dtype=torch.float64, device=T.device)
+        if q is None and want_q:
+            q = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
+        if wdot.stride(0) != ld:
+            raise ValueError("wdot must share the leading dimension of Y")
+        _check(lib().psr_eval_wdot(self._h, N, _ptr(T), _ptr(P), _ptr(Y), ld, _ptr(wdot), _ptr(q),
+                                   q.stride(0) if q is not None else 0, _stream()))
+        return (wdot, q) if (want_q or q is not None) else wdot
+
+    # --- psr_eval_residual
+    def eval_residual(self, T, P, Y, Yin, tau, F=None, wdot=None, want_wdot=False):
+        import torch
+        N, ld = T.shape[0], Y.stride(0)
+        for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)):
+            _chk_dev(nm, t)
+        if Yin.stride(0) != ld:
+            raise ValueError("Yin must share the leading dimension of Y")
+        if F is None:
+            F = torch.empty_like(Y)
+        if wdot is None and want_wdot:
+            wdot = torch.empty_like(Y)
+        _check(lib().psr_eval_residual(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(F),
+                                       _ptr(wdot), _stream()))
+        return (F, wdot) if wdot is not None else F
+
+    # --- psr_fd_jacobian
+    def fd_jacobian(self, T, P, Y, Yin, tau, J=None, F0=None, want_F0=False):
+        import torch
+        N, ld = T.shape[0], Y.stride(0)
+        n = self.K + 1
+        for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)):
+            _chk_dev(nm, t)
+        if J is None:
+            J = torch.empty((N, n, n), dtype=torch.float64, device=T.device)  # J[r, col, row]
+        if F0 is None and want_F0:
+            F0 = torch.empty((N, n), dtype=torch.float64, device=T.device)
+        _check(lib().psr_fd_jacobian(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(J),
+                                     _ptr(F0), _stream()))
+        return (J, F0) if F0 is not None else J
+
+
+def probe_fp64(kind: int, iters: int):
+    """(elapsed_ms, ops) of the FP64 pipe probe (0 DFMA, 1 exp, 2 log)."""
+    ms, ops = C.c_double(), C.c_double()
+    _check(lib().psr_probe_fp64(kind, iters, C.byref(ms), C.byref(ops)))
+    return ms.value, ops.value
+
+
+def version() -> str:
+    return lib().psr_version().decode()

@@ -1,0 +1,523 @@
+// psr_api.cu -- host side of the C ABI in include/psr.h: argument checks, mechanism table
+// construction (psr_tables.h) and kernel launches.  No reactor arithmetic runs on the host.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "../../include/psr.h"
+#include "psr_tables.h"
+
+namespace psr {
+cudaError_t launch_eval(int nw, int spw, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st);
+cudaError_t occupancy_eval(int nw, int spw, size_t smem, int* ctas_per_sm);
+cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st);
+}  // namespace psr
+
+using namespace psr;
+
+struct psr_mech {
+  MechView view{};
+  int nw = 0, spw = 0;
+  int n_sm = 0, ctas_per_sm = 0;
+  int n_falloff = 0, n_third_body = 0, nnz_nu = 0;
+  unsigned char* d_chunks = nullptr;
+  double* d_invW = nullptr;
+  double* d_W = nullptr;
+  double* d_scratch = nullptr;  // internal F0 buffer for psr_fd_jacobian when the caller passes none
+  size_t scratch_bytes = 0;
+  int device = 0;
+};
+
+namespace {
+
+thread_local std::string g_err;
+
+psr_status fail(psr_status st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return st;
+}
+
+psr_status cuda_fail(cudaError_t e, const char* what) {
+  return fail(PSR_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+constexpr long double kRgasL = 8.31446261815324e7L;
+constexpr long double kRcalL = 8.31446261815324L / 4.184L;
+constexpr long double kPatmL = 1.01325e6L;
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+double reaction_cost(int type) {  // relative FP64 cost used to balance warps inside a chunk
+  switch (type) {
+    case PSR_RX_THREE_BODY: return 1.2;
+    case PSR_RX_LINDEMANN: return 1.8;
+    case PSR_RX_TROE: return 4.5;
+    default: return 1.0;
+  }
+}
+
+struct HostRx {
+  RxRec rec;
+  bool has_aux;
+  AuxRec aux;
+  std::vector<EffEnt> eff;
+  std::vector<uint16_t> factors;  // reactants then products
+  std::vector<std::pair<int, int>> nu_net;  // (species, nu''-nu')
+  int type;
+};
+
+}  // namespace
+
+extern "C" {
+
+const char* psr_last_error(void) { return g_err.c_str(); }
+const char* psr_version(void) { return "psr-b200 0.1 (sm_100a)"; }
+
+psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
+  g_err.clear();
+  if (!d || !out) return fail(PSR_EINVAL, "psr_mech_load: null argument");
+  const int K = d->n_species, I = d->n_reactions;
+  if (K < 1 || I < 1) return fail(PSR_EINVAL, "psr_mech_load: need n_species >= 1 and n_reactions >= 1");
+  if (!d->W || !d->nasa || !d->A || !d->b || !d->Ea || !d->rtype || !d->reversible || !d->reac_ptr ||
+      !d->reac_sp || !d->reac_nu || !d->prod_ptr || !d->prod_sp || !d->prod_nu || !d->eff_ptr)
+    return fail(PSR_EINVAL, "psr_mech_load: null array in description");
+  if (K > 512) return fail(PSR_EUNSUPPORTED, "psr_mech_load: n_species %d > 512", K);
+  for (int i = 0; i < K; ++i) {
+    if (!(d->W[i] > 0.0) || !std::isfinite(d->W[i])) return fail(PSR_EINVAL, "W[%d] must be finite and > 0", i);
+    for (int j = 0; j < 7; ++j)
+      if (!std::isfinite(d->nasa[7 * i + j])) return fail(PSR_EINVAL, "nasa[%d][%d] not finite", i, j);
+  }
+  if (d->reac_ptr[0] != 0 || d->prod_ptr[0] != 0 || d->eff_ptr[0] != 0)
+    return fail(PSR_EINVAL, "CSR pointers must start at 0");
+  bool any_fall = false;
+  for (int k = 0; k < I; ++k) {
+    if (d->reac_ptr[k + 1] < d->reac_ptr[k] || d->prod_ptr[k + 1] < d->prod_ptr[k] || d->eff_ptr[k + 1] < d->eff_ptr[k])
+      return fail(PSR_EINVAL, "CSR pointers not monotone at reaction %d", k);
+    if (d->rtype[k] > 3) return fail(PSR_EINVAL, "reaction %d: unknown rtype %d", k, (int)d->rtype[k]);
+    if (!(d->A[k] > 0.0) || !std::isfinite(d->A[k]) || !std::isfinite(d->b[k]) || !std::isfinite(d->Ea[k]))
+      return fail(PSR_EINVAL, "reaction %d: A must be > 0 and A, b, Ea finite", k);
+    if (d->rtype[k] >= 2) any_fall = true;
+  }
+  if (any_fall && (!d->A0 || !d->b0 || !d->Ea0)) return fail(PSR_EINVAL, "falloff reactions need A0, b0, Ea0");
+  if (d->eff_ptr[I] > 0 && (!d->eff_sp || !d->eff_val)) return fail(PSR_EINVAL, "eff_sp/eff_val null");
+  if (d->eff_ptr[I] > 65535) return fail(PSR_EUNSUPPORTED, "more than 65535 efficiency entries");
+
+  // ---- per-reaction host records
+  std::vector<HostRx> rx(I);
+  int n_fall = 0, n_tb = 0, nnz = 0;
+  for (int k = 0; k < I; ++k) {
+    HostRx& h = rx[k];
+    std::memset(&h.rec, 0, sizeof h.rec);
+    std::memset(&h.aux, 0, sizeof h.aux);
+    h.type = d->rtype[k];
+    long double da[7] = {0, 0, 0, 0, 0, 0, 0};
+    int dnu = 0;
+    std::vector<int> net(0);
+    auto side = [&](const int32_t* ptr, const int32_t* sp, const int32_t* nu, int sign, const char* name) -> psr_status {
+      int count = 0;
+      for (int j = ptr[k]; j < ptr[k + 1]; ++j) {
+        if (sp[j] < 0 || sp[j] >= K) return fail(PSR_EINVAL, "reaction %d: %s species index %d out of range", k, name, sp[j]);
+        if (nu[j] < 1 || nu[j] > 3) return fail(PSR_EINVAL, "reaction %d: %s nu=%d outside 1..3", k, name, nu[j]);
+        for (int t = 0; t < nu[j]; ++t) h.factors.push_back((uint16_t)sp[j]);
+        count += nu[j];
+        for (int c = 0; c < 7; ++c) da[c] += (long double)(sign * nu[j]) * (long double)d->nasa[7 * sp[j] + c];
+        dnu += sign * nu[j];
+        bool found = false;
+        for (auto& pr : h.nu_net)
+          if (pr.first == sp[j]) { pr.second += sign * nu[j]; found = true; }
+        if (!found) h.nu_net.push_back({sp[j], sign * nu[j]});
+      }
+      if (count > kMaxSide) return fail(PSR_EUNSUPPORTED, "reaction %d: %d %s factors > %d", k, count, name, kMaxSide);
+      return PSR_OK;
+    };
+    psr_status st = side(d->reac_ptr, d->reac_sp, d->reac_nu, -1, "reactant");
+    if (st != PSR_OK) return st;
+    const int nr = (int)h.factors.size();
+    st = side(d->prod_ptr, d->prod_sp, d->prod_nu, +1, "product");
+    if (st != PSR_OK) return st;
+    const int np = (int)h.factors.size() - nr;
+    h.rec.c[0] = (double)logl((long double)d->A[k]);
+    h.rec.c[1] = d->b[k];
+    h.rec.c[2] = (double)(-(long double)d->Ea[k] / kRcalL);
+    // ln K_c over (1, ln T, 1/T, T, T^2, T^3, T^4)
+    h.rec.d[0] = (double)(da[6] - da[0] + (long double)dnu * logl(kPatmL / kRgasL));
+    h.rec.d[1] = (double)(da[0] - (long double)dnu);
+    h.rec.d[2] = (double)(-da[5]);
+    h.rec.d[3] = (double)(da[1] / 2);
+    h.rec.d[4] = (double)(da[2] / 6);
+    h.rec.d[5] = (double)(da[3] / 12);
+    h.rec.d[6] = (double)(da[4] / 20);
+    h.rec.korig = (uint32_t)k;
+    h.rec.meta = (uint32_t)h.type | (d->reversible[k] ? kMetaRev : 0u) | ((uint32_t)nr << kMetaNrShift) |
+                 ((uint32_t)np << kMetaNpShift);
+    h.has_aux = h.type != PSR_RX_PLAIN;
+    for (int j = d->eff_ptr[k]; j < d->eff_ptr[k + 1]; ++j) {
+      if (d->eff_sp[j] < 0 || d->eff_sp[j] >= K) return fail(PSR_EINVAL, "reaction %d: efficiency species out of range", k);
+      if (!std::isfinite(d->eff_val[j])) return fail(PSR_EINVAL, "reaction %d: efficiency not finite", k);
+      EffEnt e{};
+      e.am1 = d->eff_val[j] - 1.0;
+      e.sp = (uint32_t)d->eff_sp[j];
+      if (h.has_aux) h.eff.push_back(e);  // efficiencies on a plain reaction have no effect
+    }
+    if (h.type >= 2) {
+      if (!(d->A0[k] > 0.0) || !std::isfinite(d->A0[k]) || !std::isfinite(d->b0[k]) || !std::isfinite(d->Ea0[k]))
+        return fail(PSR_EINVAL, "reaction %d: A0 must be > 0 and A0, b0, Ea0 finite", k);
+      h.aux.c0[0] = (double)logl((long double)d->A0[k]);
+      h.aux.c0[1] = d->b0[k];
+      h.aux.c0[2] = (double)(-(long double)d->Ea0[k] / kRcalL);
+      ++n_fall;
+    }
+    if (h.type == PSR_RX_TROE) {
+      if (!d->troe) return fail(PSR_EINVAL, "Troe reactions need the troe array");
+      const double* t = d->troe + 4 * k;
+      h.aux.troe[0] = t[0];
+      h.aux.troe[1] = -1.0 / t[1];
+      h.aux.troe[2] = -1.0 / t[2];
+      h.aux.troe[3] = -t[3];
+    }
+    if (h.type == PSR_RX_THREE_BODY) ++n_tb;
+    for (auto& pr : h.nu_net) nnz += std::abs(pr.second);
+  }
+
+  // ---- launch shape
+  int nw, spw;
+  if (K <= 16) { nw = 8; spw = 2; }
+  else if (K <= 32) { nw = 8; spw = 4; }
+  else if (K <= 64) { nw = 8; spw = 8; }
+  else if (K <= 128) { nw = 16; spw = 8; }
+  else if (K <= 256) { nw = 16; spw = 16; }
+  else { nw = 16; spw = 32; }
+  int rc_target = 128;
+  if (const char* e = getenv("PSR_RC")) rc_target = std::max(8, atoi(e));
+  const int n_chunks = (I + rc_target - 1) / rc_target;
+  const int rc = (I + n_chunks - 1) / n_chunks;
+
+  // ---- distribute reactions over chunks (each type dealt round-robin so chunks cost the same),
+  //      then inside a chunk order by cost and deal to warps in snake order.
+  std::vector<int> order(I);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return reaction_cost(rx[x].type) > reaction_cost(rx[y].type); });
+  std::vector<std::vector<int>> chunk_rx(n_chunks);
+  for (int p = 0; p < I; ++p) chunk_rx[p % n_chunks].push_back(order[p]);
+  for (auto& cr : chunk_rx) {
+    // cr is cost-descending; snake-deal: position = round*nw + warp
+    const int n = (int)cr.size();
+    std::vector<int> placed(n, -1);
+    for (int p = 0; p < n; ++p) {
+      const int round = p / nw, idx = p % nw;
+      const bool last_partial = (round == n / nw);
+      const int warp = (round % 2 == 0 || last_partial) ? idx : nw - 1 - idx;
+      placed[round * nw + warp] = cr[p];
+    }
+    cr = placed;
+  }
+
+  // ---- serialise chunk blobs
+  std::vector<std::vector<unsigned char>> blobs(n_chunks);
+  size_t stride = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const auto& cr = chunk_rx[c];
+    const int n_rx = (int)cr.size();
+    std::vector<RxRec> recs(n_rx);
+    std::vector<AuxRec> auxs;
+    std::vector<EffEnt> effs;
+    std::vector<uint16_t> pool;
+    std::vector<std::vector<uint32_t>> rows(K);
+    for (int kl = 0; kl < n_rx; ++kl) {
+      HostRx& h = rx[cr[kl]];
+      RxRec rec = h.rec;
+      if ((int)h.factors.size() <= kInlineSp) {
+        for (size_t i = 0; i < h.factors.size(); ++i) rec.sp[i] = h.factors[i];
+      } else {
+        const uint32_t off = (uint32_t)pool.size();
+        rec.meta |= kMetaLong;
+        rec.sp[0] = (uint16_t)(off & 0xFFFF);
+        rec.sp[1] = (uint16_t)(off >> 16);
+        pool.insert(pool.end(), h.factors.begin(), h.factors.end());
+      }
+      if (h.has_aux) {
+        AuxRec ax = h.aux;
+        ax.eff_off = (uint32_t)effs.size();
+        ax.n_eff = (uint32_t)h.eff.size();
+        effs.insert(effs.end(), h.eff.begin(), h.eff.end());
+        rec.meta |= (uint32_t)auxs.size() << kMetaAuxShift;
+        auxs.push_back(ax);
+      }
+      recs[kl] = rec;
+      for (auto& pr : h.nu_net)
+        for (int t = 0; t < std::abs(pr.second); ++t)
+          rows[pr.first].push_back((uint32_t)kl | (pr.second < 0 ? kCsrNeg : 0u));
+    }
+    std::vector<uint32_t> cptr(K + 1, 0), cent;
+    for (int s = 0; s < K; ++s) {
+      cptr[s] = (uint32_t)cent.size();
+      cent.insert(cent.end(), rows[s].begin(), rows[s].end());
+    }
+    cptr[K] = (uint32_t)cent.size();
+
+    ChunkHdr hdr{};
+    hdr.n_rx = n_rx;
+    hdr.n_aux = (uint32_t)auxs.size();
+    hdr.n_eff = (uint32_t)effs.size();
+    hdr.n_csr = (uint32_t)cent.size();
+    size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
+    hdr.off_aux = (uint32_t)off;
+    off += sizeof(AuxRec) * auxs.size();
+    hdr.off_eff = (uint32_t)off;
+    off += sizeof(EffEnt) * effs.size();
+    hdr.off_pool = (uint32_t)off;
+    off = align_up(off + 2 * pool.size(), 16);
+    hdr.off_csr_ptr = (uint32_t)off;
+    off = align_up(off + 4 * cptr.size(), 16);
+    hdr.off_csr_ent = (uint32_t)off;
+    off = align_up(off + 4 * cent.size(), 16);
+    hdr.bytes = (uint32_t)off;
+    std::vector<unsigned char>& b = blobs[c];
+    b.assign(off, 0);
+    std::memcpy(b.data(), &hdr, sizeof hdr);
+    std::memcpy(b.data() + sizeof(ChunkHdr), recs.data(), sizeof(RxRec) * n_rx);
+    if (!auxs.empty()) std::memcpy(b.data() + hdr.off_aux, auxs.data(), sizeof(AuxRec) * auxs.size());
+    if (!effs.empty()) std::memcpy(b.data() + hdr.off_eff, effs.data(), sizeof(EffEnt) * effs.size());
+    if (!pool.empty()) std::memcpy(b.data() + hdr.off_pool, pool.data(), 2 * pool.size());
+    std::memcpy(b.data() + hdr.off_csr_ptr, cptr.data(), 4 * cptr.size());
+    if (!cent.empty()) std::memcpy(b.data() + hdr.off_csr_ent, cent.data(), 4 * cent.size());
+    stride = std::max(stride, off);
+  }
+  stride = align_up(stride, 128);
+  std::vector<unsigned char> all(stride * n_chunks, 0);
+  for (int c = 0; c < n_chunks; ++c) std::memcpy(all.data() + stride * c, blobs[c].data(), blobs[c].size());
+
+  // ---- device
+  int dev = 0, n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess || n_dev == 0) return fail(PSR_ECUDA, "psr_mech_load: no CUDA device (%s)", cudaGetErrorString(e));
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDeviceProperties");
+
+  psr_mech* m = new (std::nothrow) psr_mech();
+  if (!m) return fail(PSR_ENOMEM, "psr_mech_load: host allocation failed");
+  m->device = dev;
+  m->nw = nw;
+  m->spw = spw;
+  m->n_sm = prop.multiProcessorCount;
+  m->n_falloff = n_fall;
+  m->n_third_body = n_tb;
+  m->nnz_nu = nnz;
+  MechView& v = m->view;
+  v.K = K;
+  v.I = I;
+  v.n_chunks = n_chunks;
+  v.rc = rc;
+  v.chunk_stride = (uint32_t)stride;
+  size_t o = 0;
+  v.smem_cs = (uint32_t)o;
+  o += align_up((size_t)(K + 2) * kTile * 8, 128);  // K rows of C; K+2 so the Jacobian staging [32][n|1] fits
+  v.smem_q = (uint32_t)o;
+  o += align_up((size_t)rc * kTile * 8, 128);
+  v.smem_mech = (uint32_t)o;
+  o += stride * (n_chunks == 1 ? 1 : 2);
+  v.smem_misc = (uint32_t)o;
+  o += (size_t)2 * nw * 32 * 8 + 64;
+  v.smem_total = (uint32_t)o;
+  if (o > (size_t)prop.sharedMemPerBlockOptin) {
+    delete m;
+    return fail(PSR_EUNSUPPORTED, "mechanism needs %zu bytes of shared memory per CTA, device allows %zu", o,
+                (size_t)prop.sharedMemPerBlockOptin);
+  }
+  std::vector<double> invW(K);
+  for (int i = 0; i < K; ++i) invW[i] = 1.0 / d->W[i];
+  auto cleanup = [&]() { psr_mech_free(m); };
+  if ((e = cudaMalloc(&m->d_chunks, all.size())) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  if ((e = cudaMalloc(&m->d_invW, 8 * K)) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  if ((e = cudaMalloc(&m->d_W, 8 * K)) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  if ((e = cudaMemcpy(m->d_chunks, all.data(), all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_invW, invW.data(), 8 * K, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_W, d->W, 8 * K, cudaMemcpyHostToDevice)) != cudaSuccess) {
+    cleanup();
+    return cuda_fail(e, "cudaMemcpy (mechanism upload)");
+  }
+  v.chunks = m->d_chunks;
+  v.invW = m->d_invW;
+  v.Wm = m->d_W;
+  if ((e = occupancy_eval(nw, spw, v.smem_total, &m->ctas_per_sm)) != cudaSuccess || m->ctas_per_sm < 1) {
+    cleanup();
+    return fail(PSR_ECUDA, "kernel does not fit on this device (%s)", cudaGetErrorString(e));
+  }
+  *out = m;
+  return PSR_OK;
+}
+
+void psr_mech_free(psr_mech* m) {
+  if (!m) return;
+  cudaFree(m->d_chunks);
+  cudaFree(m->d_invW);
+  cudaFree(m->d_W);
+  cudaFree(m->d_scratch);
+  delete m;
+}
+
+psr_status psr_mech_info(const psr_mech* m, psr_mech_info_t* info) {
+  if (!m || !info) return fail(PSR_EINVAL, "psr_mech_info: null argument");
+  info->n_species = m->view.K;
+  info->n_reactions = m->view.I;
+  info->tile = kTile;
+  info->warps = m->nw;
+  info->chunk_reactions = m->view.rc;
+  info->n_chunks = m->view.n_chunks;
+  info->smem_bytes = (int32_t)m->view.smem_total;
+  info->ctas_per_sm = m->ctas_per_sm;
+  info->n_sm = m->n_sm;
+  info->n_falloff = m->n_falloff;
+  info->n_third_body = m->n_third_body;
+  info->nnz_nu = m->nnz_nu;
+  return PSR_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+psr_status check_common(const psr_mech* m, int64_t N, const double* T, const double* P, const double* Y, int64_t ld,
+                        const char* fn) {
+  if (!m) return fail(PSR_EINVAL, "%s: null mechanism", fn);
+  if (N < 0) return fail(PSR_EINVAL, "%s: N < 0", fn);
+  if (N == 0) return PSR_OK;
+  if (!T || !P || !Y) return fail(PSR_EINVAL, "%s: null state array", fn);
+  if (ld < N) return fail(PSR_EINVAL, "%s: ld (%lld) < N (%lld)", fn, (long long)ld, (long long)N);
+  return PSR_OK;
+}
+
+psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
+  const int64_t cap = (int64_t)m->n_sm * m->ctas_per_sm;
+  const int grid = (int)std::min<int64_t>(a.n_tiles, cap);
+  cudaError_t e = launch_eval(m->nw, m->spw, m->view, a, grid, (cudaStream_t)stream);
+  if (e != cudaSuccess) return cuda_fail(e, fn);
+  return PSR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+psr_status psr_eval_kf_kr(const psr_mech* m, int64_t N, const double* T, const double* P, const double* Y, int64_t ld,
+                          double* kf, double* kr, int64_t ldk, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(m, N, T, P, Y, ld, "psr_eval_kf_kr");
+  if (st != PSR_OK || N == 0) return st;
+  if (!kf && !kr) return fail(PSR_EINVAL, "psr_eval_kf_kr: both outputs null");
+  if (ldk < N) return fail(PSR_EINVAL, "psr_eval_kf_kr: ldk < N");
+  EvalArgs a{};
+  a.N = N; a.ld = ld; a.ldk = ldk; a.T = T; a.P = P; a.Y = Y; a.kf = kf; a.kr = kr;
+  a.flags = (kf ? kOutKf : 0u) | (kr ? kOutKr : 0u);
+  a.n_tiles = (N + kTile - 1) / kTile;
+  return run(m, a, stream, "psr_eval_kf_kr");
+}
+
+psr_status psr_eval_wdot(const psr_mech* m, int64_t N, const double* T, const double* P, const double* Y, int64_t ld,
+                         double* wdot, double* q, int64_t ldq, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(m, N, T, P, Y, ld, "psr_eval_wdot");
+  if (st != PSR_OK || N == 0) return st;
+  if (!wdot) return fail(PSR_EINVAL, "psr_eval_wdot: wdot null");
+  if (q && ldq < N) return fail(PSR_EINVAL, "psr_eval_wdot: ldq < N");
+  EvalArgs a{};
+  a.N = N; a.ld = ld; a.ldk = ldq; a.T = T; a.P = P; a.Y = Y; a.wdot = wdot; a.q = q;
+  a.flags = kOutWdot | (q ? kOutQ : 0u);
+  a.n_tiles = (N + kTile - 1) / kTile;
+  return run(m, a, stream, "psr_eval_wdot");
+}
+
+psr_status psr_eval_residual(const psr_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                             const double* Yin, const double* tau, int64_t ld, double* F, double* wdot, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(m, N, T, P, Y, ld, "psr_eval_residual");
+  if (st != PSR_OK || N == 0) return st;
+  if (!Yin || !tau || !F) return fail(PSR_EINVAL, "psr_eval_residual: null Yin, tau or F");
+  EvalArgs a{};
+  a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.F = F; a.wdot = wdot;
+  a.flags = kOutF | (wdot ? kOutWdot : 0u);
+  a.n_tiles = (N + kTile - 1) / kTile;
+  return run(m, a, stream, "psr_eval_residual");
+}
+
+psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const double* P, const double* Y,
+                           const double* Yin, const double* tau, int64_t ld, double* J, double* F0, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(mc, N, T, P, Y, ld, "psr_fd_jacobian");
+  if (st != PSR_OK || N == 0) return st;
+  if (!Yin || !tau || !J) return fail(PSR_EINVAL, "psr_fd_jacobian: null Yin, tau or J");
+  psr_mech* m = const_cast<psr_mech*>(mc);
+  const int64_t n = m->view.K + 1;
+  if (!F0) {
+    const size_t need = (size_t)N * n * 8;
+    if (need > m->scratch_bytes) {
+      cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+      if (e != cudaSuccess) return cuda_fail(e, "psr_fd_jacobian: sync before scratch growth");
+      cudaFree(m->d_scratch);
+      m->d_scratch = nullptr;
+      m->scratch_bytes = 0;
+      if ((e = cudaMalloc(&m->d_scratch, need)) != cudaSuccess) return fail(PSR_ENOMEM, "psr_fd_jacobian: scratch: %s", cudaGetErrorString(e));
+      m->scratch_bytes = need;
+    }
+    F0 = m->d_scratch;
+  }
+  EvalArgs a{};
+  a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.F0out = F0;
+  a.flags = kOutF0;
+  a.n_tiles = (N + kTile - 1) / kTile;
+  st = run(m, a, stream, "psr_fd_jacobian (base residual)");
+  if (st != PSR_OK) return st;
+  EvalArgs b{};
+  b.N = N; b.ld = ld; b.T = T; b.P = P; b.Y = Y; b.Yin = Yin; b.tau = tau; b.J = J; b.F0 = F0;
+  b.flags = kModeJac;
+  b.n_tiles = (N * n + kTile - 1) / kTile;
+  return run(m, b, stream, "psr_fd_jacobian (perturbed sweeps)");
+}
+
+psr_status psr_probe_fp64(int kind, int iters, double* elapsed_ms, double* ops) {
+  g_err.clear();
+  if (kind < 0 || kind > 2 || iters < 1 || !elapsed_ms || !ops) return fail(PSR_EINVAL, "psr_probe_fp64: bad argument");
+  int dev = 0;
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(e, "psr_probe_fp64");
+  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return cuda_fail(e, "psr_probe_fp64");
+  double* sink = nullptr;
+  if ((e = cudaMalloc(&sink, 8)) != cudaSuccess) return cuda_fail(e, "psr_probe_fp64");
+  const int grid = prop.multiProcessorCount * 8;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  launch_probe(kind, iters, grid, sink, 0);  // warm-up
+  cudaEventRecord(e0, 0);
+  e = launch_probe(kind, iters, grid, sink, 0);
+  cudaEventRecord(e1, 0);
+  cudaError_t e2 = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (e != cudaSuccess) return cuda_fail(e, "psr_probe_fp64 launch");
+  if (e2 != cudaSuccess) return cuda_fail(e2, "psr_probe_fp64 sync");
+  *elapsed_ms = ms;
+  *ops = (double)grid * 256.0 * (double)iters * (kind == 0 ? 64.0 : 8.0);
+  return PSR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,95 @@
+// psr_tables.h -- device-side mechanism table layout, shared by the host table builder
+// (psr_api.cu) and the kernels (psr_kernels.cu).  Internal to the library.
+//
+// The mechanism is cut into chunks of at most `rc` reactions.  Every chunk is one contiguous,
+// 16-byte aligned blob that a CTA pulls into shared memory with a single cp.async.bulk:
+//
+//   ChunkHdr | RxRec[n_rx] | AuxRec[n_aux] | EffEnt[n_eff] | u16 pool | u32 csr_ptr[K+1] | u32 csr_ent[n_csr]
+//
+// RxRec carries the log-linear rate forms that replace the paper's per-thread pow()/species sums
+// (Eq. 6, 8, 9):  ln k_f = c0 + c1 ln T + c2/T  and
+//   ln K_c = d0 + d1 ln T + d2/T + d3 T + d4 T^2 + d5 T^3 + d6 T^4,
+// the latter being sum_i nu_ik (s_i/R - h_i/RT) + (sum_i nu_ik) ln(P_atm/(R T)) with the NASA-7
+// polynomials summed per reaction at load time (exact in real arithmetic for a single range).
+#ifndef PSR_TABLES_H_
+#define PSR_TABLES_H_
+#include <stdint.h>
+
+namespace psr {
+
+constexpr int kTile = 32;       // reactors per tile = lanes of a warp
+constexpr int kInlineSp = 8;    // factor species stored inline in a reaction record
+constexpr int kMaxSide = 15;    // concentration factors per reaction side
+
+// meta bits
+constexpr uint32_t kMetaTypeMask = 0x3u;      // PSR_RX_*
+constexpr uint32_t kMetaRev = 0x4u;           // reversible
+constexpr uint32_t kMetaLong = 0x8u;          // factor list lives in the u16 pool at sp[0] | sp[1]<<16
+constexpr int kMetaNrShift = 4;               // bits 4..7  reactant factor count
+constexpr int kMetaNpShift = 8;               // bits 8..11 product factor count
+constexpr int kMetaAuxShift = 16;             // bits 16..31 index into AuxRec[]
+
+struct __attribute__((aligned(16))) RxRec {   // 112 bytes
+  double c[3];            // ln A, b, -Ea/R_c
+  double d[7];            // ln K_c coefficients over (1, ln T, 1/T, T, T^2, T^3, T^4)
+  uint32_t meta;
+  uint32_t korig;         // caller's reaction index (row of kf/kr/q outputs)
+  uint16_t sp[kInlineSp]; // factor species, reactants then products, nu expanded by repetition
+};
+static_assert(sizeof(RxRec) == 112, "RxRec layout");
+
+struct __attribute__((aligned(16))) AuxRec {  // 80 bytes; one per three-body / falloff reaction
+  double c0[3];           // ln A0, b0, -Ea0/R_c (falloff only)
+  double troe[4];         // alpha, -1/T***, -1/T*, -T**
+  uint32_t eff_off, n_eff;
+  uint32_t pad[2];
+};
+static_assert(sizeof(AuxRec) == 80, "AuxRec layout");
+
+struct __attribute__((aligned(16))) EffEnt {  // 16 bytes
+  double am1;             // alpha - 1
+  uint32_t sp;
+  uint32_t pad;
+};
+
+struct __attribute__((aligned(16))) ChunkHdr {  // 64 bytes
+  uint32_t n_rx, n_aux, n_eff, n_csr;
+  uint32_t off_aux, off_eff, off_pool, off_csr_ptr, off_csr_ent;
+  uint32_t bytes;         // bytes to copy (multiple of 16)
+  uint32_t k_first;       // first (sorted) reaction index of this chunk
+  uint32_t pad[5];
+};
+static_assert(sizeof(ChunkHdr) == 64, "ChunkHdr layout");
+
+// csr_ent: bits 0..15 local reaction index, bit 16 sign (1 = subtract).  |nu| > 1 repeats the entry.
+constexpr uint32_t kCsrNeg = 0x10000u;
+
+// Kernel-side view of a loaded mechanism (passed by value as a kernel parameter).
+struct MechView {
+  const unsigned char* chunks;  // n_chunks blobs, chunk_stride bytes apart
+  const double* invW;           // [K] 1/W
+  const double* Wm;             // [K] W
+  int32_t K, I;
+  int32_t n_chunks, rc;
+  uint32_t chunk_stride;        // bytes, multiple of 16
+  uint32_t smem_cs, smem_q, smem_mech, smem_misc, smem_total;  // byte offsets / sizes of the dynamic smem carve-up
+};
+
+// what one launch produces
+enum : uint32_t {
+  kOutWdot = 1u, kOutQ = 2u, kOutKf = 4u, kOutKr = 8u, kOutF = 16u, kModeJac = 32u, kOutF0 = 64u
+};
+
+struct EvalArgs {
+  int64_t N, ld, ldk;
+  const double *T, *P, *Y, *Yin, *tau;
+  double *wdot, *q, *kf, *kr, *F;
+  double *J;              // Jacobian mode output
+  const double* F0;       // Jacobian mode: base residual [N][K+1]
+  double* F0out;          // residual mode: also write [N][K+1] base residual (row 0 = 0)
+  uint32_t flags;
+  int64_t n_tiles;
+};
+
+}  // namespace psr
+#endif

@@ -1,0 +1,258 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Tolerances (BASELINE.json: north_star): max relative error <= 1e-10 on
+k_f, k_r, q and on wdot wherever |wdot| > 1e-12 max|wdot| (per reactor); <= 1e-9 on the residual
+(relative to max(|F_i|, 1e-12 max_i|F_i|)); Jacobian by the floor criterion of SURVEY.md 8(c)-J
+against the long-double oracle J*.
+"""
+import copy
+import json
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2005_11468_b200 import synth
+from util import jacobian_floor_ratio, oracle_mech, rel_err, residual_rel_err, wdot_masked_rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_K = 1e-10
+TOL_F = 1e-9
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def binding(torch_cuda):
+    from paper_2005_11468_b200 import binding as b
+    b.lib()
+    return b
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_eval(torch, binding, mech, batch, want_F=True):
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y = dev(torch, batch.T), dev(torch, batch.P), dev(torch, batch.Y)
+    kf, kr = gm.eval_kf_kr(T, P, Y)
+    wdot, q = gm.eval_wdot(T, P, Y, want_q=True)
+    out = dict(kf=kf.cpu().numpy(), kr=kr.cpu().numpy(), q=q.cpu().numpy(), wdot=wdot.cpu().numpy())
+    if want_F:
+        Yin, tau = dev(torch, batch.Yin), dev(torch, batch.tau)
+        F, w2 = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+        out["F"] = F.cpu().numpy()
+        out["wdot_from_residual"] = w2.cpu().numpy()
+    torch.cuda.synchronize()
+    gm.close()
+    return out
+
+
+def check_against_oracle(mech, batch, got, q_tol=TOL_K):
+    ref = orc.evaluate(oracle_mech(mech), batch.T, batch.P, batch.Y, batch.Yin, batch.tau,
+                       want=("kf", "kr", "q", "wdot", "F"))
+    assert rel_err(got["kf"], ref["kf"]).max() <= TOL_K
+    assert rel_err(got["kr"], ref["kr"]).max() <= TOL_K
+    # q = fwd - rev can cancel; the tolerance applies relative to the larger of |q| and 1e-12 of the
+    # reactor's largest |q| (same masking rule as wdot)
+    qerr, _ = wdot_masked_rel_err(got["q"], ref["q"])
+    assert qerr.max() <= q_tol
+    werr, mask = wdot_masked_rel_err(got["wdot"], ref["wdot"])
+    assert mask.any() and werr.max() <= TOL_K
+    if "F" in got:
+        assert residual_rel_err(got["F"], ref["F"]).max() <= TOL_F
+        assert np.array_equal(got["wdot_from_residual"], got["wdot"])
+    return ref
+
+
+# ------------------------------------------------------------------ configs
+def test_C0_full_kf_kr_q_wdot(torch_cuda, binding):
+    mech, batch = synth.make_config("C0")
+    got = gpu_eval(torch_cuda, binding, mech, batch)
+    check_against_oracle(mech, batch, got)
+
+
+@pytest.mark.parametrize("cfg,n", [("C1", 2000), ("C2", 333), ("C3", 97)])
+def test_configs_ragged_batches(torch_cuda, binding, cfg, n):
+    """Several tiles plus a ragged tail (n not a multiple of 32), all reaction types."""
+    mech, batch = synth.make_config(cfg, n)
+    got = gpu_eval(torch_cuda, binding, mech, batch)
+    check_against_oracle(mech, batch, got)
+
+
+def test_T3_goldens_direct(torch_cuda, binding):
+    """The GPU path against the paper-derived T3 values themselves (tests/golden/t3_pins.json)."""
+    gold = json.loads((Path(__file__).parent / "golden" / "t3_pins.json").read_text())
+    mech, batch = synth.toy_t3()
+    got = gpu_eval(torch_cuda, binding, mech, batch)
+    for k, name in enumerate(("R0", "R1", "R2")):
+        assert abs(got["kf"][k, 0] / gold[name]["kf"] - 1) <= 1e-12
+        assert abs(got["kr"][k, 0] / gold[name]["kr"] - 1) <= 1e-12
+        assert abs(got["q"][k, 0] / gold[name]["q"] - 1) <= 1e-11
+    for i in range(3):
+        assert abs(got["wdot"][i, 0] / (gold["wdot_sign"][i] * gold["wdot_abs"]) - 1) <= 1e-11
+        assert abs(got["F"][i, 0] / gold["F"][i + 1] - 1) <= 1e-11
+
+
+# ------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("n", [1, 31, 32, 33, 64])
+def test_tile_boundaries(torch_cuda, binding, n):
+    mech, batch = synth.make_config("C1", n)
+    got = gpu_eval(torch_cuda, binding, mech, batch)
+    check_against_oracle(mech, batch, got)
+
+
+def test_empty_batch_is_ok(torch_cuda, binding):
+    torch = torch_cuda
+    mech, _ = synth.make_config("C0", 1)
+    gm = binding.Mechanism.from_synth(mech)
+    z = torch.empty(0, dtype=torch.float64, device="cuda")
+    Y = torch.empty((mech.n_species, 0), dtype=torch.float64, device="cuda")
+    w = gm.eval_wdot(z, z, Y)
+    assert w.shape == (mech.n_species, 0)
+    gm.close()
+
+
+def test_leading_dimension_larger_than_N(torch_cuda, binding):
+    torch = torch_cuda
+    mech, batch = synth.make_config("C1", 100)
+    gm = binding.Mechanism.from_synth(mech)
+    ld = 160
+    Ybig = torch.full((mech.n_species, ld), float("nan"), dtype=torch.float64, device="cuda")
+    Ybig[:, :100] = dev(torch, batch.Y)
+    wbig = torch.full((mech.n_species, ld), -7.0, dtype=torch.float64, device="cuda")
+    gm.eval_wdot(dev(torch, batch.T), dev(torch, batch.P), Ybig[:, :100], wdot=wbig[:, :100])
+    ref = orc.evaluate(oracle_mech(mech), batch.T, batch.P, batch.Y, want=("wdot",))
+    w = wbig.cpu().numpy()
+    werr, _ = wdot_masked_rel_err(w[:, :100], ref["wdot"])
+    assert werr.max() <= TOL_K
+    assert np.all(w[:, 100:] == -7.0)  # padding untouched
+    gm.close()
+
+
+def _variant(mech, **kw):
+    m = copy.deepcopy(mech)
+    for k, v in kw.items():
+        setattr(m, k, v)
+    return m
+
+
+def test_lindemann_irreversible_and_falloff_efficiencies(torch_cuda, binding):
+    """Degenerate / rarely used branches: rtype 2, reversible = 0, efficiency list on a falloff
+    reaction (reading g7), nu = 3."""
+    mech, batch = synth.make_config("C1", 70)
+    rtype = mech.rtype.copy()
+    troe_idx = np.nonzero(rtype == 3)[0]
+    rtype[troe_idx[::2]] = 2                      # half the Troe reactions become Lindemann
+    reversible = mech.reversible.copy()
+    reversible[::7] = 0
+    # give the first Troe/Lindemann reactions an efficiency list
+    eff_ptr, eff_sp, eff_val = [0], [], []
+    old_ptr = mech.eff_ptr
+    for k in range(mech.n_reactions):
+        sp = list(mech.eff_sp[old_ptr[k]:old_ptr[k + 1]])
+        val = list(mech.eff_val[old_ptr[k]:old_ptr[k + 1]])
+        if k in troe_idx[:6]:
+            sp, val = [1, 5, 9], [0.3, 2.0, 11.5]
+        eff_sp += sp
+        eff_val += val
+        eff_ptr.append(len(eff_sp))
+    m2 = _variant(mech, rtype=rtype, reversible=reversible, eff_ptr=np.array(eff_ptr, dtype=np.int32),
+                  eff_sp=np.array(eff_sp, dtype=np.int32), eff_val=np.array(eff_val))
+    got = gpu_eval(torch_cuda, binding, m2, batch)
+    ref = check_against_oracle(m2, batch, got)
+    assert np.all(got["kr"][::7] == 0.0) and np.all(ref["kr"][::7] == 0.0)
+
+
+def test_long_factor_lists_and_nu3(torch_cuda, binding):
+    """A reaction with more than 8 concentration factors takes the pooled-list path; nu = 3."""
+    mech, batch = synth.make_config("C0", 40)
+    m = copy.deepcopy(mech)
+    # reaction 0: 3 A + 3 B + 2 C <=> 3 D + 3 E  (8 + 6 = 14 factors), not element balanced -- irrelevant here
+    rp, rs, rn = list(m.reac_ptr), list(m.reac_sp), list(m.reac_nu)
+    pp, ps, pn = list(m.prod_ptr), list(m.prod_sp), list(m.prod_nu)
+    n_old_r, n_old_p = rp[1] - rp[0], pp[1] - pp[0]
+    rs[rp[0]:rp[1]] = [0, 1, 2]
+    rn[rp[0]:rp[1]] = [3, 3, 2]
+    ps[pp[0]:pp[1]] = [3, 4]
+    pn[pp[0]:pp[1]] = [3, 3]
+    rp = [0] + [x + (3 - n_old_r) for x in rp[1:]]
+    pp = [0] + [x + (2 - n_old_p) for x in pp[1:]]
+    m.reac_ptr, m.reac_sp, m.reac_nu = (np.array(x, dtype=np.int32) for x in (rp, rs, rn))
+    m.prod_ptr, m.prod_sp, m.prod_nu = (np.array(x, dtype=np.int32) for x in (pp, ps, pn))
+    m.A = m.A.copy()
+    m.A[0] = 1e40  # keep the 8th-order term visible next to the others
+    got = gpu_eval(torch_cuda, binding, m, batch)
+    check_against_oracle(m, batch, got)
+
+
+def test_negative_and_zero_mass_fractions_propagate(torch_cuda, binding):
+    """Newton iterates may leave [0,1]; products by multiplication keep the sign."""
+    mech, batch = synth.make_config("C1", 64)
+    Y = batch.Y.copy()
+    Y[3, :] = 0.0
+    Y[7, ::2] *= -1e-3
+    b2 = synth.ReactorBatch(batch.T, batch.P, Y, batch.Yin, batch.tau)
+    got = gpu_eval(torch_cuda, binding, mech, b2)
+    check_against_oracle(mech, b2, got)
+
+
+# ------------------------------------------------------------------ full-size launch, sampled
+def test_C1_full_size_sampled(torch_cuda, binding):
+    """BASELINE config 1 at its full batch (65,536 reactors, the launch bench.py times): compare a
+    sample of reactors with the oracle, and check invariants over the whole output."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C1")
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y = dev(torch, batch.T), dev(torch, batch.P), dev(torch, batch.Y)
+    wdot = gm.eval_wdot(T, P, Y).cpu().numpy()
+    gm.close()
+    rng = np.random.default_rng(5)
+    idx = np.sort(rng.choice(batch.n, size=512, replace=False))
+    idx[:3] = [0, 1, 2]
+    idx[-1] = batch.n - 1
+    sub = batch.take(idx)
+    ref = orc.evaluate(oracle_mech(mech), sub.T, sub.P, sub.Y, want=("wdot",))
+    werr, _ = wdot_masked_rel_err(wdot[:, idx], ref["wdot"])
+    assert werr.max() <= TOL_K
+    assert np.all(np.isfinite(wdot))
+    # mass conservation over the whole batch (property that holds at any size)
+    ww = mech.W[:, None] * wdot
+    assert np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0)) <= 1e-12
+
+
+# ------------------------------------------------------------------ Jacobian (a10)
+@pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50)])
+def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
+    torch = torch_cuda
+    mech, batch = synth.make_config(cfg, n)
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    J, F0 = gm.fd_jacobian(*args, want_F0=True)
+    J2 = gm.fd_jacobian(*args)  # internal F0 scratch path
+    torch.cuda.synchronize()
+    J, F0, J2 = J.cpu().numpy(), F0.cpu().numpy(), J2.cpu().numpy()
+    gm.close()
+    assert np.array_equal(J, J2)
+    om = oracle_mech(mech)
+    jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=True)
+    jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=False)
+    # (1) binding criterion against the long-double reference
+    worst, fr_T, fr_Y = jacobian_floor_ratio(J, jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y)
+    # (2) the GPU is no noisier than 4x an independent FP64 CPU code
+    _, od_T, od_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
+    assert fr_T <= 4 * max(od_T, 1.0) and fr_Y <= 4 * max(od_Y, 1.0), (fr_T, od_T, fr_Y, od_Y)
+    # row 0 is e_0 exactly; base residual parity at 1e-9
+    assert np.all(J[:, 0, 0] == 1.0) and np.all(J[:, 1:, 0] == 0.0)
+    assert np.all(F0[:, 0] == 0.0)
+    assert residual_rel_err(F0[:, 1:].T, jd["F0"][:, 1:].T).max() <= TOL_F
