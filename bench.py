@@ -1,0 +1,387 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's measurement contract for the batched PSR chemistry hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A step is one pass of the hot path over BASELINE.json configs[1] ("C1": 53 species / 325
+reactions, 65,536 reactors per GPU): one psr_eval_residual call that produces wdot AND the PSR
+residual F.  The finite-difference Jacobian (row a10, configs[4]) and
+the larger mechanisms are timed once each and reported under "extra"; DESIGN.md says why they are
+not folded into the headline metric.  Inputs are seeded synthetic states (synth.py); nothing here
+reads /root/reference.
+
+value  : reactor wdot evaluations per second, inputs resident in HBM, CUDA-event time on the
+         launching stream, L2 flushed between timed steps.
+e2e    : same metric through the same C-ABI call with HOST (pinned) buffers: H2D of T,P,Y,Yin,tau
+         and D2H of wdot,F inside the timed region.
+--impl reference : the CPU oracle (oracle/), as it stands, on the host cores (the tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "reactor wdot evaluations/sec (FP64, 53sp/325rxn)"
+UNIT = "reactor-evals/s"
+WORKLOAD = "C1: 53 species / 325 reactions (28 three-body, 29 Troe), 65536 reactors per GPU"
+
+# SURVEY.md 8(d) algorithmic FP64 work per reactor evaluation:
+#   exp: 2I + 5 I_troe ; log: 1 + 2 I_troe ; div: 2 + 3 I_troe ;
+#   DFMA-class: 16K + 14I + nnz(nu) + 5 I_tb + 25 I_troe ; exp = 22, log = 28, div = 10 instructions.
+EXP_INSTR, LOG_INSTR, DIV_INSTR = 22.0, 28.0, 10.0
+N_SM, FP64_LANES_PER_SM = 148, 64     # B200: 64 FP64 FMA lanes per SM (37 TFLOP/s nominal)
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of psr_eval_kernel<8,8> on C1, from the
+# ncu --set full capture summarised in profiles/ (None until a capture exists for this kernel).
+NCU_DRAM_BYTES_PER_LAUNCH = None
+
+
+def algorithmic_fp64_instr(K, I, n_tb, n_troe, nnz):
+    n_exp = 2 * I + 5 * n_troe
+    n_log = 1 + 2 * n_troe
+    n_div = 2 + 3 * n_troe
+    dfma = 16 * K + 14 * I + nnz + 5 * n_tb + 25 * n_troe
+    return n_exp * EXP_INSTR + n_log * LOG_INSTR + n_div * DIV_INSTR + dfma
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _one(self):
+        nv = self.nv
+        self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+        except Exception:
+            r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+                 0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown"}
+        for bit, name in names.items():
+            if r & bit:
+                self.reasons.add(name)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._one()
+            except Exception:
+                pass
+            self._stop.wait(0.01)
+
+    def start(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self) -> dict:
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+        if self.nv and not self.samples:
+            try:
+                self._one()
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------ oracle legs
+def _oracle_mech(mech):
+    from oracle import oracle as orc
+    return orc.OracleMechanism.from_arrays(mech.n_species, mech.n_reactions, mech.arrays())
+
+
+def time_oracle(mech, batch, repeats: int):
+    """The oracle as it stands (g++ -O2, OpenMP over reactors) on all host cores of the affinity
+    mask; best of `repeats` passes over `batch`."""
+    from oracle import oracle as orc
+    om = _oracle_mech(mech)
+    cores = min(orc.max_threads(), orc.host_cores())
+    best = float("inf")
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        orc.evaluate(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("wdot", "F"), nthreads=cores)
+        best = min(best, time.perf_counter() - t0)
+    return batch.n / best, cores, best
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host, same metric/config/unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2005_11468_b200 import synth
+    mech, batch = synth.make_config("C1")
+    from oracle import oracle as orc
+    om = _oracle_mech(mech)
+    cores = min(orc.max_threads(), orc.host_cores())
+    # bounded sample of the 65,536-reactor workload per step, sized from a calibration pass so the
+    # whole run stays near two minutes whatever K and W are
+    cal = batch.take(np.arange(2048))
+    t0 = time.perf_counter()
+    orc.evaluate(om, cal.T, cal.P, cal.Y, cal.Yin, cal.tau, want=("wdot", "F"), nthreads=cores)
+    rate = 2048 / (time.perf_counter() - t0)
+    sample_n = int(min(batch.n, max(256, rate * 120.0 / (args.steps + args.warmup))))
+    sub = batch.take(np.arange(sample_n))
+    for _ in range(args.warmup):
+        orc.evaluate(om, sub.T, sub.P, sub.Y, sub.Yin, sub.tau, want=("wdot", "F"), nthreads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.evaluate(om, sub.T, sub.P, sub.Y, sub.Yin, sub.tau, want=("wdot", "F"), nthreads=cores)
+    dt = time.perf_counter() - t0
+    value = sample_n * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": f"first {sample_n} reactors per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"first {sample_n} of 65536 C1 reactors per step, wdot + residual"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2005_11468_b200 import binding, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # weak scaling: every rank owns its own 65,536-reactor batch (independent reactors, no
+    # data-path collective -- SURVEY.md 8(e)); rank r draws the C1 state stream with seed 2001 + 100 r
+    mech, batch = synth.make_config("C1")
+    if rank > 0:
+        batch = synth.make_states(mech.n_species, batch.n, seed=2001 + 100 * rank, **synth.CONFIGS["C1"]["state"])
+    N, K, I = batch.n, mech.n_species, mech.n_reactions
+    gm = binding.Mechanism.from_synth(mech)
+    info = gm.info()
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    F, wdot = torch.empty_like(Y), torch.empty_like(Y)
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")  # 256 MiB > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=wdot)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler.start()
+    for e0, e1 in ev:
+        flush.zero_()                       # L2 flush between timed steps (not timed)
+        e0.record(stream)
+        step()
+        e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    dev_ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
+    if world > 1:
+        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_ms = float(t.item())
+    ms_per_step = dev_ms / args.steps
+    value = world * N * args.steps / (dev_ms * 1e-3)
+
+    # ---- end to end: host pinned buffers in, host pinned buffers out, same C-ABI call
+    h_in = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    h_out = [torch.empty((K, N), dtype=torch.float64).pin_memory() for _ in range(2)]
+    d_in = [torch.empty_like(x, device="cuda") for x in h_in]
+    h2d = sum(x.numel() * 8 for x in h_in)
+    d2h = sum(x.numel() * 8 for x in h_out)
+
+    def e2e_step():
+        for hx, dx in zip(h_in, d_in):
+            dx.copy_(hx, non_blocking=True)
+        gm.eval_residual(d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], F=F, wdot=wdot)
+        h_out[0].copy_(wdot, non_blocking=True)
+        h_out[1].copy_(F, non_blocking=True)
+
+    e2e_steps = max(3, min(args.steps, 20))
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    a1.record(stream)
+    barrier()
+    e2e_ms = a0.elapsed_time(a1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = world * N * e2e_steps / (e2e_ms * 1e-3)
+    assert bool(torch.isfinite(h_out[0]).all())
+
+    # ---- roofline of the dominant (only) kernel: FP64 ALU pipe
+    instr_per_eval = algorithmic_fp64_instr(K, I, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
+    peak = N_SM * FP64_LANES_PER_SM * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12   # T FP64 thread-instr/s
+    achieved = instr_per_eval * N / (ms_per_step * 1e-3) / 1e12
+    probes = {}
+    if rank == 0:
+        for kind, name in ((0, "dfma"), (1, "exp"), (2, "log")):
+            ms, ops = binding.probe_fp64(kind, 2000 if kind == 0 else 500)
+            probes[name + "_per_s"] = ops / (ms * 1e-3)
+    hbm_bytes = (2 + 2 * K) * 8 * N + 2 * K * 8 * N    # T,P,tau~,Y,Yin in ; wdot,F out (tau counted in the 2)
+    roofline = {
+        "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T FP64 thread-instr/s",
+        "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+        "peak_source": "derived: 148 SM x 64 FP64 lanes x clocks.max.sm (DESIGN.md); measured DFMA probe in 'probes'",
+        "instr_per_eval": instr_per_eval, "probes": probes,
+        "hbm": {"algorithmic_bytes_per_launch": hbm_bytes,
+                "achieved_GBps": hbm_bytes / (ms_per_step * 1e-3) / 1e9, "peak_GBps": _hbm_peak()},
+    }
+
+    # ---- extras (rank 0, one GPU): other §8(a) rows timed once each, not part of `value`
+    extra = {}
+    if rank == 0 and not args.no_extra:
+        extra = run_extras(binding, synth, torch, flush)
+
+    # ---- cpu baseline: the oracle as it stands on the host cores, bounded sample (rank 0, N=1)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        sample_n = 4096
+        sub = batch.take(np.arange(sample_n))
+        rate, cores, secs = time_oracle(mech, sub, repeats=1)
+        # grow the sample until it is ~10 s of CPU work
+        target = int(min(N, max(sample_n, rate * 10.0)))
+        if target > sample_n:
+            sub = batch.take(np.arange(target))
+            rate, cores, secs = time_oracle(mech, sub, repeats=1)
+            sample_n = target
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {sample_n} of {N} C1 reactors, wdot + residual, one pass ({secs:.2f} s)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "call": "psr_eval_residual (wdot + F)", "l2": "flushed between timed steps (256 MiB memset)",
+                       "reaction_evals_per_s": value * I, "kernel": info},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps},
+            "gpu_launches": args.steps,
+            "roofline": roofline, "cpu_baseline": cpu, "extra": extra,
+        }
+        print(json.dumps(line), flush=True)
+    gm.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _hbm_peak():
+    p = ROOT / "MEASURED_PEAKS.json"
+    try:
+        return json.loads(p.read_text())["hbm_gbs"]
+    except Exception:
+        return 6650.0   # B200_PROFILING.md fallback
+
+
+def _time_call(torch, fn, flush, reps=5):
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    st = torch.cuda.current_stream()
+    tot = 0.0
+    for _ in range(reps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        fn()
+        e1.record(st)
+        torch.cuda.synchronize()
+        tot += e0.elapsed_time(e1)
+    return tot / reps
+
+
+def run_extras(binding, synth, torch, flush):
+    """C2, C3 residual passes and the C4 FD-Jacobian, timed once each (mean of 5, L2 flushed)."""
+    out = {}
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for cfg in ("C2", "C3", "C4"):
+        mech, batch = synth.make_config(cfg)
+        gm = binding.Mechanism.from_synth(mech)
+        info = gm.info()
+        T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+        instr = algorithmic_fp64_instr(mech.n_species, mech.n_reactions, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
+        if cfg == "C4":
+            n = mech.n_species + 1
+            J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
+            ms = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J), flush)
+            out[cfg] = {"call": "psr_fd_jacobian", "ms": ms, "jacobians_per_s": batch.n / (ms * 1e-3),
+                        "residual_evals_per_s": batch.n * (n + 1) / (ms * 1e-3),
+                        "alu_frac_unhoisted": instr * batch.n * (n + 1) / (ms * 1e-3) / (N_SM * FP64_LANES_PER_SM * 1.965e9)}
+            del J
+        else:
+            F, w = torch.empty_like(Y), torch.empty_like(Y)
+            ms = _time_call(torch, lambda: gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w), flush)
+            out[cfg] = {"call": "psr_eval_residual", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3),
+                        "reaction_evals_per_s": batch.n * mech.n_reactions / (ms * 1e-3),
+                        "alu_frac": instr * batch.n / (ms * 1e-3) / (N_SM * FP64_LANES_PER_SM * 1.965e9)}
+        gm.close()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-extra", action="store_true", help="skip the C2/C3/C4 extras")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

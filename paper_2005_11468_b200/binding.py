@@ -110,11 +110,16 @@ def _stream():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
+def _ld(Y, N):
+    """Leading dimension of a species-major [K][N] tensor (row stride; N for degenerate shapes)."""
+    return max(int(Y.stride(0)), int(N)) if (Y.dim() == 2 and Y.shape[0] > 1 and Y.shape[1] > 1) else int(N)
+
+
 def _chk_dev(name, t, rows=None, N=None):
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
         raise TypeError(f"{name}: expected a CUDA float64 tensor")
-    if t.dim() == 2 and t.stride(1) != 1:
+    if t.dim() == 2 and t.shape[1] > 1 and t.stride(1) != 1:
         raise ValueError(f"{name}: rows must be contiguous (species-major [K][ld])")
 
 
@@ -151,20 +156,22 @@ class Mechanism:
     # --- psr_eval_kf_kr
     def eval_kf_kr(self, T, P, Y, kf=None, kr=None):
         import torch
-        N, ld = T.shape[0], Y.stride(0) if Y.dim() == 2 else T.shape[0]
+        N = T.shape[0]
+        ld = _ld(Y, N)
         for nm, t in (("T", T), ("P", P), ("Y", Y)):
             _chk_dev(nm, t)
         if kf is None:
             kf = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
         if kr is None:
             kr = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
-        _check(lib().psr_eval_kf_kr(self._h, N, _ptr(T), _ptr(P), _ptr(Y), ld, _ptr(kf), _ptr(kr), kf.stride(0), _stream()))
+        _check(lib().psr_eval_kf_kr(self._h, N, _ptr(T), _ptr(P), _ptr(Y), ld, _ptr(kf), _ptr(kr), _ld(kf, N), _stream()))
         return kf, kr
 
     # --- psr_eval_wdot
     def eval_wdot(self, T, P, Y, wdot=None, q=None, want_q=False):
         import torch
-        N, ld = T.shape[0], Y.stride(0)
+        N = T.shape[0]
+        ld = _ld(Y, N)
         for nm, t in (("T", T), ("P", P), ("Y", Y)):
             _chk_dev(nm, t)
         if wdot is None:
@@ -172,19 +179,20 @@ class Mechanism:
                 torch.empty((self.K, N), dtype=torch.float64, device=T.device)
         if q is None and want_q:
             q = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
-        if wdot.stride(0) != ld:
+        if _ld(wdot, N) != ld:
             raise ValueError("wdot must share the leading dimension of Y")
         _check(lib().psr_eval_wdot(self._h, N, _ptr(T), _ptr(P), _ptr(Y), ld, _ptr(wdot), _ptr(q),
-                                   q.stride(0) if q is not None else 0, _stream()))
+                                   _ld(q, N) if q is not None else 0, _stream()))
         return (wdot, q) if (want_q or q is not None) else wdot
 
     # --- psr_eval_residual
     def eval_residual(self, T, P, Y, Yin, tau, F=None, wdot=None, want_wdot=False):
         import torch
-        N, ld = T.shape[0], Y.stride(0)
+        N = T.shape[0]
+        ld = _ld(Y, N)
         for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)):
             _chk_dev(nm, t)
-        if Yin.stride(0) != ld:
+        if _ld(Yin, N) != ld:
             raise ValueError("Yin must share the leading dimension of Y")
         if F is None:
             F = torch.empty_like(Y)
@@ -197,7 +205,8 @@ class Mechanism:
     # --- psr_fd_jacobian
     def fd_jacobian(self, T, P, Y, Yin, tau, J=None, F0=None, want_F0=False):
         import torch
-        N, ld = T.shape[0], Y.stride(0)
+        N = T.shape[0]
+        ld = _ld(Y, N)
         n = self.K + 1
         for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)):
             _chk_dev(nm, t)
