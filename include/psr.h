@@ -121,6 +121,10 @@ psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);
  * Synchronous; returns PSR_ECUDA without a device. */
 psr_status psr_probe_fp64(int kind, int iters, double* elapsed_ms, double* ops);
 
+/* Diagnostic: evaluate the kernels' table-driven exp (csrc/psr_math.cuh) on n HOST values x -> y
+ * (HOST).  Synchronous, default stream.  Used by the tests to pin its accuracy. */
+psr_status psr_probe_exp_values(const psr_mech* mech, const double* x, double* y, int32_t n);
+
 const char* psr_version(void);
 
 #ifdef __cplusplus

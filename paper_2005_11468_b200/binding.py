@@ -17,7 +17,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_fd_jacobian", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_version")
+           "psr_fd_jacobian", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -72,6 +72,8 @@ def lib():
         L.psr_mech_info.restype = C.c_int
         L.psr_probe_fp64.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.psr_probe_fp64.restype = C.c_int
+        L.psr_probe_exp_values.argtypes = [vp, dp, dp, C.c_int32]
+        L.psr_probe_exp_values.restype = C.c_int
         L.psr_version.argtypes = []
         L.psr_version.restype = C.c_char_p
         _lib = L
@@ -152,6 +154,13 @@ class Mechanism:
         inf = PsrMechInfo()
         _check(lib().psr_mech_info(self._h, C.byref(inf)))
         return {n: getattr(inf, n) for n, _ in PsrMechInfo._fields_}
+
+    def probe_exp_values(self, x):
+        """The kernels' exp on a host float64 array (diagnostic, psr_probe_exp_values)."""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.empty_like(x)
+        _check(lib().psr_probe_exp_values(self._h, x.ctypes.data, y.ctypes.data, x.size))
+        return y
 
     # --- psr_eval_kf_kr
     def eval_kf_kr(self, T, P, Y, kf=None, kr=None):

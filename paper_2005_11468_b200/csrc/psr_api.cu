@@ -17,21 +17,24 @@
 #include "psr_tables.h"
 
 namespace psr {
-cudaError_t launch_eval(int nw, int spw, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st);
-cudaError_t occupancy_eval(int nw, int spw, size_t smem, int* ctas_per_sm);
+cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st);
+cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm);
 cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st);
+cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
 }  // namespace psr
 
 using namespace psr;
 
 struct psr_mech {
   MechView view{};
-  int nw = 0, spw = 0;
+  int nw = 0, spw = 0, rl = 1;  // warps per CTA, species per warp, reactors per lane
+  int tile = kTile;             // evaluation states per tile = 32 * rl
   int n_sm = 0, ctas_per_sm = 0;
   int n_falloff = 0, n_third_body = 0, nnz_nu = 0;
   unsigned char* d_chunks = nullptr;
   double* d_invW = nullptr;
   double* d_W = nullptr;
+  double* d_exptab = nullptr;
   double* d_scratch = nullptr;  // internal F0 buffer for psr_fd_jacobian when the caller passes none
   size_t scratch_bytes = 0;
   int device = 0;
@@ -78,6 +81,7 @@ struct HostRx {
   std::vector<uint16_t> factors;  // reactants then products
   std::vector<std::pair<int, int>> nu_net;  // (species, nu''-nu')
   int type;
+  int nr = 0, np = 0;
 };
 
 }  // namespace
@@ -150,27 +154,33 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     st = side(d->prod_ptr, d->prod_sp, d->prod_nu, +1, "product");
     if (st != PSR_OK) return st;
     const int np = (int)h.factors.size() - nr;
-    h.rec.c[0] = (double)logl((long double)d->A[k]);
+    const long double lnA = logl((long double)d->A[k]);
+    const long double mEaR = -(long double)d->Ea[k] / kRcalL;
+    h.rec.c[0] = (double)lnA;
     h.rec.c[1] = d->b[k];
-    h.rec.c[2] = (double)(-(long double)d->Ea[k] / kRcalL);
-    // ln K_c over (1, ln T, 1/T, T, T^2, T^3, T^4)
-    h.rec.d[0] = (double)(da[6] - da[0] + (long double)dnu * logl(kPatmL / kRgasL));
-    h.rec.d[1] = (double)(da[0] - (long double)dnu);
-    h.rec.d[2] = (double)(-da[5]);
-    h.rec.d[3] = (double)(da[1] / 2);
-    h.rec.d[4] = (double)(da[2] / 6);
-    h.rec.d[5] = (double)(da[3] / 12);
-    h.rec.d[6] = (double)(da[4] / 20);
+    h.rec.c[2] = (double)mEaR;
+    // ln K_c over (1, ln T, 1/T, T, T^2, T^3, T^4); the record stores ln k_r = ln k_f - ln K_c
+    const long double kc0 = da[6] - da[0] + (long double)dnu * logl(kPatmL / kRgasL);
+    const long double kc1 = da[0] - (long double)dnu;
+    const long double kc2 = -da[5];
+    h.rec.e[0] = (double)(lnA - kc0);
+    h.rec.e[1] = (double)((long double)d->b[k] - kc1);
+    h.rec.e[2] = (double)(mEaR - kc2);
+    h.rec.d[0] = (double)(-da[1] / 2);
+    h.rec.d[1] = (double)(-da[2] / 6);
+    h.rec.d[2] = (double)(-da[3] / 12);
+    h.rec.d[3] = (double)(-da[4] / 20);
     h.rec.korig = (uint32_t)k;
-    h.rec.meta = (uint32_t)h.type | (d->reversible[k] ? kMetaRev : 0u) | ((uint32_t)nr << kMetaNrShift) |
-                 ((uint32_t)np << kMetaNpShift);
+    h.rec.meta = (uint32_t)h.type | (d->reversible[k] ? kMetaRev : 0u);
+    h.nr = nr;
+    h.np = np;
     h.has_aux = h.type != PSR_RX_PLAIN;
     for (int j = d->eff_ptr[k]; j < d->eff_ptr[k + 1]; ++j) {
       if (d->eff_sp[j] < 0 || d->eff_sp[j] >= K) return fail(PSR_EINVAL, "reaction %d: efficiency species out of range", k);
       if (!std::isfinite(d->eff_val[j])) return fail(PSR_EINVAL, "reaction %d: efficiency not finite", k);
       EffEnt e{};
       e.am1 = d->eff_val[j] - 1.0;
-      e.sp = (uint32_t)d->eff_sp[j];
+      e.off = (uint32_t)d->eff_sp[j];  // species index here; scaled to a row offset at serialisation
       if (h.has_aux) h.eff.push_back(e);  // efficiencies on a plain reaction have no effect
     }
     if (h.type >= 2) {
@@ -201,10 +211,13 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   else if (K <= 128) { nw = 16; spw = 8; }
   else if (K <= 256) { nw = 16; spw = 16; }
   else { nw = 16; spw = 32; }
+  int rl = spw <= 8 ? 2 : 1;  // reactors per lane: 2 while the wdot accumulators fit in registers
+  if (const char* e = getenv("PSR_R")) rl = (atoi(e) == 2 && spw <= 16) ? 2 : 1;
+  const uint32_t row_bytes = (uint32_t)kRowBytes * rl;
   int rc_target = 128;
-  if (const char* e = getenv("PSR_RC")) rc_target = std::max(8, atoi(e));
+  if (const char* e = getenv("PSR_RC")) rc_target = std::min(kMaxChunkRx, std::max(8, atoi(e)));
   const int n_chunks = (I + rc_target - 1) / rc_target;
-  const int rc = (I + n_chunks - 1) / n_chunks;
+  const int rc = (I + n_chunks - 1) / n_chunks;  // <= rc_target <= kMaxChunkRx
 
   // ---- distribute reactions over chunks (each type dealt round-robin so chunks cost the same),
   //      then inside a chunk order by cost and deal to warps in snake order.
@@ -229,6 +242,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   // ---- serialise chunk blobs
   std::vector<std::vector<unsigned char>> blobs(n_chunks);
   size_t stride = 0;
+  const uint32_t unit_off = (uint32_t)K * row_bytes;   // the all-ones row of the C tile
+  const uint32_t zero_off = (uint32_t)rc * row_bytes;  // the all-zero row of the q tile
   for (int c = 0; c < n_chunks; ++c) {
     const auto& cr = chunk_rx[c];
     const int n_rx = (int)cr.size();
@@ -236,44 +251,54 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     std::vector<AuxRec> auxs;
     std::vector<EffEnt> effs;
     std::vector<uint16_t> pool;
-    std::vector<std::vector<uint32_t>> rows(K);
+    std::vector<std::vector<uint32_t>> pos(K), neg(K);
     for (int kl = 0; kl < n_rx; ++kl) {
       HostRx& h = rx[cr[kl]];
       RxRec rec = h.rec;
-      if ((int)h.factors.size() <= kInlineSp) {
-        for (size_t i = 0; i < h.factors.size(); ++i) rec.sp[i] = h.factors[i];
+      if (h.nr <= kSlots && h.np <= kSlots) {
+        for (int i = 0; i < kSlots; ++i) {
+          rec.off[i] = i < h.nr ? (uint32_t)h.factors[i] * row_bytes : unit_off;
+          rec.off[kSlots + i] = i < h.np ? (uint32_t)h.factors[h.nr + i] * row_bytes : unit_off;
+        }
       } else {
-        const uint32_t off = (uint32_t)pool.size();
-        rec.meta |= kMetaLong;
-        rec.sp[0] = (uint16_t)(off & 0xFFFF);
-        rec.sp[1] = (uint16_t)(off >> 16);
+        rec.meta |= kMetaLong | ((uint32_t)h.nr << kMetaNrShift) | ((uint32_t)h.np << kMetaNpShift);
+        rec.off[0] = (uint32_t)pool.size();
         pool.insert(pool.end(), h.factors.begin(), h.factors.end());
       }
       if (h.has_aux) {
         AuxRec ax = h.aux;
         ax.eff_off = (uint32_t)effs.size();
         ax.n_eff = (uint32_t)h.eff.size();
-        effs.insert(effs.end(), h.eff.begin(), h.eff.end());
+        for (EffEnt ee : h.eff) {
+          ee.off *= row_bytes;
+          effs.push_back(ee);
+        }
         rec.meta |= (uint32_t)auxs.size() << kMetaAuxShift;
         auxs.push_back(ax);
       }
       recs[kl] = rec;
       for (auto& pr : h.nu_net)
         for (int t = 0; t < std::abs(pr.second); ++t)
-          rows[pr.first].push_back((uint32_t)kl | (pr.second < 0 ? kCsrNeg : 0u));
+          (pr.second < 0 ? neg : pos)[pr.first].push_back((uint32_t)kl * row_bytes);
     }
-    std::vector<uint32_t> cptr(K + 1, 0), cent;
+    std::vector<uint32_t> gptr(2 * K + 1, 0), gent;
+    auto add_group = [&](const std::vector<uint32_t>& grp) {
+      gent.insert(gent.end(), grp.begin(), grp.end());
+      while (gent.size() % 4) gent.push_back(zero_off);
+    };
     for (int s = 0; s < K; ++s) {
-      cptr[s] = (uint32_t)cent.size();
-      cent.insert(cent.end(), rows[s].begin(), rows[s].end());
+      gptr[2 * s] = (uint32_t)gent.size();
+      add_group(pos[s]);
+      gptr[2 * s + 1] = (uint32_t)gent.size();
+      add_group(neg[s]);
     }
-    cptr[K] = (uint32_t)cent.size();
+    gptr[2 * K] = (uint32_t)gent.size();
 
     ChunkHdr hdr{};
     hdr.n_rx = n_rx;
     hdr.n_aux = (uint32_t)auxs.size();
     hdr.n_eff = (uint32_t)effs.size();
-    hdr.n_csr = (uint32_t)cent.size();
+    hdr.n_g = (uint32_t)gent.size();
     size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
     hdr.off_aux = (uint32_t)off;
     off += sizeof(AuxRec) * auxs.size();
@@ -281,10 +306,10 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     off += sizeof(EffEnt) * effs.size();
     hdr.off_pool = (uint32_t)off;
     off = align_up(off + 2 * pool.size(), 16);
-    hdr.off_csr_ptr = (uint32_t)off;
-    off = align_up(off + 4 * cptr.size(), 16);
-    hdr.off_csr_ent = (uint32_t)off;
-    off = align_up(off + 4 * cent.size(), 16);
+    hdr.off_gptr = (uint32_t)off;
+    off = align_up(off + 4 * gptr.size(), 16);
+    hdr.off_gent = (uint32_t)off;
+    off = align_up(off + 4 * gent.size(), 16);
     hdr.bytes = (uint32_t)off;
     std::vector<unsigned char>& b = blobs[c];
     b.assign(off, 0);
@@ -293,8 +318,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     if (!auxs.empty()) std::memcpy(b.data() + hdr.off_aux, auxs.data(), sizeof(AuxRec) * auxs.size());
     if (!effs.empty()) std::memcpy(b.data() + hdr.off_eff, effs.data(), sizeof(EffEnt) * effs.size());
     if (!pool.empty()) std::memcpy(b.data() + hdr.off_pool, pool.data(), 2 * pool.size());
-    std::memcpy(b.data() + hdr.off_csr_ptr, cptr.data(), 4 * cptr.size());
-    if (!cent.empty()) std::memcpy(b.data() + hdr.off_csr_ent, cent.data(), 4 * cent.size());
+    std::memcpy(b.data() + hdr.off_gptr, gptr.data(), 4 * gptr.size());
+    if (!gent.empty()) std::memcpy(b.data() + hdr.off_gent, gent.data(), 4 * gent.size());
     stride = std::max(stride, off);
   }
   stride = align_up(stride, 128);
@@ -313,6 +338,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   if (!m) return fail(PSR_ENOMEM, "psr_mech_load: host allocation failed");
   m->device = dev;
   m->nw = nw;
+  m->rl = rl;
+  m->tile = kTile * rl;
   m->spw = spw;
   m->n_sm = prop.multiProcessorCount;
   m->n_falloff = n_fall;
@@ -326,13 +353,13 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.chunk_stride = (uint32_t)stride;
   size_t o = 0;
   v.smem_cs = (uint32_t)o;
-  o += align_up((size_t)(K + 2) * kTile * 8, 128);  // K rows of C; K+2 so the Jacobian staging [32][n|1] fits
+  o += align_up((size_t)(K + 2) * kTile * rl * 8, 128);  // K rows of C; K+2 so the Jacobian staging [tile][n|1] fits
   v.smem_q = (uint32_t)o;
-  o += align_up((size_t)rc * kTile * 8, 128);
+  o += align_up((size_t)(rc + 1) * kTile * rl * 8, 128);  // + the all-zero row
   v.smem_mech = (uint32_t)o;
   o += stride * (n_chunks == 1 ? 1 : 2);
   v.smem_misc = (uint32_t)o;
-  o += (size_t)2 * nw * 32 * 8 + 64;
+  o += (size_t)2 * nw * kTile * rl * 8 + (size_t)kTile * rl * 8 + 64 * 8 + 64;  // partial sums, per-lane scalars, exp table, mbarriers
   v.smem_total = (uint32_t)o;
   if (o > (size_t)prop.sharedMemPerBlockOptin) {
     delete m;
@@ -351,10 +378,20 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     cleanup();
     return cuda_fail(e, "cudaMemcpy (mechanism upload)");
   }
+  {
+    double tab[64];
+    for (int j = 0; j < 64; ++j) tab[j] = (double)exp2l((long double)j / 64.0L);
+    if ((e = cudaMalloc(&m->d_exptab, sizeof tab)) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_exptab, tab, sizeof tab, cudaMemcpyHostToDevice)) != cudaSuccess) {
+      cleanup();
+      return cuda_fail(e, "exp table upload");
+    }
+  }
+  v.exp_tab = m->d_exptab;
   v.chunks = m->d_chunks;
   v.invW = m->d_invW;
   v.Wm = m->d_W;
-  if ((e = occupancy_eval(nw, spw, v.smem_total, &m->ctas_per_sm)) != cudaSuccess || m->ctas_per_sm < 1) {
+  if ((e = occupancy_eval(nw, spw, rl, v.smem_total, &m->ctas_per_sm)) != cudaSuccess || m->ctas_per_sm < 1) {
     cleanup();
     return fail(PSR_ECUDA, "kernel does not fit on this device (%s)", cudaGetErrorString(e));
   }
@@ -367,6 +404,7 @@ void psr_mech_free(psr_mech* m) {
   cudaFree(m->d_chunks);
   cudaFree(m->d_invW);
   cudaFree(m->d_W);
+  cudaFree(m->d_exptab);
   cudaFree(m->d_scratch);
   delete m;
 }
@@ -375,7 +413,7 @@ psr_status psr_mech_info(const psr_mech* m, psr_mech_info_t* info) {
   if (!m || !info) return fail(PSR_EINVAL, "psr_mech_info: null argument");
   info->n_species = m->view.K;
   info->n_reactions = m->view.I;
-  info->tile = kTile;
+  info->tile = m->tile;
   info->warps = m->nw;
   info->chunk_reactions = m->view.rc;
   info->n_chunks = m->view.n_chunks;
@@ -405,7 +443,7 @@ psr_status check_common(const psr_mech* m, int64_t N, const double* T, const dou
 psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
   const int64_t cap = (int64_t)m->n_sm * m->ctas_per_sm;
   const int grid = (int)std::min<int64_t>(a.n_tiles, cap);
-  cudaError_t e = launch_eval(m->nw, m->spw, m->view, a, grid, (cudaStream_t)stream);
+  cudaError_t e = launch_eval(m->nw, m->spw, m->rl, m->view, a, grid, (cudaStream_t)stream);
   if (e != cudaSuccess) return cuda_fail(e, fn);
   return PSR_OK;
 }
@@ -424,7 +462,7 @@ psr_status psr_eval_kf_kr(const psr_mech* m, int64_t N, const double* T, const d
   EvalArgs a{};
   a.N = N; a.ld = ld; a.ldk = ldk; a.T = T; a.P = P; a.Y = Y; a.kf = kf; a.kr = kr;
   a.flags = (kf ? kOutKf : 0u) | (kr ? kOutKr : 0u);
-  a.n_tiles = (N + kTile - 1) / kTile;
+  a.n_tiles = (N + m->tile - 1) / m->tile;
   return run(m, a, stream, "psr_eval_kf_kr");
 }
 
@@ -438,7 +476,7 @@ psr_status psr_eval_wdot(const psr_mech* m, int64_t N, const double* T, const do
   EvalArgs a{};
   a.N = N; a.ld = ld; a.ldk = ldq; a.T = T; a.P = P; a.Y = Y; a.wdot = wdot; a.q = q;
   a.flags = kOutWdot | (q ? kOutQ : 0u);
-  a.n_tiles = (N + kTile - 1) / kTile;
+  a.n_tiles = (N + m->tile - 1) / m->tile;
   return run(m, a, stream, "psr_eval_wdot");
 }
 
@@ -451,7 +489,7 @@ psr_status psr_eval_residual(const psr_mech* m, int64_t N, const double* T, cons
   EvalArgs a{};
   a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.F = F; a.wdot = wdot;
   a.flags = kOutF | (wdot ? kOutWdot : 0u);
-  a.n_tiles = (N + kTile - 1) / kTile;
+  a.n_tiles = (N + m->tile - 1) / m->tile;
   return run(m, a, stream, "psr_eval_residual");
 }
 
@@ -479,14 +517,31 @@ psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const
   EvalArgs a{};
   a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.F0out = F0;
   a.flags = kOutF0;
-  a.n_tiles = (N + kTile - 1) / kTile;
+  a.n_tiles = (N + m->tile - 1) / m->tile;
   st = run(m, a, stream, "psr_fd_jacobian (base residual)");
   if (st != PSR_OK) return st;
   EvalArgs b{};
   b.N = N; b.ld = ld; b.T = T; b.P = P; b.Y = Y; b.Yin = Yin; b.tau = tau; b.J = J; b.F0 = F0;
   b.flags = kModeJac;
-  b.n_tiles = (N * n + kTile - 1) / kTile;
+  b.n_tiles = (N * n + m->tile - 1) / m->tile;
   return run(m, b, stream, "psr_fd_jacobian (perturbed sweeps)");
+}
+
+psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {
+  g_err.clear();
+  if (!m || !x || !y || n < 0) return fail(PSR_EINVAL, "psr_probe_exp_values: bad argument");
+  if (n == 0) return PSR_OK;
+  double *dx = nullptr, *dy = nullptr;
+  cudaError_t e;
+  if ((e = cudaMalloc(&dx, 8 * (size_t)n)) != cudaSuccess) return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e));
+  if ((e = cudaMalloc(&dy, 8 * (size_t)n)) != cudaSuccess) { cudaFree(dx); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  e = cudaMemcpy(dx, x, 8 * (size_t)n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = launch_exp_values(m->d_exptab, dx, dy, n, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(y, dy, 8 * (size_t)n, cudaMemcpyDeviceToHost);
+  cudaFree(dx);
+  cudaFree(dy);
+  if (e != cudaSuccess) return cuda_fail(e, "psr_probe_exp_values");
+  return PSR_OK;
 }
 
 psr_status psr_probe_fp64(int kind, int iters, double* elapsed_ms, double* ops) {

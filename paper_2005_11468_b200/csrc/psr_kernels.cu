@@ -1,13 +1,13 @@
 // psr_kernels.cu -- sm_100a kernels of the batched PSR chemistry hot path.
 //
-// One fused kernel evaluates SURVEY.md 8(a) steps a1..a10 for a tile of 32 evaluation states:
-//   lane  <-> reactor (or, in Jacobian mode, one perturbed copy of a reactor),
+// One fused kernel evaluates SURVEY.md 8(a) steps a1..a10 for a tile of 32 R evaluation states:
+//   lane  <-> R reactors (or, in Jacobian mode, R perturbed copies of a reactor),
 //   warp  <-> a share of the chunk's reactions (reaction phase) / a share of the species (gather).
 // Every per-reaction quantity is therefore warp-uniform: mechanism constants are shared-memory
 // broadcasts, reaction-type branches never diverge, and C[species][lane] reads are conflict-free.
 //
-// Per tile:   prologue  a1  Wbar, rho, C_i -> smem Cs[K][32]           (Eq. 5's X_i)
-//             per chunk a3-a7  k_f, K_c, k_r, [M], falloff, q -> qs[rc][32]   (Eq. 5-9)
+// Per tile:   prologue  a1  Wbar, rho, C_i -> smem Cs[K][32 R]           (Eq. 5's X_i)
+//             per chunk a3-a7  k_f, K_c, k_r, [M], falloff, q -> qs[rc][32 R]   (Eq. 5-9)
 //                       a8     wdot += nu^T q : CSR gather, accumulators in registers (Eq. 4)
 //             epilogue  a9/a10 residual (Eq. 2) / difference quotient, coalesced stores.
 // The mechanism chunk blobs (psr_tables.h) stream global -> shared through cp.async.bulk with an
@@ -15,12 +15,14 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "psr_math.cuh"
 #include "psr_tables.h"
 
 namespace psr {
 
 __device__ constexpr double kRgas = 8.31446261815324e7;  // erg/mol/K
-__device__ constexpr double kLn10 = 2.302585092994045684;
+__device__ constexpr double kLog10e = 0.43429448190325182765;
+constexpr int PSR_T_PLAIN = 0, PSR_T_THREE_BODY = 1, PSR_T_LINDEMANN = 2, PSR_T_TROE = 3;  // = PSR_RX_* of psr.h
 
 // ------------------------------------------------------------------ mbarrier / bulk copy
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -50,15 +52,47 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   } while (!done);
 }
 
+// ------------------------------------------------------------------ shared-memory access by 32-bit address
+// (volatile so that loads are neither merged across tiles nor moved over barriers by the front end)
+__device__ __forceinline__ double lds64(uint32_t addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts64(uint32_t addr, double v) {
+  asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v));
+}
+template <int R>
+struct RowIO;
+template <>
+struct RowIO<1> {
+  static __device__ __forceinline__ void ld(uint32_t addr, double (&v)[1]) { v[0] = lds64(addr); }
+  static __device__ __forceinline__ void st(uint32_t addr, const double (&v)[1]) { sts64(addr, v[0]); }
+};
+template <>
+struct RowIO<2> {
+  static __device__ __forceinline__ void ld(uint32_t addr, double (&v)[2]) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr));
+  }
+  static __device__ __forceinline__ void st(uint32_t addr, const double (&v)[2]) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v[0]), "d"(v[1]));
+  }
+};
+
 // ------------------------------------------------------------------ the fused kernel
-template <int NW, int SPW>
+// R reactors per lane: every warp-uniform instruction (mechanism loads, address arithmetic, branches)
+// is amortised over R evaluations and the R exp chains interleave in the FP64 pipe.
+template <int NW, int SPW, int R>
 __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, const EvalArgs a) {
+  constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
-  double* Cs = reinterpret_cast<double*>(smem + mv.smem_cs);          // [K][32]
-  double* qs = reinterpret_cast<double*>(smem + mv.smem_q);           // [rc][32]
+  double* Cs = reinterpret_cast<double*>(smem + mv.smem_cs);          // [K+2][TR]; row K is the unit row
+  double* qs = reinterpret_cast<double*>(smem + mv.smem_q);           // [rc+1][TR]; row rc stays zero
   unsigned char* mring = smem + mv.smem_mech;                         // stages * chunk_stride
-  double* part = reinterpret_cast<double*>(smem + mv.smem_misc);      // [2][NW][32]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(part + 2 * NW * 32);   // [2]
+  double* part = reinterpret_cast<double*>(smem + mv.smem_misc);      // [2][NW][TR] partial sums
+  double* lane_s = part + 2 * NW * TR;                                // [TR]: ln T per state
+  double* etab = lane_s + TR;                                         // [64] 2^(j/64)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(etab + kExpTabN);      // [2]
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -66,6 +100,8 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
   const int n = K + 1;
   const bool jac = (a.flags & kModeJac) != 0;
   const int nstage = mv.n_chunks == 1 ? 1 : 2;
+  const uint32_t c_lane = smem_u32(Cs) + lane * (8 * R);   // this lane's R slots of row 0 of the C tile
+  const uint32_t q_lane = smem_u32(qs) + lane * (8 * R);
 
   const int64_t my_tiles = (a.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
   const int64_t total_loads = mv.n_chunks == 1 ? 1 : my_tiles * mv.n_chunks;
@@ -81,81 +117,125 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
                mv.chunk_stride, &bars[g]);
     }
   }
+  if (threadIdx.x < kExpTabN) etab[threadIdx.x] = mv.exp_tab[threadIdx.x];
+  if (w == 0) {
+#pragma unroll
+    for (int i = 0; i < R; ++i) qs[mv.rc * TR + lane * R + i] = 0.0;
+  }
   __syncthreads();
 
   int64_t g = 0;  // chunk loads consumed so far by this CTA
   for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
     // ---------------------------------------------------------------- prologue (a1)
-    const int64_t v = tile * kTile + lane;
-    int64_t r;
-    int jcol = -1;  // perturbed unknown (Jacobian mode): 0 = T, 1.. = species jcol-1
-    bool valid;
-    if (jac) {
-      valid = v < a.N * n;
-      const int64_t vv = valid ? v : a.N * n - 1;
-      r = vv / n;
-      jcol = (int)(vv - r * n);
-    } else {
-      valid = v < a.N;
-      r = valid ? v : a.N - 1;
-    }
-    double T = a.T[r];
-    const double P = a.P[r];
-    double h = 1.0;
-    if (jcol == 0) {
-      const double d = 1e-8 * fmax(fabs(T), 1e-10);
-      const double Tp = T + d;
-      h = Tp - T;
-      T = Tp;
-    }
-    const int jsp = jcol - 1;
-    // perturbed mass fraction of species s for this lane
-    auto load_Y = [&](int s) -> double {
-      double y = a.Y[(int64_t)s * a.ld + r];
-      if (s == jsp) {
-        const double d = 1e-8 * fmax(fabs(y), 1e-10);
-        const double yp = y + d;
-        h = yp - y;
-        y = yp;
+    // state i of this lane is evaluation v = tile*TR + i*32 + lane (coalesced global access); in shared
+    // memory it lives at column lane*R + i of every row.
+    int64_t r[R];
+    int jsp[R];      // perturbed species (Jacobian mode), -1: T column, -2: none
+    bool valid[R];
+    double T[R], P[R], h[R], ypert[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+      const int64_t v = tile * TR + i * 32 + lane;
+      int jcol = -1;
+      if (jac) {
+        valid[i] = v < a.N * n;
+        const int64_t vv = valid[i] ? v : a.N * n - 1;
+        r[i] = vv / n;
+        jcol = (int)(vv - r[i] * n);
+      } else {
+        valid[i] = v < a.N;
+        r[i] = valid[i] ? v : a.N - 1;
       }
-      return y;
-    };
-
-    double sumYW = 0.0;
-#pragma unroll
-    for (int jj = 0; jj < SPW; ++jj) {
-      const int s = w + NW * jj;
-      if (s < K) sumYW = fma(load_Y(s), mv.invW[s], sumYW);
-    }
-    part[w * 32 + lane] = sumYW;
-    __syncthreads();
-    sumYW = 0.0;
-#pragma unroll
-    for (int ww = 0; ww < NW; ++ww) sumYW += part[ww * 32 + lane];
-    const double Wbar = 1.0 / sumYW;
-    const double rho = P * Wbar / (kRgas * T);
-    double cpart = 0.0;
-#pragma unroll
-    for (int jj = 0; jj < SPW; ++jj) {
-      const int s = w + NW * jj;
-      if (s < K) {
-        const double c = rho * load_Y(s) * mv.invW[s];
-        Cs[s * 32 + lane] = c;
-        cpart += c;
+      T[i] = a.T[r[i]];
+      P[i] = a.P[r[i]];
+      // forward-difference step of this state's column: x' = fl(x + delta), h = fl(x' - x)  (O11, g15)
+      jsp[i] = jcol - 1;
+      h[i] = 1.0;
+      ypert[i] = 0.0;
+      if (jcol == 0) {
+        const double Tp = T[i] + 1e-8 * fmax(fabs(T[i]), 1e-10);
+        h[i] = Tp - T[i];
+        T[i] = Tp;
+      } else if (jcol > 0) {
+        const double y = a.Y[(int64_t)jsp[i] * a.ld + r[i]];
+        ypert[i] = y + 1e-8 * fmax(fabs(y), 1e-10);
+        h[i] = ypert[i] - y;
       }
     }
-    part[(NW + w) * 32 + lane] = cpart;
+    auto load_Y = [&](int s, int i) -> double { return s == jsp[i] ? ypert[i] : a.Y[(int64_t)s * a.ld + r[i]]; };
+
+    double rho[R];
+    {
+      double yv[SPW][R];
+      double sumYW[R];
+#pragma unroll
+      for (int i = 0; i < R; ++i) sumYW[i] = 0.0;
+#pragma unroll
+      for (int jj = 0; jj < SPW; ++jj) {
+        const int s = w + NW * jj;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          yv[jj][i] = 0.0;
+          if (s < K) {
+            yv[jj][i] = load_Y(s, i) * mv.invW[s];
+            sumYW[i] += yv[jj][i];
+          }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < R; ++i) part[w * TR + lane * R + i] = sumYW[i];
+      if (w == 0) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          lane_s[lane * R + i] = log(T[i]);
+          Cs[K * TR + lane * R + i] = 1.0;
+        }
+      }
+      __syncthreads();
+      double cpart[R];
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        double sY = 0.0;
+#pragma unroll
+        for (int ww = 0; ww < NW; ++ww) sY += part[ww * TR + lane * R + i];
+        const double Wbar = 1.0 / sY;
+        rho[i] = P[i] * Wbar / (kRgas * T[i]);
+        cpart[i] = 0.0;
+      }
+#pragma unroll
+      for (int jj = 0; jj < SPW; ++jj) {
+        const int s = w + NW * jj;
+        if (s < K) {
+#pragma unroll
+          for (int i = 0; i < R; ++i) {
+            const double c = rho[i] * yv[jj][i];
+            Cs[s * TR + lane * R + i] = c;
+            cpart[i] += c;
+          }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < R; ++i) part[(NW + w) * TR + lane * R + i] = cpart[i];
+    }
     __syncthreads();
-    double Ctot = 0.0;
+    double Ctot[R], lnT[R], invT[R], lnCtot[R];
 #pragma unroll
-    for (int ww = 0; ww < NW; ++ww) Ctot += part[(NW + ww) * 32 + lane];
-
-    const double lnT = log(T);
-    const double invT = 1.0 / T;
-
-    double acc[SPW];
+    for (int i = 0; i < R; ++i) {
+      double ct = 0.0;
 #pragma unroll
-    for (int jj = 0; jj < SPW; ++jj) acc[jj] = 0.0;
+      for (int ww = 0; ww < NW; ++ww) ct += part[(NW + ww) * TR + lane * R + i];
+      Ctot[i] = ct;
+      lnT[i] = lane_s[lane * R + i];
+      invT[i] = 1.0 / T[i];
+      lnCtot[i] = 0.0;
+    }
+    bool have_lnCtot = false;  // ln C_tot is formed on first use by a Troe reaction without efficiencies
+
+    double acc[SPW][R];
+#pragma unroll
+    for (int jj = 0; jj < SPW; ++jj)
+#pragma unroll
+      for (int i = 0; i < R; ++i) acc[jj][i] = 0.0;
 
     // ---------------------------------------------------------------- chunks
     for (int c = 0; c < mv.n_chunks; ++c) {
@@ -164,89 +244,197 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
       const unsigned char* blob = mring + (size_t)stage * mv.chunk_stride;
       const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
       const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
-      const AuxRec* auxs = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux);
-      const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
-      const uint16_t* pool = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool);
       const int n_rx = (int)hdr->n_rx;
 
       // ---- reaction phase (a3..a7): warp w takes records w, w+NW, ...
+#pragma unroll 1
       for (int kl = w; kl < n_rx; kl += NW) {
         const RxRec* rec = recs + kl;
         const uint32_t meta = rec->meta;
         const int type = (int)(meta & kMetaTypeMask);
-        const double lnkinf = fma(rec->c[1], lnT, fma(rec->c[2], invT, rec->c[0]));
-        // ln K_c (Eq. 8-9 summed per reaction at load time)
-        double lnKc = fma(fma(fma(rec->d[6], T, rec->d[5]), T, rec->d[4]), T, rec->d[3]) * T;
-        lnKc += fma(rec->d[1], lnT, fma(rec->d[2], invT, rec->d[0]));
-        const bool rev = (meta & kMetaRev) != 0;
-
-        double kf, kr, M = 1.0;
-        if (type == 0) {
-          kf = exp(lnkinf);
-          kr = rev ? exp(lnkinf - lnKc) : 0.0;
-        } else {
-          const AuxRec* ax = auxs + (meta >> kMetaAuxShift);
-          M = Ctot;
-          const uint32_t e1 = ax->eff_off + ax->n_eff;
-          for (uint32_t e = ax->eff_off; e < e1; ++e) M = fma(effs[e].am1, Cs[effs[e].sp * 32 + lane], M);
-          kf = exp(lnkinf);
-          if (type >= 2) {
-            const double lnk0 = fma(ax->c0[1], lnT, fma(ax->c0[2], invT, ax->c0[0]));
-            const double Pr = exp(lnk0 - lnkinf) * M;
-            double F = 1.0;
-            if (type == 3) {
-              const double al = ax->troe[0];
-              const double Fcent =
-                  fma(1.0 - al, exp(T * ax->troe[1]), fma(al, exp(T * ax->troe[2]), exp(ax->troe[3] * invT)));
-              const double lF = log10(Fcent);
-              const double cc = fma(-0.67, lF, -0.4);
-              const double nn = fma(-1.27, lF, 0.75);
-              const double lp = log10(Pr) + cc;
-              const double f1 = lp / fma(-0.14, lp, nn);
-              F = exp(kLn10 * (lF / fma(f1, f1, 1.0)));
-            }
-            kf = kf * (Pr / (1.0 + Pr)) * F;
-          }
-          kr = rev ? kf * exp(-lnKc) : 0.0;
+        double lnkf[R], lnkr[R], pf[R], pr[R], kf[R], kr[R], M[R];
+        // Eq. 6 in log form, and ln k_r = ln k_f - ln K_c (Eq. 7-9 summed per reaction at load time)
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          lnkf[i] = fma(rec->c[1], lnT[i], fma(rec->c[2], invT[i], rec->c[0]));
+          const double pn = fma(fma(fma(rec->d[3], T[i], rec->d[2]), T[i], rec->d[1]), T[i], rec->d[0]);
+          lnkr[i] = fma(pn, T[i], fma(rec->e[1], lnT[i], fma(rec->e[2], invT[i], rec->e[0])));
+          M[i] = 1.0;
         }
 
-        // concentration products (Eq. 5), integer powers by repetition
-        const int nr = (int)((meta >> kMetaNrShift) & 0xF);
-        const int np = (int)((meta >> kMetaNpShift) & 0xF);
-        const uint16_t* sp = rec->sp;
-        if (meta & kMetaLong) sp = pool + ((uint32_t)rec->sp[0] | ((uint32_t)rec->sp[1] << 16));
-        double pf = 1.0, pr = 1.0;
-        for (int i = 0; i < nr; ++i) pf *= Cs[sp[i] * 32 + lane];
-        for (int i = 0; i < np; ++i) pr *= Cs[sp[nr + i] * 32 + lane];
-        double q = kf * pf - kr * pr;
-        if (type == 1) q *= M;
-        qs[kl * 32 + lane] = q;
+        // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
+        if (!(meta & kMetaLong)) {
+          double f0[R], f1[R], f2[R], p0[R], p1[R], p2[R];
+          RowIO<R>::ld(c_lane + rec->off[0], f0);
+          RowIO<R>::ld(c_lane + rec->off[1], f1);
+          RowIO<R>::ld(c_lane + rec->off[2], f2);
+          RowIO<R>::ld(c_lane + rec->off[3], p0);
+          RowIO<R>::ld(c_lane + rec->off[4], p1);
+          RowIO<R>::ld(c_lane + rec->off[5], p2);
+#pragma unroll
+          for (int i = 0; i < R; ++i) {
+            pf[i] = f0[i] * f1[i] * f2[i];
+            pr[i] = p0[i] * p1[i] * p2[i];
+          }
+        } else {
+          const uint16_t* sp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + rec->off[0];
+          const int nr = (int)((meta >> kMetaNrShift) & 0xF);
+          const int np = (int)((meta >> kMetaNpShift) & 0xF);
+#pragma unroll
+          for (int i = 0; i < R; ++i) {
+            pf[i] = 1.0;
+            pr[i] = 1.0;
+          }
+#pragma unroll 1
+          for (int j = 0; j < nr + np; ++j) {
+            double cv[R];
+            RowIO<R>::ld(c_lane + (uint32_t)sp[j] * (uint32_t)(TR * 8), cv);
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              if (j < nr) pf[i] *= cv[i];
+              else pr[i] *= cv[i];
+            }
+          }
+        }
 
-        if (valid && (a.flags & (kOutKf | kOutKr | kOutQ))) {
-          const int64_t o = (int64_t)rec->korig * a.ldk + r;
-          if (a.flags & kOutKf) a.kf[o] = kf;
-          if (a.flags & kOutKr) a.kr[o] = kr;
-          if (a.flags & kOutQ) a.q[o] = q;
+        if (type <= PSR_T_THREE_BODY) {
+          bool ok = true;
+#pragma unroll
+          for (int i = 0; i < R; ++i) ok = ok && exp_in_range(lnkf[i], lnkr[i]);
+          if (ok) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              kf[i] = exp_core(lnkf[i], etab);
+              kr[i] = exp_core(lnkr[i], etab);
+            }
+          } else {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              kf[i] = exp(lnkf[i]);
+              kr[i] = exp(lnkr[i]);
+            }
+          }
+        }
+        if (type != PSR_T_PLAIN) {
+          const AuxRec* ax = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux) + (meta >> kMetaAuxShift);
+          const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
+#pragma unroll
+          for (int i = 0; i < R; ++i) M[i] = Ctot[i];
+          const uint32_t e1 = ax->eff_off + ax->n_eff;
+#pragma unroll 1
+          for (uint32_t e = ax->eff_off; e < e1; ++e) {
+            double cv[R];
+            RowIO<R>::ld(c_lane + effs[e].off, cv);
+#pragma unroll
+            for (int i = 0; i < R; ++i) M[i] = fma(effs[e].am1, cv[i], M[i]);
+          }
+          if (type >= PSR_T_LINDEMANN) {
+            if (type == PSR_T_TROE && ax->n_eff == 0 && !have_lnCtot) {
+#pragma unroll
+              for (int i = 0; i < R; ++i) lnCtot[i] = log(Ctot[i]);
+              have_lnCtot = true;
+            }
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
+              if (type == PSR_T_LINDEMANN) {
+                const double Pr = exp_fast(lnk0 - lnkf[i], etab) * M[i];
+                kf[i] = exp_fast(lnkf[i], etab) * (Pr / (1.0 + Pr));
+              } else {
+                // Troe.  With ln Pr = ln k0 - ln k_inf + ln[M]:
+                //   k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
+                const double lnM = ax->n_eff == 0 ? lnCtot[i] : log(M[i]);
+                const double lnk0M = lnk0 + lnM;
+                const double lnPr = lnk0M - lnkf[i];
+                const double Pr = exp_fast(lnPr, etab);
+                const double al = ax->troe[0];
+                const double Fcent =
+                    fma(1.0 - al, exp_fast(T[i] * ax->troe[1], etab),
+                        fma(al, exp_fast(T[i] * ax->troe[2], etab), exp_fast(ax->troe[3] * invT[i], etab)));
+                const double lnFc = log(Fcent);
+                const double lF = lnFc * kLog10e;
+                const double cc = fma(-0.67, lF, -0.4);
+                const double nn = fma(-1.27, lF, 0.75);
+                const double lp = fma(lnPr, kLog10e, cc);
+                const double den = fma(-0.14, lp, nn);
+                // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
+                const double den2 = den * den;
+                const double lnF = lnFc * den2 / fma(lp, lp, den2);
+                kf[i] = exp_fast(lnk0M + lnF, etab) / (1.0 + Pr);
+              }
+              kr[i] = kf[i] * exp_fast(lnkr[i] - lnkf[i], etab);
+            }
+          }
+        }
+        double q[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          if (!(meta & kMetaRev)) kr[i] = 0.0;
+          q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
+          if (type == PSR_T_THREE_BODY) q[i] *= M[i];
+        }
+        RowIO<R>::st(q_lane + (uint32_t)kl * (uint32_t)(TR * 8), q);
+
+        if (a.flags & (kOutKf | kOutKr | kOutQ)) {
+#pragma unroll
+          for (int i = 0; i < R; ++i) {
+            if (valid[i]) {
+              const int64_t o = (int64_t)rec->korig * a.ldk + r[i];
+              if (a.flags & kOutKf) a.kf[o] = kf[i];
+              if (a.flags & kOutKr) a.kr[o] = kr[i];
+              if (a.flags & kOutQ) a.q[o] = q[i];
+            }
+          }
         }
       }
       __syncthreads();
 
-      // ---- gather phase (a8): warp w owns species w, w+NW, ...; ascending reaction order
+      // ---- gather phase (a8, Eq. 4): warp w owns species w, w+NW, ...; fixed summation order
       if (a.flags & (kOutWdot | kOutF | kModeJac | kOutF0)) {
-        const uint32_t* cptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_csr_ptr);
-        const uint32_t* cent = reinterpret_cast<const uint32_t*>(blob + hdr->off_csr_ent);
+        const uint32_t* gptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_gptr);
+        const uint4* gent = reinterpret_cast<const uint4*>(blob + hdr->off_gent);
 #pragma unroll
         for (int jj = 0; jj < SPW; ++jj) {
           const int s = w + NW * jj;
           if (s < K) {
-            const uint32_t e0 = cptr[s], e1 = cptr[s + 1];
-            double av = acc[jj];
-            for (uint32_t e = e0; e < e1; ++e) {
-              const uint32_t ent = cent[e];
-              const double qv = qs[(ent & 0xFFFFu) * 32 + lane];
-              av += (ent & kCsrNeg) ? -qv : qv;
+            const uint32_t g0 = gptr[2 * s] >> 2, g1 = gptr[2 * s + 1] >> 2, g2 = gptr[2 * s + 2] >> 2;
+            double a1[R];
+#pragma unroll
+            for (int i = 0; i < R; ++i) a1[i] = 0.0;
+#pragma unroll 1
+            for (uint32_t e = g0; e < g1; ++e) {
+              const uint4 o = gent[e];
+              double v0[R], v1[R], v2[R], v3[R];
+              RowIO<R>::ld(q_lane + o.x, v0);
+              RowIO<R>::ld(q_lane + o.y, v1);
+              RowIO<R>::ld(q_lane + o.z, v2);
+              RowIO<R>::ld(q_lane + o.w, v3);
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                acc[jj][i] += v0[i];
+                a1[i] += v1[i];
+                acc[jj][i] += v2[i];
+                a1[i] += v3[i];
+              }
             }
-            acc[jj] = av;
+#pragma unroll 1
+            for (uint32_t e = g1; e < g2; ++e) {
+              const uint4 o = gent[e];
+              double v0[R], v1[R], v2[R], v3[R];
+              RowIO<R>::ld(q_lane + o.x, v0);
+              RowIO<R>::ld(q_lane + o.y, v1);
+              RowIO<R>::ld(q_lane + o.z, v2);
+              RowIO<R>::ld(q_lane + o.w, v3);
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                acc[jj][i] -= v0[i];
+                a1[i] -= v1[i];
+                acc[jj][i] -= v2[i];
+                a1[i] -= v3[i];
+              }
+            }
+#pragma unroll
+            for (int i = 0; i < R; ++i) acc[jj][i] += a1[i];
           }
         }
       }
@@ -264,45 +452,52 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
 
     // ---------------------------------------------------------------- epilogue (a8 store, a9, a10)
     if (!jac) {
-      if (valid) {
-        const bool wantF = (a.flags & (kOutF | kOutF0)) != 0;
-        double tau = 1.0;
-        if (wantF) tau = a.tau[r];
+      const bool wantF = (a.flags & (kOutF | kOutF0)) != 0;
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        if (valid[i]) {
+          double tau = 1.0;
+          if (wantF) tau = a.tau[r[i]];
+#pragma unroll
+          for (int jj = 0; jj < SPW; ++jj) {
+            const int s = w + NW * jj;
+            if (s < K) {
+              const int64_t o = (int64_t)s * a.ld + r[i];
+              if (a.flags & kOutWdot) a.wdot[o] = acc[jj][i];
+              if (wantF) {
+                const double Fv = (a.Y[o] - a.Yin[o]) / tau - acc[jj][i] * mv.Wm[s] / rho[i];
+                if (a.flags & kOutF) a.F[o] = Fv;
+                if (a.flags & kOutF0) a.F0out[r[i] * n + 1 + s] = Fv;
+              }
+            }
+          }
+          if ((a.flags & kOutF0) && w == 0) a.F0out[r[i] * n] = 0.0;
+        }
+      }
+    } else {
+      // difference quotient, staged [state][npad] in the Cs region, then one linear coalesced store
+      const int npad = n | 1;
+      double* stg = Cs;  // needs TR*npad doubles <= (K+2)*TR (host sizes smem_cs accordingly)
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        const double tau = a.tau[r[i]];
+        const double invh = 1.0 / h[i];
+        const int st = i * 32 + lane;  // position of this state inside the tile, in evaluation order
 #pragma unroll
         for (int jj = 0; jj < SPW; ++jj) {
           const int s = w + NW * jj;
           if (s < K) {
-            const int64_t o = (int64_t)s * a.ld + r;
-            if (a.flags & kOutWdot) a.wdot[o] = acc[jj];
-            if (wantF) {
-              const double Fv = (a.Y[o] - a.Yin[o]) / tau - acc[jj] * mv.Wm[s] / rho;
-              if (a.flags & kOutF) a.F[o] = Fv;
-              if (a.flags & kOutF0) a.F0out[r * n + 1 + s] = Fv;
-            }
+            const int64_t o = (int64_t)s * a.ld + r[i];
+            const double Fv = (load_Y(s, i) - a.Yin[o]) / tau - acc[jj][i] * mv.Wm[s] / rho[i];
+            stg[st * npad + 1 + s] = (Fv - a.F0[r[i] * n + 1 + s]) * invh;
           }
         }
-        if ((a.flags & kOutF0) && w == 0) a.F0out[r * n] = 0.0;
+        if (w == 0) stg[st * npad] = (jsp[i] == -1) ? 1.0 : 0.0;  // row 0: F_T = T - T_set
       }
-    } else {
-      // difference quotient, staged [lane][npad] in the Cs region, then one linear coalesced store
-      const int npad = n | 1;
-      double* stg = Cs;  // needs 32*npad doubles <= K*32 + slack (host sizes smem_cs accordingly)
-      const double tau = a.tau[r];
-      const double invh = 1.0 / h;
-#pragma unroll
-      for (int jj = 0; jj < SPW; ++jj) {
-        const int s = w + NW * jj;
-        if (s < K) {
-          const int64_t o = (int64_t)s * a.ld + r;
-          const double Fv = (load_Y(s) - a.Yin[o]) / tau - acc[jj] * mv.Wm[s] / rho;
-          stg[lane * npad + 1 + s] = (Fv - a.F0[r * n + 1 + s]) * invh;
-        }
-      }
-      if (w == 0) stg[lane * npad] = (jcol == 0) ? 1.0 : 0.0;  // row 0: F_T = T - T_set
       __syncthreads();
-      const int64_t base = tile * kTile * (int64_t)n;
+      const int64_t base = tile * TR * (int64_t)n;
       const int64_t lim = a.N * (int64_t)n * n;
-      for (int idx = threadIdx.x; idx < kTile * n; idx += NW * 32) {
+      for (int idx = threadIdx.x; idx < TR * n; idx += NW * 32) {
         const int l = idx / n, i = idx - l * n;
         if (base + idx < lim) a.J[base + idx] = stg[l * npad + i];
       }
@@ -312,35 +507,40 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
 }
 
 // ------------------------------------------------------------------ launch wrapper
-template <int NW, int SPW>
+#define PSR_SHAPES(X) X(8, 2) X(8, 4) X(8, 8) X(16, 8) X(16, 16) X(16, 32)
+
+template <int NW, int SPW, int R>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  auto kern = psr_eval_kernel<NW, SPW>;
+  auto kern = psr_eval_kernel<NW, SPW, R>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mv.smem_total);
   if (e != cudaSuccess) return e;
   kern<<<grid, NW * 32, mv.smem_total, st>>>(mv, a);
   return cudaGetLastError();
 }
 
-cudaError_t launch_eval(int nw, int spw, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  if (nw == 8 && spw == 2) return launch_t<8, 2>(mv, a, grid, st);
-  if (nw == 8 && spw == 4) return launch_t<8, 4>(mv, a, grid, st);
-  if (nw == 8 && spw == 8) return launch_t<8, 8>(mv, a, grid, st);
-  if (nw == 16 && spw == 8) return launch_t<16, 8>(mv, a, grid, st);
-  if (nw == 16 && spw == 16) return launch_t<16, 16>(mv, a, grid, st);
-  if (nw == 16 && spw == 32) return launch_t<16, 32>(mv, a, grid, st);
+cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
+#define PSR_L(NW_, SPW_)                                                      \
+  if (nw == NW_ && spw == SPW_ && rl == 1) return launch_t<NW_, SPW_, 1>(mv, a, grid, st); \
+  if (nw == NW_ && spw == SPW_ && rl == 2) return launch_t<NW_, SPW_, 2>(mv, a, grid, st);
+  PSR_SHAPES(PSR_L)
+#undef PSR_L
   return cudaErrorInvalidConfiguration;
 }
 
-cudaError_t occupancy_eval(int nw, int spw, size_t smem, int* ctas_per_sm) {
-#define PSR_OCC(NW_, SPW_)                                                                            \
-  if (nw == NW_ && spw == SPW_) {                                                                     \
-    auto kern = psr_eval_kernel<NW_, SPW_>;                                                           \
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-    if (e != cudaSuccess) return e;                                                                   \
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, NW_ * 32, smem);          \
-  }
-  PSR_OCC(8, 2) PSR_OCC(8, 4) PSR_OCC(8, 8) PSR_OCC(16, 8) PSR_OCC(16, 16) PSR_OCC(16, 32)
-#undef PSR_OCC
+template <int NW, int SPW, int R>
+static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
+  auto kern = psr_eval_kernel<NW, SPW, R>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, NW * 32, smem);
+}
+
+cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm) {
+#define PSR_O(NW_, SPW_)                                                   \
+  if (nw == NW_ && spw == SPW_ && rl == 1) return occ_t<NW_, SPW_, 1>(smem, ctas_per_sm); \
+  if (nw == NW_ && spw == SPW_ && rl == 2) return occ_t<NW_, SPW_, 2>(smem, ctas_per_sm);
+  PSR_SHAPES(PSR_O)
+#undef PSR_O
   return cudaErrorInvalidConfiguration;
 }
 
@@ -367,6 +567,19 @@ __global__ void __launch_bounds__(256) probe_kernel(int iters, double* sink) {
   }
   const double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
   if (s == 123.456) sink[0] = s;
+}
+
+// exp_fast on an array (diagnostic behind psr_probe_exp_values)
+__global__ void exp_values_kernel(const double* __restrict__ tab, const double* __restrict__ x, double* __restrict__ y, int n) {
+  __shared__ double etab[kExpTabN];
+  if (threadIdx.x < kExpTabN) etab[threadIdx.x] = tab[threadIdx.x];
+  __syncthreads();
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = exp_fast(x[i], etab);
+}
+
+cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st) {
+  exp_values_kernel<<<148, 256, 0, st>>>(tab, x, y, n);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st) {

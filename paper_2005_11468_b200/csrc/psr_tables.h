@@ -4,12 +4,13 @@
 // The mechanism is cut into chunks of at most `rc` reactions.  Every chunk is one contiguous,
 // 16-byte aligned blob that a CTA pulls into shared memory with a single cp.async.bulk:
 //
-//   ChunkHdr | RxRec[n_rx] | AuxRec[n_aux] | EffEnt[n_eff] | u16 pool | u32 csr_ptr[K+1] | u32 csr_ent[n_csr]
+//   ChunkHdr | RxRec[n_rx] | AuxRec[n_aux] | EffEnt[n_eff] | u16 pool | u32 gptr[2K+1] | u32 gent[n_g]
 //
 // RxRec carries the log-linear rate forms that replace the paper's per-thread pow()/species sums
-// (Eq. 6, 8, 9):  ln k_f = c0 + c1 ln T + c2/T  and
-//   ln K_c = d0 + d1 ln T + d2/T + d3 T + d4 T^2 + d5 T^3 + d6 T^4,
-// the latter being sum_i nu_ik (s_i/R - h_i/RT) + (sum_i nu_ik) ln(P_atm/(R T)) with the NASA-7
+// (Eq. 6, 8, 9):
+//   ln k_f = c0 + c1 ln T + c2/T
+//   ln k_r = ln k_f - ln K_c = e0 + e1 ln T + e2/T + T (d0 + d1 T + d2 T^2 + d3 T^3)
+// where ln K_c = sum_i nu_ik (s_i/R - h_i/RT) + (sum_i nu_ik) ln(P_atm/(R T)) with the NASA-7
 // polynomials summed per reaction at load time (exact in real arithmetic for a single range).
 #ifndef PSR_TABLES_H_
 #define PSR_TABLES_H_
@@ -18,23 +19,27 @@
 namespace psr {
 
 constexpr int kTile = 32;       // reactors per tile = lanes of a warp
-constexpr int kInlineSp = 8;    // factor species stored inline in a reaction record
-constexpr int kMaxSide = 15;    // concentration factors per reaction side
+constexpr int kRowBytes = kTile * 8;  // one species / reaction row of a tile in shared memory
+constexpr int kSlots = 3;       // inline concentration-factor slots per reaction side
+constexpr int kMaxSide = 15;    // concentration factors per reaction side (long form)
+constexpr int kMaxChunkRx = 254;  // rows of the q tile addressable by a gather entry (+1 zero row)
 
 // meta bits
 constexpr uint32_t kMetaTypeMask = 0x3u;      // PSR_RX_*
 constexpr uint32_t kMetaRev = 0x4u;           // reversible
-constexpr uint32_t kMetaLong = 0x8u;          // factor list lives in the u16 pool at sp[0] | sp[1]<<16
-constexpr int kMetaNrShift = 4;               // bits 4..7  reactant factor count
-constexpr int kMetaNpShift = 8;               // bits 8..11 product factor count
+constexpr uint32_t kMetaLong = 0x8u;          // factor list lives in the u16 pool at off[0]; counts in meta
+constexpr int kMetaNrShift = 4;               // bits 4..7  reactant factor count (long form)
+constexpr int kMetaNpShift = 8;               // bits 8..11 product factor count (long form)
 constexpr int kMetaAuxShift = 16;             // bits 16..31 index into AuxRec[]
 
 struct __attribute__((aligned(16))) RxRec {   // 112 bytes
   double c[3];            // ln A, b, -Ea/R_c
-  double d[7];            // ln K_c coefficients over (1, ln T, 1/T, T, T^2, T^3, T^4)
+  double e[3];            // ln k_r coefficients over (1, ln T, 1/T)
+  double d[4];            // ln k_r coefficients over (T, T^2, T^3, T^4)
   uint32_t meta;
+  uint32_t off[2 * kSlots];  // byte offsets of the factor rows in the C tile: 3 reactant slots, 3 product
+                             // slots, nu expanded by repetition, unused slots -> the unit row (index K)
   uint32_t korig;         // caller's reaction index (row of kf/kr/q outputs)
-  uint16_t sp[kInlineSp]; // factor species, reactants then products, nu expanded by repetition
 };
 static_assert(sizeof(RxRec) == 112, "RxRec layout");
 
@@ -48,27 +53,30 @@ static_assert(sizeof(AuxRec) == 80, "AuxRec layout");
 
 struct __attribute__((aligned(16))) EffEnt {  // 16 bytes
   double am1;             // alpha - 1
-  uint32_t sp;
+  uint32_t off;           // byte offset of the species row in the C tile
   uint32_t pad;
 };
 
 struct __attribute__((aligned(16))) ChunkHdr {  // 64 bytes
-  uint32_t n_rx, n_aux, n_eff, n_csr;
-  uint32_t off_aux, off_eff, off_pool, off_csr_ptr, off_csr_ent;
+  uint32_t n_rx, n_aux, n_eff, n_g;
+  uint32_t off_aux, off_eff, off_pool, off_gptr, off_gent;
   uint32_t bytes;         // bytes to copy (multiple of 16)
-  uint32_t k_first;       // first (sorted) reaction index of this chunk
+  uint32_t k_first;       // unused
   uint32_t pad[5];
 };
 static_assert(sizeof(ChunkHdr) == 64, "ChunkHdr layout");
 
-// csr_ent: bits 0..15 local reaction index, bit 16 sign (1 = subtract).  |nu| > 1 repeats the entry.
-constexpr uint32_t kCsrNeg = 0x10000u;
+// Gather lists of nu^T (Eq. 4) per chunk: species s adds the q rows gent[gptr[2s] .. gptr[2s+1]) and
+// subtracts gent[gptr[2s+1] .. gptr[2s+2]).  An entry is the byte offset of a row of the q tile;
+// |nu| > 1 repeats the entry; every group is padded to a multiple of 4 entries with the offset of
+// the all-zero row (index rc) so the inner loop is a branch-free 4-wide step.
 
 // Kernel-side view of a loaded mechanism (passed by value as a kernel parameter).
 struct MechView {
   const unsigned char* chunks;  // n_chunks blobs, chunk_stride bytes apart
   const double* invW;           // [K] 1/W
   const double* Wm;             // [K] W
+  const double* exp_tab;        // [64] 2^(j/64), staged into shared memory by every CTA (psr_math.cuh)
   int32_t K, I;
   int32_t n_chunks, rc;
   uint32_t chunk_stride;        // bytes, multiple of 16

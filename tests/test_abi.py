@@ -1,0 +1,67 @@
+"""The C-ABI library loads without a GPU and exports every symbol include/psr.h declares; host-side
+argument checks that need no device."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import numpy as np
+
+from paper_2005_11468_b200 import binding, synth
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "psr.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(psr_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_loads_and_exports_every_declared_symbol():
+    lib = binding.lib()          # dlopen resolves every internal symbol (RTLD_NOW semantics of ctypes)
+    syms = declared_symbols()
+    assert {"psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
+            "psr_fd_jacobian", "psr_last_error"} <= set(syms)
+    for s in syms:
+        assert hasattr(lib, s), s
+    assert set(binding.EXPORTS) == set(syms)
+    assert b"sm_100a" in lib.psr_version()
+
+
+def test_mech_load_rejects_malformed_descriptions_before_touching_the_device():
+    mech, _ = synth.make_config("C0", 1)
+    lib = binding.lib()
+
+    def status(arrays, K=mech.n_species, I=mech.n_reactions):
+        desc, keep = binding.make_desc(K, I, arrays)
+        h = C.c_void_p()
+        st = lib.psr_mech_load(C.byref(desc), C.byref(h))
+        assert h.value is None or st == 0
+        if st == 0:
+            lib.psr_mech_free(h)
+        return st, lib.psr_last_error().decode()
+
+    a = mech.arrays()
+    bad = dict(a); bad["W"] = a["W"].copy(); bad["W"][3] = 0.0
+    assert status(bad)[0] == binding.PSR_EINVAL
+    bad = dict(a); bad["reac_sp"] = a["reac_sp"].copy(); bad["reac_sp"][0] = mech.n_species
+    st, msg = status(bad); assert st == binding.PSR_EINVAL and "out of range" in msg
+    bad = dict(a); bad["reac_nu"] = a["reac_nu"].copy(); bad["reac_nu"][0] = 4
+    assert status(bad)[0] == binding.PSR_EINVAL
+    bad = dict(a); bad["rtype"] = a["rtype"].copy(); bad["rtype"][0] = 7
+    assert status(bad)[0] == binding.PSR_EINVAL
+    bad = dict(a); bad["A"] = a["A"].copy(); bad["A"][0] = -1.0
+    assert status(bad)[0] == binding.PSR_EINVAL
+    bad = dict(a); bad["nasa"] = None
+    assert status(bad)[0] == binding.PSR_EINVAL
+    assert status(a, K=0)[0] == binding.PSR_EINVAL
+    assert status(a, K=513)[0] in (binding.PSR_EINVAL, binding.PSR_EUNSUPPORTED)
+
+
+def test_eval_calls_validate_arguments_without_a_device():
+    lib = binding.lib()
+    null = C.c_void_p()
+    assert lib.psr_eval_wdot(null, 4, null, null, null, 4, null, null, 0, null) == binding.PSR_EINVAL
+    assert b"null mechanism" in lib.psr_last_error()
+    assert lib.psr_eval_kf_kr(null, -1, null, null, null, 0, null, null, 0, null) == binding.PSR_EINVAL
+    assert lib.psr_fd_jacobian(null, 1, null, null, null, null, null, 1, null, null, null) == binding.PSR_EINVAL

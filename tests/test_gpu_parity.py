@@ -256,3 +256,29 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     assert np.all(J[:, 0, 0] == 1.0) and np.all(J[:, 1:, 0] == 0.0)
     assert np.all(F0[:, 0] == 0.0)
     assert residual_rel_err(F0[:, 1:].T, jd["F0"][:, 1:].T).max() <= TOL_F
+
+
+# ------------------------------------------------------------------ kernel math
+def test_table_exp_accuracy(torch_cuda, binding):
+    """csrc/psr_math.cuh exp_fast against mpmath (50 digits): <= 4e-16 relative over the argument
+    range the rate forms reach, exact special values, library path beyond |x| >= 700 and for NaN/Inf."""
+    import mpmath
+    mech, _ = synth.make_config("C0", 1)
+    gm = binding.Mechanism.from_synth(mech)
+    rng = np.random.default_rng(7)
+    x = np.concatenate([rng.uniform(-700, 700, 20000), rng.uniform(-1, 1, 5000), rng.uniform(-1e-3, 1e-3, 2000),
+                        np.arange(-64, 65) * np.log(2) / 64, [0.0, -0.0, 699.999, -699.999, 1e-300]])
+    y = gm.probe_exp_values(x)
+    mpmath.mp.dps = 50
+    ref = np.array([float(mpmath.exp(mpmath.mpf(float(v)))) for v in x])
+    err = np.abs(y - ref) / ref
+    assert err.max() <= 4e-16, err.max()
+    assert np.all(y[x == 0.0] == 1.0)
+    edge = np.array([700.0, 709.7, 710.0, -708.0, -745.0, -800.0, np.inf, -np.inf, np.nan])
+    ye = gm.probe_exp_values(edge)
+    with np.errstate(over="ignore"):
+        ne = np.exp(edge)
+    assert np.isnan(ye[-1]) and ye[6] == np.inf and ye[7] == 0.0 and ye[2] == np.inf and ye[5] == 0.0
+    fin = np.isfinite(ne) & (ne > 1e-300)
+    assert np.all(np.abs(ye[fin] - ne[fin]) <= 4e-16 * ne[fin])
+    gm.close()
