@@ -14,7 +14,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpsr_b200.so"
 SOURCES = [CSRC / "psr_api.cu", CSRC / "psr_kernels.cu"]
-HEADERS = [CSRC / "psr_tables.h", PKG.parent / "include" / "psr.h"]
+HEADERS = [CSRC / "psr_tables.h", CSRC / "psr_math.cuh", PKG.parent / "include" / "psr.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -35,6 +35,7 @@ struct psr_mech {
   double* d_invW = nullptr;
   double* d_W = nullptr;
   double* d_exptab = nullptr;
+  int32_t* d_sp_of = nullptr;
   double* d_scratch = nullptr;  // internal F0 buffer for psr_fd_jacobian when the caller passes none
   size_t scratch_bytes = 0;
   int device = 0;
@@ -66,9 +67,9 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 double reaction_cost(int type) {  // relative FP64 cost used to balance warps inside a chunk
   switch (type) {
-    case PSR_RX_THREE_BODY: return 1.2;
-    case PSR_RX_LINDEMANN: return 1.8;
-    case PSR_RX_TROE: return 4.5;
+    case PSR_RX_THREE_BODY: return 1.25;
+    case PSR_RX_LINDEMANN: return 2.0;
+    case PSR_RX_TROE: return 4.0;
     default: return 1.0;
   }
 }
@@ -203,21 +204,39 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     for (auto& pr : h.nu_net) nnz += std::abs(pr.second);
   }
 
+  // ---- device
+  int dev = 0, n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess || n_dev == 0) return fail(PSR_ECUDA, "psr_mech_load: no CUDA device (%s)", cudaGetErrorString(e));
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDeviceProperties");
+
   // ---- launch shape
-  int nw, spw;
-  if (K <= 16) { nw = 8; spw = 2; }
-  else if (K <= 32) { nw = 8; spw = 4; }
-  else if (K <= 64) { nw = 8; spw = 8; }
-  else if (K <= 128) { nw = 16; spw = 8; }
-  else if (K <= 256) { nw = 16; spw = 16; }
-  else { nw = 16; spw = 32; }
-  int rl = spw <= 8 ? 2 : 1;  // reactors per lane: 2 while the wdot accumulators fit in registers
+  int nw = 16;
+  if (const char* e = getenv("PSR_NW")) nw = atoi(e) == 16 ? 16 : 8;
+  int spw = 2;  // species per warp in the gather: smallest compiled shape with nw * spw >= K
+  while (nw * spw < K) spw *= 2;
+  if (spw > 32 || (nw == 8 && spw > 8)) { nw = 16; spw = 2; while (nw * spw < K) spw *= 2; }
+  int rl = 1;  // reactors per lane (2 is compiled for spw <= 16; PSR_R selects it)
   if (const char* e = getenv("PSR_R")) rl = (atoi(e) == 2 && spw <= 16) ? 2 : 1;
   const uint32_t row_bytes = (uint32_t)kRowBytes * rl;
-  int rc_target = 128;
+  int rc_target = 192;
   if (const char* e = getenv("PSR_RC")) rc_target = std::min(kMaxChunkRx, std::max(8, atoi(e)));
-  const int n_chunks = (I + rc_target - 1) / rc_target;
-  const int rc = (I + n_chunks - 1) / n_chunks;  // <= rc_target <= kMaxChunkRx
+  // shared memory left for the q tile and the chunk ring beside one C tile and the per-CTA scratch
+  const size_t smem_fixed = align_up((size_t)(K + 2) * kTile * rl * 8, 128) + (size_t)2 * nw * kTile * rl * 8 +
+                            (size_t)6 * kTile * rl * 8 + 64;
+  int n_chunks = 0, rc = 0;
+  size_t stride = 0;
+  std::vector<unsigned char> all;
+  std::vector<int32_t> sp_of;
+  // the chunk size shrinks until one C tile, the q tile and the (double-buffered) chunk ring fit one CTA
+  for (;; rc_target = rc_target * 3 / 4) {
+  if (rc_target < 8)
+    return fail(PSR_EUNSUPPORTED, "mechanism does not fit %zu bytes of shared memory per CTA even at 8 reactions per chunk",
+                (size_t)prop.sharedMemPerBlockOptin);
+  n_chunks = (I + rc_target - 1) / rc_target;
+  rc = (I + n_chunks - 1) / n_chunks;  // <= rc_target <= kMaxChunkRx
 
   // ---- distribute reactions over chunks (each type dealt round-robin so chunks cost the same),
   //      then inside a chunk order by cost and deal to warps in snake order.
@@ -226,22 +245,47 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return reaction_cost(rx[x].type) > reaction_cost(rx[y].type); });
   std::vector<std::vector<int>> chunk_rx(n_chunks);
   for (int p = 0; p < I; ++p) chunk_rx[p % n_chunks].push_back(order[p]);
-  for (auto& cr : chunk_rx) {
-    // cr is cost-descending; snake-deal: position = round*nw + warp
-    const int n = (int)cr.size();
-    std::vector<int> placed(n, -1);
-    for (int p = 0; p < n; ++p) {
-      const int round = p / nw, idx = p % nw;
-      const bool last_partial = (round == n / nw);
-      const int warp = (round % 2 == 0 || last_partial) ? idx : nw - 1 - idx;
-      placed[round * nw + warp] = cr[p];
+  // inside a chunk: longest-processing-time assignment of records to warps, records of a warp contiguous
+  std::vector<std::vector<int>> chunk_wptr(n_chunks);
+  for (int c = 0; c < n_chunks; ++c) {
+    auto& cr = chunk_rx[c];  // cost-descending
+    std::vector<double> load(nw, 0.0);
+    std::vector<std::vector<int>> mine(nw);
+    for (int k : cr) {
+      const int wmin = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+      mine[wmin].push_back(k);
+      load[wmin] += reaction_cost(rx[k].type);
     }
-    cr = placed;
+    cr.clear();
+    chunk_wptr[c].assign(nw + 1, 0);
+    for (int wv = 0; wv < nw; ++wv) {
+      cr.insert(cr.end(), mine[wv].begin(), mine[wv].end());
+      chunk_wptr[c][wv + 1] = (int)cr.size();
+    }
+  }
+  // gather ownership: species to (warp, slot) by longest-processing-time on the row length of nu^T
+  sp_of.assign((size_t)nw * spw, -1);
+  {
+    std::vector<int> rowlen(K, 0);
+    for (int k = 0; k < I; ++k)
+      for (auto& pr : rx[k].nu_net) rowlen[pr.first] += std::abs(pr.second);
+    std::vector<int> sorder(K);
+    std::iota(sorder.begin(), sorder.end(), 0);
+    std::stable_sort(sorder.begin(), sorder.end(), [&](int x, int y) { return rowlen[x] > rowlen[y]; });
+    std::vector<double> load(nw, 0.0);
+    std::vector<int> used(nw, 0);
+    for (int sidx : sorder) {
+      int best = -1;
+      for (int wv = 0; wv < nw; ++wv)
+        if (used[wv] < spw && (best < 0 || load[wv] < load[best])) best = wv;
+      sp_of[(size_t)best * spw + used[best]++] = sidx;
+      load[best] += rowlen[sidx] + 6.0;  // + per-species loop overhead
+    }
   }
 
   // ---- serialise chunk blobs
   std::vector<std::vector<unsigned char>> blobs(n_chunks);
-  size_t stride = 0;
+  stride = 0;
   const uint32_t unit_off = (uint32_t)K * row_bytes;   // the all-ones row of the C tile
   const uint32_t zero_off = (uint32_t)rc * row_bytes;  // the all-zero row of the q tile
   for (int c = 0; c < n_chunks; ++c) {
@@ -299,6 +343,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     hdr.n_aux = (uint32_t)auxs.size();
     hdr.n_eff = (uint32_t)effs.size();
     hdr.n_g = (uint32_t)gent.size();
+    for (int wv = 0; wv <= nw; ++wv) hdr.wptr[wv] = (uint8_t)chunk_wptr[c][wv];
+    for (int wv = nw + 1; wv < 24; ++wv) hdr.wptr[wv] = (uint8_t)n_rx;
     size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
     hdr.off_aux = (uint32_t)off;
     off += sizeof(AuxRec) * auxs.size();
@@ -323,16 +369,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     stride = std::max(stride, off);
   }
   stride = align_up(stride, 128);
-  std::vector<unsigned char> all(stride * n_chunks, 0);
+  const size_t need = smem_fixed + align_up((size_t)(rc + 1) * kTile * rl * 8, 128) + stride * (n_chunks == 1 ? 1 : 2);
+  if (need > (size_t)prop.sharedMemPerBlockOptin) continue;
+  all.assign(stride * n_chunks, 0);
   for (int c = 0; c < n_chunks; ++c) std::memcpy(all.data() + stride * c, blobs[c].data(), blobs[c].size());
-
-  // ---- device
-  int dev = 0, n_dev = 0;
-  cudaError_t e = cudaGetDeviceCount(&n_dev);
-  if (e != cudaSuccess || n_dev == 0) return fail(PSR_ECUDA, "psr_mech_load: no CUDA device (%s)", cudaGetErrorString(e));
-  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
-  cudaDeviceProp prop;
-  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDeviceProperties");
+  break;
+  }
 
   psr_mech* m = new (std::nothrow) psr_mech();
   if (!m) return fail(PSR_ENOMEM, "psr_mech_load: host allocation failed");
@@ -351,16 +393,25 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.n_chunks = n_chunks;
   v.rc = rc;
   v.chunk_stride = (uint32_t)stride;
-  size_t o = 0;
-  v.smem_cs = (uint32_t)o;
-  o += align_up((size_t)(K + 2) * kTile * rl * 8, 128);  // K rows of C; K+2 so the Jacobian staging [tile][n|1] fits
-  v.smem_q = (uint32_t)o;
-  o += align_up((size_t)(rc + 1) * kTile * rl * 8, 128);  // + the all-zero row
-  v.smem_mech = (uint32_t)o;
-  o += stride * (n_chunks == 1 ? 1 : 2);
-  v.smem_misc = (uint32_t)o;
-  o += (size_t)2 * nw * kTile * rl * 8 + (size_t)kTile * rl * 8 + 64 * 8 + 64;  // partial sums, per-lane scalars, exp table, mbarriers
-  v.smem_total = (uint32_t)o;
+  const size_t cbuf_bytes = align_up((size_t)(K + 2) * kTile * rl * 8, 128);  // K+2 rows so the Jacobian staging [tile][n|1] fits
+  auto carve = [&](int n_cbuf) {
+    size_t o = 0;
+    v.smem_cs = (uint32_t)o;
+    o += n_cbuf * cbuf_bytes;
+    v.smem_q = (uint32_t)o;
+    o += align_up((size_t)(rc + 1) * kTile * rl * 8, 128);  // + the all-zero row
+    v.smem_mech = (uint32_t)o;
+    o += stride * (n_chunks == 1 ? 1 : 2);
+    v.smem_misc = (uint32_t)o;
+    o += (size_t)2 * nw * kTile * rl * 8 + (size_t)6 * kTile * rl * 8 + 64;  // partial sums; ln T, h, T/P prefetch; mbarriers
+    v.smem_total = (uint32_t)o;
+    v.n_cbuf = n_cbuf;
+    return o;
+  };
+  // two C buffers (next tile prefetched under this tile's chunks) unless that costs a resident CTA
+  const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin, half = (size_t)prop.sharedMemPerMultiprocessor / 2 - 1024;
+  size_t o = carve(2);
+  if (o > smem_max || (o > half && carve(1) <= half)) o = carve(1);
   if (o > (size_t)prop.sharedMemPerBlockOptin) {
     delete m;
     return fail(PSR_EUNSUPPORTED, "mechanism needs %zu bytes of shared memory per CTA, device allows %zu", o,
@@ -379,14 +430,20 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     return cuda_fail(e, "cudaMemcpy (mechanism upload)");
   }
   {
-    double tab[64];
-    for (int j = 0; j < 64; ++j) tab[j] = (double)exp2l((long double)j / 64.0L);
+    double tab[32];
+    for (int j = 0; j < 32; ++j) tab[j] = (double)exp2l((long double)j / 32.0L);
     if ((e = cudaMalloc(&m->d_exptab, sizeof tab)) != cudaSuccess ||
         (e = cudaMemcpy(m->d_exptab, tab, sizeof tab, cudaMemcpyHostToDevice)) != cudaSuccess) {
       cleanup();
       return cuda_fail(e, "exp table upload");
     }
   }
+  if ((e = cudaMalloc(&m->d_sp_of, 4 * sp_of.size())) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_sp_of, sp_of.data(), 4 * sp_of.size(), cudaMemcpyHostToDevice)) != cudaSuccess) {
+    cleanup();
+    return cuda_fail(e, "species ownership upload");
+  }
+  v.sp_of = m->d_sp_of;
   v.exp_tab = m->d_exptab;
   v.chunks = m->d_chunks;
   v.invW = m->d_invW;
@@ -405,6 +462,7 @@ void psr_mech_free(psr_mech* m) {
   cudaFree(m->d_invW);
   cudaFree(m->d_W);
   cudaFree(m->d_exptab);
+  cudaFree(m->d_sp_of);
   cudaFree(m->d_scratch);
   delete m;
 }

@@ -52,6 +52,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   } while (!done);
 }
 
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_global) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src_global) : "memory");
+}
+__device__ __forceinline__ double ldg_nc(const double* p) {
+  double v;
+  asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+
 // ------------------------------------------------------------------ shared-memory access by 32-bit address
 // (volatile so that loads are neither merged across tiles nor moved over barriers by the front end)
 __device__ __forceinline__ double lds64(uint32_t addr) {
@@ -79,20 +88,24 @@ struct RowIO<2> {
   }
 };
 
+#ifndef PSR_MINB
+#define PSR_MINB(NW) ((NW) == 8 ? 2 : 1)   // CTAs per SM the register allocation is held to (128 regs/thread)
+#endif
 // ------------------------------------------------------------------ the fused kernel
 // R reactors per lane: every warp-uniform instruction (mechanism loads, address arithmetic, branches)
 // is amortised over R evaluations and the R exp chains interleave in the FP64 pipe.
 template <int NW, int SPW, int R>
-__global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, const EvalArgs a) {
+__global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const MechView mv, const EvalArgs a) {
   constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
-  double* Cs = reinterpret_cast<double*>(smem + mv.smem_cs);          // [K+2][TR]; row K is the unit row
+  double* Cs0 = reinterpret_cast<double*>(smem + mv.smem_cs);         // [2][K+2][TR]; row K is the unit row
   double* qs = reinterpret_cast<double*>(smem + mv.smem_q);           // [rc+1][TR]; row rc stays zero
   unsigned char* mring = smem + mv.smem_mech;                         // stages * chunk_stride
   double* part = reinterpret_cast<double*>(smem + mv.smem_misc);      // [2][NW][TR] partial sums
   double* lane_s = part + 2 * NW * TR;                                // [TR]: ln T per state
-  double* etab = lane_s + TR;                                         // [64] 2^(j/64)
-  uint64_t* bars = reinterpret_cast<uint64_t*>(etab + kExpTabN);      // [2]
+  double* hs = lane_s + TR;                                           // [TR]: finite-difference step per state
+  double* tp = hs + TR;                                               // [2][2][TR]: prefetched T, P
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [2]
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -100,7 +113,7 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
   const int n = K + 1;
   const bool jac = (a.flags & kModeJac) != 0;
   const int nstage = mv.n_chunks == 1 ? 1 : 2;
-  const uint32_t c_lane = smem_u32(Cs) + lane * (8 * R);   // this lane's R slots of row 0 of the C tile
+  const int cs_elems = (K + 2) * TR;
   const uint32_t q_lane = smem_u32(qs) + lane * (8 * R);
 
   const int64_t my_tiles = (a.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
@@ -117,67 +130,88 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
                mv.chunk_stride, &bars[g]);
     }
   }
-  if (threadIdx.x < kExpTabN) etab[threadIdx.x] = mv.exp_tab[threadIdx.x];
+  const ExpTab etab = exp_tab_load(mv.exp_tab);
+  int sp[SPW];  // species this warp owns in the prologue, gather and epilogue
+#pragma unroll
+  for (int jj = 0; jj < SPW; ++jj) sp[jj] = mv.sp_of[w * SPW + jj];
   if (w == 0) {
 #pragma unroll
     for (int i = 0; i < R; ++i) qs[mv.rc * TR + lane * R + i] = 0.0;
   }
+
+  // state i of this lane in tile t is evaluation v = t*TR + i*32 + lane (coalesced global access); in
+  // shared memory it lives at column lane*R + i of every row.  Jacobian mode: v = reactor*n + column.
+  auto state_of = [&](int64_t t, int i, int64_t& r_, int& jsp_, bool& valid_) {
+    const int64_t v = t * TR + i * 32 + lane;
+    if (jac) {
+      valid_ = v < a.N * n;
+      const int64_t vv = valid_ ? v : a.N * n - 1;
+      r_ = vv / n;
+      jsp_ = (int)(vv - r_ * n) - 1;   // perturbed species; -1: the T column
+    } else {
+      valid_ = v < a.N;
+      r_ = valid_ ? v : a.N - 1;
+      jsp_ = -2;                      // nothing perturbed
+    }
+  };
+  // asynchronous prefetch of a tile's T, P (warp 0) and of this thread's Y entries into C buffer `buf`
+  auto prefetch = [&](int64_t t, int buf) {
+    if (t < a.n_tiles) {
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        int64_t r_;
+        int jsp_;
+        bool valid_;
+        state_of(t, i, r_, jsp_, valid_);
+        const int col = lane * R + i;
+        if (w == 0) {
+          cp_async8(tp + (buf * 2 + 0) * TR + col, a.T + r_);
+          cp_async8(tp + (buf * 2 + 1) * TR + col, a.P + r_);
+        }
+#pragma unroll
+        for (int jj = 0; jj < SPW; ++jj)
+          if (sp[jj] >= 0) cp_async8(Cs0 + buf * cs_elems + sp[jj] * TR + col, a.Y + (int64_t)sp[jj] * a.ld + r_);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  prefetch(blockIdx.x, 0);
   __syncthreads();
 
   int64_t g = 0;  // chunk loads consumed so far by this CTA
-  for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
+  int buf = 0;
+  for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x, buf ^= (mv.n_cbuf - 1)) {
     // ---------------------------------------------------------------- prologue (a1)
-    // state i of this lane is evaluation v = tile*TR + i*32 + lane (coalesced global access); in shared
-    // memory it lives at column lane*R + i of every row.
+    double* Cs = Cs0 + buf * cs_elems;
+    const uint32_t c_lane = smem_u32(Cs) + lane * (8 * R);   // this lane's R slots of row 0 of the C tile
     int64_t r[R];
-    int jsp[R];      // perturbed species (Jacobian mode), -1: T column, -2: none
+    int jsp[R];
     bool valid[R];
-    double T[R], P[R], h[R], ypert[R];
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
-      const int64_t v = tile * TR + i * 32 + lane;
-      int jcol = -1;
-      if (jac) {
-        valid[i] = v < a.N * n;
-        const int64_t vv = valid[i] ? v : a.N * n - 1;
-        r[i] = vv / n;
-        jcol = (int)(vv - r[i] * n);
-      } else {
-        valid[i] = v < a.N;
-        r[i] = valid[i] ? v : a.N - 1;
-      }
-      T[i] = a.T[r[i]];
-      P[i] = a.P[r[i]];
-      // forward-difference step of this state's column: x' = fl(x + delta), h = fl(x' - x)  (O11, g15)
-      jsp[i] = jcol - 1;
-      h[i] = 1.0;
-      ypert[i] = 0.0;
-      if (jcol == 0) {
-        const double Tp = T[i] + 1e-8 * fmax(fabs(T[i]), 1e-10);
-        h[i] = Tp - T[i];
-        T[i] = Tp;
-      } else if (jcol > 0) {
-        const double y = a.Y[(int64_t)jsp[i] * a.ld + r[i]];
-        ypert[i] = y + 1e-8 * fmax(fabs(y), 1e-10);
-        h[i] = ypert[i] - y;
-      }
-    }
-    auto load_Y = [&](int s, int i) -> double { return s == jsp[i] ? ypert[i] : a.Y[(int64_t)s * a.ld + r[i]]; };
+    for (int i = 0; i < R; ++i) state_of(tile, i, r[i], jsp[i], valid[i]);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");   // this thread's prefetched entries have landed
 
-    double rho[R];
+    double T[R], rho[R];
     {
+      // x' = fl(x + delta), h = fl(x' - x) for the perturbed unknown of a Jacobian state (O11, g15)
       double yv[SPW][R];
       double sumYW[R];
 #pragma unroll
       for (int i = 0; i < R; ++i) sumYW[i] = 0.0;
 #pragma unroll
       for (int jj = 0; jj < SPW; ++jj) {
-        const int s = w + NW * jj;
+        const int s = sp[jj];
 #pragma unroll
         for (int i = 0; i < R; ++i) {
           yv[jj][i] = 0.0;
-          if (s < K) {
-            yv[jj][i] = load_Y(s, i) * mv.invW[s];
+          if (s >= 0) {
+            double y = Cs[s * TR + lane * R + i];
+            if (s == jsp[i]) {
+              const double yp = y + 1e-8 * fmax(fabs(y), 1e-10);
+              hs[lane * R + i] = yp - y;
+              y = yp;
+            }
+            yv[jj][i] = y * mv.invW[s];
             sumYW[i] += yv[jj][i];
           }
         }
@@ -186,26 +220,32 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
       for (int i = 0; i < R; ++i) part[w * TR + lane * R + i] = sumYW[i];
       if (w == 0) {
 #pragma unroll
-        for (int i = 0; i < R; ++i) {
-          lane_s[lane * R + i] = log(T[i]);
-          Cs[K * TR + lane * R + i] = 1.0;
-        }
+        for (int i = 0; i < R; ++i) Cs[K * TR + lane * R + i] = 1.0;
       }
-      __syncthreads();
+      __syncthreads();   // partial sums and warp 0's T, P visible; every warp has left the previous tile
+      if (mv.n_cbuf == 2) prefetch(tile + gridDim.x, buf ^ 1);
       double cpart[R];
 #pragma unroll
       for (int i = 0; i < R; ++i) {
+        T[i] = tp[(buf * 2 + 0) * TR + lane * R + i];
+        const double P = tp[(buf * 2 + 1) * TR + lane * R + i];
+        if (jsp[i] == -1) {
+          const double Tp = T[i] + 1e-8 * fmax(fabs(T[i]), 1e-10);
+          if (w == 0) hs[lane * R + i] = Tp - T[i];
+          T[i] = Tp;
+        }
+        if (w == 0) lane_s[lane * R + i] = log(T[i]);
         double sY = 0.0;
 #pragma unroll
         for (int ww = 0; ww < NW; ++ww) sY += part[ww * TR + lane * R + i];
         const double Wbar = 1.0 / sY;
-        rho[i] = P[i] * Wbar / (kRgas * T[i]);
+        rho[i] = P * Wbar / (kRgas * T[i]);
         cpart[i] = 0.0;
       }
 #pragma unroll
       for (int jj = 0; jj < SPW; ++jj) {
-        const int s = w + NW * jj;
-        if (s < K) {
+        const int s = sp[jj];
+        if (s >= 0) {
 #pragma unroll
           for (int i = 0; i < R; ++i) {
             const double c = rho[i] * yv[jj][i];
@@ -237,18 +277,85 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
 #pragma unroll
       for (int i = 0; i < R; ++i) acc[jj][i] = 0.0;
 
-    // ---------------------------------------------------------------- chunks
-    for (int c = 0; c < mv.n_chunks; ++c) {
-      const int stage = (int)(g % nstage);
-      if (mv.n_chunks > 1 || g == 0) mbar_wait(&bars[stage], (uint32_t)((g / nstage) & 1));
-      const unsigned char* blob = mring + (size_t)stage * mv.chunk_stride;
-      const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
-      const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
-      const int n_rx = (int)hdr->n_rx;
+    const bool wantF = (a.flags & (kOutF | kOutF0 | kModeJac)) != 0;
 
-      // ---- reaction phase (a3..a7): warp w takes records w, w+NW, ...
+    // ---------------------------------------------------------------- chunks
+    int stage = 0;
+    const unsigned char* blob = nullptr;
+    const ChunkHdr* hdr = nullptr;
+    // gather (a8, Eq. 4) of the chunk in `stage`: every warp sums the rows of nu^T it owns in a fixed
+    // order; afterwards the stage is handed back to the bulk-copy ring
+    auto gather_and_release = [&]() {
+      if (a.flags & (kOutWdot | kOutF | kModeJac | kOutF0)) {
+        const uint32_t* gptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_gptr);
+        const uint4* gent = reinterpret_cast<const uint4*>(blob + hdr->off_gent);
+#pragma unroll
+        for (int jj = 0; jj < SPW; ++jj) {
+          const int s = sp[jj];
+          if (s >= 0) {
+            const uint32_t g0 = gptr[2 * s] >> 2, g1 = gptr[2 * s + 1] >> 2, g2 = gptr[2 * s + 2] >> 2;
+            double a1[R];
+#pragma unroll
+            for (int i = 0; i < R; ++i) a1[i] = 0.0;
 #pragma unroll 1
-      for (int kl = w; kl < n_rx; kl += NW) {
+            for (uint32_t e = g0; e < g1; ++e) {
+              const uint4 o = gent[e];
+              double v0[R], v1[R], v2[R], v3[R];
+              RowIO<R>::ld(q_lane + o.x, v0);
+              RowIO<R>::ld(q_lane + o.y, v1);
+              RowIO<R>::ld(q_lane + o.z, v2);
+              RowIO<R>::ld(q_lane + o.w, v3);
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                acc[jj][i] += v0[i];
+                a1[i] += v1[i];
+                acc[jj][i] += v2[i];
+                a1[i] += v3[i];
+              }
+            }
+#pragma unroll 1
+            for (uint32_t e = g1; e < g2; ++e) {
+              const uint4 o = gent[e];
+              double v0[R], v1[R], v2[R], v3[R];
+              RowIO<R>::ld(q_lane + o.x, v0);
+              RowIO<R>::ld(q_lane + o.y, v1);
+              RowIO<R>::ld(q_lane + o.z, v2);
+              RowIO<R>::ld(q_lane + o.w, v3);
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                acc[jj][i] -= v0[i];
+                a1[i] -= v1[i];
+                acc[jj][i] -= v2[i];
+                a1[i] -= v3[i];
+              }
+            }
+#pragma unroll
+            for (int i = 0; i < R; ++i) acc[jj][i] += a1[i];
+          }
+        }
+      }
+      __syncthreads();
+      if (mv.n_chunks > 1) {
+        if (threadIdx.x == 0 && g + nstage < total_loads) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          mbar_expect_tx(&bars[stage], mv.chunk_stride);
+          bulk_g2s(mring + (size_t)stage * mv.chunk_stride,
+                   mv.chunks + (size_t)((g + nstage) % mv.n_chunks) * mv.chunk_stride, mv.chunk_stride, &bars[stage]);
+        }
+      }
+      ++g;
+    };
+    for (int c = 0; c < mv.n_chunks; ++c) {
+      stage = (int)(g % nstage);
+      if (mv.n_chunks > 1 || g == 0) mbar_wait(&bars[stage], (uint32_t)((g / nstage) & 1));
+      blob = mring + (size_t)stage * mv.chunk_stride;
+      hdr = reinterpret_cast<const ChunkHdr*>(blob);
+      const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
+
+      // ---- reaction phase (a3..a7): warp w takes its cost-balanced share of the chunk's records
+      const int kl_end = hdr->wptr[w + 1];
+#pragma unroll 1
+      for (int kl = hdr->wptr[w]; kl < kl_end; ++kl) {
         const RxRec* rec = recs + kl;
         const uint32_t meta = rec->meta;
         const int type = (int)(meta & kMetaTypeMask);
@@ -300,7 +407,8 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
         if (type <= PSR_T_THREE_BODY) {
           bool ok = true;
 #pragma unroll
-          for (int i = 0; i < R; ++i) ok = ok && exp_in_range(lnkf[i], lnkr[i]);
+          for (int i = 0; i < R; ++i) ok = ok && exp_in_range(lnkf[i]) && exp_in_range(lnkr[i]);
+          ok = __all_sync(kFullMask, ok);
           if (ok) {
 #pragma unroll
             for (int i = 0; i < R; ++i) {
@@ -389,83 +497,45 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
       }
       __syncthreads();
 
-      // ---- gather phase (a8, Eq. 4): warp w owns species w, w+NW, ...; fixed summation order
-      if (a.flags & (kOutWdot | kOutF | kModeJac | kOutF0)) {
-        const uint32_t* gptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_gptr);
-        const uint4* gent = reinterpret_cast<const uint4*>(blob + hdr->off_gent);
+      if (c + 1 < mv.n_chunks) gather_and_release();
+    }
+
+    // operands of the epilogue are requested now so that they arrive during the last gather
+    double e_tau[R], e_y[SPW][R], e_yin[SPW][R], e_f0[SPW][R];
+      if (wantF) {
 #pragma unroll
-        for (int jj = 0; jj < SPW; ++jj) {
-          const int s = w + NW * jj;
-          if (s < K) {
-            const uint32_t g0 = gptr[2 * s] >> 2, g1 = gptr[2 * s + 1] >> 2, g2 = gptr[2 * s + 2] >> 2;
-            double a1[R];
+        for (int i = 0; i < R; ++i) {
+          e_tau[i] = ldg_nc(a.tau + r[i]);
 #pragma unroll
-            for (int i = 0; i < R; ++i) a1[i] = 0.0;
-#pragma unroll 1
-            for (uint32_t e = g0; e < g1; ++e) {
-              const uint4 o = gent[e];
-              double v0[R], v1[R], v2[R], v3[R];
-              RowIO<R>::ld(q_lane + o.x, v0);
-              RowIO<R>::ld(q_lane + o.y, v1);
-              RowIO<R>::ld(q_lane + o.z, v2);
-              RowIO<R>::ld(q_lane + o.w, v3);
-#pragma unroll
-              for (int i = 0; i < R; ++i) {
-                acc[jj][i] += v0[i];
-                a1[i] += v1[i];
-                acc[jj][i] += v2[i];
-                a1[i] += v3[i];
-              }
+          for (int jj = 0; jj < SPW; ++jj) {
+            const int s = sp[jj];
+            if (s >= 0) {
+              const int64_t o = (int64_t)s * a.ld + r[i];
+              e_y[jj][i] = ldg_nc(a.Y + o);
+              e_yin[jj][i] = ldg_nc(a.Yin + o);
+              if (jac) e_f0[jj][i] = ldg_nc(a.F0 + r[i] * n + 1 + s);
             }
-#pragma unroll 1
-            for (uint32_t e = g1; e < g2; ++e) {
-              const uint4 o = gent[e];
-              double v0[R], v1[R], v2[R], v3[R];
-              RowIO<R>::ld(q_lane + o.x, v0);
-              RowIO<R>::ld(q_lane + o.y, v1);
-              RowIO<R>::ld(q_lane + o.z, v2);
-              RowIO<R>::ld(q_lane + o.w, v3);
-#pragma unroll
-              for (int i = 0; i < R; ++i) {
-                acc[jj][i] -= v0[i];
-                a1[i] -= v1[i];
-                acc[jj][i] -= v2[i];
-                a1[i] -= v3[i];
-              }
-            }
-#pragma unroll
-            for (int i = 0; i < R; ++i) acc[jj][i] += a1[i];
           }
         }
       }
-      __syncthreads();
-      if (mv.n_chunks > 1) {
-        if (threadIdx.x == 0 && g + nstage < total_loads) {
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          mbar_expect_tx(&bars[stage], mv.chunk_stride);
-          bulk_g2s(mring + (size_t)stage * mv.chunk_stride,
-                   mv.chunks + (size_t)((g + nstage) % mv.n_chunks) * mv.chunk_stride, mv.chunk_stride, &bars[stage]);
-        }
-      }
-      ++g;
-    }
+
+    gather_and_release();
 
     // ---------------------------------------------------------------- epilogue (a8 store, a9, a10)
     if (!jac) {
-      const bool wantF = (a.flags & (kOutF | kOutF0)) != 0;
 #pragma unroll
       for (int i = 0; i < R; ++i) {
         if (valid[i]) {
-          double tau = 1.0;
-          if (wantF) tau = a.tau[r[i]];
+          const double invtau = 1.0 / e_tau[i];
+          const double invrho = 1.0 / rho[i];
 #pragma unroll
           for (int jj = 0; jj < SPW; ++jj) {
-            const int s = w + NW * jj;
-            if (s < K) {
+            const int s = sp[jj];
+            if (s >= 0) {
               const int64_t o = (int64_t)s * a.ld + r[i];
               if (a.flags & kOutWdot) a.wdot[o] = acc[jj][i];
               if (wantF) {
-                const double Fv = (a.Y[o] - a.Yin[o]) / tau - acc[jj][i] * mv.Wm[s] / rho[i];
+                const double Fv = fma(e_y[jj][i] - e_yin[jj][i], invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
                 if (a.flags & kOutF) a.F[o] = Fv;
                 if (a.flags & kOutF0) a.F0out[r[i] * n + 1 + s] = Fv;
               }
@@ -475,21 +545,23 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
         }
       }
     } else {
-      // difference quotient, staged [state][npad] in the Cs region, then one linear coalesced store
+      // difference quotient, staged [state][npad] in this tile's C buffer, then one linear coalesced store
       const int npad = n | 1;
       double* stg = Cs;  // needs TR*npad doubles <= (K+2)*TR (host sizes smem_cs accordingly)
 #pragma unroll
       for (int i = 0; i < R; ++i) {
-        const double tau = a.tau[r[i]];
-        const double invh = 1.0 / h[i];
+        const double invtau = 1.0 / e_tau[i];
+        const double invrho = 1.0 / rho[i];
+        const double invh = 1.0 / hs[lane * R + i];
         const int st = i * 32 + lane;  // position of this state inside the tile, in evaluation order
 #pragma unroll
         for (int jj = 0; jj < SPW; ++jj) {
-          const int s = w + NW * jj;
-          if (s < K) {
-            const int64_t o = (int64_t)s * a.ld + r[i];
-            const double Fv = (load_Y(s, i) - a.Yin[o]) / tau - acc[jj][i] * mv.Wm[s] / rho[i];
-            stg[st * npad + 1 + s] = (Fv - a.F0[r[i] * n + 1 + s]) * invh;
+          const int s = sp[jj];
+          if (s >= 0) {
+            double y = e_y[jj][i];
+            if (s == jsp[i]) y = y + 1e-8 * fmax(fabs(y), 1e-10);   // the same x' as in the prologue
+            const double Fv = fma(y - e_yin[jj][i], invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
+            stg[st * npad + 1 + s] = (Fv - e_f0[jj][i]) * invh;
           }
         }
         if (w == 0) stg[st * npad] = (jsp[i] == -1) ? 1.0 : 0.0;  // row 0: F_T = T - T_set
@@ -503,11 +575,12 @@ __global__ void __launch_bounds__(NW * 32) psr_eval_kernel(const MechView mv, co
       }
       __syncthreads();
     }
+    if (mv.n_cbuf == 1) prefetch(tile + gridDim.x, 0);   // single C buffer: it is free only now
   }
 }
 
 // ------------------------------------------------------------------ launch wrapper
-#define PSR_SHAPES(X) X(8, 2) X(8, 4) X(8, 8) X(16, 8) X(16, 16) X(16, 32)
+#define PSR_SHAPES(X) X(8, 2) X(8, 4) X(8, 8) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)
 
 template <int NW, int SPW, int R>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
@@ -571,10 +644,13 @@ __global__ void __launch_bounds__(256) probe_kernel(int iters, double* sink) {
 
 // exp_fast on an array (diagnostic behind psr_probe_exp_values)
 __global__ void exp_values_kernel(const double* __restrict__ tab, const double* __restrict__ x, double* __restrict__ y, int n) {
-  __shared__ double etab[kExpTabN];
-  if (threadIdx.x < kExpTabN) etab[threadIdx.x] = tab[threadIdx.x];
-  __syncthreads();
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = exp_fast(x[i], etab);
+  const ExpTab etab = exp_tab_load(tab);
+  const int stride = gridDim.x * blockDim.x;
+  for (int i0 = blockIdx.x * blockDim.x; i0 < n; i0 += stride) {   // warp-uniform trip count
+    const int i = i0 + threadIdx.x;
+    const double v = exp_fast(x[i < n ? i : n - 1], etab);
+    if (i < n) y[i] = v;
+  }
 }
 
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st) {

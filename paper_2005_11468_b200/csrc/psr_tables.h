@@ -61,8 +61,7 @@ struct __attribute__((aligned(16))) ChunkHdr {  // 64 bytes
   uint32_t n_rx, n_aux, n_eff, n_g;
   uint32_t off_aux, off_eff, off_pool, off_gptr, off_gent;
   uint32_t bytes;         // bytes to copy (multiple of 16)
-  uint32_t k_first;       // unused
-  uint32_t pad[5];
+  uint8_t wptr[24];       // warp w evaluates records wptr[w] .. wptr[w+1]-1 (cost-balanced at load time)
 };
 static_assert(sizeof(ChunkHdr) == 64, "ChunkHdr layout");
 
@@ -76,9 +75,11 @@ struct MechView {
   const unsigned char* chunks;  // n_chunks blobs, chunk_stride bytes apart
   const double* invW;           // [K] 1/W
   const double* Wm;             // [K] W
-  const double* exp_tab;        // [64] 2^(j/64), staged into shared memory by every CTA (psr_math.cuh)
+  const int32_t* sp_of;         // [nw*spw] species owned by (warp, slot) in the gather, -1 = none (nnz-balanced)
+  const double* exp_tab;        // [32] 2^(j/32), one entry per lane (psr_math.cuh)
   int32_t K, I;
   int32_t n_chunks, rc;
+  int32_t n_cbuf;               // C-tile buffers: 2 = the next tile's state is prefetched during this tile's chunks
   uint32_t chunk_stride;        // bytes, multiple of 16
   uint32_t smem_cs, smem_q, smem_mech, smem_misc, smem_total;  // byte offsets / sizes of the dynamic smem carve-up
 };
