@@ -123,7 +123,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
 
   // ---- per-reaction host records
   std::vector<HostRx> rx(I);
-  int n_fall = 0, n_tb = 0, nnz = 0;
+  int n_fall = 0, n_tb = 0, nnz = 0, need_lnctot = 0;
   for (int k = 0; k < I; ++k) {
     HostRx& h = rx[k];
     std::memset(&h.rec, 0, sizeof h.rec);
@@ -193,6 +193,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
       ++n_fall;
     }
     if (h.type == PSR_RX_TROE) {
+      if (h.eff.empty()) need_lnctot = 1;
       if (!d->troe) return fail(PSR_EINVAL, "Troe reactions need the troe array");
       const double* t = d->troe + 4 * k;
       h.aux.troe[0] = t[0];
@@ -214,26 +215,32 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
 
   // ---- launch shape
   int nw = 16;
-  if (const char* e = getenv("PSR_NW")) nw = atoi(e) == 16 ? 16 : 8;
-  int spw = 2;  // species per warp in the gather: smallest compiled shape with nw * spw >= K
-  while (nw * spw < K) spw *= 2;
-  if (spw > 32 || (nw == 8 && spw > 8)) { nw = 16; spw = 2; while (nw * spw < K) spw *= 2; }
+  // species per warp in the gather: smallest compiled shape (PSR_SHAPES in psr_kernels.cu) with nw * spw >= K
+  auto pick_spw = [&](int nw_) {
+    static const int s8[] = {2, 4, 7, 8, 0}, s12[] = {5, 0}, s16[] = {2, 4, 8, 16, 32, 0};
+    for (const int* p = nw_ == 8 ? s8 : nw_ == 12 ? s12 : s16; *p; ++p)
+      if (nw_ * *p >= K) return *p;
+    return 0;
+  };
+  int spw = pick_spw(nw);
+  if (!spw) { nw = 16; spw = pick_spw(nw); }
   int rl = 1;  // reactors per lane (2 is compiled for spw <= 16; PSR_R selects it)
   if (const char* e = getenv("PSR_R")) rl = (atoi(e) == 2 && spw <= 16) ? 2 : 1;
   const uint32_t row_bytes = (uint32_t)kRowBytes * rl;
-  int rc_target = 192;
-  if (const char* e = getenv("PSR_RC")) rc_target = std::min(kMaxChunkRx, std::max(8, atoi(e)));
+  int rc_target = std::min(I, 384);
+  if (const char* e = getenv("PSR_RC")) rc_target = std::min(std::min(I, kMaxChunkRx), std::max(8, atoi(e)));
   // shared memory left for the q tile and the chunk ring beside one C tile and the per-CTA scratch
-  const size_t smem_fixed = align_up((size_t)(K + 2) * kTile * rl * 8, 128) + (size_t)2 * nw * kTile * rl * 8 +
-                            (size_t)6 * kTile * rl * 8 + 64;
+  const size_t smem_fixed = align_up((size_t)(K + 2) * kTile * rl * 8, 128) + (size_t)nw * kTile * rl * 8 +
+                            (size_t)9 * kTile * rl * 8 + 64;
   int n_chunks = 0, rc = 0;
+  bool resident = false;
   size_t stride = 0;
   std::vector<unsigned char> all;
   std::vector<int32_t> sp_of;
   // the chunk size shrinks until one C tile, the q tile and the (double-buffered) chunk ring fit one CTA
   for (;; rc_target = rc_target * 3 / 4) {
-  if (rc_target < 8)
-    return fail(PSR_EUNSUPPORTED, "mechanism does not fit %zu bytes of shared memory per CTA even at 8 reactions per chunk",
+  if (rc_target < 1)
+    return fail(PSR_EUNSUPPORTED, "mechanism does not fit %zu bytes of shared memory per CTA even at one reaction per chunk",
                 (size_t)prop.sharedMemPerBlockOptin);
   n_chunks = (I + rc_target - 1) / rc_target;
   rc = (I + n_chunks - 1) / n_chunks;  // <= rc_target <= kMaxChunkRx
@@ -287,6 +294,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   std::vector<std::vector<unsigned char>> blobs(n_chunks);
   stride = 0;
   const uint32_t unit_off = (uint32_t)K * row_bytes;   // the all-ones row of the C tile
+  const uint32_t zero_c_off = (uint32_t)(K + 1) * row_bytes;  // the all-zero row of the C tile
   const uint32_t zero_off = (uint32_t)rc * row_bytes;  // the all-zero row of the q tile
   for (int c = 0; c < n_chunks; ++c) {
     const auto& cr = chunk_rx[c];
@@ -304,10 +312,17 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
           rec.off[i] = i < h.nr ? (uint32_t)h.factors[i] * row_bytes : unit_off;
           rec.off[kSlots + i] = i < h.np ? (uint32_t)h.factors[h.nr + i] * row_bytes : unit_off;
         }
+        // irreversible: the product-side factor is the zero row, so k_r * prod = 0 without a select
+        // (and below ln k_r := ln k_f keeps the unused exp finite whenever k_f is)
+        if (!(rec.meta & kMetaRev)) rec.off[kSlots] = zero_c_off;
       } else {
         rec.meta |= kMetaLong | ((uint32_t)h.nr << kMetaNrShift) | ((uint32_t)h.np << kMetaNpShift);
         rec.off[0] = (uint32_t)pool.size();
         pool.insert(pool.end(), h.factors.begin(), h.factors.end());
+      }
+      if (!(rec.meta & kMetaRev)) {
+        for (int j = 0; j < 3; ++j) rec.e[j] = rec.c[j];
+        for (int j = 0; j < 4; ++j) rec.d[j] = 0.0;
       }
       if (h.has_aux) {
         AuxRec ax = h.aux;
@@ -343,8 +358,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     hdr.n_aux = (uint32_t)auxs.size();
     hdr.n_eff = (uint32_t)effs.size();
     hdr.n_g = (uint32_t)gent.size();
-    for (int wv = 0; wv <= nw; ++wv) hdr.wptr[wv] = (uint8_t)chunk_wptr[c][wv];
-    for (int wv = nw + 1; wv < 24; ++wv) hdr.wptr[wv] = (uint8_t)n_rx;
+    for (int wv = 0; wv <= nw; ++wv) hdr.wptr[wv] = (uint16_t)chunk_wptr[c][wv];
+    for (int wv = nw + 1; wv < 20; ++wv) hdr.wptr[wv] = (uint16_t)n_rx;
     size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
     hdr.off_aux = (uint32_t)off;
     off += sizeof(AuxRec) * auxs.size();
@@ -369,7 +384,11 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     stride = std::max(stride, off);
   }
   stride = align_up(stride, 128);
-  const size_t need = smem_fixed + align_up((size_t)(rc + 1) * kTile * rl * 8, 128) + stride * (n_chunks == 1 ? 1 : 2);
+  // all chunk blobs resident in shared memory (loaded once per CTA) when they fit, else a 2-stage ring
+  const size_t q_bytes = align_up((size_t)(rc + 1) * kTile * rl * 8, 128);
+  resident = n_chunks <= kMaxStages && smem_fixed + q_bytes + stride * n_chunks <= (size_t)prop.sharedMemPerBlockOptin &&
+             (n_chunks == 1 || stride * n_chunks <= 48 * 1024);
+  const size_t need = smem_fixed + q_bytes + stride * (resident ? n_chunks : 2);
   if (need > (size_t)prop.sharedMemPerBlockOptin) continue;
   all.assign(stride * n_chunks, 0);
   for (int c = 0; c < n_chunks; ++c) std::memcpy(all.data() + stride * c, blobs[c].data(), blobs[c].size());
@@ -392,6 +411,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.I = I;
   v.n_chunks = n_chunks;
   v.rc = rc;
+  v.resident = resident ? 1 : 0;
+  v.need_lnctot = need_lnctot;
   v.chunk_stride = (uint32_t)stride;
   const size_t cbuf_bytes = align_up((size_t)(K + 2) * kTile * rl * 8, 128);  // K+2 rows so the Jacobian staging [tile][n|1] fits
   auto carve = [&](int n_cbuf) {
@@ -401,9 +422,9 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     v.smem_q = (uint32_t)o;
     o += align_up((size_t)(rc + 1) * kTile * rl * 8, 128);  // + the all-zero row
     v.smem_mech = (uint32_t)o;
-    o += stride * (n_chunks == 1 ? 1 : 2);
+    o += stride * (resident ? n_chunks : 2);
     v.smem_misc = (uint32_t)o;
-    o += (size_t)2 * nw * kTile * rl * 8 + (size_t)6 * kTile * rl * 8 + 64;  // partial sums; ln T, h, T/P prefetch; mbarriers
+    o += (size_t)nw * kTile * rl * 8 + (size_t)9 * kTile * rl * 8 + 64;  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P prefetch; mbarriers
     v.smem_total = (uint32_t)o;
     v.n_cbuf = n_cbuf;
     return o;

@@ -101,27 +101,30 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   double* Cs0 = reinterpret_cast<double*>(smem + mv.smem_cs);         // [2][K+2][TR]; row K is the unit row
   double* qs = reinterpret_cast<double*>(smem + mv.smem_q);           // [rc+1][TR]; row rc stays zero
   unsigned char* mring = smem + mv.smem_mech;                         // stages * chunk_stride
-  double* part = reinterpret_cast<double*>(smem + mv.smem_misc);      // [2][NW][TR] partial sums
-  double* lane_s = part + 2 * NW * TR;                                // [TR]: ln T per state
+  double* part = reinterpret_cast<double*>(smem + mv.smem_misc);      // [NW][TR] partial sums
+  double* lane_s = part + NW * TR;                                    // [TR]: ln T per state
   double* hs = lane_s + TR;                                           // [TR]: finite-difference step per state
-  double* tp = hs + TR;                                               // [2][2][TR]: prefetched T, P
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [2]
+  double* rho_s = hs + TR;                                            // [TR]: density per state
+  double* ctot_s = rho_s + TR;                                        // [TR]: C_tot per state
+  double* lnctot_s = ctot_s + TR;                                     // [TR]: ln C_tot (formed on first use)
+  double* tp = lnctot_s + TR;                                         // [2][2][TR]: prefetched T, P
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [kMaxStages]
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
   const int K = mv.K;
   const int n = K + 1;
   const bool jac = (a.flags & kModeJac) != 0;
-  const int nstage = mv.n_chunks == 1 ? 1 : 2;
+  const bool resident = mv.resident != 0;   // every chunk blob has its own stage and is loaded once per CTA
+  const int nstage = resident ? mv.n_chunks : 2;
   const int cs_elems = (K + 2) * TR;
   const uint32_t q_lane = smem_u32(qs) + lane * (8 * R);
 
   const int64_t my_tiles = (a.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
-  const int64_t total_loads = mv.n_chunks == 1 ? 1 : my_tiles * mv.n_chunks;
+  const int64_t total_loads = resident ? mv.n_chunks : my_tiles * mv.n_chunks;
 
   if (threadIdx.x == 0) {
-    mbar_init(&bars[0], 1);
-    mbar_init(&bars[1], 1);
+    for (int g = 0; g < kMaxStages; ++g) mbar_init(&bars[g], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     for (int g = 0; g < nstage && g < total_loads; ++g) {
@@ -184,15 +187,18 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     // ---------------------------------------------------------------- prologue (a1)
     double* Cs = Cs0 + buf * cs_elems;
     const uint32_t c_lane = smem_u32(Cs) + lane * (8 * R);   // this lane's R slots of row 0 of the C tile
-    int64_t r[R];
-    int jsp[R];
-    bool valid[R];
-#pragma unroll
-    for (int i = 0; i < R; ++i) state_of(tile, i, r[i], jsp[i], valid[i]);
     asm volatile("cp.async.wait_group 0;" ::: "memory");   // this thread's prefetched entries have landed
 
-    double T[R], rho[R];
+    double T[R];
     {
+      int jsp[R];
+      double rho[R];
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        int64_t r_;
+        bool valid_;
+        state_of(tile, i, r_, jsp[i], valid_);
+      }
       // x' = fl(x + delta), h = fl(x' - x) for the perturbed unknown of a Jacobian state (O11, g15)
       double yv[SPW][R];
       double sumYW[R];
@@ -220,11 +226,13 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       for (int i = 0; i < R; ++i) part[w * TR + lane * R + i] = sumYW[i];
       if (w == 0) {
 #pragma unroll
-        for (int i = 0; i < R; ++i) Cs[K * TR + lane * R + i] = 1.0;
+        for (int i = 0; i < R; ++i) {
+          Cs[K * TR + lane * R + i] = 1.0;         // unit row: unused factor slots
+          Cs[(K + 1) * TR + lane * R + i] = 0.0;   // zero row: product side of an irreversible reaction
+        }
       }
       __syncthreads();   // partial sums and warp 0's T, P visible; every warp has left the previous tile
       if (mv.n_cbuf == 2) prefetch(tile + gridDim.x, buf ^ 1);
-      double cpart[R];
 #pragma unroll
       for (int i = 0; i < R; ++i) {
         T[i] = tp[(buf * 2 + 0) * TR + lane * R + i];
@@ -234,42 +242,37 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           if (w == 0) hs[lane * R + i] = Tp - T[i];
           T[i] = Tp;
         }
-        if (w == 0) lane_s[lane * R + i] = log(T[i]);
         double sY = 0.0;
 #pragma unroll
         for (int ww = 0; ww < NW; ++ww) sY += part[ww * TR + lane * R + i];
         const double Wbar = 1.0 / sY;
         rho[i] = P * Wbar / (kRgas * T[i]);
-        cpart[i] = 0.0;
+        if (w == 0) {
+          // C_tot = sum_i C_i = rho * sum_i Y_i/W_i: formed from the sum already at hand (differs from
+          // the species-by-species sum by rounding only)
+          const double ct = rho[i] * sY;
+          lane_s[lane * R + i] = log(T[i]);
+          rho_s[lane * R + i] = rho[i];
+          ctot_s[lane * R + i] = ct;
+          if (mv.need_lnctot) lnctot_s[lane * R + i] = log(ct);   // Troe reactions without efficiencies
+        }
       }
 #pragma unroll
       for (int jj = 0; jj < SPW; ++jj) {
         const int s = sp[jj];
         if (s >= 0) {
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            const double c = rho[i] * yv[jj][i];
-            Cs[s * TR + lane * R + i] = c;
-            cpart[i] += c;
-          }
+          for (int i = 0; i < R; ++i) Cs[s * TR + lane * R + i] = rho[i] * yv[jj][i];
         }
       }
-#pragma unroll
-      for (int i = 0; i < R; ++i) part[(NW + w) * TR + lane * R + i] = cpart[i];
     }
     __syncthreads();
-    double Ctot[R], lnT[R], invT[R], lnCtot[R];
+    double lnT[R], invT[R];
 #pragma unroll
     for (int i = 0; i < R; ++i) {
-      double ct = 0.0;
-#pragma unroll
-      for (int ww = 0; ww < NW; ++ww) ct += part[(NW + ww) * TR + lane * R + i];
-      Ctot[i] = ct;
       lnT[i] = lane_s[lane * R + i];
       invT[i] = 1.0 / T[i];
-      lnCtot[i] = 0.0;
     }
-    bool have_lnCtot = false;  // ln C_tot is formed on first use by a Troe reaction without efficiencies
 
     double acc[SPW][R];
 #pragma unroll
@@ -335,7 +338,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         }
       }
       __syncthreads();
-      if (mv.n_chunks > 1) {
+      if (!resident) {
         if (threadIdx.x == 0 && g + nstage < total_loads) {
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           mbar_expect_tx(&bars[stage], mv.chunk_stride);
@@ -347,15 +350,18 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     };
     for (int c = 0; c < mv.n_chunks; ++c) {
       stage = (int)(g % nstage);
-      if (mv.n_chunks > 1 || g == 0) mbar_wait(&bars[stage], (uint32_t)((g / nstage) & 1));
+      if (!resident || g < nstage) mbar_wait(&bars[stage], (uint32_t)((g / nstage) & 1));
       blob = mring + (size_t)stage * mv.chunk_stride;
       hdr = reinterpret_cast<const ChunkHdr*>(blob);
       const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
 
       // ---- reaction phase (a3..a7): warp w takes its cost-balanced share of the chunk's records
-      const int kl_end = hdr->wptr[w + 1];
+      // the warp's record range is the same in every lane: say so (REDUX writes a uniform register), which
+      // keeps the loop counter, the record addresses and the type branches in the uniform datapath
+      const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wptr[w]);
+      const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wptr[w + 1]);
 #pragma unroll 1
-      for (int kl = hdr->wptr[w]; kl < kl_end; ++kl) {
+      for (int kl = kl_begin; kl < kl_end; ++kl) {
         const RxRec* rec = recs + kl;
         const uint32_t meta = rec->meta;
         const int type = (int)(meta & kMetaTypeMask);
@@ -402,32 +408,31 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               else pr[i] *= cv[i];
             }
           }
+          if (!(meta & kMetaRev)) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) pr[i] = 0.0;
+          }
         }
 
         if (type <= PSR_T_THREE_BODY) {
-          bool ok = true;
+          double ex[2 * R], ey[2 * R];
 #pragma unroll
-          for (int i = 0; i < R; ++i) ok = ok && exp_in_range(lnkf[i]) && exp_in_range(lnkr[i]);
-          ok = __all_sync(kFullMask, ok);
-          if (ok) {
+          for (int i = 0; i < R; ++i) {
+            ex[2 * i] = lnkf[i];
+            ex[2 * i + 1] = lnkr[i];
+          }
+          exp_fast_n<2 * R>(ex, ey, etab);
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-              kf[i] = exp_core(lnkf[i], etab);
-              kr[i] = exp_core(lnkr[i], etab);
-            }
-          } else {
-#pragma unroll
-            for (int i = 0; i < R; ++i) {
-              kf[i] = exp(lnkf[i]);
-              kr[i] = exp(lnkr[i]);
-            }
+          for (int i = 0; i < R; ++i) {
+            kf[i] = ey[2 * i];
+            kr[i] = ey[2 * i + 1];
           }
         }
         if (type != PSR_T_PLAIN) {
           const AuxRec* ax = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux) + (meta >> kMetaAuxShift);
           const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
 #pragma unroll
-          for (int i = 0; i < R; ++i) M[i] = Ctot[i];
+          for (int i = 0; i < R; ++i) M[i] = ctot_s[lane * R + i];
           const uint32_t e1 = ax->eff_off + ax->n_eff;
 #pragma unroll 1
           for (uint32_t e = ax->eff_off; e < e1; ++e) {
@@ -436,60 +441,80 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
             for (int i = 0; i < R; ++i) M[i] = fma(effs[e].am1, cv[i], M[i]);
           }
-          if (type >= PSR_T_LINDEMANN) {
-            if (type == PSR_T_TROE && ax->n_eff == 0 && !have_lnCtot) {
+          if (type == PSR_T_THREE_BODY) {
 #pragma unroll
-              for (int i = 0; i < R; ++i) lnCtot[i] = log(Ctot[i]);
-              have_lnCtot = true;
+            for (int i = 0; i < R; ++i) {
+              pf[i] *= M[i];
+              pr[i] *= M[i];
             }
+          } else if (type == PSR_T_LINDEMANN) {
+            // k_f = k_inf Pr/(1+Pr), Pr = k0 [M]/k_inf
+            double ex[3 * R], ey[3 * R];
 #pragma unroll
             for (int i = 0; i < R; ++i) {
               const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
-              if (type == PSR_T_LINDEMANN) {
-                const double Pr = exp_fast(lnk0 - lnkf[i], etab) * M[i];
-                kf[i] = exp_fast(lnkf[i], etab) * (Pr / (1.0 + Pr));
-              } else {
-                // Troe.  With ln Pr = ln k0 - ln k_inf + ln[M]:
-                //   k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
-                const double lnM = ax->n_eff == 0 ? lnCtot[i] : log(M[i]);
-                const double lnk0M = lnk0 + lnM;
-                const double lnPr = lnk0M - lnkf[i];
-                const double Pr = exp_fast(lnPr, etab);
-                const double al = ax->troe[0];
-                const double Fcent =
-                    fma(1.0 - al, exp_fast(T[i] * ax->troe[1], etab),
-                        fma(al, exp_fast(T[i] * ax->troe[2], etab), exp_fast(ax->troe[3] * invT[i], etab)));
-                const double lnFc = log(Fcent);
-                const double lF = lnFc * kLog10e;
-                const double cc = fma(-0.67, lF, -0.4);
-                const double nn = fma(-1.27, lF, 0.75);
-                const double lp = fma(lnPr, kLog10e, cc);
-                const double den = fma(-0.14, lp, nn);
-                // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
-                const double den2 = den * den;
-                const double lnF = lnFc * den2 / fma(lp, lp, den2);
-                kf[i] = exp_fast(lnk0M + lnF, etab) / (1.0 + Pr);
-              }
-              kr[i] = kf[i] * exp_fast(lnkr[i] - lnkf[i], etab);
+              ex[3 * i] = lnk0 - lnkf[i];
+              ex[3 * i + 1] = lnkf[i];
+              ex[3 * i + 2] = lnkr[i] - lnkf[i];
+            }
+            exp_fast_n<3 * R>(ex, ey, etab);
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              const double Pr = ey[3 * i] * M[i];
+              kf[i] = ey[3 * i + 1] * (Pr / (1.0 + Pr));
+              kr[i] = kf[i] * ey[3 * i + 2];
+            }
+          } else if (type == PSR_T_TROE) {
+            // With ln Pr = ln k0 - ln k_inf + ln[M]:  k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
+            // one reactor at a time: five exps in lock step are enough to fill the FP64 pipe
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
+              const double lnM = ax->n_eff == 0 ? lnctot_s[lane * R + i] : log(M[i]);
+              const double lnk0M = lnk0 + lnM;
+              double ex[5], ey[5];
+              ex[0] = lnk0M - lnkf[i];          // ln Pr
+              ex[1] = T[i] * ax->troe[1];
+              ex[2] = T[i] * ax->troe[2];
+              ex[3] = ax->troe[3] * invT[i];
+              ex[4] = lnkr[i] - lnkf[i];        // ln(k_r/k_f) = -ln K_c
+              exp_fast_n<5>(ex, ey, etab);
+              const double al = ax->troe[0];
+              const double Fcent = fma(1.0 - al, ey[1], fma(al, ey[2], ey[3]));
+              const double lnFc = log(Fcent);
+              const double lF = lnFc * kLog10e;
+              const double cc = fma(-0.67, lF, -0.4);
+              const double nn = fma(-1.27, lF, 0.75);
+              const double lp = fma(ex[0], kLog10e, cc);
+              const double den = fma(-0.14, lp, nn);
+              // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
+              const double den2 = den * den;
+              double e2[1], k2[1];
+              e2[0] = lnk0M + lnFc * den2 / fma(lp, lp, den2);
+              exp_fast_n<1>(e2, k2, etab);
+              kf[i] = k2[0] / (1.0 + ey[0]);
+              kr[i] = kf[i] * ey[4];
             }
           }
         }
+        // an irreversible reaction has its product side on the zero row (pr = 0), a three-body reaction
+        // carries [M] in both products (pf, pr scaled below): no per-lane selects here
         double q[R];
 #pragma unroll
-        for (int i = 0; i < R; ++i) {
-          if (!(meta & kMetaRev)) kr[i] = 0.0;
-          q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
-          if (type == PSR_T_THREE_BODY) q[i] *= M[i];
-        }
+        for (int i = 0; i < R; ++i) q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
         RowIO<R>::st(q_lane + (uint32_t)kl * (uint32_t)(TR * 8), q);
 
         if (a.flags & (kOutKf | kOutKr | kOutQ)) {
 #pragma unroll
           for (int i = 0; i < R; ++i) {
-            if (valid[i]) {
-              const int64_t o = (int64_t)rec->korig * a.ldk + r[i];
+            int64_t r_;
+            int jsp_;
+            bool valid_;
+            state_of(tile, i, r_, jsp_, valid_);
+            if (valid_) {
+              const int64_t o = (int64_t)rec->korig * a.ldk + r_;
               if (a.flags & kOutKf) a.kf[o] = kf[i];
-              if (a.flags & kOutKr) a.kr[o] = kr[i];
+              if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr[i] : 0.0;
               if (a.flags & kOutQ) a.q[o] = q[i];
             }
           }
@@ -502,6 +527,11 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 
     // operands of the epilogue are requested now so that they arrive during the last gather
     double e_tau[R], e_y[SPW][R], e_yin[SPW][R], e_f0[SPW][R];
+    int64_t r[R];
+    int jsp[R];
+    bool valid[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) state_of(tile, i, r[i], jsp[i], valid[i]);
       if (wantF) {
 #pragma unroll
         for (int i = 0; i < R; ++i) {
@@ -527,7 +557,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       for (int i = 0; i < R; ++i) {
         if (valid[i]) {
           const double invtau = 1.0 / e_tau[i];
-          const double invrho = 1.0 / rho[i];
+          const double invrho = 1.0 / rho_s[lane * R + i];
 #pragma unroll
           for (int jj = 0; jj < SPW; ++jj) {
             const int s = sp[jj];
@@ -551,7 +581,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
       for (int i = 0; i < R; ++i) {
         const double invtau = 1.0 / e_tau[i];
-        const double invrho = 1.0 / rho[i];
+        const double invrho = 1.0 / rho_s[lane * R + i];
         const double invh = 1.0 / hs[lane * R + i];
         const int st = i * 32 + lane;  // position of this state inside the tile, in evaluation order
 #pragma unroll
@@ -580,7 +610,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 }
 
 // ------------------------------------------------------------------ launch wrapper
-#define PSR_SHAPES(X) X(8, 2) X(8, 4) X(8, 8) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)
+#define PSR_SHAPES(X) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)
 
 template <int NW, int SPW, int R>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
@@ -592,7 +622,7 @@ static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cud
 }
 
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-#define PSR_L(NW_, SPW_)                                                      \
+#define PSR_L(NW_, SPW_)                                                                     \
   if (nw == NW_ && spw == SPW_ && rl == 1) return launch_t<NW_, SPW_, 1>(mv, a, grid, st); \
   if (nw == NW_ && spw == SPW_ && rl == 2) return launch_t<NW_, SPW_, 2>(mv, a, grid, st);
   PSR_SHAPES(PSR_L)
@@ -609,7 +639,7 @@ static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
 }
 
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm) {
-#define PSR_O(NW_, SPW_)                                                   \
+#define PSR_O(NW_, SPW_)                                                                    \
   if (nw == NW_ && spw == SPW_ && rl == 1) return occ_t<NW_, SPW_, 1>(smem, ctas_per_sm); \
   if (nw == NW_ && spw == SPW_ && rl == 2) return occ_t<NW_, SPW_, 2>(smem, ctas_per_sm);
   PSR_SHAPES(PSR_O)

@@ -22,7 +22,8 @@ constexpr int kTile = 32;       // reactors per tile = lanes of a warp
 constexpr int kRowBytes = kTile * 8;  // one species / reaction row of a tile in shared memory
 constexpr int kSlots = 3;       // inline concentration-factor slots per reaction side
 constexpr int kMaxSide = 15;    // concentration factors per reaction side (long form)
-constexpr int kMaxChunkRx = 254;  // rows of the q tile addressable by a gather entry (+1 zero row)
+constexpr int kMaxStages = 8;     // chunk blobs that can be resident in shared memory at once
+constexpr int kMaxChunkRx = 1024; // reactions per chunk (rows of the q tile, +1 zero row)
 
 // meta bits
 constexpr uint32_t kMetaTypeMask = 0x3u;      // PSR_RX_*
@@ -57,13 +58,13 @@ struct __attribute__((aligned(16))) EffEnt {  // 16 bytes
   uint32_t pad;
 };
 
-struct __attribute__((aligned(16))) ChunkHdr {  // 64 bytes
+struct __attribute__((aligned(16))) ChunkHdr {  // 80 bytes
   uint32_t n_rx, n_aux, n_eff, n_g;
   uint32_t off_aux, off_eff, off_pool, off_gptr, off_gent;
   uint32_t bytes;         // bytes to copy (multiple of 16)
-  uint8_t wptr[24];       // warp w evaluates records wptr[w] .. wptr[w+1]-1 (cost-balanced at load time)
+  uint16_t wptr[20];      // warp w evaluates records wptr[w] .. wptr[w+1]-1 (cost-balanced at load time)
 };
-static_assert(sizeof(ChunkHdr) == 64, "ChunkHdr layout");
+static_assert(sizeof(ChunkHdr) == 80, "ChunkHdr layout");
 
 // Gather lists of nu^T (Eq. 4) per chunk: species s adds the q rows gent[gptr[2s] .. gptr[2s+1]) and
 // subtracts gent[gptr[2s+1] .. gptr[2s+2]).  An entry is the byte offset of a row of the q tile;
@@ -79,6 +80,8 @@ struct MechView {
   const double* exp_tab;        // [32] 2^(j/32), one entry per lane (psr_math.cuh)
   int32_t K, I;
   int32_t n_chunks, rc;
+  int32_t need_lnctot;          // some Troe reaction has no efficiency list (uses ln C_tot)
+  int32_t resident;             // every chunk blob stays in shared memory (loaded once per CTA)
   int32_t n_cbuf;               // C-tile buffers: 2 = the next tile's state is prefetched during this tile's chunks
   uint32_t chunk_stride;        // bytes, multiple of 16
   uint32_t smem_cs, smem_q, smem_mech, smem_misc, smem_total;  // byte offsets / sizes of the dynamic smem carve-up
