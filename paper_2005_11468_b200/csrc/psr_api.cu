@@ -253,7 +253,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   std::vector<std::vector<int>> chunk_rx(n_chunks);
   for (int p = 0; p < I; ++p) chunk_rx[p % n_chunks].push_back(order[p]);
   // inside a chunk: longest-processing-time assignment of records to warps, records of a warp contiguous
-  std::vector<std::vector<int>> chunk_wptr(n_chunks);
+  auto cls_of = [&](int k) { return (rx[k].nr > kSlots || rx[k].np > kSlots) ? kClsLong : rx[k].type; };
+  std::vector<std::vector<int>> chunk_wb(n_chunks);   // [warp][class boundary], kClsLong + 2 per warp
   for (int c = 0; c < n_chunks; ++c) {
     auto& cr = chunk_rx[c];  // cost-descending
     std::vector<double> load(nw, 0.0);
@@ -264,10 +265,17 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
       load[wmin] += reaction_cost(rx[k].type);
     }
     cr.clear();
-    chunk_wptr[c].assign(nw + 1, 0);
+    chunk_wb[c].assign((size_t)kMaxWarps * (kClsLong + 2), 0);
     for (int wv = 0; wv < nw; ++wv) {
+      std::stable_sort(mine[wv].begin(), mine[wv].end(), [&](int x, int y) { return cls_of(x) < cls_of(y); });
+      int* wb = &chunk_wb[c][(size_t)wv * (kClsLong + 2)];
+      size_t p = 0;
+      for (int cl = 0; cl <= kClsLong; ++cl) {
+        wb[cl] = (int)(cr.size() + p);
+        while (p < mine[wv].size() && cls_of(mine[wv][p]) == cl) ++p;
+      }
       cr.insert(cr.end(), mine[wv].begin(), mine[wv].end());
-      chunk_wptr[c][wv + 1] = (int)cr.size();
+      wb[kClsLong + 1] = (int)cr.size();
     }
   }
   // gather ownership: species to (warp, slot) by longest-processing-time on the row length of nu^T
@@ -358,8 +366,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     hdr.n_aux = (uint32_t)auxs.size();
     hdr.n_eff = (uint32_t)effs.size();
     hdr.n_g = (uint32_t)gent.size();
-    for (int wv = 0; wv <= nw; ++wv) hdr.wptr[wv] = (uint16_t)chunk_wptr[c][wv];
-    for (int wv = nw + 1; wv < 20; ++wv) hdr.wptr[wv] = (uint16_t)n_rx;
+    for (int wv = 0; wv < kMaxWarps; ++wv)
+      for (int cl = 0; cl < kClsLong + 2; ++cl) hdr.wb[wv][cl] = (uint16_t)chunk_wb[c][(size_t)wv * (kClsLong + 2) + cl];
     size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
     hdr.off_aux = (uint32_t)off;
     off += sizeof(AuxRec) * auxs.size();

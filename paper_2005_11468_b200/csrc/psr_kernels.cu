@@ -15,6 +15,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "psr_math.cuh"
 #include "psr_tables.h"
 
@@ -355,172 +357,205 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       hdr = reinterpret_cast<const ChunkHdr*>(blob);
       const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
 
-      // ---- reaction phase (a3..a7): warp w takes its cost-balanced share of the chunk's records
-      // the warp's record range is the same in every lane: say so (REDUX writes a uniform register), which
-      // keeps the loop counter, the record addresses and the type branches in the uniform datapath
-      const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wptr[w]);
-      const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wptr[w + 1]);
+      // ---- reaction phase (a3..a7): warp w takes its cost-balanced share of the chunk's records, sorted
+      // by class (plain, three-body, Lindemann, Troe in the 3+3 slot form; then the long-list form), one
+      // loop per class so that no reaction-type test is left inside a loop.  FAST: every exp takes the
+      // table form and a lane only notes an out-of-range argument; the CTA then repeats the phase with
+      // the library exp (IEEE results for NaN, Inf, overflow, gradual underflow).  That never happens for
+      // physical states, so the range test costs two compares per reaction and no vote or branch.
+      bool bad = false;
+      auto run_class = [&](auto cls_tag, auto fast_tag) {
+        constexpr int CLS = decltype(cls_tag)::value;
+        constexpr bool FAST = decltype(fast_tag)::value;
+        // the record range is the same in every lane: say so (REDUX writes a uniform register), which
+        // keeps the loop counter and the record addresses in the uniform datapath
+        const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
+        const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS + 1]);
+        auto exps = [&](auto& ex, auto& ey) {
+          constexpr int N = sizeof(ex) / sizeof(double);
+          if constexpr (FAST) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) bad = bad || !exp_in_range(ex[i]);
+            exp_core_n<N>(ex, ey, etab);
+          } else {
+#pragma unroll
+            for (int i = 0; i < N; ++i) ey[i] = exp(ex[i]);
+          }
+        };
 #pragma unroll 1
-      for (int kl = kl_begin; kl < kl_end; ++kl) {
-        const RxRec* rec = recs + kl;
-        const uint32_t meta = rec->meta;
-        const int type = (int)(meta & kMetaTypeMask);
-        double lnkf[R], lnkr[R], pf[R], pr[R], kf[R], kr[R], M[R];
-        // Eq. 6 in log form, and ln k_r = ln k_f - ln K_c (Eq. 7-9 summed per reaction at load time)
+        for (int kl = kl_begin; kl < kl_end; ++kl) {
+          const RxRec* rec = recs + kl;
+          const uint32_t meta = rec->meta;
+          const int type = CLS < kClsLong ? CLS : (int)(meta & kMetaTypeMask);
+          double lnkf[R], lnkr[R], pf[R], pr[R], kf[R], kr[R], M[R];
+          // Eq. 6 in log form, and ln k_r = ln k_f - ln K_c (Eq. 7-9 summed per reaction at load time)
 #pragma unroll
-        for (int i = 0; i < R; ++i) {
-          lnkf[i] = fma(rec->c[1], lnT[i], fma(rec->c[2], invT[i], rec->c[0]));
-          const double pn = fma(fma(fma(rec->d[3], T[i], rec->d[2]), T[i], rec->d[1]), T[i], rec->d[0]);
-          lnkr[i] = fma(pn, T[i], fma(rec->e[1], lnT[i], fma(rec->e[2], invT[i], rec->e[0])));
-          M[i] = 1.0;
-        }
+          for (int i = 0; i < R; ++i) {
+            lnkf[i] = fma(rec->c[1], lnT[i], fma(rec->c[2], invT[i], rec->c[0]));
+            const double pn = fma(fma(fma(rec->d[3], T[i], rec->d[2]), T[i], rec->d[1]), T[i], rec->d[0]);
+            lnkr[i] = fma(pn, T[i], fma(rec->e[1], lnT[i], fma(rec->e[2], invT[i], rec->e[0])));
+            M[i] = 1.0;
+          }
 
-        // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
-        if (!(meta & kMetaLong)) {
-          double f0[R], f1[R], f2[R], p0[R], p1[R], p2[R];
-          RowIO<R>::ld(c_lane + rec->off[0], f0);
-          RowIO<R>::ld(c_lane + rec->off[1], f1);
-          RowIO<R>::ld(c_lane + rec->off[2], f2);
-          RowIO<R>::ld(c_lane + rec->off[3], p0);
-          RowIO<R>::ld(c_lane + rec->off[4], p1);
-          RowIO<R>::ld(c_lane + rec->off[5], p2);
+          // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
+          if constexpr (CLS < kClsLong) {
+            double f0[R], f1[R], f2[R], p0[R], p1[R], p2[R];
+            RowIO<R>::ld(c_lane + rec->off[0], f0);
+            RowIO<R>::ld(c_lane + rec->off[1], f1);
+            RowIO<R>::ld(c_lane + rec->off[2], f2);
+            RowIO<R>::ld(c_lane + rec->off[3], p0);
+            RowIO<R>::ld(c_lane + rec->off[4], p1);
+            RowIO<R>::ld(c_lane + rec->off[5], p2);
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            pf[i] = f0[i] * f1[i] * f2[i];
-            pr[i] = p0[i] * p1[i] * p2[i];
-          }
-        } else {
-          const uint16_t* sp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + rec->off[0];
-          const int nr = (int)((meta >> kMetaNrShift) & 0xF);
-          const int np = (int)((meta >> kMetaNpShift) & 0xF);
+            for (int i = 0; i < R; ++i) {
+              pf[i] = f0[i] * f1[i] * f2[i];
+              pr[i] = p0[i] * p1[i] * p2[i];
+            }
+          } else {
+            const uint16_t* fsp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + rec->off[0];
+            const int nr = (int)((meta >> kMetaNrShift) & 0xF);
+            const int np = (int)((meta >> kMetaNpShift) & 0xF);
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            pf[i] = 1.0;
-            pr[i] = 1.0;
-          }
+            for (int i = 0; i < R; ++i) {
+              pf[i] = 1.0;
+              pr[i] = 1.0;
+            }
 #pragma unroll 1
-          for (int j = 0; j < nr + np; ++j) {
-            double cv[R];
-            RowIO<R>::ld(c_lane + (uint32_t)sp[j] * (uint32_t)(TR * 8), cv);
+            for (int j = 0; j < nr + np; ++j) {
+              double cv[R];
+              RowIO<R>::ld(c_lane + (uint32_t)fsp[j] * (uint32_t)(TR * 8), cv);
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-              if (j < nr) pf[i] *= cv[i];
-              else pr[i] *= cv[i];
+              for (int i = 0; i < R; ++i) {
+                if (j < nr) pf[i] *= cv[i];
+                else pr[i] *= cv[i];
+              }
+            }
+            if (!(meta & kMetaRev)) {
+#pragma unroll
+              for (int i = 0; i < R; ++i) pr[i] = 0.0;
             }
           }
-          if (!(meta & kMetaRev)) {
-#pragma unroll
-            for (int i = 0; i < R; ++i) pr[i] = 0.0;
-          }
-        }
 
-        if (type <= PSR_T_THREE_BODY) {
-          double ex[2 * R], ey[2 * R];
+          if (type <= PSR_T_THREE_BODY) {
+            double ex[2 * R], ey[2 * R];
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            ex[2 * i] = lnkf[i];
-            ex[2 * i + 1] = lnkr[i];
+            for (int i = 0; i < R; ++i) {
+              ex[2 * i] = lnkf[i];
+              ex[2 * i + 1] = lnkr[i];
+            }
+            exps(ex, ey);
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+              kf[i] = ey[2 * i];
+              kr[i] = ey[2 * i + 1];
+            }
           }
-          exp_fast_n<2 * R>(ex, ey, etab);
+          if (type != PSR_T_PLAIN) {
+            const AuxRec* ax = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux) + (meta >> kMetaAuxShift);
+            const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            kf[i] = ey[2 * i];
-            kr[i] = ey[2 * i + 1];
-          }
-        }
-        if (type != PSR_T_PLAIN) {
-          const AuxRec* ax = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux) + (meta >> kMetaAuxShift);
-          const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
-#pragma unroll
-          for (int i = 0; i < R; ++i) M[i] = ctot_s[lane * R + i];
-          const uint32_t e1 = ax->eff_off + ax->n_eff;
+            for (int i = 0; i < R; ++i) M[i] = ctot_s[lane * R + i];
+            const uint32_t e1 = ax->eff_off + ax->n_eff;
 #pragma unroll 1
-          for (uint32_t e = ax->eff_off; e < e1; ++e) {
-            double cv[R];
-            RowIO<R>::ld(c_lane + effs[e].off, cv);
+            for (uint32_t e = ax->eff_off; e < e1; ++e) {
+              double cv[R];
+              RowIO<R>::ld(c_lane + effs[e].off, cv);
 #pragma unroll
-            for (int i = 0; i < R; ++i) M[i] = fma(effs[e].am1, cv[i], M[i]);
+              for (int i = 0; i < R; ++i) M[i] = fma(effs[e].am1, cv[i], M[i]);
+            }
+            if (type == PSR_T_THREE_BODY) {
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                pf[i] *= M[i];
+                pr[i] *= M[i];
+              }
+            } else if (type == PSR_T_LINDEMANN) {
+              // k_f = k_inf Pr/(1+Pr), Pr = k0 [M]/k_inf
+              double ex[3 * R], ey[3 * R];
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
+                ex[3 * i] = lnk0 - lnkf[i];
+                ex[3 * i + 1] = lnkf[i];
+                ex[3 * i + 2] = lnkr[i] - lnkf[i];
+              }
+              exps(ex, ey);
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                const double Pr = ey[3 * i] * M[i];
+                kf[i] = ey[3 * i + 1] * (Pr / (1.0 + Pr));
+                kr[i] = kf[i] * ey[3 * i + 2];
+              }
+            } else {
+              // Troe.  With ln Pr = ln k0 - ln k_inf + ln[M]:
+              //   k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
+              // one reactor at a time: five exps in lock step are enough to fill the FP64 pipe
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
+                const double lnM = ax->n_eff == 0 ? lnctot_s[lane * R + i] : log(M[i]);
+                const double lnk0M = lnk0 + lnM;
+                double ex[5], ey[5];
+                ex[0] = lnk0M - lnkf[i];          // ln Pr
+                ex[1] = T[i] * ax->troe[1];
+                ex[2] = T[i] * ax->troe[2];
+                ex[3] = ax->troe[3] * invT[i];
+                ex[4] = lnkr[i] - lnkf[i];        // ln(k_r/k_f) = -ln K_c
+                exps(ex, ey);
+                const double al = ax->troe[0];
+                const double Fcent = fma(1.0 - al, ey[1], fma(al, ey[2], ey[3]));
+                const double lnFc = log(Fcent);
+                const double lF = lnFc * kLog10e;
+                const double cc = fma(-0.67, lF, -0.4);
+                const double nn = fma(-1.27, lF, 0.75);
+                const double lp = fma(ex[0], kLog10e, cc);
+                const double den = fma(-0.14, lp, nn);
+                // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
+                const double den2 = den * den;
+                double e2[1], k2[1];
+                e2[0] = lnk0M + lnFc * den2 / fma(lp, lp, den2);
+                exps(e2, k2);
+                kf[i] = k2[0] / (1.0 + ey[0]);
+                kr[i] = kf[i] * ey[4];
+              }
+            }
           }
-          if (type == PSR_T_THREE_BODY) {
+          // an irreversible reaction has its product side on the zero row (pr = 0), a three-body reaction
+          // carries [M] in both products: no per-lane selects here
+          double q[R];
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-              pf[i] *= M[i];
-              pr[i] *= M[i];
-            }
-          } else if (type == PSR_T_LINDEMANN) {
-            // k_f = k_inf Pr/(1+Pr), Pr = k0 [M]/k_inf
-            double ex[3 * R], ey[3 * R];
-#pragma unroll
-            for (int i = 0; i < R; ++i) {
-              const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
-              ex[3 * i] = lnk0 - lnkf[i];
-              ex[3 * i + 1] = lnkf[i];
-              ex[3 * i + 2] = lnkr[i] - lnkf[i];
-            }
-            exp_fast_n<3 * R>(ex, ey, etab);
-#pragma unroll
-            for (int i = 0; i < R; ++i) {
-              const double Pr = ey[3 * i] * M[i];
-              kf[i] = ey[3 * i + 1] * (Pr / (1.0 + Pr));
-              kr[i] = kf[i] * ey[3 * i + 2];
-            }
-          } else if (type == PSR_T_TROE) {
-            // With ln Pr = ln k0 - ln k_inf + ln[M]:  k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
-            // one reactor at a time: five exps in lock step are enough to fill the FP64 pipe
-#pragma unroll
-            for (int i = 0; i < R; ++i) {
-              const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
-              const double lnM = ax->n_eff == 0 ? lnctot_s[lane * R + i] : log(M[i]);
-              const double lnk0M = lnk0 + lnM;
-              double ex[5], ey[5];
-              ex[0] = lnk0M - lnkf[i];          // ln Pr
-              ex[1] = T[i] * ax->troe[1];
-              ex[2] = T[i] * ax->troe[2];
-              ex[3] = ax->troe[3] * invT[i];
-              ex[4] = lnkr[i] - lnkf[i];        // ln(k_r/k_f) = -ln K_c
-              exp_fast_n<5>(ex, ey, etab);
-              const double al = ax->troe[0];
-              const double Fcent = fma(1.0 - al, ey[1], fma(al, ey[2], ey[3]));
-              const double lnFc = log(Fcent);
-              const double lF = lnFc * kLog10e;
-              const double cc = fma(-0.67, lF, -0.4);
-              const double nn = fma(-1.27, lF, 0.75);
-              const double lp = fma(ex[0], kLog10e, cc);
-              const double den = fma(-0.14, lp, nn);
-              // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
-              const double den2 = den * den;
-              double e2[1], k2[1];
-              e2[0] = lnk0M + lnFc * den2 / fma(lp, lp, den2);
-              exp_fast_n<1>(e2, k2, etab);
-              kf[i] = k2[0] / (1.0 + ey[0]);
-              kr[i] = kf[i] * ey[4];
-            }
-          }
-        }
-        // an irreversible reaction has its product side on the zero row (pr = 0), a three-body reaction
-        // carries [M] in both products (pf, pr scaled below): no per-lane selects here
-        double q[R];
-#pragma unroll
-        for (int i = 0; i < R; ++i) q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
-        RowIO<R>::st(q_lane + (uint32_t)kl * (uint32_t)(TR * 8), q);
+          for (int i = 0; i < R; ++i) q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
+          RowIO<R>::st(q_lane + (uint32_t)kl * (uint32_t)(TR * 8), q);
 
-        if (a.flags & (kOutKf | kOutKr | kOutQ)) {
+          if (a.flags & (kOutKf | kOutKr | kOutQ)) {
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            int64_t r_;
-            int jsp_;
-            bool valid_;
-            state_of(tile, i, r_, jsp_, valid_);
-            if (valid_) {
-              const int64_t o = (int64_t)rec->korig * a.ldk + r_;
-              if (a.flags & kOutKf) a.kf[o] = kf[i];
-              if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr[i] : 0.0;
-              if (a.flags & kOutQ) a.q[o] = q[i];
+            for (int i = 0; i < R; ++i) {
+              int64_t r_;
+              int jsp_;
+              bool valid_;
+              state_of(tile, i, r_, jsp_, valid_);
+              if (valid_) {
+                const int64_t o = (int64_t)rec->korig * a.ldk + r_;
+                if (a.flags & kOutKf) a.kf[o] = kf[i];
+                if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr[i] : 0.0;
+                if (a.flags & kOutQ) a.q[o] = q[i];
+              }
             }
           }
         }
+      };
+      auto run_all = [&](auto fast_tag) {
+        run_class(std::integral_constant<int, 0>{}, fast_tag);
+        run_class(std::integral_constant<int, 1>{}, fast_tag);
+        run_class(std::integral_constant<int, 2>{}, fast_tag);
+        run_class(std::integral_constant<int, 3>{}, fast_tag);
+        run_class(std::integral_constant<int, kClsLong>{}, fast_tag);
+      };
+      run_all(std::true_type{});
+      if (__syncthreads_or(bad)) {   // also the barrier that publishes the q tile
+        run_all(std::false_type{});
+        __syncthreads();
       }
-      __syncthreads();
 
       if (c + 1 < mv.n_chunks) gather_and_release();
     }

@@ -58,13 +58,18 @@ struct __attribute__((aligned(16))) EffEnt {  // 16 bytes
   uint32_t pad;
 };
 
-struct __attribute__((aligned(16))) ChunkHdr {  // 80 bytes
+constexpr int kClsLong = 4;      // record classes: 0..3 = PSR_RX_* type in the 3+3 slot form, 4 = long factor lists (any type)
+constexpr int kMaxWarps = 16;
+
+struct __attribute__((aligned(16))) ChunkHdr {  // 240 bytes
   uint32_t n_rx, n_aux, n_eff, n_g;
   uint32_t off_aux, off_eff, off_pool, off_gptr, off_gent;
   uint32_t bytes;         // bytes to copy (multiple of 16)
-  uint16_t wptr[20];      // warp w evaluates records wptr[w] .. wptr[w+1]-1 (cost-balanced at load time)
+  // warp w evaluates the records wb[w][c] .. wb[w][c+1]-1 of class c (cost-balanced over warps at load
+  // time; a warp's records are contiguous and sorted by class)
+  uint16_t wb[kMaxWarps][kClsLong + 2];
 };
-static_assert(sizeof(ChunkHdr) == 80, "ChunkHdr layout");
+static_assert(sizeof(ChunkHdr) == 240, "ChunkHdr layout");
 
 // Gather lists of nu^T (Eq. 4) per chunk: species s adds the q rows gent[gptr[2s] .. gptr[2s+1]) and
 // subtracts gent[gptr[2s+1] .. gptr[2s+2]).  An entry is the byte offset of a row of the q tile;
