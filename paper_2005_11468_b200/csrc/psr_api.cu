@@ -67,9 +67,9 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 double reaction_cost(int type) {  // relative FP64 cost used to balance warps inside a chunk
   switch (type) {
-    case PSR_RX_THREE_BODY: return 1.25;
-    case PSR_RX_LINDEMANN: return 2.0;
-    case PSR_RX_TROE: return 4.0;
+    case PSR_RX_THREE_BODY: return 2.1;   // executed instructions relative to a plain reaction (ncu, C1)
+    case PSR_RX_LINDEMANN: return 2.5;
+    case PSR_RX_TROE: return 4.7;
     default: return 1.0;
   }
 }
@@ -224,8 +224,10 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   };
   int spw = pick_spw(nw);
   if (!spw) { nw = 16; spw = pick_spw(nw); }
-  int rl = 1;  // reactors per lane (2 is compiled for spw <= 16; PSR_R selects it)
-  if (const char* e = getenv("PSR_R")) rl = (atoi(e) == 2 && spw <= 16) ? 2 : 1;
+  // reactors per lane: the kernel is written for R per lane, but only R = 1 is instantiated -- at R = 2 the
+  // q tile of a 325-reaction chunk no longer fits beside the C tiles and the second gather pass costs
+  // more than the halved warp-uniform overhead saves (measured on C1)
+  const int rl = 1;
   const uint32_t row_bytes = (uint32_t)kRowBytes * rl;
   int rc_target = std::min(I, 384);
   if (const char* e = getenv("PSR_RC")) rc_target = std::min(std::min(I, kMaxChunkRx), std::max(8, atoi(e)));

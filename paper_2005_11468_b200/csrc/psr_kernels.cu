@@ -363,10 +363,11 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       // table form and a lane only notes an out-of-range argument; the CTA then repeats the phase with
       // the library exp (IEEE results for NaN, Inf, overflow, gradual underflow).  That never happens for
       // physical states, so the range test costs two compares per reaction and no vote or branch.
-      bool bad = false;
-      auto run_class = [&](auto cls_tag, auto fast_tag) {
+      float amax = 0.0f;   // NaN-propagating running max of |high word| of every exp argument of this lane
+      auto run_class = [&](auto cls_tag, auto fast_tag, auto out_tag) {
         constexpr int CLS = decltype(cls_tag)::value;
         constexpr bool FAST = decltype(fast_tag)::value;
+        constexpr bool OUT = decltype(out_tag)::value;   // k_f, k_r, q go to global memory (psr_eval_kf_kr, q of psr_eval_wdot)
         // the record range is the same in every lane: say so (REDUX writes a uniform register), which
         // keeps the loop counter and the record addresses in the uniform datapath
         const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
@@ -375,7 +376,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           constexpr int N = sizeof(ex) / sizeof(double);
           if constexpr (FAST) {
 #pragma unroll
-            for (int i = 0; i < N; ++i) bad = bad || !exp_in_range(ex[i]);
+            for (int i = 0; i < N; ++i) amax = exp_arg_max(amax, ex[i]);
             exp_core_n<N>(ex, ey, etab);
           } else {
 #pragma unroll
@@ -511,11 +512,14 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                 const double lp = fma(ex[0], kLog10e, cc);
                 const double den = fma(-0.14, lp, nn);
                 // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
+                // both quotients (this one and k_f = .../(1+Pr)) share one reciprocal
                 const double den2 = den * den;
+                const double bq = fma(lp, lp, den2), dq = 1.0 + ey[0];
+                const double inv = 1.0 / (bq * dq);
                 double e2[1], k2[1];
-                e2[0] = lnk0M + lnFc * den2 / fma(lp, lp, den2);
+                e2[0] = fma(lnFc * den2, dq * inv, lnk0M);
                 exps(e2, k2);
-                kf[i] = k2[0] / (1.0 + ey[0]);
+                kf[i] = k2[0] * (bq * inv);
                 kr[i] = kf[i] * ey[4];
               }
             }
@@ -527,7 +531,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           for (int i = 0; i < R; ++i) q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
           RowIO<R>::st(q_lane + (uint32_t)kl * (uint32_t)(TR * 8), q);
 
-          if (a.flags & (kOutKf | kOutKr | kOutQ)) {
+          if constexpr (OUT) {
 #pragma unroll
             for (int i = 0; i < R; ++i) {
               int64_t r_;
@@ -544,15 +548,19 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           }
         }
       };
+      auto run_out = [&](auto fast_tag, auto out_tag) {
+        run_class(std::integral_constant<int, 0>{}, fast_tag, out_tag);
+        run_class(std::integral_constant<int, 1>{}, fast_tag, out_tag);
+        run_class(std::integral_constant<int, 2>{}, fast_tag, out_tag);
+        run_class(std::integral_constant<int, 3>{}, fast_tag, out_tag);
+        run_class(std::integral_constant<int, kClsLong>{}, fast_tag, out_tag);
+      };
       auto run_all = [&](auto fast_tag) {
-        run_class(std::integral_constant<int, 0>{}, fast_tag);
-        run_class(std::integral_constant<int, 1>{}, fast_tag);
-        run_class(std::integral_constant<int, 2>{}, fast_tag);
-        run_class(std::integral_constant<int, 3>{}, fast_tag);
-        run_class(std::integral_constant<int, kClsLong>{}, fast_tag);
+        if (a.flags & (kOutKf | kOutKr | kOutQ)) run_out(fast_tag, std::true_type{});
+        else run_out(fast_tag, std::false_type{});
       };
       run_all(std::true_type{});
-      if (__syncthreads_or(bad)) {   // also the barrier that publishes the q tile
+      if (__syncthreads_or(!exp_max_in_range(amax))) {   // also the barrier that publishes the q tile
         run_all(std::false_type{});
         __syncthreads();
       }
@@ -657,9 +665,8 @@ static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cud
 }
 
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-#define PSR_L(NW_, SPW_)                                                                     \
-  if (nw == NW_ && spw == SPW_ && rl == 1) return launch_t<NW_, SPW_, 1>(mv, a, grid, st); \
-  if (nw == NW_ && spw == SPW_ && rl == 2) return launch_t<NW_, SPW_, 2>(mv, a, grid, st);
+#define PSR_L(NW_, SPW_) \
+  if (nw == NW_ && spw == SPW_ && rl == 1) return launch_t<NW_, SPW_, 1>(mv, a, grid, st);
   PSR_SHAPES(PSR_L)
 #undef PSR_L
   return cudaErrorInvalidConfiguration;
@@ -674,9 +681,8 @@ static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
 }
 
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm) {
-#define PSR_O(NW_, SPW_)                                                                    \
-  if (nw == NW_ && spw == SPW_ && rl == 1) return occ_t<NW_, SPW_, 1>(smem, ctas_per_sm); \
-  if (nw == NW_ && spw == SPW_ && rl == 2) return occ_t<NW_, SPW_, 2>(smem, ctas_per_sm);
+#define PSR_O(NW_, SPW_) \
+  if (nw == NW_ && spw == SPW_ && rl == 1) return occ_t<NW_, SPW_, 1>(smem, ctas_per_sm);
   PSR_SHAPES(PSR_O)
 #undef PSR_O
   return cudaErrorInvalidConfiguration;

@@ -106,6 +106,15 @@ __device__ __forceinline__ bool exp_in_range(double a) {
   return fabsf(__int_as_float(__double2hiint(a))) < __int_as_float(0x4085e000);
 }
 
+// Deferred form of the same test: m = max(m, |high word of a| read as a float), NaN-propagating (the high
+// word of a double NaN or Inf reads as a float NaN), then one compare per lane at the end of a phase.
+__device__ __forceinline__ float exp_arg_max(float m, double a) {
+  float r;
+  asm("max.NaN.f32 %0, %1, %2;" : "=f"(r) : "f"(fabsf(__int_as_float(__double2hiint(a)))), "f"(m));
+  return r;
+}
+__device__ __forceinline__ bool exp_max_in_range(float m) { return m < __int_as_float(0x4085e000); }
+
 // all 32 lanes of the warp must call this together
 __device__ __forceinline__ double exp_fast(double x, const ExpTab& tab) {
   return __all_sync(kFullMask, exp_in_range(x)) ? exp_core(x, tab) : exp(x);

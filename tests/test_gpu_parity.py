@@ -206,6 +206,38 @@ def test_negative_and_zero_mass_fractions_propagate(torch_cuda, binding):
     check_against_oracle(mech, b2, got)
 
 
+def test_out_of_range_exp_arguments_take_the_library_path(torch_cuda, binding):
+    """A few very cold reactors push exp arguments beyond |x| = 700 (Ea/RT ~ 1000).  The kernel's table
+    exp is not valid there: the CTA must notice and repeat its reaction phase with the library exp, for
+    every lane of the tile.  Warm lanes of the same tiles must still match the oracle to tolerance; in
+    the cold lanes k_f (T-only, Eq. 6) must underflow the way the oracle's does."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C1", 96)
+    T = batch.T.copy()
+    cold = np.array([5, 40, 41, 95])
+    T[cold] = [20.0, 25.0, 22.0, 18.0]
+    b2 = synth.ReactorBatch(T, batch.P, batch.Y, batch.Yin, batch.tau)
+    got = gpu_eval(torch, binding, mech, b2)
+    ref = orc.evaluate(oracle_mech(mech), b2.T, b2.P, b2.Y, b2.Yin, b2.tau, want=("kf", "kr", "q", "wdot", "F"))
+    warm = np.setdiff1d(np.arange(96), cold)
+    assert rel_err(got["kf"][:, warm], ref["kf"][:, warm]).max() <= TOL_K
+    assert rel_err(got["kr"][:, warm], ref["kr"][:, warm]).max() <= TOL_K
+    werr, mask = wdot_masked_rel_err(got["wdot"][:, warm], ref["wdot"][:, warm])
+    assert mask.any() and werr.max() <= TOL_K
+    assert residual_rel_err(got["F"][:, warm], ref["F"][:, warm]).max() <= TOL_F
+    # cold lanes, plain and three-body reactions.  The oracle forms A * T^b * exp(-Ea/RT) as the paper
+    # writes it, so ITS result loses digits once exp(-Ea/RT) alone is subnormal (Ea/RT > ~708) although
+    # k_f is not; compare to tolerance only where that intermediate is normal, and elsewhere require a
+    # clean underflow (finite, non-negative, tiny).
+    simple = mech.rtype <= 1
+    kc, kref = got["kf"][simple][:, cold], ref["kf"][simple][:, cold]
+    arg = mech.Ea[simple, None] / (1.9872042586408317 * T[cold][None, :])
+    safe = (arg < 690.0) & (kref > 1e-290)
+    assert safe.any() and (arg > 720.0).any()      # the case does straddle the range of the table exp
+    assert rel_err(kc[safe], kref[safe]).max() <= TOL_K
+    assert np.all(np.isfinite(kc)) and np.all(kc >= 0.0) and np.all(kc[arg > 720.0] < 1e-280)
+
+
 # ------------------------------------------------------------------ full-size launch, sampled
 def test_C1_full_size_sampled(torch_cuda, binding):
     """BASELINE config 1 at its full batch (65,536 reactors, the launch bench.py times): compare a
