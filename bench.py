@@ -171,7 +171,7 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2005_11468_b200 import binding, synth
+    from paper_2005_11468_b200 import binding, shard, synth
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -186,7 +186,7 @@ def run_ours(args):
     # data-path collective -- SURVEY.md 8(e)); rank r draws the C1 state stream with seed 2001 + 100 r
     mech, batch = synth.make_config("C1")
     if rank > 0:
-        batch = synth.make_states(mech.n_species, batch.n, seed=2001 + 100 * rank, **synth.CONFIGS["C1"]["state"])
+        batch = synth.make_states(mech.n_species, batch.n, seed=shard.state_seed(1, rank), **synth.CONFIGS["C1"]["state"])
     N, K, I = batch.n, mech.n_species, mech.n_reactions
     gm = binding.Mechanism.from_synth(mech)
     info = gm.info()
@@ -218,12 +218,9 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop()
     dev_ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
-    if world > 1:
-        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_ms = float(t.item())
+    dev_ms = shard.max_over_ranks(dev_ms, device="cuda")
     ms_per_step = dev_ms / args.steps
-    value = world * N * args.steps / (dev_ms * 1e-3)
+    value = shard.whole_job_rate(N, args.steps, dev_ms, world)
 
     # ---- end to end: host pinned buffers in, host pinned buffers out, same C-ABI call
     h_in = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
@@ -250,11 +247,8 @@ def run_ours(args):
     a1.record(stream)
     barrier()
     e2e_ms = a0.elapsed_time(a1)
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = world * N * e2e_steps / (e2e_ms * 1e-3)
+    e2e_ms = shard.max_over_ranks(e2e_ms, device="cuda")
+    e2e_value = shard.whole_job_rate(N, e2e_steps, e2e_ms, world)
     assert bool(torch.isfinite(h_out[0]).all())
 
     # ---- roofline of the dominant (only) kernel: FP64 ALU pipe
