@@ -36,7 +36,8 @@ struct psr_mech {
   double* d_W = nullptr;
   double* d_exptab = nullptr;
   int32_t* d_sp_of = nullptr;
-  double* d_scratch = nullptr;  // internal F0 buffer for psr_fd_jacobian when the caller passes none
+  int32_t* d_rec_base = nullptr;  // [n_chunks + 1]
+  double* d_scratch = nullptr;  // psr_fd_jacobian: rate table [N][I][kRateVals], then F0 when the caller passes none
   size_t scratch_bytes = 0;
   int device = 0;
 };
@@ -233,12 +234,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   if (const char* e = getenv("PSR_RC")) rc_target = std::min(std::min(I, kMaxChunkRx), std::max(8, atoi(e)));
   // shared memory left for the q tile and the chunk ring beside one C tile and the per-CTA scratch
   const size_t smem_fixed = align_up((size_t)(K + 2) * kTile * rl * 8, 128) + (size_t)nw * kTile * rl * 8 +
-                            (size_t)9 * kTile * rl * 8 + 64;
+                            (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages);
   int n_chunks = 0, rc = 0;
   bool resident = false;
   size_t stride = 0;
   std::vector<unsigned char> all;
-  std::vector<int32_t> sp_of;
+  std::vector<int32_t> sp_of, rec_base_of;
   // the chunk size shrinks until one C tile, the q tile and the (double-buffered) chunk ring fit one CTA
   for (;; rc_target = rc_target * 3 / 4) {
   if (rc_target < 1)
@@ -301,6 +302,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   }
 
   // ---- serialise chunk blobs
+  rec_base_of.assign(n_chunks + 1, 0);
+  for (int c = 0; c < n_chunks; ++c) rec_base_of[c + 1] = rec_base_of[c] + (int32_t)chunk_rx[c].size();
   std::vector<std::vector<unsigned char>> blobs(n_chunks);
   stride = 0;
   const uint32_t unit_off = (uint32_t)K * row_bytes;   // the all-ones row of the C tile
@@ -367,7 +370,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     hdr.n_rx = n_rx;
     hdr.n_aux = (uint32_t)auxs.size();
     hdr.n_eff = (uint32_t)effs.size();
-    hdr.n_g = (uint32_t)gent.size();
+    hdr.rec_base = (uint32_t)rec_base_of[c];
     for (int wv = 0; wv < kMaxWarps; ++wv)
       for (int cl = 0; cl < kClsLong + 2; ++cl) hdr.wb[wv][cl] = (uint16_t)chunk_wb[c][(size_t)wv * (kClsLong + 2) + cl];
     size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
@@ -395,7 +398,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   }
   stride = align_up(stride, 128);
   // all chunk blobs resident in shared memory (loaded once per CTA) when they fit, else a 2-stage ring
-  const size_t q_bytes = align_up((size_t)(rc + 1) * kTile * rl * 8, 128);
+  // q tile plus the rate-table slice of one chunk (Y-column launch of psr_fd_jacobian)
+  const size_t q_bytes = align_up((size_t)(rc + 1) * kTile * rl * 8, 128) + align_up((size_t)rc * kRateVals * 8, 128);
   resident = n_chunks <= kMaxStages && smem_fixed + q_bytes + stride * n_chunks <= (size_t)prop.sharedMemPerBlockOptin &&
              (n_chunks == 1 || stride * n_chunks <= 48 * 1024);
   const size_t need = smem_fixed + q_bytes + stride * (resident ? n_chunks : 2);
@@ -433,8 +437,10 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     o += align_up((size_t)(rc + 1) * kTile * rl * 8, 128);  // + the all-zero row
     v.smem_mech = (uint32_t)o;
     o += stride * (resident ? n_chunks : 2);
+    v.smem_tab = (uint32_t)o;
+    o += align_up((size_t)rc * kRateVals * 8, 128);
     v.smem_misc = (uint32_t)o;
-    o += (size_t)nw * kTile * rl * 8 + (size_t)9 * kTile * rl * 8 + 64;  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P prefetch; mbarriers
+    o += (size_t)nw * kTile * rl * 8 + (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages);  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P prefetch; mbarriers
     v.smem_total = (uint32_t)o;
     v.n_cbuf = n_cbuf;
     return o;
@@ -474,6 +480,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     cleanup();
     return cuda_fail(e, "species ownership upload");
   }
+  if ((e = cudaMalloc(&m->d_rec_base, 4 * rec_base_of.size())) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_rec_base, rec_base_of.data(), 4 * rec_base_of.size(), cudaMemcpyHostToDevice)) != cudaSuccess) {
+    cleanup();
+    return cuda_fail(e, "chunk record bases upload");
+  }
+  v.chunk_rec_base = m->d_rec_base;
   v.sp_of = m->d_sp_of;
   v.exp_tab = m->d_exptab;
   v.chunks = m->d_chunks;
@@ -494,6 +506,7 @@ void psr_mech_free(psr_mech* m) {
   cudaFree(m->d_W);
   cudaFree(m->d_exptab);
   cudaFree(m->d_sp_of);
+  cudaFree(m->d_rec_base);
   cudaFree(m->d_scratch);
   delete m;
 }
@@ -589,31 +602,65 @@ psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const
   if (st != PSR_OK || N == 0) return st;
   if (!Yin || !tau || !J) return fail(PSR_EINVAL, "psr_fd_jacobian: null Yin, tau or J");
   psr_mech* m = const_cast<psr_mech*>(mc);
-  const int64_t n = m->view.K + 1;
-  if (!F0) {
-    const size_t need = (size_t)N * n * 8;
-    if (need > m->scratch_bytes) {
-      cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
-      if (e != cudaSuccess) return cuda_fail(e, "psr_fd_jacobian: sync before scratch growth");
-      cudaFree(m->d_scratch);
-      m->d_scratch = nullptr;
-      m->scratch_bytes = 0;
-      if ((e = cudaMalloc(&m->d_scratch, need)) != cudaSuccess) return fail(PSR_ENOMEM, "psr_fd_jacobian: scratch: %s", cudaGetErrorString(e));
-      m->scratch_bytes = need;
-    }
-    F0 = m->d_scratch;
+  const int64_t K = m->view.K, n = K + 1, I = m->view.I;
+
+  // The sweep runs in sub-batches of Nb reactors so that the rate table (I * kRateVals doubles per reactor)
+  // written by the base launch is still in L2 when the Y-column launch reads it.
+  const size_t row_bytes = (size_t)I * kRateVals * 8;
+  const int64_t wave = (int64_t)m->n_sm * m->ctas_per_sm * m->tile;   // reactors per full wave of base tiles
+  int64_t Nb = std::max<int64_t>(1, (int64_t)((size_t)64 * 1024 * 1024 / row_bytes));
+  if (Nb > wave) Nb -= Nb % wave;
+  Nb = std::min(Nb, N);
+  bool unhoisted = false;   // diagnostic: every column a full evaluation (tests compare the two sweeps)
+  if (const char* e = getenv("PSR_JAC_UNHOISTED")) unhoisted = atoi(e) != 0;
+
+  const size_t tab_bytes = align_up((size_t)Nb * row_bytes, 256);
+  const size_t need = tab_bytes + (F0 ? 0 : (size_t)N * n * 8);
+  if (need > m->scratch_bytes) {
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "psr_fd_jacobian: sync before scratch growth");
+    cudaFree(m->d_scratch);
+    m->d_scratch = nullptr;
+    m->scratch_bytes = 0;
+    if ((e = cudaMalloc(&m->d_scratch, need)) != cudaSuccess) return fail(PSR_ENOMEM, "psr_fd_jacobian: scratch: %s", cudaGetErrorString(e));
+    m->scratch_bytes = need;
   }
-  EvalArgs a{};
-  a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.F0out = F0;
-  a.flags = kOutF0;
-  a.n_tiles = (N + m->tile - 1) / m->tile;
-  st = run(m, a, stream, "psr_fd_jacobian (base residual)");
-  if (st != PSR_OK) return st;
-  EvalArgs b{};
-  b.N = N; b.ld = ld; b.T = T; b.P = P; b.Y = Y; b.Yin = Yin; b.tau = tau; b.J = J; b.F0 = F0;
-  b.flags = kModeJac;
-  b.n_tiles = (N * n + m->tile - 1) / m->tile;
-  return run(m, b, stream, "psr_fd_jacobian (perturbed sweeps)");
+  double* tab = m->d_scratch;
+  if (!F0) F0 = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(m->d_scratch) + tab_bytes);
+
+  const int tpr = (int)((K + 31) / 32);
+  for (int64_t r0 = 0; r0 < N; r0 += Nb) {
+    const int64_t nb = std::min(Nb, N - r0);
+    EvalArgs a{};
+    a.N = nb; a.ld = ld; a.T = T + r0; a.P = P + r0; a.Y = Y + r0; a.Yin = Yin + r0; a.tau = tau + r0;
+    a.F0out = F0 + r0 * n;
+    a.tab_out = tab;
+    a.flags = kOutF0 | (unhoisted ? 0u : kOutTab);
+    a.n_tiles = (nb + m->tile - 1) / m->tile;
+    st = run(m, a, stream, "psr_fd_jacobian (base residual)");
+    if (st != PSR_OK) return st;
+    EvalArgs b{};
+    b.N = nb; b.ld = ld; b.T = a.T; b.P = a.P; b.Y = a.Y; b.Yin = a.Yin; b.tau = a.tau;
+    b.J = J + r0 * n * n;
+    b.F0 = a.F0out;
+    if (unhoisted) {
+      b.flags = kModeJac;
+      b.n_tiles = (nb * n + m->tile - 1) / m->tile;
+      st = run(m, b, stream, "psr_fd_jacobian (all columns)");
+      if (st != PSR_OK) return st;
+      continue;
+    }
+    b.flags = kModeJacT;                       // column 0: T perturbed, every factor changes
+    b.n_tiles = (nb + m->tile - 1) / m->tile;
+    st = run(m, b, stream, "psr_fd_jacobian (T column)");
+    if (st != PSR_OK) return st;
+    b.flags = kModeJacY;                       // columns 1..K: T-only factors from the rate table
+    b.tab = tab;
+    b.n_tiles = nb * tpr;
+    st = run(m, b, stream, "psr_fd_jacobian (Y columns)");
+    if (st != PSR_OK) return st;
+  }
+  return PSR_OK;
 }
 
 psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {

@@ -96,8 +96,12 @@ struct RowIO<2> {
 // ------------------------------------------------------------------ the fused kernel
 // R reactors per lane: every warp-uniform instruction (mechanism loads, address arithmetic, branches)
 // is amortised over R evaluations and the R exp chains interleave in the FP64 pipe.
-template <int NW, int SPW, int R>
+// JY: the Y-column launch of psr_fd_jacobian (kModeJacY) -- tiles are aligned to reactors (the 32 lanes of
+// a tile are 32 Y columns of ONE reactor) and the T-only factors of every reaction come from the rate
+// table that the base-residual launch wrote, as warp-uniform broadcasts, instead of being recomputed.
+template <int NW, int SPW, int R, bool JY>
 __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const MechView mv, const EvalArgs a) {
+  static_assert(!JY || R == 1, "the Y-column mode maps one column to a lane");
   constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
   double* Cs0 = reinterpret_cast<double*>(smem + mv.smem_cs);         // [2][K+2][TR]; row K is the unit row
@@ -110,13 +114,16 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   double* ctot_s = rho_s + TR;                                        // [TR]: C_tot per state
   double* lnctot_s = ctot_s + TR;                                     // [TR]: ln C_tot (formed on first use)
   double* tp = lnctot_s + TR;                                         // [2][2][TR]: prefetched T, P
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [kMaxStages]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [kMaxStages] chunk stages, [kMaxStages] rate table
+  double* tab_s = reinterpret_cast<double*>(smem + mv.smem_tab);      // [rc][kRateVals]: this reactor's slice (JY)
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
   const int K = mv.K;
   const int n = K + 1;
-  const bool jac = (a.flags & kModeJac) != 0;
+  const bool jac = (a.flags & (kModeJac | kModeJacT | kModeJacY)) != 0;
+  const bool jacT = (a.flags & kModeJacT) != 0;
+  const int tpr = (K + 31) / 32;   // JY: tiles per reactor
   const bool resident = mv.resident != 0;   // every chunk blob has its own stage and is loaded once per CTA
   const int nstage = resident ? mv.n_chunks : 2;
   const int cs_elems = (K + 2) * TR;
@@ -126,7 +133,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   const int64_t total_loads = resident ? mv.n_chunks : my_tiles * mv.n_chunks;
 
   if (threadIdx.x == 0) {
-    for (int g = 0; g < kMaxStages; ++g) mbar_init(&bars[g], 1);
+    for (int g = 0; g <= kMaxStages; ++g) mbar_init(&bars[g], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     for (int g = 0; g < nstage && g < total_loads; ++g) {
@@ -148,7 +155,17 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   // shared memory it lives at column lane*R + i of every row.  Jacobian mode: v = reactor*n + column.
   auto state_of = [&](int64_t t, int i, int64_t& r_, int& jsp_, bool& valid_) {
     const int64_t v = t * TR + i * 32 + lane;
-    if (jac) {
+    if constexpr (JY) {
+      const uint32_t tr = (uint32_t)t / (uint32_t)tpr;   // tiles of a sub-batch fit 32 bits (psr_fd_jacobian)
+      r_ = tr;
+      const int j = (int)((uint32_t)t - tr * (uint32_t)tpr) * 32 + lane;
+      valid_ = j < K;
+      jsp_ = valid_ ? j : -2;         // lanes beyond the last species evaluate the unperturbed state, unused
+    } else if (jacT) {
+      valid_ = v < a.N;
+      r_ = valid_ ? v : a.N - 1;
+      jsp_ = -1;
+    } else if (jac) {
       valid_ = v < a.N * n;
       const int64_t vv = valid_ ? v : a.N * n - 1;
       r_ = vv / n;
@@ -181,6 +198,18 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
   prefetch(blockIdx.x, 0);
+  // JY: bulk copy of the rate-table slice of tile t's reactor for chunk c into tab_s (thread 0 only)
+  auto load_tab = [&](int64_t t, int c) {
+    const int b0 = mv.chunk_rec_base[c], b1 = mv.chunk_rec_base[c + 1];
+    const uint32_t bytes = (uint32_t)(b1 - b0) * (kRateVals * 8);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_expect_tx(&bars[kMaxStages], bytes);
+    bulk_g2s(tab_s, a.tab + ((size_t)((uint32_t)t / (uint32_t)tpr) * mv.I + b0) * kRateVals, bytes, &bars[kMaxStages]);
+  };
+  int64_t gt = 0;  // rate-table slices consumed so far by this CTA
+  if constexpr (JY) {
+    if (threadIdx.x == 0 && blockIdx.x < a.n_tiles) load_tab(blockIdx.x, 0);
+  }
   __syncthreads();
 
   int64_t g = 0;  // chunk loads consumed so far by this CTA
@@ -282,7 +311,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
       for (int i = 0; i < R; ++i) acc[jj][i] = 0.0;
 
-    const bool wantF = (a.flags & (kOutF | kOutF0 | kModeJac)) != 0;
+    const bool wantF = jac || (a.flags & (kOutF | kOutF0)) != 0;
 
     // ---------------------------------------------------------------- chunks
     int stage = 0;
@@ -291,7 +320,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     // gather (a8, Eq. 4) of the chunk in `stage`: every warp sums the rows of nu^T it owns in a fixed
     // order; afterwards the stage is handed back to the bulk-copy ring
     auto gather_and_release = [&]() {
-      if (a.flags & (kOutWdot | kOutF | kModeJac | kOutF0)) {
+      if (jac || (a.flags & (kOutWdot | kOutF | kOutF0))) {
         const uint32_t* gptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_gptr);
         const uint4* gent = reinterpret_cast<const uint4*>(blob + hdr->off_gent);
 #pragma unroll
@@ -367,7 +396,12 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       auto run_class = [&](auto cls_tag, auto fast_tag, auto out_tag) {
         constexpr int CLS = decltype(cls_tag)::value;
         constexpr bool FAST = decltype(fast_tag)::value;
-        constexpr bool OUT = decltype(out_tag)::value;   // k_f, k_r, q go to global memory (psr_eval_kf_kr, q of psr_eval_wdot)
+        // 0: nothing leaves the loop but q; 1: k_f, k_r, q go to global memory (psr_eval_kf_kr, q of
+        // psr_eval_wdot); 2: the T-only factors go to the rate table (base launch of psr_fd_jacobian);
+        // 3: decided by the flags at run time (the rare library-exp repeat, to keep the code small)
+        constexpr int OUTT = decltype(out_tag)::value;
+        const bool out_k = OUTT == 1 || (OUTT == 3 && (a.flags & (kOutKf | kOutKr | kOutQ)) != 0);
+        const bool out_tab = OUTT == 2 || (OUTT == 3 && (a.flags & kOutTab) != 0);
         // the record range is the same in every lane: say so (REDUX writes a uniform register), which
         // keeps the loop counter and the record addresses in the uniform datapath
         const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
@@ -383,20 +417,31 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
             for (int i = 0; i < N; ++i) ey[i] = exp(ex[i]);
           }
         };
+        // rate table row of this lane's reactor (OUT == 2 only)
+        auto tab_row = [&](int kl, int i, bool& valid_) -> double* {
+          int64_t r_;
+          int jsp_;
+          state_of(tile, i, r_, jsp_, valid_);
+          return a.tab_out + ((size_t)r_ * mv.I + hdr->rec_base + kl) * kRateVals;
+        };
 #pragma unroll 1
         for (int kl = kl_begin; kl < kl_end; ++kl) {
           const RxRec* rec = recs + kl;
           const uint32_t meta = rec->meta;
           const int type = CLS < kClsLong ? CLS : (int)(meta & kMetaTypeMask);
+          const double* tv = tab_s + kl * kRateVals;   // JY: the reactor's T-only factors of this reaction
           double lnkf[R], lnkr[R], pf[R], pr[R], kf[R], kr[R], M[R];
           // Eq. 6 in log form, and ln k_r = ln k_f - ln K_c (Eq. 7-9 summed per reaction at load time)
+          if constexpr (!JY) {
 #pragma unroll
-          for (int i = 0; i < R; ++i) {
-            lnkf[i] = fma(rec->c[1], lnT[i], fma(rec->c[2], invT[i], rec->c[0]));
-            const double pn = fma(fma(fma(rec->d[3], T[i], rec->d[2]), T[i], rec->d[1]), T[i], rec->d[0]);
-            lnkr[i] = fma(pn, T[i], fma(rec->e[1], lnT[i], fma(rec->e[2], invT[i], rec->e[0])));
-            M[i] = 1.0;
+            for (int i = 0; i < R; ++i) {
+              lnkf[i] = fma(rec->c[1], lnT[i], fma(rec->c[2], invT[i], rec->c[0]));
+              const double pn = fma(fma(fma(rec->d[3], T[i], rec->d[2]), T[i], rec->d[1]), T[i], rec->d[0]);
+              lnkr[i] = fma(pn, T[i], fma(rec->e[1], lnT[i], fma(rec->e[2], invT[i], rec->e[0])));
+            }
           }
+#pragma unroll
+          for (int i = 0; i < R; ++i) M[i] = 1.0;
 
           // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
           if constexpr (CLS < kClsLong) {
@@ -438,17 +483,36 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           }
 
           if (type <= PSR_T_THREE_BODY) {
-            double ex[2 * R], ey[2 * R];
+            if constexpr (JY) {
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-              ex[2 * i] = lnkf[i];
-              ex[2 * i + 1] = lnkr[i];
-            }
-            exps(ex, ey);
+              for (int i = 0; i < R; ++i) {
+                kf[i] = tv[0];
+                kr[i] = tv[1];
+              }
+            } else {
+              double ex[2 * R], ey[2 * R];
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-              kf[i] = ey[2 * i];
-              kr[i] = ey[2 * i + 1];
+              for (int i = 0; i < R; ++i) {
+                ex[2 * i] = lnkf[i];
+                ex[2 * i + 1] = lnkr[i];
+              }
+              exps(ex, ey);
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                kf[i] = ey[2 * i];
+                kr[i] = ey[2 * i + 1];
+              }
+              if (out_tab) {
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                  bool valid_;
+                  double* row = tab_row(kl, i, valid_);
+                  if (valid_) {
+                    row[0] = kf[i];
+                    row[1] = kr[i];
+                  }
+                }
+              }
             }
           }
           if (type != PSR_T_PLAIN) {
@@ -472,15 +536,37 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               }
             } else if (type == PSR_T_LINDEMANN) {
               // k_f = k_inf Pr/(1+Pr), Pr = k0 [M]/k_inf
-              double ex[3 * R], ey[3 * R];
+              double ey[3 * R];
+              if constexpr (JY) {
 #pragma unroll
-              for (int i = 0; i < R; ++i) {
-                const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
-                ex[3 * i] = lnk0 - lnkf[i];
-                ex[3 * i + 1] = lnkf[i];
-                ex[3 * i + 2] = lnkr[i] - lnkf[i];
+                for (int i = 0; i < R; ++i) {
+                  ey[3 * i] = tv[2];
+                  ey[3 * i + 1] = tv[0];
+                  ey[3 * i + 2] = tv[1];
+                }
+              } else {
+                double ex[3 * R];
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                  const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
+                  ex[3 * i] = lnk0 - lnkf[i];
+                  ex[3 * i + 1] = lnkf[i];
+                  ex[3 * i + 2] = lnkr[i] - lnkf[i];
+                }
+                exps(ex, ey);
+                if (out_tab) {
+#pragma unroll
+                  for (int i = 0; i < R; ++i) {
+                    bool valid_;
+                    double* row = tab_row(kl, i, valid_);
+                    if (valid_) {
+                      row[0] = ey[3 * i + 1];
+                      row[1] = ey[3 * i + 2];
+                      row[2] = ey[3 * i];
+                    }
+                  }
+                }
               }
-              exps(ex, ey);
 #pragma unroll
               for (int i = 0; i < R; ++i) {
                 const double Pr = ey[3 * i] * M[i];
@@ -490,37 +576,68 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
             } else {
               // Troe.  With ln Pr = ln k0 - ln k_inf + ln[M]:
               //   k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
-              // one reactor at a time: five exps in lock step are enough to fill the FP64 pipe
+              // one reactor at a time: five exps in lock step are enough to fill the FP64 pipe.  The JY
+              // form repeats the same operations on the tabulated ln k0, ln k_inf, ln F_cent, 1/K_c, so the
+              // T-only part of a perturbed state is bit-identical to that of the base state.
 #pragma unroll
               for (int i = 0; i < R; ++i) {
-                const double lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
                 const double lnM = ax->n_eff == 0 ? lnctot_s[lane * R + i] : log(M[i]);
+                double lnk0, lnkinf, lnFc, invKc, Pr;
+                if constexpr (JY) {
+                  lnk0 = tv[0];
+                  invKc = tv[1];
+                  lnkinf = tv[2];
+                  lnFc = tv[3];
+                } else {
+                  lnk0 = fma(ax->c0[1], lnT[i], fma(ax->c0[2], invT[i], ax->c0[0]));
+                  lnkinf = lnkf[i];
+                }
                 const double lnk0M = lnk0 + lnM;
-                double ex[5], ey[5];
-                ex[0] = lnk0M - lnkf[i];          // ln Pr
-                ex[1] = T[i] * ax->troe[1];
-                ex[2] = T[i] * ax->troe[2];
-                ex[3] = ax->troe[3] * invT[i];
-                ex[4] = lnkr[i] - lnkf[i];        // ln(k_r/k_f) = -ln K_c
-                exps(ex, ey);
-                const double al = ax->troe[0];
-                const double Fcent = fma(1.0 - al, ey[1], fma(al, ey[2], ey[3]));
-                const double lnFc = log(Fcent);
+                const double lnPr = lnk0M - lnkinf;
+                if constexpr (JY) {
+                  double ex[1], ey[1];
+                  ex[0] = lnPr;
+                  exps(ex, ey);
+                  Pr = ey[0];
+                } else {
+                  double ex[5], ey[5];
+                  ex[0] = lnPr;
+                  ex[1] = T[i] * ax->troe[1];
+                  ex[2] = T[i] * ax->troe[2];
+                  ex[3] = ax->troe[3] * invT[i];
+                  ex[4] = lnkr[i] - lnkf[i];        // ln(k_r/k_f) = -ln K_c
+                  exps(ex, ey);
+                  Pr = ey[0];
+                  invKc = ey[4];
+                  const double al = ax->troe[0];
+                  const double Fcent = fma(1.0 - al, ey[1], fma(al, ey[2], ey[3]));
+                  lnFc = log(Fcent);
+                  if (out_tab) {
+                    bool valid_;
+                    double* row = tab_row(kl, i, valid_);
+                    if (valid_) {
+                      row[0] = lnk0;
+                      row[1] = invKc;
+                      row[2] = lnkinf;
+                      row[3] = lnFc;
+                    }
+                  }
+                }
                 const double lF = lnFc * kLog10e;
                 const double cc = fma(-0.67, lF, -0.4);
                 const double nn = fma(-1.27, lF, 0.75);
-                const double lp = fma(ex[0], kLog10e, cc);
+                const double lp = fma(lnPr, kLog10e, cc);
                 const double den = fma(-0.14, lp, nn);
                 // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
                 // both quotients (this one and k_f = .../(1+Pr)) share one reciprocal
                 const double den2 = den * den;
-                const double bq = fma(lp, lp, den2), dq = 1.0 + ey[0];
+                const double bq = fma(lp, lp, den2), dq = 1.0 + Pr;
                 const double inv = 1.0 / (bq * dq);
                 double e2[1], k2[1];
                 e2[0] = fma(lnFc * den2, dq * inv, lnk0M);
                 exps(e2, k2);
                 kf[i] = k2[0] * (bq * inv);
-                kr[i] = kf[i] * ey[4];
+                kr[i] = kf[i] * invKc;
               }
             }
           }
@@ -531,7 +648,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           for (int i = 0; i < R; ++i) q[i] = fma(kf[i], pf[i], -(kr[i] * pr[i]));
           RowIO<R>::st(q_lane + (uint32_t)kl * (uint32_t)(TR * 8), q);
 
-          if constexpr (OUT) {
+          if (out_k) {
 #pragma unroll
             for (int i = 0; i < R; ++i) {
               int64_t r_;
@@ -556,13 +673,28 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         run_class(std::integral_constant<int, kClsLong>{}, fast_tag, out_tag);
       };
       auto run_all = [&](auto fast_tag) {
-        if (a.flags & (kOutKf | kOutKr | kOutQ)) run_out(fast_tag, std::true_type{});
-        else run_out(fast_tag, std::false_type{});
+        if constexpr (JY) {
+          run_out(fast_tag, std::integral_constant<int, 0>{});
+        } else if constexpr (!decltype(fast_tag)::value) {
+          run_out(fast_tag, std::integral_constant<int, 3>{});
+        } else {
+          if (a.flags & (kOutKf | kOutKr | kOutQ)) run_out(fast_tag, std::integral_constant<int, 1>{});
+          else if (a.flags & kOutTab) run_out(fast_tag, std::integral_constant<int, 2>{});
+          else run_out(fast_tag, std::integral_constant<int, 0>{});
+        }
       };
+      if constexpr (JY) mbar_wait(&bars[kMaxStages], (uint32_t)(gt & 1));   // this reactor's rate table slice
       run_all(std::true_type{});
       if (__syncthreads_or(!exp_max_in_range(amax))) {   // also the barrier that publishes the q tile
         run_all(std::false_type{});
         __syncthreads();
+      }
+      if constexpr (JY) {
+        // the table buffer is free: request the slice of the next (tile, chunk) of this CTA
+        ++gt;
+        const bool more_chunks = c + 1 < mv.n_chunks;
+        const int64_t nt = more_chunks ? tile : tile + gridDim.x;
+        if (threadIdx.x == 0 && nt < a.n_tiles) load_tab(nt, more_chunks ? c + 1 : 0);
       }
 
       if (c + 1 < mv.n_chunks) gather_and_release();
@@ -640,11 +772,30 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         if (w == 0) stg[st * npad] = (jsp[i] == -1) ? 1.0 : 0.0;  // row 0: F_T = T - T_set
       }
       __syncthreads();
-      const int64_t base = tile * TR * (int64_t)n;
-      const int64_t lim = a.N * (int64_t)n * n;
-      for (int idx = threadIdx.x; idx < TR * n; idx += NW * 32) {
-        const int l = idx / n, i = idx - l * n;
-        if (base + idx < lim) a.J[base + idx] = stg[l * npad + i];
+      if constexpr (JY) {
+        // columns 1 + cb*32 .. of reactor r: contiguous in J (column-major per reactor)
+        const int64_t r_ = (uint32_t)tile / (uint32_t)tpr;
+        const int cb = (int)(tile - r_ * tpr);
+        const int ncol = min(32, K - cb * 32);
+        double* dst = a.J + (r_ * n + 1 + cb * 32) * (int64_t)n;
+        for (int idx = threadIdx.x; idx < ncol * n; idx += NW * 32) {
+          const int l = idx / n, i = idx - l * n;
+          dst[idx] = stg[l * npad + i];
+        }
+      } else if (jacT) {
+        // column 0 of reactors tile*TR ..: n contiguous doubles each, n*n apart
+        for (int idx = threadIdx.x; idx < TR * n; idx += NW * 32) {
+          const int l = idx / n, i = idx - l * n;
+          const int64_t r_ = tile * TR + l;
+          if (r_ < a.N) a.J[r_ * n * n + i] = stg[l * npad + i];
+        }
+      } else {
+        const int64_t base = tile * TR * (int64_t)n;
+        const int64_t lim = a.N * (int64_t)n * n;
+        for (int idx = threadIdx.x; idx < TR * n; idx += NW * 32) {
+          const int l = idx / n, i = idx - l * n;
+          if (base + idx < lim) a.J[base + idx] = stg[l * npad + i];
+        }
       }
       __syncthreads();
     }
@@ -655,9 +806,9 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 // ------------------------------------------------------------------ launch wrapper
 #define PSR_SHAPES(X) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)
 
-template <int NW, int SPW, int R>
+template <int NW, int SPW, int R, bool JY>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  auto kern = psr_eval_kernel<NW, SPW, R>;
+  auto kern = psr_eval_kernel<NW, SPW, R, JY>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mv.smem_total);
   if (e != cudaSuccess) return e;
   kern<<<grid, NW * 32, mv.smem_total, st>>>(mv, a);
@@ -665,8 +816,10 @@ static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cud
 }
 
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
+  const bool jy = (a.flags & kModeJacY) != 0;
 #define PSR_L(NW_, SPW_) \
-  if (nw == NW_ && spw == SPW_ && rl == 1) return launch_t<NW_, SPW_, 1>(mv, a, grid, st);
+  if (nw == NW_ && spw == SPW_ && rl == 1) \
+    return jy ? launch_t<NW_, SPW_, 1, true>(mv, a, grid, st) : launch_t<NW_, SPW_, 1, false>(mv, a, grid, st);
   PSR_SHAPES(PSR_L)
 #undef PSR_L
   return cudaErrorInvalidConfiguration;
@@ -674,10 +827,15 @@ cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalA
 
 template <int NW, int SPW, int R>
 static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
-  auto kern = psr_eval_kernel<NW, SPW, R>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, NW * 32, smem);
+  int n0 = 0, n1 = 0;
+  auto k0 = psr_eval_kernel<NW, SPW, R, false>;
+  auto k1 = psr_eval_kernel<NW, SPW, R, true>;
+  cudaError_t e = cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n0, k0, NW * 32, smem);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k1, NW * 32, smem);
+  *ctas_per_sm = n0 < n1 ? n0 : n1;
+  return e;
 }
 
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm) {

@@ -62,7 +62,7 @@ constexpr int kClsLong = 4;      // record classes: 0..3 = PSR_RX_* type in the 
 constexpr int kMaxWarps = 16;
 
 struct __attribute__((aligned(16))) ChunkHdr {  // 240 bytes
-  uint32_t n_rx, n_aux, n_eff, n_g;
+  uint32_t n_rx, n_aux, n_eff, rec_base;   // rec_base: mechanism-wide index of the chunk's first record (rate table row)
   uint32_t off_aux, off_eff, off_pool, off_gptr, off_gent;
   uint32_t bytes;         // bytes to copy (multiple of 16)
   // warp w evaluates the records wb[w][c] .. wb[w][c+1]-1 of class c (cost-balanced over warps at load
@@ -83,25 +83,39 @@ struct MechView {
   const double* Wm;             // [K] W
   const int32_t* sp_of;         // [nw*spw] species owned by (warp, slot) in the gather, -1 = none (nnz-balanced)
   const double* exp_tab;        // [32] 2^(j/32), one entry per lane (psr_math.cuh)
+  const int32_t* chunk_rec_base;  // [n_chunks + 1] mechanism-wide index of each chunk's first record
   int32_t K, I;
   int32_t n_chunks, rc;
   int32_t need_lnctot;          // some Troe reaction has no efficiency list (uses ln C_tot)
   int32_t resident;             // every chunk blob stays in shared memory (loaded once per CTA)
   int32_t n_cbuf;               // C-tile buffers: 2 = the next tile's state is prefetched during this tile's chunks
   uint32_t chunk_stride;        // bytes, multiple of 16
-  uint32_t smem_cs, smem_q, smem_mech, smem_misc, smem_total;  // byte offsets / sizes of the dynamic smem carve-up
+  uint32_t smem_cs, smem_q, smem_mech, smem_tab, smem_misc, smem_total;  // byte offsets / sizes of the dynamic smem carve-up
 };
 
 // what one launch produces
 enum : uint32_t {
-  kOutWdot = 1u, kOutQ = 2u, kOutKf = 4u, kOutKr = 8u, kOutF = 16u, kModeJac = 32u, kOutF0 = 64u
+  kOutWdot = 1u, kOutQ = 2u, kOutKf = 4u, kOutKr = 8u, kOutF = 16u, kOutF0 = 64u,
+  kModeJac = 32u,    // states are (reactor, column) pairs over all K+1 columns, every state a full evaluation
+  kModeJacT = 128u,  // states are the T columns only (one per reactor), full evaluation
+  kModeJacY = 256u,  // states are the Y columns, tiles aligned to reactors, T-only factors from the rate table
+  kOutTab = 512u     // also write the rate table (kRateVals doubles per reactor and reaction)
 };
+
+// Rate table written by the base-residual launch of psr_fd_jacobian and read by the Y-column launch:
+// the factors of a reaction that depend on T only, which a Y perturbation leaves unchanged.
+//   plain, three-body: k_f, k_r            Lindemann: k_inf, 1/K_c, k_0/k_inf
+//   Troe: ln k_0, 1/K_c, ln k_inf, ln F_cent
+// Row of reactor r, record index j (chunk order): tab[(r * I + j) * kRateVals ...].
+constexpr int kRateVals = 4;
 
 struct EvalArgs {
   int64_t N, ld, ldk;
   const double *T, *P, *Y, *Yin, *tau;
   double *wdot, *q, *kf, *kr, *F;
   double *J;              // Jacobian mode output
+  double* tab_out;        // kOutTab: rate table [N][I][kRateVals]
+  const double* tab;      // kModeJacY: the same table
   const double* F0;       // Jacobian mode: base residual [N][K+1]
   double* F0out;          // residual mode: also write [N][K+1] base residual (row 0 = 0)
   uint32_t flags;

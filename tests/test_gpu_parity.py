@@ -7,6 +7,7 @@ against the long-double oracle J*.
 """
 import copy
 import json
+import os
 from pathlib import Path
 
 import numpy as np
@@ -263,7 +264,7 @@ def test_C1_full_size_sampled(torch_cuda, binding):
 
 
 # ------------------------------------------------------------------ Jacobian (a10)
-@pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50)])
+@pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50), ("C2", 3)])
 def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     torch = torch_cuda
     mech, batch = synth.make_config(cfg, n)
@@ -271,10 +272,18 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
     J, F0 = gm.fd_jacobian(*args, want_F0=True)
     J2 = gm.fd_jacobian(*args)  # internal F0 scratch path
+    # diagnostic sweep in which every column is a full evaluation: the production sweep takes the T-only
+    # factors of the Y columns from the base state's rate table and must give the same bits
+    os.environ["PSR_JAC_UNHOISTED"] = "1"
+    try:
+        J3 = gm.fd_jacobian(*args)
+    finally:
+        del os.environ["PSR_JAC_UNHOISTED"]
     torch.cuda.synchronize()
-    J, F0, J2 = J.cpu().numpy(), F0.cpu().numpy(), J2.cpu().numpy()
+    J, F0, J2, J3 = J.cpu().numpy(), F0.cpu().numpy(), J2.cpu().numpy(), J3.cpu().numpy()
     gm.close()
     assert np.array_equal(J, J2)
+    assert np.array_equal(J, J3)
     om = oracle_mech(mech)
     jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=True)
     jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=False)
