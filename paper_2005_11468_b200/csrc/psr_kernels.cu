@@ -143,9 +143,32 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     }
   }
   const ExpTab etab = exp_tab_load(mv.exp_tab);
-  int sp[SPW];  // species this warp owns in the prologue, gather and epilogue
+  // Species this warp owns in the prologue, gather and epilogue.  Up to 4 per warp they and their
+  // accumulators live in registers across the chunks.  Beyond that (GA, K > 64) registers would spill:
+  // the slot loops are not unrolled, the species index is re-read, and the running sum of a species goes
+  // through the output array between chunks (L2-resident for the tile) instead of a register.
+  constexpr bool GA = SPW > 4;
+  constexpr int SPR = GA ? 1 : SPW;
+  int sp[SPR];
+  if constexpr (!GA) {
 #pragma unroll
-  for (int jj = 0; jj < SPW; ++jj) sp[jj] = mv.sp_of[w * SPW + jj];
+    for (int jj = 0; jj < SPW; ++jj) sp[jj] = mv.sp_of[w * SPW + jj];
+  }
+  auto for_species = [&](auto&& f) {
+    if constexpr (GA) {
+#pragma unroll 1
+      for (int jj = 0; jj < SPW; ++jj) {
+        const int s = __ldg(mv.sp_of + w * SPW + jj);
+        if (s >= 0) f(0, s);
+      }
+    } else {
+#pragma unroll
+      for (int jj = 0; jj < SPW; ++jj) {
+        const int s = sp[jj];
+        if (s >= 0) f(jj, s);
+      }
+    }
+  };
   if (w == 0) {
 #pragma unroll
     for (int i = 0; i < R; ++i) qs[mv.rc * TR + lane * R + i] = 0.0;
@@ -190,9 +213,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           cp_async8(tp + (buf * 2 + 0) * TR + col, a.T + r_);
           cp_async8(tp + (buf * 2 + 1) * TR + col, a.P + r_);
         }
-#pragma unroll
-        for (int jj = 0; jj < SPW; ++jj)
-          if (sp[jj] >= 0) cp_async8(Cs0 + buf * cs_elems + sp[jj] * TR + col, a.Y + (int64_t)sp[jj] * a.ld + r_);
+        for_species([&](int, int s) { cp_async8(Cs0 + buf * cs_elems + s * TR + col, a.Y + (int64_t)s * a.ld + r_); });
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -231,28 +252,24 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         state_of(tile, i, r_, jsp[i], valid_);
       }
       // x' = fl(x + delta), h = fl(x' - x) for the perturbed unknown of a Jacobian state (O11, g15)
-      double yv[SPW][R];
+      // pass 1: Y_i/W_i summed; a perturbed entry is replaced in the tile.  pass 2 (below) re-reads it.
       double sumYW[R];
 #pragma unroll
       for (int i = 0; i < R; ++i) sumYW[i] = 0.0;
-#pragma unroll
-      for (int jj = 0; jj < SPW; ++jj) {
-        const int s = sp[jj];
+      for_species([&](int, int s) {
+        const double iw = mv.invW[s];
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-          yv[jj][i] = 0.0;
-          if (s >= 0) {
-            double y = Cs[s * TR + lane * R + i];
-            if (s == jsp[i]) {
-              const double yp = y + 1e-8 * fmax(fabs(y), 1e-10);
-              hs[lane * R + i] = yp - y;
-              y = yp;
-            }
-            yv[jj][i] = y * mv.invW[s];
-            sumYW[i] += yv[jj][i];
+          double y = Cs[s * TR + lane * R + i];
+          if (s == jsp[i]) {
+            const double yp = y + 1e-8 * fmax(fabs(y), 1e-10);
+            hs[lane * R + i] = yp - y;
+            Cs[s * TR + lane * R + i] = yp;
+            y = yp;
           }
+          sumYW[i] += y * iw;
         }
-      }
+      });
 #pragma unroll
       for (int i = 0; i < R; ++i) part[w * TR + lane * R + i] = sumYW[i];
       if (w == 0) {
@@ -288,14 +305,11 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           if (mv.need_lnctot) lnctot_s[lane * R + i] = log(ct);   // Troe reactions without efficiencies
         }
       }
+      for_species([&](int, int s) {
+        const double iw = mv.invW[s];
 #pragma unroll
-      for (int jj = 0; jj < SPW; ++jj) {
-        const int s = sp[jj];
-        if (s >= 0) {
-#pragma unroll
-          for (int i = 0; i < R; ++i) Cs[s * TR + lane * R + i] = rho[i] * yv[jj][i];
-        }
-      }
+        for (int i = 0; i < R; ++i) Cs[s * TR + lane * R + i] = rho[i] * (Cs[s * TR + lane * R + i] * iw);
+      });
     }
     __syncthreads();
     double lnT[R], invT[R];
@@ -305,9 +319,9 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       invT[i] = 1.0 / T[i];
     }
 
-    double acc[SPW][R];
+    double acc[SPR][R];
 #pragma unroll
-    for (int jj = 0; jj < SPW; ++jj)
+    for (int jj = 0; jj < SPR; ++jj)
 #pragma unroll
       for (int i = 0; i < R; ++i) acc[jj][i] = 0.0;
 
@@ -319,53 +333,101 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     const ChunkHdr* hdr = nullptr;
     // gather (a8, Eq. 4) of the chunk in `stage`: every warp sums the rows of nu^T it owns in a fixed
     // order; afterwards the stage is handed back to the bulk-copy ring
-    auto gather_and_release = [&]() {
+    // adds the chunk's rows of nu^T q for species s to a0, in the fixed order of the gather lists
+    auto sum_rows = [&](const uint32_t* gptr, const uint4* gent, int s, double (&a0)[R]) {
+      const uint32_t g0 = gptr[2 * s] >> 2, g1 = gptr[2 * s + 1] >> 2, g2 = gptr[2 * s + 2] >> 2;
+      double a1[R];
+#pragma unroll
+      for (int i = 0; i < R; ++i) a1[i] = 0.0;
+#pragma unroll 1
+      for (uint32_t e = g0; e < g1; ++e) {
+        const uint4 o = gent[e];
+        double v0[R], v1[R], v2[R], v3[R];
+        RowIO<R>::ld(q_lane + o.x, v0);
+        RowIO<R>::ld(q_lane + o.y, v1);
+        RowIO<R>::ld(q_lane + o.z, v2);
+        RowIO<R>::ld(q_lane + o.w, v3);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          a0[i] += v0[i];
+          a1[i] += v1[i];
+          a0[i] += v2[i];
+          a1[i] += v3[i];
+        }
+      }
+#pragma unroll 1
+      for (uint32_t e = g1; e < g2; ++e) {
+        const uint4 o = gent[e];
+        double v0[R], v1[R], v2[R], v3[R];
+        RowIO<R>::ld(q_lane + o.x, v0);
+        RowIO<R>::ld(q_lane + o.y, v1);
+        RowIO<R>::ld(q_lane + o.z, v2);
+        RowIO<R>::ld(q_lane + o.w, v3);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          a0[i] -= v0[i];
+          a1[i] -= v1[i];
+          a0[i] -= v2[i];
+          a1[i] -= v3[i];
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < R; ++i) a0[i] += a1[i];
+    };
+    // GA: where the running sum of (species s, state i of this lane) rests between chunks, and the
+    // outputs of that entry once the last chunk is in (same arithmetic as the epilogue below)
+    auto ga_slot = [&](int s, int64_t r_, int jsp_) -> double* {
+      if (jac) return a.J + ((int64_t)r_ * n + (jsp_ + 1)) * n + 1 + s;
+      if (a.flags & kOutWdot) return a.wdot + (int64_t)s * a.ld + r_;
+      if (a.flags & kOutF) return a.F + (int64_t)s * a.ld + r_;
+      return a.F0out + r_ * n + 1 + s;
+    };
+    auto ga_finish = [&](int s, int i, int64_t r_, int jsp_, double accv) {
+      const int64_t o = (int64_t)s * a.ld + r_;
+      if (!jac) {
+        if (a.flags & kOutWdot) a.wdot[o] = accv;
+        if (wantF) {
+          const double invtau = 1.0 / ldg_nc(a.tau + r_);
+          const double invrho = 1.0 / rho_s[lane * R + i];
+          const double Fv = fma(ldg_nc(a.Y + o) - ldg_nc(a.Yin + o), invtau, -(accv * (mv.Wm[s] * invrho)));
+          if (a.flags & kOutF) a.F[o] = Fv;
+          if (a.flags & kOutF0) a.F0out[r_ * n + 1 + s] = Fv;
+        }
+      } else {
+        const double invtau = 1.0 / ldg_nc(a.tau + r_);
+        const double invrho = 1.0 / rho_s[lane * R + i];
+        const double invh = 1.0 / hs[lane * R + i];
+        double y = ldg_nc(a.Y + o);
+        if (s == jsp_) y = y + 1e-8 * fmax(fabs(y), 1e-10);   // the same x' as in the prologue
+        const double Fv = fma(y - ldg_nc(a.Yin + o), invtau, -(accv * (mv.Wm[s] * invrho)));
+        *ga_slot(s, r_, jsp_) = (Fv - ldg_nc(a.F0 + r_ * n + 1 + s)) * invh;
+      }
+    };
+    auto gather_and_release = [&](bool first, bool last) {
       if (jac || (a.flags & (kOutWdot | kOutF | kOutF0))) {
         const uint32_t* gptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_gptr);
         const uint4* gent = reinterpret_cast<const uint4*>(blob + hdr->off_gent);
+        if constexpr (GA) {
+          int64_t r_[R];
+          int jsp_[R];
+          bool valid_[R];
 #pragma unroll
-        for (int jj = 0; jj < SPW; ++jj) {
-          const int s = sp[jj];
-          if (s >= 0) {
-            const uint32_t g0 = gptr[2 * s] >> 2, g1 = gptr[2 * s + 1] >> 2, g2 = gptr[2 * s + 2] >> 2;
-            double a1[R];
+          for (int i = 0; i < R; ++i) state_of(tile, i, r_[i], jsp_[i], valid_[i]);
+          for_species([&](int, int s) {
+            double a0[R];
 #pragma unroll
-            for (int i = 0; i < R; ++i) a1[i] = 0.0;
-#pragma unroll 1
-            for (uint32_t e = g0; e < g1; ++e) {
-              const uint4 o = gent[e];
-              double v0[R], v1[R], v2[R], v3[R];
-              RowIO<R>::ld(q_lane + o.x, v0);
-              RowIO<R>::ld(q_lane + o.y, v1);
-              RowIO<R>::ld(q_lane + o.z, v2);
-              RowIO<R>::ld(q_lane + o.w, v3);
+            for (int i = 0; i < R; ++i) a0[i] = (first || !valid_[i]) ? 0.0 : *ga_slot(s, r_[i], jsp_[i]);
+            sum_rows(gptr, gent, s, a0);
 #pragma unroll
-              for (int i = 0; i < R; ++i) {
-                acc[jj][i] += v0[i];
-                a1[i] += v1[i];
-                acc[jj][i] += v2[i];
-                a1[i] += v3[i];
+            for (int i = 0; i < R; ++i) {
+              if (valid_[i]) {
+                if (last) ga_finish(s, i, r_[i], jsp_[i], a0[i]);
+                else *ga_slot(s, r_[i], jsp_[i]) = a0[i];
               }
             }
-#pragma unroll 1
-            for (uint32_t e = g1; e < g2; ++e) {
-              const uint4 o = gent[e];
-              double v0[R], v1[R], v2[R], v3[R];
-              RowIO<R>::ld(q_lane + o.x, v0);
-              RowIO<R>::ld(q_lane + o.y, v1);
-              RowIO<R>::ld(q_lane + o.z, v2);
-              RowIO<R>::ld(q_lane + o.w, v3);
-#pragma unroll
-              for (int i = 0; i < R; ++i) {
-                acc[jj][i] -= v0[i];
-                a1[i] -= v1[i];
-                acc[jj][i] -= v2[i];
-                a1[i] -= v3[i];
-              }
-            }
-#pragma unroll
-            for (int i = 0; i < R; ++i) acc[jj][i] += a1[i];
-          }
+          });
+        } else {
+          for_species([&](int jj, int s) { sum_rows(gptr, gent, s, acc[jj]); });
         }
       }
       __syncthreads();
@@ -697,11 +759,11 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         if (threadIdx.x == 0 && nt < a.n_tiles) load_tab(nt, more_chunks ? c + 1 : 0);
       }
 
-      if (c + 1 < mv.n_chunks) gather_and_release();
+      if (c + 1 < mv.n_chunks) gather_and_release(c == 0, false);
     }
 
     // operands of the epilogue are requested now so that they arrive during the last gather
-    double e_tau[R], e_y[SPW][R], e_yin[SPW][R], e_f0[SPW][R];
+    double e_tau[R], e_y[SPR][R], e_yin[SPR][R], e_f0[SPR][R];
     int64_t r[R];
     int jsp[R];
     bool valid[R];
@@ -711,23 +773,32 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
         for (int i = 0; i < R; ++i) {
           e_tau[i] = ldg_nc(a.tau + r[i]);
-#pragma unroll
-          for (int jj = 0; jj < SPW; ++jj) {
-            const int s = sp[jj];
-            if (s >= 0) {
+          if constexpr (!GA) {
+            for_species([&](int jj, int s) {
               const int64_t o = (int64_t)s * a.ld + r[i];
               e_y[jj][i] = ldg_nc(a.Y + o);
               e_yin[jj][i] = ldg_nc(a.Yin + o);
               if (jac) e_f0[jj][i] = ldg_nc(a.F0 + r[i] * n + 1 + s);
-            }
+            });
           }
         }
       }
 
-    gather_and_release();
+    gather_and_release(mv.n_chunks == 1, true);
 
     // ---------------------------------------------------------------- epilogue (a8 store, a9, a10)
-    if (!jac) {
+    if constexpr (GA) {
+      // every (species, state) entry left with the last gather; what remains is row 0 of the unknowns
+      if (w == 0) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          if (valid[i]) {
+            if (jac) a.J[((int64_t)r[i] * n + (jsp[i] + 1)) * n] = (jsp[i] == -1) ? 1.0 : 0.0;   // F_T = T - T_set
+            else if (a.flags & kOutF0) a.F0out[r[i] * n] = 0.0;
+          }
+        }
+      }
+    } else if (!jac) {
 #pragma unroll
       for (int i = 0; i < R; ++i) {
         if (valid[i]) {
