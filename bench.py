@@ -43,7 +43,7 @@ N_SM, FP64_LANES_PER_SM = 148, 64     # B200: 64 FP64 FMA lanes per SM (37 TFLOP
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of psr_eval_kernel<16,4,1> on C1, from the
 # ncu --set full capture summarised in profiles/.
-NCU_DRAM_BYTES_PER_LAUNCH = 77.6e6   # 59.5 MB read + 18.1 MB written (profiles/r1b_psr_eval_kernel_C1.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 74.8e6   # 59.3 MB read + 15.5 MB written (profiles/r1c_psr_eval_kernel_C1.md)
 
 
 def algorithmic_fp64_instr(K, I, n_tb, n_troe, nnz):
