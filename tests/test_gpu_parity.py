@@ -263,6 +263,61 @@ def test_C1_full_size_sampled(torch_cuda, binding):
     assert np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0)) <= 1e-12
 
 
+@pytest.mark.parametrize("cfg,n_sample", [("C2", 96), ("C3", 48)])
+def test_large_configs_full_size_sampled(torch_cuda, binding, cfg, n_sample):
+    """BASELINE configs 2 and 3 at their full batches through psr_eval_residual (the launches bench.py
+    times under `extra`): sampled reactors against the oracle, invariants over the whole output."""
+    torch = torch_cuda
+    mech, batch = synth.make_config(cfg)
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    F, wdot = gm.eval_residual(*args, want_wdot=True)
+    F, wdot = F.cpu().numpy(), wdot.cpu().numpy()
+    gm.close()
+    rng = np.random.default_rng(11)
+    idx = np.sort(rng.choice(batch.n, size=n_sample, replace=False))
+    idx[0], idx[-1] = 0, batch.n - 1
+    sub = batch.take(idx)
+    ref = orc.evaluate(oracle_mech(mech), sub.T, sub.P, sub.Y, sub.Yin, sub.tau, want=("wdot", "F"))
+    werr, mask = wdot_masked_rel_err(wdot[:, idx], ref["wdot"])
+    assert mask.any() and werr.max() <= TOL_K
+    assert residual_rel_err(F[:, idx], ref["F"]).max() <= TOL_F
+    assert np.all(np.isfinite(wdot)) and np.all(np.isfinite(F))
+    ww = mech.W[:, None] * wdot
+    assert np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0)) <= 1e-12
+    # sum_i F_i = (sum Y - sum Y_in)/tau - sum_i wdot_i W_i / rho, and the last sum vanishes (mass conservation)
+    lhs = F.sum(axis=0)
+    rhs = (batch.Y.sum(axis=0) - batch.Yin.sum(axis=0)) / batch.tau
+    scale = np.abs(F).sum(axis=0)
+    assert np.median(np.abs(lhs - rhs) / scale) <= 1e-12
+
+
+def test_C4_full_size_jacobian_sampled(torch_cuda, binding):
+    """BASELINE config 4 at its full 8,192 reactors (the psr_fd_jacobian launch sequence bench.py times,
+    two sub-batches): sampled reactors by the floor criterion against the long-double oracle, structural
+    invariants over every Jacobian."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C4")
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    J = gm.fd_jacobian(*args).cpu().numpy()
+    gm.close()
+    assert np.all(np.isfinite(J))
+    assert np.all(J[:, 0, 0] == 1.0) and np.all(J[:, 1:, 0] == 0.0)          # row 0 = e_0 (g13)
+    # species rows of a Y column sum to 1/tau, of the T column to 0 (mass conservation), up to FD noise
+    col_sums = J[:, :, 1:].sum(axis=2)
+    scale = np.abs(J[:, :, 1:]).sum(axis=2)
+    assert np.median(np.abs(col_sums[:, 1:] - 1.0 / batch.tau[:, None]) / scale[:, 1:]) <= 1e-6
+    assert np.median(np.abs(col_sums[:, 0]) / scale[:, 0]) <= 1e-6
+    rng = np.random.default_rng(13)
+    idx = np.sort(rng.choice(batch.n, size=24, replace=False))
+    idx[0], idx[-1] = 0, batch.n - 1          # first and last reactor; the sample spans both sub-batches
+    sub = batch.take(idx)
+    jl = orc.jacobian(oracle_mech(mech), sub.T, sub.P, sub.Y, sub.Yin, sub.tau, long_double=True)
+    worst, fr_T, fr_Y = jacobian_floor_ratio(J[idx], jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y)
+
+
 # ------------------------------------------------------------------ Jacobian (a10)
 @pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50), ("C2", 3)])
 def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
