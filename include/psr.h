@@ -99,7 +99,14 @@ psr_status psr_eval_residual(const psr_mech* mech, int64_t N, const double* T, c
  * h_j = fl(x'_j - x_j), J_ij = (F_i(x') - F_i(x))/h_j.  Row 0 is the fixed-temperature equation
  * F_T = T - T_set with T_set the input T, so row 0 of J is e_0.
  * J: [N][(K+1)*(K+1)], column-major per reactor (entry (i,j) of reactor r at J[r*n*n + j*n + i],
- * n = K+1), directly usable by a batched LU.  F0: [N][K+1] residual at x (row 0 = 0), may be NULL. */
+ * n = K+1), directly usable by a batched LU.  F0: [N][K+1] residual at x (row 0 = 0), may be NULL.
+ * Enqueues, per sub-batch of reactors, three launches on `stream`: the base residual (which also
+ * tabulates the reaction factors that depend on T only), the T column, and the K species columns
+ * (which reuse those factors: a Y perturbation leaves them unchanged; the result is bit-identical to
+ * evaluating every column in full).  The rate table (and F0 when NULL is passed) live in a scratch
+ * buffer owned by `mech`, grown on demand with a stream synchronisation the first time a larger N is
+ * seen: calls of psr_fd_jacobian on ONE mechanism handle must therefore not run concurrently on
+ * different streams.  PSR_ENOMEM if the scratch buffer cannot be allocated. */
 psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, const double* P,
                            const double* Y, const double* Yin, const double* tau, int64_t ld,
                            double* J, double* F0, void* stream);
