@@ -68,9 +68,9 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 double reaction_cost(int type) {  // relative FP64 cost used to balance warps inside a chunk
   switch (type) {
-    case PSR_RX_THREE_BODY: return 2.1;   // executed instructions relative to a plain reaction (ncu, C1)
-    case PSR_RX_LINDEMANN: return 2.5;
-    case PSR_RX_TROE: return 4.7;
+    case PSR_RX_THREE_BODY: return 1.5;   // executed instructions relative to a plain reaction (ncu, C1)
+    case PSR_RX_LINDEMANN: return 2.0;
+    case PSR_RX_TROE: return 3.8;
     default: return 1.0;
   }
 }
@@ -261,6 +261,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   for (int c = 0; c < n_chunks; ++c) {
     auto& cr = chunk_rx[c];  // cost-descending
     std::vector<double> load(nw, 0.0);
+    load[0] = 2.0;   // warp 0 also forms ln T, rho, C_tot of the tile (about two plain reactions' worth)
     std::vector<std::vector<int>> mine(nw);
     for (int k : cr) {
       const int wmin = (int)(std::min_element(load.begin(), load.end()) - load.begin());
