@@ -354,6 +354,43 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     assert residual_rel_err(F0[:, 1:].T, jd["F0"][:, 1:].T).max() <= TOL_F
 
 
+# ------------------------------------------------------------------ streams and graphs
+def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, binding):
+    """Every evaluation call only enqueues work on the caller's stream (psr.h), so a Newton iteration
+    (residual + Jacobian) can be captured once in a CUDA graph and replayed on new states."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C1", 200)
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y, Yin, tau = (dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    n = mech.n_species + 1
+    F, w = torch.empty_like(Y), torch.empty_like(Y)
+    J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
+    gm.fd_jacobian(T, P, Y, Yin, tau, J=J)            # sizes the scratch buffer outside the capture
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w)
+            gm.fd_jacobian(T, P, Y, Yin, tau, J=J)
+    # new state in the same buffers, replay, compare with direct calls on the default stream
+    _, b2 = synth.make_config("C4", 200)
+    for dst, src in ((T, b2.T), (P, b2.P), (Y, b2.Y), (Yin, b2.Yin), (tau, b2.tau)):
+        dst.copy_(dev(torch, src))
+    F.zero_(); w.zero_(); J.zero_()
+    torch.cuda.synchronize()
+    graph.replay()
+    torch.cuda.synchronize()
+    F_g, w_g, J_g = F.clone(), w.clone(), J.clone()
+    F_d, w_d = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+    J_d = gm.fd_jacobian(T, P, Y, Yin, tau)
+    torch.cuda.synchronize()
+    gm.close()
+    assert torch.equal(F_g, F_d) and torch.equal(w_g, w_d) and torch.equal(J_g, J_d)
+    ref = orc.evaluate(oracle_mech(mech), b2.T, b2.P, b2.Y, b2.Yin, b2.tau, want=("wdot", "F"))
+    assert residual_rel_err(F_g.cpu().numpy(), ref["F"]).max() <= TOL_F
+
+
 # ------------------------------------------------------------------ kernel math
 def test_table_exp_accuracy(torch_cuda, binding):
     """csrc/psr_math.cuh exp_fast against mpmath (50 digits): <= 4e-16 relative over the argument
