@@ -99,6 +99,21 @@ def evaluate(mech: OracleMechanism, T, P, Y, Yin=None, tau=None, *, want=("kf", 
     return {k: v for k, v in out.items() if v is not None}
 
 
+def evaluate_energy(mech: OracleMechanism, T, P, Y, Tin, Yin, tau, *, long_double: bool = False,
+                    nthreads: int = 0) -> dict:
+    """Adiabatic PSR residual (energy row NEXT-1 + species rows O10).  Returns F [K][N], FT [N], wdot [K][N]."""
+    arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (T, P, Y, Tin, Yin, tau)]
+    T, P, Y, Tin, Yin, tau = arrs
+    N = T.shape[0]
+    assert Y.shape == (mech.K, N) and Yin.shape == (mech.K, N) and Tin.shape == (N,)
+    F, wdot, FT = np.empty((mech.K, N)), np.empty((mech.K, N)), np.empty(N)
+    rc = lib().oracle_eval_energy(C.byref(mech.c), C.c_int64(N), _p(T), _p(P), _p(Y), _p(Tin), _p(Yin), _p(tau),
+                                  C.c_int64(N), _p(F), _p(FT), _p(wdot), C.c_int(int(long_double)), C.c_int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"oracle_eval_energy failed rc={rc}")
+    return dict(F=F, FT=FT, wdot=wdot)
+
+
 def jacobian(mech: OracleMechanism, T, P, Y, Yin, tau, *, long_double: bool = False, nthreads: int = 0) -> dict:
     """O11. Returns J [N][K+1][K+1] indexed J[r, col, row] (column-major per reactor), F0, S, H: [N][K+1]."""
     T = np.ascontiguousarray(T, dtype=np.float64)

@@ -21,6 +21,8 @@
 //   k_f/k_r = K_c; sum_k W_k wdot_k = 0 on element-balanced mechanisms; Lindemann limits
 //   k->k0[M], k->k_inf; Troe F=F_cent at log10 Pr=-c; sum_i F_i = (sum Y - sum Y_in)/tau;
 //   Jacobian species rows of a Y column sum to 1/tau; J row 0 = e_0.
+//   Energy row (NEXT-1): T3 values of h_i, C_p,mix and F_T from SURVEY.md 8(c), re-derived with mpmath;
+//   F_T = 0 for an inert mechanism at T_in = T; linearity in 1/tau; enthalpy-balance identity.
 //
 // Units (paper silent; CHEMKIN cgs, reading g4): T [K], P [dyn/cm^2], C [mol/cm^3],
 // rho [g/cm^3], W [g/mol], wdot [mol/cm^3/s], Ea [cal/mol].
@@ -184,6 +186,63 @@ void eval_one(const oracle_mech& m, R T, R P, const R* Y, const R* Yin, R tau, R
   if (rho_out) *rho_out = rho;
 }
 
+// Energy row: the steady form of Eq. 3 with Qdot = 0 and dP/dt = 0,
+//   C_p,mix dT/dt = (mdot / rho V) sum_i Y_i,in (h_i,in - h_i) - (sum_i h_i wdot_i W_i) / rho,
+// written as the residual F_T = -dT/dt with mdot/(rho V) = 1/tau.  h_i [erg/g] =
+// (h/RT)_i R T / W_i at the reactor temperature, h_i,in the same at the inlet temperature T_in,
+// C_p,mix = sum_i Y_i (cp/R)_i R / W_i  [erg/g/K]; NASA-7 fits as in O2.
+template <class R>
+R energy_row(const oracle_mech& m, R T, R Tin, const R* Y, const R* Yin, R tau, const R* wdot, R rho) {
+  const int K = m.n_species;
+  const R Rg = Consts<R>::Rgas;
+  R inflow = 0, reaction = 0, cp_mix = 0;
+  for (int i = 0; i < K; ++i) {
+    R cp_R, h_RT, s_R, cpin_R, hin_RT, sin_R;
+    nasa7<R>(m.nasa + 7 * i, T, cp_R, h_RT, s_R);
+    nasa7<R>(m.nasa + 7 * i, Tin, cpin_R, hin_RT, sin_R);
+    const R W = (R)m.W[i];
+    const R h = h_RT * Rg * T / W;
+    const R hin = hin_RT * Rg * Tin / W;
+    inflow += Yin[i] * (hin - h);
+    reaction += h * wdot[i] * W;
+    cp_mix += Y[i] * cp_R * Rg / W;
+  }
+  const R dTdt = (inflow / tau - reaction / rho) / cp_mix;
+  return -dTdt;
+}
+
+// Batch form of the adiabatic residual: species rows F [K][ld] as O10 and F_T [N] from energy_row.
+template <class R>
+int energy_batch(const oracle_mech& m, int64_t N, const double* T, const double* P, const double* Y,
+                 const double* Tin, const double* Yin, const double* tau, int64_t ld, double* F, double* FT,
+                 double* wdot, int nthreads) {
+  const int K = m.n_species;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+#endif
+  {
+    std::vector<R> y(K), yin(K), ow(K), oF(K + 1);
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+    for (int64_t r = 0; r < N; ++r) {
+      for (int i = 0; i < K; ++i) {
+        y[i] = Y[(int64_t)i * ld + r];
+        yin[i] = Yin[(int64_t)i * ld + r];
+      }
+      R rho;
+      eval_one<R>(m, (R)T[r], (R)P[r], y.data(), yin.data(), (R)tau[r], (R)T[r], nullptr, nullptr, nullptr,
+                  ow.data(), oF.data(), nullptr, nullptr, &rho);
+      const R ft = energy_row<R>(m, (R)T[r], (R)Tin[r], y.data(), yin.data(), (R)tau[r], ow.data(), rho);
+      if (F) for (int i = 0; i < K; ++i) F[(int64_t)i * ld + r] = (double)oF[1 + i];
+      if (FT) FT[r] = (double)ft;
+      if (wdot) for (int i = 0; i < K; ++i) wdot[(int64_t)i * ld + r] = (double)ow[i];
+    }
+  }
+  return 0;
+}
+
 template <class R>
 int eval_batch(const oracle_mech& m, int64_t N, const double* T, const double* P, const double* Y,
                const double* Yin, const double* tau, int64_t ld, double* kf, double* kr, double* q,
@@ -303,6 +362,14 @@ int oracle_eval(const oracle_mech* m, int64_t N, const double* T, const double* 
   if (use_long_double)
     return eval_batch<long double>(*m, N, T, P, Y, Yin, tau, ld, kf, kr, q, ldk, wdot, F, nthreads);
   return eval_batch<double>(*m, N, T, P, Y, Yin, tau, ld, kf, kr, q, ldk, wdot, F, nthreads);
+}
+
+// Adiabatic PSR residual: F [K][ld] (species rows, O10), FT [N] (energy row), wdot [K][ld]; any may be null.
+int oracle_eval_energy(const oracle_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                       const double* Tin, const double* Yin, const double* tau, int64_t ld, double* F, double* FT,
+                       double* wdot, int use_long_double, int nthreads) {
+  if (use_long_double) return energy_batch<long double>(*m, N, T, P, Y, Tin, Yin, tau, ld, F, FT, wdot, nthreads);
+  return energy_batch<double>(*m, N, T, P, Y, Tin, Yin, tau, ld, F, FT, wdot, nthreads);
 }
 
 // J: [N][(K+1)*(K+1)] column-major per reactor; F0, S, H: [N][K+1] (may be null).

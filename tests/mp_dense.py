@@ -25,9 +25,10 @@ def dense_nu(mech):
     return nup, nupp
 
 
-def evaluate(mech, T, P, Y, Yin=None, tau=None, Tset=None, lindemann_only=False, M_scale=None):
+def evaluate(mech, T, P, Y, Yin=None, tau=None, Tset=None, lindemann_only=False, M_scale=None, Tin=None):
     """Returns dict with mp values: Wbar, rho, C, Ctot, per-reaction kinf,k0,Pr,Fcent,F,M,Kp,Kc,kf,kr,q,
-    wdot, F (K+1 entries, row 0 = T - Tset)."""
+    wdot, F (K+1 entries, row 0 = T - Tset).  With Tin: also h (erg/g), cp_mix and the energy row F_T
+    (steady Eq. 3 of the paper, Qdot = 0, dP/dt = 0, as a residual: F_T = -dT/dt)."""
     K, I = mech.n_species, mech.n_reactions
     T, P = mpf(T), mpf(P)
     Y = [mpf(float(y)) for y in Y]
@@ -88,4 +89,16 @@ def evaluate(mech, T, P, Y, Yin=None, tau=None, Tset=None, lindemann_only=False,
         tau = mpf(float(tau))
         Tset = T if Tset is None else mpf(Tset)
         out["F"] = [T - Tset] + [(Y[i] - Yin[i]) / tau - wdot[i] * W[i] / rho for i in range(K)]
+        if Tin is not None:
+            Tin = mpf(Tin)
+            h, hin, cp = [], [], []
+            for i in range(K):
+                a = [mpf(float(v)) for v in mech.nasa[i]]
+                enth = lambda t: (a[0] + a[1] * t / 2 + a[2] * t**2 / 3 + a[3] * t**3 / 4 + a[4] * t**4 / 5 + a[5] / t) * RGAS * t / W[i]
+                h.append(enth(T))
+                hin.append(enth(Tin))
+                cp.append((a[0] + a[1] * T + a[2] * T**2 + a[3] * T**3 + a[4] * T**4) * RGAS / W[i])
+            cp_mix = sum(Y[i] * cp[i] for i in range(K))
+            rhs = sum(Yin[i] * (hin[i] - h[i]) for i in range(K)) / tau - sum(h[i] * wdot[i] * W[i] for i in range(K)) / rho
+            out.update(h=h, cp_mix=cp_mix, FT=-rhs / cp_mix)
     return out

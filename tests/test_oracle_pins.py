@@ -421,3 +421,60 @@ def test_O11_linear_part_exact():
         tol = 4 * EPS * (np.abs(batch.Y[:, r] - batch.Yin[:, r]) / batch.tau[r])[:, None] / j["H"][r][None, 1:]
         assert np.all(np.abs(Jr[1:, 1:] - expect[1:, 1:]) <= tol + 1e-9 * expect[1:, 1:])
         assert np.all(Jr[1:, 0] == 0.0) and np.all(Jr[0] == expect[0])
+
+
+# ------------------------------------------------------------------ energy row
+def test_energy_row_T3_golden_rederived_and_matched(t3):
+    """Steady Eq. 3 as the residual F_T = -dT/dt: the T3 values printed in SURVEY.md 8(c)
+    re-derived with mpmath, then the oracle against them."""
+    mech, batch, om = t3
+    g = GOLD["energy_Tin300"]
+    m = mp_dense.evaluate(mech, batch.T[0], batch.P[0], batch.Y[:, 0], batch.Yin[:, 0], batch.tau[0], Tin=300.0)
+    for i in range(3):
+        assert close(m["h"][i], g["h_erg_per_g"][i], 1e-15)
+    assert close(m["cp_mix"], g["cp_mix"], 1e-15) and close(m["FT"], g["F_T"], 1e-15)
+    out = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.array([300.0]), batch.Yin, batch.tau)
+    assert close(out["FT"][0], g["F_T"], 1e-12)
+    for i in range(3):
+        assert close(out["F"][i, 0], GOLD["F"][1 + i], 1e-12)          # species rows unchanged (O10)
+
+
+def test_energy_row_vanishes_without_inflow_enthalpy_difference_or_reaction():
+    """With every rate constant negligible (A -> 1e-300) and T_in = T the energy row is 0; with T_in != T it
+    is the pure inflow term -(1/tau) sum Y_in (h_in - h) / cp_mix, linear in 1/tau."""
+    mech, batch = synth.make_config("C0", 4)
+    mech.A[:] = 1e-300
+    om = oracle_mech(mech)
+    same = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, batch.T, batch.Yin, batch.tau)
+    assert np.all(np.abs(same["FT"]) <= 1e-250)
+    Tin = np.full(4, 300.0)
+    a = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, Tin, batch.Yin, batch.tau)
+    b = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, Tin, batch.Yin, 2.0 * batch.tau)
+    assert np.allclose(a["FT"], 2.0 * b["FT"], rtol=1e-13, atol=0)
+    for r in range(4):
+        hin = np.array([orc.nasa7(mech.nasa[i], 300.0)[1] * RGAS * 300.0 / mech.W[i] for i in range(mech.n_species)])
+        h = np.array([orc.nasa7(mech.nasa[i], batch.T[r])[1] * RGAS * batch.T[r] / mech.W[i] for i in range(mech.n_species)])
+        cp = sum(batch.Y[i, r] * orc.nasa7(mech.nasa[i], batch.T[r])[0] * RGAS / mech.W[i] for i in range(mech.n_species))
+        expect = -(batch.Yin[:, r] @ (hin - h)) / batch.tau[r] / cp
+        assert close(a["FT"][r], expect, 1e-12)
+
+
+@pytest.mark.parametrize("cfg,n", [("C0", 3), ("C1", 1)])
+def test_energy_row_brute_force_mpmath(cfg, n):
+    """Whole adiabatic residual on generated mechanisms against the dense 50-digit evaluation."""
+    mech, batch = synth.make_config(cfg, n)
+    om = oracle_mech(mech)
+    Tin = np.linspace(300.0, 600.0, n)
+    out = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, Tin, batch.Yin, batch.tau)
+    for r in range(n):
+        m = mp_dense.evaluate(mech, batch.T[r], batch.P[r], batch.Y[:, r], batch.Yin[:, r], batch.tau[r], Tin=Tin[r])
+        # the energy row is a difference of large terms: compare on the scale of its parts
+        scale = max(abs(float(m["FT"])), 1e-12 * float(sum(abs(x) for x in m["h"])) / float(m["cp_mix"]) / float(batch.tau[r]))
+        assert abs(out["FT"][r] - float(m["FT"])) <= 1e-10 * scale
+
+
+def test_energy_row_long_double_agrees_with_double(t3):
+    mech, batch, om = t3
+    d = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.array([300.0]), batch.Yin, batch.tau)
+    l = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.array([300.0]), batch.Yin, batch.tau, long_double=True)
+    assert close(d["FT"][0], l["FT"][0], 1e-13)
