@@ -335,9 +335,19 @@ def _time_call(torch, fn, flush, reps=5):
 
 
 def run_extras(binding, synth, torch, flush):
-    """C2, C3 residual passes and the C4 FD-Jacobian, timed once each (mean of 5, L2 flushed)."""
+    """C2, C3 residual passes, the C4 FD-Jacobian and the C1 adiabatic residual, timed once each (mean of
+    5, L2 flushed)."""
     out = {}
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    # NEXT-1: the adiabatic residual (species rows + energy row) on the headline workload
+    mech, batch = synth.make_config("C1")
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    Tin = torch.full_like(T, 300.0)
+    F, FT = torch.empty_like(Y), torch.empty_like(T)
+    ms = _time_call(torch, lambda: gm.eval_residual_energy(T, P, Y, Tin, Yin, tau, F=F, FT=FT), flush)
+    out["C1_energy"] = {"call": "psr_eval_residual_energy", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3)}
+    gm.close()
     for cfg in ("C2", "C3", "C4"):
         mech, batch = synth.make_config(cfg)
         gm = binding.Mechanism.from_synth(mech)

@@ -94,6 +94,16 @@ psr_status psr_eval_residual(const psr_mech* mech, int64_t N, const double* T, c
                              const double* Y, const double* Yin, const double* tau, int64_t ld,
                              double* F, double* wdot, void* stream);
 
+/* Adiabatic PSR residual: the species rows F [K][ld] exactly as psr_eval_residual,
+ * plus the energy row FT [N], the steady form of the paper's Eq. 3 with Qdot = 0 and
+ * dP/dt = 0 written as a residual,
+ *   F_T = -[ (1/tau) sum_i Yin_i (h_i(Tin) - h_i(T)) - (sum_i h_i(T) wdot_i W_i)/rho ] / cp_mix,
+ * h_i [erg/g] = (h/RT)_i R T / W_i and cp_mix = sum_i Y_i (cp/R)_i R / W_i from the NASA-7 fits of the
+ * mechanism.  Tin [N]: inlet temperature [K].  wdot [K][ld] may be NULL.  F_T is in K/s. */
+psr_status psr_eval_residual_energy(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                                    const double* Y, const double* Tin, const double* Yin, const double* tau,
+                                    int64_t ld, double* F, double* FT, double* wdot, void* stream);
+
 /* Forward finite-difference Jacobian of the residual in x = (T, Y_1..Y_K) (
  * BASELINE.json configs[4]): delta_j = 1e-8 max(|x_j|, 1e-10), x'_j = fl(x_j + delta_j),
  * h_j = fl(x'_j - x_j), J_ij = (F_i(x') - F_i(x))/h_j.  Row 0 is the fixed-temperature equation

@@ -17,7 +17,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_fd_jacobian", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -64,6 +64,8 @@ def lib():
         L.psr_eval_wdot.restype = C.c_int
         L.psr_eval_residual.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_eval_residual.restype = C.c_int
+        L.psr_eval_residual_energy.argtypes = [vp, i64, dp, dp, dp, dp, dp, dp, i64, dp, dp, dp, vp]
+        L.psr_eval_residual_energy.restype = C.c_int
         L.psr_fd_jacobian.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_fd_jacobian.restype = C.c_int
         L.psr_last_error.argtypes = []
@@ -210,6 +212,25 @@ class Mechanism:
         _check(lib().psr_eval_residual(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(F),
                                        _ptr(wdot), _stream()))
         return (F, wdot) if wdot is not None else F
+
+    # --- psr_eval_residual_energy
+    def eval_residual_energy(self, T, P, Y, Tin, Yin, tau, F=None, FT=None, wdot=None, want_wdot=False):
+        import torch
+        N = T.shape[0]
+        ld = _ld(Y, N)
+        for nm, t in (("T", T), ("P", P), ("Y", Y), ("Tin", Tin), ("Yin", Yin), ("tau", tau)):
+            _chk_dev(nm, t)
+        if _ld(Yin, N) != ld:
+            raise ValueError("Yin must share the leading dimension of Y")
+        if F is None:
+            F = torch.empty_like(Y)
+        if FT is None:
+            FT = torch.empty_like(T)
+        if wdot is None and want_wdot:
+            wdot = torch.empty_like(Y)
+        _check(lib().psr_eval_residual_energy(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Tin), _ptr(Yin), _ptr(tau),
+                                              ld, _ptr(F), _ptr(FT), _ptr(wdot), _stream()))
+        return (F, FT, wdot) if wdot is not None else (F, FT)
 
     # --- psr_fd_jacobian
     def fd_jacobian(self, T, P, Y, Yin, tau, J=None, F0=None, want_F0=False):

@@ -34,6 +34,7 @@ struct psr_mech {
   unsigned char* d_chunks = nullptr;
   double* d_invW = nullptr;
   double* d_W = nullptr;
+  double* d_nasa = nullptr;
   double* d_exptab = nullptr;
   int32_t* d_sp_of = nullptr;
   int32_t* d_rec_base = nullptr;  // [n_chunks + 1]
@@ -400,7 +401,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   stride = align_up(stride, 128);
   // all chunk blobs resident in shared memory (loaded once per CTA) when they fit, else a 2-stage ring
   // q tile plus the rate-table slice of one chunk (Y-column launch of psr_fd_jacobian)
-  const size_t q_bytes = align_up((size_t)(rc + 1) * kTile * rl * 8, 128) + align_up((size_t)rc * kRateVals * 8, 128);
+  // (the q tile also hosts the 3 x nw partial-sum rows of the energy row, hence the lower bound)
+  const size_t q_bytes = align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128) + align_up((size_t)rc * kRateVals * 8, 128);
   resident = n_chunks <= kMaxStages && smem_fixed + q_bytes + stride * n_chunks <= (size_t)prop.sharedMemPerBlockOptin &&
              (n_chunks == 1 || stride * n_chunks <= 48 * 1024);
   const size_t need = smem_fixed + q_bytes + stride * (resident ? n_chunks : 2);
@@ -435,7 +437,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     v.smem_cs = (uint32_t)o;
     o += n_cbuf * cbuf_bytes;
     v.smem_q = (uint32_t)o;
-    o += align_up((size_t)(rc + 1) * kTile * rl * 8, 128);  // + the all-zero row
+    o += align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128);  // + the all-zero row; >= energy-row scratch
     v.smem_mech = (uint32_t)o;
     o += stride * (resident ? n_chunks : 2);
     v.smem_tab = (uint32_t)o;
@@ -461,9 +463,11 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   if ((e = cudaMalloc(&m->d_chunks, all.size())) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
   if ((e = cudaMalloc(&m->d_invW, 8 * K)) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
   if ((e = cudaMalloc(&m->d_W, 8 * K)) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+  if ((e = cudaMalloc(&m->d_nasa, 8 * 7 * (size_t)K)) != cudaSuccess) { cleanup(); return fail(PSR_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
   if ((e = cudaMemcpy(m->d_chunks, all.data(), all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMemcpy(m->d_invW, invW.data(), 8 * K, cudaMemcpyHostToDevice)) != cudaSuccess ||
-      (e = cudaMemcpy(m->d_W, d->W, 8 * K, cudaMemcpyHostToDevice)) != cudaSuccess) {
+      (e = cudaMemcpy(m->d_W, d->W, 8 * K, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_nasa, d->nasa, 8 * 7 * (size_t)K, cudaMemcpyHostToDevice)) != cudaSuccess) {
     cleanup();
     return cuda_fail(e, "cudaMemcpy (mechanism upload)");
   }
@@ -492,6 +496,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.chunks = m->d_chunks;
   v.invW = m->d_invW;
   v.Wm = m->d_W;
+  v.nasa = m->d_nasa;
   if ((e = occupancy_eval(nw, spw, rl, v.smem_total, &m->ctas_per_sm)) != cudaSuccess || m->ctas_per_sm < 1) {
     cleanup();
     return fail(PSR_ECUDA, "kernel does not fit on this device (%s)", cudaGetErrorString(e));
@@ -505,6 +510,7 @@ void psr_mech_free(psr_mech* m) {
   cudaFree(m->d_chunks);
   cudaFree(m->d_invW);
   cudaFree(m->d_W);
+  cudaFree(m->d_nasa);
   cudaFree(m->d_exptab);
   cudaFree(m->d_sp_of);
   cudaFree(m->d_rec_base);
@@ -594,6 +600,20 @@ psr_status psr_eval_residual(const psr_mech* m, int64_t N, const double* T, cons
   a.flags = kOutF | (wdot ? kOutWdot : 0u);
   a.n_tiles = (N + m->tile - 1) / m->tile;
   return run(m, a, stream, "psr_eval_residual");
+}
+
+psr_status psr_eval_residual_energy(const psr_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                                    const double* Tin, const double* Yin, const double* tau, int64_t ld, double* F,
+                                    double* FT, double* wdot, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(m, N, T, P, Y, ld, "psr_eval_residual_energy");
+  if (st != PSR_OK || N == 0) return st;
+  if (!Tin || !Yin || !tau || !F || !FT) return fail(PSR_EINVAL, "psr_eval_residual_energy: null Tin, Yin, tau, F or FT");
+  EvalArgs a{};
+  a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Tin = Tin; a.Yin = Yin; a.tau = tau; a.F = F; a.FT = FT; a.wdot = wdot;
+  a.flags = kOutF | kOutFT | (wdot ? kOutWdot : 0u);
+  a.n_tiles = (N + m->tile - 1) / m->tile;
+  return run(m, a, stream, "psr_eval_residual_energy");
 }
 
 psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const double* P, const double* Y,

@@ -99,8 +99,13 @@ struct RowIO<2> {
 // JY: the Y-column launch of psr_fd_jacobian (kModeJacY) -- tiles are aligned to reactors (the 32 lanes of
 // a tile are 32 Y columns of ONE reactor) and the T-only factors of every reaction come from the rate
 // table that the base-residual launch wrote, as warp-uniform broadcasts, instead of being recomputed.
-template <int NW, int SPW, int R, bool JY>
+// EN: psr_eval_residual_energy -- the epilogue also forms the energy row (kOutFT).  Its own instantiation so
+// that the extra registers and code stay out of the other calls (measured: 2.7 % on C1 when shared).
+constexpr int kVarPlain = 0, kVarJacY = 1, kVarEnergy = 2;
+template <int NW, int SPW, int R, int VAR>
 __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const MechView mv, const EvalArgs a) {
+  constexpr bool JY = VAR == kVarJacY;
+  constexpr bool EN = VAR == kVarEnergy;
   static_assert(!JY || R == 1, "the Y-column mode maps one column to a lane");
   constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
@@ -116,6 +121,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   double* tp = lnctot_s + TR;                                         // [2][2][TR]: prefetched T, P
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [kMaxStages] chunk stages, [kMaxStages] rate table
   double* tab_s = reinterpret_cast<double*>(smem + mv.smem_tab);      // [rc][kRateVals]: this reactor's slice (JY)
+  double* en_s = qs;   // [3][NW][TR]: partial sums of the energy row (the q tile is free after the last gather)
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -374,6 +380,28 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
       for (int i = 0; i < R; ++i) a0[i] += a1[i];
     };
+    // Energy row (steady Eq. 3): this thread's share of  sum Yin_i (h_i(Tin) - h_i(T)),
+    // sum h_i wdot_i W_i  and  sum Y_i cp_i  over the species it owns; h [erg/g] = (h/RT) R T / W (NASA-7).
+    double en[3][R];
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int i = 0; i < R; ++i) en[k][i] = 0.0;
+    auto energy_terms = [&](int s, int i, double Tin_, double y, double yin, double wd) {
+      if constexpr (!EN) return;
+      const double* c = mv.nasa + 7 * s;
+      const double a0 = c[0], a1 = c[1], a2 = c[2], a3 = c[3], a4 = c[4], a5 = c[5];
+      const double RoW = kRgas * mv.invW[s];
+      auto h_of = [&](double t) {
+        const double hRT = fma(fma(fma(fma(a4 * 0.2, t, a3 * 0.25), t, a2 * (1.0 / 3.0)), t, a1 * 0.5), t, a0) + a5 / t;
+        return hRT * RoW * t;
+      };
+      const double h = h_of(T[i]);
+      const double cp = fma(fma(fma(fma(a4, T[i], a3), T[i], a2), T[i], a1), T[i], a0) * RoW;
+      en[0][i] = fma(yin, h_of(Tin_) - h, en[0][i]);
+      en[1][i] = fma(h * wd, mv.Wm[s], en[1][i]);
+      en[2][i] = fma(y, cp, en[2][i]);
+    };
     // GA: where the running sum of (species s, state i of this lane) rests between chunks, and the
     // outputs of that entry once the last chunk is in (same arithmetic as the epilogue below)
     auto ga_slot = [&](int s, int64_t r_, int jsp_) -> double* {
@@ -392,6 +420,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           const double Fv = fma(ldg_nc(a.Y + o) - ldg_nc(a.Yin + o), invtau, -(accv * (mv.Wm[s] * invrho)));
           if (a.flags & kOutF) a.F[o] = Fv;
           if (a.flags & kOutF0) a.F0out[r_ * n + 1 + s] = Fv;
+          if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r_), ldg_nc(a.Y + o), ldg_nc(a.Yin + o), accv);
         }
       } else {
         const double invtau = 1.0 / ldg_nc(a.tau + r_);
@@ -814,6 +843,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                 const double Fv = fma(e_y[jj][i] - e_yin[jj][i], invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
                 if (a.flags & kOutF) a.F[o] = Fv;
                 if (a.flags & kOutF0) a.F0out[r[i] * n + 1 + s] = Fv;
+                if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), e_y[jj][i], e_yin[jj][i], acc[jj][i]);
               }
             }
           }
@@ -870,6 +900,35 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       }
       __syncthreads();
     }
+    if constexpr (EN) {
+      // the three sums over all species: per-warp shares through shared memory, added in warp order
+#pragma unroll
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int i = 0; i < R; ++i) en_s[(k * NW + w) * TR + lane * R + i] = en[k][i];
+      __syncthreads();
+      if (w == 0) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+          if (valid[i]) {
+            double e[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+              e[k] = 0.0;
+#pragma unroll
+              for (int ww = 0; ww < NW; ++ww) e[k] += en_s[(k * NW + ww) * TR + lane * R + i];
+            }
+            const double dTdt = (e[0] / ldg_nc(a.tau + r[i]) - e[1] / rho_s[lane * R + i]) / e[2];
+            a.FT[r[i]] = -dTdt;
+          }
+        }
+      }
+      __syncthreads();
+      if (w == 0) {   // the partial sums may have covered the q tile's zero row
+#pragma unroll
+        for (int i = 0; i < R; ++i) qs[mv.rc * TR + lane * R + i] = 0.0;
+      }
+    }
     if (mv.n_cbuf == 1) prefetch(tile + gridDim.x, 0);   // single C buffer: it is free only now
   }
 }
@@ -877,9 +936,9 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 // ------------------------------------------------------------------ launch wrapper
 #define PSR_SHAPES(X) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)
 
-template <int NW, int SPW, int R, bool JY>
+template <int NW, int SPW, int R, int VAR>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  auto kern = psr_eval_kernel<NW, SPW, R, JY>;
+  auto kern = psr_eval_kernel<NW, SPW, R, VAR>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mv.smem_total);
   if (e != cudaSuccess) return e;
   kern<<<grid, NW * 32, mv.smem_total, st>>>(mv, a);
@@ -887,10 +946,13 @@ static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cud
 }
 
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  const bool jy = (a.flags & kModeJacY) != 0;
-#define PSR_L(NW_, SPW_) \
-  if (nw == NW_ && spw == SPW_ && rl == 1) \
-    return jy ? launch_t<NW_, SPW_, 1, true>(mv, a, grid, st) : launch_t<NW_, SPW_, 1, false>(mv, a, grid, st);
+  const int var = (a.flags & kModeJacY) ? kVarJacY : (a.flags & kOutFT) ? kVarEnergy : kVarPlain;
+#define PSR_L(NW_, SPW_)                                                                        \
+  if (nw == NW_ && spw == SPW_ && rl == 1) {                                                    \
+    if (var == kVarJacY) return launch_t<NW_, SPW_, 1, kVarJacY>(mv, a, grid, st);              \
+    if (var == kVarEnergy) return launch_t<NW_, SPW_, 1, kVarEnergy>(mv, a, grid, st);          \
+    return launch_t<NW_, SPW_, 1, kVarPlain>(mv, a, grid, st);                                  \
+  }
   PSR_SHAPES(PSR_L)
 #undef PSR_L
   return cudaErrorInvalidConfiguration;
@@ -898,14 +960,17 @@ cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalA
 
 template <int NW, int SPW, int R>
 static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
-  int n0 = 0, n1 = 0;
-  auto k0 = psr_eval_kernel<NW, SPW, R, false>;
-  auto k1 = psr_eval_kernel<NW, SPW, R, true>;
+  int n0 = 0, n1 = 0, n2 = 0;
+  auto k0 = psr_eval_kernel<NW, SPW, R, kVarPlain>;
+  auto k1 = psr_eval_kernel<NW, SPW, R, kVarJacY>;
+  auto k2 = psr_eval_kernel<NW, SPW, R, kVarEnergy>;
   cudaError_t e = cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n0, k0, NW * 32, smem);
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k1, NW * 32, smem);
-  *ctas_per_sm = n0 < n1 ? n0 : n1;
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n2, k2, NW * 32, smem);
+  *ctas_per_sm = n0 < n1 ? (n0 < n2 ? n0 : n2) : (n1 < n2 ? n1 : n2);
   return e;
 }
 

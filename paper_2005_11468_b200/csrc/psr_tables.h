@@ -81,6 +81,7 @@ struct MechView {
   const unsigned char* chunks;  // n_chunks blobs, chunk_stride bytes apart
   const double* invW;           // [K] 1/W
   const double* Wm;             // [K] W
+  const double* nasa;           // [K][7] NASA-7 coefficients a0..a6 (energy row only)
   const int32_t* sp_of;         // [nw*spw] species owned by (warp, slot) in the gather, -1 = none (nnz-balanced)
   const double* exp_tab;        // [32] 2^(j/32), one entry per lane (psr_math.cuh)
   const int32_t* chunk_rec_base;  // [n_chunks + 1] mechanism-wide index of each chunk's first record
@@ -99,7 +100,8 @@ enum : uint32_t {
   kModeJac = 32u,    // states are (reactor, column) pairs over all K+1 columns, every state a full evaluation
   kModeJacT = 128u,  // states are the T columns only (one per reactor), full evaluation
   kModeJacY = 256u,  // states are the Y columns, tiles aligned to reactors, T-only factors from the rate table
-  kOutTab = 512u     // also write the rate table (kRateVals doubles per reactor and reaction)
+  kOutTab = 512u,    // also write the rate table (kRateVals doubles per reactor and reaction)
+  kOutFT = 1024u     // also write the energy row F_T [N] (needs Tin)
 };
 
 // Rate table written by the base-residual launch of psr_fd_jacobian and read by the Y-column launch:
@@ -112,6 +114,8 @@ constexpr int kRateVals = 4;
 struct EvalArgs {
   int64_t N, ld, ldk;
   const double *T, *P, *Y, *Yin, *tau;
+  const double* Tin;      // kOutFT: inlet temperature [N]
+  double* FT;             // kOutFT: energy row [N]
   double *wdot, *q, *kf, *kr, *F;
   double *J;              // Jacobian mode output
   double* tab_out;        // kOutTab: rate table [N][I][kRateVals]

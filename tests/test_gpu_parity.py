@@ -354,6 +354,57 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     assert residual_rel_err(F0[:, 1:].T, jd["F0"][:, 1:].T).max() <= TOL_F
 
 
+# ------------------------------------------------------------------ energy row (NEXT-1)
+def energy_scale(mech, batch, Tin, wdot_ref, rho):
+    """Sum of the absolute terms of the energy row, per reactor: the row is a difference of large numbers,
+    so its error is judged relative to max(|F_T|, 1e-3 of this scale)."""
+    K, N = mech.n_species, batch.n
+    S = np.zeros(N)
+    cp_mix = np.zeros(N)
+    for r in range(N):
+        for i in range(K):
+            cp_R, h_RT, _ = orc.nasa7(mech.nasa[i], float(batch.T[r]))
+            _, hin_RT, _ = orc.nasa7(mech.nasa[i], float(Tin[r]))
+            h = h_RT * 8.31446261815324e7 * batch.T[r] / mech.W[i]
+            hin = hin_RT * 8.31446261815324e7 * Tin[r] / mech.W[i]
+            S[r] += abs(batch.Yin[i, r] * (hin - h)) / batch.tau[r] + abs(h * wdot_ref[i, r] * mech.W[i]) / rho[r]
+            cp_mix[r] += batch.Y[i, r] * cp_R * 8.31446261815324e7 / mech.W[i]
+    return S / cp_mix
+
+
+@pytest.mark.parametrize("cfg,n", [("C0", 100), ("C1", 333), ("C2", 70)])
+def test_energy_residual_against_oracle(torch_cuda, binding, cfg, n):
+    torch = torch_cuda
+    mech, batch = synth.make_config(cfg, n)
+    Tin = np.random.default_rng(3).uniform(300.0, 700.0, n)
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, Tin, batch.Yin, batch.tau)]
+    F, FT, wdot = gm.eval_residual_energy(*args, want_wdot=True)
+    F2 = gm.eval_residual(args[0], args[1], args[2], args[4], args[5])
+    torch.cuda.synchronize()
+    F, FT, wdot, F2 = F.cpu().numpy(), FT.cpu().numpy(), wdot.cpu().numpy(), F2.cpu().numpy()
+    gm.close()
+    ref = orc.evaluate_energy(oracle_mech(mech), batch.T, batch.P, batch.Y, Tin, batch.Yin, batch.tau)
+    assert np.array_equal(F, F2)                                       # species rows: the same path
+    assert residual_rel_err(F, ref["F"]).max() <= TOL_F
+    rho = batch.P / (8.31446261815324e7 * batch.T * (batch.Y / mech.W[:, None]).sum(axis=0))
+    S = energy_scale(mech, batch, Tin, ref["wdot"], rho)
+    err = np.abs(FT - ref["FT"]) / np.maximum(np.abs(ref["FT"]), 1e-3 * S)
+    assert err.max() <= TOL_F, err.max()
+
+
+def test_energy_residual_T3_golden(torch_cuda, binding):
+    torch = torch_cuda
+    gold = json.loads((Path(__file__).parent / "golden" / "t3_pins.json").read_text())["energy_Tin300"]
+    mech, batch = synth.toy_t3()
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, np.array([300.0]), batch.Yin, batch.tau)]
+    _, FT = gm.eval_residual_energy(*args)
+    torch.cuda.synchronize()
+    assert abs(float(FT[0]) - gold["F_T"]) <= 1e-9 * abs(gold["F_T"])
+    gm.close()
+
+
 # ------------------------------------------------------------------ streams and graphs
 def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, binding):
     """Every evaluation call only enqueues work on the caller's stream (psr.h), so a Newton iteration
