@@ -114,8 +114,9 @@ def evaluate_energy(mech: OracleMechanism, T, P, Y, Tin, Yin, tau, *, long_doubl
     return dict(F=F, FT=FT, wdot=wdot)
 
 
-def jacobian(mech: OracleMechanism, T, P, Y, Yin, tau, *, long_double: bool = False, nthreads: int = 0) -> dict:
-    """O11. Returns J [N][K+1][K+1] indexed J[r, col, row] (column-major per reactor), F0, S, H: [N][K+1]."""
+def jacobian(mech: OracleMechanism, T, P, Y, Yin, tau, *, Tin=None, long_double: bool = False, nthreads: int = 0) -> dict:
+    """O11. Returns J [N][K+1][K+1] indexed J[r, col, row] (column-major per reactor), F0, S, H: [N][K+1].
+    With Tin [N]: row 0 of the residual is the energy row (NEXT-1) instead of T - T_set."""
     T = np.ascontiguousarray(T, dtype=np.float64)
     P = np.ascontiguousarray(P, dtype=np.float64)
     Y = np.ascontiguousarray(Y, dtype=np.float64)
@@ -124,8 +125,14 @@ def jacobian(mech: OracleMechanism, T, P, Y, Yin, tau, *, long_double: bool = Fa
     N, n = T.shape[0], mech.K + 1
     J = np.empty((N, n, n))
     F0, S, H = np.empty((N, n)), np.empty((N, n)), np.empty((N, n))
-    rc = lib().oracle_jacobian(C.byref(mech.c), C.c_int64(N), _p(T), _p(P), _p(Y), _p(Yin), _p(tau), C.c_int64(N),
-                               _p(J), _p(F0), _p(S), _p(H), C.c_int(int(long_double)), C.c_int(nthreads))
+    if Tin is not None:
+        Tin = np.ascontiguousarray(Tin, dtype=np.float64)
+        rc = lib().oracle_jacobian_energy(C.byref(mech.c), C.c_int64(N), _p(T), _p(P), _p(Y), _p(Tin), _p(Yin), _p(tau),
+                                          C.c_int64(N), _p(J), _p(F0), _p(S), _p(H), C.c_int(int(long_double)),
+                                          C.c_int(nthreads))
+    else:
+        rc = lib().oracle_jacobian(C.byref(mech.c), C.c_int64(N), _p(T), _p(P), _p(Y), _p(Yin), _p(tau), C.c_int64(N),
+                                   _p(J), _p(F0), _p(S), _p(H), C.c_int(int(long_double)), C.c_int(nthreads))
     if rc != 0:
         raise RuntimeError(f"oracle_jacobian failed rc={rc}")
     return dict(J=J, F0=F0, S=S, H=H)

@@ -284,8 +284,8 @@ int eval_batch(const oracle_mech& m, int64_t N, const double* T, const double* P
 // of 8(c)-J, row 0 = |T|... row 0 is exact (S_0 = 0).
 template <class R>
 int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P, const double* Y,
-              const double* Yin, const double* tau, int64_t ld, double* J, double* F0, double* S,
-              double* H, int nthreads) {
+              const double* Tin /* null: row 0 is T - T_set; else the energy row */, const double* Yin,
+              const double* tau, int64_t ld, double* J, double* F0, double* S, double* H, int nthreads) {
   const int K = m.n_species, I = m.n_reactions, n = K + 1;
 #ifdef _OPENMP
   if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -293,7 +293,7 @@ int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P,
 #endif
   {
     std::vector<double> x(n), xp(n);
-    std::vector<R> y(K), yin(K), f0(n), f1(n), okf(I), okr(I), C(K);
+    std::vector<R> y(K), yin(K), f0(n), f1(n), okf(I), okr(I), C(K), ow(K);
 #ifdef _OPENMP
 #pragma omp for schedule(static)
 #endif
@@ -307,7 +307,8 @@ int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P,
       const R Tset = (R)T[r];
       R rho;
       eval_one<R>(m, (R)x[0], (R)P[r], y.data(), yin.data(), (R)tau[r], Tset, okf.data(), okr.data(),
-                  nullptr, nullptr, f0.data(), nullptr, C.data(), &rho);
+                  nullptr, ow.data(), f0.data(), nullptr, C.data(), &rho);
+      if (Tin) f0[0] = energy_row<R>(m, (R)x[0], (R)Tin[r], y.data(), yin.data(), (R)tau[r], ow.data(), rho);
       double* Jr = J + (int64_t)r * n * n;
       if (F0) for (int i = 0; i < n; ++i) F0[(int64_t)r * n + i] = (double)f0[i];
       if (S) {
@@ -330,6 +331,21 @@ int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P,
         }
         for (int i = 0; i < K; ++i)
           Sr[1 + i] = (double)(std::fabs((double)((y[i] - yin[i]) / (R)tau[r])) + (R)m.W[i] / rho * acc[i]);
+        if (Tin) {
+          // round-off scale of the energy row: its terms in absolute value, the reaction part through the
+          // same |nu| (|kf prod| + |kr prod|) sums as the species rows
+          R st = 0, cp_mix = 0;
+          for (int i = 0; i < K; ++i) {
+            R cp_R, h_RT, s_R, cpin_R, hin_RT, sin_R;
+            nasa7<R>(m.nasa + 7 * i, (R)x[0], cp_R, h_RT, s_R);
+            nasa7<R>(m.nasa + 7 * i, (R)Tin[r], cpin_R, hin_RT, sin_R);
+            const R W = (R)m.W[i];
+            const R h = h_RT * Consts<R>::Rgas * (R)x[0] / W, hin = hin_RT * Consts<R>::Rgas * (R)Tin[r] / W;
+            st += std::fabs((double)(yin[i] * (hin - h))) / (R)tau[r] + std::fabs((double)h) * W / rho * acc[i];
+            cp_mix += y[i] * cp_R * Consts<R>::Rgas / W;
+          }
+          Sr[0] = (double)(st / cp_mix);
+        }
       }
       for (int j = 0; j < n; ++j) {
         double ax = std::fabs(x[j]);
@@ -340,8 +356,10 @@ int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P,
         xp[j] = xpj;
         if (H) H[(int64_t)r * n + j] = hj;
         for (int i = 0; i < K; ++i) y[i] = (R)xp[1 + i];
+        R rho1;
         eval_one<R>(m, (R)xp[0], (R)P[r], y.data(), yin.data(), (R)tau[r], Tset, nullptr, nullptr, nullptr,
-                    nullptr, f1.data(), nullptr, nullptr, nullptr);
+                    ow.data(), f1.data(), nullptr, nullptr, &rho1);
+        if (Tin) f1[0] = energy_row<R>(m, (R)xp[0], (R)Tin[r], y.data(), yin.data(), (R)tau[r], ow.data(), rho1);
         for (int i = 0; i < n; ++i) Jr[(int64_t)j * n + i] = (double)((f1[i] - f0[i]) / (R)hj);
       }
       for (int i = 0; i < K; ++i) y[i] = (R)x[1 + i];
@@ -376,8 +394,16 @@ int oracle_eval_energy(const oracle_mech* m, int64_t N, const double* T, const d
 int oracle_jacobian(const oracle_mech* m, int64_t N, const double* T, const double* P, const double* Y,
                     const double* Yin, const double* tau, int64_t ld, double* J, double* F0, double* S,
                     double* H, int use_long_double, int nthreads) {
-  if (use_long_double) return jac_batch<long double>(*m, N, T, P, Y, Yin, tau, ld, J, F0, S, H, nthreads);
-  return jac_batch<double>(*m, N, T, P, Y, Yin, tau, ld, J, F0, S, H, nthreads);
+  if (use_long_double) return jac_batch<long double>(*m, N, T, P, Y, nullptr, Yin, tau, ld, J, F0, S, H, nthreads);
+  return jac_batch<double>(*m, N, T, P, Y, nullptr, Yin, tau, ld, J, F0, S, H, nthreads);
+}
+
+// The same with the energy row (NEXT-1) as row 0 of the residual: the adiabatic PSR system.
+int oracle_jacobian_energy(const oracle_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                           const double* Tin, const double* Yin, const double* tau, int64_t ld, double* J, double* F0,
+                           double* S, double* H, int use_long_double, int nthreads) {
+  if (use_long_double) return jac_batch<long double>(*m, N, T, P, Y, Tin, Yin, tau, ld, J, F0, S, H, nthreads);
+  return jac_batch<double>(*m, N, T, P, Y, Tin, Yin, tau, ld, J, F0, S, H, nthreads);
 }
 
 // Single-reactor detail for the pins: per reaction 11 doubles

@@ -478,3 +478,40 @@ def test_energy_row_long_double_agrees_with_double(t3):
     d = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.array([300.0]), batch.Yin, batch.tau)
     l = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.array([300.0]), batch.Yin, batch.tau, long_double=True)
     assert close(d["FT"][0], l["FT"][0], 1e-13)
+
+
+def test_energy_jacobian_row0_against_exact_quotients_and_species_rows_unchanged(t3):
+    """Adiabatic Jacobian on T3: row 0 (energy row) of every column against the exact difference quotient
+    from 50-digit arithmetic with the double-precision step h_j (g15), inside the round-off floor of the
+    method; rows 1..K are the species rows of the fixed-temperature Jacobian, bit for bit."""
+    mech, batch, om = t3
+    Tin = np.array([300.0])
+    jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin, long_double=True)
+    jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin)
+    j0 = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau)
+    assert np.array_equal(jd["J"][:, :, 1:], j0["J"][:, :, 1:])
+    assert close(jd["F0"][0, 0], GOLD["energy_Tin300"]["F_T"], 1e-12)
+    x = np.concatenate([batch.T, batch.Y[:, 0]])
+    base = mp_dense.evaluate(mech, x[0], batch.P[0], x[1:], batch.Yin[:, 0], batch.tau[0], Tin=300.0)
+    for j in range(4):
+        delta = 1e-8 * max(abs(x[j]), 1e-10)
+        xp = x.copy()
+        xp[j] = x[j] + delta
+        h = xp[j] - x[j]
+        assert jl["H"][0, j] == h
+        pert = mp_dense.evaluate(mech, xp[0], batch.P[0], xp[1:], batch.Yin[:, 0], batch.tau[0], Tin=300.0)
+        exact = float((pert["FT"] - base["FT"]) / mpf(float(h)))
+        floor = EPS * jl["S"][0, 0] / h
+        assert abs(jl["J"][0, j, 0] - exact) <= 1e-9 * abs(exact) + 1.0 * floor, j      # 80-bit: well inside
+        assert abs(jd["J"][0, j, 0] - exact) <= 1e-9 * abs(exact) + (1024.0 if j == 0 else 32.0) * floor, j
+
+
+def test_energy_jacobian_double_within_floor_of_long_double_C4():
+    mech, batch = synth.make_config("C4", 6)
+    om = oracle_mech(mech)
+    Tin = np.linspace(300.0, 650.0, 6)
+    jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin, long_double=True)
+    jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin)
+    worst, fr_T, fr_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y)
+    assert np.all(jl["S"][:, 0] > 0)
