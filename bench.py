@@ -361,6 +361,9 @@ def run_extras(binding, synth, torch, flush):
             n = mech.n_species + 1
             J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
             ms = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J), flush)
+            Tin = torch.full_like(T, 300.0)
+            ms_en = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J, Tin=Tin), flush)
+            out["C4_energy"] = {"call": "psr_fd_jacobian_energy", "ms": ms_en, "jacobians_per_s": batch.n / (ms_en * 1e-3)}
             out[cfg] = {"call": "psr_fd_jacobian", "ms": ms, "jacobians_per_s": batch.n / (ms * 1e-3),
                         "residual_evals_per_s": batch.n * (n + 1) / (ms * 1e-3),
                         "alu_frac_unhoisted": instr * batch.n * (n + 1) / (ms * 1e-3) / (N_SM * FP64_LANES_PER_SM * 1.965e9)}

@@ -121,6 +121,14 @@ psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, con
                            const double* Y, const double* Yin, const double* tau, int64_t ld,
                            double* J, double* F0, void* stream);
 
+/* The same sweep for the adiabatic system (NEXT-1): row 0 of the residual is the energy row F_T of
+ * psr_eval_residual_energy instead of T - T_set, so row 0 of J is dF_T/dx_j by the same forward
+ * differences and F0[r][0] = F_T.  Tin [N]: inlet temperature.  Rows 1..K are bit-identical to
+ * psr_fd_jacobian's. */
+psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                                  const double* Y, const double* Tin, const double* Yin, const double* tau,
+                                  int64_t ld, double* J, double* F0, void* stream);
+
 /* Thread-local description of the last failure on this thread; valid until its next psr_* call. */
 const char* psr_last_error(void);
 

@@ -17,7 +17,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -66,6 +66,8 @@ def lib():
         L.psr_eval_residual.restype = C.c_int
         L.psr_eval_residual_energy.argtypes = [vp, i64, dp, dp, dp, dp, dp, dp, i64, dp, dp, dp, vp]
         L.psr_eval_residual_energy.restype = C.c_int
+        L.psr_fd_jacobian_energy.argtypes = [vp, i64, dp, dp, dp, dp, dp, dp, i64, dp, dp, vp]
+        L.psr_fd_jacobian_energy.restype = C.c_int
         L.psr_fd_jacobian.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_fd_jacobian.restype = C.c_int
         L.psr_last_error.argtypes = []
@@ -233,19 +235,24 @@ class Mechanism:
         return (F, FT, wdot) if wdot is not None else (F, FT)
 
     # --- psr_fd_jacobian
-    def fd_jacobian(self, T, P, Y, Yin, tau, J=None, F0=None, want_F0=False):
+    def fd_jacobian(self, T, P, Y, Yin, tau, J=None, F0=None, want_F0=False, Tin=None):
+        """Tin given: psr_fd_jacobian_energy (row 0 = energy row), else psr_fd_jacobian (row 0 = T - T_set)."""
         import torch
         N = T.shape[0]
         ld = _ld(Y, N)
         n = self.K + 1
-        for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)):
+        for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)) + ((("Tin", Tin),) if Tin is not None else ()):
             _chk_dev(nm, t)
         if J is None:
             J = torch.empty((N, n, n), dtype=torch.float64, device=T.device)  # J[r, col, row]
         if F0 is None and want_F0:
             F0 = torch.empty((N, n), dtype=torch.float64, device=T.device)
-        _check(lib().psr_fd_jacobian(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(J),
-                                     _ptr(F0), _stream()))
+        if Tin is not None:
+            _check(lib().psr_fd_jacobian_energy(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Tin), _ptr(Yin), _ptr(tau),
+                                                ld, _ptr(J), _ptr(F0), _stream()))
+        else:
+            _check(lib().psr_fd_jacobian(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(J),
+                                         _ptr(F0), _stream()))
         return (J, F0) if F0 is not None else J
 
 

@@ -616,12 +616,19 @@ psr_status psr_eval_residual_energy(const psr_mech* m, int64_t N, const double* 
   return run(m, a, stream, "psr_eval_residual_energy");
 }
 
-psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const double* P, const double* Y,
-                           const double* Yin, const double* tau, int64_t ld, double* J, double* F0, void* stream) {
+}  // extern "C"
+
+namespace {
+
+// psr_fd_jacobian (Tin == nullptr: row 0 is T - T_set) and psr_fd_jacobian_energy (row 0 is the energy row)
+psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, const double* P, const double* Y,
+                            const double* Tin, const double* Yin, const double* tau, int64_t ld, double* J, double* F0,
+                            void* stream, const char* fn) {
   g_err.clear();
-  psr_status st = check_common(mc, N, T, P, Y, ld, "psr_fd_jacobian");
+  psr_status st = check_common(mc, N, T, P, Y, ld, fn);
   if (st != PSR_OK || N == 0) return st;
-  if (!Yin || !tau || !J) return fail(PSR_EINVAL, "psr_fd_jacobian: null Yin, tau or J");
+  if (!Yin || !tau || !J) return fail(PSR_EINVAL, "%s: null Yin, tau or J", fn);
+  const uint32_t en = Tin ? kOutFT : 0u;
   psr_mech* m = const_cast<psr_mech*>(mc);
   const int64_t K = m->view.K, n = K + 1, I = m->view.I;
 
@@ -656,7 +663,8 @@ psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const
     a.N = nb; a.ld = ld; a.T = T + r0; a.P = P + r0; a.Y = Y + r0; a.Yin = Yin + r0; a.tau = tau + r0;
     a.F0out = F0 + r0 * n;
     a.tab_out = tab;
-    a.flags = kOutF0 | (unhoisted ? 0u : kOutTab);
+    a.Tin = Tin ? Tin + r0 : nullptr;
+    a.flags = kOutF0 | en | (unhoisted ? 0u : kOutTab);
     a.n_tiles = (nb + m->tile - 1) / m->tile;
     st = run(m, a, stream, "psr_fd_jacobian (base residual)");
     if (st != PSR_OK) return st;
@@ -664,24 +672,44 @@ psr_status psr_fd_jacobian(const psr_mech* mc, int64_t N, const double* T, const
     b.N = nb; b.ld = ld; b.T = a.T; b.P = a.P; b.Y = a.Y; b.Yin = a.Yin; b.tau = a.tau;
     b.J = J + r0 * n * n;
     b.F0 = a.F0out;
+    b.Tin = a.Tin;
     if (unhoisted) {
-      b.flags = kModeJac;
+      b.flags = kModeJac | en;
       b.n_tiles = (nb * n + m->tile - 1) / m->tile;
       st = run(m, b, stream, "psr_fd_jacobian (all columns)");
       if (st != PSR_OK) return st;
       continue;
     }
-    b.flags = kModeJacT;                       // column 0: T perturbed, every factor changes
+    b.flags = kModeJacT | en;                  // column 0: T perturbed, every factor changes
     b.n_tiles = (nb + m->tile - 1) / m->tile;
     st = run(m, b, stream, "psr_fd_jacobian (T column)");
     if (st != PSR_OK) return st;
-    b.flags = kModeJacY;                       // columns 1..K: T-only factors from the rate table
+    b.flags = kModeJacY | en;                  // columns 1..K: T-only factors from the rate table
     b.tab = tab;
     b.n_tiles = nb * tpr;
     st = run(m, b, stream, "psr_fd_jacobian (Y columns)");
     if (st != PSR_OK) return st;
   }
   return PSR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, const double* P, const double* Y,
+                           const double* Yin, const double* tau, int64_t ld, double* J, double* F0, void* stream) {
+  return fd_jacobian_impl(mech, N, T, P, Y, nullptr, Yin, tau, ld, J, F0, stream, "psr_fd_jacobian");
+}
+
+psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double* T, const double* P, const double* Y,
+                                  const double* Tin, const double* Yin, const double* tau, int64_t ld, double* J,
+                                  double* F0, void* stream) {
+  if (!Tin) {
+    g_err = "psr_fd_jacobian_energy: null Tin";
+    return PSR_EINVAL;
+  }
+  return fd_jacobian_impl(mech, N, T, P, Y, Tin, Yin, tau, ld, J, F0, stream, "psr_fd_jacobian_energy");
 }
 
 psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {

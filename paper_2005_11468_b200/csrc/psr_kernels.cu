@@ -101,11 +101,11 @@ struct RowIO<2> {
 // table that the base-residual launch wrote, as warp-uniform broadcasts, instead of being recomputed.
 // EN: psr_eval_residual_energy -- the epilogue also forms the energy row (kOutFT).  Its own instantiation so
 // that the extra registers and code stay out of the other calls (measured: 2.7 % on C1 when shared).
-constexpr int kVarPlain = 0, kVarJacY = 1, kVarEnergy = 2;
+constexpr int kVarPlain = 0, kVarJacY = 1, kVarEnergy = 2;   // bit flags: 3 = Y-column launch of the adiabatic Jacobian
 template <int NW, int SPW, int R, int VAR>
 __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const MechView mv, const EvalArgs a) {
-  constexpr bool JY = VAR == kVarJacY;
-  constexpr bool EN = VAR == kVarEnergy;
+  constexpr bool JY = (VAR & kVarJacY) != 0;
+  constexpr bool EN = (VAR & kVarEnergy) != 0;
   static_assert(!JY || R == 1, "the Y-column mode maps one column to a lane");
   constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
@@ -428,8 +428,10 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         const double invh = 1.0 / hs[lane * R + i];
         double y = ldg_nc(a.Y + o);
         if (s == jsp_) y = y + 1e-8 * fmax(fabs(y), 1e-10);   // the same x' as in the prologue
-        const double Fv = fma(y - ldg_nc(a.Yin + o), invtau, -(accv * (mv.Wm[s] * invrho)));
+        const double yin = ldg_nc(a.Yin + o);
+        const double Fv = fma(y - yin, invtau, -(accv * (mv.Wm[s] * invrho)));
         *ga_slot(s, r_, jsp_) = (Fv - ldg_nc(a.F0 + r_ * n + 1 + s)) * invh;
+        if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r_), y, yin, accv);
       }
     };
     auto gather_and_release = [&](bool first, bool last) {
@@ -815,6 +817,36 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 
     gather_and_release(mv.n_chunks == 1, true);
 
+    // Energy row: the three sums over all species -- per-warp shares through shared memory (the q tile is
+    // free by now), added in warp order by warp 0, whose lanes get F_T = -dT/dt of their states.  Every
+    // thread of the CTA calls this.
+    auto energy_reduce = [&](double (&ft)[R]) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int i = 0; i < R; ++i) en_s[(k * NW + w) * TR + lane * R + i] = en[k][i];
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < R; ++i) {
+        ft[i] = 0.0;
+        if (w == 0) {
+          double e[3];
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            e[k] = 0.0;
+#pragma unroll
+            for (int ww = 0; ww < NW; ++ww) e[k] += en_s[(k * NW + ww) * TR + lane * R + i];
+          }
+          ft[i] = -((e[0] / ldg_nc(a.tau + r[i]) - e[1] / rho_s[lane * R + i]) / e[2]);
+        }
+      }
+      __syncthreads();
+      if (w == 0) {   // the partial sums may have covered the q tile's zero row
+#pragma unroll
+        for (int i = 0; i < R; ++i) qs[mv.rc * TR + lane * R + i] = 0.0;
+      }
+    };
+
     // ---------------------------------------------------------------- epilogue (a8 store, a9, a10)
     if constexpr (GA) {
       // every (species, state) entry left with the last gather; what remains is row 0 of the unknowns
@@ -822,8 +854,24 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
         for (int i = 0; i < R; ++i) {
           if (valid[i]) {
+            if (EN) continue;
             if (jac) a.J[((int64_t)r[i] * n + (jsp[i] + 1)) * n] = (jsp[i] == -1) ? 1.0 : 0.0;   // F_T = T - T_set
             else if (a.flags & kOutF0) a.F0out[r[i] * n] = 0.0;
+          }
+        }
+      }
+      if constexpr (EN) {
+        double ft[R];
+        energy_reduce(ft);
+        if (w == 0) {
+#pragma unroll
+          for (int i = 0; i < R; ++i) {
+            if (!valid[i]) continue;
+            if (jac) a.J[((int64_t)r[i] * n + (jsp[i] + 1)) * n] = (ft[i] - ldg_nc(a.F0 + r[i] * n)) / hs[lane * R + i];
+            else {
+              if (a.FT) a.FT[r[i]] = ft[i];
+              if (a.flags & kOutF0) a.F0out[r[i] * n] = ft[i];
+            }
           }
         }
       }
@@ -847,7 +895,19 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               }
             }
           }
-          if ((a.flags & kOutF0) && w == 0) a.F0out[r[i] * n] = 0.0;
+          if (!EN && (a.flags & kOutF0) && w == 0) a.F0out[r[i] * n] = 0.0;
+        }
+      }
+      if constexpr (EN) {
+        double ft[R];
+        energy_reduce(ft);
+        if (w == 0) {
+#pragma unroll
+          for (int i = 0; i < R; ++i) {
+            if (!valid[i]) continue;
+            if (a.FT) a.FT[r[i]] = ft[i];
+            if (a.flags & kOutF0) a.F0out[r[i] * n] = ft[i];
+          }
         }
       }
     } else {
@@ -868,9 +928,19 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
             if (s == jsp[i]) y = y + 1e-8 * fmax(fabs(y), 1e-10);   // the same x' as in the prologue
             const double Fv = fma(y - e_yin[jj][i], invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
             stg[st * npad + 1 + s] = (Fv - e_f0[jj][i]) * invh;
+            if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), y, e_yin[jj][i], acc[jj][i]);
           }
         }
-        if (w == 0) stg[st * npad] = (jsp[i] == -1) ? 1.0 : 0.0;  // row 0: F_T = T - T_set
+        if (!EN && w == 0) stg[st * npad] = (jsp[i] == -1) ? 1.0 : 0.0;  // row 0: F_T = T - T_set
+      }
+      if constexpr (EN) {   // row 0: the energy row's difference quotient
+        double ft[R];
+        energy_reduce(ft);
+        if (w == 0) {
+#pragma unroll
+          for (int i = 0; i < R; ++i)
+            stg[(i * 32 + lane) * npad] = (ft[i] - ldg_nc(a.F0 + r[i] * n)) / hs[lane * R + i];
+        }
       }
       __syncthreads();
       if constexpr (JY) {
@@ -900,35 +970,6 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       }
       __syncthreads();
     }
-    if constexpr (EN) {
-      // the three sums over all species: per-warp shares through shared memory, added in warp order
-#pragma unroll
-      for (int k = 0; k < 3; ++k)
-#pragma unroll
-        for (int i = 0; i < R; ++i) en_s[(k * NW + w) * TR + lane * R + i] = en[k][i];
-      __syncthreads();
-      if (w == 0) {
-#pragma unroll
-        for (int i = 0; i < R; ++i) {
-          if (valid[i]) {
-            double e[3];
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-              e[k] = 0.0;
-#pragma unroll
-              for (int ww = 0; ww < NW; ++ww) e[k] += en_s[(k * NW + ww) * TR + lane * R + i];
-            }
-            const double dTdt = (e[0] / ldg_nc(a.tau + r[i]) - e[1] / rho_s[lane * R + i]) / e[2];
-            a.FT[r[i]] = -dTdt;
-          }
-        }
-      }
-      __syncthreads();
-      if (w == 0) {   // the partial sums may have covered the q tile's zero row
-#pragma unroll
-        for (int i = 0; i < R; ++i) qs[mv.rc * TR + lane * R + i] = 0.0;
-      }
-    }
     if (mv.n_cbuf == 1) prefetch(tile + gridDim.x, 0);   // single C buffer: it is free only now
   }
 }
@@ -946,9 +987,10 @@ static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cud
 }
 
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  const int var = (a.flags & kModeJacY) ? kVarJacY : (a.flags & kOutFT) ? kVarEnergy : kVarPlain;
+  const int var = ((a.flags & kModeJacY) ? kVarJacY : 0) | ((a.flags & kOutFT) ? kVarEnergy : 0);
 #define PSR_L(NW_, SPW_)                                                                        \
   if (nw == NW_ && spw == SPW_ && rl == 1) {                                                    \
+    if (var == 3) return launch_t<NW_, SPW_, 1, 3>(mv, a, grid, st);                            \
     if (var == kVarJacY) return launch_t<NW_, SPW_, 1, kVarJacY>(mv, a, grid, st);              \
     if (var == kVarEnergy) return launch_t<NW_, SPW_, 1, kVarEnergy>(mv, a, grid, st);          \
     return launch_t<NW_, SPW_, 1, kVarPlain>(mv, a, grid, st);                                  \
@@ -960,18 +1002,19 @@ cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalA
 
 template <int NW, int SPW, int R>
 static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
-  int n0 = 0, n1 = 0, n2 = 0;
-  auto k0 = psr_eval_kernel<NW, SPW, R, kVarPlain>;
-  auto k1 = psr_eval_kernel<NW, SPW, R, kVarJacY>;
-  auto k2 = psr_eval_kernel<NW, SPW, R, kVarEnergy>;
-  cudaError_t e = cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n0, k0, NW * 32, smem);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k1, NW * 32, smem);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n2, k2, NW * 32, smem);
-  *ctas_per_sm = n0 < n1 ? (n0 < n2 ? n0 : n2) : (n1 < n2 ? n1 : n2);
-  return e;
+  // every variant is launched with the same grid: size it for the one with the lowest occupancy
+  const void* kerns[4] = {(const void*)psr_eval_kernel<NW, SPW, R, 0>, (const void*)psr_eval_kernel<NW, SPW, R, 1>,
+                          (const void*)psr_eval_kernel<NW, SPW, R, 2>, (const void*)psr_eval_kernel<NW, SPW, R, 3>};
+  int least = 1 << 30;
+  for (const void* k : kerns) {
+    int nb = 0;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, NW * 32, smem);
+    if (e != cudaSuccess) return e;
+    least = nb < least ? nb : least;
+  }
+  *ctas_per_sm = least;
+  return cudaSuccess;
 }
 
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm) {

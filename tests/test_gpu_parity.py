@@ -405,6 +405,39 @@ def test_energy_residual_T3_golden(torch_cuda, binding):
     gm.close()
 
 
+@pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50), ("C2", 3)])
+def test_fd_jacobian_energy_floor_criterion(torch_cuda, binding, cfg, n):
+    """Adiabatic Jacobian (row 0 = energy row): floor criterion against the long-double oracle, species rows
+    bit-identical to psr_fd_jacobian, hoisted sweep bit-identical to the all-columns sweep."""
+    torch = torch_cuda
+    mech, batch = synth.make_config(cfg, n)
+    Tin = np.random.default_rng(4).uniform(300.0, 700.0, n)
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    dTin = dev(torch, Tin)
+    J, F0 = gm.fd_jacobian(*args, want_F0=True, Tin=dTin)
+    Jp = gm.fd_jacobian(*args)
+    os.environ["PSR_JAC_UNHOISTED"] = "1"
+    try:
+        J3 = gm.fd_jacobian(*args, Tin=dTin)
+    finally:
+        del os.environ["PSR_JAC_UNHOISTED"]
+    _, FT = gm.eval_residual_energy(args[0], args[1], args[2], dTin, args[3], args[4])
+    torch.cuda.synchronize()
+    J, F0, Jp, J3, FT = (x.cpu().numpy() for x in (J, F0, Jp, J3, FT))
+    gm.close()
+    assert np.array_equal(J, J3)
+    assert np.array_equal(J[:, :, 1:], Jp[:, :, 1:])
+    assert np.array_equal(F0[:, 0], FT)
+    om = oracle_mech(mech)
+    jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin, long_double=True)
+    jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin)
+    worst, fr_T, fr_Y = jacobian_floor_ratio(J, jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y)
+    _, od_T, od_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
+    assert fr_T <= 4 * max(od_T, 1.0) and fr_Y <= 4 * max(od_Y, 1.0), (fr_T, od_T, fr_Y, od_Y)
+
+
 # ------------------------------------------------------------------ streams and graphs
 def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, binding):
     """Every evaluation call only enqueues work on the caller's stream (psr.h), so a Newton iteration
