@@ -138,6 +138,19 @@ def jacobian(mech: OracleMechanism, T, P, Y, Yin, tau, *, Tin=None, long_double:
     return dict(J=J, F0=F0, S=S, H=H)
 
 
+def lu_solve(A, b, *, long_double: bool = False):
+    """NEXT-2: batched A x = b by Gaussian elimination with partial pivoting.  A: [N][n][n] with A[r, j, i] =
+    entry (row i, column j) (column-major per system, the layout of J), b: [N][n].  Returns x [N][n], info [N]."""
+    A = np.ascontiguousarray(A, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    N, n = b.shape
+    assert A.shape == (N, n, n)
+    x = np.full((N, n), np.nan)
+    info = np.zeros(N, dtype=np.int32)
+    lib().oracle_lu_solve(C.c_int64(N), C.c_int(n), _p(A), _p(b), _p(x), _p(info), C.c_int(int(long_double)))
+    return x, info
+
+
 _DETAIL_COLS = ("kinf", "k0", "Pr", "Fcent", "F", "M", "Kp", "Kc", "kf", "kr", "q")
 
 

@@ -23,6 +23,8 @@
 //   Jacobian species rows of a Y column sum to 1/tau; J row 0 = e_0.
 //   Energy row (NEXT-1): T3 values of h_i, C_p,mix and F_T from SURVEY.md 8(c), re-derived with mpmath;
 //   F_T = 0 for an inert mechanism at T_in = T; linearity in 1/tau; enthalpy-balance identity.
+//   Linear solve (NEXT-2): exact rational solutions of small integer systems, a system that needs a row
+//   exchange, a singular system, LAPACK (numpy.linalg.solve) on random systems, backward error bound.
 //
 // Units (paper silent; CHEMKIN cgs, reading g4): T [K], P [dyn/cm^2], C [mol/cm^3],
 // rho [g/cm^3], W [g/mol], wdot [mol/cm^3/s], Ea [cal/mol].
@@ -368,9 +370,58 @@ int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P,
   return 0;
 }
 
+// NEXT-2: the Newton step's linear solve ("The Jacobian matrix is decomposed into lower and upper
+// triangular matrices, and then a back-solving operation is carried out"): Gaussian
+// elimination with partial pivoting (row of largest |a_ik|, the first one on ties), then forward and back
+// substitution.  A: n x n column-major (entry (i,j) at A[j*n+i]), not modified; b -> x.  Returns 0, or
+// k+1 if the pivot of step k is exactly zero (x is then left unset).
+template <class R>
+int lu_solve_one(int n, const double* A, const double* b, double* x) {
+  std::vector<R> a((size_t)n * n), y(n);
+  for (size_t t = 0; t < (size_t)n * n; ++t) a[t] = (R)A[t];
+  for (int i = 0; i < n; ++i) y[i] = (R)b[i];
+  for (int k = 0; k < n; ++k) {
+    int p = k;
+    R best = a[(size_t)k * n + k] < 0 ? -a[(size_t)k * n + k] : a[(size_t)k * n + k];
+    for (int i = k + 1; i < n; ++i) {
+      const R v = a[(size_t)k * n + i] < 0 ? -a[(size_t)k * n + i] : a[(size_t)k * n + i];
+      if (v > best) { best = v; p = i; }
+    }
+    if (best == (R)0) return k + 1;
+    if (p != k) {
+      for (int j = 0; j < n; ++j) std::swap(a[(size_t)j * n + k], a[(size_t)j * n + p]);
+      std::swap(y[k], y[p]);
+    }
+    for (int i = k + 1; i < n; ++i) {
+      const R l = a[(size_t)k * n + i] / a[(size_t)k * n + k];
+      a[(size_t)k * n + i] = l;
+      for (int j = k + 1; j < n; ++j) a[(size_t)j * n + i] -= l * a[(size_t)j * n + k];
+      y[i] -= l * y[k];
+    }
+  }
+  for (int i = n - 1; i >= 0; --i) {
+    R sum = y[i];
+    for (int j = i + 1; j < n; ++j) sum -= a[(size_t)j * n + i] * y[j];
+    y[i] = sum / a[(size_t)i * n + i];
+  }
+  for (int i = 0; i < n; ++i) x[i] = (double)y[i];
+  return 0;
+}
+
 }  // namespace
 
 extern "C" {
+
+// Batched A x = b: A [N][n*n] column-major per system, b, x [N][n], info [N] (0 or k+1, see lu_solve_one).
+int oracle_lu_solve(int64_t N, int n, const double* A, const double* b, double* x, int32_t* info,
+                    int use_long_double) {
+  for (int64_t r = 0; r < N; ++r) {
+    const double* Ar = A + (size_t)r * n * n;
+    info[r] = use_long_double ? lu_solve_one<long double>(n, Ar, b + r * n, x + r * n)
+                              : lu_solve_one<double>(n, Ar, b + r * n, x + r * n);
+  }
+  return 0;
+}
 
 // Batch evaluation, species-major SoA (element (k, r) at [k*ld + r]).  Any output may be null.
 // use_long_double: 0 -> double (the oracle), 1 -> long double reference.

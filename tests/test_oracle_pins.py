@@ -515,3 +515,51 @@ def test_energy_jacobian_double_within_floor_of_long_double_C4():
     worst, fr_T, fr_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
     assert worst <= 1.0, (worst, fr_T, fr_Y)
     assert np.all(jl["S"][:, 0] > 0)
+
+
+# ------------------------------------------------------------------ linear solve (SURVEY.md 8(f) NEXT-2)
+def _colmajor(M):
+    """[N][n][n] row-major matrices -> the J layout A[r, col, row]."""
+    return np.ascontiguousarray(np.swapaxes(np.asarray(M, dtype=np.float64), 1, 2))
+
+
+def test_lu_solve_exact_small_systems_and_row_exchange():
+    from fractions import Fraction
+    mats = [[[2, 1], [1, 3]], [[0, 2], [3, 1]],                       # the second needs a row exchange
+            [[4, -2, 1], [-2, 4, -2], [1, -2, 4]], [[1, 2, 3], [4, 5, 6], [7, 8, 10]]]
+    rhs = [[3, 5], [4, 5], [11, -16, 17], [6, 15, 25]]
+    for M, b in zip(mats, rhs):
+        n = len(b)
+        # exact solution by Cramer-free rational elimination
+        A = [[Fraction(v) for v in row] + [Fraction(bb)] for row, bb in zip(M, b)]
+        for k in range(n):
+            p = next(i for i in range(k, n) if A[i][k] != 0)
+            A[k], A[p] = A[p], A[k]
+            for i in range(n):
+                if i != k:
+                    f = A[i][k] / A[k][k]
+                    A[i] = [u - f * v for u, v in zip(A[i], A[k])]
+        exact = np.array([float(A[i][n] / A[i][i]) for i in range(n)])
+        x, info = orc.lu_solve(_colmajor([M]), np.array([b], dtype=np.float64))
+        assert info[0] == 0 and np.allclose(x[0], exact, rtol=1e-14, atol=0)
+
+
+def test_lu_solve_reports_a_zero_pivot():
+    x, info = orc.lu_solve(_colmajor([[[1, 2], [2, 4]], [[0, 0], [0, 1]]]), np.ones((2, 2)))
+    assert info[0] == 2 and info[1] == 1
+
+
+def test_lu_solve_matches_lapack_and_is_backward_stable():
+    rng = np.random.default_rng(21)
+    N, n = 16, 54
+    M = rng.standard_normal((N, n, n)) + 4.0 * np.eye(n)
+    b = rng.standard_normal((N, n))
+    x, info = orc.lu_solve(_colmajor(M), b)
+    assert np.all(info == 0)
+    ref = np.linalg.solve(M, b[:, :, None])[:, :, 0]                    # LAPACK dgesv
+    assert np.abs(x - ref).max() <= 1e-12 * np.abs(ref).max()
+    res = np.abs(np.einsum("rij,rj->ri", M, x) - b).max(axis=1)
+    bound = n * EPS * (np.abs(M).sum(axis=2).max(axis=1) * np.abs(x).max(axis=1) + np.abs(b).max(axis=1))
+    assert np.all(res <= 8 * bound)
+    xl, _ = orc.lu_solve(_colmajor(M), b, long_double=True)
+    assert np.abs(x - xl).max() <= 1e-12 * np.abs(xl).max()
