@@ -129,6 +129,16 @@ psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double*
                                   const double* Y, const double* Tin, const double* Yin, const double* tau,
                                   int64_t ld, double* J, double* F0, void* stream);
 
+/* Newton step's linear solve ("The Jacobian matrix is decomposed into
+ * lower and upper triangular matrices, and then a back-solving operation is carried out"): N independent
+ * dense systems A x = b by Gaussian elimination with partial pivoting, one warp per system.
+ * A: DEVICE [N][n*n], column-major per system (the layout psr_fd_jacobian writes), not modified.
+ * b: DEVICE [N][n], right-hand side in, solution out (unchanged for a system that fails).
+ * info: DEVICE [N], 0 on success, k+1 if the pivot column of step k (0-based) is exactly zero.
+ * n <= 168 on a 227 KB shared-memory device (PSR_EUNSUPPORTED beyond).  The Newton update is the solve of
+ * J dx = -F: pass b = -F0.  Asynchronous on `stream`. */
+psr_status psr_lu_solve(int64_t N, int32_t n, const double* A, double* b, int32_t* info, void* stream);
+
 /* Thread-local description of the last failure on this thread; valid until its next psr_* call. */
 const char* psr_last_error(void);
 

@@ -17,7 +17,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -68,6 +68,8 @@ def lib():
         L.psr_eval_residual_energy.restype = C.c_int
         L.psr_fd_jacobian_energy.argtypes = [vp, i64, dp, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_fd_jacobian_energy.restype = C.c_int
+        L.psr_lu_solve.argtypes = [i64, C.c_int32, dp, dp, dp, vp]
+        L.psr_lu_solve.restype = C.c_int
         L.psr_fd_jacobian.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_fd_jacobian.restype = C.c_int
         L.psr_last_error.argtypes = []
@@ -265,3 +267,18 @@ def probe_fp64(kind: int, iters: int):
 
 def version() -> str:
     return lib().psr_version().decode()
+
+
+def lu_solve(A, b, info=None):
+    """psr_lu_solve: A [N][n][n] (A[r, col, row], the layout of J), b [N][n] overwritten by the solution.
+    Returns (b, info) with info [N] int32 (0 = solved)."""
+    import torch
+    N, n = b.shape
+    if A.shape != (N, n, n) or not A.is_contiguous() or not b.is_contiguous():
+        raise ValueError("A must be contiguous [N][n][n] and b contiguous [N][n]")
+    for nm, t in (("A", A), ("b", b)):
+        _chk_dev(nm, t)
+    if info is None:
+        info = torch.empty(N, dtype=torch.int32, device=b.device)
+    _check(lib().psr_lu_solve(N, n, _ptr(A), _ptr(b), _ptr(info), _stream()))
+    return b, info

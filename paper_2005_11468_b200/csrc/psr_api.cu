@@ -20,6 +20,8 @@ namespace psr {
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st);
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm);
 cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st);
+cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
+                            cudaStream_t st);
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
 }  // namespace psr
 
@@ -710,6 +712,25 @@ psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double*
     return PSR_EINVAL;
   }
   return fd_jacobian_impl(mech, N, T, P, Y, Tin, Yin, tau, ld, J, F0, stream, "psr_fd_jacobian_energy");
+}
+
+psr_status psr_lu_solve(int64_t N, int32_t n, const double* A, double* b, int32_t* info, void* stream) {
+  g_err.clear();
+  if (N < 0 || n < 1) return fail(PSR_EINVAL, "psr_lu_solve: N < 0 or n < 1");
+  if (N == 0) return PSR_OK;
+  if (!A || !b || !info) return fail(PSR_EINVAL, "psr_lu_solve: null A, b or info");
+  int dev = 0, n_sm = 0, optin = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return cuda_fail(e, "psr_lu_solve");
+  const size_t per_sys = ((size_t)n * (n | 1) + ((n + 1) & ~1)) * 8;
+  if (n > 192 || per_sys > (size_t)optin)
+    return fail(PSR_EUNSUPPORTED, "psr_lu_solve: a %d x %d system needs %zu bytes of shared memory, device allows %d", n, n,
+                per_sys, optin);
+  e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream);
+  if (e != cudaSuccess) return cuda_fail(e, "psr_lu_solve");
+  return PSR_OK;
 }
 
 psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {

@@ -438,6 +438,83 @@ def test_fd_jacobian_energy_floor_criterion(torch_cuda, binding, cfg, n):
     assert fr_T <= 4 * max(od_T, 1.0) and fr_Y <= 4 * max(od_Y, 1.0), (fr_T, od_T, fr_Y, od_Y)
 
 
+# ------------------------------------------------------------------ linear solve of the Newton step (NEXT-2)
+EPS64 = 2.0 ** -53
+
+
+def _backward_error_ok(A, x, b, n, factor=8.0):
+    """Row-wise bound of Gaussian elimination with partial pivoting: |Ax - b|_inf <= c n eps (|A|_inf |x|_inf + |b|_inf).
+    A: [N][col][row]."""
+    M = np.swapaxes(A, 1, 2)
+    res = np.abs(np.einsum("rij,rj->ri", M, x) - b).max(axis=1)
+    bound = n * EPS64 * (np.abs(M).sum(axis=2).max(axis=1) * np.abs(x).max(axis=1) + np.abs(b).max(axis=1))
+    return np.all(res <= factor * bound), float((res / bound).max())
+
+
+@pytest.mark.parametrize("n,N", [(1, 5), (3, 7), (11, 33), (32, 40), (33, 9), (54, 300), (64, 17), (101, 6), (168, 2)])
+def test_lu_solve_random_systems(torch_cuda, binding, n, N):
+    torch = torch_cuda
+    rng = np.random.default_rng(100 + n)
+    M = rng.standard_normal((N, n, n)) + 3.0 * np.eye(n)
+    if n > 1:
+        M[0, 0, 0] = 0.0                                 # forces a row exchange in the first step of system 0
+    b = rng.standard_normal((N, n))
+    A = np.ascontiguousarray(np.swapaxes(M, 1, 2))       # A[r, col, row]
+    x, info = binding.lu_solve(dev(torch, A), dev(torch, b.copy()))
+    torch.cuda.synchronize()
+    x, info = x.cpu().numpy(), info.cpu().numpy()
+    xr, ir = orc.lu_solve(A, b)
+    assert np.array_equal(info, ir) and np.all(info == 0)
+    ok, worst = _backward_error_ok(A, x, b, n)
+    assert ok, worst
+    # same pivots, same elimination order: the two agree far inside the conditioning of these systems
+    assert np.abs(x - xr).max() <= 1e-11 * np.abs(xr).max()
+
+
+def test_lu_solve_flags_singular_systems_and_leaves_their_rhs(torch_cuda, binding):
+    torch = torch_cuda
+    M = np.stack([np.eye(4), np.array([[1.0, 2, 0, 0], [2, 4, 0, 0], [0, 0, 1, 0], [0, 0, 0, 1]]), np.zeros((4, 4))])
+    b = np.arange(12, dtype=np.float64).reshape(3, 4) + 1.0
+    A = np.ascontiguousarray(np.swapaxes(M, 1, 2))
+    x, info = binding.lu_solve(dev(torch, A), dev(torch, b.copy()))
+    torch.cuda.synchronize()
+    x, info = x.cpu().numpy(), info.cpu().numpy()
+    _, ir = orc.lu_solve(A, b)
+    assert np.array_equal(info, ir) and list(info) == [0, 2, 1]
+    assert np.array_equal(x[0], b[0]) and np.array_equal(x[1], b[1]) and np.array_equal(x[2], b[2])
+
+
+def test_newton_step_on_device_matches_the_oracle_solve(torch_cuda, binding):
+    """One Newton update of the C4 system entirely on the device: J, F0 from psr_fd_jacobian, then J dx = -F0
+    by psr_lu_solve; compared with the oracle's elimination of the same J (long double) and by backward error."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C4", 64)
+    gm = binding.Mechanism.from_synth(mech)
+    args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    J, F0 = gm.fd_jacobian(*args, want_F0=True)
+    rhs = (-F0).contiguous()
+    dx, info = binding.lu_solve(J, rhs.clone())
+    torch.cuda.synchronize()
+    gm.close()
+    Jh, bh, dx, info = J.cpu().numpy(), rhs.cpu().numpy(), dx.cpu().numpy(), info.cpu().numpy()
+    assert np.all(info == 0) and np.all(np.isfinite(dx))
+    n = mech.n_species + 1
+    ok, worst = _backward_error_ok(Jh, dx, bh, n)
+    assert ok, worst
+    xr, ir = orc.lu_solve(Jh, bh)
+    xl, _ = orc.lu_solve(Jh, bh, long_double=True)
+    assert np.all(ir == 0)
+    # forward error (these Jacobians are ill-conditioned, both FP64 solves sit 1e-9..1e-5 from the long-double
+    # one): the GPU's distance is of the size of the FP64 oracle's -- typically (median) within 4x, never
+    # beyond 64x; the rigorous statement is the backward error above
+    e_gpu = np.abs(dx - xl).max(axis=1)
+    e_ref = np.abs(xr - xl).max(axis=1)
+    scale = np.abs(xl).max(axis=1)
+    ratio = e_gpu / (e_ref + 1e-13 * scale)
+    assert np.median(ratio) <= 4.0 and ratio.max() <= 64.0, (float(np.median(ratio)), float(ratio.max()))
+    assert np.all(np.abs(dx[:, 0]) <= 1e-8 * scale)      # fixed-temperature row: dT = -F_T = 0 up to the solve's round-off
+
+
 # ------------------------------------------------------------------ streams and graphs
 def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, binding):
     """Every evaluation call only enqueues work on the caller's stream (psr.h), so a Newton iteration
