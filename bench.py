@@ -364,6 +364,16 @@ def run_extras(binding, synth, torch, flush):
             Tin = torch.full_like(T, 300.0)
             ms_en = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J, Tin=Tin), flush)
             out["C4_energy"] = {"call": "psr_fd_jacobian_energy", "ms": ms_en, "jacobians_per_s": batch.n / (ms_en * 1e-3)}
+            # NEXT-2: the Newton step's solve J dx = -F0 on the Jacobians just computed
+            J0, F0 = gm.fd_jacobian(T, P, Y, Yin, tau, want_F0=True)
+            rhs0, rhs = (-F0).contiguous(), torch.empty_like(F0)
+            def solve():
+                rhs.copy_(rhs0)
+                binding.lu_solve(J0, rhs)
+            ms_lu = _time_call(torch, solve, flush)
+            out["C4_solve"] = {"call": "psr_lu_solve (+ 3.5 MB rhs copy)", "ms": ms_lu, "systems_per_s": batch.n / (ms_lu * 1e-3),
+                               "n": n, "hbm_GBps_on_J": batch.n * n * n * 8 / (ms_lu * 1e-3) / 1e9}
+            del J0
             out[cfg] = {"call": "psr_fd_jacobian", "ms": ms, "jacobians_per_s": batch.n / (ms * 1e-3),
                         "residual_evals_per_s": batch.n * (n + 1) / (ms * 1e-3),
                         "alu_frac_unhoisted": instr * batch.n * (n + 1) / (ms * 1e-3) / (N_SM * FP64_LANES_PER_SM * 1.965e9)}

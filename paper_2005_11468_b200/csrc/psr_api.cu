@@ -724,10 +724,7 @@ psr_status psr_lu_solve(int64_t N, int32_t n, const double* A, double* b, int32_
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (e != cudaSuccess) return cuda_fail(e, "psr_lu_solve");
-  const size_t per_sys = ((size_t)n * (n | 1) + ((n + 1) & ~1)) * 8;
-  if (n > 192 || per_sys > (size_t)optin)
-    return fail(PSR_EUNSUPPORTED, "psr_lu_solve: a %d x %d system needs %zu bytes of shared memory, device allows %d", n, n,
-                per_sys, optin);
+  if (n > 168) return fail(PSR_EUNSUPPORTED, "psr_lu_solve: n = %d, the one-warp-per-system kernel takes n <= 168", n);
   e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream);
   if (e != cudaSuccess) return cuda_fail(e, "psr_lu_solve");
   return PSR_OK;

@@ -16,7 +16,10 @@ namespace psr {
 
 constexpr unsigned kFull = 0xffffffffu;
 
-// RPL: rows per lane (n <= 32 * RPL)
+// RPL: rows per lane (n <= 32 * RPL).  The column stride ld = n | 1 is a run-time value, so the update walks
+// the columns with two running pointers (pivot-row entry, this lane's rows) instead of forming j*ld + i for
+// every access (that index arithmetic cost more instructions than the elimination itself: 51 k
+// instructions per 54 x 54 system, 4 k of them FMA, in the first version).
 template <int RPL>
 __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const double* __restrict__ A,
                                                        double* __restrict__ b, int32_t* __restrict__ info,
@@ -24,20 +27,36 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
   extern __shared__ __align__(16) double sm[];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, wpc = blockDim.x >> 5;
   const int ld = n | 1;
-  double* As = sm + (size_t)w * sys_doubles;   // [n][ld], entry (i, j) at As[j*ld + i]
+  double* As = sm + (size_t)w * sys_doubles;   // entry (i, j) at As[j*ld + i]
   double* bs = As + (size_t)n * ld;            // [n]
 
   for (int64_t r = (int64_t)blockIdx.x * wpc + w; r < N; r += (int64_t)gridDim.x * wpc) {
     const double* Ar = A + (size_t)r * n * n;
-    for (int t = lane; t < n * n; t += 32) {
-      const int j = t / n, i = t - j * n;
-      As[j * ld + i] = Ar[t];
+    {
+      // column-major stream, 32 consecutive entries per trip, 4 trips in flight; (i, j) tracked without a divide
+      int i = lane, j = 0;
+      while (i >= n) { i -= n; ++j; }
+      for (int t = lane; t < n * n; t += 128) {
+        double v[4];
+        int off[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          off[u] = j * ld + i;
+          v[u] = (t + 32 * u < n * n) ? Ar[t + 32 * u] : 0.0;
+          i += 32;
+          while (i >= n) { i -= n; ++j; }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (t + 32 * u < n * n) As[off[u]] = v[u];
+      }
     }
     for (int i = lane; i < n; i += 32) bs[i] = b[r * n + i];
     __syncwarp();
 
     int fail = 0;
-    for (int k = 0; k < n; ++k) {
+    double* colk = As;   // column k
+    for (int k = 0; k < n; ++k, colk += ld) {
       // pivot: largest |a_ik| over rows i >= k, the smallest i on ties
       double best = -1.0;
       int p = k;
@@ -45,7 +64,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
       for (int rr = 0; rr < RPL; ++rr) {
         const int i = lane + 32 * rr;
         if (i >= k && i < n) {
-          const double v = fabs(As[k * ld + i]);
+          const double v = fabs(colk[i]);
           if (v > best) { best = v; p = i; }
         }
       }
@@ -60,10 +79,11 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
         break;
       }
       if (p != k) {
-        for (int j = lane; j < n; j += 32) {
-          const double u = As[j * ld + k];
-          As[j * ld + k] = As[j * ld + p];
-          As[j * ld + p] = u;
+        double* pj = As + lane * ld;
+        for (int j = lane; j < n; j += 32, pj += 32 * ld) {
+          const double u = pj[k];
+          pj[k] = pj[p];
+          pj[p] = u;
         }
         if (lane == 0) {
           const double u = bs[k];
@@ -72,39 +92,62 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
         }
       }
       __syncwarp();
-      const double piv = As[k * ld + k];
+      const double piv = colk[k];
       const double bk = bs[k];
       double l[RPL];
+      bool mine[RPL];
 #pragma unroll
       for (int rr = 0; rr < RPL; ++rr) {
         const int i = lane + 32 * rr;
+        mine[rr] = i > k && i < n;
         l[rr] = 0.0;
-        if (i > k && i < n) {
-          l[rr] = As[k * ld + i] / piv;
-          As[k * ld + i] = l[rr];
+        if (mine[rr]) {
+          l[rr] = colk[i] / piv;
+          colk[i] = l[rr];
           bs[i] = fma(-l[rr], bk, bs[i]);
         }
       }
-      for (int j = k + 1; j < n; ++j) {
-        const double akj = As[j * ld + k];   // broadcast
+      // rank-1 update of the trailing columns, kCB columns per trip: all loads of a trip are issued before
+      // its first store (stores to As would otherwise order every later load behind them)
+      constexpr int kCB = RPL <= 2 ? 8 : 4;
+      const double* pk = colk + ld + k;      // pivot-row entry of the current column
+      double* pl = colk + ld + lane;         // this lane's first row of the current column
+      int j0 = k + 1;
+      for (; j0 + kCB <= n; j0 += kCB) {
+        double akj[kCB], av[kCB][RPL];
+        const double* qk = pk;
+        const double* ql = pl;
 #pragma unroll
-        for (int rr = 0; rr < RPL; ++rr) {
-          const int i = lane + 32 * rr;
-          if (i > k && i < n) As[j * ld + i] = fma(-l[rr], akj, As[j * ld + i]);
+        for (int u = 0; u < kCB; ++u, qk += ld, ql += ld) {
+          akj[u] = *qk;   // broadcast
+#pragma unroll
+          for (int rr = 0; rr < RPL; ++rr) av[u][rr] = mine[rr] ? ql[32 * rr] : 0.0;
         }
+#pragma unroll
+        for (int u = 0; u < kCB; ++u, pk += ld, pl += ld)
+#pragma unroll
+          for (int rr = 0; rr < RPL; ++rr)
+            if (mine[rr]) pl[32 * rr] = fma(-l[rr], akj[u], av[u][rr]);
+      }
+      for (; j0 < n; ++j0, pk += ld, pl += ld) {
+        const double akj = *pk;
+#pragma unroll
+        for (int rr = 0; rr < RPL; ++rr)
+          if (mine[rr]) pl[32 * rr] = fma(-l[rr], akj, pl[32 * rr]);
       }
       __syncwarp();
     }
     if (!fail) {
       // back substitution, column oriented: x_i = b_i / u_ii, then b_r -= u_ri x_i for r < i
-      for (int i = n - 1; i >= 0; --i) {
-        const double xi = bs[i] / As[i * ld + i];
+      const double* coli = As + (size_t)(n - 1) * ld;
+      for (int i = n - 1; i >= 0; --i, coli -= ld) {
+        const double xi = bs[i] / coli[i];
         __syncwarp();
         if (lane == 0) bs[i] = xi;
 #pragma unroll
         for (int rr = 0; rr < RPL; ++rr) {
           const int rw = lane + 32 * rr;
-          if (rw < i) bs[rw] = fma(-As[i * ld + rw], xi, bs[rw]);
+          if (rw < i) bs[rw] = fma(-coli[rw], xi, bs[rw]);
         }
         __syncwarp();
       }
@@ -120,13 +163,19 @@ cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_
   const int ld = n | 1;
   const int sys_doubles = n * ld + ((n + 1) & ~1);
   const size_t per_sys = (size_t)sys_doubles * 8;
-  int wpc = (int)(smem_optin / per_sys);
-  if (wpc < 1) return cudaErrorInvalidConfiguration;
-  if (wpc > 4) wpc = 4;
+  if (per_sys > smem_optin) return cudaErrorInvalidConfiguration;
+  // systems (warps) per CTA: the count, up to 4, that packs the most systems into one SM's shared memory
+  const size_t sm_total = smem_optin + 1024;
+  int wpc = 1, best_sys = 0;
+  for (int c = 1; c <= 4; ++c) {
+    if (c * per_sys > smem_optin) break;
+    const int sys = (int)(sm_total / (c * per_sys + 1024)) * c;
+    if (sys >= best_sys) { best_sys = sys; wpc = c; }
+  }
   const size_t smem = per_sys * wpc;
   const int rpl = (n + 31) / 32;
   int64_t ctas = (N + wpc - 1) / wpc;
-  const int64_t cap = (int64_t)n_sm * 8;   // persistent: every CTA strides over the systems
+  const int64_t cap = (int64_t)n_sm * (best_sys / wpc);   // persistent: every CTA strides over the systems
   if (ctas > cap) ctas = cap;
 #define PSR_LU(RPL_)                                                                                         \
   if (rpl <= RPL_) {                                                                                         \
