@@ -240,11 +240,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
                             (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages);
   int n_chunks = 0, rc = 0;
   bool resident = false;
+  int ring_stages = 2;
   size_t stride = 0;
   std::vector<unsigned char> all;
   std::vector<int32_t> sp_of, rec_base_of;
   // the chunk size shrinks until one C tile, the q tile and the (double-buffered) chunk ring fit one CTA
-  for (;; rc_target = rc_target * 3 / 4) {
+  for (;; rc_target = std::min(rc_target - 1, rc_target * 15 / 16)) {
   if (rc_target < 1)
     return fail(PSR_EUNSUPPORTED, "mechanism does not fit %zu bytes of shared memory per CTA even at one reaction per chunk",
                 (size_t)prop.sharedMemPerBlockOptin);
@@ -401,13 +402,18 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     stride = std::max(stride, off);
   }
   stride = align_up(stride, 128);
-  // all chunk blobs resident in shared memory (loaded once per CTA) when they fit, else a 2-stage ring
+  // all chunk blobs resident in shared memory (loaded once per CTA) when they fit; else a ring of two
+  // stages, or of one when that is what lets this chunk size fit: a tile of a mechanism that large runs
+  // for hundreds of microseconds, the exposed ~1 us copy per chunk costs less than a smaller chunk's extra
+  // gather pass
   // q tile plus the rate-table slice of one chunk (Y-column launch of psr_fd_jacobian)
   // (the q tile also hosts the 3 x nw partial-sum rows of the energy row, hence the lower bound)
   const size_t q_bytes = align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128) + align_up((size_t)rc * kRateVals * 8, 128);
   resident = n_chunks <= kMaxStages && smem_fixed + q_bytes + stride * n_chunks <= (size_t)prop.sharedMemPerBlockOptin &&
              (n_chunks == 1 || stride * n_chunks <= 48 * 1024);
-  const size_t need = smem_fixed + q_bytes + stride * (resident ? n_chunks : 2);
+  ring_stages = 2;
+  if (!resident && smem_fixed + q_bytes + stride * 2 > (size_t)prop.sharedMemPerBlockOptin) ring_stages = 1;
+  const size_t need = smem_fixed + q_bytes + stride * (resident ? n_chunks : ring_stages);
   if (need > (size_t)prop.sharedMemPerBlockOptin) continue;
   all.assign(stride * n_chunks, 0);
   for (int c = 0; c < n_chunks; ++c) std::memcpy(all.data() + stride * c, blobs[c].data(), blobs[c].size());
@@ -431,6 +437,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.n_chunks = n_chunks;
   v.rc = rc;
   v.resident = resident ? 1 : 0;
+  v.ring_stages = ring_stages;
   v.need_lnctot = need_lnctot;
   v.chunk_stride = (uint32_t)stride;
   const size_t cbuf_bytes = align_up((size_t)(K + 2) * kTile * rl * 8, 128);  // K+2 rows so the Jacobian staging [tile][n|1] fits
@@ -441,7 +448,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     v.smem_q = (uint32_t)o;
     o += align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128);  // + the all-zero row; >= energy-row scratch
     v.smem_mech = (uint32_t)o;
-    o += stride * (resident ? n_chunks : 2);
+    o += stride * (resident ? n_chunks : ring_stages);
     v.smem_tab = (uint32_t)o;
     o += align_up((size_t)rc * kRateVals * 8, 128);
     v.smem_misc = (uint32_t)o;

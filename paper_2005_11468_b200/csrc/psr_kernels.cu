@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   const bool jacT = (a.flags & kModeJacT) != 0;
   const int tpr = (K + 31) / 32;   // JY: tiles per reactor
   const bool resident = mv.resident != 0;   // every chunk blob has its own stage and is loaded once per CTA
-  const int nstage = resident ? mv.n_chunks : 2;
+  const int nstage = resident ? mv.n_chunks : mv.ring_stages;
   const int cs_elems = (K + 2) * TR;
   const uint32_t q_lane = smem_u32(qs) + lane * (8 * R);
 
