@@ -15,6 +15,7 @@
 namespace psr {
 
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kNB = 8;   // pivots per pass over the trailing matrix
 
 // RPL: rows per lane (n <= 32 * RPL).  The column stride ld = n | 1 is a run-time value, so the update walks
 // the columns with two running pointers (pivot-row entry, this lane's rows) instead of forming j*ld + i for
@@ -29,6 +30,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
   const int ld = n | 1;
   double* As = sm + (size_t)w * sys_doubles;   // entry (i, j) at As[j*ld + i]
   double* bs = As + (size_t)n * ld;            // [n]
+  double* dinv = bs + n;                       // [n] reciprocals of the pivots
 
   for (int64_t r = (int64_t)blockIdx.x * wpc + w; r < N; r += (int64_t)gridDim.x * wpc) {
     const double* Ar = A + (size_t)r * n * n;
@@ -54,86 +56,152 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
     for (int i = lane; i < n; i += 32) bs[i] = b[r * n + i];
     __syncwarp();
 
+    // Blocked right-looking elimination, kNB pivots per pass over the trailing matrix: every trailing entry
+    // is read and written once per kNB pivots instead of once per pivot (shared-memory traffic is what bounds
+    // this kernel), with the kNB multipliers of a lane's rows held in registers.
     int fail = 0;
-    double* colk = As;   // column k
-    for (int k = 0; k < n; ++k, colk += ld) {
-      // pivot: largest |a_ik| over rows i >= k, the smallest i on ties
-      double best = -1.0;
-      int p = k;
+    for (int k0 = 0; k0 < n && !fail; k0 += kNB) {
+      const int nb = min(kNB, n - k0);
+      // ---- panel: columns k0 .. k0+nb-1, one pivot at a time; row exchanges span the whole row
+      double* colk = As + (size_t)k0 * ld;
+      for (int k = k0; k < k0 + nb; ++k, colk += ld) {
+        // pivot: largest |a_ik| over rows i >= k, the smallest i on ties.  |a| as an integer is ordered like
+        // the double, so the warp arg-max is three REDUX steps (high word, low word among the ties, row
+        // index among those) instead of five shuffle rounds.
+        double best = -1.0;
+        int p = n;
 #pragma unroll
-      for (int rr = 0; rr < RPL; ++rr) {
-        const int i = lane + 32 * rr;
-        if (i >= k && i < n) {
-          const double v = fabs(colk[i]);
-          if (v > best) { best = v; p = i; }
+        for (int rr = 0; rr < RPL; ++rr) {
+          const int i = lane + 32 * rr;
+          if (i >= k && i < n) {
+            const double v = fabs(colk[i]);
+            if (v > best) { best = v; p = i; }
+          }
         }
-      }
+        const unsigned bhi = best >= 0.0 ? (unsigned)__double2hiint(best) : 0u;
+        const unsigned blo = best >= 0.0 ? (unsigned)__double2loint(best) : 0u;
+        const unsigned mhi = __reduce_max_sync(kFull, bhi);
+        const unsigned mlo = __reduce_max_sync(kFull, (best >= 0.0 && bhi == mhi) ? blo : 0u);
+        p = (int)__reduce_min_sync(kFull, (best >= 0.0 && bhi == mhi && blo == mlo) ? (unsigned)p : 0xffffffffu);
+        best = __hiloint2double((int)mhi, (int)mlo);
+        if (!(best > 0.0) || p >= n) {   // zero (or NaN) pivot column
+          fail = k + 1;
+          break;
+        }
+        if (p != k) {
+          double* pj = As + lane * ld;
+          for (int j = lane; j < n; j += 32, pj += 32 * ld) {
+            const double u = pj[k];
+            pj[k] = pj[p];
+            pj[p] = u;
+          }
+          if (lane == 0) {
+            const double u = bs[k];
+            bs[k] = bs[p];
+            bs[p] = u;
+          }
+        }
+        __syncwarp();
+        const double rinv = 1.0 / colk[k];   // one division per pivot: multipliers and the back substitution use it
+        const double bk = bs[k];
+        if (lane == 0) dinv[k] = rinv;
+        double l[RPL];
+        bool mine[RPL];
 #pragma unroll
-      for (int off = 16; off > 0; off >>= 1) {
-        const double ob = __shfl_xor_sync(kFull, best, off);
-        const int op = __shfl_xor_sync(kFull, p, off);
-        if (ob > best || (ob == best && op < p)) { best = ob; p = op; }
-      }
-      if (!(best > 0.0)) {   // zero (or NaN) pivot column
-        fail = k + 1;
-        break;
-      }
-      if (p != k) {
-        double* pj = As + lane * ld;
-        for (int j = lane; j < n; j += 32, pj += 32 * ld) {
-          const double u = pj[k];
-          pj[k] = pj[p];
-          pj[p] = u;
+        for (int rr = 0; rr < RPL; ++rr) {
+          const int i = lane + 32 * rr;
+          mine[rr] = i > k && i < n;
+          l[rr] = 0.0;
+          if (mine[rr]) {
+            l[rr] = colk[i] * rinv;
+            colk[i] = l[rr];
+            bs[i] = fma(-l[rr], bk, bs[i]);
+          }
         }
-        if (lane == 0) {
-          const double u = bs[k];
-          bs[k] = bs[p];
-          bs[p] = u;
+        // the remaining columns of the panel (at most kNB - 1)
+        const double* pk = colk + ld + k;
+        double* pl = colk + ld + lane;
+        for (int j = k + 1; j < k0 + nb; ++j, pk += ld, pl += ld) {
+          const double akj = *pk;
+#pragma unroll
+          for (int rr = 0; rr < RPL; ++rr)
+            if (mine[rr]) pl[32 * rr] = fma(-l[rr], akj, pl[32 * rr]);
+        }
+        __syncwarp();
+      }
+      if (fail) break;
+      const int jt = k0 + nb;   // first trailing column
+      if (jt >= n) break;
+      // ---- U12: the pivot rows of the trailing columns, forward substitution with the unit-lower panel
+      // block; lanes over columns (a column's nb entries are contiguous, columns an odd stride apart)
+      for (int j = jt + lane; j < n; j += 32) {
+        double* cj = As + (size_t)j * ld + k0;
+        double u[kNB];
+#pragma unroll
+        for (int t = 0; t < kNB; ++t) u[t] = t < nb ? cj[t] : 0.0;
+#pragma unroll
+        for (int t = 1; t < kNB; ++t) {
+          if (t < nb) {
+#pragma unroll
+            for (int s2 = 0; s2 < t; ++s2) u[t] = fma(-As[(size_t)(k0 + s2) * ld + k0 + t], u[s2], u[t]);
+            cj[t] = u[t];
+          }
         }
       }
       __syncwarp();
-      const double piv = colk[k];
-      const double bk = bs[k];
-      double l[RPL];
-      bool mine[RPL];
+      // ---- A22 -= L21 U12: lanes over rows, the nb multipliers of each row in registers, two columns per trip
+      double lm[RPL][kNB];
+      bool below[RPL];
 #pragma unroll
       for (int rr = 0; rr < RPL; ++rr) {
         const int i = lane + 32 * rr;
-        mine[rr] = i > k && i < n;
-        l[rr] = 0.0;
-        if (mine[rr]) {
-          l[rr] = colk[i] / piv;
-          colk[i] = l[rr];
-          bs[i] = fma(-l[rr], bk, bs[i]);
-        }
+        below[rr] = i >= jt && i < n;
+#pragma unroll
+        for (int t = 0; t < kNB; ++t) lm[rr][t] = (below[rr] && t < nb) ? As[(size_t)(k0 + t) * ld + i] : 0.0;
       }
-      // rank-1 update of the trailing columns, kCB columns per trip: all loads of a trip are issued before
-      // its first store (stores to As would otherwise order every later load behind them)
-      constexpr int kCB = RPL <= 2 ? 8 : 4;
-      const double* pk = colk + ld + k;      // pivot-row entry of the current column
-      double* pl = colk + ld + lane;         // this lane's first row of the current column
-      int j0 = k + 1;
-      for (; j0 + kCB <= n; j0 += kCB) {
-        double akj[kCB], av[kCB][RPL];
-        const double* qk = pk;
-        const double* ql = pl;
+      double* cu = As + (size_t)jt * ld + k0;     // U12 entries of the current column
+      double* cl = As + (size_t)jt * ld + lane;   // this lane's rows of the current column
+      int j = jt;
+      for (; j + 2 <= n; j += 2, cu += 2 * ld, cl += 2 * ld) {
+        double u0[kNB], u1[kNB], a0[RPL], a1[RPL];
 #pragma unroll
-        for (int u = 0; u < kCB; ++u, qk += ld, ql += ld) {
-          akj[u] = *qk;   // broadcast
-#pragma unroll
-          for (int rr = 0; rr < RPL; ++rr) av[u][rr] = mine[rr] ? ql[32 * rr] : 0.0;
+        for (int t = 0; t < kNB; ++t) {
+          u0[t] = cu[t];          // entries beyond nb belong to other rows; their multipliers are 0
+          u1[t] = cu[ld + t];
         }
 #pragma unroll
-        for (int u = 0; u < kCB; ++u, pk += ld, pl += ld)
+        for (int rr = 0; rr < RPL; ++rr) {
+          a0[rr] = below[rr] ? cl[32 * rr] : 0.0;
+          a1[rr] = below[rr] ? cl[ld + 32 * rr] : 0.0;
+        }
 #pragma unroll
-          for (int rr = 0; rr < RPL; ++rr)
-            if (mine[rr]) pl[32 * rr] = fma(-l[rr], akj[u], av[u][rr]);
+        for (int t = 0; t < kNB; ++t)
+#pragma unroll
+          for (int rr = 0; rr < RPL; ++rr) {
+            a0[rr] = fma(-lm[rr][t], u0[t], a0[rr]);
+            a1[rr] = fma(-lm[rr][t], u1[t], a1[rr]);
+          }
+#pragma unroll
+        for (int rr = 0; rr < RPL; ++rr) {
+          if (below[rr]) {
+            cl[32 * rr] = a0[rr];
+            cl[ld + 32 * rr] = a1[rr];
+          }
+        }
       }
-      for (; j0 < n; ++j0, pk += ld, pl += ld) {
-        const double akj = *pk;
+      if (j < n) {
+        double a0[RPL];
+#pragma unroll
+        for (int rr = 0; rr < RPL; ++rr) a0[rr] = below[rr] ? cl[32 * rr] : 0.0;
+#pragma unroll
+        for (int t = 0; t < kNB; ++t) {
+          const double ut = cu[t];
+#pragma unroll
+          for (int rr = 0; rr < RPL; ++rr) a0[rr] = fma(-lm[rr][t], ut, a0[rr]);
+        }
 #pragma unroll
         for (int rr = 0; rr < RPL; ++rr)
-          if (mine[rr]) pl[32 * rr] = fma(-l[rr], akj, pl[32 * rr]);
+          if (below[rr]) cl[32 * rr] = a0[rr];
       }
       __syncwarp();
     }
@@ -141,7 +209,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
       // back substitution, column oriented: x_i = b_i / u_ii, then b_r -= u_ri x_i for r < i
       const double* coli = As + (size_t)(n - 1) * ld;
       for (int i = n - 1; i >= 0; --i, coli -= ld) {
-        const double xi = bs[i] / coli[i];
+        const double xi = bs[i] * dinv[i];
         __syncwarp();
         if (lane == 0) bs[i] = xi;
 #pragma unroll
@@ -161,7 +229,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
                             cudaStream_t st) {
   const int ld = n | 1;
-  const int sys_doubles = n * ld + ((n + 1) & ~1);
+  const int sys_doubles = n * ld + 2 * n + (n & 1);   // matrix, right-hand side, pivot reciprocals; even
   const size_t per_sys = (size_t)sys_doubles * 8;
   if (per_sys > smem_optin) return cudaErrorInvalidConfiguration;
   // systems (warps) per CTA: the count, up to 4, that packs the most systems into one SM's shared memory
