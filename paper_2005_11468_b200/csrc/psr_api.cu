@@ -238,6 +238,10 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   // shared memory left for the q tile and the chunk ring beside one C tile and the per-CTA scratch
   const size_t smem_fixed = align_up((size_t)(K + 2) * kTile * rl * 8, 128) + (size_t)nw * kTile * rl * 8 +
                             (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages);
+  // Y-column launch of psr_fd_jacobian: dense column packing for small mechanisms (a tile then spans several
+  // reactors and needs their rate-table slices side by side), whole tiles per reactor for large ones
+  const bool jy_dense = K <= 64;
+  const int jy_slices = jy_dense ? 31 / K + 2 : 1;
   int n_chunks = 0, rc = 0;
   bool resident = false;
   int ring_stages = 2;
@@ -408,7 +412,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   // gather pass
   // q tile plus the rate-table slice of one chunk (Y-column launch of psr_fd_jacobian)
   // (the q tile also hosts the 3 x nw partial-sum rows of the energy row, hence the lower bound)
-  const size_t q_bytes = align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128) + align_up((size_t)rc * kRateVals * 8, 128);
+  const size_t tab_bytes_smem = align_up((size_t)jy_slices * rc * kRateVals * 8, 128);   // slices of the reactors a column tile spans
+  const size_t q_bytes = align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128) + tab_bytes_smem;
   resident = n_chunks <= kMaxStages && smem_fixed + q_bytes + stride * n_chunks <= (size_t)prop.sharedMemPerBlockOptin &&
              (n_chunks == 1 || stride * n_chunks <= 48 * 1024);
   ring_stages = 2;
@@ -438,6 +443,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.rc = rc;
   v.resident = resident ? 1 : 0;
   v.ring_stages = ring_stages;
+  v.jy_dense = jy_dense ? 1 : 0;
   v.need_lnctot = need_lnctot;
   v.chunk_stride = (uint32_t)stride;
   const size_t cbuf_bytes = align_up((size_t)(K + 2) * kTile * rl * 8, 128);  // K+2 rows so the Jacobian staging [tile][n|1] fits
@@ -449,10 +455,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     o += align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128);  // + the all-zero row; >= energy-row scratch
     v.smem_mech = (uint32_t)o;
     o += stride * (resident ? n_chunks : ring_stages);
-    v.smem_tab = (uint32_t)o;
-    o += align_up((size_t)rc * kRateVals * 8, 128);
     v.smem_misc = (uint32_t)o;
-    o += (size_t)nw * kTile * rl * 8 + (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages);  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P prefetch; mbarriers
+    o += align_up((size_t)nw * kTile * rl * 8 + (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages), 128);  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P prefetch; mbarriers
+    // the rate-table slices come last: only the Y-column launch of psr_fd_jacobian asks for them, every other
+    // launch requests smem_tab bytes and leaves the rest of the SM's 256 KB to the L1 cache
+    v.smem_tab = (uint32_t)o;
+    o += align_up((size_t)jy_slices * rc * kRateVals * 8, 128);
     v.smem_total = (uint32_t)o;
     v.n_cbuf = n_cbuf;
     return o;
@@ -648,6 +656,7 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
   int64_t Nb = std::max<int64_t>(1, (int64_t)((size_t)64 * 1024 * 1024 / row_bytes));
   if (Nb > wave) Nb -= Nb % wave;
   Nb = std::min(Nb, N);
+  Nb = std::min<int64_t>(Nb, ((int64_t)1 << 31) / (n + 32) - 1);   // state indices of a launch fit 32 bits
   bool unhoisted = false;   // diagnostic: every column a full evaluation (tests compare the two sweeps)
   if (const char* e = getenv("PSR_JAC_UNHOISTED")) unhoisted = atoi(e) != 0;
 
@@ -665,7 +674,6 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
   double* tab = m->d_scratch;
   if (!F0) F0 = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(m->d_scratch) + tab_bytes);
 
-  const int tpr = (int)((K + 31) / 32);
   for (int64_t r0 = 0; r0 < N; r0 += Nb) {
     const int64_t nb = std::min(Nb, N - r0);
     EvalArgs a{};
@@ -695,7 +703,9 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
     if (st != PSR_OK) return st;
     b.flags = kModeJacY | en;                  // columns 1..K: T-only factors from the rate table
     b.tab = tab;
-    b.n_tiles = nb * tpr;
+    // states = (reactor, species column): packed densely, or padded to whole tiles per reactor (MechView::jy_dense)
+    const int64_t Kp = m->view.jy_dense ? K : (K + m->tile - 1) / m->tile * m->tile;
+    b.n_tiles = (nb * Kp + m->tile - 1) / m->tile;
     st = run(m, b, stream, "psr_fd_jacobian (Y columns)");
     if (st != PSR_OK) return st;
   }

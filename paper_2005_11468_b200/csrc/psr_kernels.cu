@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   double* lnctot_s = ctot_s + TR;                                     // [TR]: ln C_tot (formed on first use)
   double* tp = lnctot_s + TR;                                         // [2][2][TR]: prefetched T, P
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [kMaxStages] chunk stages, [kMaxStages] rate table
-  double* tab_s = reinterpret_cast<double*>(smem + mv.smem_tab);      // [rc][kRateVals]: this reactor's slice (JY)
+  double* tab_s = reinterpret_cast<double*>(smem + mv.smem_tab);      // [kslices][rc][kRateVals]: rate table slices of the tile's reactors (JY)
   double* en_s = qs;   // [3][NW][TR]: partial sums of the energy row (the q tile is free after the last gather)
 
   const int lane = threadIdx.x & 31;
@@ -129,7 +129,12 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   const int n = K + 1;
   const bool jac = (a.flags & (kModeJac | kModeJacT | kModeJacY)) != 0;
   const bool jacT = (a.flags & kModeJacT) != 0;
-  const int tpr = (K + 31) / 32;   // JY: tiles per reactor
+  // JY: state v = reactor * Kp + species column; a tile is 32 consecutive states.  Small mechanisms pack the
+  // columns densely (Kp = K: a tile spans up to 31/K + 2 reactors, whose rate-table slices sit side by side
+  // in tab_s); large ones (K > 64, where padding wastes little and shared memory is short) pad every
+  // reactor to whole tiles (Kp = 32 ceil(K/32): one reactor, one slice per tile).
+  const int Kp = mv.jy_dense ? K : ((K + 31) / 32) * 32;
+  const int64_t n_states = a.N * Kp;
   const bool resident = mv.resident != 0;   // every chunk blob has its own stage and is loaded once per CTA
   const int nstage = resident ? mv.n_chunks : mv.ring_stages;
   const int cs_elems = (K + 2) * TR;
@@ -185,11 +190,13 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   auto state_of = [&](int64_t t, int i, int64_t& r_, int& jsp_, bool& valid_) {
     const int64_t v = t * TR + i * 32 + lane;
     if constexpr (JY) {
-      const uint32_t tr = (uint32_t)t / (uint32_t)tpr;   // tiles of a sub-batch fit 32 bits (psr_fd_jacobian)
-      r_ = tr;
-      const int j = (int)((uint32_t)t - tr * (uint32_t)tpr) * 32 + lane;
-      valid_ = j < K;
-      jsp_ = valid_ ? j : -2;         // lanes beyond the last species evaluate the unperturbed state, unused
+      valid_ = v < n_states;
+      const uint32_t vv = (uint32_t)(valid_ ? v : n_states - 1);   // states of a sub-batch fit 32 bits (psr_fd_jacobian)
+      const uint32_t rr = vv / (uint32_t)Kp;
+      const int j = (int)(vv - rr * (uint32_t)Kp);
+      r_ = rr;
+      valid_ = valid_ && j < K;
+      jsp_ = valid_ ? j : -2;   // padding lanes evaluate an unperturbed state, unused
     } else if (jacT) {
       valid_ = v < a.N;
       r_ = valid_ ? v : a.N - 1;
@@ -225,13 +232,22 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
   prefetch(blockIdx.x, 0);
-  // JY: bulk copy of the rate-table slice of tile t's reactor for chunk c into tab_s (thread 0 only)
+  // JY: bulk copies of the rate-table slices of tile t's reactors for chunk c into tab_s (thread 0 only)
+  auto tile_reactors = [&](int64_t t, uint32_t& r_first, uint32_t& r_last) {
+    const int64_t v0 = t * TR, v1 = min(v0 + TR, n_states) - 1;
+    r_first = (uint32_t)v0 / (uint32_t)Kp;
+    r_last = (uint32_t)v1 / (uint32_t)Kp;
+  };
   auto load_tab = [&](int64_t t, int c) {
     const int b0 = mv.chunk_rec_base[c], b1 = mv.chunk_rec_base[c + 1];
     const uint32_t bytes = (uint32_t)(b1 - b0) * (kRateVals * 8);
+    uint32_t r0, r1;
+    tile_reactors(t, r0, r1);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    mbar_expect_tx(&bars[kMaxStages], bytes);
-    bulk_g2s(tab_s, a.tab + ((size_t)((uint32_t)t / (uint32_t)tpr) * mv.I + b0) * kRateVals, bytes, &bars[kMaxStages]);
+    mbar_expect_tx(&bars[kMaxStages], bytes * (r1 - r0 + 1));
+    for (uint32_t rr = r0; rr <= r1; ++rr)
+      bulk_g2s(tab_s + (size_t)(rr - r0) * mv.rc * kRateVals, a.tab + ((size_t)rr * mv.I + b0) * kRateVals, bytes,
+               &bars[kMaxStages]);
   };
   int64_t gt = 0;  // rate-table slices consumed so far by this CTA
   if constexpr (JY) {
@@ -485,6 +501,16 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       // table form and a lane only notes an out-of-range argument; the CTA then repeats the phase with
       // the library exp (IEEE results for NaN, Inf, overflow, gradual underflow).  That never happens for
       // physical states, so the range test costs two compares per reaction and no vote or branch.
+      const double* tvb = tab_s;   // JY: the table slice of this lane's reactor
+      if constexpr (JY) {
+        int64_t r_;
+        int jsp_;
+        bool valid_;
+        uint32_t r0, r1;
+        state_of(tile, 0, r_, jsp_, valid_);
+        tile_reactors(tile, r0, r1);
+        tvb = tab_s + (size_t)((uint32_t)r_ - r0) * mv.rc * kRateVals;
+      }
       float amax = 0.0f;   // NaN-propagating running max of |high word| of every exp argument of this lane
       auto run_class = [&](auto cls_tag, auto fast_tag, auto out_tag) {
         constexpr int CLS = decltype(cls_tag)::value;
@@ -522,7 +548,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           const RxRec* rec = recs + kl;
           const uint32_t meta = rec->meta;
           const int type = CLS < kClsLong ? CLS : (int)(meta & kMetaTypeMask);
-          const double* tv = tab_s + kl * kRateVals;   // JY: the reactor's T-only factors of this reaction
+          const double* tv = tvb + kl * kRateVals;     // JY: the T-only factors of this reaction for the lane's reactor
           double lnkf[R], lnkr[R], pf[R], pr[R], kf[R], kr[R], M[R];
           // Eq. 6 in log form, and ln k_r = ln k_f - ln K_c (Eq. 7-9 summed per reaction at load time)
           if constexpr (!JY) {
@@ -776,7 +802,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           else run_out(fast_tag, std::integral_constant<int, 0>{});
         }
       };
-      if constexpr (JY) mbar_wait(&bars[kMaxStages], (uint32_t)(gt & 1));   // this reactor's rate table slice
+      if constexpr (JY) mbar_wait(&bars[kMaxStages], (uint32_t)(gt & 1));   // the rate table slices of this tile
       run_all(std::true_type{});
       if (__syncthreads_or(!exp_max_in_range(amax))) {   // also the barrier that publishes the q tile
         run_all(std::false_type{});
@@ -944,14 +970,16 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       }
       __syncthreads();
       if constexpr (JY) {
-        // columns 1 + cb*32 .. of reactor r: contiguous in J (column-major per reactor)
-        const int64_t r_ = (uint32_t)tile / (uint32_t)tpr;
-        const int cb = (int)(tile - r_ * tpr);
-        const int ncol = min(32, K - cb * 32);
-        double* dst = a.J + (r_ * n + 1 + cb * 32) * (int64_t)n;
-        for (int idx = threadIdx.x; idx < ncol * n; idx += NW * 32) {
+        // state l of the tile is column 1 + j of reactor r: n contiguous doubles in J; consecutive states are
+        // consecutive columns except across a reactor boundary (the T column lies between)
+        for (int idx = threadIdx.x; idx < TR * n; idx += NW * 32) {
           const int l = idx / n, i = idx - l * n;
-          dst[idx] = stg[l * npad + i];
+          const int64_t v = tile * TR + l;
+          if (v < n_states) {
+            const uint32_t rr = (uint32_t)v / (uint32_t)Kp;
+            const uint32_t j = (uint32_t)v - rr * (uint32_t)Kp;
+            if (j < (uint32_t)K) a.J[((int64_t)rr * n + 1 + j) * n + i] = stg[l * npad + i];
+          }
         }
       } else if (jacT) {
         // column 0 of reactors tile*TR ..: n contiguous doubles each, n*n apart
@@ -982,7 +1010,8 @@ static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cud
   auto kern = psr_eval_kernel<NW, SPW, R, VAR>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mv.smem_total);
   if (e != cudaSuccess) return e;
-  kern<<<grid, NW * 32, mv.smem_total, st>>>(mv, a);
+  const uint32_t smem = (VAR & kVarJacY) ? mv.smem_total : mv.smem_tab;   // the table slices are the last region
+  kern<<<grid, NW * 32, smem, st>>>(mv, a);
   return cudaGetLastError();
 }
 

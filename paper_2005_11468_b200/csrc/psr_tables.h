@@ -89,6 +89,7 @@ struct MechView {
   int32_t n_chunks, rc;
   int32_t need_lnctot;          // some Troe reaction has no efficiency list (uses ln C_tot)
   int32_t resident;             // every chunk blob stays in shared memory (loaded once per CTA)
+  int32_t jy_dense;             // Y-column launch packs the columns of consecutive reactors densely (K <= 64)
   int32_t ring_stages;          // otherwise: stages of the chunk ring (2, or 1 when only that fits)
   int32_t n_cbuf;               // C-tile buffers: 2 = the next tile's state is prefetched during this tile's chunks
   uint32_t chunk_stride;        // bytes, multiple of 16
