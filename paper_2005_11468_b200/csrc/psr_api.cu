@@ -236,8 +236,11 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   int rc_target = std::min(I, 384);
   if (const char* e = getenv("PSR_RC")) rc_target = std::min(std::min(I, kMaxChunkRx), std::max(8, atoi(e)));
   // shared memory left for the q tile and the chunk ring beside one C tile and the per-CTA scratch
+  // Y - Y_in tile beside every C tile when the species' accumulators live in registers (spw <= 4); it shares
+  // its region with the rate-table slices, which only the Y-column launch (that has no such tile) uses
+  const size_t ds_bytes = spw <= 4 ? align_up((size_t)K * kTile * rl * 8, 128) : 0;
   const size_t smem_fixed = align_up((size_t)(K + 2) * kTile * rl * 8, 128) + (size_t)nw * kTile * rl * 8 +
-                            (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages);
+                            (size_t)11 * kTile * rl * 8 + 8 * (2 * kMaxStages);
   // Y-column launch of psr_fd_jacobian: dense column packing for small mechanisms (a tile then spans several
   // reactors and needs their rate-table slices side by side), whole tiles per reactor for large ones
   const bool jy_dense = K <= 64;
@@ -412,7 +415,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   // gather pass
   // q tile plus the rate-table slice of one chunk (Y-column launch of psr_fd_jacobian)
   // (the q tile also hosts the 3 x nw partial-sum rows of the energy row, hence the lower bound)
-  const size_t tab_bytes_smem = align_up((size_t)jy_slices * rc * kRateVals * 8, 128);   // slices of the reactors a column tile spans
+  const size_t tab_bytes_smem = std::max(align_up((size_t)jy_slices * rc * kRateVals * 8, 128), ds_bytes);   // slices of the reactors a column tile spans | one Y - Y_in tile
   const size_t q_bytes = align_up((size_t)std::max(rc + 1, 3 * nw) * kTile * rl * 8, 128) + tab_bytes_smem;
   resident = n_chunks <= kMaxStages && smem_fixed + q_bytes + stride * n_chunks <= (size_t)prop.sharedMemPerBlockOptin &&
              (n_chunks == 1 || stride * n_chunks <= 48 * 1024);
@@ -456,11 +459,10 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     v.smem_mech = (uint32_t)o;
     o += stride * (resident ? n_chunks : ring_stages);
     v.smem_misc = (uint32_t)o;
-    o += align_up((size_t)nw * kTile * rl * 8 + (size_t)9 * kTile * rl * 8 + 8 * (2 * kMaxStages), 128);  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P prefetch; mbarriers
-    // the rate-table slices come last: only the Y-column launch of psr_fd_jacobian asks for them, every other
-    // launch requests smem_tab bytes and leaves the rest of the SM's 256 KB to the L1 cache
+    o += align_up((size_t)nw * kTile * rl * 8 + (size_t)11 * kTile * rl * 8 + 8 * (2 * kMaxStages), 128);  // partial sums; ln T, h, rho, C_tot, ln C_tot, T/P/tau prefetch; mbarriers
+    // the rate-table slices of the Y-column launch of psr_fd_jacobian | the Y - Y_in tiles of every other launch
     v.smem_tab = (uint32_t)o;
-    o += align_up((size_t)jy_slices * rc * kRateVals * 8, 128);
+    o += std::max(align_up((size_t)jy_slices * rc * kRateVals * 8, 128), n_cbuf * ds_bytes);
     v.smem_total = (uint32_t)o;
     v.n_cbuf = n_cbuf;
     return o;

@@ -106,6 +106,10 @@ template <int NW, int SPW, int R, int VAR>
 __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const MechView mv, const EvalArgs a) {
   constexpr bool JY = (VAR & kVarJacY) != 0;
   constexpr bool EN = (VAR & kVarEnergy) != 0;
+  // DS: the epilogue's operands Y - Y_in and tau come with the tile's prefetch (shared memory) instead of
+  // being loaded into registers before the last gather, where they were spilled at once (measured: the
+  // spill stores waited for the loads, 5 % of the kernel)
+  constexpr bool DS = SPW <= 4 && !EN && !JY;   // (the Y-column launch has registers to spare and keeps the loads)
   static_assert(!JY || R == 1, "the Y-column mode maps one column to a lane");
   constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
@@ -118,9 +122,10 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   double* rho_s = hs + TR;                                            // [TR]: density per state
   double* ctot_s = rho_s + TR;                                        // [TR]: C_tot per state
   double* lnctot_s = ctot_s + TR;                                     // [TR]: ln C_tot (formed on first use)
-  double* tp = lnctot_s + TR;                                         // [2][2][TR]: prefetched T, P
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 4 * TR);          // [kMaxStages] chunk stages, [kMaxStages] rate table
+  double* tp = lnctot_s + TR;                                         // [2][3][TR]: prefetched T, P, tau
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tp + 6 * TR);          // [kMaxStages] chunk stages, [kMaxStages] rate table
   double* tab_s = reinterpret_cast<double*>(smem + mv.smem_tab);      // [kslices][rc][kRateVals]: rate table slices of the tile's reactors (JY)
+  double* Ds0 = reinterpret_cast<double*>(smem + mv.smem_tab);        // [2][K][TR]: Y_in, then Y - Y_in, of the tile (DS; shares the region of the JY table slices)
   double* en_s = qs;   // [3][NW][TR]: partial sums of the energy row (the q tile is free after the last gather)
 
   const int lane = threadIdx.x & 31;
@@ -138,6 +143,8 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   const bool resident = mv.resident != 0;   // every chunk blob has its own stage and is loaded once per CTA
   const int nstage = resident ? mv.n_chunks : mv.ring_stages;
   const int cs_elems = (K + 2) * TR;
+  const int ds_elems = K * TR;
+  const bool wantF = jac || (a.flags & (kOutF | kOutF0)) != 0;
   const uint32_t q_lane = smem_u32(qs) + lane * (8 * R);
 
   const int64_t my_tiles = (a.n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
@@ -223,10 +230,14 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         state_of(t, i, r_, jsp_, valid_);
         const int col = lane * R + i;
         if (w == 0) {
-          cp_async8(tp + (buf * 2 + 0) * TR + col, a.T + r_);
-          cp_async8(tp + (buf * 2 + 1) * TR + col, a.P + r_);
+          cp_async8(tp + (buf * 3 + 0) * TR + col, a.T + r_);
+          cp_async8(tp + (buf * 3 + 1) * TR + col, a.P + r_);
+          if (DS && wantF) cp_async8(tp + (buf * 3 + 2) * TR + col, a.tau + r_);
         }
-        for_species([&](int, int s) { cp_async8(Cs0 + buf * cs_elems + s * TR + col, a.Y + (int64_t)s * a.ld + r_); });
+        for_species([&](int, int s) {
+          cp_async8(Cs0 + buf * cs_elems + s * TR + col, a.Y + (int64_t)s * a.ld + r_);
+          if (DS && wantF) cp_async8(Ds0 + buf * ds_elems + s * TR + col, a.Yin + (int64_t)s * a.ld + r_);
+        });
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -260,6 +271,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x, buf ^= (mv.n_cbuf - 1)) {
     // ---------------------------------------------------------------- prologue (a1)
     double* Cs = Cs0 + buf * cs_elems;
+    double* Ds = Ds0 + buf * ds_elems;
     const uint32_t c_lane = smem_u32(Cs) + lane * (8 * R);   // this lane's R slots of row 0 of the C tile
     asm volatile("cp.async.wait_group 0;" ::: "memory");   // this thread's prefetched entries have landed
 
@@ -305,8 +317,8 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       if (mv.n_cbuf == 2) prefetch(tile + gridDim.x, buf ^ 1);
 #pragma unroll
       for (int i = 0; i < R; ++i) {
-        T[i] = tp[(buf * 2 + 0) * TR + lane * R + i];
-        const double P = tp[(buf * 2 + 1) * TR + lane * R + i];
+        T[i] = tp[(buf * 3 + 0) * TR + lane * R + i];
+        const double P = tp[(buf * 3 + 1) * TR + lane * R + i];
         if (jsp[i] == -1) {
           const double Tp = T[i] + 1e-8 * fmax(fabs(T[i]), 1e-10);
           if (w == 0) hs[lane * R + i] = Tp - T[i];
@@ -330,7 +342,11 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       for_species([&](int, int s) {
         const double iw = mv.invW[s];
 #pragma unroll
-        for (int i = 0; i < R; ++i) Cs[s * TR + lane * R + i] = rho[i] * (Cs[s * TR + lane * R + i] * iw);
+        for (int i = 0; i < R; ++i) {
+          const double y = Cs[s * TR + lane * R + i];   // the perturbed value where this state perturbs s
+          if (DS && wantF) Ds[s * TR + lane * R + i] = y - Ds[s * TR + lane * R + i];
+          Cs[s * TR + lane * R + i] = rho[i] * (y * iw);
+        }
       });
     }
     __syncthreads();
@@ -346,8 +362,6 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     for (int jj = 0; jj < SPR; ++jj)
 #pragma unroll
       for (int i = 0; i < R; ++i) acc[jj][i] = 0.0;
-
-    const bool wantF = jac || (a.flags & (kOutF | kOutF0)) != 0;
 
     // ---------------------------------------------------------------- chunks
     int stage = 0;
@@ -829,12 +843,14 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       if (wantF) {
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-          e_tau[i] = ldg_nc(a.tau + r[i]);
+          e_tau[i] = DS ? tp[(buf * 3 + 2) * TR + lane * R + i] : ldg_nc(a.tau + r[i]);
           if constexpr (!GA) {
             for_species([&](int jj, int s) {
               const int64_t o = (int64_t)s * a.ld + r[i];
-              e_y[jj][i] = ldg_nc(a.Y + o);
-              e_yin[jj][i] = ldg_nc(a.Yin + o);
+              if constexpr (!DS) {
+                e_y[jj][i] = ldg_nc(a.Y + o);
+                e_yin[jj][i] = ldg_nc(a.Yin + o);
+              }
               if (jac) e_f0[jj][i] = ldg_nc(a.F0 + r[i] * n + 1 + s);
             });
           }
@@ -914,7 +930,8 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               const int64_t o = (int64_t)s * a.ld + r[i];
               if (a.flags & kOutWdot) a.wdot[o] = acc[jj][i];
               if (wantF) {
-                const double Fv = fma(e_y[jj][i] - e_yin[jj][i], invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
+                const double dy = DS ? Ds[s * TR + lane * R + i] : e_y[jj][i] - e_yin[jj][i];
+                const double Fv = fma(dy, invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
                 if (a.flags & kOutF) a.F[o] = Fv;
                 if (a.flags & kOutF0) a.F0out[r[i] * n + 1 + s] = Fv;
                 if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), e_y[jj][i], e_yin[jj][i], acc[jj][i]);
@@ -950,9 +967,15 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         for (int jj = 0; jj < SPW; ++jj) {
           const int s = sp[jj];
           if (s >= 0) {
-            double y = e_y[jj][i];
-            if (s == jsp[i]) y = y + 1e-8 * fmax(fabs(y), 1e-10);   // the same x' as in the prologue
-            const double Fv = fma(y - e_yin[jj][i], invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
+            double y = 0.0, dy;
+            if constexpr (DS) {
+              dy = Ds[s * TR + lane * R + i];   // formed in the prologue from the perturbed y
+            } else {
+              y = e_y[jj][i];
+              if (s == jsp[i]) y = y + 1e-8 * fmax(fabs(y), 1e-10);   // the same x' as in the prologue
+              dy = y - e_yin[jj][i];
+            }
+            const double Fv = fma(dy, invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
             stg[st * npad + 1 + s] = (Fv - e_f0[jj][i]) * invh;
             if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), y, e_yin[jj][i], acc[jj][i]);
           }
@@ -1003,14 +1026,18 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 }
 
 // ------------------------------------------------------------------ launch wrapper
+#ifdef PSR_EXP_SHAPES   // development builds: one shape compiles in a third of the time
+#define PSR_SHAPES(X) X(16, 4)
+#else
 #define PSR_SHAPES(X) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)
+#endif
 
 template <int NW, int SPW, int R, int VAR>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
   auto kern = psr_eval_kernel<NW, SPW, R, VAR>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mv.smem_total);
   if (e != cudaSuccess) return e;
-  const uint32_t smem = (VAR & kVarJacY) ? mv.smem_total : mv.smem_tab;   // the table slices are the last region
+  const uint32_t smem = mv.smem_total;
   kern<<<grid, NW * 32, smem, st>>>(mv, a);
   return cudaGetLastError();
 }
