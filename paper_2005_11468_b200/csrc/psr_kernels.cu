@@ -557,10 +557,33 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           state_of(tile, i, r_, jsp_, valid_);
           return a.tab_out + ((size_t)r_ * mv.I + hdr->rec_base + kl) * kRateVals;
         };
+        // The slot offsets (and meta, korig) of a record are read one trip ahead: they head the longest
+        // chain of the trip (offsets -> C tile loads -> products), and read at the top of their own trip
+        // they cost a shared-memory round trip before anything else can start.  Reading one record past
+        // the warp's range stays inside the chunk blob.
+        // (Not in the energy-row instantiation, whose epilogue operands leave no registers for it.)
+        constexpr int PF = EN ? 0 : 1;
+        uint4 nxa, nxb;
+        if constexpr (PF) {
+          const uint32_t ra = smem_u32(recs + kl_begin) + 80;
+          asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(nxa.x), "=r"(nxa.y), "=r"(nxa.z), "=r"(nxa.w) : "r"(ra));
+          asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+16];" : "=r"(nxb.x), "=r"(nxb.y), "=r"(nxb.z), "=r"(nxb.w) : "r"(ra));
+        }
 #pragma unroll 1
         for (int kl = kl_begin; kl < kl_end; ++kl) {
           const RxRec* rec = recs + kl;
-          const uint32_t meta = rec->meta;
+          if constexpr (!PF) {
+            const uint32_t ra = smem_u32(rec) + 80;
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(nxa.x), "=r"(nxa.y), "=r"(nxa.z), "=r"(nxa.w) : "r"(ra));
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+16];" : "=r"(nxb.x), "=r"(nxb.y), "=r"(nxb.z), "=r"(nxb.w) : "r"(ra));
+          }
+          const uint4 ra_ = nxa, rb_ = nxb;   // {meta, off[0..2]}, {off[3..5], korig} of this record
+          if constexpr (PF) {
+            const uint32_t ra = smem_u32(rec) + (112 + 80);
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(nxa.x), "=r"(nxa.y), "=r"(nxa.z), "=r"(nxa.w) : "r"(ra));
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+16];" : "=r"(nxb.x), "=r"(nxb.y), "=r"(nxb.z), "=r"(nxb.w) : "r"(ra));
+          }
+          const uint32_t meta = ra_.x;
           const int type = CLS < kClsLong ? CLS : (int)(meta & kMetaTypeMask);
           const double* tv = tvb + kl * kRateVals;     // JY: the T-only factors of this reaction for the lane's reactor
           double lnkf[R], lnkr[R], pf[R], pr[R], kf[R], kr[R], M[R];
@@ -579,19 +602,19 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
           if constexpr (CLS < kClsLong) {
             double f0[R], f1[R], f2[R], p0[R], p1[R], p2[R];
-            RowIO<R>::ld(c_lane + rec->off[0], f0);
-            RowIO<R>::ld(c_lane + rec->off[1], f1);
-            RowIO<R>::ld(c_lane + rec->off[2], f2);
-            RowIO<R>::ld(c_lane + rec->off[3], p0);
-            RowIO<R>::ld(c_lane + rec->off[4], p1);
-            RowIO<R>::ld(c_lane + rec->off[5], p2);
+            RowIO<R>::ld(c_lane + ra_.y, f0);
+            RowIO<R>::ld(c_lane + ra_.z, f1);
+            RowIO<R>::ld(c_lane + ra_.w, f2);
+            RowIO<R>::ld(c_lane + rb_.x, p0);
+            RowIO<R>::ld(c_lane + rb_.y, p1);
+            RowIO<R>::ld(c_lane + rb_.z, p2);
 #pragma unroll
             for (int i = 0; i < R; ++i) {
               pf[i] = f0[i] * f1[i] * f2[i];
               pr[i] = p0[i] * p1[i] * p2[i];
             }
           } else {
-            const uint16_t* fsp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + rec->off[0];
+            const uint16_t* fsp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + ra_.y;
             const int nr = (int)((meta >> kMetaNrShift) & 0xF);
             const int np = (int)((meta >> kMetaNpShift) & 0xF);
 #pragma unroll
@@ -789,7 +812,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               bool valid_;
               state_of(tile, i, r_, jsp_, valid_);
               if (valid_) {
-                const int64_t o = (int64_t)rec->korig * a.ldk + r_;
+                const int64_t o = (int64_t)rb_.w * a.ldk + r_;
                 if (a.flags & kOutKf) a.kf[o] = kf[i];
                 if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr[i] : 0.0;
                 if (a.flags & kOutQ) a.q[o] = q[i];
@@ -1026,7 +1049,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 }
 
 // ------------------------------------------------------------------ launch wrapper
-#ifdef PSR_EXP_SHAPES   // development builds: one shape compiles in a third of the time
+#ifdef PSR_EXP_SHAPES   // development builds: fewer shapes compile in a fraction of the time
 #define PSR_SHAPES(X) X(16, 4)
 #else
 #define PSR_SHAPES(X) X(16, 2) X(16, 4) X(16, 8) X(16, 16) X(16, 32)

@@ -75,11 +75,13 @@ __device__ __forceinline__ void exp_core_n(const double (&x)[N], double (&y)[N],
     n[i] = __double2loint(t[i]);
     t[i] = t[i] - kMagic;
   }
+  // the table entries are requested now and first touched after the polynomial: a shuffle takes about as
+  // long as three dependent DFMAs, and a consumer placed right behind it stalls the warp for that time
+  int thi[N], tlo[N];
 #pragma unroll
   for (int i = 0; i < N; ++i) {
-    const int thi = __shfl_sync(kFullMask, tab.hi, n[i]);
-    const int tlo = __shfl_sync(kFullMask, tab.lo, n[i]);
-    tj[i] = __hiloint2double(thi + ((n[i] >> 5) << 20), tlo);
+    thi[i] = __shfl_sync(kFullMask, tab.hi, n[i]);
+    tlo[i] = __shfl_sync(kFullMask, tab.lo, n[i]);
   }
 #pragma unroll
   for (int i = 0; i < N; ++i) r[i] = fma(t[i], -kLn2o32Hi, x[i]);
@@ -97,6 +99,14 @@ __device__ __forceinline__ void exp_core_n(const double (&x)[N], double (&y)[N],
   for (int i = 0; i < N; ++i) s[i] = fma(s[i], r[i], 1.0);
 #pragma unroll
   for (int i = 0; i < N; ++i) s[i] = s[i] * r[i];
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    // 2^m * 2^(j/32): m = n >> 5 added to the exponent field.  The asm keeps the assembler from moving the
+    // integer work back up to the shuffles.
+    int hi;
+    asm volatile("mad.lo.s32 %0, %1, 32768, %2;" : "=r"(hi) : "r"(n[i] & ~31), "r"(thi[i]));
+    tj[i] = __hiloint2double(hi, tlo[i]);
+  }
 #pragma unroll
   for (int i = 0; i < N; ++i) y[i] = fma(tj[i], s[i], tj[i]);
 }
