@@ -154,6 +154,20 @@ def lu_solve(A, b, *, long_double: bool = False):
 _DETAIL_COLS = ("kinf", "k0", "Pr", "Fcent", "F", "M", "Kp", "Kc", "kf", "kr", "q")
 
 
+def ptc_step(J, F, dt, *, long_double: bool = False):
+    """NEXT-4: one pseudo-transient (implicit Euler) step (I/dt + J) dx = -F per system.
+    J: [N][n][n] with J[r, j, i] = entry (row i, column j); F: [N][n]; dt: [N].  Returns dx [N][n], info [N]."""
+    J = np.ascontiguousarray(J, dtype=np.float64)
+    F = np.ascontiguousarray(F, dtype=np.float64)
+    dt = np.ascontiguousarray(dt, dtype=np.float64)
+    N, n = F.shape
+    assert J.shape == (N, n, n) and dt.shape == (N,)
+    dx = np.empty_like(F)
+    info = np.zeros(N, dtype=np.int32)
+    lib().oracle_ptc_step(C.c_int64(N), C.c_int(n), _p(J), _p(F), _p(dt), _p(dx), _p(info), C.c_int(int(long_double)))
+    return dx, info
+
+
 def detail(mech: OracleMechanism, T: float, P: float, Y) -> dict:
     """Per-reaction intermediates of one reactor (for the pins)."""
     Y = np.ascontiguousarray(Y, dtype=np.float64).reshape(-1)

@@ -25,6 +25,8 @@
 //   F_T = 0 for an inert mechanism at T_in = T; linearity in 1/tau; enthalpy-balance identity.
 //   Linear solve (NEXT-2): exact rational solutions of small integer systems, a system that needs a row
 //   exchange, a singular system, LAPACK (numpy.linalg.solve) on random systems, backward error bound.
+//   Pseudo-transient step (NEXT-4): exact rational solutions, the Newton limit dt -> inf, the explicit-Euler
+//   limit dt -> 0 (dx -> -dt F), the scalar closed form dx = -F/(1/dt + J), LAPACK on the shifted matrix.
 //
 // Units (paper silent; CHEMKIN cgs, reading g4): T [K], P [dyn/cm^2], C [mol/cm^3],
 // rho [g/cm^3], W [g/mol], wdot [mol/cm^3/s], Ea [cal/mol].
@@ -419,6 +421,26 @@ int oracle_lu_solve(int64_t N, int n, const double* A, const double* b, double* 
     const double* Ar = A + (size_t)r * n * n;
     info[r] = use_long_double ? lu_solve_one<long double>(n, Ar, b + r * n, x + r * n)
                               : lu_solve_one<double>(n, Ar, b + r * n, x + r * n);
+  }
+  return 0;
+}
+
+// NEXT-4: one pseudo-transient (implicit Euler) step.  "If the Newton algorithm fails to converge, then the
+// solution estimate is conditioned by a pseudo-transient time integration of the governing equations"
+// (PAPER.md:44).  The transient equations are dx/dt = -F(x) (Eq. 2 with this build's sign of F); implicit
+// Euler over dt, linearised about x:  (x' - x)/dt = -F(x') ~ -F(x) - J (x' - x)   =>   (I/dt + J) dx = -F.
+// Written out as that: form A = J + I/dt entry by entry, b = -F, then the elimination above.
+// J: [N][n*n] column-major per system, F: [N][n], dt: [N] (> 0; +inf gives the Newton step), dx: [N][n].
+int oracle_ptc_step(int64_t N, int n, const double* J, const double* F, const double* dt, double* dx, int32_t* info,
+                    int use_long_double) {
+  std::vector<double> A((size_t)n * n), b(n);
+  for (int64_t r = 0; r < N; ++r) {
+    const double shift = 1.0 / dt[r];
+    for (int j = 0; j < n; ++j)
+      for (int i = 0; i < n; ++i) A[(size_t)j * n + i] = J[(size_t)r * n * n + (size_t)j * n + i] + (i == j ? shift : 0.0);
+    for (int i = 0; i < n; ++i) b[i] = -F[r * n + i];
+    info[r] = use_long_double ? lu_solve_one<long double>(n, A.data(), b.data(), dx + r * n)
+                              : lu_solve_one<double>(n, A.data(), b.data(), dx + r * n);
   }
   return 0;
 }

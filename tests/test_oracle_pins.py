@@ -563,3 +563,54 @@ def test_lu_solve_matches_lapack_and_is_backward_stable():
     assert np.all(res <= 8 * bound)
     xl, _ = orc.lu_solve(_colmajor(M), b, long_double=True)
     assert np.abs(x - xl).max() <= 1e-12 * np.abs(xl).max()
+
+
+# ------------------------------------------------------------------ pseudo-transient step
+def test_ptc_step_exact_rational_and_scalar_closed_form():
+    """(I/dt + J) dx = -F (implicit Euler on dx/dt = -F).  Expected values by exact rational
+    arithmetic on the shifted system, written out here; the scalar case is dx = -F/(1/dt + J)."""
+    from fractions import Fraction
+    J = [[2, 1], [1, 3]]
+    F = [3, 5]
+    dt = Fraction(1, 2)                              # 1/dt = 2 -> A = [[4, 1], [1, 5]], b = (-3, -5)
+    det = Fraction(4 * 5 - 1 * 1)
+    exact = [float((Fraction(-3) * 5 - Fraction(-5) * 1) / det), float((Fraction(4) * -5 - Fraction(1) * -3) / det)]
+    assert exact == [float(Fraction(-10, 19)), float(Fraction(-17, 19))]
+    dx, info = orc.ptc_step(_colmajor([J]), np.array([F], dtype=np.float64), np.array([float(dt)]))
+    assert info[0] == 0 and np.allclose(dx[0], exact, rtol=1e-15, atol=0)
+    # scalar systems: dx = -F / (1/dt + J)
+    Js = np.array([[[3.0]], [[-0.25]], [[1e6]]])
+    Fs = np.array([[2.0], [1.0], [-4.0]])
+    dts = np.array([0.5, 2.0, 1e-3])
+    dx, info = orc.ptc_step(Js, Fs, dts)
+    want = -Fs[:, 0] / (1.0 / dts + Js[:, 0, 0])
+    assert np.all(info == 0) and np.allclose(dx[:, 0], want, rtol=2e-16 * 4, atol=0)
+    # a transposed operand would show here: non-symmetric J
+    Jn = [[1, 4], [0, 1]]                            # dt = 1: A = [[2, 4], [0, 2]], b = (-2, -2) -> dx = (1, -1)
+    dx, _ = orc.ptc_step(_colmajor([Jn]), np.array([[2.0, 2.0]]), np.array([1.0]))
+    assert np.array_equal(dx[0], [1.0, -1.0])
+
+
+def test_ptc_step_limits_newton_and_explicit_euler():
+    rng = np.random.default_rng(44)
+    N, n = 8, 54
+    M = rng.standard_normal((N, n, n)) + 4.0 * np.eye(n)
+    F = rng.standard_normal((N, n))
+    # dt = inf: the shift vanishes and the step is the Newton step J dx = -F (NEXT-2's solve, LAPACK here)
+    dx, info = orc.ptc_step(_colmajor(M), F, np.full(N, np.inf))
+    newton = np.linalg.solve(M, -F[:, :, None])[:, :, 0]
+    assert np.all(info == 0) and np.abs(dx - newton).max() <= 1e-12 * np.abs(newton).max()
+    # dt -> 0: (I/dt + J)^-1 = dt (I - dt J + ...), so dx = -dt F + dt^2 J F + O(dt^3)
+    dt = np.full(N, 1e-7)
+    dx, _ = orc.ptc_step(_colmajor(M), F, dt)
+    euler = -dt[:, None] * F
+    second = dt[:, None] ** 2 * np.einsum("rij,rj->ri", M, F)
+    assert np.abs(dx - euler).max() <= 2e-7 * 60 * np.abs(euler).max()       # |dt J| ~ 1e-7 * ||J||
+    assert np.abs(dx - (euler + second)).max() <= 1e-11 * np.abs(euler).max()
+    # general dt against LAPACK on the shifted matrix, plus a system the shift makes singular
+    dt = 10.0 ** rng.uniform(-4, 1, N)
+    dx, info = orc.ptc_step(_colmajor(M), F, dt)
+    ref = np.linalg.solve(M + np.eye(n)[None] / dt[:, None, None], -F[:, :, None])[:, :, 0]
+    assert np.all(info == 0) and np.abs(dx - ref).max() <= 1e-12 * np.abs(ref).max()
+    _, info = orc.ptc_step(np.array([[[-2.0]]]), np.array([[1.0]]), np.array([0.5]))   # 1/dt + J = 0
+    assert info[0] == 1
