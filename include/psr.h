@@ -139,6 +139,20 @@ psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double*
  * J dx = -F: pass b = -F0.  Asynchronous on `stream`. */
 psr_status psr_lu_solve(int64_t N, int32_t n, const double* A, double* b, int32_t* info, void* stream);
 
+/* One pseudo-transient (implicit Euler) step ("If the Newton algorithm
+ * fails to converge, then the solution estimate is conditioned by a pseudo-transient time integration of the
+ * governing equations"): the transient system dx/dt = -F(x) stepped by implicit Euler and linearised about x,
+ *     (I/dt + J) dx = -F,
+ * solved for N independent reactors by the elimination of psr_lu_solve (one warp per system; the shift and the
+ * sign are applied while J is staged into shared memory, so J and F are read once and not modified).
+ * J: DEVICE [N][n*n] column-major per system (psr_fd_jacobian's layout); F: DEVICE [N][n] residual at x (the F0 of
+ * psr_fd_jacobian); dt: DEVICE [N] pseudo-time step per reactor, > 0 (+inf gives the Newton step exactly);
+ * dx: DEVICE [N][n] out, must not alias F (unchanged for a system that fails); info: DEVICE [N] as in psr_lu_solve.
+ * The paper gives neither the step-size control nor the Newton/pseudo-transient switching constants ("See
+ * [5]"): choosing dt and accepting steps is the caller's.  Asynchronous on `stream`. */
+psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F, const double* dt, double* dx,
+                         int32_t* info, void* stream);
+
 /* Thread-local description of the last failure on this thread; valid until its next psr_* call. */
 const char* psr_last_error(void);
 

@@ -17,7 +17,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -70,6 +70,8 @@ def lib():
         L.psr_fd_jacobian_energy.restype = C.c_int
         L.psr_lu_solve.argtypes = [i64, C.c_int32, dp, dp, dp, vp]
         L.psr_lu_solve.restype = C.c_int
+        L.psr_ptc_solve.argtypes = [i64, C.c_int32, dp, dp, dp, dp, dp, vp]
+        L.psr_ptc_solve.restype = C.c_int
         L.psr_fd_jacobian.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_fd_jacobian.restype = C.c_int
         L.psr_last_error.argtypes = []
@@ -282,3 +284,20 @@ def lu_solve(A, b, info=None):
         info = torch.empty(N, dtype=torch.int32, device=b.device)
     _check(lib().psr_lu_solve(N, n, _ptr(A), _ptr(b), _ptr(info), _stream()))
     return b, info
+
+
+def ptc_solve(J, F, dt, dx=None, info=None):
+    """psr_ptc_solve: one pseudo-transient step (I/dt + J) dx = -F per reactor.  J [N][n][n] (J[r, col, row]),
+    F [N][n], dt [N]; returns (dx [N][n], info [N] int32)."""
+    import torch
+    N, n = F.shape
+    if J.shape != (N, n, n) or dt.shape != (N,) or not (J.is_contiguous() and F.is_contiguous() and dt.is_contiguous()):
+        raise ValueError("J must be contiguous [N][n][n], F contiguous [N][n], dt contiguous [N]")
+    for nm, t in (("J", J), ("F", F), ("dt", dt)):
+        _chk_dev(nm, t)
+    if dx is None:
+        dx = torch.empty_like(F)
+    if info is None:
+        info = torch.empty(N, dtype=torch.int32, device=F.device)
+    _check(lib().psr_ptc_solve(N, n, _ptr(J), _ptr(F), _ptr(dt), _ptr(dx), _ptr(info), _stream()))
+    return dx, info

@@ -21,7 +21,7 @@ cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalA
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm);
 cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st);
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
-                            cudaStream_t st);
+                            cudaStream_t st, const double* F, const double* dt);
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
 }  // namespace psr
 
@@ -733,20 +733,35 @@ psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double*
   return fd_jacobian_impl(mech, N, T, P, Y, Tin, Yin, tau, ld, J, F0, stream, "psr_fd_jacobian_energy");
 }
 
+static psr_status solve_impl(const char* who, int64_t N, int32_t n, const double* A, double* b, int32_t* info,
+                             const double* F, const double* dt, void* stream) {
+  int dev = 0, n_sm = 0, optin = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return cuda_fail(e, who);
+  if (n > 168) return fail(PSR_EUNSUPPORTED, "%s: n = %d, the one-warp-per-system kernel takes n <= 168", who, n);
+  e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream, F, dt);
+  if (e != cudaSuccess) return cuda_fail(e, who);
+  return PSR_OK;
+}
+
 psr_status psr_lu_solve(int64_t N, int32_t n, const double* A, double* b, int32_t* info, void* stream) {
   g_err.clear();
   if (N < 0 || n < 1) return fail(PSR_EINVAL, "psr_lu_solve: N < 0 or n < 1");
   if (N == 0) return PSR_OK;
   if (!A || !b || !info) return fail(PSR_EINVAL, "psr_lu_solve: null A, b or info");
-  int dev = 0, n_sm = 0, optin = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (e != cudaSuccess) return cuda_fail(e, "psr_lu_solve");
-  if (n > 168) return fail(PSR_EUNSUPPORTED, "psr_lu_solve: n = %d, the one-warp-per-system kernel takes n <= 168", n);
-  e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream);
-  if (e != cudaSuccess) return cuda_fail(e, "psr_lu_solve");
-  return PSR_OK;
+  return solve_impl("psr_lu_solve", N, n, A, b, info, nullptr, nullptr, stream);
+}
+
+psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F, const double* dt, double* dx,
+                         int32_t* info, void* stream) {
+  g_err.clear();
+  if (N < 0 || n < 1) return fail(PSR_EINVAL, "psr_ptc_solve: N < 0 or n < 1");
+  if (N == 0) return PSR_OK;
+  if (!J || !F || !dt || !dx || !info) return fail(PSR_EINVAL, "psr_ptc_solve: null J, F, dt, dx or info");
+  if (dx == F) return fail(PSR_EINVAL, "psr_ptc_solve: dx must not alias F");
+  return solve_impl("psr_ptc_solve", N, n, J, dx, info, F, dt, stream);
 }
 
 psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {

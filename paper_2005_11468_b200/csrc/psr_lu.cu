@@ -24,7 +24,8 @@ constexpr int kNB = 8;   // pivots per pass over the trailing matrix
 template <int RPL>
 __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const double* __restrict__ A,
                                                        double* __restrict__ b, int32_t* __restrict__ info,
-                                                       int sys_doubles) {
+                                                       int sys_doubles, const double* __restrict__ F,
+                                                       const double* __restrict__ dt) {
   extern __shared__ __align__(16) double sm[];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, wpc = blockDim.x >> 5;
   const int ld = n | 1;
@@ -34,6 +35,8 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
 
   for (int64_t r = (int64_t)blockIdx.x * wpc + w; r < N; r += (int64_t)gridDim.x * wpc) {
     const double* Ar = A + (size_t)r * n * n;
+    // pseudo-transient step (psr_ptc_solve): the matrix is J + I/dt, the right-hand side -F
+    const double shift = dt ? 1.0 / dt[r] : 0.0;
     {
       // column-major stream, 32 consecutive entries per trip, 4 trips in flight; (i, j) tracked without a divide
       int i = lane, j = 0;
@@ -45,6 +48,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
         for (int u = 0; u < 4; ++u) {
           off[u] = j * ld + i;
           v[u] = (t + 32 * u < n * n) ? Ar[t + 32 * u] : 0.0;
+          if (dt && i == j) v[u] += shift;
           i += 32;
           while (i >= n) { i -= n; ++j; }
         }
@@ -53,7 +57,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
           if (t + 32 * u < n * n) As[off[u]] = v[u];
       }
     }
-    for (int i = lane; i < n; i += 32) bs[i] = b[r * n + i];
+    for (int i = lane; i < n; i += 32) bs[i] = F ? -F[r * n + i] : b[r * n + i];
     __syncwarp();
 
     // Blocked right-looking elimination, kNB pivots per pass over the trailing matrix: every trailing entry
@@ -227,7 +231,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
 }
 
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
-                            cudaStream_t st) {
+                            cudaStream_t st, const double* F, const double* dt) {
   const int ld = n | 1;
   const int sys_doubles = n * ld + 2 * n + (n & 1);   // matrix, right-hand side, pivot reciprocals; even
   const size_t per_sys = (size_t)sys_doubles * 8;
@@ -250,7 +254,7 @@ cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_
     cudaError_t e = cudaFuncSetAttribute(lu_solve_kernel<RPL_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                          (int)smem);                                                         \
     if (e != cudaSuccess) return e;                                                                          \
-    lu_solve_kernel<RPL_><<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles);                 \
+    lu_solve_kernel<RPL_><<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles, F, dt);                 \
     return cudaGetLastError();                                                                               \
   }
   PSR_LU(1) PSR_LU(2) PSR_LU(4) PSR_LU(6)

@@ -515,6 +515,88 @@ def test_newton_step_on_device_matches_the_oracle_solve(torch_cuda, binding):
     assert np.all(np.abs(dx[:, 0]) <= 1e-8 * scale)      # fixed-temperature row: dT = -F_T = 0 up to the solve's round-off
 
 
+# ------------------------------------------------------------------ pseudo-transient step (NEXT-4)
+@pytest.mark.parametrize("n,N", [(1, 5), (3, 7), (33, 9), (54, 300), (101, 6), (168, 2)])
+def test_ptc_solve_random_systems(torch_cuda, binding, n, N):
+    """(I/dt + J) dx = -F element by element against the oracle (same shift, same sign, same elimination),
+    J and F left untouched, dt = inf bit-identical to psr_lu_solve on (J, -F)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(300 + n)
+    M = rng.standard_normal((N, n, n)) + 1.0 * np.eye(n)
+    F = rng.standard_normal((N, n))
+    dt = 10.0 ** rng.uniform(-3, 1, N)
+    J = np.ascontiguousarray(np.swapaxes(M, 1, 2))
+    Jd, Fd = dev(torch, J), dev(torch, F)
+    dx, info = binding.ptc_solve(Jd, Fd, dev(torch, dt))
+    torch.cuda.synchronize()
+    assert np.array_equal(Jd.cpu().numpy(), J) and np.array_equal(Fd.cpu().numpy(), F)
+    dx, info = dx.cpu().numpy(), info.cpu().numpy()
+    xr, ir = orc.ptc_step(J, F, dt)
+    assert np.array_equal(info, ir) and np.all(info == 0)
+    assert np.abs(dx - xr).max() <= 1e-11 * np.abs(xr).max()
+    A = J + (np.eye(n)[None] / dt[:, None, None])
+    ok, worst = _backward_error_ok(A, dx, -F, n)
+    assert ok, worst
+    # Newton limit: no shift
+    dxn, _ = binding.ptc_solve(Jd, Fd, dev(torch, np.full(N, np.inf)))
+    xn, _ = binding.lu_solve(Jd, (-Fd).contiguous())
+    torch.cuda.synchronize()
+    assert np.array_equal(dxn.cpu().numpy(), xn.cpu().numpy())
+
+
+def test_ptc_solve_edge_cases(torch_cuda, binding):
+    torch = torch_cuda
+    # a system the shift makes singular is flagged and its dx left as it was; N = 0 is a no-op
+    J = np.array([[[-2.0]], [[1.0]]])
+    F = np.array([[1.0], [3.0]])
+    dx0 = dev(torch, np.full((2, 1), 7.0))
+    dx, info = binding.ptc_solve(dev(torch, J), dev(torch, F), dev(torch, np.array([0.5, 0.5])), dx=dx0)
+    torch.cuda.synchronize()
+    assert list(info.cpu().numpy()) == [1, 0]
+    assert dx.cpu().numpy()[0, 0] == 7.0 and dx.cpu().numpy()[1, 0] == -3.0 / 3.0
+    e = torch.empty((0, 4), dtype=torch.float64, device="cuda")
+    binding.ptc_solve(torch.empty((0, 4, 4), dtype=torch.float64, device="cuda"), e, torch.empty(0, dtype=torch.float64, device="cuda"))
+    with pytest.raises(binding.PsrError):
+        f = dev(torch, F)
+        binding.ptc_solve(dev(torch, J), f, dev(torch, np.array([0.5, 0.5])), dx=f)      # dx aliases F
+
+
+def test_pseudo_transient_iteration_on_device_reduces_the_residual(torch_cuda, binding):
+    """The fallback loop the paper describes with this library's calls only: residual + Jacobian
+    (psr_fd_jacobian), one implicit-Euler step (psr_ptc_solve), update -- on C4 states.  Every step is checked
+    against the oracle's step on the same J, F0, dt (backward error of the shifted system; forward error against
+    the long-double solve, relative to the FP64 oracle's own), and the residual norm must fall.  The paper gives
+    no step-size rule ("See [5]"); the test takes dt = 0.1 / max_j sum_i |J_ij| per reactor."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C4", 32)
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y, Yin, tau = (dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    n = mech.n_species + 1
+    norms = []
+    for _ in range(3):
+        J, F0 = gm.fd_jacobian(T, P, Y, Yin, tau, want_F0=True)
+        dt = (0.1 / J.abs().sum(dim=2).max(dim=1).values).contiguous()
+        dx, info = binding.ptc_solve(J, F0, dt)
+        torch.cuda.synchronize()
+        assert int(info.abs().max()) == 0
+        Jh, Fh, dth, d = J.cpu().numpy(), F0.cpu().numpy(), dt.cpu().numpy(), dx.cpu().numpy()
+        A = Jh + np.eye(n)[None] / dth[:, None, None]
+        ok, worst = _backward_error_ok(A, d, -Fh, n)
+        assert ok, worst
+        xr, ir = orc.ptc_step(Jh, Fh, dth)
+        xl, _ = orc.ptc_step(Jh, Fh, dth, long_double=True)
+        assert np.all(ir == 0)
+        scale = np.abs(xl).max(axis=1)
+        ratio = np.abs(d - xl).max(axis=1) / (np.abs(xr - xl).max(axis=1) + 1e-13 * scale)
+        assert np.median(ratio) <= 4.0 and ratio.max() <= 64.0, (float(np.median(ratio)), float(ratio.max()))
+        assert np.all(np.abs(d - xr).max(axis=1) <= 1e-9 * scale)     # the shift makes these systems well conditioned
+        norms.append(float(F0[:, 1:].abs().max()))
+        Y = (Y + dx[:, 1:].t()).contiguous()           # x = (T, Y): row 0 is the fixed-temperature equation, dT = 0
+        assert float(dx[:, 0].abs().max()) <= 1e-12 * float(scale.max())
+    gm.close()
+    assert norms[2] < norms[1] < norms[0], norms
+
+
 # ------------------------------------------------------------------ streams and graphs
 def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, binding):
     """Every evaluation call only enqueues work on the caller's stream (psr.h), so a Newton iteration
