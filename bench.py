@@ -388,6 +388,77 @@ def run_extras(binding, synth, torch, flush):
     return out
 
 
+# ------------------------------------------------------------------------------ paper-shaped sweep (NEXT-3)
+def run_sweep(args):
+    """bench.py --sweep: the AXES of the paper's Fig. 5 (one Newton iteration of a batch of
+    10^2..10^6 identical reactors, 101 species / 542 reactions, T = 1800 K, tau = 50 ms) on a synthetic
+    mechanism of that shape (config P5; the real mechanism [27] is not in this container).  Per batch size:
+    the residual pass (device-resident, and with the paper's offload pattern: inputs copied in, outputs copied
+    out), and the Newton iteration's device work -- FD Jacobian + linear solve -- up to 10^5 reactors (the
+    Jacobians of 10^6 reactors are 83 GB).  The oracle is timed on a bounded sample on the host cores."""
+    import torch
+    from oracle import oracle as orc
+    from paper_2005_11468_b200 import binding, synth
+    torch.cuda.set_device(0)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    mech, _ = synth.make_config("P5", 1)
+    gm = binding.Mechanism.from_synth(mech)
+    n = mech.n_species + 1
+    om = _oracle_mech(mech)
+    cores = min(orc.max_threads(), orc.host_cores())
+    # oracle rates on bounded samples: residual on 4096 reactors, Jacobian + solve on 128
+    _, sb = synth.make_config("P5", 4096)
+    t_res = min(_wall(lambda: orc.evaluate(om, sb.T, sb.P, sb.Y, sb.Yin, sb.tau, want=("wdot", "F"), nthreads=cores)) for _ in range(3)) / sb.n
+    _, jb = synth.make_config("P5", 128)
+    def cpu_newton():
+        j = orc.jacobian(om, jb.T, jb.P, jb.Y, jb.Yin, jb.tau, nthreads=cores)
+        orc.lu_solve(j["J"], -j["F0"])
+    t_newton = min(_wall(cpu_newton) for _ in range(2)) / jb.n
+    t_res_1 = _wall(lambda: orc.evaluate(om, sb.T[:256], sb.P[:256], sb.Y[:, :256].copy(), sb.Yin[:, :256].copy(), sb.tau[:256],
+                                         want=("wdot", "F"), nthreads=1)) / 256
+    rows = []
+    for N in (100, 1000, 10000, 100000, 1000000):
+        _, b = synth.make_config("P5", N)
+        T, P, Y, Yin, tau = (dev(x) for x in (b.T, b.P, b.Y, b.Yin, b.tau))
+        F = torch.empty_like(Y)
+        ms_res = _time_call(torch, lambda: gm.eval_residual(T, P, Y, Yin, tau, F=F), flush)
+        hT, hP, hY, hYin, htau = (torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in (b.T, b.P, b.Y, b.Yin, b.tau))
+        hF = torch.empty(Y.shape, dtype=torch.float64).pin_memory()
+        def offload():
+            for d_, h_ in ((T, hT), (P, hP), (Y, hY), (Yin, hYin), (tau, htau)):
+                d_.copy_(h_, non_blocking=True)
+            gm.eval_residual(T, P, Y, Yin, tau, F=F)
+            hF.copy_(F, non_blocking=True)
+        ms_off = _time_call(torch, offload, flush)
+        row = {"batch": N, "residual_ms": ms_res, "residual_offload_ms": ms_off,
+               "cpu_residual_ms_all_cores": t_res * N * 1e3, "cpu_residual_ms_1_core": t_res_1 * N * 1e3}
+        if N <= 100000:
+            J = torch.empty((N, n, n), dtype=torch.float64, device="cuda")
+            F0 = torch.empty((N, n), dtype=torch.float64, device="cuda")
+            rhs = torch.empty_like(F0)
+            def newton():
+                gm.fd_jacobian(T, P, Y, Yin, tau, J=J, F0=F0)
+                torch.neg(F0, out=rhs)
+                binding.lu_solve(J, rhs)
+            row["newton_iteration_ms"] = _time_call(torch, newton, flush, reps=3)
+            row["cpu_newton_iteration_ms_all_cores"] = t_newton * N * 1e3
+            del J, F0, rhs
+        rows.append(row)
+        del T, P, Y, Yin, tau, F
+        torch.cuda.empty_cache()
+    gm.close()
+    print(json.dumps({"sweep": "paper-shaped (PAPER.md:129-137), synthetic 101 species / 542 reactions, T=1800 K, tau=50 ms, 1 atm",
+                      "cpu": {"kind": "oracle", "cores": cores, "sample": "residual: 4096 reactors; Newton iteration (n+1 = 103 residuals + LU): 128 reactors"},
+                      "rows": rows}), flush=True)
+
+
+def _wall(fn):
+    t0 = time.perf_counter()
+    fn()
+    return time.perf_counter() - t0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -396,8 +467,11 @@ def main():
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-extra", action="store_true", help="skip the C2/C3/C4 extras")
+    ap.add_argument("--sweep", action="store_true", help="paper-shaped batch sweep (NEXT-3) instead of the headline line")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

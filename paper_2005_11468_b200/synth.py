@@ -286,6 +286,25 @@ def make_states(K: int, N: int, seed: int, T_range=(800.0, 2500.0), P_atm=(1.0, 
     return ReactorBatch(T=T, P=P, Y=Y, Yin=Yin, tau=tau)
 
 
+def make_uniform_states(mech: "Mechanism", N: int, seed: int, T: float = 1800.0, P_atm: float = 1.0, tau: float = 50e-3,
+                        inlet_X=(0.15, 0.18, 0.67)) -> ReactorBatch:
+    """The shape of the paper's timing experiment: N identical reactors at T = 1800 K,
+    tau = 50 ms, 1 atm, inlet mole fractions 0.15 / 0.18 / 0.67 on three species (stand-ins for the
+    fuel, oxidiser and diluent of a mechanism that is not in this container: species 0, 1, 2).  The reactor
+    composition is the same for every reactor: half the inlet, half one seeded Dirichlet(1) draw, so that
+    every reaction has non-zero rates."""
+    rng = np.random.default_rng(np.random.PCG64(seed))
+    K = mech.n_species
+    x = np.zeros(K)
+    x[:3] = inlet_X
+    yin = x * mech.W
+    yin /= yin.sum()
+    y = 0.5 * yin + 0.5 * _dirichlet_floored(rng, 1.0, K, 1)[:, 0]
+    y /= y.sum()
+    rep = lambda v: np.ascontiguousarray(np.repeat(v[:, None], N, axis=1))
+    return ReactorBatch(T=np.full(N, T), P=np.full(N, P_atm * P_ATM_CGS), Y=rep(y), Yin=rep(yin), tau=np.full(N, tau))
+
+
 # ----------------------------------------------------------------------------- configs
 CONFIGS = {
     # name: mechanism kwargs, state kwargs, N  (BASELINE.json: configs, zero-indexed)
@@ -300,17 +319,23 @@ CONFIGS = {
     # C4: the C1 mechanism (same mechanism seed), its own state seed
     "C4": dict(mech=dict(n_species=53, n_reactions=325, n_third_body=28, n_troe=29, mmax=3), mech_cfg=1,
                state=dict(T_range=(800.0, 2500.0), P_atm=(0.5, 10.0), dirichlet_alpha=1.0), N=8192),
+    # P5: the SHAPE of the paper's speed-up experiment, 101 species / 542 reactions
+    # (PAPER.md:137), identical reactors at 1800 K, 50 ms (make_uniform_states); batch swept by bench.py --sweep
+    "P5": dict(mech=dict(n_species=101, n_reactions=542, n_third_body=47, n_troe=48, mmax=3), mech_cfg=5,
+               state=None, N=10000),
 }
 
 
 def make_config(name: str, n_reactors: int | None = None):
-    """Return (Mechanism, ReactorBatch) for config 'C0'..'C4'. n_reactors overrides the batch size
+    """Return (Mechanism, ReactorBatch) for config 'C0'..'C4' (BASELINE.json) or 'P5' (paper-shaped sweep). n_reactors overrides the batch size
     (the state stream is seeded per config, so the first n reactors of a larger draw differ from a
     smaller draw; parity tests always pass the same arrays to both sides)."""
     cfg = CONFIGS[name]
     c = int(name[1:])
     mech = make_mechanism(seed=1000 + cfg["mech_cfg"], **cfg["mech"])
     N = cfg["N"] if n_reactors is None else int(n_reactors)
+    if cfg["state"] is None:
+        return mech, make_uniform_states(mech, N, seed=2000 + c)
     batch = make_states(mech.n_species, N, seed=2000 + c, **cfg["state"])
     return mech, batch
 

@@ -82,7 +82,7 @@ def test_C0_full_kf_kr_q_wdot(torch_cuda, binding):
     check_against_oracle(mech, batch, got)
 
 
-@pytest.mark.parametrize("cfg,n", [("C1", 2000), ("C2", 333), ("C3", 97)])
+@pytest.mark.parametrize("cfg,n", [("C1", 2000), ("C2", 333), ("C3", 97), ("P5", 150)])
 def test_configs_ragged_batches(torch_cuda, binding, cfg, n):
     """Several tiles plus a ragged tail (n not a multiple of 32), all reaction types."""
     mech, batch = synth.make_config(cfg, n)
@@ -319,7 +319,7 @@ def test_C4_full_size_jacobian_sampled(torch_cuda, binding):
 
 
 # ------------------------------------------------------------------ Jacobian (a10)
-@pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50), ("C2", 3)])
+@pytest.mark.parametrize("cfg,n", [("C4", 40), ("C0", 50), ("C2", 3), ("P5", 4)])
 def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     torch = torch_cuda
     mech, batch = synth.make_config(cfg, n)
