@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
   // DS: the epilogue's operands Y - Y_in and tau come with the tile's prefetch (shared memory) instead of
   // being loaded into registers before the last gather, where they were spilled at once (measured: the
   // spill stores waited for the loads, 5 % of the kernel)
-  constexpr bool DS = SPW <= 4 && !EN && !JY;   // (the Y-column launch has registers to spare and keeps the loads)
+  constexpr bool DS = SPW <= 4 && !JY;   // (the Y-column launch has registers to spare and keeps the loads)
   static_assert(!JY || R == 1, "the Y-column mode maps one column to a lane");
   constexpr int TR = 32 * R;  // evaluation states per tile
   extern __shared__ __align__(128) unsigned char smem[];
@@ -276,14 +276,44 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
     asm volatile("cp.async.wait_group 0;" ::: "memory");   // this thread's prefetched entries have landed
 
     double T[R];
+    // Energy row (steady Eq. 3, PAPER.md:37-40): this thread's share of  sum Yin_i (h_i(Tin) - h_i(T)),
+    // sum h_i wdot_i W_i  and  sum Y_i cp_i  over the species it owns; h [erg/g] = (h/RT) R T / W (NASA-7).
+    // The first and the last sum do not need wdot: with the Y - Y_in tile (DS) they are formed in the
+    // prologue, where Y and Y_in are at hand, and the epilogue adds the middle one (same h, same order).
+    double en[3][R];
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int i = 0; i < R; ++i) en[k][i] = 0.0;
+    auto h_of = [&](int s, double t) {
+      const double* c = mv.nasa + 7 * s;
+      const double hRT = fma(fma(fma(fma(c[4] * 0.2, t, c[3] * 0.25), t, c[2] * (1.0 / 3.0)), t, c[1] * 0.5), t, c[0]) + c[5] / t;
+      return hRT * (kRgas * mv.invW[s]) * t;
+    };
+    auto energy_pre = [&](int s, int i, double Tin_, double y, double yin) {
+      if constexpr (!EN) return;
+      const double* c = mv.nasa + 7 * s;
+      const double cp = fma(fma(fma(fma(c[4], T[i], c[3]), T[i], c[2]), T[i], c[1]), T[i], c[0]) * (kRgas * mv.invW[s]);
+      en[0][i] = fma(yin, h_of(s, Tin_) - h_of(s, T[i]), en[0][i]);
+      en[2][i] = fma(y, cp, en[2][i]);
+    };
+    auto energy_post = [&](int s, int i, double wd) {
+      if constexpr (!EN) return;
+      en[1][i] = fma(h_of(s, T[i]) * wd, mv.Wm[s], en[1][i]);
+    };
+    auto energy_terms = [&](int s, int i, double Tin_, double y, double yin, double wd) {
+      energy_pre(s, i, Tin_, y, yin);
+      energy_post(s, i, wd);
+    };
     {
       int jsp[R];
-      double rho[R];
+      double rho[R], tin[R];
 #pragma unroll
       for (int i = 0; i < R; ++i) {
         int64_t r_;
         bool valid_;
         state_of(tile, i, r_, jsp[i], valid_);
+        tin[i] = (EN && DS && wantF) ? ldg_nc(a.Tin + r_) : 0.0;
       }
       // x' = fl(x + delta), h = fl(x' - x) for the perturbed unknown of a Jacobian state (O11, g15)
       // pass 1: Y_i/W_i summed; a perturbed entry is replaced in the tile.  pass 2 (below) re-reads it.
@@ -344,7 +374,11 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
         for (int i = 0; i < R; ++i) {
           const double y = Cs[s * TR + lane * R + i];   // the perturbed value where this state perturbs s
-          if (DS && wantF) Ds[s * TR + lane * R + i] = y - Ds[s * TR + lane * R + i];
+          if (DS && wantF) {
+            const double yin = Ds[s * TR + lane * R + i];
+            Ds[s * TR + lane * R + i] = y - yin;
+            energy_pre(s, i, tin[i], y, yin);
+          }
           Cs[s * TR + lane * R + i] = rho[i] * (y * iw);
         }
       });
@@ -409,28 +443,6 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       }
 #pragma unroll
       for (int i = 0; i < R; ++i) a0[i] += a1[i];
-    };
-    // Energy row (steady Eq. 3, PAPER.md:37-40): this thread's share of  sum Yin_i (h_i(Tin) - h_i(T)),
-    // sum h_i wdot_i W_i  and  sum Y_i cp_i  over the species it owns; h [erg/g] = (h/RT) R T / W (NASA-7).
-    double en[3][R];
-#pragma unroll
-    for (int k = 0; k < 3; ++k)
-#pragma unroll
-      for (int i = 0; i < R; ++i) en[k][i] = 0.0;
-    auto energy_terms = [&](int s, int i, double Tin_, double y, double yin, double wd) {
-      if constexpr (!EN) return;
-      const double* c = mv.nasa + 7 * s;
-      const double a0 = c[0], a1 = c[1], a2 = c[2], a3 = c[3], a4 = c[4], a5 = c[5];
-      const double RoW = kRgas * mv.invW[s];
-      auto h_of = [&](double t) {
-        const double hRT = fma(fma(fma(fma(a4 * 0.2, t, a3 * 0.25), t, a2 * (1.0 / 3.0)), t, a1 * 0.5), t, a0) + a5 / t;
-        return hRT * RoW * t;
-      };
-      const double h = h_of(T[i]);
-      const double cp = fma(fma(fma(fma(a4, T[i], a3), T[i], a2), T[i], a1), T[i], a0) * RoW;
-      en[0][i] = fma(yin, h_of(Tin_) - h, en[0][i]);
-      en[1][i] = fma(h * wd, mv.Wm[s], en[1][i]);
-      en[2][i] = fma(y, cp, en[2][i]);
     };
     // GA: where the running sum of (species s, state i of this lane) rests between chunks, and the
     // outputs of that entry once the last chunk is in (same arithmetic as the epilogue below)
@@ -957,7 +969,8 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                 const double Fv = fma(dy, invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
                 if (a.flags & kOutF) a.F[o] = Fv;
                 if (a.flags & kOutF0) a.F0out[r[i] * n + 1 + s] = Fv;
-                if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), e_y[jj][i], e_yin[jj][i], acc[jj][i]);
+                if constexpr (EN && DS) energy_post(s, i, acc[jj][i]);
+                else if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), e_y[jj][i], e_yin[jj][i], acc[jj][i]);
               }
             }
           }
@@ -1000,7 +1013,8 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
             }
             const double Fv = fma(dy, invtau, -(acc[jj][i] * (mv.Wm[s] * invrho)));
             stg[st * npad + 1 + s] = (Fv - e_f0[jj][i]) * invh;
-            if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), y, e_yin[jj][i], acc[jj][i]);
+            if constexpr (EN && DS) energy_post(s, i, acc[jj][i]);
+            else if constexpr (EN) energy_terms(s, i, ldg_nc(a.Tin + r[i]), y, e_yin[jj][i], acc[jj][i]);
           }
         }
         if (!EN && w == 0) stg[st * npad] = (jsp[i] == -1) ? 1.0 : 0.0;  // row 0: F_T = T - T_set

@@ -21,7 +21,8 @@ constexpr int kNB = 8;   // pivots per pass over the trailing matrix
 // the columns with two running pointers (pivot-row entry, this lane's rows) instead of forming j*ld + i for
 // every access (that index arithmetic cost more instructions than the elimination itself: 51 k
 // instructions per 54 x 54 system, 4 k of them FMA, in the first version).
-template <int RPL>
+// PTC: the pseudo-transient variant (psr_ptc_solve): matrix J + I/dt, right-hand side -F.
+template <int RPL, bool PTC>
 __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const double* __restrict__ A,
                                                        double* __restrict__ b, int32_t* __restrict__ info,
                                                        int sys_doubles, const double* __restrict__ F,
@@ -36,7 +37,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
   for (int64_t r = (int64_t)blockIdx.x * wpc + w; r < N; r += (int64_t)gridDim.x * wpc) {
     const double* Ar = A + (size_t)r * n * n;
     // pseudo-transient step (psr_ptc_solve): the matrix is J + I/dt, the right-hand side -F
-    const double shift = dt ? 1.0 / dt[r] : 0.0;
+    const double shift = PTC ? 1.0 / dt[r] : 0.0;
     {
       // column-major stream, 32 consecutive entries per trip, 4 trips in flight; (i, j) tracked without a divide
       int i = lane, j = 0;
@@ -48,7 +49,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
         for (int u = 0; u < 4; ++u) {
           off[u] = j * ld + i;
           v[u] = (t + 32 * u < n * n) ? Ar[t + 32 * u] : 0.0;
-          if (dt && i == j) v[u] += shift;
+          if (PTC && i == j) v[u] += shift;
           i += 32;
           while (i >= n) { i -= n; ++j; }
         }
@@ -57,7 +58,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
           if (t + 32 * u < n * n) As[off[u]] = v[u];
       }
     }
-    for (int i = lane; i < n; i += 32) bs[i] = F ? -F[r * n + i] : b[r * n + i];
+    for (int i = lane; i < n; i += 32) bs[i] = PTC ? -F[r * n + i] : b[r * n + i];
     __syncwarp();
 
     // Blocked right-looking elimination, kNB pivots per pass over the trailing matrix: every trailing entry
@@ -251,10 +252,10 @@ cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_
   if (ctas > cap) ctas = cap;
 #define PSR_LU(RPL_)                                                                                         \
   if (rpl <= RPL_) {                                                                                         \
-    cudaError_t e = cudaFuncSetAttribute(lu_solve_kernel<RPL_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                         (int)smem);                                                         \
+    auto kern = dt ? lu_solve_kernel<RPL_, true> : lu_solve_kernel<RPL_, false>;                             \
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);      \
     if (e != cudaSuccess) return e;                                                                          \
-    lu_solve_kernel<RPL_><<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles, F, dt);                 \
+    kern<<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles, F, dt);                           \
     return cudaGetLastError();                                                                               \
   }
   PSR_LU(1) PSR_LU(2) PSR_LU(4) PSR_LU(6)
