@@ -206,7 +206,8 @@ def run_ours(args):
 
     sampler = ClockSampler(local)   # samples SM clock / throttle reasons from the warm-up to the end of the e2e leg
     sampler.start()
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(args.warmup, 3)):   # warm-up steps are the timed steps without the events: flush, then call
+        flush.zero_()
         step()
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
@@ -347,6 +348,7 @@ def _hbm_peak():
 
 def _time_call(torch, fn, flush, reps=5):
     for _ in range(3):
+        flush.zero_()
         fn()
     torch.cuda.synchronize()
     st = torch.cuda.current_stream()
