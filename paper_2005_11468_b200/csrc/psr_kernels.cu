@@ -486,10 +486,26 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           bool valid_[R];
 #pragma unroll
           for (int i = 0; i < R; ++i) state_of(tile, i, r_[i], jsp_[i], valid_[i]);
-          for_species([&](int, int s) {
+          // the running sum of the NEXT species is requested before this species' rows are added, so that its
+          // trip to L2 runs beside the summation instead of in front of it
+          auto fetch = [&](int s, double (&v)[R]) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) v[i] = (first || !valid_[i] || s < 0) ? 0.0 : *ga_slot(s, r_[i], jsp_[i]);
+          };
+          int s_nxt = __ldg(mv.sp_of + w * SPW);
+          double nxt[R];
+          fetch(s_nxt, nxt);
+#pragma unroll 1
+          for (int jj = 0; jj < SPW; ++jj) {
+            const int s = s_nxt;
             double a0[R];
 #pragma unroll
-            for (int i = 0; i < R; ++i) a0[i] = (first || !valid_[i]) ? 0.0 : *ga_slot(s, r_[i], jsp_[i]);
+            for (int i = 0; i < R; ++i) a0[i] = nxt[i];
+            if (jj + 1 < SPW) {
+              s_nxt = __ldg(mv.sp_of + w * SPW + jj + 1);
+              fetch(s_nxt, nxt);
+            }
+            if (s < 0) continue;
             sum_rows(gptr, gent, s, a0);
 #pragma unroll
             for (int i = 0; i < R; ++i) {
@@ -498,7 +514,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                 else *ga_slot(s, r_[i], jsp_[i]) = a0[i];
               }
             }
-          });
+          }
         } else {
           for_species([&](int jj, int s) { sum_rows(gptr, gent, s, acc[jj]); });
         }
