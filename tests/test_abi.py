@@ -65,3 +65,34 @@ def test_eval_calls_validate_arguments_without_a_device():
     assert b"null mechanism" in lib.psr_last_error()
     assert lib.psr_eval_kf_kr(null, -1, null, null, null, 0, null, null, 0, null) == binding.PSR_EINVAL
     assert lib.psr_fd_jacobian(null, 1, null, null, null, null, null, 1, null, null, null) == binding.PSR_EINVAL
+
+
+def test_solve_calls_validate_arguments_without_a_device():
+    lib = binding.lib()
+    null = C.c_void_p()
+    one = C.c_void_p(8)          # any non-null address: the checks below fail before anything is dereferenced
+    assert lib.psr_lu_solve(-1, 4, one, one, one, null) == binding.PSR_EINVAL
+    assert lib.psr_lu_solve(3, 0, one, one, one, null) == binding.PSR_EINVAL
+    assert lib.psr_lu_solve(3, 4, null, one, one, null) == binding.PSR_EINVAL
+    assert lib.psr_lu_solve(0, 4, null, null, null, null) == binding.PSR_OK          # N = 0: nothing to do
+    assert lib.psr_ptc_solve(2, 4, one, one, null, one, one, null) == binding.PSR_EINVAL   # null dt
+    assert b"psr_ptc_solve" in lib.psr_last_error()
+    two = C.c_void_p(16)
+    assert lib.psr_ptc_solve(2, 4, one, two, one, two, one, null) == binding.PSR_EINVAL    # dx aliases F
+    assert b"alias" in lib.psr_last_error()
+    assert lib.psr_ptc_solve(0, 4, null, null, null, null, null, null) == binding.PSR_OK
+
+
+def test_paper_shaped_config_is_a_batch_of_identical_reactors():
+    """P5: the shape of the paper's timing case -- 101 species,
+    542 reactions, every reactor at 1800 K, 1 atm, 50 ms, inlet mole fractions 0.15 / 0.18 / 0.67."""
+    mech, b = synth.make_config("P5", 7)
+    assert (mech.n_species, mech.n_reactions) == (101, 542)
+    assert np.all(b.T == 1800.0) and np.all(b.tau == 50e-3) and np.allclose(b.P, 1.01325e6)
+    assert np.all(b.Y == b.Y[:, :1]) and np.all(b.Yin == b.Yin[:, :1])
+    assert np.allclose(b.Y.sum(axis=0), 1.0, rtol=0, atol=1e-14) and np.all(b.Y > 0)
+    x = b.Yin[:, 0] / mech.W
+    x /= x.sum()
+    assert np.allclose(x[:3], [0.15, 0.18, 0.67], rtol=1e-13) and np.all(x[3:] == 0)
+    m2, _ = synth.make_config("P5", 1)
+    assert np.array_equal(m2.A, mech.A)                       # seeded: the same mechanism every time

@@ -223,7 +223,7 @@ def test_O8_q_sign_flip_under_swap():
         assert np.all(np.sign(ds["q"][plain]) == -np.sign(d["q"][plain]))
 
 
-@pytest.mark.parametrize("cfg,n", [("C0", 64), ("C1", 32), ("C2", 4)])
+@pytest.mark.parametrize("cfg,n", [("C0", 64), ("C1", 32), ("C2", 4), ("P5", 2)])
 def test_O9_mass_conservation(cfg, n):
     """sum_k W_k wdot_k = 0 on element-balanced mechanisms, relative <= 1e-12 of sum |W_k wdot_k|."""
     mech, batch = synth.make_config(cfg, n)
