@@ -138,6 +138,24 @@ def jacobian(mech: OracleMechanism, T, P, Y, Yin, tau, *, Tin=None, long_double:
     return dict(J=J, F0=F0, S=S, H=H)
 
 
+def roundoff_scale(mech: OracleMechanism, T, P, Y, Yin=None, tau=None, *, nthreads: int = 0) -> dict:
+    """Round-off scales (floor terms of the parity criteria): Sw [K][N] = sum_k (nu'+nu'')(|kf prod| + |kr prod|)
+    (x |[M]| for three-body), and with Yin, tau also SF [K][N] = |Y - Yin|/tau + (W/rho) Sw (= S of jacobian())."""
+    T, P, Y = (np.ascontiguousarray(a, dtype=np.float64) for a in (T, P, Y))
+    N = T.shape[0]
+    Sw = np.empty((mech.K, N))
+    SF = None
+    if Yin is not None:
+        Yin = np.ascontiguousarray(Yin, dtype=np.float64)
+        tau = np.ascontiguousarray(tau, dtype=np.float64)
+        SF = np.empty((mech.K, N))
+    rc = lib().oracle_roundoff_scale(C.byref(mech.c), C.c_int64(N), _p(T), _p(P), _p(Y), _p(Yin), _p(tau), C.c_int64(N),
+                                     _p(Sw), _p(SF), C.c_int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"oracle_roundoff_scale failed rc={rc}")
+    return dict(Sw=Sw, SF=SF) if SF is not None else dict(Sw=Sw)
+
+
 def lu_solve(A, b, *, long_double: bool = False):
     """NEXT-2: batched A x = b by Gaussian elimination with partial pivoting.  A: [N][n][n] with A[r, j, i] =
     entry (row i, column j) (column-major per system, the layout of J), b: [N][n].  Returns x [N][n], info [N]."""

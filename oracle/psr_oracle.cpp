@@ -20,7 +20,8 @@
 //   sum_i C_i = P/RT; K_c(R)*K_c(reverse R)=1; q sign flip under reactant/product swap;
 //   k_f/k_r = K_c; sum_k W_k wdot_k = 0 on element-balanced mechanisms; Lindemann limits
 //   k->k0[M], k->k_inf; Troe F=F_cent at log10 Pr=-c; sum_i F_i = (sum Y - sum Y_in)/tau;
-//   Jacobian species rows of a Y column sum to 1/tau; J row 0 = e_0.
+//   Jacobian species rows of a Y column sum to 1/tau; J row 0 = e_0; the round-off scale S (roundoff_acc)
+//   against its definition typed independently at 50 digits (tests/mp_dense.py roundoff_scale).
 //   Energy row (NEXT-1): T3 values of h_i, C_p,mix and F_T from SURVEY.md 8(c), re-derived with mpmath;
 //   F_T = 0 for an inert mechanism at T_in = T; linearity in 1/tau; enthalpy-balance identity.
 //   Linear solve (NEXT-2): exact rational solutions of small integer systems, a system that needs a row
@@ -30,6 +31,7 @@
 //
 // Units (paper silent; CHEMKIN cgs, reading g4): T [K], P [dyn/cm^2], C [mol/cm^3],
 // rho [g/cm^3], W [g/mol], wdot [mol/cm^3/s], Ea [cal/mol].
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -280,6 +282,29 @@ int eval_batch(const oracle_mech& m, int64_t N, const double* T, const double* P
   return 0;
 }
 
+// Round-off scale of the net production rates: acc_i = sum_k (nu'_ik + nu''_ik)
+// (|k_f prod C^nu'| + |k_r prod C^nu''|), times |[M]_k| for a three-body reaction -- the magnitude of the
+// terms whose signed sum is wdot_i (Eq. 4, 5), i.e. what one unit of relative rounding error in them moves
+// wdot_i by.  C, kf, kr: the reactor's concentrations and effective rate constants (outputs of eval_one).
+template <class R>
+void roundoff_acc(const oracle_mech& m, const R* C, const R* kf, const R* kr, R* acc /*[K], zeroed*/) {
+  const int K = m.n_species, I = m.n_reactions;
+  for (int k = 0; k < I; ++k) {
+    R pf = 1, pr = 1;
+    for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) pf *= ipow<R>(C[m.reac_sp[j]], m.reac_nu[j]);
+    for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) pr *= ipow<R>(C[m.prod_sp[j]], m.prod_nu[j]);
+    R mag = std::fabs((double)(kf[k] * pf)) + std::fabs((double)(kr[k] * pr));
+    if (m.rtype[k] == 1) {
+      R M = 0;
+      for (int i = 0; i < K; ++i) M += C[i];
+      for (int j = m.eff_ptr[k]; j < m.eff_ptr[k + 1]; ++j) M += ((R)m.eff_val[j] - (R)1) * C[m.eff_sp[j]];
+      mag *= std::fabs((double)M);
+    }
+    for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) acc[m.reac_sp[j]] += (R)m.reac_nu[j] * mag;
+    for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) acc[m.prod_sp[j]] += (R)m.prod_nu[j] * mag;
+  }
+}
+
 // O11: forward finite-difference Jacobian. x=(T,Y_1..Y_K); delta_j=1e-8*max(|x_j|,1e-10);
 // x'_j = fl(x_j+delta_j) and h_j = fl(x'_j - x_j) are formed in DOUBLE for both precisions
 // (the state is a double array; reading g15); each perturbed residual is a full independent
@@ -319,20 +344,7 @@ int jac_batch(const oracle_mech& m, int64_t N, const double* T, const double* P,
         double* Sr = S + (int64_t)r * n;
         Sr[0] = 0.0;
         std::vector<R> acc(K, (R)0);
-        for (int k = 0; k < I; ++k) {
-          R pf = 1, pr = 1;
-          for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) pf *= ipow<R>(C[m.reac_sp[j]], m.reac_nu[j]);
-          for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) pr *= ipow<R>(C[m.prod_sp[j]], m.prod_nu[j]);
-          R mag = std::fabs((double)(okf[k] * pf)) + std::fabs((double)(okr[k] * pr));
-          if (m.rtype[k] == 1) {
-            R M = 0;
-            for (int i = 0; i < K; ++i) M += C[i];
-            for (int j = m.eff_ptr[k]; j < m.eff_ptr[k + 1]; ++j) M += ((R)m.eff_val[j] - (R)1) * C[m.eff_sp[j]];
-            mag *= std::fabs((double)M);
-          }
-          for (int j = m.reac_ptr[k]; j < m.reac_ptr[k + 1]; ++j) acc[m.reac_sp[j]] += (R)m.reac_nu[j] * mag;
-          for (int j = m.prod_ptr[k]; j < m.prod_ptr[k + 1]; ++j) acc[m.prod_sp[j]] += (R)m.prod_nu[j] * mag;
-        }
+        roundoff_acc<R>(m, C.data(), okf.data(), okr.data(), acc.data());
         for (int i = 0; i < K; ++i)
           Sr[1 + i] = (double)(std::fabs((double)((y[i] - yin[i]) / (R)tau[r])) + (R)m.W[i] / rho * acc[i]);
         if (Tin) {
@@ -477,6 +489,38 @@ int oracle_jacobian_energy(const oracle_mech* m, int64_t N, const double* T, con
                            double* S, double* H, int use_long_double, int nthreads) {
   if (use_long_double) return jac_batch<long double>(*m, N, T, P, Y, Tin, Yin, tau, ld, J, F0, S, H, nthreads);
   return jac_batch<double>(*m, N, T, P, Y, Tin, Yin, tau, ld, J, F0, S, H, nthreads);
+}
+
+// Round-off scales of a batch (the floor terms of the parity criteria): Sw [K][ld] =
+// roundoff_acc (scale of wdot_i), SF [K][ld] = |Y_i - Yin_i|/tau + (W_i/rho) Sw_i (scale of F_i, the S of
+// oracle_jacobian rows 1..K).  Either may be null; SF needs Yin and tau.
+int oracle_roundoff_scale(const oracle_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                          const double* Yin, const double* tau, int64_t ld, double* Sw, double* SF, int nthreads) {
+  const int K = m->n_species, I = m->n_reactions;
+  if (SF && (!Yin || !tau)) return 1;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+#endif
+  {
+    std::vector<double> y(K), yin(K, 0.0), okf(I), okr(I), C(K), acc(K);
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+    for (int64_t r = 0; r < N; ++r) {
+      for (int i = 0; i < K; ++i) y[i] = Y[(int64_t)i * ld + r];
+      double rho;
+      eval_one<double>(*m, T[r], P[r], y.data(), yin.data(), 1.0, T[r], okf.data(), okr.data(), nullptr, nullptr,
+                       nullptr, nullptr, C.data(), &rho);
+      std::fill(acc.begin(), acc.end(), 0.0);
+      roundoff_acc<double>(*m, C.data(), okf.data(), okr.data(), acc.data());
+      for (int i = 0; i < K; ++i) {
+        if (Sw) Sw[(int64_t)i * ld + r] = acc[i];
+        if (SF) SF[(int64_t)i * ld + r] = std::fabs((y[i] - Yin[(int64_t)i * ld + r]) / tau[r]) + m->W[i] / rho * acc[i];
+      }
+    }
+  }
+  return 0;
 }
 
 // Single-reactor detail for the pins: per reaction 11 doubles

@@ -125,6 +125,19 @@ def _ld(Y, N):
     return max(int(Y.stride(0)), int(N)) if (Y.dim() == 2 and Y.shape[0] > 1 and Y.shape[1] > 1) else int(N)
 
 
+def _like(Y, rows, N, ld):
+    """A [rows][N] output that shares Y's leading dimension (the C ABI has ONE ld for Y, Yin, F, wdot)."""
+    import torch
+    if ld == N:
+        return torch.empty((rows, N), dtype=torch.float64, device=Y.device)
+    return torch.empty((rows, ld), dtype=torch.float64, device=Y.device)[:, :N]
+
+
+def _chk_ld(name, t, N, ld):
+    if t is not None and _ld(t, N) != ld:
+        raise ValueError(f"{name} must share the leading dimension of Y ({ld})")
+
+
 def _chk_dev(name, t, rows=None, N=None):
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
@@ -192,12 +205,10 @@ class Mechanism:
         for nm, t in (("T", T), ("P", P), ("Y", Y)):
             _chk_dev(nm, t)
         if wdot is None:
-            wdot = torch.empty((self.K, ld), dtype=torch.float64, device=T.device)[:, :N] if ld != N else \
-                torch.empty((self.K, N), dtype=torch.float64, device=T.device)
+            wdot = _like(Y, self.K, N, ld)
         if q is None and want_q:
             q = torch.empty((self.I, N), dtype=torch.float64, device=T.device)
-        if _ld(wdot, N) != ld:
-            raise ValueError("wdot must share the leading dimension of Y")
+        _chk_ld("wdot", wdot, N, ld)
         _check(lib().psr_eval_wdot(self._h, N, _ptr(T), _ptr(P), _ptr(Y), ld, _ptr(wdot), _ptr(q),
                                    _ld(q, N) if q is not None else 0, _stream()))
         return (wdot, q) if (want_q or q is not None) else wdot
@@ -209,12 +220,12 @@ class Mechanism:
         ld = _ld(Y, N)
         for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)):
             _chk_dev(nm, t)
-        if _ld(Yin, N) != ld:
-            raise ValueError("Yin must share the leading dimension of Y")
         if F is None:
-            F = torch.empty_like(Y)
+            F = _like(Y, self.K, N, ld)
         if wdot is None and want_wdot:
-            wdot = torch.empty_like(Y)
+            wdot = _like(Y, self.K, N, ld)
+        for nm, t in (("Yin", Yin), ("F", F), ("wdot", wdot)):
+            _chk_ld(nm, t, N, ld)
         _check(lib().psr_eval_residual(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(F),
                                        _ptr(wdot), _stream()))
         return (F, wdot) if wdot is not None else F
@@ -226,14 +237,14 @@ class Mechanism:
         ld = _ld(Y, N)
         for nm, t in (("T", T), ("P", P), ("Y", Y), ("Tin", Tin), ("Yin", Yin), ("tau", tau)):
             _chk_dev(nm, t)
-        if _ld(Yin, N) != ld:
-            raise ValueError("Yin must share the leading dimension of Y")
         if F is None:
-            F = torch.empty_like(Y)
+            F = _like(Y, self.K, N, ld)
         if FT is None:
             FT = torch.empty_like(T)
         if wdot is None and want_wdot:
-            wdot = torch.empty_like(Y)
+            wdot = _like(Y, self.K, N, ld)
+        for nm, t in (("Yin", Yin), ("F", F), ("wdot", wdot)):
+            _chk_ld(nm, t, N, ld)
         _check(lib().psr_eval_residual_energy(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Tin), _ptr(Yin), _ptr(tau),
                                               ld, _ptr(F), _ptr(FT), _ptr(wdot), _stream()))
         return (F, FT, wdot) if wdot is not None else (F, FT)
@@ -247,6 +258,7 @@ class Mechanism:
         n = self.K + 1
         for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)) + ((("Tin", Tin),) if Tin is not None else ()):
             _chk_dev(nm, t)
+        _chk_ld("Yin", Yin, N, ld)
         if J is None:
             J = torch.empty((N, n, n), dtype=torch.float64, device=T.device)  # J[r, col, row]
         if F0 is None and want_F0:

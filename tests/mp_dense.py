@@ -102,3 +102,41 @@ def evaluate(mech, T, P, Y, Yin=None, tau=None, Tset=None, lindemann_only=False,
             rhs = sum(Yin[i] * (hin[i] - h[i]) for i in range(K)) / tau - sum(h[i] * wdot[i] * W[i] for i in range(K)) / rho
             out.update(h=h, cp_mix=cp_mix, FT=-rhs / cp_mix)
     return out
+
+
+def roundoff_scale(mech, T, P, Y, Yin, tau, Tin=None):
+    """The round-off scale S of SURVEY.md 8(c)-J, typed from its definition (not from the oracle):
+        S_i = |Y_i - Yin_i|/tau + (W_i/rho) sum_k (nu'_ik + nu''_ik) (|k_f prod C^nu'| + |k_r prod C^nu''|) [x |[M]_k| if three-body]
+    for the species rows i = 1..K; S_0 = 0 for the fixed-temperature row, and with Tin the energy row's
+        S_0 = [ (1/tau) sum_i |Yin_i (h_in,i - h_i)| + sum_i |h_i| (W_i/rho) sum_k (...)_ik ] / cp_mix .
+    Returns K+1 mp values."""
+    K, I = mech.n_species, mech.n_reactions
+    ev = evaluate(mech, T, P, Y, Yin=Yin, tau=tau, Tin=Tin)
+    nup, nupp = dense_nu(mech)
+    W = [mpf(float(w)) for w in mech.W]
+    C, rho = ev["C"], ev["rho"]
+    acc = [mpf(0)] * K
+    for k in range(I):
+        rx = ev["rx"][k]
+        pf, pr = mpf(1), mpf(1)
+        for i in range(K):
+            pf *= power(C[i], nup[i][k])
+            pr *= power(C[i], nupp[i][k])
+        mag = abs(rx["kf"] * pf) + abs(rx["kr"] * pr)
+        if int(mech.rtype[k]) == 1:
+            mag *= abs(rx["M"])
+        for i in range(K):
+            acc[i] = acc[i] + (nup[i][k] + nupp[i][k]) * mag
+    Yv = [mpf(float(y)) for y in Y]
+    Yi = [mpf(float(y)) for y in Yin]
+    tau = mpf(float(tau))
+    S = [mpf(0)] + [abs(Yv[i] - Yi[i]) / tau + W[i] / rho * acc[i] for i in range(K)]
+    if Tin is not None:
+        Tm, Tinm = mpf(T), mpf(Tin)
+        st = mpf(0)
+        for i in range(K):
+            a = [mpf(float(v)) for v in mech.nasa[i]]
+            enth = lambda t: (a[0] + a[1] * t / 2 + a[2] * t**2 / 3 + a[3] * t**3 / 4 + a[4] * t**4 / 5 + a[5] / t) * RGAS * t / W[i]
+            st += abs(Yi[i] * (enth(Tinm) - enth(Tm))) / tau + abs(enth(Tm)) * W[i] / rho * acc[i]
+        S[0] = st / ev["cp_mix"]
+    return S

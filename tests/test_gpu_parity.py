@@ -15,11 +15,12 @@ import pytest
 
 from oracle import oracle as orc
 from paper_2005_11468_b200 import synth
-from util import jacobian_floor_ratio, oracle_mech, rel_err, residual_rel_err, wdot_masked_rel_err
+from util import floor_criterion, jacobian_floor_ratio, oracle_mech, rel_err, residual_rel_err, wdot_masked_rel_err
 
 pytestmark = pytest.mark.gpu
 
 TOL_K = 1e-10
+RGAS = 8.31446261815324e7
 TOL_F = 1e-9
 
 
@@ -137,6 +138,36 @@ def test_leading_dimension_larger_than_N(torch_cuda, binding):
     werr, _ = wdot_masked_rel_err(w[:, :100], ref["wdot"])
     assert werr.max() <= TOL_K
     assert np.all(w[:, 100:] == -7.0)  # padding untouched
+    # psr_eval_residual / psr_eval_residual_energy take ONE ld for Y, Yin, F and wdot: outputs the binding
+    # allocates must share it (a dense [K][N] tensor would be overrun), outputs the caller passes are checked
+    Yinbig = torch.full((mech.n_species, ld), float("nan"), dtype=torch.float64, device="cuda")
+    Yinbig[:, :100] = dev(torch, batch.Yin)
+    T, P, tau, Tin = dev(torch, batch.T), dev(torch, batch.P), dev(torch, batch.tau), torch.full((100,), 300.0, dtype=torch.float64, device="cuda")
+    refF = orc.evaluate(oracle_mech(mech), batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("wdot", "F"))
+    Fbig = torch.full((mech.n_species, ld), -7.0, dtype=torch.float64, device="cuda")
+    w2big = torch.full((mech.n_species, ld), -7.0, dtype=torch.float64, device="cuda")
+    gm.eval_residual(T, P, Ybig[:, :100], Yinbig[:, :100], tau, F=Fbig[:, :100], wdot=w2big[:, :100])
+    Fa, wa = gm.eval_residual(T, P, Ybig[:, :100], Yinbig[:, :100], tau, want_wdot=True)   # binding-allocated
+    assert Fa.stride(0) == ld and wa.stride(0) == ld
+    Fe, FTe, we = gm.eval_residual_energy(T, P, Ybig[:, :100], Tin, Yinbig[:, :100], tau, want_wdot=True)
+    assert Fe.stride(0) == ld and we.stride(0) == ld
+    Fe2 = torch.full((mech.n_species, ld), -7.0, dtype=torch.float64, device="cuda")
+    gm.eval_residual_energy(T, P, Ybig[:, :100], Tin, Yinbig[:, :100], tau, F=Fe2[:, :100])
+    torch.cuda.synchronize()
+    for Fx in (Fbig[:, :100], Fa, Fe, Fe2[:, :100]):
+        assert residual_rel_err(Fx.cpu().numpy(), refF["F"]).max() <= TOL_F
+    for wx in (w2big[:, :100], wa, we):
+        assert np.array_equal(wx.cpu().numpy(), w[:, :100])
+    for big in (Fbig, w2big, Fe2):
+        assert bool((big[:, 100:] == -7.0).all())  # padding untouched
+    dense = torch.empty((mech.n_species, 100), dtype=torch.float64, device="cuda")
+    for kw in (dict(F=dense), dict(wdot=dense)):
+        with pytest.raises(ValueError):
+            gm.eval_residual(T, P, Ybig[:, :100], Yinbig[:, :100], tau, **kw)
+        with pytest.raises(ValueError):
+            gm.eval_residual_energy(T, P, Ybig[:, :100], Tin, Yinbig[:, :100], tau, **kw)
+    with pytest.raises(ValueError):
+        gm.eval_residual(T, P, Ybig[:, :100], dev(torch, batch.Yin), tau)
     gm.close()
 
 
@@ -239,34 +270,77 @@ def test_out_of_range_exp_arguments_take_the_library_path(torch_cuda, binding):
     assert np.all(np.isfinite(kc)) and np.all(kc >= 0.0) and np.all(kc[arg > 720.0] < 1e-280)
 
 
-# ------------------------------------------------------------------ full-size launch, sampled
-def test_C1_full_size_sampled(torch_cuda, binding):
-    """BASELINE config 1 at its full batch (65,536 reactors, the launch bench.py times): compare a
-    sample of reactors with the oracle, and check invariants over the whole output."""
+# ------------------------------------------------------------------ full-size launches, every reactor
+def _mass_conservation(mech, wdot):
+    ww = mech.W[:, None] * wdot
+    return np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0))
+
+
+def check_full_batch(mech, batch, wdot, F):
+    """Every reactor of a full-size batch.  At this size some wdot_i are the small remainder of terms 1e9 times
+    larger (e.g. C1 reactor 64738, species 17: |wdot| = 6e-10 of the reactor's largest), where the FP64 oracle
+    itself is 1.6e-10 from the long-double oracle: the literal 1e-10 is then below what FP64 can resolve, so the
+    bar is the conditioning-aware one (util.floor_criterion) against the LONG-DOUBLE oracle, plus:
+    the GPU is no noisier than 4x the independent FP64 oracle, and the literal 1e-10 / 1e-9 holds on all but a
+    1e-5 fraction of the entries north_star's mask selects."""
+    om = oracle_mech(mech)
+    star = orc.evaluate(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("wdot", "F"), long_double=True)
+    dbl = orc.evaluate(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, want=("wdot", "F"))
+    S = orc.roundoff_scale(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau)
+    _, mask = wdot_masked_rel_err(wdot, star["wdot"])
+    assert mask.any()
+    worst_w, fr_w = floor_criterion(wdot, star["wdot"], S["Sw"], rtol=TOL_K, mask=mask)
+    worst_F, fr_F = floor_criterion(F, star["F"], S["SF"], rtol=TOL_F)
+    _, od_w = floor_criterion(dbl["wdot"], star["wdot"], S["Sw"], rtol=TOL_K, mask=mask)
+    _, od_F = floor_criterion(dbl["F"], star["F"], S["SF"], rtol=TOL_F)
+    assert worst_w <= 1.0 and worst_F <= 1.0, (worst_w, worst_F)
+    assert fr_w <= 4 * max(od_w, 1.0) and fr_F <= 4 * max(od_F, 1.0), (fr_w, od_w, fr_F, od_F)
+    werr, _ = wdot_masked_rel_err(wdot, dbl["wdot"])
+    assert (werr > TOL_K).sum() <= 1e-5 * mask.sum()
+    assert (residual_rel_err(F, dbl["F"]) > TOL_F).mean() <= 1e-5
+    return dbl
+
+
+def test_C1_full_size_residual_every_reactor(torch_cuda, binding):
+    """BASELINE config 1 at its full batch through the exact launch bench.py times -- psr_eval_residual on
+    65,536 reactors into preallocated F and wdot (the multi-tile, double-buffered Y - Y_in path of a
+    persistent CTA) -- compared with the oracle on EVERY reactor; the same for psr_eval_residual_energy,
+    psr_eval_wdot and psr_eval_kf_kr (c-J: every perf number rests on parity of the launch
+    that is timed)."""
     torch = torch_cuda
     mech, batch = synth.make_config("C1")
     gm = binding.Mechanism.from_synth(mech)
-    T, P, Y = dev(torch, batch.T), dev(torch, batch.P), dev(torch, batch.Y)
-    wdot = gm.eval_wdot(T, P, Y).cpu().numpy()
+    T, P, Y, Yin, tau = (dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    F, wdot = torch.empty_like(Y), torch.empty_like(Y)
+    for _ in range(2):   # twice: the second call runs with warm L2 / resident tables, as in bench.py
+        gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=wdot)
+    om = oracle_mech(mech)
+    Fh, wh = F.cpu().numpy(), wdot.cpu().numpy()
+    ref = check_full_batch(mech, batch, wh, Fh)
+    ref.update(orc.evaluate(om, batch.T, batch.P, batch.Y, want=("kf", "kr")))
+    assert _mass_conservation(mech, wh) <= 1e-12
+    # psr_eval_wdot alone gives the same bits
+    assert np.array_equal(gm.eval_wdot(T, P, Y).cpu().numpy(), wh)
+    # adiabatic residual: species rows bit-identical, energy row against the oracle
+    Tin = torch.full_like(T, 300.0)
+    Fe, FTe, we = gm.eval_residual_energy(T, P, Y, Tin, Yin, tau, want_wdot=True)
+    assert np.array_equal(Fe.cpu().numpy(), Fh) and np.array_equal(we.cpu().numpy(), wh)
+    refe = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.full(batch.n, 300.0), batch.Yin, batch.tau)
+    rho = batch.P / (RGAS * batch.T * (batch.Y / mech.W[:, None]).sum(axis=0))
+    scale = energy_scale(mech, batch, np.full(batch.n, 300.0), ref["wdot"], rho)
+    err = np.abs(FTe.cpu().numpy() - refe["FT"]) / np.maximum(np.abs(refe["FT"]), 1e-3 * scale)
+    assert err.max() <= TOL_F
+    # rate constants of all 325 reactions x 65,536 reactors
+    kf, kr = gm.eval_kf_kr(T, P, Y)
+    assert rel_err(kf.cpu().numpy(), ref["kf"]).max() <= TOL_K
+    assert rel_err(kr.cpu().numpy(), ref["kr"]).max() <= TOL_K
     gm.close()
-    rng = np.random.default_rng(5)
-    idx = np.sort(rng.choice(batch.n, size=512, replace=False))
-    idx[:3] = [0, 1, 2]
-    idx[-1] = batch.n - 1
-    sub = batch.take(idx)
-    ref = orc.evaluate(oracle_mech(mech), sub.T, sub.P, sub.Y, want=("wdot",))
-    werr, _ = wdot_masked_rel_err(wdot[:, idx], ref["wdot"])
-    assert werr.max() <= TOL_K
-    assert np.all(np.isfinite(wdot))
-    # mass conservation over the whole batch (property that holds at any size)
-    ww = mech.W[:, None] * wdot
-    assert np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0)) <= 1e-12
 
 
-@pytest.mark.parametrize("cfg,n_sample", [("C2", 96), ("C3", 48)])
-def test_large_configs_full_size_sampled(torch_cuda, binding, cfg, n_sample):
+@pytest.mark.parametrize("cfg", ["C2", "C3"])
+def test_large_configs_full_size_every_reactor(torch_cuda, binding, cfg):
     """BASELINE configs 2 and 3 at their full batches through psr_eval_residual (the launches bench.py
-    times under `extra`): sampled reactors against the oracle, invariants over the whole output."""
+    times under `extra`): every reactor against the oracle, invariants over the whole output."""
     torch = torch_cuda
     mech, batch = synth.make_config(cfg)
     gm = binding.Mechanism.from_synth(mech)
@@ -274,17 +348,8 @@ def test_large_configs_full_size_sampled(torch_cuda, binding, cfg, n_sample):
     F, wdot = gm.eval_residual(*args, want_wdot=True)
     F, wdot = F.cpu().numpy(), wdot.cpu().numpy()
     gm.close()
-    rng = np.random.default_rng(11)
-    idx = np.sort(rng.choice(batch.n, size=n_sample, replace=False))
-    idx[0], idx[-1] = 0, batch.n - 1
-    sub = batch.take(idx)
-    ref = orc.evaluate(oracle_mech(mech), sub.T, sub.P, sub.Y, sub.Yin, sub.tau, want=("wdot", "F"))
-    werr, mask = wdot_masked_rel_err(wdot[:, idx], ref["wdot"])
-    assert mask.any() and werr.max() <= TOL_K
-    assert residual_rel_err(F[:, idx], ref["F"]).max() <= TOL_F
-    assert np.all(np.isfinite(wdot)) and np.all(np.isfinite(F))
-    ww = mech.W[:, None] * wdot
-    assert np.median(np.abs(ww.sum(axis=0)) / np.abs(ww).sum(axis=0)) <= 1e-12
+    check_full_batch(mech, batch, wdot, F)
+    assert _mass_conservation(mech, wdot) <= 1e-12
     # sum_i F_i = (sum Y - sum Y_in)/tau - sum_i wdot_i W_i / rho, and the last sum vanishes (mass conservation)
     lhs = F.sum(axis=0)
     rhs = (batch.Y.sum(axis=0) - batch.Yin.sum(axis=0)) / batch.tau
@@ -292,15 +357,19 @@ def test_large_configs_full_size_sampled(torch_cuda, binding, cfg, n_sample):
     assert np.median(np.abs(lhs - rhs) / scale) <= 1e-12
 
 
-def test_C4_full_size_jacobian_sampled(torch_cuda, binding):
-    """BASELINE config 4 at its full 8,192 reactors (the psr_fd_jacobian launch sequence bench.py times,
-    two sub-batches): sampled reactors by the floor criterion against the long-double oracle, structural
-    invariants over every Jacobian."""
+def test_C4_full_size_jacobian_every_reactor(torch_cuda, binding):
+    """BASELINE config 4 at its full 8,192 reactors (the psr_fd_jacobian launch sequence bench.py times):
+    every Jacobian by the floor criterion against the long-double oracle, structural invariants too.
+    Over the 23.9 M entries of the whole batch the tail of the round-off noise is longer than on the samples
+    SURVEY.md 8(c)-J calibrated K_j on (there an FP64 code reached 4 eps S/h in the Y columns; here the
+    independent FP64 ORACLE reaches 21.2 and 627 in the T column, measured): the Y-column constant of this
+    test is 64 instead of 32, and the GPU must in addition be no noisier than 4x the FP64 oracle."""
     torch = torch_cuda
     mech, batch = synth.make_config("C4")
     gm = binding.Mechanism.from_synth(mech)
     args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
-    J = gm.fd_jacobian(*args).cpu().numpy()
+    J, F0 = gm.fd_jacobian(*args, want_F0=True)
+    J, F0 = J.cpu().numpy(), F0.cpu().numpy()
     gm.close()
     assert np.all(np.isfinite(J))
     assert np.all(J[:, 0, 0] == 1.0) and np.all(J[:, 1:, 0] == 0.0)          # row 0 = e_0 (g13)
@@ -309,13 +378,19 @@ def test_C4_full_size_jacobian_sampled(torch_cuda, binding):
     scale = np.abs(J[:, :, 1:]).sum(axis=2)
     assert np.median(np.abs(col_sums[:, 1:] - 1.0 / batch.tau[:, None]) / scale[:, 1:]) <= 1e-6
     assert np.median(np.abs(col_sums[:, 0]) / scale[:, 0]) <= 1e-6
-    rng = np.random.default_rng(13)
-    idx = np.sort(rng.choice(batch.n, size=24, replace=False))
-    idx[0], idx[-1] = 0, batch.n - 1          # first and last reactor; the sample spans both sub-batches
-    sub = batch.take(idx)
-    jl = orc.jacobian(oracle_mech(mech), sub.T, sub.P, sub.Y, sub.Yin, sub.tau, long_double=True)
-    worst, fr_T, fr_Y = jacobian_floor_ratio(J[idx], jl["J"], jl["S"], jl["H"])
-    assert worst <= 1.0, (worst, fr_T, fr_Y)
+    om = oracle_mech(mech)
+    worst = fr_T = fr_Y = 0.0
+    for r0 in range(0, batch.n, 2048):   # the long-double reference in blocks (its J is 191 MB for the batch)
+        sub = batch.take(np.arange(r0, min(r0 + 2048, batch.n)))
+        jl = orc.jacobian(om, sub.T, sub.P, sub.Y, sub.Yin, sub.tau, long_double=True)
+        w, ft, fy = jacobian_floor_ratio(J[r0:r0 + sub.n], jl["J"], jl["S"], jl["H"], K_y=64.0)
+        worst, fr_T, fr_Y = max(worst, w), max(fr_T, ft), max(fr_Y, fy)
+        assert residual_rel_err(F0[r0:r0 + sub.n, 1:].T, jl["F0"][:, 1:].T).max() <= TOL_F
+        if r0 == 0:   # the independent FP64 oracle on the first block (a lower bound of its worst over the batch)
+            jd = orc.jacobian(om, sub.T, sub.P, sub.Y, sub.Yin, sub.tau)
+            _, od_T, od_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
+    assert worst <= 1.0, (worst, fr_T, fr_Y, od_T, od_Y)
+    assert fr_T <= 4 * max(od_T, 1.0) and fr_Y <= 4 * max(od_Y, 1.0), (fr_T, od_T, fr_Y, od_Y)
 
 
 # ------------------------------------------------------------------ Jacobian (a10)
@@ -357,19 +432,19 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
 # ------------------------------------------------------------------ energy row (NEXT-1)
 def energy_scale(mech, batch, Tin, wdot_ref, rho):
     """Sum of the absolute terms of the energy row, per reactor: the row is a difference of large numbers,
-    so its error is judged relative to max(|F_T|, 1e-3 of this scale)."""
-    K, N = mech.n_species, batch.n
-    S = np.zeros(N)
-    cp_mix = np.zeros(N)
-    for r in range(N):
-        for i in range(K):
-            cp_R, h_RT, _ = orc.nasa7(mech.nasa[i], float(batch.T[r]))
-            _, hin_RT, _ = orc.nasa7(mech.nasa[i], float(Tin[r]))
-            h = h_RT * 8.31446261815324e7 * batch.T[r] / mech.W[i]
-            hin = hin_RT * 8.31446261815324e7 * Tin[r] / mech.W[i]
-            S[r] += abs(batch.Yin[i, r] * (hin - h)) / batch.tau[r] + abs(h * wdot_ref[i, r] * mech.W[i]) / rho[r]
-            cp_mix[r] += batch.Y[i, r] * cp_R * 8.31446261815324e7 / mech.W[i]
-    return S / cp_mix
+    so its error is judged relative to max(|F_T|, 1e-3 of this scale).  NASA-7 forms of
+    include/psr.h, vectorised over the batch (a tolerance scale, not an expected value)."""
+    a = mech.nasa[:, :, None]                                   # [K][7][1]
+    W = mech.W[:, None]
+
+    def h_of(T):                                                # erg/g, [K][N]
+        hRT = a[:, 0] + a[:, 1] * T / 2 + a[:, 2] * T**2 / 3 + a[:, 3] * T**3 / 4 + a[:, 4] * T**4 / 5 + a[:, 5] / T
+        return hRT * RGAS * T / W
+    T = batch.T[None, :]
+    h, hin = h_of(T), h_of(np.asarray(Tin, dtype=np.float64)[None, :])
+    cp = (a[:, 0] + a[:, 1] * T + a[:, 2] * T**2 + a[:, 3] * T**3 + a[:, 4] * T**4) * RGAS / W
+    S = (np.abs(batch.Yin * (hin - h)) / batch.tau[None, :] + np.abs(h * wdot_ref * W) / rho[None, :]).sum(axis=0)
+    return S / (batch.Y * cp).sum(axis=0)
 
 
 @pytest.mark.parametrize("cfg,n", [("C0", 100), ("C1", 333), ("C2", 70)])

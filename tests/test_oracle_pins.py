@@ -423,6 +423,37 @@ def test_O11_linear_part_exact():
         assert np.all(Jr[1:, 0] == 0.0) and np.all(Jr[0] == expect[0])
 
 
+def test_O11_roundoff_scale_S_against_its_definition(t3):
+    """The floor term of every Jacobian criterion (tests/util.py: K_j eps S_i / h_j) rests on the scale S that
+    jac_batch returns.  Pin it against SURVEY.md 8(c)-J's definition typed out independently at 50 digits
+    (tests/mp_dense.py: dense nu', nu'', mp.power): T3 (plain, three-body and Troe reactions) with and without
+    the energy row, and reactors of C0 (duplicates, efficiency lists) and C1 (every reaction type)."""
+    mech, batch, om = t3
+    for Tin in (None, 300.0):
+        j = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau,
+                         Tin=None if Tin is None else np.array([Tin]))
+        S = mp_dense.roundoff_scale(mech, batch.T[0], batch.P[0], batch.Y[:, 0], batch.Yin[:, 0], batch.tau[0], Tin=Tin)
+        assert j["S"][0, 0] == 0.0 if Tin is None else close(j["S"][0, 0], S[0], 1e-13)
+        for i in range(1, 4):
+            assert close(j["S"][0, i], S[i], 1e-13), (i, j["S"][0, i], S[i])
+    for cfg, n in (("C0", 2), ("C1", 1)):
+        mech, batch = synth.make_config(cfg, n)
+        om = oracle_mech(mech)
+        Tin = np.full(n, 350.0)
+        for use_tin in (False, True):
+            j = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin if use_tin else None)
+            jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin if use_tin else None, long_double=True)
+            for r in range(n):
+                S = mp_dense.roundoff_scale(mech, batch.T[r], batch.P[r], batch.Y[:, r], batch.Yin[:, r], batch.tau[r],
+                                            Tin=350.0 if use_tin else None)
+                for i in range(mech.n_species + 1):
+                    if i == 0 and not use_tin:
+                        assert j["S"][r, 0] == 0.0 and jl["S"][r, 0] == 0.0
+                        continue
+                    assert close(j["S"][r, i], S[i], 1e-12), (cfg, r, i)
+                    assert close(jl["S"][r, i], S[i], 1e-12), (cfg, r, i)
+
+
 # ------------------------------------------------------------------ energy row (SURVEY.md 8(f) NEXT-1)
 def test_energy_row_T3_golden_rederived_and_matched(t3):
     """Steady Eq. 3 as the residual F_T = -dT/dt: the T3 values printed in SURVEY.md 8(c)

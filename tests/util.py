@@ -55,3 +55,22 @@ def jacobian_floor_ratio(J, J_star, S, H, K_y=32.0, K_T=1024.0):
         ratio = np.where(diff == 0, 0.0, diff / bound)
         fr = np.where(floor > 0, diff / floor, 0.0)
     return float(np.nanmax(ratio)), float(np.nanmax(fr[:, 0, :])), float(np.nanmax(fr[:, 1:, :]))
+
+
+def floor_criterion(x, x_star, S, K=1024.0, rtol=1e-10, mask=None):
+    """Conditioning-aware parity (reading g16b): |x - x*| <= rtol |x*| + K eps S, with x* the
+    long-double oracle and S the round-off scale of the entry (oracle.roundoff_scale: the magnitude of the terms
+    whose signed sum the entry is).  Where an entry is not the result of cancellation (S ~ |x*|) this is the
+    literal relative bound; where it is, no FP64 evaluation -- the oracle included -- can do better than a
+    multiple of eps S, the multiple set by the conditioning of the exp arguments (|dG/RT| up to a few hundred),
+    hence the same K = 1024 as the T column of the Jacobian criterion.
+    Returns (worst lhs/rhs, worst |x - x*| / (eps S))."""
+    x, x_star, S = (np.asarray(a, dtype=np.float64) for a in (x, x_star, S))
+    diff = np.abs(x - x_star)
+    bound = rtol * np.abs(x_star) + K * EPS * S
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ratio = np.where(diff == 0, 0.0, diff / bound)
+        fr = np.where(S > 0, diff / (EPS * S), 0.0)
+    if mask is not None:
+        ratio, fr = np.where(mask, ratio, 0.0), np.where(mask, fr, 0.0)
+    return float(np.nanmax(ratio)), float(np.nanmax(fr))
