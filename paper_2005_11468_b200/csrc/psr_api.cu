@@ -23,6 +23,8 @@ cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
                             cudaStream_t st, const double* F, const double* dt);
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
+cudaError_t ws_set_smem(size_t smem);
+cudaError_t launch_ws(const WsView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st);
 }  // namespace psr
 
 using namespace psr;
@@ -40,6 +42,12 @@ struct psr_mech {
   double* d_exptab = nullptr;
   int32_t* d_sp_of = nullptr;
   int32_t* d_rec_base = nullptr;  // [n_chunks + 1]
+  WsView ws{};                  // warp-specialised kernel (psr_ws.cu), when its tables fit (ws_ok)
+  bool ws_ok = false;
+  unsigned char* d_ws_chunks = nullptr;
+  int32_t* d_ws_sp_of = nullptr;
+  int opt_fused_only = 0;       // diagnostic (psr_mech_set_option): never take the warp-specialised kernel
+  int opt_jac_unhoisted = 0;    // diagnostic: every Jacobian column a full evaluation
   double* d_scratch = nullptr;  // psr_fd_jacobian: rate table [N][I][kRateVals], then F0 when the caller passes none
   size_t scratch_bytes = 0;
   int device = 0;
@@ -88,6 +96,177 @@ struct HostRx {
   int type;
   int nr = 0, np = 0;
 };
+
+struct BlobSet {
+  std::vector<unsigned char> all;   // n_chunks blobs, stride bytes apart
+  std::vector<int32_t> rec_base;    // [n_chunks + 1] mechanism-wide index of each chunk's first record
+  size_t stride = 0;
+  int n_chunks = 0, rc = 0;         // rc: most reactions in a chunk (rows of the q tile, +1 zero row)
+};
+
+// Cuts the mechanism into n_chunks chunks, deals every chunk's records to nw warps and serialises the chunk
+// blobs (psr_tables.h): records, aux records, efficiency entries, factor pool, per-species gather lists.
+void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out) {
+  const uint32_t row_bytes = (uint32_t)kRowBytes;
+  const int rc = (I + n_chunks - 1) / n_chunks;
+  out.n_chunks = n_chunks;
+  out.rc = rc;
+  // ---- distribute reactions over chunks (each type dealt round-robin so chunks cost the same),
+  //      then inside a chunk order by cost and deal to warps in snake order.
+  std::vector<int> order(I);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return reaction_cost(rx[x].type) > reaction_cost(rx[y].type); });
+  std::vector<std::vector<int>> chunk_rx(n_chunks);
+  for (int p = 0; p < I; ++p) chunk_rx[p % n_chunks].push_back(order[p]);
+  // inside a chunk: longest-processing-time assignment of records to warps, records of a warp contiguous
+  auto cls_of = [&](int k) { return (rx[k].nr > kSlots || rx[k].np > kSlots) ? kClsLong : rx[k].type; };
+  std::vector<std::vector<int>> chunk_wb(n_chunks);   // [warp][class boundary], kClsLong + 2 per warp
+  for (int c = 0; c < n_chunks; ++c) {
+    auto& cr = chunk_rx[c];  // cost-descending
+    std::vector<double> load(nw, 0.0);
+    load[0] = warp0_load;   // extra work of warp 0 in units of a plain reaction (it forms ln T, rho, C_tot of the tile)
+    std::vector<std::vector<int>> mine(nw);
+    for (int k : cr) {
+      const int wmin = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+      mine[wmin].push_back(k);
+      load[wmin] += reaction_cost(rx[k].type);
+    }
+    cr.clear();
+    chunk_wb[c].assign((size_t)kMaxWarps * (kClsLong + 2), 0);
+    for (int wv = 0; wv < nw; ++wv) {
+      std::stable_sort(mine[wv].begin(), mine[wv].end(), [&](int x, int y) { return cls_of(x) < cls_of(y); });
+      int* wb = &chunk_wb[c][(size_t)wv * (kClsLong + 2)];
+      size_t p = 0;
+      for (int cl = 0; cl <= kClsLong; ++cl) {
+        wb[cl] = (int)(cr.size() + p);
+        while (p < mine[wv].size() && cls_of(mine[wv][p]) == cl) ++p;
+      }
+      cr.insert(cr.end(), mine[wv].begin(), mine[wv].end());
+      wb[kClsLong + 1] = (int)cr.size();
+    }
+  }
+  // ---- serialise chunk blobs
+  out.rec_base.assign(n_chunks + 1, 0);
+  for (int c = 0; c < n_chunks; ++c) out.rec_base[c + 1] = out.rec_base[c] + (int32_t)chunk_rx[c].size();
+  std::vector<std::vector<unsigned char>> blobs(n_chunks);
+  size_t stride = 0;
+  const uint32_t unit_off = (uint32_t)K * row_bytes;   // the all-ones row of the C tile
+  const uint32_t zero_c_off = (uint32_t)(K + 1) * row_bytes;  // the all-zero row of the C tile
+  const uint32_t zero_off = (uint32_t)rc * row_bytes;  // the all-zero row of the q tile
+  for (int c = 0; c < n_chunks; ++c) {
+    const auto& cr = chunk_rx[c];
+    const int n_rx = (int)cr.size();
+    std::vector<RxRec> recs(n_rx);
+    std::vector<AuxRec> auxs;
+    std::vector<EffEnt> effs;
+    std::vector<uint16_t> pool;
+    std::vector<std::vector<uint32_t>> pos(K), neg(K);
+    for (int kl = 0; kl < n_rx; ++kl) {
+      const HostRx& h = rx[cr[kl]];
+      RxRec rec = h.rec;
+      if (h.nr <= kSlots && h.np <= kSlots) {
+        for (int i = 0; i < kSlots; ++i) {
+          rec.off[i] = i < h.nr ? (uint32_t)h.factors[i] * row_bytes : unit_off;
+          rec.off[kSlots + i] = i < h.np ? (uint32_t)h.factors[h.nr + i] * row_bytes : unit_off;
+        }
+        // irreversible: the product-side factor is the zero row, so k_r * prod = 0 without a select
+        // (and below ln k_r := ln k_f keeps the unused exp finite whenever k_f is)
+        if (!(rec.meta & kMetaRev)) rec.off[kSlots] = zero_c_off;
+      } else {
+        rec.meta |= kMetaLong | ((uint32_t)h.nr << kMetaNrShift) | ((uint32_t)h.np << kMetaNpShift);
+        rec.off[0] = (uint32_t)pool.size();
+        pool.insert(pool.end(), h.factors.begin(), h.factors.end());
+      }
+      if (!(rec.meta & kMetaRev)) {
+        for (int j = 0; j < 3; ++j) rec.e[j] = rec.c[j];
+        for (int j = 0; j < 4; ++j) rec.d[j] = 0.0;
+      }
+      if (h.has_aux) {
+        AuxRec ax = h.aux;
+        ax.eff_off = (uint32_t)effs.size();
+        ax.n_eff = (uint32_t)h.eff.size();
+        for (EffEnt ee : h.eff) {
+          ee.off *= row_bytes;
+          effs.push_back(ee);
+        }
+        rec.meta |= (uint32_t)auxs.size() << kMetaAuxShift;
+        auxs.push_back(ax);
+      }
+      recs[kl] = rec;
+      for (auto& pr : h.nu_net)
+        for (int t = 0; t < std::abs(pr.second); ++t)
+          (pr.second < 0 ? neg : pos)[pr.first].push_back((uint32_t)kl * row_bytes);
+    }
+    std::vector<uint32_t> gptr(2 * K + 1, 0), gent;
+    auto add_group = [&](const std::vector<uint32_t>& grp) {
+      gent.insert(gent.end(), grp.begin(), grp.end());
+      while (gent.size() % 4) gent.push_back(zero_off);
+    };
+    for (int s = 0; s < K; ++s) {
+      gptr[2 * s] = (uint32_t)gent.size();
+      add_group(pos[s]);
+      gptr[2 * s + 1] = (uint32_t)gent.size();
+      add_group(neg[s]);
+    }
+    gptr[2 * K] = (uint32_t)gent.size();
+
+    ChunkHdr hdr{};
+    hdr.n_rx = n_rx;
+    hdr.n_aux = (uint32_t)auxs.size();
+    hdr.n_eff = (uint32_t)effs.size();
+    hdr.rec_base = (uint32_t)out.rec_base[c];
+    for (int wv = 0; wv < kMaxWarps; ++wv)
+      for (int cl = 0; cl < kClsLong + 2; ++cl) hdr.wb[wv][cl] = (uint16_t)chunk_wb[c][(size_t)wv * (kClsLong + 2) + cl];
+    size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
+    hdr.off_aux = (uint32_t)off;
+    off += sizeof(AuxRec) * auxs.size();
+    hdr.off_eff = (uint32_t)off;
+    off += sizeof(EffEnt) * effs.size();
+    hdr.off_pool = (uint32_t)off;
+    off = align_up(off + 2 * pool.size(), 16);
+    hdr.off_gptr = (uint32_t)off;
+    off = align_up(off + 4 * gptr.size(), 16);
+    hdr.off_gent = (uint32_t)off;
+    off = align_up(off + 4 * gent.size(), 16);
+    hdr.bytes = (uint32_t)off;
+    std::vector<unsigned char>& b = blobs[c];
+    b.assign(off, 0);
+    std::memcpy(b.data(), &hdr, sizeof hdr);
+    std::memcpy(b.data() + sizeof(ChunkHdr), recs.data(), sizeof(RxRec) * n_rx);
+    if (!auxs.empty()) std::memcpy(b.data() + hdr.off_aux, auxs.data(), sizeof(AuxRec) * auxs.size());
+    if (!effs.empty()) std::memcpy(b.data() + hdr.off_eff, effs.data(), sizeof(EffEnt) * effs.size());
+    if (!pool.empty()) std::memcpy(b.data() + hdr.off_pool, pool.data(), 2 * pool.size());
+    std::memcpy(b.data() + hdr.off_gptr, gptr.data(), 4 * gptr.size());
+    if (!gent.empty()) std::memcpy(b.data() + hdr.off_gent, gent.data(), 4 * gent.size());
+    stride = std::max(stride, off);
+  }
+  stride = align_up(stride, 128);
+  out.stride = stride;
+  out.all.assign(stride * n_chunks, 0);
+  for (int c = 0; c < n_chunks; ++c) std::memcpy(out.all.data() + stride * c, blobs[c].data(), blobs[c].size());
+}
+
+// Gather ownership: species to (warp, slot) by longest-processing-time on the row length of nu^T; a warp's
+// owned species come first in its slots, -1 pads.
+std::vector<int32_t> assign_species(const std::vector<HostRx>& rx, int K, int I, int nw, int spw) {
+  std::vector<int32_t> sp_of((size_t)nw * spw, -1);
+  std::vector<int> rowlen(K, 0);
+  for (int k = 0; k < I; ++k)
+    for (auto& pr : rx[k].nu_net) rowlen[pr.first] += std::abs(pr.second);
+  std::vector<int> sorder(K);
+  std::iota(sorder.begin(), sorder.end(), 0);
+  std::stable_sort(sorder.begin(), sorder.end(), [&](int x, int y) { return rowlen[x] > rowlen[y]; });
+  std::vector<double> load(nw, 0.0);
+  std::vector<int> used(nw, 0);
+  for (int sidx : sorder) {
+    int best = -1;
+    for (int wv = 0; wv < nw; ++wv)
+      if (used[wv] < spw && (best < 0 || load[wv] < load[best])) best = wv;
+    sp_of[(size_t)best * spw + used[best]++] = sidx;
+    load[best] += rowlen[sidx] + 6.0;  // + per-species loop overhead
+  }
+  return sp_of;
+}
 
 }  // namespace
 
@@ -234,7 +413,6 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   const int rl = 1;
   const uint32_t row_bytes = (uint32_t)kRowBytes * rl;
   int rc_target = std::min(I, 384);
-  if (const char* e = getenv("PSR_RC")) rc_target = std::min(std::min(I, kMaxChunkRx), std::max(8, atoi(e)));
   // shared memory left for the q tile and the chunk ring beside one C tile and the per-CTA scratch
   // Y - Y_in tile beside every C tile when the species' accumulators live in registers (spw <= 4); it shares
   // its region with the rate-table slices, which only the Y-column launch (that has no such tile) uses
@@ -249,8 +427,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   bool resident = false;
   int ring_stages = 2;
   size_t stride = 0;
-  std::vector<unsigned char> all;
-  std::vector<int32_t> sp_of, rec_base_of;
+  BlobSet bs;
   // the chunk size shrinks until one C tile, the q tile and the (double-buffered) chunk ring fit one CTA
   for (;; rc_target = std::min(rc_target - 1, rc_target * 15 / 16)) {
   if (rc_target < 1)
@@ -259,156 +436,9 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   n_chunks = (I + rc_target - 1) / rc_target;
   rc = (I + n_chunks - 1) / n_chunks;  // <= rc_target <= kMaxChunkRx
 
-  // ---- distribute reactions over chunks (each type dealt round-robin so chunks cost the same),
-  //      then inside a chunk order by cost and deal to warps in snake order.
-  std::vector<int> order(I);
-  std::iota(order.begin(), order.end(), 0);
-  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return reaction_cost(rx[x].type) > reaction_cost(rx[y].type); });
-  std::vector<std::vector<int>> chunk_rx(n_chunks);
-  for (int p = 0; p < I; ++p) chunk_rx[p % n_chunks].push_back(order[p]);
-  // inside a chunk: longest-processing-time assignment of records to warps, records of a warp contiguous
-  auto cls_of = [&](int k) { return (rx[k].nr > kSlots || rx[k].np > kSlots) ? kClsLong : rx[k].type; };
-  std::vector<std::vector<int>> chunk_wb(n_chunks);   // [warp][class boundary], kClsLong + 2 per warp
-  for (int c = 0; c < n_chunks; ++c) {
-    auto& cr = chunk_rx[c];  // cost-descending
-    std::vector<double> load(nw, 0.0);
-    load[0] = 2.0;   // warp 0 also forms ln T, rho, C_tot of the tile (about two plain reactions' worth)
-    std::vector<std::vector<int>> mine(nw);
-    for (int k : cr) {
-      const int wmin = (int)(std::min_element(load.begin(), load.end()) - load.begin());
-      mine[wmin].push_back(k);
-      load[wmin] += reaction_cost(rx[k].type);
-    }
-    cr.clear();
-    chunk_wb[c].assign((size_t)kMaxWarps * (kClsLong + 2), 0);
-    for (int wv = 0; wv < nw; ++wv) {
-      std::stable_sort(mine[wv].begin(), mine[wv].end(), [&](int x, int y) { return cls_of(x) < cls_of(y); });
-      int* wb = &chunk_wb[c][(size_t)wv * (kClsLong + 2)];
-      size_t p = 0;
-      for (int cl = 0; cl <= kClsLong; ++cl) {
-        wb[cl] = (int)(cr.size() + p);
-        while (p < mine[wv].size() && cls_of(mine[wv][p]) == cl) ++p;
-      }
-      cr.insert(cr.end(), mine[wv].begin(), mine[wv].end());
-      wb[kClsLong + 1] = (int)cr.size();
-    }
-  }
-  // gather ownership: species to (warp, slot) by longest-processing-time on the row length of nu^T
-  sp_of.assign((size_t)nw * spw, -1);
-  {
-    std::vector<int> rowlen(K, 0);
-    for (int k = 0; k < I; ++k)
-      for (auto& pr : rx[k].nu_net) rowlen[pr.first] += std::abs(pr.second);
-    std::vector<int> sorder(K);
-    std::iota(sorder.begin(), sorder.end(), 0);
-    std::stable_sort(sorder.begin(), sorder.end(), [&](int x, int y) { return rowlen[x] > rowlen[y]; });
-    std::vector<double> load(nw, 0.0);
-    std::vector<int> used(nw, 0);
-    for (int sidx : sorder) {
-      int best = -1;
-      for (int wv = 0; wv < nw; ++wv)
-        if (used[wv] < spw && (best < 0 || load[wv] < load[best])) best = wv;
-      sp_of[(size_t)best * spw + used[best]++] = sidx;
-      load[best] += rowlen[sidx] + 6.0;  // + per-species loop overhead
-    }
-  }
-
-  // ---- serialise chunk blobs
-  rec_base_of.assign(n_chunks + 1, 0);
-  for (int c = 0; c < n_chunks; ++c) rec_base_of[c + 1] = rec_base_of[c] + (int32_t)chunk_rx[c].size();
-  std::vector<std::vector<unsigned char>> blobs(n_chunks);
-  stride = 0;
-  const uint32_t unit_off = (uint32_t)K * row_bytes;   // the all-ones row of the C tile
-  const uint32_t zero_c_off = (uint32_t)(K + 1) * row_bytes;  // the all-zero row of the C tile
-  const uint32_t zero_off = (uint32_t)rc * row_bytes;  // the all-zero row of the q tile
-  for (int c = 0; c < n_chunks; ++c) {
-    const auto& cr = chunk_rx[c];
-    const int n_rx = (int)cr.size();
-    std::vector<RxRec> recs(n_rx);
-    std::vector<AuxRec> auxs;
-    std::vector<EffEnt> effs;
-    std::vector<uint16_t> pool;
-    std::vector<std::vector<uint32_t>> pos(K), neg(K);
-    for (int kl = 0; kl < n_rx; ++kl) {
-      HostRx& h = rx[cr[kl]];
-      RxRec rec = h.rec;
-      if (h.nr <= kSlots && h.np <= kSlots) {
-        for (int i = 0; i < kSlots; ++i) {
-          rec.off[i] = i < h.nr ? (uint32_t)h.factors[i] * row_bytes : unit_off;
-          rec.off[kSlots + i] = i < h.np ? (uint32_t)h.factors[h.nr + i] * row_bytes : unit_off;
-        }
-        // irreversible: the product-side factor is the zero row, so k_r * prod = 0 without a select
-        // (and below ln k_r := ln k_f keeps the unused exp finite whenever k_f is)
-        if (!(rec.meta & kMetaRev)) rec.off[kSlots] = zero_c_off;
-      } else {
-        rec.meta |= kMetaLong | ((uint32_t)h.nr << kMetaNrShift) | ((uint32_t)h.np << kMetaNpShift);
-        rec.off[0] = (uint32_t)pool.size();
-        pool.insert(pool.end(), h.factors.begin(), h.factors.end());
-      }
-      if (!(rec.meta & kMetaRev)) {
-        for (int j = 0; j < 3; ++j) rec.e[j] = rec.c[j];
-        for (int j = 0; j < 4; ++j) rec.d[j] = 0.0;
-      }
-      if (h.has_aux) {
-        AuxRec ax = h.aux;
-        ax.eff_off = (uint32_t)effs.size();
-        ax.n_eff = (uint32_t)h.eff.size();
-        for (EffEnt ee : h.eff) {
-          ee.off *= row_bytes;
-          effs.push_back(ee);
-        }
-        rec.meta |= (uint32_t)auxs.size() << kMetaAuxShift;
-        auxs.push_back(ax);
-      }
-      recs[kl] = rec;
-      for (auto& pr : h.nu_net)
-        for (int t = 0; t < std::abs(pr.second); ++t)
-          (pr.second < 0 ? neg : pos)[pr.first].push_back((uint32_t)kl * row_bytes);
-    }
-    std::vector<uint32_t> gptr(2 * K + 1, 0), gent;
-    auto add_group = [&](const std::vector<uint32_t>& grp) {
-      gent.insert(gent.end(), grp.begin(), grp.end());
-      while (gent.size() % 4) gent.push_back(zero_off);
-    };
-    for (int s = 0; s < K; ++s) {
-      gptr[2 * s] = (uint32_t)gent.size();
-      add_group(pos[s]);
-      gptr[2 * s + 1] = (uint32_t)gent.size();
-      add_group(neg[s]);
-    }
-    gptr[2 * K] = (uint32_t)gent.size();
-
-    ChunkHdr hdr{};
-    hdr.n_rx = n_rx;
-    hdr.n_aux = (uint32_t)auxs.size();
-    hdr.n_eff = (uint32_t)effs.size();
-    hdr.rec_base = (uint32_t)rec_base_of[c];
-    for (int wv = 0; wv < kMaxWarps; ++wv)
-      for (int cl = 0; cl < kClsLong + 2; ++cl) hdr.wb[wv][cl] = (uint16_t)chunk_wb[c][(size_t)wv * (kClsLong + 2) + cl];
-    size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
-    hdr.off_aux = (uint32_t)off;
-    off += sizeof(AuxRec) * auxs.size();
-    hdr.off_eff = (uint32_t)off;
-    off += sizeof(EffEnt) * effs.size();
-    hdr.off_pool = (uint32_t)off;
-    off = align_up(off + 2 * pool.size(), 16);
-    hdr.off_gptr = (uint32_t)off;
-    off = align_up(off + 4 * gptr.size(), 16);
-    hdr.off_gent = (uint32_t)off;
-    off = align_up(off + 4 * gent.size(), 16);
-    hdr.bytes = (uint32_t)off;
-    std::vector<unsigned char>& b = blobs[c];
-    b.assign(off, 0);
-    std::memcpy(b.data(), &hdr, sizeof hdr);
-    std::memcpy(b.data() + sizeof(ChunkHdr), recs.data(), sizeof(RxRec) * n_rx);
-    if (!auxs.empty()) std::memcpy(b.data() + hdr.off_aux, auxs.data(), sizeof(AuxRec) * auxs.size());
-    if (!effs.empty()) std::memcpy(b.data() + hdr.off_eff, effs.data(), sizeof(EffEnt) * effs.size());
-    if (!pool.empty()) std::memcpy(b.data() + hdr.off_pool, pool.data(), 2 * pool.size());
-    std::memcpy(b.data() + hdr.off_gptr, gptr.data(), 4 * gptr.size());
-    if (!gent.empty()) std::memcpy(b.data() + hdr.off_gent, gent.data(), 4 * gent.size());
-    stride = std::max(stride, off);
-  }
-  stride = align_up(stride, 128);
+  build_blobs(rx, K, I, n_chunks, nw, 2.0, bs);
+  rc = bs.rc;
+  stride = bs.stride;
   // all chunk blobs resident in shared memory (loaded once per CTA) when they fit; else a ring of two
   // stages, or of one when that is what lets this chunk size fit: a tile of a mechanism that large runs
   // for hundreds of microseconds, the exposed ~1 us copy per chunk costs less than a smaller chunk's extra
@@ -423,9 +453,50 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   if (!resident && smem_fixed + q_bytes + stride * 2 > (size_t)prop.sharedMemPerBlockOptin) ring_stages = 1;
   const size_t need = smem_fixed + q_bytes + stride * (resident ? n_chunks : ring_stages);
   if (need > (size_t)prop.sharedMemPerBlockOptin) continue;
-  all.assign(stride * n_chunks, 0);
-  for (int c = 0; c < n_chunks; ++c) std::memcpy(all.data() + stride * c, blobs[c].data(), blobs[c].size());
   break;
+  }
+  const std::vector<unsigned char>& all = bs.all;
+  const std::vector<int32_t>& rec_base_of = bs.rec_base;
+  const std::vector<int32_t> sp_of = assign_species(rx, K, I, nw, spw);
+
+  // ---- warp-specialised kernel (psr_ws.cu): the mechanism in the fewest parts whose tables, two C tiles, two
+  // Y - Y_in tiles, two q buffers and the partial-sum tile fit one CTA together (all parts resident)
+  BlobSet wbs;
+  WsView wv{};
+  bool ws_ok = false;
+  std::vector<int32_t> ws_sp_of;
+  if (K <= 32 * kWsHelpWarps) {
+    const int spw_h = (K + kWsHelpWarps - 1) / kWsHelpWarps;
+    const int Kp = (K + 1) & ~1;
+    for (int n_parts = 1; n_parts <= kWsMaxParts && n_parts <= I && !ws_ok; ++n_parts) {
+      build_blobs(rx, K, I, n_parts, kWsRxWarps, 0.0, wbs);
+      size_t o = 0;
+      wv.smem_cs = (uint32_t)o;
+      o += align_up((size_t)2 * (K + 2) * kTile * 8, 128);
+      wv.smem_ds = (uint32_t)o;
+      o += align_up((size_t)2 * K * kTile * 8, 128);
+      wv.smem_q = (uint32_t)o;
+      o += align_up((size_t)2 * (wbs.rc + 1) * kTile * 8, 128);
+      wv.smem_acc = (uint32_t)o;
+      o += align_up((size_t)K * kTile * 8, 128);
+      wv.smem_mech = (uint32_t)o;
+      o += wbs.stride * n_parts;
+      wv.smem_misc = (uint32_t)o;
+      o += align_up((size_t)2 * Kp * 8 + (size_t)2 * kWsStRows * kTile * 8 + (size_t)2 * 3 * kTile * 8 + 16 * 8 +
+                        (size_t)kWsHelpWarps * spw_h * 4, 128);
+      wv.smem_total = (uint32_t)o;
+      if (o <= (size_t)prop.sharedMemPerBlockOptin) {
+        ws_ok = true;
+        wv.K = K;
+        wv.I = I;
+        wv.n_parts = n_parts;
+        wv.rc = wbs.rc;
+        wv.spw = spw_h;
+        wv.need_lnctot = need_lnctot;
+        wv.chunk_stride = (uint32_t)wbs.stride;
+        ws_sp_of = assign_species(rx, K, I, kWsHelpWarps, spw_h);
+      }
+    }
   }
 
   psr_mech* m = new (std::nothrow) psr_mech();
@@ -520,6 +591,23 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     cleanup();
     return fail(PSR_ECUDA, "kernel does not fit on this device (%s)", cudaGetErrorString(e));
   }
+  if (ws_ok) {
+    if ((e = cudaMalloc(&m->d_ws_chunks, wbs.all.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_ws_chunks, wbs.all.data(), wbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_ws_sp_of, 4 * ws_sp_of.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_ws_sp_of, ws_sp_of.data(), 4 * ws_sp_of.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = ws_set_smem(wv.smem_total)) != cudaSuccess) {
+      cleanup();
+      return cuda_fail(e, "warp-specialised kernel tables");
+    }
+    wv.chunks = m->d_ws_chunks;
+    wv.sp_of = m->d_ws_sp_of;
+    wv.invW = m->d_invW;
+    wv.Wm = m->d_W;
+    wv.exp_tab = m->d_exptab;
+    m->ws = wv;
+    m->ws_ok = true;
+  }
   *out = m;
   return PSR_OK;
 }
@@ -534,6 +622,8 @@ void psr_mech_free(psr_mech* m) {
   cudaFree(m->d_sp_of);
   cudaFree(m->d_rec_base);
   cudaFree(m->d_scratch);
+  cudaFree(m->d_ws_chunks);
+  cudaFree(m->d_ws_sp_of);
   delete m;
 }
 
@@ -569,6 +659,17 @@ psr_status check_common(const psr_mech* m, int64_t N, const double* T, const dou
 }
 
 psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
+  // wdot / residual / rate-constant calls of a mechanism whose tables stay resident: the warp-specialised kernel
+  if (m->ws_ok && !m->opt_fused_only && (a.flags & ~(kOutWdot | kOutF | kOutKf | kOutKr | kOutQ)) == 0) {
+    auto al16 = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; };
+    const bool wantF = (a.flags & kOutF) != 0;
+    // whole tiles come by one bulk copy per species row: needs 16-byte aligned rows
+    const int bulk_ok = al16(a.T) && al16(a.P) && al16(a.Y) && (a.ld % 2 == 0) && (!wantF || (al16(a.Yin) && al16(a.tau)));
+    const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
+    cudaError_t e = launch_ws(m->ws, a, grid, bulk_ok, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, fn);
+    return PSR_OK;
+  }
   const int64_t cap = (int64_t)m->n_sm * m->ctas_per_sm;
   const int grid = (int)std::min<int64_t>(a.n_tiles, cap);
   cudaError_t e = launch_eval(m->nw, m->spw, m->rl, m->view, a, grid, (cudaStream_t)stream);
@@ -659,8 +760,7 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
   if (Nb > wave) Nb -= Nb % wave;
   Nb = std::min(Nb, N);
   Nb = std::min<int64_t>(Nb, ((int64_t)1 << 31) / (n + 32) - 1);   // state indices of a launch fit 32 bits
-  bool unhoisted = false;   // diagnostic: every column a full evaluation (tests compare the two sweeps)
-  if (const char* e = getenv("PSR_JAC_UNHOISTED")) unhoisted = atoi(e) != 0;
+  const bool unhoisted = m->opt_jac_unhoisted != 0;   // diagnostic: every column a full evaluation (tests compare the two sweeps)
 
   const size_t tab_bytes = align_up((size_t)Nb * row_bytes, 256);
   const size_t need = tab_bytes + (F0 ? 0 : (size_t)N * n * 8);
@@ -762,6 +862,16 @@ psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F,
   if (!J || !F || !dt || !dx || !info) return fail(PSR_EINVAL, "psr_ptc_solve: null J, F, dt, dx or info");
   if (dx == F) return fail(PSR_EINVAL, "psr_ptc_solve: dx must not alias F");
   return solve_impl("psr_ptc_solve", N, n, J, dx, info, F, dt, stream);
+}
+
+psr_status psr_mech_set_option(psr_mech* m, int32_t option, int32_t value) {
+  g_err.clear();
+  if (!m) return fail(PSR_EINVAL, "psr_mech_set_option: null mechanism");
+  switch (option) {
+    case PSR_OPT_JAC_UNHOISTED: m->opt_jac_unhoisted = value != 0; return PSR_OK;
+    case PSR_OPT_FUSED_ONLY: m->opt_fused_only = value != 0; return PSR_OK;
+    default: return fail(PSR_EINVAL, "psr_mech_set_option: unknown option %d", (int)option);
+  }
 }
 
 psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {

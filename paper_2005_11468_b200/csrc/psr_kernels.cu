@@ -18,6 +18,7 @@
 #include <type_traits>
 
 #include "psr_math.cuh"
+#include "psr_ptx.cuh"
 #include "psr_tables.h"
 
 namespace psr {
@@ -26,53 +27,6 @@ __device__ constexpr double kRgas = 8.31446261815324e7;  // erg/mol/K
 __device__ constexpr double kLog10e = 0.43429448190325182765;
 constexpr int PSR_T_PLAIN = 0, PSR_T_THREE_BODY = 1, PSR_T_LINDEMANN = 2, PSR_T_TROE = 3;  // = PSR_RX_* of psr.h
 
-// ------------------------------------------------------------------ mbarrier / bulk copy
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar))
-      : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t done;
-  do {
-    asm volatile(
-        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.b32 %0, 1, 0, p;\n}"
-        : "=r"(done)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-  } while (!done);
-}
-
-__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_global) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src_global) : "memory");
-}
-__device__ __forceinline__ double ldg_nc(const double* p) {
-  double v;
-  asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
-  return v;
-}
-
-// ------------------------------------------------------------------ shared-memory access by 32-bit address
-// (volatile so that loads are neither merged across tiles nor moved over barriers by the front end)
-__device__ __forceinline__ double lds64(uint32_t addr) {
-  double v;
-  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ void sts64(uint32_t addr, double v) {
-  asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v));
-}
 template <int R>
 struct RowIO;
 template <>

@@ -96,6 +96,27 @@ struct MechView {
   uint32_t smem_cs, smem_q, smem_mech, smem_tab, smem_misc, smem_total;  // byte offsets / sizes of the dynamic smem carve-up
 };
 
+
+// ---- warp-specialised kernel (psr_ws.cu): 12 reaction warps + 4 helper warps per CTA, the mechanism cut into
+// n_parts resident blobs (same ChunkHdr layout, records dealt to the 12 reaction warps, gather lists per part)
+constexpr int kWsRxWarps = 12, kWsHelpWarps = 4, kWsWarps = kWsRxWarps + kWsHelpWarps;
+constexpr int kWsStRows = 8;      // per-tile state rows: T, ln T, 1/T, rho, C_tot, ln C_tot, 1/tau, 1/rho
+constexpr int kWsMaxParts = 8;
+
+struct WsView {
+  const unsigned char* chunks;  // n_parts blobs, chunk_stride bytes apart
+  const double* invW;           // [K] 1/W
+  const double* Wm;             // [K] W
+  const int32_t* sp_of;         // [kWsHelpWarps][spw] species owned by a helper warp (owned ones first, then -1)
+  const double* exp_tab;        // [32] 2^(j/32)
+  int32_t K, I;
+  int32_t n_parts, rc;          // rc: rows of a q buffer (+1 zero row)
+  int32_t spw;                  // species slots per helper warp (<= 32)
+  int32_t need_lnctot;
+  uint32_t chunk_stride;
+  uint32_t smem_cs, smem_ds, smem_q, smem_acc, smem_mech, smem_misc, smem_total;
+};
+
 // what one launch produces
 enum : uint32_t {
   kOutWdot = 1u, kOutQ = 2u, kOutKf = 4u, kOutKr = 8u, kOutF = 16u, kOutF0 = 64u,

@@ -156,8 +156,9 @@ def test_leading_dimension_larger_than_N(torch_cuda, binding):
     torch.cuda.synchronize()
     for Fx in (Fbig[:, :100], Fa, Fe, Fe2[:, :100]):
         assert residual_rel_err(Fx.cpu().numpy(), refF["F"]).max() <= TOL_F
-    for wx in (w2big[:, :100], wa, we):
+    for wx in (w2big[:, :100], wa):
         assert np.array_equal(wx.cpu().numpy(), w[:, :100])
+    assert wdot_masked_rel_err(we.cpu().numpy(), w[:, :100])[0].max() <= 1e-11   # fused kernel vs warp-specialised one
     for big in (Fbig, w2big, Fe2):
         assert bool((big[:, 100:] == -7.0).all())  # padding untouched
     dense = torch.empty((mech.n_species, 100), dtype=torch.float64, device="cuda")
@@ -324,7 +325,13 @@ def test_C1_full_size_residual_every_reactor(torch_cuda, binding):
     # adiabatic residual: species rows bit-identical, energy row against the oracle
     Tin = torch.full_like(T, 300.0)
     Fe, FTe, we = gm.eval_residual_energy(T, P, Y, Tin, Yin, tau, want_wdot=True)
-    assert np.array_equal(Fe.cpu().numpy(), Fh) and np.array_equal(we.cpu().numpy(), wh)
+    # (the energy-row call runs the fused kernel, the plain one the warp-specialised kernel: same arithmetic per
+    # reaction, another summation order in nu^T q and in sum Y_i/W_i)
+    gm.set_option(binding.OPT_FUSED_ONLY, 1)
+    Ff, wf = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+    gm.set_option(binding.OPT_FUSED_ONLY, 0)
+    assert np.array_equal(Fe.cpu().numpy(), Ff.cpu().numpy()) and np.array_equal(we.cpu().numpy(), wf.cpu().numpy())
+    check_full_batch(mech, batch, wf.cpu().numpy(), Ff.cpu().numpy())
     refe = orc.evaluate_energy(om, batch.T, batch.P, batch.Y, np.full(batch.n, 300.0), batch.Yin, batch.tau)
     rho = batch.P / (RGAS * batch.T * (batch.Y / mech.W[:, None]).sum(axis=0))
     scale = energy_scale(mech, batch, np.full(batch.n, 300.0), ref["wdot"], rho)
@@ -404,11 +411,9 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     J2 = gm.fd_jacobian(*args)  # internal F0 scratch path
     # diagnostic sweep in which every column is a full evaluation: the production sweep takes the T-only
     # factors of the Y columns from the base state's rate table and must give the same bits
-    os.environ["PSR_JAC_UNHOISTED"] = "1"
-    try:
-        J3 = gm.fd_jacobian(*args)
-    finally:
-        del os.environ["PSR_JAC_UNHOISTED"]
+    gm.set_option(binding.OPT_JAC_UNHOISTED, 1)
+    J3 = gm.fd_jacobian(*args)
+    gm.set_option(binding.OPT_JAC_UNHOISTED, 0)
     torch.cuda.synchronize()
     J, F0, J2, J3 = J.cpu().numpy(), F0.cpu().numpy(), J2.cpu().numpy(), J3.cpu().numpy()
     gm.close()
@@ -455,12 +460,14 @@ def test_energy_residual_against_oracle(torch_cuda, binding, cfg, n):
     gm = binding.Mechanism.from_synth(mech)
     args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, Tin, batch.Yin, batch.tau)]
     F, FT, wdot = gm.eval_residual_energy(*args, want_wdot=True)
+    gm.set_option(binding.OPT_FUSED_ONLY, 1)
     F2 = gm.eval_residual(args[0], args[1], args[2], args[4], args[5])
+    gm.set_option(binding.OPT_FUSED_ONLY, 0)
     torch.cuda.synchronize()
     F, FT, wdot, F2 = F.cpu().numpy(), FT.cpu().numpy(), wdot.cpu().numpy(), F2.cpu().numpy()
     gm.close()
     ref = orc.evaluate_energy(oracle_mech(mech), batch.T, batch.P, batch.Y, Tin, batch.Yin, batch.tau)
-    assert np.array_equal(F, F2)                                       # species rows: the same path
+    assert np.array_equal(F, F2)                                       # species rows: the same path (fused kernel)
     assert residual_rel_err(F, ref["F"]).max() <= TOL_F
     rho = batch.P / (8.31446261815324e7 * batch.T * (batch.Y / mech.W[:, None]).sum(axis=0))
     S = energy_scale(mech, batch, Tin, ref["wdot"], rho)
@@ -492,11 +499,9 @@ def test_fd_jacobian_energy_floor_criterion(torch_cuda, binding, cfg, n):
     dTin = dev(torch, Tin)
     J, F0 = gm.fd_jacobian(*args, want_F0=True, Tin=dTin)
     Jp = gm.fd_jacobian(*args)
-    os.environ["PSR_JAC_UNHOISTED"] = "1"
-    try:
-        J3 = gm.fd_jacobian(*args, Tin=dTin)
-    finally:
-        del os.environ["PSR_JAC_UNHOISTED"]
+    gm.set_option(binding.OPT_JAC_UNHOISTED, 1)
+    J3 = gm.fd_jacobian(*args, Tin=dTin)
+    gm.set_option(binding.OPT_JAC_UNHOISTED, 0)
     _, FT = gm.eval_residual_energy(args[0], args[1], args[2], dTin, args[3], args[4])
     torch.cuda.synchronize()
     J, F0, Jp, J3, FT = (x.cpu().numpy() for x in (J, F0, Jp, J3, FT))
