@@ -106,7 +106,10 @@ struct BlobSet {
 
 // Cuts the mechanism into n_chunks chunks, deals every chunk's records to nw warps and serialises the chunk
 // blobs (psr_tables.h): records, aux records, efficiency entries, factor pool, per-species gather lists.
-void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out) {
+// ws_sp_of (may be null): species ownership [kWsHelpWarps][ws_spw] of the warp-specialised kernel, whose gather
+// lists are one flat stream of 4-entry groups per helper warp (see psr_tables.h) instead of lists per species.
+void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out,
+                 const std::vector<int32_t>* ws_sp_of = nullptr, int ws_spw = 0) {
   const uint32_t row_bytes = (uint32_t)kRowBytes;
   const int rc = (I + n_chunks - 1) / n_chunks;
   out.n_chunks = n_chunks;
@@ -202,13 +205,40 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
       gent.insert(gent.end(), grp.begin(), grp.end());
       while (gent.size() % 4) gent.push_back(zero_off);
     };
-    for (int s = 0; s < K; ++s) {
-      gptr[2 * s] = (uint32_t)gent.size();
-      add_group(pos[s]);
-      gptr[2 * s + 1] = (uint32_t)gent.size();
-      add_group(neg[s]);
+    std::vector<uint16_t> ws_range(2 * kWsHelpWarps, 0);   // [helper warp] first group, one past its last group
+    if (!ws_sp_of) {
+      for (int s = 0; s < K; ++s) {
+        gptr[2 * s] = (uint32_t)gent.size();
+        add_group(pos[s]);
+        gptr[2 * s + 1] = (uint32_t)gent.size();
+        add_group(neg[s]);
+      }
+      gptr[2 * K] = (uint32_t)gent.size();
+    } else {
+      // flat streams: for every helper warp the groups of its species in ownership order, "+" groups then "-"
+      // groups of a species; every owned species ends with a group that carries kGatherLast (a species without
+      // a reaction in this part gets one all-zero group), the stream has an even number of groups and four
+      // all-zero groups behind it so that the kernel's reads two trips ahead stay inside the blob
+      gptr.assign(1, 0);
+      for (int hw = 0; hw < kWsHelpWarps; ++hw) {
+        ws_range[2 * hw] = (uint16_t)(gent.size() / 4);
+        for (int jj = 0; jj < ws_spw; ++jj) {
+          const int s = (*ws_sp_of)[(size_t)hw * ws_spw + jj];
+          if (s < 0) break;
+          const size_t first = gent.size();
+          add_group(pos[s]);
+          const size_t first_neg = gent.size();
+          add_group(neg[s]);
+          if (gent.size() == first) gent.insert(gent.end(), 4, zero_off);
+          for (size_t g = first_neg; g < gent.size(); g += 4)
+            if (!neg[s].empty()) gent[g] |= kGatherNeg;
+          gent[gent.size() - 4] |= kGatherLast;
+        }
+        if ((gent.size() / 4 - ws_range[2 * hw]) % 2) gent.insert(gent.end(), 4, zero_off);   // the kernel takes two groups per trip
+        ws_range[2 * hw + 1] = (uint16_t)(gent.size() / 4);
+        gent.insert(gent.end(), 16, zero_off);
+      }
     }
-    gptr[2 * K] = (uint32_t)gent.size();
 
     ChunkHdr hdr{};
     hdr.n_rx = n_rx;
@@ -217,6 +247,11 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
     hdr.rec_base = (uint32_t)out.rec_base[c];
     for (int wv = 0; wv < kMaxWarps; ++wv)
       for (int cl = 0; cl < kClsLong + 2; ++cl) hdr.wb[wv][cl] = (uint16_t)chunk_wb[c][(size_t)wv * (kClsLong + 2) + cl];
+    if (ws_sp_of)
+      for (int hw = 0; hw < kWsHelpWarps; ++hw) {
+        hdr.wb[kWsRxWarps + hw][0] = ws_range[2 * hw];
+        hdr.wb[kWsRxWarps + hw][1] = ws_range[2 * hw + 1];
+      }
     size_t off = sizeof(ChunkHdr) + sizeof(RxRec) * n_rx;
     hdr.off_aux = (uint32_t)off;
     off += sizeof(AuxRec) * auxs.size();
@@ -468,8 +503,9 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   if (K <= 32 * kWsHelpWarps) {
     const int spw_h = (K + kWsHelpWarps - 1) / kWsHelpWarps;
     const int Kp = (K + 1) & ~1;
+    ws_sp_of = assign_species(rx, K, I, kWsHelpWarps, spw_h);
     for (int n_parts = 1; n_parts <= kWsMaxParts && n_parts <= I && !ws_ok; ++n_parts) {
-      build_blobs(rx, K, I, n_parts, kWsRxWarps, 0.0, wbs);
+      build_blobs(rx, K, I, n_parts, kWsRxWarps, 0.0, wbs, &ws_sp_of, spw_h);
       size_t o = 0;
       wv.smem_cs = (uint32_t)o;
       o += align_up((size_t)2 * (K + 2) * kTile * 8, 128);
@@ -483,7 +519,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
       o += wbs.stride * n_parts;
       wv.smem_misc = (uint32_t)o;
       o += align_up((size_t)2 * Kp * 8 + (size_t)2 * kWsStRows * kTile * 8 + (size_t)2 * 3 * kTile * 8 + 16 * 8 +
-                        (size_t)kWsHelpWarps * spw_h * 4, 128);
+                        align_up((size_t)kWsHelpWarps * spw_h * 4, 32) + (size_t)kWsHelpWarps * spw_h * 32, 128);
       wv.smem_total = (uint32_t)o;
       if (o <= (size_t)prop.sharedMemPerBlockOptin) {
         ws_ok = true;
@@ -494,7 +530,6 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         wv.spw = spw_h;
         wv.need_lnctot = need_lnctot;
         wv.chunk_stride = (uint32_t)wbs.stride;
-        ws_sp_of = assign_species(rx, K, I, kWsHelpWarps, spw_h);
       }
     }
   }

@@ -99,9 +99,15 @@ struct MechView {
 
 // ---- warp-specialised kernel (psr_ws.cu): 12 reaction warps + 4 helper warps per CTA, the mechanism cut into
 // n_parts resident blobs (same ChunkHdr layout, records dealt to the 12 reaction warps, gather lists per part)
-constexpr int kWsRxWarps = 12, kWsHelpWarps = 4, kWsWarps = kWsRxWarps + kWsHelpWarps;
+constexpr int kWsRxWarps = 11, kWsHelpWarps = 5, kWsWarps = kWsRxWarps + kWsHelpWarps;
 constexpr int kWsStRows = 8;      // per-tile state rows: T, ln T, 1/T, rho, C_tot, ln C_tot, 1/tau, 1/rho
 constexpr int kWsMaxParts = 8;
+// Gather lists of the warp-specialised kernel: one flat stream of 4-entry groups per (part, helper warp), groups
+// wb[kWsRxWarps + hw][0] .. wb[kWsRxWarps + hw][1] - 1 of the part's gent array.  A group holds four byte offsets
+// of q rows (multiples of kRowBytes, the zero row pads) that belong to ONE species and ONE sign; the low bits of
+// its first entry say what to do with the group's sum.
+constexpr uint32_t kGatherNeg = 1u;    // subtract the group's sum instead of adding it
+constexpr uint32_t kGatherLast = 2u;   // last group of the species: its row of nu^T q is complete for this part
 
 struct WsView {
   const unsigned char* chunks;  // n_parts blobs, chunk_stride bytes apart

@@ -6,10 +6,10 @@
 // the barriers 0.05 ms, the gather 0.035 ms, the epilogue 0.01 ms, none of it overlapped).  Here the phases
 // are roles of different warps that meet only through mbarriers:
 //
-//   reaction warps (12)  a3..a7: k_f, K_c, k_r, [M], falloff, q of their share of the reactions, tile after
+//   reaction warps (11)  a3..a7: k_f, K_c, k_r, [M], falloff, q of their share of the reactions, tile after
 //                        tile without a CTA barrier; q goes to one of two q buffers (one "part" of the
 //                        mechanism each), concentrations and per-reactor state come from one of two C tiles.
-//   helper warps (4)     a1: TMA bulk loads of the tile after next, state preparation (Wbar, rho, C_i, ln T,
+//   helper warps (5)     a1: TMA bulk loads of the tile after next, state preparation (Wbar, rho, C_i, ln T,
 //                        ln C_tot) of the next tile;  a8: gather of the q buffer the reaction warps have just
 //                        filled (nu^T q, fixed order, partial sums in shared memory between parts);
 //                        a9: residual and stores.
@@ -43,6 +43,16 @@ constexpr int T_PLAIN = 0, T_THREE_BODY = 1, T_LINDEMANN = 2, T_TROE = 3;  // = 
 constexpr int B_BLOB = 0, B_IN = 1, B_FULLC = 3, B_EMPTYC = 5, B_FULLQ = 7, B_EMPTYQ = 9, B_COUNT = 11;
 // per-tile state rows St[b][row][lane]
 constexpr int ST_T = 0, ST_LNT = 1, ST_INVT = 2, ST_RHO = 3, ST_CTOT = 4, ST_LNCTOT = 5, ST_INVTAU = 6, ST_INVRHO = 7;
+
+// what the gather needs when a species' row of nu^T q is complete (one entry per helper warp and species slot)
+struct __align__(16) SpEnt {
+  uint32_t row_off;        // byte offset of the species' row in a [K][32] tile
+  uint32_t next_row_off;   // the same of the warp's next owned species
+  uint64_t pad_;
+  int64_t goff;            // byte offset of the species' row in the [K][ld] outputs
+  double W;                // molar mass
+};
+static_assert(sizeof(SpEnt) == 32, "SpEnt layout");
 
 struct RxCtx {
   double T, lnT, invT;
@@ -225,7 +235,8 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
   double* St0 = W_s + Kp;                                          // [2][kWsStRows][32]
   double* tp0 = St0 + 2 * kWsStRows * kTile;                       // [2][3][32]: T, P, tau as loaded
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp0 + 2 * 3 * kTile);
-  int32_t* sp_s = reinterpret_cast<int32_t*>(bars + B_COUNT + 1);  // [4][spw]
+  int32_t* sp_s = reinterpret_cast<int32_t*>(bars + B_COUNT + 1);  // [helper warps][spw]
+  SpEnt* sptab = reinterpret_cast<SpEnt*>(sp_s + ((kWsHelpWarps * mv.spw + 7) & ~7));   // [helper warps][spw]
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -257,7 +268,19 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     invW_s[i] = mv.invW[i];
     W_s[i] = mv.Wm[i];
   }
-  for (int i = threadIdx.x; i < kWsHelpWarps * mv.spw; i += kWsWarps * 32) sp_s[i] = mv.sp_of[i];
+  for (int i = threadIdx.x; i < kWsHelpWarps * mv.spw; i += kWsWarps * 32) {
+    sp_s[i] = mv.sp_of[i];
+    // the flush table of the gather: slots past a warp's last owned species repeat that species
+    const int hw_ = i / mv.spw;
+    int jj = i - hw_ * mv.spw, jn = jj + 1;
+    while (jj > 0 && mv.sp_of[hw_ * mv.spw + jj] < 0) --jj;
+    if (jn >= mv.spw || mv.sp_of[hw_ * mv.spw + jn] < 0) jn = jj;
+    const int s_ = max(mv.sp_of[hw_ * mv.spw + jj], 0), sn_ = max(mv.sp_of[hw_ * mv.spw + jn], 0);
+    sptab[i].row_off = (uint32_t)s_ * kRowBytes;
+    sptab[i].next_row_off = (uint32_t)sn_ * kRowBytes;
+    sptab[i].goff = (int64_t)s_ * a.ld * 8;
+    sptab[i].W = mv.Wm[s_];
+  }
   __syncthreads();
 
   if (w < kWsRxWarps) {
@@ -389,6 +412,77 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
       if (lane == 0) mbar_arrive(&bars[B_FULLC + b]);
     };
 
+    // a8 (Eq. 4) and a9 (Eq. 2): this warp's stream of 4-entry groups of nu^T q of one part (psr_tables.h), in a fixed
+    // order, two groups per trip.  Software-pipelined: the q rows of a pair are read one trip before they are
+    // added and its offsets two trips before (the stream ends with padding groups), so a trip adds values that
+    // have already arrived.  A group's sum enters the species' running sum with the group's sign; the group that
+    // ends a species stores the sum -- to the partial-sum tile, or (last part) as wdot and F to global memory.
+    auto gather_part = [&](auto first_tag, auto last_tag, const uint32_t gs, const int n_groups, const uint32_t q_lane,
+                           const int b, const int64_t r, const bool valid) {
+      constexpr bool FIRST = decltype(first_tag)::value, LAST = decltype(last_tag)::value;
+      auto ld_group = [&](uint32_t addr, uint4& o) {
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w) : "r"(addr));
+      };
+      const uint32_t acc_lane = smem_u32(acc_s) + lane * 8;
+      const uint32_t d_lane = smem_u32(Ds0 + b * ds_elems) + lane * 8;
+      const uint32_t tbl = smem_u32(sptab + hw * mv.spw);
+      double invtau = 0.0, invrho = 0.0;
+      if (LAST && wantF) {
+        invtau = St0[(b * kWsStRows + ST_INVTAU) * kTile + lane];
+        invrho = St0[(b * kWsStRows + ST_INVRHO) * kTile + lane];
+      }
+      const bool out_w = (a.flags & kOutWdot) != 0;
+      const char* wdot_r = reinterpret_cast<const char*>(a.wdot + r);
+      const char* F_r = reinterpret_cast<const char*>(a.F + r);
+      uint32_t te = tbl;   // table entry of the species being summed
+      double acc = 0.0;
+      if (!FIRST && n_groups > 0) acc = lds64(acc_lane + reinterpret_cast<const SpEnt*>(sptab + hw * mv.spw)->row_off);
+      auto flush = [&]() {
+        uint32_t row_off, pad;
+        double W;
+        int64_t goff;
+        asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(row_off), "=r"(pad) : "r"(te));
+        if (LAST) {
+          asm volatile("ld.shared.v2.b64 {%0, %1}, [%2+16];" : "=l"(goff), "=d"(W) : "r"(te));
+          if (valid) {
+            if (out_w) *reinterpret_cast<double*>(const_cast<char*>(wdot_r) + goff) = acc;
+            if (wantF)
+              *reinterpret_cast<double*>(const_cast<char*>(F_r) + goff) = fma(lds64(d_lane + row_off), invtau, -(acc * (W * invrho)));
+          }
+        } else {
+          sts64(acc_lane + row_off, acc);
+        }
+        te += sizeof(SpEnt);
+        // (the entry after the last owned species is a copy of the last one: harmless read)
+        if (FIRST) acc = 0.0;
+        else acc = lds64(acc_lane + pad);   // pad = row offset of the NEXT owned species
+      };
+      auto sgn = [](uint32_t ctl) { return __hiloint2double((int)(0x3ff00000u ^ (ctl << 31)), 0); };
+      uint4 oa, ob;
+      ld_group(gs, oa);
+      ld_group(gs + 16, ob);
+      double a0 = lds64(q_lane + (oa.x & ~3u)), a1 = lds64(q_lane + oa.y), a2 = lds64(q_lane + oa.z), a3 = lds64(q_lane + oa.w);
+      double b0 = lds64(q_lane + (ob.x & ~3u)), b1 = lds64(q_lane + ob.y), b2 = lds64(q_lane + ob.z), b3 = lds64(q_lane + ob.w);
+      uint32_t ca = oa.x, cb = ob.x;
+      ld_group(gs + 32, oa);
+      ld_group(gs + 48, ob);
+#pragma unroll 1
+      for (int i = 0; i < n_groups; i += 2) {
+        const double ta = (a0 + a2) + (a1 + a3), tb = (b0 + b2) + (b1 + b3);
+        const uint32_t c0 = ca, c1 = cb;
+        ca = oa.x;
+        cb = ob.x;
+        a0 = lds64(q_lane + (oa.x & ~3u)), a1 = lds64(q_lane + oa.y), a2 = lds64(q_lane + oa.z), a3 = lds64(q_lane + oa.w);
+        b0 = lds64(q_lane + (ob.x & ~3u)), b1 = lds64(q_lane + ob.y), b2 = lds64(q_lane + ob.z), b3 = lds64(q_lane + ob.w);
+        ld_group(gs + (uint32_t)(i + 4) * 16u, oa);
+        ld_group(gs + (uint32_t)(i + 5) * 16u, ob);
+        acc = fma(ta, sgn(c0), acc);
+        if (c0 & kGatherLast) flush();
+        acc = fma(tb, sgn(c1), acc);
+        if (c1 & kGatherLast) flush();
+      }
+    };
+
     const int64_t stride = gridDim.x;
     int64_t tile = blockIdx.x;
     if (tile < a.n_tiles) issue_loads(tile, 0);
@@ -398,8 +492,6 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += stride) {
       const int b = lt & 1;
       if (tile + stride < a.n_tiles) prologue(lt + 1);
-      const double* Db = Ds0 + b * ds_elems;
-      const double* St = St0 + b * kWsStRows * kTile;
       const int64_t r = tile * kTile + lane;
       const bool valid = r < a.N;
       for (int p = 0; p < mv.n_parts; ++p) {
@@ -407,50 +499,14 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
         const bool first = p == 0, last = p == mv.n_parts - 1;
         const unsigned char* blob = mech + (size_t)p * mv.chunk_stride;
         const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
-        const uint32_t* gptr = reinterpret_cast<const uint32_t*>(blob + hdr->off_gptr);
-        const uint4* gent = reinterpret_cast<const uint4*>(blob + hdr->off_gent);
+        const uint32_t gs = smem_u32(blob + hdr->off_gent) + (uint32_t)hdr->wb[kWsRxWarps + hw][0] * 16u;
+        const int n_groups = (int)hdr->wb[kWsRxWarps + hw][1] - (int)hdr->wb[kWsRxWarps + hw][0];   // even
         const uint32_t q_lane = smem_u32(qh0 + qb * q_elems) + lane * 8;
-        double invtau = 0.0, invrho = 0.0;
-        if (last && wantF) {
-          invtau = St[ST_INVTAU * kTile + lane];
-          invrho = St[ST_INVRHO * kTile + lane];
-        }
         mbar_wait(&bars[B_FULLQ + qb], u & 1);
-        // a8 (Eq. 4): rows of nu^T q of this part for the species this warp owns, in the fixed order of the
-        // gather lists, 4 entries per step ("+" list, then "-" list; groups padded with the zero row)
-#pragma unroll 1
-        for (int jj = 0; jj < n_my; ++jj) {
-          const int s = my_sp[jj];
-          const uint32_t g0 = gptr[2 * s] >> 2, g1 = gptr[2 * s + 1] >> 2, g2 = gptr[2 * s + 2] >> 2;
-          double a0 = first ? 0.0 : acc_s[s * kTile + lane], a1 = 0.0;
-#pragma unroll 1
-          for (uint32_t e = g0; e < g1; ++e) {
-            const uint4 o = gent[e];
-            const double v0 = lds64(q_lane + o.x), v1 = lds64(q_lane + o.y), v2 = lds64(q_lane + o.z), v3 = lds64(q_lane + o.w);
-            a0 += v0;
-            a1 += v1;
-            a0 += v2;
-            a1 += v3;
-          }
-#pragma unroll 1
-          for (uint32_t e = g1; e < g2; ++e) {
-            const uint4 o = gent[e];
-            const double v0 = lds64(q_lane + o.x), v1 = lds64(q_lane + o.y), v2 = lds64(q_lane + o.z), v3 = lds64(q_lane + o.w);
-            a0 -= v0;
-            a1 -= v1;
-            a0 -= v2;
-            a1 -= v3;
-          }
-          a0 += a1;
-          if (!last) {
-            acc_s[s * kTile + lane] = a0;
-          } else if (valid) {
-            // a9 (Eq. 2 at steady state): F_i = (Y_i - Y_in,i)/tau - wdot_i W_i/rho
-            const int64_t o = (int64_t)s * a.ld + r;
-            if (a.flags & kOutWdot) a.wdot[o] = a0;
-            if (wantF) a.F[o] = fma(Db[s * kTile + lane], invtau, -(a0 * (W_s[s] * invrho)));
-          }
-        }
+        if (first && last) gather_part(std::true_type{}, std::true_type{}, gs, n_groups, q_lane, b, r, valid);
+        else if (first) gather_part(std::true_type{}, std::false_type{}, gs, n_groups, q_lane, b, r, valid);
+        else if (last) gather_part(std::false_type{}, std::true_type{}, gs, n_groups, q_lane, b, r, valid);
+        else gather_part(std::false_type{}, std::false_type{}, gs, n_groups, q_lane, b, r, valid);
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[B_EMPTYQ + qb]);
       }
