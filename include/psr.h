@@ -59,7 +59,8 @@ typedef struct {
                                 cp/R = a0+a1 T+a2 T^2+a3 T^3+a4 T^4
                                 h/RT = a0+a1 T/2+a2 T^2/3+a3 T^3/4+a4 T^4/5+a5/T
                                 s/R  = a0 ln T+a1 T+a2 T^2/2+a3 T^3/3+a4 T^4/4+a6 */
-  const double *A, *b, *Ea;  /* [I]   k = A T^b exp(-Ea/(R_c T)) (Eq. 6); the high-pressure limit for falloff */
+  const double *A, *b, *Ea;  /* [I]   k = A T^b exp(-Ea/(R_c T)) (Eq. 6); the high-pressure limit for falloff.
+                                Any finite A: negative (duplicate reactions) and zero are evaluated as defined */
   const uint8_t* rtype;      /* [I]   PSR_RX_* */
   const uint8_t* reversible; /* [I]   1: k_r = k_f/K_c (Eq. 7); 0: k_r = 0 */
   const int32_t *reac_ptr, *reac_sp, *reac_nu; /* CSR over reactions: reactant species and nu' in {1,2,3} */
@@ -67,13 +68,15 @@ typedef struct {
   const int32_t *eff_ptr, *eff_sp;             /* CSR over reactions: third-body efficiencies (default 1) */
   const double* eff_val;
   const double *A0, *b0, *Ea0; /* [I]   low-pressure limit, read when rtype >= 2 */
-  const double* troe;          /* [I][4] alpha, T***, T*, T**, read when rtype == 3 */
+  const double* troe;          /* [I][4] alpha, T***, T*, T**, read when rtype == 3; T***, T* != 0; the
+                                  three-parameter form (no exp(-T** / T) term) is written T** = +inf */
 } psr_mech_desc;
 
 /* psr_mech_load: validate the description, build the device tables (per-reaction log-linear rate and
  * equilibrium coefficients, factor lists, per-chunk CSR of nu^T) and upload them once.
  * PSR_EINVAL: null pointers, K or I < 1, species index out of range, nu outside 1..3, W <= 0,
- *   non-monotone CSR pointers, unknown rtype, A <= 0 (A0 <= 0 for falloff).
+ *   non-monotone CSR pointers, unknown rtype, non-finite coefficients (A, b, Ea, A0, b0, Ea0, NASA, efficiencies;
+ *   T** of a Troe reaction may be +inf), T*** or T* = 0.
  * PSR_EUNSUPPORTED: K > 512, more than 15 concentration factors on one side of a reaction, more
  *   than 65535 efficiency entries.  *out is set only on PSR_OK.  Synchronous. */
 psr_status psr_mech_load(const psr_mech_desc* desc, psr_mech** out);
@@ -114,12 +117,19 @@ psr_status psr_eval_residual_energy(const psr_mech* mech, int64_t N, const doubl
  * tabulates the reaction factors that depend on T only), the T column, and the K species columns
  * (which reuse those factors: a Y perturbation leaves them unchanged; the result is bit-identical to
  * evaluating every column in full).  The rate table (and F0 when NULL is passed) live in a scratch
- * buffer owned by `mech`, grown on demand with a stream synchronisation the first time a larger N is
- * seen: calls of psr_fd_jacobian on ONE mechanism handle must therefore not run concurrently on
- * different streams.  PSR_ENOMEM if the scratch buffer cannot be allocated. */
+ * buffer owned by `mech`: calls of psr_fd_jacobian on ONE mechanism handle must therefore not run
+ * concurrently on different streams.  The buffer grows (cudaMalloc, PSR_ENOMEM on failure) the first time a
+ * larger N is seen, or ahead of time through psr_mech_reserve; an outgrown buffer stays allocated until
+ * psr_mech_free, so work already enqueued and captured graphs that point at it stay valid.
+ * Stream capture: the call allocates nothing when the scratch is large enough, and returns PSR_EINVAL
+ * instead of allocating inside a capture -- call psr_mech_reserve(mech, N) before capturing. */
 psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, const double* P,
                            const double* Y, const double* Yin, const double* tau, int64_t ld,
                            double* J, double* F0, void* stream);
+
+/* Sizes the scratch of psr_fd_jacobian / psr_fd_jacobian_energy for batches of up to N reactors (including the
+ * internal F0 used when the caller passes none).  Synchronous (cudaMalloc); never shrinks. */
+psr_status psr_mech_reserve(psr_mech* mech, int64_t N);
 
 /* The same sweep for the adiabatic system (NEXT-1): row 0 of the residual is the energy row F_T of
  * psr_eval_residual_energy instead of T - T_set, so row 0 of J is dF_T/dx_j by the same forward

@@ -18,7 +18,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -79,6 +79,8 @@ def lib():
         L.psr_last_error.restype = C.c_char_p
         L.psr_mech_info.argtypes = [vp, C.POINTER(PsrMechInfo)]
         L.psr_mech_info.restype = C.c_int
+        L.psr_mech_reserve.argtypes = [vp, i64]
+        L.psr_mech_reserve.restype = C.c_int
         L.psr_mech_set_option.argtypes = [vp, C.c_int32, C.c_int32]
         L.psr_mech_set_option.restype = C.c_int
         L.psr_probe_fp64.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -178,6 +180,10 @@ class Mechanism:
         inf = PsrMechInfo()
         _check(lib().psr_mech_info(self._h, C.byref(inf)))
         return {n: getattr(inf, n) for n, _ in PsrMechInfo._fields_}
+
+    def reserve(self, N: int):
+        """psr_mech_reserve: size the Jacobian sweep's scratch for batches of up to N reactors (before a capture)."""
+        _check(lib().psr_mech_reserve(self._h, int(N)))
 
     def set_option(self, option: int, value: int):
         """psr_mech_set_option: diagnostic switches (OPT_JAC_UNHOISTED, OPT_FUSED_ONLY)."""

@@ -18,7 +18,7 @@
 
 namespace psr {
 cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st);
-cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm);
+cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, size_t smem_optin, int* ctas_per_sm);
 cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st);
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
                             cudaStream_t st, const double* F, const double* dt);
@@ -50,6 +50,7 @@ struct psr_mech {
   int opt_jac_unhoisted = 0;    // diagnostic: every Jacobian column a full evaluation
   double* d_scratch = nullptr;  // psr_fd_jacobian: rate table [N][I][kRateVals], then F0 when the caller passes none
   size_t scratch_bytes = 0;
+  std::vector<void*> retired;   // outgrown scratch buffers, freed with the mechanism
   int device = 0;
 };
 
@@ -95,6 +96,7 @@ struct HostRx {
   std::vector<std::pair<int, int>> nu_net;  // (species, nu''-nu')
   int type;
   int nr = 0, np = 0;
+  bool special_sign = false;   // A <= 0 or A0 <= 0: stored in the long form (kMetaSgnShift)
 };
 
 struct BlobSet {
@@ -122,7 +124,7 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
   std::vector<std::vector<int>> chunk_rx(n_chunks);
   for (int p = 0; p < I; ++p) chunk_rx[p % n_chunks].push_back(order[p]);
   // inside a chunk: longest-processing-time assignment of records to warps, records of a warp contiguous
-  auto cls_of = [&](int k) { return (rx[k].nr > kSlots || rx[k].np > kSlots) ? kClsLong : rx[k].type; };
+  auto cls_of = [&](int k) { return (rx[k].nr > kSlots || rx[k].np > kSlots || rx[k].special_sign) ? kClsLong : rx[k].type; };
   std::vector<std::vector<int>> chunk_wb(n_chunks);   // [warp][class boundary], kClsLong + 2 per warp
   for (int c = 0; c < n_chunks; ++c) {
     auto& cr = chunk_rx[c];  // cost-descending
@@ -167,7 +169,7 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
     for (int kl = 0; kl < n_rx; ++kl) {
       const HostRx& h = rx[cr[kl]];
       RxRec rec = h.rec;
-      if (h.nr <= kSlots && h.np <= kSlots) {
+      if (h.nr <= kSlots && h.np <= kSlots && !h.special_sign) {
         for (int i = 0; i < kSlots; ++i) {
           rec.off[i] = i < h.nr ? (uint32_t)h.factors[i] * row_bytes : unit_off;
           rec.off[kSlots + i] = i < h.np ? (uint32_t)h.factors[h.nr + i] * row_bytes : unit_off;
@@ -331,8 +333,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     if (d->reac_ptr[k + 1] < d->reac_ptr[k] || d->prod_ptr[k + 1] < d->prod_ptr[k] || d->eff_ptr[k + 1] < d->eff_ptr[k])
       return fail(PSR_EINVAL, "CSR pointers not monotone at reaction %d", k);
     if (d->rtype[k] > 3) return fail(PSR_EINVAL, "reaction %d: unknown rtype %d", k, (int)d->rtype[k]);
-    if (!(d->A[k] > 0.0) || !std::isfinite(d->A[k]) || !std::isfinite(d->b[k]) || !std::isfinite(d->Ea[k]))
-      return fail(PSR_EINVAL, "reaction %d: A must be > 0 and A, b, Ea finite", k);
+    if (!std::isfinite(d->A[k]) || !std::isfinite(d->b[k]) || !std::isfinite(d->Ea[k]))
+      return fail(PSR_EINVAL, "reaction %d: A, b, Ea must be finite", k);
     if (d->rtype[k] >= 2) any_fall = true;
   }
   if (any_fall && (!d->A0 || !d->b0 || !d->Ea0)) return fail(PSR_EINVAL, "falloff reactions need A0, b0, Ea0");
@@ -373,7 +375,11 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     st = side(d->prod_ptr, d->prod_sp, d->prod_nu, +1, "product");
     if (st != PSR_OK) return st;
     const int np = (int)h.factors.size() - nr;
-    const long double lnA = logl((long double)d->A[k]);
+    // ln|A| and the sign (kMetaSgnShift): A < 0 (a duplicate reaction with a negative pre-exponential) and A = 0 are
+    // ordinary input; such records take the long form, whose code applies the sign
+    auto sgn_code = [](double x) -> uint32_t { return x > 0.0 ? 0u : x < 0.0 ? 1u : 2u; };
+    uint32_t sg = sgn_code(d->A[k]);
+    const long double lnA = d->A[k] != 0.0 ? logl(fabsl((long double)d->A[k])) : 0.0L;
     const long double mEaR = -(long double)d->Ea[k] / kRcalL;
     h.rec.c[0] = (double)lnA;
     h.rec.c[1] = d->b[k];
@@ -403,17 +409,25 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
       if (h.has_aux) h.eff.push_back(e);  // efficiencies on a plain reaction have no effect
     }
     if (h.type >= 2) {
-      if (!(d->A0[k] > 0.0) || !std::isfinite(d->A0[k]) || !std::isfinite(d->b0[k]) || !std::isfinite(d->Ea0[k]))
-        return fail(PSR_EINVAL, "reaction %d: A0 must be > 0 and A0, b0, Ea0 finite", k);
-      h.aux.c0[0] = (double)logl((long double)d->A0[k]);
+      if (!std::isfinite(d->A0[k]) || !std::isfinite(d->b0[k]) || !std::isfinite(d->Ea0[k]))
+        return fail(PSR_EINVAL, "reaction %d: A0, b0, Ea0 must be finite", k);
+      sg |= sgn_code(d->A0[k]) << 2;
+      h.aux.c0[0] = d->A0[k] != 0.0 ? (double)logl(fabsl((long double)d->A0[k])) : 0.0;
       h.aux.c0[1] = d->b0[k];
       h.aux.c0[2] = (double)(-(long double)d->Ea0[k] / kRcalL);
       ++n_fall;
     }
+    h.special_sign = sg != 0;
+    h.rec.meta |= sg << kMetaSgnShift;
     if (h.type == PSR_RX_TROE) {
       if (h.eff.empty()) need_lnctot = 1;
       if (!d->troe) return fail(PSR_EINVAL, "Troe reactions need the troe array");
       const double* t = d->troe + 4 * k;
+      // alpha, T***, T* finite and the temperatures non-zero (they divide T); T** finite or +inf (+inf is how the
+      // three-parameter form, without the exp(-T**/T) term, is written)
+      if (!std::isfinite(t[0]) || !std::isfinite(t[1]) || !std::isfinite(t[2]) || t[1] == 0.0 || t[2] == 0.0 ||
+          std::isnan(t[3]) || t[3] == -INFINITY)
+        return fail(PSR_EINVAL, "reaction %d: Troe parameters must be finite with T***, T* != 0 (T** may be +inf)", k);
       h.aux.troe[0] = t[0];
       h.aux.troe[1] = -1.0 / t[1];
       h.aux.troe[2] = -1.0 / t[2];
@@ -622,7 +636,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
   v.invW = m->d_invW;
   v.Wm = m->d_W;
   v.nasa = m->d_nasa;
-  if ((e = occupancy_eval(nw, spw, rl, v.smem_total, &m->ctas_per_sm)) != cudaSuccess || m->ctas_per_sm < 1) {
+  if ((e = occupancy_eval(nw, spw, rl, v.smem_total, (size_t)prop.sharedMemPerBlockOptin, &m->ctas_per_sm)) != cudaSuccess || m->ctas_per_sm < 1) {
     cleanup();
     return fail(PSR_ECUDA, "kernel does not fit on this device (%s)", cudaGetErrorString(e));
   }
@@ -631,7 +645,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         (e = cudaMemcpy(m->d_ws_chunks, wbs.all.data(), wbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMalloc(&m->d_ws_sp_of, 4 * ws_sp_of.size())) != cudaSuccess ||
         (e = cudaMemcpy(m->d_ws_sp_of, ws_sp_of.data(), 4 * ws_sp_of.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
-        (e = ws_set_smem(wv.smem_total)) != cudaSuccess) {
+        (e = ws_set_smem((size_t)prop.sharedMemPerBlockOptin)) != cudaSuccess) {
       cleanup();
       return cuda_fail(e, "warp-specialised kernel tables");
     }
@@ -657,6 +671,7 @@ void psr_mech_free(psr_mech* m) {
   cudaFree(m->d_sp_of);
   cudaFree(m->d_rec_base);
   cudaFree(m->d_scratch);
+  for (void* q : m->retired) cudaFree(q);
   cudaFree(m->d_ws_chunks);
   cudaFree(m->d_ws_sp_of);
   delete m;
@@ -775,6 +790,21 @@ psr_status psr_eval_residual_energy(const psr_mech* m, int64_t N, const double* 
 
 namespace {
 
+// Scratch of the Jacobian sweep for N reactors: the rate table of one sub-batch, plus the base residual when the
+// caller passes no F0.  The sweep runs in sub-batches of *Nb reactors so that the rate table (I * kRateVals
+// doubles per reactor) written by the base launch is still in L2 when the Y-column launch reads it.
+size_t jac_scratch_bytes(const psr_mech* m, int64_t N, bool with_F0, int64_t* Nb_out) {
+  const int64_t n = m->view.K + 1;
+  const size_t row_bytes = (size_t)m->view.I * kRateVals * 8;
+  const int64_t wave = (int64_t)m->n_sm * m->ctas_per_sm * m->tile;   // reactors per full wave of base tiles
+  int64_t Nb = std::max<int64_t>(1, (int64_t)((size_t)64 * 1024 * 1024 / row_bytes));
+  if (Nb > wave) Nb -= Nb % wave;
+  Nb = std::min(Nb, std::max<int64_t>(N, 1));
+  Nb = std::min<int64_t>(Nb, ((int64_t)1 << 31) / (n + 32) - 1);   // state indices of a launch fit 32 bits
+  if (Nb_out) *Nb_out = Nb;
+  return align_up((size_t)Nb * row_bytes, 256) + (with_F0 ? (size_t)N * n * 8 : 0);
+}
+
 // psr_fd_jacobian (Tin == nullptr: row 0 is T - T_set) and psr_fd_jacobian_energy (row 0 is the energy row)
 psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, const double* P, const double* Y,
                             const double* Tin, const double* Yin, const double* tau, int64_t ld, double* J, double* F0,
@@ -787,25 +817,24 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
   psr_mech* m = const_cast<psr_mech*>(mc);
   const int64_t K = m->view.K, n = K + 1, I = m->view.I;
 
-  // The sweep runs in sub-batches of Nb reactors so that the rate table (I * kRateVals doubles per reactor)
-  // written by the base launch is still in L2 when the Y-column launch reads it.
   const size_t row_bytes = (size_t)I * kRateVals * 8;
-  const int64_t wave = (int64_t)m->n_sm * m->ctas_per_sm * m->tile;   // reactors per full wave of base tiles
-  int64_t Nb = std::max<int64_t>(1, (int64_t)((size_t)64 * 1024 * 1024 / row_bytes));
-  if (Nb > wave) Nb -= Nb % wave;
-  Nb = std::min(Nb, N);
-  Nb = std::min<int64_t>(Nb, ((int64_t)1 << 31) / (n + 32) - 1);   // state indices of a launch fit 32 bits
+  int64_t Nb = 0;
+  const size_t need = jac_scratch_bytes(m, N, F0 == nullptr, &Nb);
   const bool unhoisted = m->opt_jac_unhoisted != 0;   // diagnostic: every column a full evaluation (tests compare the two sweeps)
 
   const size_t tab_bytes = align_up((size_t)Nb * row_bytes, 256);
-  const size_t need = tab_bytes + (F0 ? 0 : (size_t)N * n * 8);
   if (need > m->scratch_bytes) {
-    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
-    if (e != cudaSuccess) return cuda_fail(e, "psr_fd_jacobian: sync before scratch growth");
-    cudaFree(m->d_scratch);
-    m->d_scratch = nullptr;
-    m->scratch_bytes = 0;
-    if ((e = cudaMalloc(&m->d_scratch, need)) != cudaSuccess) return fail(PSR_ENOMEM, "psr_fd_jacobian: scratch: %s", cudaGetErrorString(e));
+    // grow the mechanism-owned scratch.  Never inside a stream capture (an allocation would invalidate it: reserve
+    // first with psr_mech_reserve), and the outgrown buffer is kept until psr_mech_free, because kernels already
+    // enqueued -- or a captured graph replayed later -- may still point at it.
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing((cudaStream_t)stream, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
+      return fail(PSR_EINVAL, "%s: scratch for %lld reactors not reserved before stream capture (psr_mech_reserve)", fn, (long long)N);
+    void* grown = nullptr;
+    cudaError_t e = cudaMalloc(&grown, need);
+    if (e != cudaSuccess) return fail(PSR_ENOMEM, "%s: scratch: %s", fn, cudaGetErrorString(e));
+    if (m->d_scratch) m->retired.push_back(m->d_scratch);
+    m->d_scratch = static_cast<double*>(grown);
     m->scratch_bytes = need;
   }
   double* tab = m->d_scratch;
@@ -853,6 +882,20 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
 
 extern "C" {
 
+psr_status psr_mech_reserve(psr_mech* m, int64_t N) {
+  g_err.clear();
+  if (!m || N < 0) return fail(PSR_EINVAL, "psr_mech_reserve: null mechanism or N < 0");
+  const size_t need = jac_scratch_bytes(m, N, true, nullptr);
+  if (need <= m->scratch_bytes) return PSR_OK;
+  void* grown = nullptr;
+  cudaError_t e = cudaMalloc(&grown, need);
+  if (e != cudaSuccess) return fail(PSR_ENOMEM, "psr_mech_reserve: %s", cudaGetErrorString(e));
+  if (m->d_scratch) m->retired.push_back(m->d_scratch);
+  m->d_scratch = static_cast<double*>(grown);
+  m->scratch_bytes = need;
+  return PSR_OK;
+}
+
 psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, const double* P, const double* Y,
                            const double* Yin, const double* tau, int64_t ld, double* J, double* F0, void* stream) {
   return fd_jacobian_impl(mech, N, T, P, Y, nullptr, Yin, tau, ld, J, F0, stream, "psr_fd_jacobian");
@@ -870,11 +913,24 @@ psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double*
 
 static psr_status solve_impl(const char* who, int64_t N, int32_t n, const double* A, double* b, int32_t* info,
                              const double* F, const double* dt, void* stream) {
-  int dev = 0, n_sm = 0, optin = 0;
+  // SM count and shared-memory limit of the current device, looked up once per device
+  static int s_sm[64], s_optin[64];
+  int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (e != cudaSuccess) return cuda_fail(e, who);
+  int n_sm = 0, optin = 0;
+  if (dev >= 0 && dev < 64 && s_sm[dev] > 0) {
+    n_sm = s_sm[dev];
+    optin = s_optin[dev];
+  } else {
+    e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return cuda_fail(e, who);
+    if (dev >= 0 && dev < 64) {
+      s_optin[dev] = optin;
+      s_sm[dev] = n_sm;
+    }
+  }
   if (n > 168) return fail(PSR_EUNSUPPORTED, "%s: n = %d, the one-warp-per-system kernel takes n <= 168", who, n);
   e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream, F, dt);
   if (e != cudaSuccess) return cuda_fail(e, who);

@@ -620,6 +620,17 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
             }
           }
 
+          // sign of A and of A0/A (psr.h accepts any finite A: negative pre-exponentials of duplicate reactions, A = 0):
+          // only long-form records carry them (psr_tables.h), so this folds away in the other class loops
+          double sA = 1.0, sPr = 1.0;
+          if constexpr (CLS == kClsLong) {
+            const uint32_t sg = (meta >> kMetaSgnShift) & 0xFu;
+            if (sg) {
+              const double s0 = (sg >> 2) == 0 ? 1.0 : (sg >> 2) == 1 ? -1.0 : 0.0;
+              sA = (sg & 3u) == 0 ? 1.0 : (sg & 3u) == 1 ? -1.0 : 0.0;
+              sPr = sA == 0.0 ? __longlong_as_double(0x7ff8000000000000LL) : s0 * sA;   // k0 [M] / 0 is not a number
+            }
+          }
           if (type <= PSR_T_THREE_BODY) {
             if constexpr (JY) {
 #pragma unroll
@@ -650,6 +661,15 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                     row[1] = kr[i];
                   }
                 }
+              }
+            }
+          }
+          if constexpr (CLS == kClsLong) {
+            if (type <= PSR_T_THREE_BODY) {
+#pragma unroll
+              for (int i = 0; i < R; ++i) {
+                kf[i] *= sA;
+                kr[i] *= sA;
               }
             }
           }
@@ -707,8 +727,10 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               }
 #pragma unroll
               for (int i = 0; i < R; ++i) {
-                const double Pr = ey[3 * i] * M[i];
+                double Pr = ey[3 * i] * M[i];
+                if constexpr (CLS == kClsLong) Pr *= sPr;
                 kf[i] = ey[3 * i + 1] * (Pr / (1.0 + Pr));
+                if constexpr (CLS == kClsLong) kf[i] *= sA;
                 kr[i] = kf[i] * ey[3 * i + 2];
               }
             } else {
@@ -766,7 +788,8 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                 const double nn = fma(-1.27, lF, 0.75);
                 const double lp = fma(lnPr, kLog10e, cc);
                 const double den = fma(-0.14, lp, nn);
-                // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 gives F = 1 (g17)
+                // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); den = 0 with lp != 0 gives F = 1 (g17);
+                // den = lp = 0 (0/0) and Pr = inf (inf/inf) are not numbers here as in the definition
                 // both quotients (this one and k_f = .../(1+Pr)) share one reciprocal
                 const double den2 = den * den;
                 const double bq = fma(lp, lp, den2), dq = 1.0 + Pr;
@@ -775,6 +798,9 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
                 e2[0] = fma(lnFc * den2, dq * inv, lnk0M);
                 exps(e2, k2);
                 kf[i] = k2[0] * (bq * inv);
+                // the log form above needs Pr > 0; otherwise log10(Pr) of the definition is not a number (or -inf,
+                // which makes F not a number): same result here
+                if constexpr (CLS == kClsLong) kf[i] = sPr > 0.0 ? kf[i] * sA : __longlong_as_double(0x7ff8000000000000LL);
                 kr[i] = kf[i] * invKc;
               }
             }
@@ -921,6 +947,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
             }
           }
         }
+        __syncthreads();   // warp 0 has read the steps hs[] before the next tile's prologue writes them
       }
     } else if (!jac) {
 #pragma unroll
@@ -1041,9 +1068,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 
 template <int NW, int SPW, int R, int VAR>
 static cudaError_t launch_t(const MechView& mv, const EvalArgs& a, int grid, cudaStream_t st) {
-  auto kern = psr_eval_kernel<NW, SPW, R, VAR>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mv.smem_total);
-  if (e != cudaSuccess) return e;
+  auto kern = psr_eval_kernel<NW, SPW, R, VAR>;   // its dynamic shared-memory limit was raised once, at load (occupancy_eval)
   const uint32_t smem = mv.smem_total;
   kern<<<grid, NW * 32, smem, st>>>(mv, a);
   return cudaGetLastError();
@@ -1064,14 +1089,16 @@ cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalA
 }
 
 template <int NW, int SPW, int R>
-static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
+static cudaError_t occ_t(size_t smem, size_t smem_optin, int* ctas_per_sm) {
   // every variant is launched with the same grid: size it for the one with the lowest occupancy
   const void* kerns[4] = {(const void*)psr_eval_kernel<NW, SPW, R, 0>, (const void*)psr_eval_kernel<NW, SPW, R, 1>,
                           (const void*)psr_eval_kernel<NW, SPW, R, 2>, (const void*)psr_eval_kernel<NW, SPW, R, 3>};
   int least = 1 << 30;
   for (const void* k : kerns) {
     int nb = 0;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // raised to the device's limit once per kernel instance: mechanisms of different sizes share the instance,
+    // so the attribute must not follow the mechanism loaded last
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_optin);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, NW * 32, smem);
     if (e != cudaSuccess) return e;
     least = nb < least ? nb : least;
@@ -1080,9 +1107,9 @@ static cudaError_t occ_t(size_t smem, int* ctas_per_sm) {
   return cudaSuccess;
 }
 
-cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, int* ctas_per_sm) {
+cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, size_t smem_optin, int* ctas_per_sm) {
 #define PSR_O(NW_, SPW_) \
-  if (nw == NW_ && spw == SPW_ && rl == 1) return occ_t<NW_, SPW_, 1>(smem, ctas_per_sm);
+  if (nw == NW_ && spw == SPW_ && rl == 1) return occ_t<NW_, SPW_, 1>(smem, smem_optin, ctas_per_sm);
   PSR_SHAPES(PSR_O)
 #undef PSR_O
   return cudaErrorInvalidConfiguration;

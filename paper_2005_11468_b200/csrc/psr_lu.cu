@@ -253,8 +253,12 @@ cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_
 #define PSR_LU(RPL_)                                                                                         \
   if (rpl <= RPL_) {                                                                                         \
     auto kern = dt ? lu_solve_kernel<RPL_, true> : lu_solve_kernel<RPL_, false>;                             \
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);      \
-    if (e != cudaSuccess) return e;                                                                          \
+    static bool raised[2] = {false, false};   /* dynamic shared-memory limit: once per kernel instance */    \
+    if (!raised[dt ? 1 : 0]) {                                                                               \
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_optin); \
+      if (e != cudaSuccess) return e;                                                                        \
+      raised[dt ? 1 : 0] = true;                                                                             \
+    }                                                                                                        \
     kern<<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles, F, dt);                           \
     return cudaGetLastError();                                                                               \
   }

@@ -31,6 +31,10 @@ constexpr uint32_t kMetaRev = 0x4u;           // reversible
 constexpr uint32_t kMetaLong = 0x8u;          // factor list lives in the u16 pool at off[0]; counts in meta
 constexpr int kMetaNrShift = 4;               // bits 4..7  reactant factor count (long form)
 constexpr int kMetaNpShift = 8;               // bits 8..11 product factor count (long form)
+constexpr int kMetaSgnShift = 12;              // bits 12..13 sign of A, bits 14..15 sign of A0: 0 positive, 1 negative, 2 zero
+                                              // (non-zero only in long-form records: a reaction with A <= 0 or A0 <= 0
+                                              // is stored in the long form, so the class loops of ordinary reactions
+                                              // carry no sign handling; c[0], c0[0] then hold ln|A|, or 0 for A = 0)
 constexpr int kMetaAuxShift = 16;             // bits 16..31 index into AuxRec[]
 
 struct __attribute__((aligned(16))) RxRec {   // 112 bytes

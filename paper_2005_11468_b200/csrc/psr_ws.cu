@@ -128,6 +128,17 @@ __device__ __forceinline__ void ws_run_class(RxCtx& cx, const unsigned char* blo
       if (!(meta & kMetaRev)) pr = 0.0;
     }
 
+    // sign of A and of A0/A (any finite A is accepted: negative pre-exponentials of duplicate reactions, A = 0): only
+    // long-form records carry them (psr_tables.h), so this folds away in the other class loops
+    double sA = 1.0, sPr = 1.0;
+    if constexpr (CLS == kClsLong) {
+      const uint32_t sg = (meta >> kMetaSgnShift) & 0xFu;
+      if (sg) {
+        const double s0 = (sg >> 2) == 0 ? 1.0 : (sg >> 2) == 1 ? -1.0 : 0.0;
+        sA = (sg & 3u) == 0 ? 1.0 : (sg & 3u) == 1 ? -1.0 : 0.0;
+        sPr = sA == 0.0 ? __longlong_as_double(0x7ff8000000000000LL) : s0 * sA;   // k0 [M] / 0 is not a number
+      }
+    }
     if (type <= T_THREE_BODY) {
       double ex[2], ey[2];
       ex[0] = lnkf;
@@ -135,6 +146,10 @@ __device__ __forceinline__ void ws_run_class(RxCtx& cx, const unsigned char* blo
       exps(ex, ey);
       kf = ey[0];
       kr = ey[1];
+      if constexpr (CLS == kClsLong) {
+        kf *= sA;
+        kr *= sA;
+      }
     }
     if (type != T_PLAIN) {
       const AuxRec* ax = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux) + (meta >> kMetaAuxShift);
@@ -154,8 +169,10 @@ __device__ __forceinline__ void ws_run_class(RxCtx& cx, const unsigned char* blo
         ex[1] = lnkf;
         ex[2] = lnkr - lnkf;
         exps(ex, ey);
-        const double Pr = ey[0] * M;
+        double Pr = ey[0] * M;
+        if constexpr (CLS == kClsLong) Pr *= sPr;
         kf = ey[1] * (Pr / (1.0 + Pr));
+        if constexpr (CLS == kClsLong) kf *= sA;
         kr = kf * ey[2];
       } else {
         // Troe.  With ln Pr = ln k0 - ln k_inf + ln[M]:  k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
@@ -188,6 +205,8 @@ __device__ __forceinline__ void ws_run_class(RxCtx& cx, const unsigned char* blo
         e2[0] = fma(lnFc * den2, dq * inv, lnk0M);
         exps(e2, k2);
         kf = k2[0] * (bq * inv);
+        // the log form above needs Pr > 0; otherwise log10(Pr) of the definition is not a number
+        if constexpr (CLS == kClsLong) kf = sPr > 0.0 ? kf * sA : __longlong_as_double(0x7ff8000000000000LL);
         kr = kf * invKc;
       }
     }
@@ -519,6 +538,8 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
   }
 }
 
+// once per process: the kernels' dynamic shared-memory limit raised to the device's (mechanisms of different sizes
+// share the kernel instances)
 cudaError_t ws_set_smem(size_t smem) {
   cudaError_t e = cudaFuncSetAttribute(psr_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -50,11 +50,34 @@ def test_mech_load_rejects_malformed_descriptions_before_touching_the_device():
     assert status(bad)[0] == binding.PSR_EINVAL
     bad = dict(a); bad["rtype"] = a["rtype"].copy(); bad["rtype"][0] = 7
     assert status(bad)[0] == binding.PSR_EINVAL
-    bad = dict(a); bad["A"] = a["A"].copy(); bad["A"][0] = -1.0
+    bad = dict(a); bad["A"] = a["A"].copy(); bad["A"][0] = float("nan")
+    st, msg = status(bad); assert st == binding.PSR_EINVAL and "finite" in msg
+    bad = dict(a); bad["A"] = a["A"].copy(); bad["A"][0] = float("inf")
     assert status(bad)[0] == binding.PSR_EINVAL
+    # any finite A is a valid mechanism: negative and zero pre-exponentials pass validation
+    # (without a device the load then stops at PSR_ECUDA, with one it succeeds)
+    for v in (-1.0, 0.0):
+        ok = dict(a); ok["A"] = a["A"].copy(); ok["A"][0] = v
+        assert status(ok)[0] in (binding.PSR_OK, binding.PSR_ECUDA)
     bad = dict(a); bad["nasa"] = None
     assert status(bad)[0] == binding.PSR_EINVAL
     assert status(a, K=0)[0] == binding.PSR_EINVAL
+    # Troe parameters: finite, T*** and T* non-zero, T** finite or +inf
+    m1, _ = synth.make_config("C1", 1)
+    a1 = m1.arrays()
+    k = int(np.flatnonzero(np.asarray(a1["rtype"]) == 3)[0])
+    def status1(arrs):
+        desc, keep = binding.make_desc(m1.n_species, m1.n_reactions, arrs)
+        h = C.c_void_p()
+        st = lib.psr_mech_load(C.byref(desc), C.byref(h))
+        if st == 0:
+            lib.psr_mech_free(h)
+        return st
+    for col, v, want in ((1, 0.0, False), (2, float("nan"), False), (0, float("inf"), False), (3, float("-inf"), False),
+                         (3, float("inf"), True)):
+        t = dict(a1); t["troe"] = np.array(a1["troe"], dtype=np.float64).copy(); t["troe"][k, col] = v
+        st = status1(t)
+        assert (st in (binding.PSR_OK, binding.PSR_ECUDA)) if want else st == binding.PSR_EINVAL, (col, v, st)
     assert status(a, K=513)[0] in (binding.PSR_EINVAL, binding.PSR_EUNSUPPORTED)
 
 

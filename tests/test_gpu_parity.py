@@ -228,6 +228,48 @@ def test_long_factor_lists_and_nu3(torch_cuda, binding):
     check_against_oracle(m, batch, got)
 
 
+def test_negative_and_zero_pre_exponentials(torch_cuda, binding):
+    """Any finite A is valid input: a duplicate pair with a negative pre-exponential, A = 0 (a
+    zero-rate reaction), on plain, three-body and Lindemann reactions, and a negative A and A0 together on Troe
+    reactions (P_r stays positive).  Where the definition gives no number -- A0 <= 0 or A = 0 on a Troe reaction:
+    log10 P_r of a non-positive P_r -- both sides must give NaN."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C1", 150)
+    m = copy.deepcopy(mech)
+    rt = np.asarray(m.rtype)
+    plain, tb, troe = np.flatnonzero(rt == 0), np.flatnonzero(rt == 1), np.flatnonzero(rt == 3)
+    m.A = m.A.copy(); m.A0 = m.A0.copy(); m.rtype = m.rtype.copy()
+    m.A[plain[0]] *= -1.0          # negative pre-exponential (CHEMKIN duplicate)
+    m.A[plain[1]] = 0.0            # zero-rate reaction
+    m.A[tb[0]] *= -0.5
+    m.A[tb[1]] = 0.0
+    m.rtype[troe[0]] = 2           # Lindemann: k_inf < 0, k_0 > 0 (P_r < 0 is a number there)
+    m.A[troe[0]] *= -1.0
+    m.rtype[troe[1]] = 2           # Lindemann with A0 = 0: k_f = 0
+    m.A0[troe[1]] = 0.0
+    m.A[troe[2]] *= -1.0           # Troe, both negative: P_r > 0, k_f < 0
+    m.A0[troe[2]] *= -1.0
+    got = gpu_eval(torch, binding, m, batch)
+    ref = check_against_oracle(m, batch, got)
+    assert np.all(got["kf"][plain[0]] < 0) and np.all(got["kf"][plain[1]] == 0) and np.all(got["q"][plain[1]] == 0)
+    assert np.all(got["kf"][troe[2]] < 0) and np.all(got["kf"][troe[1]] == 0)
+    assert np.array_equal(np.sign(got["kr"]), np.sign(ref["kr"]))
+    # no number by the definition: NaN on both sides, and only there
+    m2 = copy.deepcopy(mech)
+    m2.A = m2.A.copy(); m2.A0 = m2.A0.copy()
+    m2.A0[troe[0]] = 0.0
+    m2.A0[troe[1]] *= -1.0
+    m2.A[troe[2]] = 0.0
+    sub = batch.take(np.arange(40))
+    got2 = gpu_eval(torch, binding, m2, sub, want_F=False)
+    ref2 = orc.evaluate(oracle_mech(m2), sub.T, sub.P, sub.Y, want=("kf", "kr", "q", "wdot"))
+    for name in ("kf", "q", "wdot"):
+        assert np.array_equal(np.isnan(got2[name]), np.isnan(ref2[name])), name
+    assert np.isnan(ref2["kf"][troe[:3]]).all() and not np.isnan(ref2["kf"][plain]).any()
+    ok = ~np.isnan(ref2["kf"])
+    assert rel_err(got2["kf"][ok], ref2["kf"][ok]).max() <= TOL_K
+
+
 def test_negative_and_zero_mass_fractions_propagate(torch_cuda, binding):
     """Newton iterates may leave [0,1]; products by multiplication keep the sign."""
     mech, batch = synth.make_config("C1", 64)
@@ -688,14 +730,28 @@ def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, 
     n = mech.n_species + 1
     F, w = torch.empty_like(Y), torch.empty_like(Y)
     J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
-    gm.fd_jacobian(T, P, Y, Yin, tau, J=J)            # sizes the scratch buffer outside the capture
-    torch.cuda.synchronize()
     side = torch.cuda.Stream()
+    # the Jacobian sweep's scratch belongs to the mechanism: without a reservation the call refuses to allocate
+    # inside a capture (psr.h) instead of invalidating it
+    probe = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(probe, stream=side):
+            with pytest.raises(binding.PsrError) as ei:
+                gm.fd_jacobian(T, P, Y, Yin, tau, J=J)
+            assert ei.value.status == binding.PSR_EINVAL and "psr_mech_reserve" in str(ei.value)
+    del probe
+    gm.reserve(batch.n)                                # sizes the scratch buffer outside the capture
+    torch.cuda.synchronize()
     graph = torch.cuda.CUDAGraph()
     with torch.cuda.stream(side):
         with torch.cuda.graph(graph, stream=side):
             gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w)
             gm.fd_jacobian(T, P, Y, Yin, tau, J=J)
+    # a later, larger eager call outgrows the scratch: the captured graph keeps pointing at the buffer it was
+    # captured with, which stays allocated until the mechanism is freed
+    _, big = synth.make_config("C4", 6000)
+    gm.fd_jacobian(*(dev(torch, x) for x in (big.T, big.P, big.Y, big.Yin, big.tau)))
+    torch.cuda.synchronize()
     # new state in the same buffers, replay, compare with direct calls on the default stream
     _, b2 = synth.make_config("C4", 200)
     for dst, src in ((T, b2.T), (P, b2.P), (Y, b2.Y), (Yin, b2.Yin), (tau, b2.tau)):
