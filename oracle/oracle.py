@@ -216,3 +216,30 @@ def max_threads() -> int:
 
 def host_cores() -> int:
     return len(os.sched_getaffinity(0))
+
+
+class SolveOpts(C.Structure):
+    """Constants of the hybrid solver (the paper leaves them to its ref. [5]: the caller's)."""
+    _fields_ = [("atol", C.c_double), ("rtol", C.c_double), ("max_iter", C.c_int32), ("max_newton", C.c_int32),
+                ("max_ptc", C.c_int32), ("reserved", C.c_int32), ("dt0", C.c_double), ("dt_grow", C.c_double),
+                ("dt_shrink", C.c_double), ("y_floor", C.c_double)]
+
+
+def solve_hybrid(mech: OracleMechanism, T, P, Y, Yin, tau, *, Tin=None, atol=1e-12, rtol=1e-8, max_iter=50,
+                 max_newton=10, max_ptc=10, dt0=1e-6, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9, nthreads: int = 0) -> dict:
+    """NEXT-4: hybrid Newton / pseudo-transient solve of the PSR equations, one reactor at a time.
+    Returns T [N], Y [K][N] (the solution estimates), status [N] (0 converged, 1 budget exhausted), n_newton, n_ptc."""
+    T = np.array(T, dtype=np.float64)
+    Y = np.array(Y, dtype=np.float64, order="C")
+    P, Yin, tau = (np.ascontiguousarray(a, dtype=np.float64) for a in (P, Yin, tau))
+    N = T.shape[0]
+    assert Y.shape == (mech.K, N) and Yin.shape == (mech.K, N)
+    if Tin is not None:
+        Tin = np.ascontiguousarray(Tin, dtype=np.float64)
+    o = SolveOpts(atol, rtol, max_iter, max_newton, max_ptc, 0, dt0, dt_grow, dt_shrink, y_floor)
+    status, nn, npt = (np.zeros(N, dtype=np.int32) for _ in range(3))
+    rc = lib().oracle_solve_hybrid(C.byref(mech.c), C.c_int64(N), _p(T), _p(P), _p(Y), _p(Tin), _p(Yin), _p(tau),
+                                   C.c_int64(N), C.byref(o), _p(status), _p(nn), _p(npt), C.c_int(nthreads))
+    if rc != 0:
+        raise RuntimeError(f"oracle_solve_hybrid failed rc={rc}")
+    return dict(T=T, Y=Y, status=status, n_newton=nn, n_ptc=npt)

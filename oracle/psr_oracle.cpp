@@ -28,6 +28,12 @@
 //   exchange, a singular system, LAPACK (numpy.linalg.solve) on random systems, backward error bound.
 //   Pseudo-transient step (NEXT-4): exact rational solutions, the Newton limit dt -> inf, the explicit-Euler
 //   limit dt -> 0 (dx -> -dt F), the scalar closed form dx = -F/(1/dt + J), LAPACK on the shifted matrix.
+//   Hybrid solver (NEXT-4): an inert mechanism reaches Y = Y_in in one Newton step (to the forward-difference
+//   accuracy) and stops after the confirming one; the closed-form steady state of A <=> B (a linear residual);
+//   the root of 2A <=> B found with mpmath from the dense restatement, reached by Newton alone from a near guess
+//   and through pseudo-transient stages from a guess whose Newton trial is inadmissible; exhausted budgets;
+//   pseudo-transient steps with dt = 1e300 retrace the Newton iterates; the adiabatic inert reactor settles at
+//   (T_in, Y_in).
 //
 // Units (paper silent; CHEMKIN cgs, reading g4): T [K], P [dyn/cm^2], C [mol/cm^3],
 // rho [g/cm^3], W [g/mol], wdot [mol/cm^3/s], Ea [cal/mol].
@@ -553,5 +559,128 @@ int oracle_max_threads(void) {
 #else
   return 1;
 #endif
+}
+}
+
+// NEXT-4, second half: the hybrid Newton / pseudo-transient solver of PAPER.md:44 --
+//   "one of the first steps involves constructing an error vector by substituting the initial guesses into the
+//    nonlinear-algebraic equations.  The next step is to construct a Jacobian matrix.  The Jacobian matrix is
+//    decomposed into lower and upper triangular matrices, and then a back-solving operation is carried out ...
+//    The hybrid approach consists of two steps: a steady state Newton iteration and a pseudo-transient time
+//    integration.  If convergence is not achieved using the Newton iteration, the solution estimate is conditioned
+//    using the time integration.  The process of switching between the Newton iteration and time integration
+//    approaches continues until convergence is achieved, which is based on very specific criteria related to
+//    absolute and relative tolerances."
+// The paper leaves every constant and the step-size rule to its ref. [5]; they are the caller's (opts), and the
+// points the paper does not fix are read as follows (readings g21-g25):
+//   g21  unknowns x = (T, Y_1..Y_K); residual F of O10 (row 0 = T - T_set), or with Tin the adiabatic system
+//        whose row 0 is the energy row; Jacobian by O11 (forward differences) at every iteration.
+//   g22  Newton iteration: solve J dx = -F, trial x' = x + dx (full step).  Converged when
+//        max_i |dx_i| / (atol + rtol |x_i|) <= 1 with x the estimate the correction was computed at; the
+//        correction is applied before stopping.  A trial is admissible when dx is finite (the system solved
+//        without a zero pivot) and every mass fraction of x' is >= -y_floor (the solver this one descends from,
+//        PAPER.md:158 ref. [3], bounds its unknowns the same way; y_floor = +inf switches the bound off).
+//   g23  "convergence is not achieved": the trial of a Newton iteration is not admissible (x then stays), or
+//        max_newton admissible iterations of a Newton stage have passed without convergence.  The estimate is
+//        then conditioned by max_ptc pseudo-transient steps ((I/dt + J) dx = -F, oracle_ptc_step's system)
+//        before Newton resumes.
+//   g24  step size: dt starts at dt0 and persists across stages; an admissible step is taken and
+//        dt <- dt * dt_grow, otherwise x stays and dt <- dt * dt_shrink (either way it counts as one step).
+//   g25  budget: every linear solve (Newton or pseudo-transient) counts; after max_iter of them a reactor that has
+//        not converged is reported as such (status 1).  status 0 = converged.
+// One reactor at a time, every step a call of the plain routines above (jac_batch on one reactor, lu_solve_one).
+extern "C" {
+struct oracle_solve_opts {
+  double atol, rtol;
+  int32_t max_iter, max_newton, max_ptc, reserved;
+  double dt0, dt_grow, dt_shrink, y_floor;
+};
+
+int oracle_solve_hybrid(const oracle_mech* m, int64_t N, double* T, const double* P, double* Y, const double* Tin,
+                        const double* Yin, const double* tau, int64_t ld, const oracle_solve_opts* o, int32_t* status,
+                        int32_t* n_newton, int32_t* n_ptc, int nthreads) {
+  const int K = m->n_species, n = K + 1;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+#endif
+  {
+    std::vector<double> x(n), xt(n), y(K), yin(K), J((size_t)n * n), F(n), A((size_t)n * n), b(n), dx(n);
+#ifdef _OPENMP
+#pragma omp for schedule(dynamic, 1)
+#endif
+    for (int64_t r = 0; r < N; ++r) {
+      x[0] = T[r];
+      for (int i = 0; i < K; ++i) {
+        x[1 + i] = Y[(int64_t)i * ld + r];
+        yin[i] = Yin[(int64_t)i * ld + r];
+      }
+      const double Tset = T[r];   // the fixed-temperature equation holds T at its initial value
+      const double Pr = P[r], taur = tau[r], Tinr = Tin ? Tin[r] : 0.0;
+      bool newton = true, converged = false;
+      int it = 0, nn = 0, np = 0;
+      double dt = o->dt0;
+      for (int iter = 0; iter < o->max_iter && !converged; ++iter) {
+        // error vector and Jacobian at the current estimate (O10 / energy row, O11)
+        for (int i = 0; i < K; ++i) y[i] = x[1 + i];
+        const double Tr = x[0];
+        jac_batch<double>(*m, 1, &Tr, &Pr, y.data(), Tin ? &Tinr : nullptr, yin.data(), &taur, 1, J.data(), F.data(),
+                          nullptr, nullptr, 1);
+        if (!Tin) F[0] = x[0] - Tset;   // jac_batch measures row 0 from its own input T; the equation is T - T_set
+        // (I/dt + J) dx = -F; a Newton iteration is the same system without the shift
+        const double shift = newton ? 0.0 : 1.0 / dt;
+        for (int j = 0; j < n; ++j)
+          for (int i = 0; i < n; ++i) A[(size_t)j * n + i] = J[(size_t)j * n + i] + (i == j ? shift : 0.0);
+        for (int i = 0; i < n; ++i) b[i] = -F[i];
+        const int info = lu_solve_one<double>(n, A.data(), b.data(), dx.data());
+        bool ok = info == 0;
+        for (int i = 0; ok && i < n; ++i) ok = std::isfinite(dx[i]);
+        // the trial estimate; admissible when dx is finite and every mass fraction stays >= -y_floor
+        double err = 0.0;
+        bool admissible = ok;
+        if (ok) {
+          for (int i = 0; i < n; ++i) {
+            err = std::fmax(err, std::fabs(dx[i]) / (o->atol + o->rtol * std::fabs(x[i])));
+            xt[i] = x[i] + dx[i];
+          }
+          for (int i = 1; i < n; ++i) admissible = admissible && xt[i] >= -o->y_floor;
+        }
+        if (newton) {
+          ++nn;
+          if (admissible && err <= 1.0) {
+            x = xt;
+            converged = true;
+          } else if (admissible) {
+            x = xt;
+            if (++it >= o->max_newton) {   // the stage is over without convergence: condition the estimate
+              newton = false;
+              it = 0;
+            }
+          } else {
+            newton = false;
+            it = 0;
+          }
+        } else {
+          ++np;
+          if (admissible) {
+            x = xt;
+            dt *= o->dt_grow;
+          } else {
+            dt *= o->dt_shrink;
+          }
+          if (++it >= o->max_ptc) {   // back to the Newton iteration from the conditioned estimate
+            newton = true;
+            it = 0;
+          }
+        }
+      }
+      T[r] = x[0];
+      for (int i = 0; i < K; ++i) Y[(int64_t)i * ld + r] = x[1 + i];
+      status[r] = converged ? 0 : 1;
+      if (n_newton) n_newton[r] = nn;
+      if (n_ptc) n_ptc[r] = np;
+    }
+  }
+  return 0;
 }
 }

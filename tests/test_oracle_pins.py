@@ -645,3 +645,130 @@ def test_ptc_step_limits_newton_and_explicit_euler():
     assert np.all(info == 0) and np.abs(dx - ref).max() <= 1e-12 * np.abs(ref).max()
     _, info = orc.ptc_step(np.array([[[-2.0]]]), np.array([[1.0]]), np.array([0.5]))   # 1/dt + J = 0
     assert info[0] == 1
+
+
+# ------------------------------------------------------------------ hybrid Newton / pseudo-transient solver (NEXT-4)
+def _two_species(rx, W, A, b=0.0, Ea=5e3, a6B=3.0):
+    """One reversible reaction between two species (inputs only; a6 of the second species sets the equilibrium)."""
+    nasa = np.array([[3.5, 1e-4, 0.0, 0.0, 0.0, -1000.0, 2.0],
+                     [3.9, 3e-4, -2e-8, 0.0, 0.0, -1600.0, a6B]])
+    reac_ptr, reac_sp, reac_nu = synth._side_csr([rx[0]])
+    prod_ptr, prod_sp, prod_nu = synth._side_csr([rx[1]])
+    return synth.Mechanism(
+        n_species=2, n_reactions=1, atoms=np.zeros((2, 4), dtype=np.int32), W=np.array(W, dtype=np.float64), nasa=nasa,
+        A=np.array([A]), b=np.array([b]), Ea=np.array([Ea]), rtype=np.zeros(1, dtype=np.uint8),
+        reversible=np.ones(1, dtype=np.uint8), reac_ptr=reac_ptr, reac_sp=reac_sp, reac_nu=reac_nu,
+        prod_ptr=prod_ptr, prod_sp=prod_sp, prod_nu=prod_nu, eff_ptr=np.zeros(2, dtype=np.int32),
+        eff_sp=np.zeros(0, dtype=np.int32), eff_val=np.zeros(0), A0=np.zeros(1), b0=np.zeros(1), Ea0=np.zeros(1),
+        troe=np.zeros((1, 4)), meta={"name": "two-species"})
+
+
+def test_solver_inert_mechanism_reaches_the_inlet_composition_in_one_newton_step():
+    """Without chemistry F = (Y - Y_in)/tau is linear: one Newton step lands on Y = Y_in up to the accuracy of the
+    forward-difference Jacobian (eps |Y - Y_in| / h ~ 1e-8 relative), the next iteration's correction is that
+    small and passes a 1e-6 tolerance test (2 Newton iterations, no pseudo-transient step), and has refined the
+    estimate to round-off."""
+    mech, batch = synth.make_config("C0", 12)
+    mm = copy.deepcopy(mech)
+    mm.A = np.zeros_like(mech.A)
+    om = oracle_mech(mm)
+    one = orc.solve_hybrid(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, atol=1e-9, rtol=1e-6, max_iter=1)
+    assert np.all(one["status"] == 1) and np.all(one["n_newton"] == 1)
+    assert np.abs(one["Y"] - batch.Yin).max() <= 1e-6 * np.abs(batch.Y - batch.Yin).max()
+    r = orc.solve_hybrid(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, atol=1e-9, rtol=1e-6)
+    assert np.all(r["status"] == 0) and np.all(r["n_newton"] == 2) and np.all(r["n_ptc"] == 0)
+    assert np.allclose(r["Y"], batch.Yin, rtol=1e-12, atol=1e-15) and np.array_equal(r["T"], batch.T)
+
+
+def test_solver_isomerisation_closed_form_steady_state():
+    """A <=> B with equal molar masses: wdot_A W/rho = -(k_f Y_A - k_r Y_B) whatever rho is, so the steady
+    residual is LINEAR in Y and has the closed-form root
+        Y_A = (Y_A,in / tau + k_r S) / (1/tau + k_f + k_r),  S = Y_A,in + Y_B,in,
+    with k_f from Eq. 6 and k_r = k_f / K_c (Eq. 7-9, sum nu = 0) evaluated here with mpmath.  Newton on a linear
+    residual converges in one step (+ one to confirm, which also removes the forward-difference error)."""
+    from mpmath import exp as mexp, log as mlog, power as mpow
+    mech = _two_species(((0,), (1,)), W=[28.0, 28.0], A=3.0e3, b=0.3, Ea=4.0e3)
+    T, P, tau = 1400.0, 2.0 * PATM, 2e-3
+    Yin = np.array([[0.7], [0.3]])
+    Y0 = np.array([[0.2], [0.8]])
+    r = orc.solve_hybrid(oracle_mech(mech), np.array([T]), np.array([P]), Y0, Yin, np.array([tau]), atol=1e-9, rtol=1e-6)
+    Tm = mpf(T)
+    kf = mpf(float(mech.A[0])) * mpow(Tm, mpf(float(mech.b[0]))) * mexp(-mpf(float(mech.Ea[0])) / (mp_dense.RCAL * Tm))
+    def g(a):
+        a = [mpf(float(v)) for v in a]
+        hRT = a[0] + a[1] * Tm / 2 + a[2] * Tm**2 / 3 + a[3] * Tm**3 / 4 + a[4] * Tm**4 / 5 + a[5] / Tm
+        sR = a[0] * mlog(Tm) + a[1] * Tm + a[2] * Tm**2 / 2 + a[3] * Tm**3 / 3 + a[4] * Tm**4 / 4 + a[6]
+        return sR - hRT
+    Kc = mexp(g(mech.nasa[1]) - g(mech.nasa[0]))
+    kr = kf / Kc
+    yA = (mpf("0.7") / mpf(tau) + kr) / (1 / mpf(tau) + kf + kr)
+    assert r["status"][0] == 0 and r["n_newton"][0] == 2 and r["n_ptc"][0] == 0
+    assert close(r["Y"][0, 0], yA, 1e-10) and close(r["Y"][1, 0], 1 - yA, 1e-10)
+    assert 0.05 < float(yA) < 0.95 and abs(float(yA) - 0.7) > 0.05     # chemistry matters in this case
+
+
+def _dimerisation_root(mech, T, P, Yin, tau):
+    """Root of the steady residual of 2A <=> B (W_B = 2 W_A) with mpmath: Y_A + Y_B = 1 at steady state, so
+    F_A(y) = 0 in one unknown, the residual taken from the dense 50-digit restatement (mp_dense)."""
+    from mpmath import findroot
+    def FA(y):
+        return mp_dense.evaluate(mech, T, P, [y, 1 - y], Yin=Yin, tau=tau)["F"][1]
+    return findroot(FA, (mpf("1e-6"), mpf("0.999999")), solver="illinois", maxsteps=400, verify=False)
+
+
+def test_solver_nonlinear_root_and_the_switch_to_pseudo_transient():
+    """2A <=> B (second order): the converged estimate is the root computed independently with mpmath.  From a
+    good guess Newton alone converges; from a guess whose Newton trial leaves the admissible region
+    (Y < -y_floor) the estimate is first conditioned by pseudo-transient steps (whole stages of max_ptc steps),
+    then Newton converges to the same root; a budget too small is reported as not converged."""
+    mech = _two_species(((0, 0), (1,)), W=[15.0, 30.0], A=2.0e9, b=0.0, Ea=2.0e3, a6B=23.0)
+    T, P, tau = 1200.0, PATM, 1e-3
+    Yin = np.array([[0.9], [0.1]])
+    root = _dimerisation_root(mech, T, P, Yin[:, 0], tau)
+    om = oracle_mech(mech)
+    args = (np.array([T]), np.array([P]))
+    good = orc.solve_hybrid(om, *args, np.array([[float(root) * 1.05], [1 - float(root) * 1.05]]), Yin, np.array([tau]),
+                            atol=1e-14, rtol=1e-10, max_newton=20)
+    assert good["status"][0] == 0 and good["n_ptc"][0] == 0 and 2 <= good["n_newton"][0] <= 8
+    assert close(good["Y"][0, 0], root, 1e-8) and close(good["Y"][1, 0], 1 - root, 1e-8)
+    # far guess: the first Newton trial is not admissible -> pseudo-transient conditioning -> Newton
+    far = orc.solve_hybrid(om, *args, np.array([[1.0 - 1e-9], [1e-9]]), Yin, np.array([tau]), atol=1e-14, rtol=1e-10,
+                           max_iter=400, max_newton=6, max_ptc=10, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=0.0)
+    bad = orc.solve_hybrid(om, *args, np.array([[1.0 - 1e-9], [1e-9]]), Yin, np.array([tau]), atol=1e-14, rtol=1e-10,
+                           max_iter=100, max_newton=100, max_ptc=0 + 1, dt0=1e-30, dt_grow=1.0, y_floor=0.0)
+    assert far["status"][0] == 0 and far["n_ptc"][0] > 0 and far["n_ptc"][0] % 10 == 0
+    assert close(far["Y"][0, 0], root, 1e-8)
+    assert far["n_newton"][0] + far["n_ptc"][0] <= 400
+    # (with a vanishing pseudo-time step the estimate cannot move: Newton keeps failing from the same point)
+    assert bad["status"][0] == 1 and bad["n_newton"][0] + bad["n_ptc"][0] == 100
+    short = orc.solve_hybrid(om, *args, np.array([[0.5], [0.5]]), Yin, np.array([tau]), atol=1e-14, rtol=1e-10, max_iter=1)
+    assert short["status"][0] == 1 and short["n_newton"][0] == 1 and short["n_ptc"][0] == 0
+
+
+def test_solver_pseudo_transient_steps_with_a_huge_dt_are_newton_steps():
+    """(I/dt + J) dx = -F tends to the Newton system as dt -> inf: a run that is forced through pseudo-transient
+    stages (max_newton = 1) with dt0 = 1e300 walks through the same estimates as the pure Newton iteration.
+    Tolerances are set so that neither run stops early."""
+    mech = _two_species(((0, 0), (1,)), W=[15.0, 30.0], A=2.0e9, b=0.0, Ea=2.0e3, a6B=23.0)
+    om = oracle_mech(mech)
+    T, P, tau = np.array([1200.0]), np.array([PATM]), np.array([1e-3])
+    Yin, Y0 = np.array([[0.9], [0.1]]), np.array([[0.55], [0.45]])
+    for budget in (1, 2, 3, 4):
+        kw = dict(atol=1e-300, rtol=1e-300, max_iter=budget, y_floor=np.inf)
+        a = orc.solve_hybrid(om, T, P, Y0, Yin, tau, max_newton=100, **kw)
+        b = orc.solve_hybrid(om, T, P, Y0, Yin, tau, max_newton=1, max_ptc=100, dt0=1e300, dt_grow=1.0, **kw)
+        assert a["n_newton"][0] == budget and b["n_newton"][0] == 1 and b["n_ptc"][0] == budget - 1
+        assert np.allclose(a["Y"], b["Y"], rtol=1e-12, atol=0)
+
+
+def test_solver_adiabatic_inert_reactor_settles_at_the_inlet_state():
+    """Energy row as row 0 (Tin given), no chemistry: the steady state is Y = Y_in, T = T_in (the inflow enthalpy
+    difference sum Y_in (h_in - h(T)) vanishes only there, h being monotone in T)."""
+    mech, batch = synth.make_config("C0", 6)
+    mm = copy.deepcopy(mech)
+    mm.A = np.zeros_like(mech.A)
+    Tin = np.linspace(600.0, 900.0, 6)
+    r = orc.solve_hybrid(oracle_mech(mm), batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin, atol=1e-12, rtol=1e-10,
+                         max_newton=30, y_floor=np.inf)
+    assert np.all(r["status"] == 0) and np.all(r["n_ptc"] == 0)
+    assert np.allclose(r["T"], Tin, rtol=1e-9) and np.allclose(r["Y"], batch.Yin, rtol=1e-10, atol=1e-14)
