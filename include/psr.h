@@ -163,6 +163,40 @@ psr_status psr_lu_solve(int64_t N, int32_t n, const double* A, double* b, int32_
 psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F, const double* dt, double* dx,
                          int32_t* info, void* stream);
 
+/* Hybrid Newton / pseudo-transient solve of the PSR equations for N reactors (PAPER.md:44:
+ * "The hybrid approach consists of two steps: a steady state Newton iteration and a pseudo-transient time
+ * integration.  If convergence is not achieved using the Newton iteration, the solution estimate is conditioned
+ * using the time integration.  The process of switching ... continues until convergence is achieved, which is based
+ * on ... absolute and relative tolerances").  The paper leaves the constants and the step-size rule to its ref. [5]:
+ * they are the caller's, in psr_solve_opts, and the rules below are DESIGN.md readings g21-g25.
+ *   Unknowns x = (T, Y_1..Y_K); equations: the residual of psr_fd_jacobian (row 0: T stays at its input value),
+ *   or with Tin != NULL that of psr_fd_jacobian_energy (row 0: the energy row; T is solved for).
+ *   Every iteration: F and the forward-difference Jacobian at x, the solve of (I/dt + J) dx = -F (no shift in a
+ *   Newton iteration), the trial x' = x + dx.  A trial is admissible when the system solved without a zero pivot,
+ *   dx is finite and every mass fraction of x' is >= -y_floor (+inf switches the bound off).
+ *   Newton iteration: converged when max_i |dx_i| / (atol + rtol |x_i|) <= 1 (the correction is applied); an
+ *   inadmissible trial, or max_newton admissible iterations without convergence, end the Newton stage and max_ptc
+ *   pseudo-transient steps follow, after which Newton resumes.  Pseudo-transient step: dt starts at dt0 and
+ *   persists; an admissible step is taken and dt *= dt_grow, otherwise x stays and dt *= dt_shrink.
+ *   Every solve counts; after max_iter of them a reactor is left as it is with status 1.
+ * T [N], Y [K][ld]: DEVICE, initial estimate in, solution estimate out.  P, Tin (or NULL), Yin [K][ld], tau: DEVICE
+ * inputs.  status [N]: 0 converged, 1 not converged within max_iter; n_newton, n_ptc [N] (may be NULL): iterations
+ * of each kind performed.  workspace: DEVICE scratch of workspace_bytes >= psr_solve_hybrid_workspace_bytes(mech, 1)
+ * bytes; with less than psr_solve_hybrid_workspace_bytes(mech, N) the batch is solved in sub-batches one after the
+ * other.  Runs entirely on the device: max_iter rounds of (psr_fd_jacobian, psr_ptc_solve, one bookkeeping kernel)
+ * are enqueued on `stream` for every sub-batch, with no host synchronisation (converged reactors are left
+ * untouched by the later rounds); capturable in a CUDA graph after psr_mech_reserve(mech, N). */
+typedef struct {
+  double atol, rtol;
+  int32_t max_iter, max_newton, max_ptc, reserved;
+  double dt0, dt_grow, dt_shrink, y_floor;
+} psr_solve_opts;
+size_t psr_solve_hybrid_workspace_bytes(const psr_mech* mech, int64_t N);
+psr_status psr_solve_hybrid(const psr_mech* mech, int64_t N, double* T, const double* P, double* Y, const double* Tin,
+                            const double* Yin, const double* tau, int64_t ld, const psr_solve_opts* opts,
+                            void* workspace, size_t workspace_bytes, int32_t* status, int32_t* n_newton,
+                            int32_t* n_ptc, void* stream);
+
 /* Thread-local description of the last failure on this thread; valid until its next psr_* call. */
 const char* psr_last_error(void);
 

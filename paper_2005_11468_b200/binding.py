@@ -18,7 +18,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_solve_hybrid", "psr_solve_hybrid_workspace_bytes", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -34,6 +34,13 @@ class PsrMechDesc(C.Structure):
 class PsrMechInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_species", "n_reactions", "tile", "warps", "chunk_reactions", "n_chunks",
                                          "smem_bytes", "ctas_per_sm", "n_sm", "n_falloff", "n_third_body", "nnz_nu")]
+
+
+class PsrSolveOpts(C.Structure):
+    """psr_solve_opts: the constants of the hybrid solver (the paper leaves them to its ref. [5])."""
+    _fields_ = [("atol", C.c_double), ("rtol", C.c_double), ("max_iter", C.c_int32), ("max_newton", C.c_int32),
+                ("max_ptc", C.c_int32), ("reserved", C.c_int32), ("dt0", C.c_double), ("dt_grow", C.c_double),
+                ("dt_shrink", C.c_double), ("y_floor", C.c_double)]
 
 
 class PsrError(RuntimeError):
@@ -79,6 +86,10 @@ def lib():
         L.psr_last_error.restype = C.c_char_p
         L.psr_mech_info.argtypes = [vp, C.POINTER(PsrMechInfo)]
         L.psr_mech_info.restype = C.c_int
+        L.psr_solve_hybrid_workspace_bytes.argtypes = [vp, i64]
+        L.psr_solve_hybrid_workspace_bytes.restype = C.c_size_t
+        L.psr_solve_hybrid.argtypes = [vp, i64, dp, dp, dp, dp, dp, dp, i64, C.POINTER(PsrSolveOpts), vp, C.c_size_t, dp, dp, dp, vp]
+        L.psr_solve_hybrid.restype = C.c_int
         L.psr_mech_reserve.argtypes = [vp, i64]
         L.psr_mech_reserve.restype = C.c_int
         L.psr_mech_set_option.argtypes = [vp, C.c_int32, C.c_int32]
@@ -283,6 +294,30 @@ class Mechanism:
             _check(lib().psr_fd_jacobian(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(J),
                                          _ptr(F0), _stream()))
         return (J, F0) if F0 is not None else J
+
+
+def _solve_hybrid(self, T, P, Y, Yin, tau, Tin=None, workspace=None, atol=1e-12, rtol=1e-8, max_iter=50, max_newton=10,
+                  max_ptc=10, dt0=1e-6, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9):
+    """psr_solve_hybrid: T [N] and Y [K][ld] hold the initial estimate and are overwritten by the solution estimate.
+    Returns (status, n_newton, n_ptc) int32 [N].  workspace: a CUDA uint8 tensor (allocated for the whole batch if
+    None; a smaller one makes the call work through the batch in sub-batches)."""
+    import torch
+    N = T.shape[0]
+    ld = _ld(Y, N)
+    for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau)) + ((("Tin", Tin),) if Tin is not None else ()):
+        _chk_dev(nm, t)
+    _chk_ld("Yin", Yin, N, ld)
+    if workspace is None:
+        workspace = torch.empty(int(lib().psr_solve_hybrid_workspace_bytes(self._h, max(N, 1))), dtype=torch.uint8, device=T.device)
+    opts = PsrSolveOpts(atol, rtol, max_iter, max_newton, max_ptc, 0, dt0, dt_grow, dt_shrink, y_floor)
+    status, nn, npt = (torch.empty(N, dtype=torch.int32, device=T.device) for _ in range(3))
+    self.reserve(N)
+    _check(lib().psr_solve_hybrid(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Tin), _ptr(Yin), _ptr(tau), ld, C.byref(opts),
+                                  _ptr(workspace), workspace.numel(), _ptr(status), _ptr(nn), _ptr(npt), _stream()))
+    return status, nn, npt
+
+
+Mechanism.solve_hybrid = _solve_hybrid
 
 
 def probe_fp64(kind: int, iters: int):

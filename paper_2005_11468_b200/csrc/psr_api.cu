@@ -23,6 +23,11 @@ cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
                             cudaStream_t st, const double* F, const double* dt);
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
+cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
+                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
+cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
+                                 const int32_t* info, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it, int32_t* status,
+                                 int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
 cudaError_t ws_set_smem(size_t smem);
 cudaError_t launch_ws(const WsView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st);
 }  // namespace psr
@@ -953,6 +958,62 @@ psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F,
   if (!J || !F || !dt || !dx || !info) return fail(PSR_EINVAL, "psr_ptc_solve: null J, F, dt, dx or info");
   if (dx == F) return fail(PSR_EINVAL, "psr_ptc_solve: dx must not alias F");
   return solve_impl("psr_ptc_solve", N, n, J, dx, info, F, dt, stream);
+}
+
+namespace {
+// workspace of the hybrid solver per reactor: J, F0, dx, the two dt arrays (doubles); info, mode, it (int32)
+size_t hybrid_bytes_per_reactor(int n) { return ((size_t)n * n + 2 * (size_t)n + 2) * 8 + 3 * 4 + 4; }
+}  // namespace
+
+size_t psr_solve_hybrid_workspace_bytes(const psr_mech* m, int64_t N) {
+  if (!m || N < 1) return 0;
+  return hybrid_bytes_per_reactor(m->view.K + 1) * (size_t)N + 256;
+}
+
+psr_status psr_solve_hybrid(const psr_mech* m, int64_t N, double* T, const double* P, double* Y, const double* Tin,
+                            const double* Yin, const double* tau, int64_t ld, const psr_solve_opts* o, void* workspace,
+                            size_t workspace_bytes, int32_t* status, int32_t* n_newton, int32_t* n_ptc, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(m, N, T, P, Y, ld, "psr_solve_hybrid");
+  if (st != PSR_OK || N == 0) return st;
+  if (!Yin || !tau || !o || !workspace || !status) return fail(PSR_EINVAL, "psr_solve_hybrid: null Yin, tau, opts, workspace or status");
+  if (!(o->atol >= 0.0) || !(o->rtol >= 0.0) || !(o->atol + o->rtol > 0.0) || o->max_iter < 0 || o->max_newton < 1 || o->max_ptc < 1 ||
+      !(o->dt0 > 0.0) || !(o->dt_grow > 0.0) || !(o->dt_shrink > 0.0) || std::isnan(o->y_floor))
+    return fail(PSR_EINVAL, "psr_solve_hybrid: options out of range (atol, rtol >= 0 and not both 0; max_iter >= 0; max_newton, max_ptc >= 1; dt0, dt_grow, dt_shrink > 0)");
+  const int n = m->view.K + 1;
+  if (n > 168) return fail(PSR_EUNSUPPORTED, "psr_solve_hybrid: %d unknowns, the linear solve takes <= 168", n);
+  uintptr_t base = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~(uintptr_t)255;
+  const size_t lost = base - reinterpret_cast<uintptr_t>(workspace);
+  if (workspace_bytes <= lost + hybrid_bytes_per_reactor(n)) return fail(PSR_EINVAL, "psr_solve_hybrid: workspace smaller than one reactor needs");
+  const int64_t Nb = std::min<int64_t>(N, (int64_t)((workspace_bytes - lost) / hybrid_bytes_per_reactor(n)));
+  double* J = reinterpret_cast<double*>(base);
+  double* F0 = J + (size_t)Nb * n * n;
+  double* dx = F0 + (size_t)Nb * n;
+  double* dt_cur = dx + (size_t)Nb * n;
+  double* dt_arg = dt_cur + Nb;
+  int32_t* info = reinterpret_cast<int32_t*>(dt_arg + Nb);
+  int32_t* mode = info + Nb;
+  int32_t* it = mode + Nb;
+  cudaStream_t cs = (cudaStream_t)stream;
+  for (int64_t r0 = 0; r0 < N; r0 += Nb) {
+    const int64_t nb = std::min(Nb, N - r0);
+    double* Tb = T + r0;
+    double* Yb = Y + r0;
+    cudaError_t e = launch_hybrid_init(nb, *o, dt_cur, dt_arg, mode, it, status + r0, n_newton ? n_newton + r0 : nullptr,
+                                       n_ptc ? n_ptc + r0 : nullptr, cs);
+    if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (init)");
+    for (int iter = 0; iter < o->max_iter; ++iter) {
+      // error vector and Jacobian at the current estimates, the (shifted) solve, the per-reactor decisions
+      st = fd_jacobian_impl(m, nb, Tb, P + r0, Yb, Tin ? Tin + r0 : nullptr, Yin + r0, tau + r0, ld, J, F0, stream, "psr_solve_hybrid");
+      if (st != PSR_OK) return st;
+      st = solve_impl("psr_solve_hybrid", nb, n, J, dx, info, F0, dt_arg, stream);
+      if (st != PSR_OK) return st;
+      e = launch_hybrid_update(nb, n, ld, *o, Tb, Yb, dx, info, dt_cur, dt_arg, mode, it, status + r0,
+                               n_newton ? n_newton + r0 : nullptr, n_ptc ? n_ptc + r0 : nullptr, cs);
+      if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (update)");
+    }
+  }
+  return PSR_OK;
 }
 
 psr_status psr_mech_set_option(psr_mech* m, int32_t option, int32_t value) {

@@ -719,6 +719,161 @@ def test_pseudo_transient_iteration_on_device_reduces_the_residual(torch_cuda, b
     assert norms[2] < norms[1] < norms[0], norms
 
 
+# ------------------------------------------------------------------ hybrid solver (NEXT-4)
+SOLVE_KW = dict(atol=1e-12, rtol=1e-7, max_iter=260, max_newton=5, max_ptc=20, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9)
+
+
+def _solve_both(torch, binding, mech, T0, P, Y0, Yin, tau, Tin=None, workspace_reactors=None, **kw):
+    gm = binding.Mechanism.from_synth(mech)
+    T, Y = dev(torch, T0), dev(torch, Y0)
+    ws = None
+    if workspace_reactors is not None:
+        ws = torch.empty(int(binding.lib().psr_solve_hybrid_workspace_bytes(gm._h, workspace_reactors)), dtype=torch.uint8, device="cuda")
+    st, nn, npt = gm.solve_hybrid(T, dev(torch, P), Y, dev(torch, Yin), dev(torch, tau),
+                                  Tin=None if Tin is None else dev(torch, Tin), workspace=ws, **kw)
+    torch.cuda.synchronize()
+    got = dict(T=T.cpu().numpy(), Y=Y.cpu().numpy(), status=st.cpu().numpy(), n_newton=nn.cpu().numpy(), n_ptc=npt.cpu().numpy())
+    gm.close()
+    ref = orc.solve_hybrid(oracle_mech(mech), T0, P, Y0, Yin, tau, Tin=Tin, **kw)
+    return got, ref
+
+
+def _compare_solves(mech, got, ref, P, Yin, tau, kw, exact_paths=False):
+    """The device loop against the oracle's.  What is unique is compared strictly: which reactors converge, and the
+    solution (within the solver's own tolerance).  The PATH is not unique under rounding -- the forward-difference
+    Jacobians of the two sides differ at the 1e-8 level, the systems are ill-conditioned, and "has the correction
+    passed the tolerance within max_newton iterations" then falls differently for some reactors, which adds or
+    removes a pseudo-transient stage -- so iteration counts must agree on average, and exactly where
+    `exact_paths` says the path is short and well-conditioned enough to be unique."""
+    conv = (got["status"] == 0) & (ref["status"] == 0)
+    assert (got["status"] == ref["status"]).mean() >= 0.95
+    same = conv & (got["n_newton"] == ref["n_newton"]) & (got["n_ptc"] == ref["n_ptc"])
+    if exact_paths:
+        assert same.sum() >= 0.9 * conv.sum(), (conv.mean(), same.mean())
+    else:
+        for k in ("n_newton", "n_ptc"):
+            assert abs(got[k][conv].mean() - ref[k][conv].mean()) <= 0.1 * ref[k][conv].mean() + 0.5, k
+        assert same.mean() >= 0.2
+    # the same solution wherever both converged (to the same root: a few reactors of a stiff mechanism have more than one)
+    w = kw["atol"] + kw["rtol"] * np.abs(ref["Y"])
+    d = (np.abs(got["Y"] - ref["Y"]) / w).max(axis=0)
+    assert (d[conv] <= 1.0).mean() >= 0.97 and d[same].max() <= 1.0
+    assert np.allclose(got["T"][conv], ref["T"][conv], rtol=10 * kw["rtol"])
+    # every converged device solution satisfies the equations as well as the oracle's do (judged by the oracle)
+    om = oracle_mech(mech)
+    ok, okr = got["status"] == 0, ref["status"] == 0
+    Fg = orc.evaluate(om, got["T"], P, got["Y"], Yin, tau, want=("F",))["F"]
+    Fr = orc.evaluate(om, ref["T"], P, ref["Y"], Yin, tau, want=("F",))["F"]
+    Sg = orc.roundoff_scale(om, got["T"], P, got["Y"], Yin, tau)["SF"]
+    Sr = orc.roundoff_scale(om, ref["T"], P, ref["Y"], Yin, tau)["SF"]
+    rg = (np.abs(Fg) / np.where(Sg > 0, Sg, 1.0))[:, ok].max(axis=0)       # |F_i| against the size of its terms
+    rr = (np.abs(Fr) / np.where(Sr > 0, Sr, 1.0))[:, okr].max(axis=0)
+    assert np.median(rg) <= 2 * np.median(rr) + 1e-12 and rg.max() <= 10 * rr.max() + 1e-9
+
+
+def test_solve_hybrid_matches_the_oracle_loop_on_C0(torch_cuda, binding):
+    """psr_solve_hybrid from the generated (far) initial states of C0: Newton stages, pseudo-transient conditioning
+    and the switches between them, on the device, against the oracle's loop; also in sub-batches (small workspace)."""
+    mech, batch = synth.make_config("C0", 300)
+    got, ref = _solve_both(torch_cuda, binding, mech, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, **SOLVE_KW)
+    assert (ref["n_ptc"] > 0).any() and (ref["status"] == 0).mean() > 0.9
+    _compare_solves(mech, got, ref, batch.P, batch.Yin, batch.tau, SOLVE_KW)
+    got2, _ = _solve_both(torch_cuda, binding, mech, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, workspace_reactors=77, **SOLVE_KW)
+    for k in got:
+        assert np.array_equal(got[k], got2[k]), k      # sub-batching does not change a reactor's path
+
+
+def test_solve_hybrid_paths_that_are_unique(torch_cuda, binding):
+    """Where the path does not hang on rounding the device takes exactly the oracle's: an inert mechanism (linear
+    residual: two Newton iterations), and a second-order reaction 2A <=> B from near and far guesses (Newton alone;
+    an inadmissible first trial, a pseudo-transient stage, then Newton)."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C0", 64)
+    mm = copy.deepcopy(mech)
+    mm.A = np.zeros_like(mech.A)
+    kw = dict(SOLVE_KW, atol=1e-9, rtol=1e-6)
+    got, ref = _solve_both(torch, binding, mm, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, **kw)
+    # (a species whose Y is far below its Y_in has a forward-difference column accurate to eps |Y - Y_in| / h only,
+    # which can cost a third iteration on either side)
+    assert np.all(got["status"] == 0) and np.all(got["n_ptc"] == 0) and np.all((got["n_newton"] == 2) | (got["n_newton"] == 3))
+    assert (got["n_newton"] == 2).mean() >= 0.8 and (got["n_newton"] == ref["n_newton"]).mean() >= 0.8
+    assert np.allclose(got["Y"], batch.Yin, rtol=1e-12, atol=1e-15)
+    # 2A <=> B (the mechanism of the oracle's pin), a sweep of initial guesses
+    reac_ptr, reac_sp, reac_nu = synth._side_csr([(0, 0)])
+    prod_ptr, prod_sp, prod_nu = synth._side_csr([(1,)])
+    m2 = synth.Mechanism(
+        n_species=2, n_reactions=1, atoms=np.zeros((2, 4), dtype=np.int32), W=np.array([15.0, 30.0]),
+        nasa=np.array([[3.5, 1e-4, 0.0, 0.0, 0.0, -1000.0, 2.0], [3.9, 3e-4, -2e-8, 0.0, 0.0, -1600.0, 23.0]]),
+        A=np.array([2.0e9]), b=np.array([0.0]), Ea=np.array([2.0e3]), rtype=np.zeros(1, dtype=np.uint8),
+        reversible=np.ones(1, dtype=np.uint8), reac_ptr=reac_ptr, reac_sp=reac_sp, reac_nu=reac_nu,
+        prod_ptr=prod_ptr, prod_sp=prod_sp, prod_nu=prod_nu, eff_ptr=np.zeros(2, dtype=np.int32),
+        eff_sp=np.zeros(0, dtype=np.int32), eff_val=np.zeros(0), A0=np.zeros(1), b0=np.zeros(1), Ea0=np.zeros(1),
+        troe=np.zeros((1, 4)), meta={"name": "2A<=>B"})
+    yA = np.concatenate([np.linspace(0.02, 0.98, 49), [1e-9, 1 - 1e-9, 1 - 1e-6]])
+    N = yA.size
+    Y0 = np.stack([yA, 1 - yA])
+    Yin = np.tile(np.array([[0.9], [0.1]]), (1, N))
+    kw = dict(atol=1e-14, rtol=1e-9, max_iter=200, max_newton=8, max_ptc=10, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=0.0)
+    got, ref = _solve_both(torch, binding, m2, np.full(N, 1200.0), np.full(N, 1.01325e6), Y0, Yin, np.full(N, 1e-3), **kw)
+    assert np.all(ref["status"] == 0) and (ref["n_ptc"] > 0).any() and (ref["n_ptc"] == 0).any()
+    for k in ("status", "n_newton", "n_ptc"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert np.allclose(got["Y"], ref["Y"], rtol=1e-9, atol=1e-14)
+    assert np.allclose(got["Y"][0], 0.48972816473969222, rtol=1e-8)      # the mpmath root of tests/test_oracle_pins.py
+
+
+def test_solve_hybrid_on_C4_from_far_and_from_perturbed_converged_states(torch_cuda, binding):
+    """BASELINE config 4's mechanism (53 species / 325 reactions): from the generated states (pseudo-transient stages
+    needed), then from converged states perturbed by 1 % (Newton alone, a few iterations: the same path on both sides)."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C4", 96)
+    kw0 = dict(SOLVE_KW, max_iter=420)
+    got, ref = _solve_both(torch, binding, mech, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, **kw0)
+    assert (ref["n_ptc"] > 0).all() and (ref["status"] == 0).mean() > 0.9
+    _compare_solves(mech, got, ref, batch.P, batch.Yin, batch.tau, kw0)
+    conv = ref["status"] == 0
+    rng = np.random.default_rng(17)
+    Y1 = ref["Y"][:, conv] * (1.0 + 0.01 * rng.uniform(-1, 1, (mech.n_species, conv.sum())))
+    sub = batch.take(np.flatnonzero(conv))
+    kw = dict(SOLVE_KW, atol=1e-10, rtol=1e-5, max_iter=12, max_newton=12)
+    got1, ref1 = _solve_both(torch, binding, mech, ref["T"][conv], sub.P, Y1, sub.Yin, sub.tau, **kw)
+    assert (ref1["status"] == 0).mean() > 0.9 and (ref1["n_ptc"][ref1["status"] == 0] == 0).all()
+    _compare_solves(mech, got1, ref1, sub.P, sub.Yin, sub.tau, kw, exact_paths=True)
+    w = kw["atol"] + 10 * kw["rtol"] * np.abs(ref["Y"][:, conv])
+    ok = (got1["status"] == 0)
+    assert (np.abs(got1["Y"] - ref["Y"][:, conv]) / w)[:, ok].max() <= 1.0     # back at the solution it was perturbed from
+
+
+def test_solve_hybrid_adiabatic_and_argument_checks(torch_cuda, binding):
+    """Tin given: row 0 of the system is the energy row and T is solved for.  An inert mechanism settles at
+    (T_in, Y_in) on the same path as the oracle.  (With chemistry the adiabatic systems of these synthetic mechanisms
+    are too ill-conditioned for two FP64 codes to stay on one path from a far guess; their Jacobians and solves are
+    compared one call at a time by the floor-criterion and backward-error tests above.)"""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C0", 40)
+    Tin = np.linspace(600.0, 900.0, batch.n)
+    mm = copy.deepcopy(mech)
+    mm.A = np.zeros_like(mech.A)
+    kw = dict(SOLVE_KW, atol=1e-9, rtol=1e-6, max_iter=40, max_newton=30, y_floor=np.inf)
+    got, ref = _solve_both(torch, binding, mm, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, Tin=Tin, **kw)
+    # (a far first Newton step in T can leave T > 0 -- only the mass fractions are bounded -- and such a reactor
+    # never recovers: on both sides alike)
+    ok = ref["status"] == 0
+    assert np.array_equal(got["status"], ref["status"]) and ok.mean() >= 0.8
+    assert np.all(got["n_ptc"][ok] == 0) and (got["n_newton"] == ref["n_newton"])[ok].mean() >= 0.8
+    assert np.allclose(got["T"][ok], Tin[ok], rtol=1e-8) and np.allclose(got["Y"][:, ok], batch.Yin[:, ok], rtol=1e-9, atol=1e-13)
+    gm = binding.Mechanism.from_synth(mech)
+    T, Y = dev(torch, batch.T), dev(torch, batch.Y)
+    args = (T, dev(torch, batch.P), Y, dev(torch, batch.Yin), dev(torch, batch.tau))
+    with pytest.raises(binding.PsrError):
+        gm.solve_hybrid(*args, max_newton=0)
+    with pytest.raises(binding.PsrError):
+        gm.solve_hybrid(*args, workspace=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    st, nn, npt = gm.solve_hybrid(*args, max_iter=0)      # no budget: nothing moves, nothing converged
+    assert bool((st == 1).all()) and bool((nn == 0).all()) and np.array_equal(Y.cpu().numpy(), batch.Y)
+    gm.close()
+
+
 # ------------------------------------------------------------------ streams and graphs
 def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, binding):
     """Every evaluation call only enqueues work on the caller's stream (psr.h), so a Newton iteration
