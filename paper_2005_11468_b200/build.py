@@ -14,7 +14,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpsr_b200.so"
 SOURCES = [CSRC / "psr_api.cu", CSRC / "psr_kernels.cu", CSRC / "psr_ws.cu", CSRC / "psr_lu.cu", CSRC / "psr_solve.cu"]
-HEADERS = [CSRC / "psr_tables.h", CSRC / "psr_math.cuh", CSRC / "psr_ptx.cuh", PKG.parent / "include" / "psr.h"]
+HEADERS = [CSRC / "psr_tables.h", CSRC / "psr_math.cuh", CSRC / "psr_ptx.cuh", CSRC / "psr_rx.cuh", PKG.parent / "include" / "psr.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

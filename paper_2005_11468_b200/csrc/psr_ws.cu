@@ -29,6 +29,7 @@
 
 #include "psr_math.cuh"
 #include "psr_ptx.cuh"
+#include "psr_rx.cuh"
 #include "psr_tables.h"
 
 namespace psr {
@@ -36,8 +37,6 @@ namespace psr {
 namespace {
 
 __device__ constexpr double kRgasW = 8.31446261815324e7;  // erg/mol/K
-__device__ constexpr double kLog10eW = 0.43429448190325182765;
-constexpr int T_PLAIN = 0, T_THREE_BODY = 1, T_LINDEMANN = 2, T_TROE = 3;  // = PSR_RX_* of psr.h
 
 // mbarrier slots
 constexpr int B_BLOB = 0, B_IN = 1, B_FULLC = 3, B_EMPTYC = 5, B_FULLQ = 7, B_EMPTYQ = 9, B_COUNT = 11;
@@ -53,188 +52,6 @@ struct __align__(16) SpEnt {
   double W;                // molar mass
 };
 static_assert(sizeof(SpEnt) == 32, "SpEnt layout");
-
-struct RxCtx {
-  double T, lnT, invT;
-  uint32_t c_lane;    // this lane's column of row 0 of the C tile (shared-memory address)
-  uint32_t q_lane;    // this lane's column of row 0 of the q buffer
-  uint32_t st_lane;   // this lane's column of row 0 of the tile's state rows
-  ExpTab etab;
-  float amax;         // NaN-propagating running max of |high word| of the exp arguments of this lane
-};
-
-// One record class of one warp's share of a part (a3..a7).  CLS: 0..3 = reaction type in the 3+3 slot form,
-// kClsLong = long factor lists.  FAST: table exp, range noted in cx.amax; else the library exp.  OUTK: k_f, k_r,
-// q also go to global memory (psr_eval_kf_kr, q of psr_eval_wdot).
-template <int CLS, bool FAST, bool OUTK>
-__device__ __forceinline__ void ws_run_class(RxCtx& cx, const unsigned char* blob, const ChunkHdr* hdr, const RxRec* recs,
-                                             int w, const EvalArgs& a, int64_t r, bool valid) {
-  const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
-  const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS + 1]);
-  auto exps = [&](auto& ex, auto& ey) {
-    constexpr int N = sizeof(ex) / sizeof(double);
-    if constexpr (FAST) {
-#pragma unroll
-      for (int i = 0; i < N; ++i) cx.amax = exp_arg_max(cx.amax, ex[i]);
-      exp_core_n<N>(ex, ey, cx.etab);
-    } else {
-#pragma unroll
-      for (int i = 0; i < N; ++i) ey[i] = exp(ex[i]);
-    }
-  };
-  // slot offsets (and meta, korig) of a record are read one trip ahead: they head the longest chain of a trip
-  uint4 nxa, nxb;
-  {
-    const uint32_t ra = smem_u32(recs + kl_begin) + 80;
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(nxa.x), "=r"(nxa.y), "=r"(nxa.z), "=r"(nxa.w) : "r"(ra));
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+16];" : "=r"(nxb.x), "=r"(nxb.y), "=r"(nxb.z), "=r"(nxb.w) : "r"(ra));
-  }
-#pragma unroll 1
-  for (int kl = kl_begin; kl < kl_end; ++kl) {
-    const RxRec* rec = recs + kl;
-    const uint4 ra_ = nxa, rb_ = nxb;   // {meta, off[0..2]}, {off[3..5], korig} of this record
-    {
-      const uint32_t ra = smem_u32(rec) + (112 + 80);
-      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(nxa.x), "=r"(nxa.y), "=r"(nxa.z), "=r"(nxa.w) : "r"(ra));
-      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4+16];" : "=r"(nxb.x), "=r"(nxb.y), "=r"(nxb.z), "=r"(nxb.w) : "r"(ra));
-    }
-    const uint32_t meta = ra_.x;
-    const int type = CLS < kClsLong ? CLS : (int)(meta & kMetaTypeMask);
-    const double T = cx.T, lnT = cx.lnT, invT = cx.invT;
-    // Eq. 6 in log form, and ln k_r = ln k_f - ln K_c (Eq. 7-9 summed per reaction at load time)
-    const double lnkf = fma(rec->c[1], lnT, fma(rec->c[2], invT, rec->c[0]));
-    const double pn = fma(fma(fma(rec->d[3], T, rec->d[2]), T, rec->d[1]), T, rec->d[0]);
-    const double lnkr = fma(pn, T, fma(rec->e[1], lnT, fma(rec->e[2], invT, rec->e[0])));
-    double pf, pr, kf = 0.0, kr = 0.0;
-
-    // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
-    if constexpr (CLS < kClsLong) {
-      const double f0 = lds64(cx.c_lane + ra_.y), f1 = lds64(cx.c_lane + ra_.z), f2 = lds64(cx.c_lane + ra_.w);
-      const double p0 = lds64(cx.c_lane + rb_.x), p1 = lds64(cx.c_lane + rb_.y), p2 = lds64(cx.c_lane + rb_.z);
-      pf = f0 * f1 * f2;
-      pr = p0 * p1 * p2;
-    } else {
-      const uint16_t* fsp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + ra_.y;
-      const int nr = (int)((meta >> kMetaNrShift) & 0xF);
-      const int np = (int)((meta >> kMetaNpShift) & 0xF);
-      pf = 1.0;
-      pr = 1.0;
-#pragma unroll 1
-      for (int j = 0; j < nr + np; ++j) {
-        const double cv = lds64(cx.c_lane + (uint32_t)fsp[j] * (uint32_t)kRowBytes);
-        if (j < nr) pf *= cv;
-        else pr *= cv;
-      }
-      if (!(meta & kMetaRev)) pr = 0.0;
-    }
-
-    // sign of A and of A0/A (any finite A is accepted: negative pre-exponentials of duplicate reactions, A = 0): only
-    // long-form records carry them (psr_tables.h), so this folds away in the other class loops
-    double sA = 1.0, sPr = 1.0;
-    if constexpr (CLS == kClsLong) {
-      const uint32_t sg = (meta >> kMetaSgnShift) & 0xFu;
-      if (sg) {
-        const double s0 = (sg >> 2) == 0 ? 1.0 : (sg >> 2) == 1 ? -1.0 : 0.0;
-        sA = (sg & 3u) == 0 ? 1.0 : (sg & 3u) == 1 ? -1.0 : 0.0;
-        sPr = sA == 0.0 ? __longlong_as_double(0x7ff8000000000000LL) : s0 * sA;   // k0 [M] / 0 is not a number
-      }
-    }
-    if (type <= T_THREE_BODY) {
-      double ex[2], ey[2];
-      ex[0] = lnkf;
-      ex[1] = lnkr;
-      exps(ex, ey);
-      kf = ey[0];
-      kr = ey[1];
-      if constexpr (CLS == kClsLong) {
-        kf *= sA;
-        kr *= sA;
-      }
-    }
-    if (type != T_PLAIN) {
-      const AuxRec* ax = reinterpret_cast<const AuxRec*>(blob + hdr->off_aux) + (meta >> kMetaAuxShift);
-      const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
-      double M = lds64(cx.st_lane + ST_CTOT * kRowBytes);
-      const uint32_t e1 = ax->eff_off + ax->n_eff;
-#pragma unroll 1
-      for (uint32_t e = ax->eff_off; e < e1; ++e) M = fma(effs[e].am1, lds64(cx.c_lane + effs[e].off), M);
-      if (type == T_THREE_BODY) {
-        pf *= M;
-        pr *= M;
-      } else if (type == T_LINDEMANN) {
-        // k_f = k_inf Pr/(1+Pr), Pr = k0 [M]/k_inf
-        double ex[3], ey[3];
-        const double lnk0 = fma(ax->c0[1], lnT, fma(ax->c0[2], invT, ax->c0[0]));
-        ex[0] = lnk0 - lnkf;
-        ex[1] = lnkf;
-        ex[2] = lnkr - lnkf;
-        exps(ex, ey);
-        double Pr = ey[0] * M;
-        if constexpr (CLS == kClsLong) Pr *= sPr;
-        kf = ey[1] * (Pr / (1.0 + Pr));
-        if constexpr (CLS == kClsLong) kf *= sA;
-        kr = kf * ey[2];
-      } else {
-        // Troe.  With ln Pr = ln k0 - ln k_inf + ln[M]:  k_f = k_inf Pr/(1+Pr) F = exp(ln k0 + ln[M] + ln F)/(1+Pr)
-        const double lnM = ax->n_eff == 0 ? lds64(cx.st_lane + ST_LNCTOT * kRowBytes) : log(M);
-        const double lnk0 = fma(ax->c0[1], lnT, fma(ax->c0[2], invT, ax->c0[0]));
-        const double lnk0M = lnk0 + lnM;
-        const double lnPr = lnk0M - lnkf;
-        double ex[5], ey[5];
-        ex[0] = lnPr;
-        ex[1] = T * ax->troe[1];
-        ex[2] = T * ax->troe[2];
-        ex[3] = ax->troe[3] * invT;
-        ex[4] = lnkr - lnkf;        // ln(k_r/k_f) = -ln K_c
-        exps(ex, ey);
-        const double Pr = ey[0], invKc = ey[4];
-        const double al = ax->troe[0];
-        const double Fcent = fma(1.0 - al, ey[1], fma(al, ey[2], ey[3]));
-        const double lnFc = log(Fcent);
-        const double lF = lnFc * kLog10eW;
-        const double cc = fma(-0.67, lF, -0.4);
-        const double nn = fma(-1.27, lF, 0.75);
-        const double lp = fma(lnPr, kLog10eW, cc);
-        const double den = fma(-0.14, lp, nn);
-        // ln F = ln Fcent / (1 + (lp/den)^2) = ln Fcent den^2 / (den^2 + lp^2); both quotients (this one and
-        // k_f = .../(1+Pr)) share one reciprocal
-        const double den2 = den * den;
-        const double bq = fma(lp, lp, den2), dq = 1.0 + Pr;
-        const double inv = 1.0 / (bq * dq);
-        double e2[1], k2[1];
-        e2[0] = fma(lnFc * den2, dq * inv, lnk0M);
-        exps(e2, k2);
-        kf = k2[0] * (bq * inv);
-        // the log form above needs Pr > 0; otherwise log10(Pr) of the definition is not a number
-        if constexpr (CLS == kClsLong) kf = sPr > 0.0 ? kf * sA : __longlong_as_double(0x7ff8000000000000LL);
-        kr = kf * invKc;
-      }
-    }
-    // an irreversible reaction has its product side on the zero row (pr = 0), a three-body reaction carries
-    // [M] in both products: no per-lane selects here
-    const double q = fma(kf, pf, -(kr * pr));
-    sts64(cx.q_lane + (uint32_t)kl * (uint32_t)kRowBytes, q);
-    if constexpr (OUTK) {
-      if (valid) {
-        const int64_t o = (int64_t)rb_.w * a.ldk + r;
-        if (a.flags & kOutKf) a.kf[o] = kf;
-        if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr : 0.0;
-        if (a.flags & kOutQ) a.q[o] = q;
-      }
-    }
-  }
-}
-
-template <bool FAST, bool OUTK>
-__device__ __forceinline__ void ws_run_part(RxCtx& cx, const unsigned char* blob, int w, const EvalArgs& a, int64_t r, bool valid) {
-  const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
-  const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
-  ws_run_class<0, FAST, OUTK>(cx, blob, hdr, recs, w, a, r, valid);
-  ws_run_class<1, FAST, OUTK>(cx, blob, hdr, recs, w, a, r, valid);
-  ws_run_class<2, FAST, OUTK>(cx, blob, hdr, recs, w, a, r, valid);
-  ws_run_class<3, FAST, OUTK>(cx, blob, hdr, recs, w, a, r, valid);
-  ws_run_class<kClsLong, FAST, OUTK>(cx, blob, hdr, recs, w, a, r, valid);
-}
 
 }  // namespace
 
@@ -311,23 +128,43 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += gridDim.x) {
       const int b = lt & 1;
       mbar_wait(&bars[B_FULLC + b], (lt >> 1) & 1);
-      cx.st_lane = smem_u32(St0 + b * kWsStRows * kTile) + lane * 8;
+      const uint32_t st_lane = smem_u32(St0 + b * kWsStRows * kTile) + lane * 8;
       cx.c_lane = smem_u32(Cs0 + b * cs_elems) + lane * 8;
-      cx.T = lds64(cx.st_lane + ST_T * kRowBytes);
-      cx.lnT = lds64(cx.st_lane + ST_LNT * kRowBytes);
-      cx.invT = lds64(cx.st_lane + ST_INVT * kRowBytes);
+      cx.ctot_lane = st_lane + ST_CTOT * kRowBytes;
+      cx.lnctot_lane = st_lane + ST_LNCTOT * kRowBytes;
+      cx.T = lds64(st_lane + ST_T * kRowBytes);
+      cx.lnT = lds64(st_lane + ST_LNT * kRowBytes);
+      cx.invT = lds64(st_lane + ST_INVT * kRowBytes);
       const int64_t r = tile * kTile + lane;
       const bool valid = r < a.N;
       for (int p = 0; p < mv.n_parts; ++p) {
         const uint32_t g = lt * (uint32_t)mv.n_parts + (uint32_t)p, qb = g & 1, u = g >> 1;
         if (u > 0) mbar_wait(&bars[B_EMPTYQ + qb], (u - 1) & 1);   // the part that used this buffer before has been gathered
-        cx.q_lane = smem_u32(qh0 + qb * q_elems) + lane * 8;
+        const uint32_t q_lane = smem_u32(qh0 + qb * q_elems) + lane * 8;
         const unsigned char* blob = mech + (size_t)p * mv.chunk_stride;
+        // Eq. 5: q = k_f prod C^nu' - k_r prod C^nu'' (x [M] for a three-body reaction).  An irreversible reaction has
+        // its product side on the zero row (pr = 0): no per-lane selects here.
+        auto sink = [&](int kl, uint32_t meta, uint32_t korig, int type, double kf, double kr, double pf, double pr, double M) {
+          if (type == RX_THREE_BODY) {
+            pf *= M;
+            pr *= M;
+          }
+          const double q = fma(kf, pf, -(kr * pr));
+          sts64(q_lane + (uint32_t)kl * (uint32_t)kRowBytes, q);
+          if constexpr (OUTK) {
+            if (valid) {
+              const int64_t o = (int64_t)korig * a.ldk + r;
+              if (a.flags & kOutKf) a.kf[o] = kf;
+              if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr : 0.0;
+              if (a.flags & kOutQ) a.q[o] = q;
+            }
+          }
+        };
         cx.amax = 0.0f;
-        ws_run_part<true, OUTK>(cx, blob, w, a, r, valid);
+        rx_run_chunk<true>(cx, blob, w, sink);
         // an exp argument out of the table form's range (NaN, Inf, overflow, underflow: never for physical
         // states): this warp repeats its records with the library exp, which keeps IEEE results
-        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) ws_run_part<false, OUTK>(cx, blob, w, a, r, valid);
+        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<false>(cx, blob, w, sink);
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[B_FULLQ + qb]);
       }
