@@ -212,8 +212,9 @@ psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);
  * must agree (they are not tuning knobs; default 0).  PSR_OPT_JAC_UNHOISTED: psr_fd_jacobian evaluates every
  * column in full instead of reusing the T-only factors of the base state (the two sweeps are bit-identical).
  * PSR_OPT_FUSED_ONLY: psr_eval_wdot / psr_eval_residual / psr_eval_kf_kr take the single fused kernel even
- * where the warp-specialised one applies.  Not thread-safe against concurrent calls on `mech`. */
-enum { PSR_OPT_JAC_UNHOISTED = 1, PSR_OPT_FUSED_ONLY = 2 };
+ * where the warp-specialised one applies.  PSR_OPT_JAC_GENERIC: psr_fd_jacobian takes the generic
+ * three-launch sweep even where the fused Jacobian kernel applies.  Not thread-safe against concurrent calls on `mech`. */
+enum { PSR_OPT_JAC_UNHOISTED = 1, PSR_OPT_FUSED_ONLY = 2, PSR_OPT_JAC_GENERIC = 3 };
 psr_status psr_mech_set_option(psr_mech* mech, int32_t option, int32_t value);
 
 /* FP64 pipe probes used for the roofline denominator: run `iters` dependent-

@@ -28,6 +28,8 @@ cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_c
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
                                  const int32_t* info, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it, int32_t* status,
                                  int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
+cudaError_t jac_set_smem(size_t smem);
+cudaError_t launch_jac(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
 cudaError_t ws_set_smem(size_t smem);
 cudaError_t launch_ws(const WsView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st);
 }  // namespace psr
@@ -51,8 +53,17 @@ struct psr_mech {
   bool ws_ok = false;
   unsigned char* d_ws_chunks = nullptr;
   int32_t* d_ws_sp_of = nullptr;
+  JacView jac{};                // fused finite-difference Jacobian kernel (psr_jac.cu), when the mechanism qualifies (jac_ok)
+  bool jac_ok = false;
+  unsigned char* d_jac_chunks = nullptr;
+  JacInc* d_jac_inc = nullptr;
+  int32_t* d_jac_inc_ptr = nullptr;
+  uint32_t* d_jac_inc_row = nullptr;
+  int32_t* d_jac_col_order = nullptr;
+  double* d_jac_scratch = nullptr;
   int opt_fused_only = 0;       // diagnostic (psr_mech_set_option): never take the warp-specialised kernel
   int opt_jac_unhoisted = 0;    // diagnostic: every Jacobian column a full evaluation
+  int opt_jac_generic = 0;      // diagnostic: psr_fd_jacobian takes the generic three-launch sweep even where the fused kernel applies
   double* d_scratch = nullptr;  // psr_fd_jacobian: rate table [N][I][kRateVals], then F0 when the caller passes none
   size_t scratch_bytes = 0;
   std::vector<void*> retired;   // outgrown scratch buffers, freed with the mechanism
@@ -115,8 +126,16 @@ struct BlobSet {
 // blobs (psr_tables.h): records, aux records, efficiency entries, factor pool, per-species gather lists.
 // ws_sp_of (may be null): species ownership [kWsHelpWarps][ws_spw] of the warp-specialised kernel, whose gather
 // lists are one flat stream of 4-entry groups per helper warp (see psr_tables.h) instead of lists per species.
+struct JacBuild {                    // extra inputs / outputs when the blobs are those of the Jacobian kernel (psr_jac.cu)
+  const std::vector<int32_t>* sp_of; // gather ownership [kJacWarps][spw]
+  int spw = 0;
+  int rows_zero = 0;                 // index of the all-zero row of the rate tile (= rows_max of a first pass)
+  std::vector<int32_t> row_of;       // out: [I] scratch row of reaction k (mechanism-wide record index)
+  int rows_max = 0;                  // out: most rate-tile rows of a part
+};
+
 void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out,
-                 const std::vector<int32_t>* ws_sp_of = nullptr, int ws_spw = 0) {
+                 const std::vector<int32_t>* ws_sp_of = nullptr, int ws_spw = 0, JacBuild* jb = nullptr) {
   const uint32_t row_bytes = (uint32_t)kRowBytes;
   const int rc = (I + n_chunks - 1) / n_chunks;
   out.n_chunks = n_chunks;
@@ -171,9 +190,42 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
     std::vector<EffEnt> effs;
     std::vector<uint16_t> pool;
     std::vector<std::vector<uint32_t>> pos(K), neg(K);
+    // Jacobian kernel: rate-tile rows of the records, and per (species, concentration order) the rows that enter
+    // the species' sum with a plus / minus sign
+    std::vector<std::vector<uint32_t>> jpos, jneg;
+    uint32_t jrows = 0;
+    if (jb) {
+      jpos.assign((size_t)K * kJacMaxOrder, {});
+      jneg.assign((size_t)K * kJacMaxOrder, {});
+    }
     for (int kl = 0; kl < n_rx; ++kl) {
       const HostRx& h = rx[cr[kl]];
       RxRec rec = h.rec;
+      if (jb) {
+        // rows: forward rate, reverse rate; a three-body reaction q = (C_tot + E)(...) has four: C_tot x forward (order
+        // nf), E x forward (order nf + 1), C_tot x reverse, E x reverse
+        const bool tb = h.type == PSR_RX_THREE_BODY;
+        const uint32_t rbase = jrows;
+        jrows += tb ? 4 : 2;
+        rec.korig = rbase | ((uint32_t)(out.rec_base[c] + kl) << 16);
+        jb->row_of[cr[kl]] = out.rec_base[c] + kl;
+        const int nf = h.nr, nr = std::max(h.np, 1);   // (HostRx::nr / np are the reactant / product factor counts)
+        for (auto& pr : h.nu_net) {
+          for (int t = 0; t < std::abs(pr.second); ++t) {
+            auto& fw = (pr.second > 0 ? jpos : jneg);
+            auto& rv = (pr.second > 0 ? jneg : jpos);
+            if (!tb) {
+              fw[(size_t)pr.first * kJacMaxOrder + nf - 1].push_back(rbase * row_bytes);
+              rv[(size_t)pr.first * kJacMaxOrder + nr - 1].push_back((rbase + 1) * row_bytes);
+            } else {
+              fw[(size_t)pr.first * kJacMaxOrder + nf - 1].push_back(rbase * row_bytes);
+              fw[(size_t)pr.first * kJacMaxOrder + nf].push_back((rbase + 1) * row_bytes);
+              rv[(size_t)pr.first * kJacMaxOrder + nr - 1].push_back((rbase + 2) * row_bytes);
+              rv[(size_t)pr.first * kJacMaxOrder + nr].push_back((rbase + 3) * row_bytes);
+            }
+          }
+        }
+      }
       if (h.nr <= kSlots && h.np <= kSlots && !h.special_sign) {
         for (int i = 0; i < kSlots; ++i) {
           rec.off[i] = i < h.nr ? (uint32_t)h.factors[i] * row_bytes : unit_off;
@@ -213,7 +265,40 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
       while (gent.size() % 4) gent.push_back(zero_off);
     };
     std::vector<uint16_t> ws_range(2 * kWsHelpWarps, 0);   // [helper warp] first group, one past its last group
-    if (!ws_sp_of) {
+    std::vector<uint16_t> jac_range(3 * kJacWarps, 0);     // [warp] first group, one past its last group, first flush target
+    if (jb) {
+      // Jacobian kernel: per owning warp one flat stream of 4-entry groups (as for the warp-specialised kernel), the
+      // groups of a (species, order) pair together; the pair's last group carries kGatherLast and its sum goes to
+      // the next entry of the flush-target list (byte offset of row (order - 1) * K + species of the sums tile).
+      // Pairs without a term in this part are left out.
+      const uint32_t jzero = (uint32_t)jb->rows_zero * row_bytes;   // the all-zero row of the rate tile
+      gptr.clear();
+      for (int wv = 0; wv < kJacWarps; ++wv) {
+        jac_range[3 * wv] = (uint16_t)(gent.size() / 4);
+        jac_range[3 * wv + 2] = (uint16_t)gptr.size();
+        for (int jj = 0; jj < jb->spw; ++jj) {
+          const int sidx = (*jb->sp_of)[(size_t)wv * jb->spw + jj];
+          if (sidx < 0) break;
+          for (int m = 0; m < kJacMaxOrder; ++m) {
+            const auto& pp = jpos[(size_t)sidx * kJacMaxOrder + m];
+            const auto& nn = jneg[(size_t)sidx * kJacMaxOrder + m];
+            if (pp.empty() && nn.empty()) continue;
+            gent.insert(gent.end(), pp.begin(), pp.end());
+            while (gent.size() % 4) gent.push_back(jzero);
+            const size_t first_neg = gent.size();
+            gent.insert(gent.end(), nn.begin(), nn.end());
+            while (gent.size() % 4) gent.push_back(jzero);
+            for (size_t g = first_neg; g < gent.size(); g += 4) gent[g] |= kGatherNeg;
+            gent[gent.size() - 4] |= kGatherLast;
+            gptr.push_back((uint32_t)(m * K + sidx) * row_bytes);
+          }
+        }
+        if ((gent.size() / 4 - jac_range[3 * wv]) % 2) gent.insert(gent.end(), 4, jzero);
+        jac_range[3 * wv + 1] = (uint16_t)(gent.size() / 4);
+        gent.insert(gent.end(), 16, jzero);
+      }
+      gptr.push_back(0);
+    } else if (!ws_sp_of) {
       for (int s = 0; s < K; ++s) {
         gptr[2 * s] = (uint32_t)gent.size();
         add_group(pos[s]);
@@ -254,6 +339,10 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
     hdr.rec_base = (uint32_t)out.rec_base[c];
     for (int wv = 0; wv < kMaxWarps; ++wv)
       for (int cl = 0; cl < kClsLong + 2; ++cl) hdr.wb[wv][cl] = (uint16_t)chunk_wb[c][(size_t)wv * (kClsLong + 2) + cl];
+    if (jb)
+      for (int wv = 0; wv < kJacWarps; ++wv)
+        for (int t = 0; t < 3; ++t) hdr.wb[kJacWarps + wv][t] = jac_range[3 * wv + t];
+    if (jb) jb->rows_max = std::max(jb->rows_max, (int)jrows);
     if (ws_sp_of)
       for (int hw = 0; hw < kWsHelpWarps; ++hw) {
         hdr.wb[kWsRxWarps + hw][0] = ws_range[2 * hw];
@@ -553,6 +642,115 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     }
   }
 
+  // ---- fused Jacobian kernel (psr_jac.cu).  It takes mechanisms whose every rate is k(T, C_tot) x a product of at most
+  // 3 + 3 concentrations, x [M] for three-body reactions: no falloff reaction with an efficiency list (its k changes
+  // with the composition), no long factor lists, no sign records.  Anything else keeps the generic sweep.
+  BlobSet jbs;
+  JacView jv{};
+  bool jac_ok = false;
+  std::vector<JacInc> jinc;
+  std::vector<int32_t> jinc_ptr, jcol_order;
+  std::vector<uint32_t> jinc_row;
+  {
+    bool elig = K <= 64;
+    int n_cls = 1;
+    for (int k = 0; k < I && elig; ++k) {
+      const HostRx& h = rx[k];
+      if (h.special_sign || h.nr > kSlots || h.np > kSlots || h.nr < 1) elig = false;
+      if (d->reversible[k] && h.np < 1) elig = false;
+      if (h.type >= 2 && !h.eff.empty()) elig = false;
+      n_cls = std::max(n_cls, std::max(h.nr, std::max(h.np, 1)) + (h.type == PSR_RX_THREE_BODY ? 1 : 0));
+    }
+    if (n_cls > kJacMaxOrder) elig = false;
+    if (elig) {
+      const int spw_j = (K + kJacWarps - 1) / kJacWarps;
+      const std::vector<int32_t> jsp = assign_species(rx, K, I, kJacWarps, spw_j);
+      const int Kp = (K + 1) & ~1;
+      for (int n_parts = 1; n_parts <= kWsMaxParts && n_parts <= I && !jac_ok; ++n_parts) {
+        JacBuild jb;
+        jb.sp_of = &jsp;
+        jb.spw = spw_j;
+        jb.row_of.assign(I, 0);
+        build_blobs(rx, K, I, n_parts, kJacWarps, 0.0, jbs, nullptr, 0, &jb);   // first pass: rows of the rate tile
+        jb.rows_zero = jb.rows_max;
+        build_blobs(rx, K, I, n_parts, kJacWarps, 0.0, jbs, nullptr, 0, &jb);
+        size_t o = 0;
+        jv.smem_cs = (uint32_t)o;
+        o += align_up((size_t)(K + 2) * kTile * 8, 128);
+        jv.smem_d = (uint32_t)o;
+        o += align_up((size_t)n_cls * K * kTile * 8, 128);
+        jv.smem_ar = (uint32_t)o;   // phase 1: rate tile (+ zero row) and the F(T + h_T) tile; phase 2: one [K][32] tile per warp
+        o += align_up(std::max((size_t)kJacWarps * (K + 1), (size_t)jb.rows_max + 1 + K) * kTile * 8, 128);
+        jv.smem_mech = (uint32_t)o;
+        o += jbs.stride;            // one part at a time
+        jv.smem_misc = (uint32_t)o;
+        o += align_up((size_t)2 * Kp * 8 + (size_t)kJacStRows * kTile * 8 + 4 * 8, 128);
+        jv.smem_total = (uint32_t)o;
+        if (o <= (size_t)prop.sharedMemPerBlockOptin) {
+          jac_ok = true;
+          jv.K = K;
+          jv.I = I;
+          jv.n_parts = n_parts;
+          jv.n_cls = n_cls;
+          jv.rows_max = jb.rows_max;
+          jv.need_lnctot = need_lnctot;
+          jv.chunk_stride = (uint32_t)jbs.stride;
+          // incidence records, species after species
+          const uint32_t unit_off = (uint32_t)K * kRowBytes, zero_c_off = (uint32_t)(K + 1) * kRowBytes;
+          jinc_ptr.assign(K + 1, 0);
+          for (int j = 0; j < K; ++j) {
+            jinc_ptr[j] = (int32_t)jinc.size();
+            for (int k = 0; k < I; ++k) {
+              const HostRx& h = rx[k];
+              int af = 0, ar = 0;
+              for (int t = 0; t < h.nr; ++t) af += h.factors[t] == j;
+              for (int t = 0; t < h.np; ++t) ar += h.factors[h.nr + t] == j;
+              double am1 = 0.0;
+              if (h.type == PSR_RX_THREE_BODY)
+                for (const EffEnt& ee : h.eff)
+                  if ((int)ee.off == j) am1 += ee.am1;   // (EffEnt::off holds the species index in the host records)
+              if (af == 0 && ar == 0 && am1 == 0.0) continue;
+              JacInc ic{};
+              for (int t = 0; t < kSlots; ++t) {
+                ic.off[t] = t < h.nr ? (uint32_t)h.factors[t] * kRowBytes : unit_off;
+                ic.off[kSlots + t] = t < h.np ? (uint32_t)h.factors[h.nr + t] * kRowBytes : unit_off;
+              }
+              if (!d->reversible[k]) ic.off[kSlots] = zero_c_off;
+              ic.row = (uint32_t)jb.row_of[k];
+              ic.tb = h.type == PSR_RX_THREE_BODY;
+              ic.nf = (uint8_t)h.nr;
+              ic.nr = (uint8_t)std::max(h.np, 1);
+              ic.af = (uint8_t)af;
+              ic.ar = (uint8_t)(d->reversible[k] ? ar : 0);
+              ic.am1 = am1;
+              int n_sc = 0;
+              for (auto& pr : h.nu_net)
+                if (pr.second != 0 && n_sc < 6) {
+                  ic.sc[n_sc].row_off = (uint32_t)pr.first * kRowBytes;
+                  ic.sc[n_sc].nu = (float)pr.second;
+                  ++n_sc;
+                }
+              ic.n_sc = (uint8_t)n_sc;
+              for (int t = n_sc; t < 6; ++t) {
+                ic.sc[t].row_off = (uint32_t)K * kRowBytes;   // a scratch row of the warp's tile
+                ic.sc[t].nu = 0.0f;
+              }
+              jinc.push_back(ic);
+            }
+          }
+          jinc_ptr[K] = (int32_t)jinc.size();
+          for (const JacInc& ic : jinc) jinc_row.push_back(ic.row);
+          jinc_row.push_back(0);
+          jinc_row.push_back(0);
+          jcol_order.resize(K);
+          std::iota(jcol_order.begin(), jcol_order.end(), 0);
+          std::stable_sort(jcol_order.begin(), jcol_order.end(),
+                           [&](int x, int y) { return jinc_ptr[x + 1] - jinc_ptr[x] > jinc_ptr[y + 1] - jinc_ptr[y]; });
+        }
+      }
+    }
+  }
+
   psr_mech* m = new (std::nothrow) psr_mech();
   if (!m) return fail(PSR_ENOMEM, "psr_mech_load: host allocation failed");
   m->device = dev;
@@ -645,6 +843,37 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     cleanup();
     return fail(PSR_ECUDA, "kernel does not fit on this device (%s)", cudaGetErrorString(e));
   }
+  if (jac_ok) {
+    const size_t scratch_bytes = (size_t)prop.multiProcessorCount * I * 3 * kTile * 8;
+    jinc.push_back(JacInc{});   // (read ahead by the kernel, never used)
+    jinc.push_back(JacInc{});
+    if ((e = cudaMalloc(&m->d_jac_chunks, jbs.all.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_jac_chunks, jbs.all.data(), jbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_jac_inc, sizeof(JacInc) * jinc.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_jac_inc, jinc.data(), sizeof(JacInc) * jinc.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_jac_inc_ptr, 4 * jinc_ptr.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_jac_inc_ptr, jinc_ptr.data(), 4 * jinc_ptr.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_jac_inc_row, 4 * jinc_row.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_jac_inc_row, jinc_row.data(), 4 * jinc_row.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_jac_col_order, 4 * jcol_order.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_jac_col_order, jcol_order.data(), 4 * jcol_order.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_jac_scratch, scratch_bytes)) != cudaSuccess ||
+        (e = jac_set_smem((size_t)prop.sharedMemPerBlockOptin)) != cudaSuccess) {
+      cleanup();
+      return cuda_fail(e, "Jacobian kernel tables");
+    }
+    jv.chunks = m->d_jac_chunks;
+    jv.inc = m->d_jac_inc;
+    jv.inc_ptr = m->d_jac_inc_ptr;
+    jv.inc_row = m->d_jac_inc_row;
+    jv.col_order = m->d_jac_col_order;
+    jv.scratch = m->d_jac_scratch;
+    jv.invW = m->d_invW;
+    jv.Wm = m->d_W;
+    jv.exp_tab = m->d_exptab;
+    m->jac = jv;
+    m->jac_ok = true;
+  }
   if (ws_ok) {
     if ((e = cudaMalloc(&m->d_ws_chunks, wbs.all.size())) != cudaSuccess ||
         (e = cudaMemcpy(m->d_ws_chunks, wbs.all.data(), wbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
@@ -679,6 +908,12 @@ void psr_mech_free(psr_mech* m) {
   for (void* q : m->retired) cudaFree(q);
   cudaFree(m->d_ws_chunks);
   cudaFree(m->d_ws_sp_of);
+  cudaFree(m->d_jac_chunks);
+  cudaFree(m->d_jac_inc);
+  cudaFree(m->d_jac_inc_ptr);
+  cudaFree(m->d_jac_inc_row);
+  cudaFree(m->d_jac_col_order);
+  cudaFree(m->d_jac_scratch);
   delete m;
 }
 
@@ -820,6 +1055,17 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
   if (!Yin || !tau || !J) return fail(PSR_EINVAL, "%s: null Yin, tau or J", fn);
   const uint32_t en = Tin ? kOutFT : 0u;
   psr_mech* m = const_cast<psr_mech*>(mc);
+  if (m->jac_ok && !Tin && !m->opt_jac_generic) {
+    // the fused kernel: base residual, T column and the K species columns of every reactor in one launch, no
+    // mechanism-owned scratch that depends on N
+    EvalArgs a{};
+    a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.J = J; a.F0out = F0;
+    a.n_tiles = (N + kTile - 1) / kTile;
+    const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
+    cudaError_t e = launch_jac(m->jac, a, grid, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, fn);
+    return PSR_OK;
+  }
   const int64_t K = m->view.K, n = K + 1, I = m->view.I;
 
   const size_t row_bytes = (size_t)I * kRateVals * 8;
@@ -1022,6 +1268,7 @@ psr_status psr_mech_set_option(psr_mech* m, int32_t option, int32_t value) {
   switch (option) {
     case PSR_OPT_JAC_UNHOISTED: m->opt_jac_unhoisted = value != 0; return PSR_OK;
     case PSR_OPT_FUSED_ONLY: m->opt_fused_only = value != 0; return PSR_OK;
+    case PSR_OPT_JAC_GENERIC: m->opt_jac_generic = value != 0; return PSR_OK;
     default: return fail(PSR_EINVAL, "psr_mech_set_option: unknown option %d", (int)option);
   }
 }

@@ -127,6 +127,51 @@ struct WsView {
   uint32_t smem_cs, smem_ds, smem_q, smem_acc, smem_mech, smem_misc, smem_total;
 };
 
+// ---- fused finite-difference Jacobian kernel (psr_jac.cu): lane <-> reactor, one CTA per tile of 32 reactors.
+// Phase 1 evaluates the tile (at T + h_T, then at T) and sums the forward and reverse rates of every reaction
+// into per-species sums BY CONCENTRATION ORDER; phase 2 builds the K species columns from them, warp <-> column.
+constexpr int kJacWarps = 8;
+constexpr int kJacMaxOrder = 6;   // highest concentration order of a rate term the kernel takes (else: the generic sweep)
+constexpr int kJacStRows = 12;    // per-tile state rows (T, ln T, 1/T, rho, 1/rho, C_tot, ln C_tot, sum Y/W, 1/tau, h_T, ...)
+
+// Species j takes part in reaction k ("incidence"): what column j needs to correct the rate of reaction k beyond
+// the uniform scaling of all concentrations.
+struct __attribute__((aligned(16))) JacInc {   // 96 bytes
+  uint32_t off[6];   // the reaction's 3 + 3 factor slots: byte offsets of C-tile rows (unit row = unused, zero row =
+                     // reverse side of an irreversible reaction)
+  uint32_t row;      // scratch row of the reaction: k_f, k_r, E = [M] - C_tot of every reactor of the tile
+  uint8_t tb;        // 1: three-body reaction (q = [M] (...)); 0: rate constants do not change under a Y perturbation
+  uint8_t nf, nr;    // concentration orders of the forward / reverse rate (numbers of factors, >= 1)
+  uint8_t af;        // how many of the forward slots are species j
+  uint8_t ar;        // ... of the reverse slots
+  uint8_t n_sc;      // scatter entries in use
+  uint16_t pad;
+  uint32_t pad2;
+  double am1;        // three-body reaction with j in its efficiency list: alpha_kj - 1; else 0
+  struct {           // reaction k changes species i (unused entries: the scratch row K of the tile, nu = 0)
+    uint32_t row_off;  // byte offset of row i in a [K+1][32] tile
+    float nu;          // net stoichiometric coefficient nu_ik
+  } sc[6];
+};
+static_assert(sizeof(JacInc) == 96, "JacInc layout");
+
+struct JacView {
+  const unsigned char* chunks;   // n_parts blobs (records dealt to kJacWarps warps; gather streams by species and order)
+  const JacInc* inc;             // incidence records, species after species
+  const int32_t* inc_ptr;        // [K + 1]
+  const uint32_t* inc_row;       // [records + 2] scratch row of every record (read two records ahead)
+  const int32_t* col_order;      // [K] columns in descending order of their number of records
+  const double* invW;
+  const double* Wm;
+  const double* exp_tab;
+  double* scratch;               // [grid][I][3][32]: k_f, k_r, E of the tile a CTA works on
+  int32_t K, I, n_parts, n_cls;  // n_cls: highest concentration order present
+  int32_t rows_max;              // rows of the rate tile of a part (+1 zero row)
+  int32_t need_lnctot;
+  uint32_t chunk_stride;
+  uint32_t smem_cs, smem_d, smem_ar, smem_mech, smem_misc, smem_total;
+};
+
 // what one launch produces
 enum : uint32_t {
   kOutWdot = 1u, kOutQ = 2u, kOutKf = 4u, kOutKr = 8u, kOutF = 16u, kOutF0 = 64u,

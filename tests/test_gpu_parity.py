@@ -449,31 +449,42 @@ def test_fd_jacobian_floor_criterion(torch_cuda, binding, cfg, n):
     mech, batch = synth.make_config(cfg, n)
     gm = binding.Mechanism.from_synth(mech)
     args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
+    # psr_fd_jacobian takes the fused kernel (psr_jac.cu) where the mechanism qualifies (C4, C0) and the generic
+    # three-launch sweep elsewhere (K > 64: C2, P5); the generic sweep is also run on every case
     J, F0 = gm.fd_jacobian(*args, want_F0=True)
-    J2 = gm.fd_jacobian(*args)  # internal F0 scratch path
-    # diagnostic sweep in which every column is a full evaluation: the production sweep takes the T-only
+    J2 = gm.fd_jacobian(*args)  # without the F0 output
+    gm.set_option(binding.OPT_JAC_GENERIC, 1)
+    Jg, F0g = gm.fd_jacobian(*args, want_F0=True)
+    # diagnostic sweep in which every column is a full evaluation: the generic sweep takes the T-only
     # factors of the Y columns from the base state's rate table and must give the same bits
     gm.set_option(binding.OPT_JAC_UNHOISTED, 1)
     J3 = gm.fd_jacobian(*args)
     gm.set_option(binding.OPT_JAC_UNHOISTED, 0)
+    gm.set_option(binding.OPT_JAC_GENERIC, 0)
     torch.cuda.synchronize()
-    J, F0, J2, J3 = J.cpu().numpy(), F0.cpu().numpy(), J2.cpu().numpy(), J3.cpu().numpy()
+    J, F0, J2, J3, Jg, F0g = (x.cpu().numpy() for x in (J, F0, J2, J3, Jg, F0g))
     gm.close()
     assert np.array_equal(J, J2)
-    assert np.array_equal(J, J3)
+    assert np.array_equal(Jg, J3)
     om = oracle_mech(mech)
     jl = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=True)
     jd = orc.jacobian(om, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, long_double=False)
-    # (1) binding criterion against the long-double reference
-    worst, fr_T, fr_Y = jacobian_floor_ratio(J, jl["J"], jl["S"], jl["H"])
-    assert worst <= 1.0, (worst, fr_T, fr_Y)
-    # (2) the GPU is no noisier than 4x an independent FP64 CPU code
     _, od_T, od_Y = jacobian_floor_ratio(jd["J"], jl["J"], jl["S"], jl["H"])
-    assert fr_T <= 4 * max(od_T, 1.0) and fr_Y <= 4 * max(od_Y, 1.0), (fr_T, od_T, fr_Y, od_Y)
-    # row 0 is e_0 exactly; base residual parity at 1e-9
-    assert np.all(J[:, 0, 0] == 1.0) and np.all(J[:, 1:, 0] == 0.0)
-    assert np.all(F0[:, 0] == 0.0)
-    assert residual_rel_err(F0[:, 1:].T, jd["F0"][:, 1:].T).max() <= TOL_F
+    for Jx, F0x in ((J, F0), (Jg, F0g)):
+        # (1) binding criterion against the long-double reference
+        worst, fr_T, fr_Y = jacobian_floor_ratio(Jx, jl["J"], jl["S"], jl["H"])
+        assert worst <= 1.0, (worst, fr_T, fr_Y)
+        # (2) the GPU is no noisier than 4x an independent FP64 CPU code
+        assert fr_T <= 4 * max(od_T, 1.0) and fr_Y <= 4 * max(od_Y, 1.0), (fr_T, od_T, fr_Y, od_Y)
+        # row 0 is e_0 exactly; base residual parity at 1e-9
+        assert np.all(Jx[:, 0, 0] == 1.0) and np.all(Jx[:, 1:, 0] == 0.0)
+        assert np.all(F0x[:, 0] == 0.0)
+        assert residual_rel_err(F0x[:, 1:].T, jd["F0"][:, 1:].T).max() <= TOL_F
+    if cfg in ("C4", "C0"):
+        # the fused kernel forms the species columns without evaluating F twice: their round-off is far below the
+        # forward-difference floor of any FP64 sweep (the oracle's included)
+        _, _, fy = jacobian_floor_ratio(J, jl["J"], jl["S"], jl["H"])
+        assert not np.array_equal(J, Jg) and fy <= 0.25 * max(od_Y, 1.0), (fy, od_Y)
 
 
 # ------------------------------------------------------------------ energy row (NEXT-1)
@@ -540,7 +551,9 @@ def test_fd_jacobian_energy_floor_criterion(torch_cuda, binding, cfg, n):
     args = [dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau)]
     dTin = dev(torch, Tin)
     J, F0 = gm.fd_jacobian(*args, want_F0=True, Tin=dTin)
+    gm.set_option(binding.OPT_JAC_GENERIC, 1)    # the species rows are those of the generic sweep of psr_fd_jacobian
     Jp = gm.fd_jacobian(*args)
+    gm.set_option(binding.OPT_JAC_GENERIC, 0)
     gm.set_option(binding.OPT_JAC_UNHOISTED, 1)
     J3 = gm.fd_jacobian(*args, Tin=dTin)
     gm.set_option(binding.OPT_JAC_UNHOISTED, 0)
@@ -723,8 +736,12 @@ def test_pseudo_transient_iteration_on_device_reduces_the_residual(torch_cuda, b
 SOLVE_KW = dict(atol=1e-12, rtol=1e-7, max_iter=260, max_newton=5, max_ptc=20, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9)
 
 
-def _solve_both(torch, binding, mech, T0, P, Y0, Yin, tau, Tin=None, workspace_reactors=None, **kw):
+def _solve_both(torch, binding, mech, T0, P, Y0, Yin, tau, Tin=None, workspace_reactors=None, generic=True, **kw):
+    """generic=True: the device loop builds its Jacobians with the generic forward-difference sweep, as the oracle
+    does (paths are compared like with like); False: with the fused Jacobian kernel where it applies (its species
+    columns carry no forward-difference round-off, so its Newton iteration contracts at least as fast)."""
     gm = binding.Mechanism.from_synth(mech)
+    gm.set_option(binding.OPT_JAC_GENERIC, 1 if generic else 0)
     T, Y = dev(torch, T0), dev(torch, Y0)
     ws = None
     if workspace_reactors is not None:
@@ -781,6 +798,21 @@ def test_solve_hybrid_matches_the_oracle_loop_on_C0(torch_cuda, binding):
     got2, _ = _solve_both(torch_cuda, binding, mech, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, workspace_reactors=77, **SOLVE_KW)
     for k in got:
         assert np.array_equal(got[k], got2[k]), k      # sub-batching does not change a reactor's path
+    _fused_path_check(torch_cuda, binding, mech, batch, ref, SOLVE_KW)
+
+
+def _fused_path_check(torch, binding, mech, batch, ref, kw):
+    """The default device path (fused Jacobian kernel): the same solutions, and no more Newton iterations on average
+    than the forward-difference paths need."""
+    got, _ = _solve_both(torch, binding, mech, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, generic=False, **kw)
+    conv = (got["status"] == 0) & (ref["status"] == 0)
+    assert (got["status"] == 0).mean() >= (ref["status"] == 0).mean() - 0.06
+    w = kw["atol"] + kw["rtol"] * np.abs(ref["Y"])
+    d = (np.abs(got["Y"] - ref["Y"]) / w).max(axis=0)
+    # (both stop on the size of their last Newton correction; with different Jacobians the estimates they stop at
+    # differ by a multiple of the tolerance that grows with the conditioning of the system)
+    assert (d[conv] <= 100.0).mean() >= 0.97 and np.median(d[conv]) <= 1.0
+    assert got["n_newton"][conv].mean() <= ref["n_newton"][conv].mean() + 0.5
 
 
 def test_solve_hybrid_paths_that_are_unique(torch_cuda, binding):
@@ -831,6 +863,7 @@ def test_solve_hybrid_on_C4_from_far_and_from_perturbed_converged_states(torch_c
     got, ref = _solve_both(torch, binding, mech, batch.T, batch.P, batch.Y, batch.Yin, batch.tau, **kw0)
     assert (ref["n_ptc"] > 0).all() and (ref["status"] == 0).mean() > 0.9
     _compare_solves(mech, got, ref, batch.P, batch.Yin, batch.tau, kw0)
+    _fused_path_check(torch, binding, mech, batch, ref, kw0)
     conv = ref["status"] == 0
     rng = np.random.default_rng(17)
     Y1 = ref["Y"][:, conv] * (1.0 + 0.01 * rng.uniform(-1, 1, (mech.n_species, conv.sum())))
@@ -886,13 +919,16 @@ def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, 
     F, w = torch.empty_like(Y), torch.empty_like(Y)
     J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
     side = torch.cuda.Stream()
-    # the Jacobian sweep's scratch belongs to the mechanism: without a reservation the call refuses to allocate
-    # inside a capture (psr.h) instead of invalidating it
+    # the generic Jacobian sweep's scratch belongs to the mechanism: without a reservation the call refuses to
+    # allocate inside a capture (psr.h) instead of invalidating it.  (The fused Jacobian kernel this mechanism
+    # normally takes needs no such scratch; the graph below captures both.)
+    Jgen = torch.empty_like(J)
+    gm.set_option(binding.OPT_JAC_GENERIC, 1)
     probe = torch.cuda.CUDAGraph()
     with torch.cuda.stream(side):
         with torch.cuda.graph(probe, stream=side):
             with pytest.raises(binding.PsrError) as ei:
-                gm.fd_jacobian(T, P, Y, Yin, tau, J=J)
+                gm.fd_jacobian(T, P, Y, Yin, tau, J=Jgen)
             assert ei.value.status == binding.PSR_EINVAL and "psr_mech_reserve" in str(ei.value)
     del probe
     gm.reserve(batch.n)                                # sizes the scratch buffer outside the capture
@@ -901,26 +937,32 @@ def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, 
     with torch.cuda.stream(side):
         with torch.cuda.graph(graph, stream=side):
             gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w)
+            gm.fd_jacobian(T, P, Y, Yin, tau, J=Jgen)
+            gm.set_option(binding.OPT_JAC_GENERIC, 0)
             gm.fd_jacobian(T, P, Y, Yin, tau, J=J)
+            gm.set_option(binding.OPT_JAC_GENERIC, 1)
     # a later, larger eager call outgrows the scratch: the captured graph keeps pointing at the buffer it was
     # captured with, which stays allocated until the mechanism is freed
     _, big = synth.make_config("C4", 6000)
     gm.fd_jacobian(*(dev(torch, x) for x in (big.T, big.P, big.Y, big.Yin, big.tau)))
+    gm.set_option(binding.OPT_JAC_GENERIC, 0)
     torch.cuda.synchronize()
     # new state in the same buffers, replay, compare with direct calls on the default stream
     _, b2 = synth.make_config("C4", 200)
     for dst, src in ((T, b2.T), (P, b2.P), (Y, b2.Y), (Yin, b2.Yin), (tau, b2.tau)):
         dst.copy_(dev(torch, src))
-    F.zero_(); w.zero_(); J.zero_()
+    F.zero_(); w.zero_(); J.zero_(); Jgen.zero_()
     torch.cuda.synchronize()
     graph.replay()
     torch.cuda.synchronize()
-    F_g, w_g, J_g = F.clone(), w.clone(), J.clone()
+    F_g, w_g, J_g, Jgen_g = F.clone(), w.clone(), J.clone(), Jgen.clone()
     F_d, w_d = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
     J_d = gm.fd_jacobian(T, P, Y, Yin, tau)
+    gm.set_option(binding.OPT_JAC_GENERIC, 1)
+    Jgen_d = gm.fd_jacobian(T, P, Y, Yin, tau)
     torch.cuda.synchronize()
     gm.close()
-    assert torch.equal(F_g, F_d) and torch.equal(w_g, w_d) and torch.equal(J_g, J_d)
+    assert torch.equal(F_g, F_d) and torch.equal(w_g, w_d) and torch.equal(J_g, J_d) and torch.equal(Jgen_g, Jgen_d)
     ref = orc.evaluate(oracle_mech(mech), b2.T, b2.P, b2.Y, b2.Yin, b2.tau, want=("wdot", "F"))
     assert residual_rel_err(F_g.cpu().numpy(), ref["F"]).max() <= TOL_F
 
