@@ -680,11 +680,13 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         jv.smem_d = (uint32_t)o;
         o += align_up((size_t)n_cls * K * kTile * 8, 128);
         jv.smem_ar = (uint32_t)o;   // phase 1: rate tile (+ zero row) and the F(T + h_T) tile; phase 2: one [K][32] tile per warp
-        o += align_up(std::max((size_t)kJacWarps * (K + 1), (size_t)jb.rows_max + 1 + K) * kTile * 8, 128);
+        o += align_up(std::max((size_t)kJacWarps * (K + 1) * kJacAccLd, ((size_t)jb.rows_max + 1 + K) * kTile) * 8, 128);
         jv.smem_mech = (uint32_t)o;
         o += jbs.stride;            // one part at a time
         jv.smem_misc = (uint32_t)o;
-        o += align_up((size_t)2 * Kp * 8 + (size_t)kJacStRows * kTile * 8 + 4 * 8, 128);
+        o += align_up((size_t)2 * Kp * 8 + (size_t)kJacStRows * kTile * 8 + (2 + 2 * kJacWarps) * 8, 128);
+        jv.smem_stage = (uint32_t)o;   // per warp: two chunks of kJacStage incidence records
+        o += (size_t)kJacWarps * 2 * kJacStage * sizeof(JacInc);
         jv.smem_total = (uint32_t)o;
         if (o <= (size_t)prop.sharedMemPerBlockOptin) {
           jac_ok = true;
@@ -726,13 +728,13 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
               int n_sc = 0;
               for (auto& pr : h.nu_net)
                 if (pr.second != 0 && n_sc < 6) {
-                  ic.sc[n_sc].row_off = (uint32_t)pr.first * kRowBytes;
+                  ic.sc[n_sc].row_off = (uint32_t)pr.first * (kJacAccLd * 8);
                   ic.sc[n_sc].nu = (float)pr.second;
                   ++n_sc;
                 }
               ic.n_sc = (uint8_t)n_sc;
               for (int t = n_sc; t < 6; ++t) {
-                ic.sc[t].row_off = (uint32_t)K * kRowBytes;   // a scratch row of the warp's tile
+                ic.sc[t].row_off = (uint32_t)K * (kJacAccLd * 8);   // a scratch row of the warp's tile
                 ic.sc[t].nu = 0.0f;
               }
               jinc.push_back(ic);

@@ -56,12 +56,15 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
   double* St = W_s + Kp;                                            // [kJacStRows][32]
   uint64_t* bar = reinterpret_cast<uint64_t*>(St + kJacStRows * kTile);
   int* col_next = reinterpret_cast<int*>(bar + 1);                   // phase 2: the next column to hand out
+  uint64_t* wbar = bar + 2 + 2 * (threadIdx.x >> 5);                 // this warp's two staging barriers
+  unsigned char* stage = smem + jv.smem_stage + (threadIdx.x >> 5) * (2 * kJacStage * sizeof(JacInc));
   double* Fp = AR + (size_t)(jv.rows_max + 1) * kTile;              // F(T + h_T) of the tile
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nthr = kJacWarps * 32;
 
   if (threadIdx.x == 0) {
     mbar_init(bar, 1);
+    for (int q = 0; q < 2 * kJacWarps; ++q) mbar_init(bar + 2 + q, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   for (int i = threadIdx.x; i < K; i += nthr) {
@@ -82,6 +85,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
   const uint32_t r_lane = smem_u32(AR) + lane * 8;
   const uint32_t d_lane = smem_u32(Dt) + lane * 8;
   uint32_t n_loads = 0;   // blob loads this CTA has waited for (mbarrier phase)
+  uint32_t n_iss = 0, n_use = 0;   // staging chunks this warp has requested / consumed
 
   for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
     const int64_t r = tile * kTile + lane;
@@ -232,7 +236,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
 
     // ================================================================ phase 2: the species columns, warp <-> column
     // (columns in descending order of their number of records, handed out through a shared counter)
-    double* acc_t = AR + (size_t)w * (K + 1) * kTile;   // this warp's [K+1][32] tile (row K: unused scatter slots)
+    double* acc_t = AR + (size_t)w * (K + 1) * kJacAccLd;   // this warp's [K+1][33] tile (row K: unused scatter slots)
     const uint32_t acc_lane = smem_u32(acc_t) + lane * 8;
     const double ctot = St[JS_CTOT * kTile + lane];
     for (;;) {
@@ -265,92 +269,138 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
         for (int e = 2; e <= kJacMaxOrder; ++e) v = q == e ? sp[e] : v;
         return v;
       };
-      // the first records of the column are requested before the polynomial part is formed
+      // The incidence records of the column (contiguous in global memory, L2-resident) come through this warp's
+      // staging ring in shared memory: chunks of kJacStage records by bulk copies, two in flight; the first two
+      // are requested before the polynomial part is formed.
       const int e0 = __ldg(jv.inc_ptr + j), e1 = __ldg(jv.inc_ptr + j + 1);
-      uint4 B[6];
-      uint32_t row_b = __ldg(jv.inc_row + e0), row_c = __ldg(jv.inc_row + e0 + 1);
-      {
-        const uint4* ic = reinterpret_cast<const uint4*>(jv.inc + e0);
-#pragma unroll
-        for (int q = 0; q < 6; ++q) B[q] = __ldg(ic + q);
-      }
-      double kf_b, kr_b, E_b;
-      {
-        const double* sr = scr + (size_t)row_b * 3 * kTile;
-        kf_b = sr[0];
-        kr_b = sr[kTile];
-        E_b = sr[2 * kTile];
-      }
+      const int n_chunks = (e1 - e0 + kJacStage - 1) / kJacStage;
+      int ci = 0;   // chunks of this column requested so far
+      auto issue = [&]() {
+        if (ci < n_chunks) {
+          const int first = e0 + ci * kJacStage;
+          const uint32_t bytes = (uint32_t)min(kJacStage, e1 - first) * (uint32_t)sizeof(JacInc);
+          const uint32_t b = n_iss & 1;
+          if (lane == 0) {
+            fence_proxy_async();
+            mbar_expect_tx(&wbar[b], bytes);
+            bulk_g2s(stage + b * kJacStage * sizeof(JacInc), jv.inc + first, bytes, &wbar[b]);
+          }
+          ++n_iss;
+          ++ci;
+        }
+      };
+      issue();
+      issue();
       // polynomial part: sum_n (s^(n-1) - 1) D_i^(n)
       for (int i = 0; i < K; ++i) {
         double v = 0.0;
 #pragma unroll
         for (int c = 1; c < kJacMaxOrder; ++c)
           if (c < n_cls) v = fma(u[c], Dt[(c * K + i) * kTile + lane], v);
-        acc_t[i * kTile + lane] = v;
+        acc_t[i * kJacAccLd + lane] = v;
       }
-      // the reactions species j takes part in: record e is worked on while record e + 1 and its rate constants are
-      // on their way (the tables sit in L2), the scratch row of record e + 2 is known
+      // the reactions species j takes part in
       const double cj = Cs[j * kTile + lane], cjp = cj + dc;
       const uint32_t off_j = (uint32_t)j * kRowBytes;
-#pragma unroll 1
-      for (int e = e0; e < e1; ++e) {
-        uint4 A[6];
-#pragma unroll
-        for (int q = 0; q < 6; ++q) A[q] = B[q];
-        const double kf = kf_b, kr = kr_b, E = E_b;
+      auto ld4 = [&](uint32_t addr, uint4& o) {
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w) : "r"(addr));
+      };
+      auto ld_row = [&](uint32_t rec_addr) {
+        uint32_t row;
+        asm volatile("ld.shared.u32 %0, [%1+24];" : "=r"(row) : "r"(rec_addr));
+        return row;
+      };
+      for (int c = 0; c < n_chunks; ++c) {
+        const uint32_t b = n_use & 1;
+        mbar_wait(&wbar[b], (n_use >> 1) & 1);
+        ++n_use;
+        const int cnt = min(kJacStage, e1 - (e0 + c * kJacStage));
+        const uint32_t sb = smem_u32(stage + b * kJacStage * sizeof(JacInc));
+        // k_f, k_r, E of a record's reaction (this tile's scratch, L2) are requested two records ahead
+        double kf_b, kr_b, E_b, kf_c = 0.0, kr_c = 0.0, E_c = 0.0;
         {
-          const uint4* ic = reinterpret_cast<const uint4*>(jv.inc + e + 1);
-#pragma unroll
-          for (int q = 0; q < 6; ++q) B[q] = __ldg(ic + q);
-          const double* sr = scr + (size_t)row_c * 3 * kTile;
+          const double* sr = scr + (size_t)ld_row(sb) * 3 * kTile;
           kf_b = sr[0];
           kr_b = sr[kTile];
           E_b = sr[2 * kTile];
-          row_c = __ldg(jv.inc_row + e + 2);
+          if (cnt > 1) {
+            const double* sr2 = scr + (size_t)ld_row(sb + (uint32_t)sizeof(JacInc)) * 3 * kTile;
+            kf_c = sr2[0];
+            kr_c = sr2[kTile];
+            E_c = sr2[2 * kTile];
+          }
         }
-        const uint32_t meta = A[1].w;
-        const int tb = meta & 0xff, nf = (meta >> 8) & 0xff, nr = (meta >> 16) & 0xff, af = meta >> 24;
-        const int ar = A[2].x & 0xff;
-        const double am1 = __hiloint2double((int)A[2].w, (int)A[2].z);
-        auto other = [&](uint32_t off) { return off == off_j ? 1.0 : lds64(cx.c_lane + off); };
-        // (C + dc)^a - C^a, a = 0..3, without cancellation
-        auto grow = [&](int aa) {
-          return aa == 0 ? 0.0 : aa == 1 ? dc : aa == 2 ? dc * (cj + cjp) : dc * fma(cj, cj, fma(cj, cjp, cjp * cjp));
-        };
-        // the targets of the record's scatter are read now, added to below
-        const uint32_t t0 = acc_lane + A[3].x, t1 = acc_lane + A[3].z, t2 = acc_lane + A[4].x, t3 = acc_lane + A[4].z,
-                       t4 = acc_lane + A[5].x, t5 = acc_lane + A[5].z;
-        const double v0 = lds64(t0), v1 = lds64(t1), v2 = lds64(t2), v3 = lds64(t3), v4 = lds64(t4), v5 = lds64(t5);
-        const double Pof = other(A[0].x) * other(A[0].y) * other(A[0].z), Por = other(A[0].w) * other(A[1].x) * other(A[1].y);
-        const double dPf = Pof * grow(af), dPr = Por * grow(ar);
-        const double kfs = kf * pw(nf), krs = kr * pw(nr);
-        double dq = fma(kfs, dPf, -(krs * dPr));
-        if (tb) {
-          // [M]' = C_tot + s (E + (alpha_kj - 1) dc); the uniform-scaling part (C_tot + s E)(...) is in D
-          auto power = [&](int aa) { return aa == 0 ? 1.0 : aa == 1 ? cj : aa == 2 ? cj * cj : cj * cj * cj; };
-          const double Pf1 = fma(Pof, power(af), dPf), Pr1 = fma(Por, power(ar), dPr);   // perturbed products (unscaled)
-          dq = fma(fma(s, E, ctot), dq, (s * am1 * dc) * fma(kfs, Pf1, -(krs * Pr1)));
+#pragma unroll 1
+        for (int t = 0; t < cnt; ++t) {
+          const uint32_t ra = sb + (uint32_t)t * (uint32_t)sizeof(JacInc);
+          uint4 A[6];
+#pragma unroll
+          for (int q = 0; q < 6; ++q) ld4(ra + 16 * q, A[q]);
+          const double kf = kf_b, kr = kr_b, E = E_b;
+          kf_b = kf_c;
+          kr_b = kr_c;
+          E_b = E_c;
+          if (t + 2 < cnt) {
+            const double* sr = scr + (size_t)ld_row(ra + 2 * (uint32_t)sizeof(JacInc)) * 3 * kTile;
+            kf_c = sr[0];
+            kr_c = sr[kTile];
+            E_c = sr[2 * kTile];
+          }
+          const uint32_t meta = A[1].w;
+          const int tb = meta & 0xff, nf = (meta >> 8) & 0xff, nr = (meta >> 16) & 0xff, af = meta >> 24;
+          const int ar = A[2].x & 0xff;
+          const double am1 = __hiloint2double((int)A[2].w, (int)A[2].z);
+          auto other = [&](uint32_t off) { return off == off_j ? 1.0 : lds64(cx.c_lane + off); };
+          // (C + dc)^a - C^a, a = 0..3, without cancellation
+          auto grow = [&](int aa) {
+            return aa == 0 ? 0.0 : aa == 1 ? dc : aa == 2 ? dc * (cj + cjp) : dc * fma(cj, cj, fma(cj, cjp, cjp * cjp));
+          };
+          // the targets of the record's scatter are read now, added to below
+          const uint32_t t0 = acc_lane + A[3].x, t1 = acc_lane + A[3].z, t2 = acc_lane + A[4].x, t3 = acc_lane + A[4].z,
+                         t4 = acc_lane + A[5].x, t5 = acc_lane + A[5].z;
+          const double v0 = lds64(t0), v1 = lds64(t1), v2 = lds64(t2), v3 = lds64(t3), v4 = lds64(t4), v5 = lds64(t5);
+          const double Pof = other(A[0].x) * other(A[0].y) * other(A[0].z), Por = other(A[0].w) * other(A[1].x) * other(A[1].y);
+          const double dPf = Pof * grow(af), dPr = Por * grow(ar);
+          const double kfs = kf * pw(nf), krs = kr * pw(nr);
+          double dq = fma(kfs, dPf, -(krs * dPr));
+          if (tb) {
+            // [M]' = C_tot + s (E + (alpha_kj - 1) dc); the uniform-scaling part (C_tot + s E)(...) is in D
+            auto power = [&](int aa) { return aa == 0 ? 1.0 : aa == 1 ? cj : aa == 2 ? cj * cj : cj * cj * cj; };
+            const double Pf1 = fma(Pof, power(af), dPf), Pr1 = fma(Por, power(ar), dPr);   // perturbed products (unscaled)
+            dq = fma(fma(s, E, ctot), dq, (s * am1 * dc) * fma(kfs, Pf1, -(krs * Pr1)));
+          }
+          dq *= inv_s;
+          // (the six targets of a record are distinct species, or the unused row with nu = 0)
+          sts64(t0, fma((double)__uint_as_float(A[3].y), dq, v0));
+          sts64(t1, fma((double)__uint_as_float(A[3].w), dq, v1));
+          sts64(t2, fma((double)__uint_as_float(A[4].y), dq, v2));
+          sts64(t3, fma((double)__uint_as_float(A[4].w), dq, v3));
+          sts64(t4, fma((double)__uint_as_float(A[5].y), dq, v4));
+          sts64(t5, fma((double)__uint_as_float(A[5].w), dq, v5));
         }
-        dq *= inv_s;
-        // (the six targets of a record are distinct species, or the unused row with nu = 0)
-        sts64(t0, fma((double)__uint_as_float(A[3].y), dq, v0));
-        sts64(t1, fma((double)__uint_as_float(A[3].w), dq, v1));
-        sts64(t2, fma((double)__uint_as_float(A[4].y), dq, v2));
-        sts64(t3, fma((double)__uint_as_float(A[4].w), dq, v3));
-        sts64(t4, fma((double)__uint_as_float(A[5].y), dq, v4));
-        sts64(t5, fma((double)__uint_as_float(A[5].w), dq, v5));
+        __syncwarp();   // every lane has read the chunk: its buffer takes the chunk after next
+        issue();
       }
-      // the quotient: J_ij = (delta_ij h/tau - (W_i/rho)(wdot_i'/s - wdot_i)) / h
-      if (valid) {
-        double* Jc = a.J + ((r * n) + 1 + j) * n;
+      // the quotient: J_ij = (delta_ij h/tau - (W_i/rho)(wdot_i'/s - wdot_i)) / h, formed in place; then the warp
+      // writes the column of one reactor after the other (n contiguous doubles each: lanes over the rows; the
+      // tile's row stride of 33 keeps both access directions free of bank conflicts)
+      {
         const double invh = 1.0 / h;
-        Jc[0] = 0.0;   // row 0: F_T = T - T_set does not depend on Y
         for (int i = 0; i < K; ++i) {
-          const double d = -(W_s[i] * invrho) * acc_t[i * kTile + lane];
-          Jc[1 + i] = (i == j ? fma(h, invtau, d) : d) * invh;
+          const double d = -(W_s[i] * invrho) * acc_t[i * kJacAccLd + lane];
+          acc_t[i * kJacAccLd + lane] = (i == j ? fma(h, invtau, d) : d) * invh;
         }
       }
+      __syncwarp();
+      {
+        const int n_valid = (int)min((int64_t)kTile, a.N - tile * kTile);
+        double* Jc = a.J + ((tile * kTile * n) + 1 + j) * n;   // column 1 + j of the tile's first reactor
+        for (int l = 0; l < n_valid; ++l, Jc += (int64_t)n * n) {
+          for (int e = lane; e < n; e += 32)
+            Jc[e] = e == 0 ? 0.0 : acc_t[(e - 1) * kJacAccLd + l];   // row 0: F_T = T - T_set does not depend on Y
+        }
+      }
+      __syncwarp();
     }
     __syncthreads();   // the next tile's phase 1 reuses every tile
   }

@@ -132,7 +132,9 @@ struct WsView {
 // into per-species sums BY CONCENTRATION ORDER; phase 2 builds the K species columns from them, warp <-> column.
 constexpr int kJacWarps = 8;
 constexpr int kJacMaxOrder = 6;   // highest concentration order of a rate term the kernel takes (else: the generic sweep)
-constexpr int kJacStRows = 12;    // per-tile state rows (T, ln T, 1/T, rho, 1/rho, C_tot, ln C_tot, sum Y/W, 1/tau, h_T, ...)
+constexpr int kJacAccLd = 33;     // row stride (doubles) of a warp's phase-2 tile: conflict-free by rows and by columns
+constexpr int kJacStage = 8;       // incidence records per staging chunk of a warp (two chunks in flight)
+constexpr int kJacStRows = 4;     // per-tile state rows (T, ln T, 1/T, rho, 1/rho, C_tot, ln C_tot, sum Y/W, 1/tau, h_T, ...)
 
 // Species j takes part in reaction k ("incidence"): what column j needs to correct the rate of reaction k beyond
 // the uniform scaling of all concentrations.
@@ -149,7 +151,7 @@ struct __attribute__((aligned(16))) JacInc {   // 96 bytes
   uint32_t pad2;
   double am1;        // three-body reaction with j in its efficiency list: alpha_kj - 1; else 0
   struct {           // reaction k changes species i (unused entries: the scratch row K of the tile, nu = 0)
-    uint32_t row_off;  // byte offset of row i in a [K+1][32] tile
+    uint32_t row_off;  // byte offset of row i in a [K+1][kJacAccLd] tile
     float nu;          // net stoichiometric coefficient nu_ik
   } sc[6];
 };
@@ -169,7 +171,7 @@ struct JacView {
   int32_t rows_max;              // rows of the rate tile of a part (+1 zero row)
   int32_t need_lnctot;
   uint32_t chunk_stride;
-  uint32_t smem_cs, smem_d, smem_ar, smem_mech, smem_misc, smem_total;
+  uint32_t smem_cs, smem_d, smem_ar, smem_mech, smem_misc, smem_stage, smem_total;
 };
 
 // what one launch produces
