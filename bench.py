@@ -41,9 +41,18 @@ WORKLOAD = "C1: 53 species / 325 reactions (28 three-body, 29 Troe), 65536 react
 EXP_INSTR, LOG_INSTR, DIV_INSTR = 22.0, 28.0, 10.0
 N_SM, FP64_LANES_PER_SM = 148, 64     # B200: 64 FP64 FMA lanes per SM (37 TFLOP/s nominal)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of psr_eval_kernel<16,4,1> on C1, from the
-# ncu --set full capture summarised in profiles/.
-NCU_DRAM_BYTES_PER_LAUNCH = 73.6e6   # 59.3 MB read + 14.3 MB written (profiles/r1d_psr_eval_kernel_C1.md)
+# FP64 instructions of one FD Jacobian of the C1 mechanism with the T-only factors hoisted (the naive
+# count is 55 full evaluations)
+C4_HOISTED_INSTR_PER_JACOBIAN = 410e3
+
+
+def ncu_summary(key: str) -> dict:
+    """Numbers that only a profiler sees (DRAM bytes per launch, FP64-pipe utilisation), read from the committed
+    summary of the ncu --set full captures under profiles/ -- never measured under the profiler in this run."""
+    try:
+        return json.loads((ROOT / "profiles" / "ncu_summary.json").read_text()).get(key, {})
+    except Exception:
+        return {}
 
 
 def algorithmic_fp64_instr(K, I, n_tb, n_troe, nnz):
@@ -233,13 +242,15 @@ def run_ours(args):
     blocks = []
     for c in range(E2E_CHUNKS):
         c0, c1 = bounds[c], bounds[c + 1]
-        hin = [pin(batch.T[c0:c1]), pin(batch.P[c0:c1]), pin(batch.Y[:, c0:c1]), pin(batch.Yin[:, c0:c1]), pin(batch.tau[c0:c1])]
-        hout = [torch.empty((K, c1 - c0), dtype=torch.float64).pin_memory() for _ in range(2)]
-        din = [torch.empty_like(x, device="cuda") for x in hin]
-        dout = [torch.empty((K, c1 - c0), dtype=torch.float64, device="cuda") for _ in range(2)]
+        # one pinned array per direction and block: rows T, P, tau, Y[0..K), Yin[0..K) in; wdot[0..K), F[0..K) out
+        hin = pin(np.concatenate([batch.T[None, c0:c1], batch.P[None, c0:c1], batch.tau[None, c0:c1],
+                                  batch.Y[:, c0:c1], batch.Yin[:, c0:c1]], axis=0))
+        hout = torch.empty((2 * K, c1 - c0), dtype=torch.float64).pin_memory()
+        din = torch.empty_like(hin, device="cuda")
+        dout = torch.empty((2 * K, c1 - c0), dtype=torch.float64, device="cuda")
         blocks.append((hin, hout, din, dout))
-    h2d = sum(x.numel() * 8 for b in blocks for x in b[0])
-    d2h = sum(x.numel() * 8 for b in blocks for x in b[1])
+    h2d = sum(b[0].numel() * 8 for b in blocks)
+    d2h = sum(b[1].numel() * 8 for b in blocks)
     side = [torch.cuda.Stream() for _ in range(3)]
 
     def e2e_step():
@@ -249,11 +260,9 @@ def run_ours(args):
             st = side[c % len(side)]
             st.wait_event(start)
             with torch.cuda.stream(st):
-                for hx, dx in zip(hin, din):
-                    dx.copy_(hx, non_blocking=True)
-                gm.eval_residual(din[0], din[1], din[2], din[3], din[4], F=dout[1], wdot=dout[0])
-                hout[0].copy_(dout[0], non_blocking=True)
-                hout[1].copy_(dout[1], non_blocking=True)
+                din.copy_(hin, non_blocking=True)
+                gm.eval_residual(din[0], din[1], din[3:3 + K], din[3 + K:3 + 2 * K], din[2], F=dout[K:], wdot=dout[:K])
+                hout.copy_(dout, non_blocking=True)
         for st in side:
             done = torch.cuda.Event()
             done.record(st)
@@ -273,9 +282,10 @@ def run_ours(args):
     clocks = sampler.stop()
     e2e_ms = shard.max_over_ranks(e2e_ms, device="cuda")
     e2e_value = shard.whole_job_rate(N, e2e_steps, e2e_ms, world)
-    assert all(bool(torch.isfinite(b[1][0]).all()) for b in blocks)
+    assert all(bool(torch.isfinite(b[1]).all()) for b in blocks)
     # the blocks together are the device-resident result
-    assert torch.equal(torch.cat([b[1][0] for b in blocks], dim=1), wdot.cpu())
+    assert torch.equal(torch.cat([b[1][:K] for b in blocks], dim=1), wdot.cpu())
+    assert torch.equal(torch.cat([b[1][K:] for b in blocks], dim=1), F.cpu())
 
     # ---- roofline of the dominant (only) kernel: FP64 ALU pipe
     instr_per_eval = algorithmic_fp64_instr(K, I, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
@@ -286,10 +296,14 @@ def run_ours(args):
         for kind, name in ((0, "dfma"), (1, "exp"), (2, "log")):
             ms, ops = binding.probe_fp64(kind, 2000 if kind == 0 else 500)
             probes[name + "_per_s"] = ops / (ms * 1e-3)
-    hbm_bytes = (2 + 2 * K) * 8 * N + 2 * K * 8 * N    # T,P,tau~,Y,Yin in ; wdot,F out (tau counted in the 2)
+    hbm_bytes = (3 + 4 * K) * 8 * N    # T, P, tau, Y, Yin in; wdot, F out
+    prof = ncu_summary("C1_residual")
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "T FP64 thread-instr/s",
-        "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+        "frac": achieved / peak, "traffic": prof.get("dram_bytes_per_launch"),
+        "frac_is": "algorithmic FP64 instruction count of the METHOD with library exp/log/div costs (SURVEY.md 8(d)) / time / peak; "
+                   "the kernel executes fewer FP64 instructions than that (log-linear rate forms, table exp): see fp64_pipe_util_ncu",
+        "fp64_pipe_util_ncu": prof.get("fp64_pipe_pct"), "ncu_capture": prof.get("capture"),
         "peak_source": "derived: 148 SM x 64 FP64 lanes x clocks.max.sm (DESIGN.md); measured DFMA probe in 'probes'",
         "instr_per_eval": instr_per_eval, "probes": probes,
         "hbm": {"algorithmic_bytes_per_launch": hbm_bytes,
@@ -299,7 +313,7 @@ def run_ours(args):
     # ---- extras (rank 0, one GPU): other §8(a) rows timed once each, not part of `value`
     extra = {}
     if rank == 0 and not args.no_extra:
-        extra = run_extras(binding, synth, torch, flush)
+        extra = run_extras(binding, synth, torch, flush, cpu=not args.no_cpu)
 
     # ---- cpu baseline: the oracle as it stands on the host cores, bounded sample (rank 0, N=1)
     cpu = None
@@ -328,7 +342,7 @@ def run_ours(args):
                        "reaction_evals_per_s": value * I, "kernel": info},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps, "pipeline": f"{E2E_CHUNKS} blocks of reactors on 3 streams (copy-in, kernel, copy-out overlapped)"},
+                    "steps": e2e_steps, "pipeline": f"{E2E_CHUNKS} blocks of reactors on 3 streams (one copy in, kernel, one copy out per block, overlapped)"},
             "gpu_launches": args.steps,
             "roofline": roofline, "cpu_baseline": cpu, "extra": extra,
         }
@@ -364,53 +378,137 @@ def _time_call(torch, fn, flush, reps=5):
     return tot / reps
 
 
-def run_extras(binding, synth, torch, flush):
-    """C2, C3 residual passes, the C4 FD-Jacobian and the C1 adiabatic residual, timed once each (mean of
-    5, L2 flushed)."""
+PEAK_INSTR = N_SM * FP64_LANES_PER_SM * 1.965e9    # FP64 thread-instructions/s at clocks.max.sm
+
+
+def _oracle_rates(mech, batch, n_sample, jacobian=False):
+    """The oracle as it stands on a bounded sample (SURVEY.md 8(d) "Oracle timing"): single thread and all host
+    cores, best of 2.  Rates in reactor evaluations (or Jacobians) per second."""
+    from oracle import oracle as orc
+    om = _oracle_mech(mech)
+    sub = batch.take(np.arange(min(n_sample, batch.n)))
+    cores = min(orc.max_threads(), orc.host_cores())
+    out = {"sample": f"first {sub.n} reactors", "cores": cores}
+    for name, nt in (("per_s_1_thread", 1), ("per_s_all_cores", cores)):
+        one = sub if nt > 1 else sub.take(np.arange(max(1, sub.n // 8)))
+        best = float("inf")
+        for _ in range(2):
+            t0 = time.perf_counter()
+            if jacobian:
+                orc.jacobian(om, one.T, one.P, one.Y, one.Yin, one.tau, nthreads=nt)
+            else:
+                orc.evaluate(om, one.T, one.P, one.Y, one.Yin, one.tau, want=("wdot", "F"), nthreads=nt)
+            best = min(best, time.perf_counter() - t0)
+        out[name] = one.n / best
+    return out
+
+
+def run_extras(binding, synth, torch, flush, only=None, cpu=True):
+    """The other rows of SURVEY.md 8(a)/(f), each timed on its own (mean of 5 launches, L2 flushed): psr_eval_wdot and
+    the adiabatic residual on C1, the C2 / C3 residual passes, the C4 FD Jacobian (plain and adiabatic), the Newton
+    step's solve, a Newton iteration, and the hybrid solver; beside them the oracle on bounded samples.
+    only: run just that leg (ncu captures name it)."""
     out = {}
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
-    # NEXT-1: the adiabatic residual (species rows + energy row) on the headline workload
-    mech, batch = synth.make_config("C1")
-    gm = binding.Mechanism.from_synth(mech)
-    T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
-    Tin = torch.full_like(T, 300.0)
-    F, FT = torch.empty_like(Y), torch.empty_like(T)
-    ms = _time_call(torch, lambda: gm.eval_residual_energy(T, P, Y, Tin, Yin, tau, F=F, FT=FT), flush)
-    out["C1_energy"] = {"call": "psr_eval_residual_energy", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3)}
-    gm.close()
-    for cfg in ("C2", "C3", "C4"):
+    want = lambda k: only is None or only == k
+    if want("C1_wdot") or want("C1_energy"):
+        mech, batch = synth.make_config("C1")
+        gm = binding.Mechanism.from_synth(mech)
+        T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+        info = gm.info()
+        instr = algorithmic_fp64_instr(mech.n_species, mech.n_reactions, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
+        if want("C1_wdot"):   # the metric is wdot evaluations: the call that produces nothing else
+            w = torch.empty_like(Y)
+            ms = _time_call(torch, lambda: gm.eval_wdot(T, P, Y, wdot=w), flush)
+            out["C1_wdot"] = {"call": "psr_eval_wdot", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3),
+                              "alu_frac": instr * batch.n / (ms * 1e-3) / PEAK_INSTR}
+        if want("C1_energy"):   # NEXT-1: the adiabatic residual (species rows + energy row)
+            Tin = torch.full_like(T, 300.0)
+            F, FT = torch.empty_like(Y), torch.empty_like(T)
+            ms = _time_call(torch, lambda: gm.eval_residual_energy(T, P, Y, Tin, Yin, tau, F=F, FT=FT), flush)
+            out["C1_energy"] = {"call": "psr_eval_residual_energy", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3)}
+        gm.close()
+    for cfg in ("C2", "C3"):
+        if not want(cfg):
+            continue
         mech, batch = synth.make_config(cfg)
         gm = binding.Mechanism.from_synth(mech)
         info = gm.info()
         T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
         instr = algorithmic_fp64_instr(mech.n_species, mech.n_reactions, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
-        if cfg == "C4":
-            n = mech.n_species + 1
-            J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
+        F, w = torch.empty_like(Y), torch.empty_like(Y)
+        ms = _time_call(torch, lambda: gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w), flush)
+        out[cfg] = {"call": "psr_eval_residual", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3),
+                    "reaction_evals_per_s": batch.n * mech.n_reactions / (ms * 1e-3),
+                    "alu_frac": instr * batch.n / (ms * 1e-3) / PEAK_INSTR}
+        if cpu:
+            out[cfg]["cpu_oracle"] = _oracle_rates(mech, batch, 2048)
+        gm.close()
+    if any(want(k) for k in ("C4", "C4_energy", "C4_solve", "C4_newton", "C4_hybrid")):
+        mech, batch = synth.make_config("C4")
+        gm = binding.Mechanism.from_synth(mech)
+        info = gm.info()
+        T, P, Y, Yin, tau = (dev(x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+        instr = algorithmic_fp64_instr(mech.n_species, mech.n_reactions, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
+        n = mech.n_species + 1
+        J = torch.empty((batch.n, n, n), dtype=torch.float64, device="cuda")
+        F0 = torch.empty((batch.n, n), dtype=torch.float64, device="cuda")
+        if want("C4"):
             ms = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J), flush)
+            prof = ncu_summary("C4_jacobian")
+            out["C4"] = {"call": "psr_fd_jacobian (fused kernel)", "ms": ms, "jacobians_per_s": batch.n / (ms * 1e-3),
+                         "residual_evals_per_s": batch.n * (n + 1) / (ms * 1e-3),
+                         # BASELINE's unit (55 full evaluations per Jacobian) and SURVEY 8(d)'s hoisted count; the fused
+                         # kernel does less work than either (DESIGN.md 5.5), so these compare times, not pipe use
+                         "alu_frac_unhoisted": instr * batch.n * (n + 1) / (ms * 1e-3) / PEAK_INSTR,
+                         "alu_frac_hoisted": C4_HOISTED_INSTR_PER_JACOBIAN * batch.n / (ms * 1e-3) / PEAK_INSTR,
+                         "hbm_GBps_on_J": batch.n * n * n * 8 / (ms * 1e-3) / 1e9,
+                         "fp64_pipe_util_ncu": prof.get("fp64_pipe_pct"), "ncu_capture": prof.get("capture")}
+            gm.set_option(binding.OPT_JAC_GENERIC, 1)
+            ms_g = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J), flush)
+            gm.set_option(binding.OPT_JAC_GENERIC, 0)
+            out["C4"]["generic_sweep_ms"] = ms_g
+            if cpu:
+                out["C4"]["cpu_oracle"] = _oracle_rates(mech, batch, 256, jacobian=True)
+        if want("C4_energy"):
             Tin = torch.full_like(T, 300.0)
             ms_en = _time_call(torch, lambda: gm.fd_jacobian(T, P, Y, Yin, tau, J=J, Tin=Tin), flush)
-            out["C4_energy"] = {"call": "psr_fd_jacobian_energy", "ms": ms_en, "jacobians_per_s": batch.n / (ms_en * 1e-3)}
-            # NEXT-2: the Newton step's solve J dx = -F0 on the Jacobians just computed
-            J0, F0 = gm.fd_jacobian(T, P, Y, Yin, tau, want_F0=True)
-            rhs0, rhs = (-F0).contiguous(), torch.empty_like(F0)
-            def solve():
-                rhs.copy_(rhs0)
-                binding.lu_solve(J0, rhs)
-            ms_lu = _time_call(torch, solve, flush)
-            out["C4_solve"] = {"call": "psr_lu_solve (+ 3.5 MB rhs copy)", "ms": ms_lu, "systems_per_s": batch.n / (ms_lu * 1e-3),
+            out["C4_energy"] = {"call": "psr_fd_jacobian_energy (generic sweep)", "ms": ms_en, "jacobians_per_s": batch.n / (ms_en * 1e-3)}
+        if want("C4_solve") or want("C4_newton"):
+            gm.fd_jacobian(T, P, Y, Yin, tau, J=J, F0=F0)
+            rhs = torch.empty_like(F0)
+            dt_inf = torch.full((batch.n,), float("inf"), dtype=torch.float64, device="cuda")
+            info_t = torch.empty(batch.n, dtype=torch.int32, device="cuda")
+            # NEXT-2: the Newton step's solve J dx = -F0 (psr_ptc_solve with dt = inf reads F0 and negates it itself)
+            ms_lu = _time_call(torch, lambda: binding.ptc_solve(J, F0, dt_inf, dx=rhs, info=info_t), flush)
+            out["C4_solve"] = {"call": "psr_ptc_solve (dt = inf: the Newton step)", "ms": ms_lu, "systems_per_s": batch.n / (ms_lu * 1e-3),
                                "n": n, "hbm_GBps_on_J": batch.n * n * n * 8 / (ms_lu * 1e-3) / 1e9}
-            del J0
-            out[cfg] = {"call": "psr_fd_jacobian", "ms": ms, "jacobians_per_s": batch.n / (ms * 1e-3),
-                        "residual_evals_per_s": batch.n * (n + 1) / (ms * 1e-3),
-                        "alu_frac_unhoisted": instr * batch.n * (n + 1) / (ms * 1e-3) / (N_SM * FP64_LANES_PER_SM * 1.965e9)}
-            del J
-        else:
-            F, w = torch.empty_like(Y), torch.empty_like(Y)
-            ms = _time_call(torch, lambda: gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w), flush)
-            out[cfg] = {"call": "psr_eval_residual", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3),
-                        "reaction_evals_per_s": batch.n * mech.n_reactions / (ms * 1e-3),
-                        "alu_frac": instr * batch.n / (ms * 1e-3) / (N_SM * FP64_LANES_PER_SM * 1.965e9)}
+            def newton():
+                gm.fd_jacobian(T, P, Y, Yin, tau, J=J, F0=F0)
+                binding.ptc_solve(J, F0, dt_inf, dx=rhs, info=info_t)
+            ms_n = _time_call(torch, newton, flush)
+            out["C4_newton"] = {"call": "psr_fd_jacobian + psr_ptc_solve (one Newton iteration's device work)", "ms": ms_n,
+                                "iterations_per_s": batch.n / (ms_n * 1e-3)}
+        if want("C4_hybrid"):
+            # NEXT-4: the whole hybrid solve from the generated (far) states, 2,048 reactors, fixed budget of 420 solves
+            nb = 2048
+            a0 = [x[..., :nb].contiguous() for x in (T, P, Y, Yin, tau)]
+            kw = dict(atol=1e-12, rtol=1e-7, max_iter=420, max_newton=5, max_ptc=20, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9)
+            ws = torch.empty(int(binding.lib().psr_solve_hybrid_workspace_bytes(gm._h, nb)), dtype=torch.uint8, device="cuda")
+            def hybrid():
+                Tt, Yt = a0[0].clone(), a0[2].clone()
+                return gm.solve_hybrid(Tt, a0[1], Yt, a0[3], a0[4], workspace=ws, **kw)
+            st, nn, npt = hybrid()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(torch.cuda.current_stream())
+            st, nn, npt = hybrid()
+            e1.record(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            ms_h = e0.elapsed_time(e1)
+            out["C4_hybrid"] = {"call": "psr_solve_hybrid", "reactors": nb, "options": kw, "ms": ms_h,
+                                "converged_frac": float((st == 0).float().mean()), "mean_newton": float(nn.float().mean()),
+                                "mean_ptc": float(npt.float().mean()), "ms_per_solve_round": ms_h / kw["max_iter"]}
         gm.close()
     return out
 
@@ -495,8 +593,16 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-extra", action="store_true", help="skip the C2/C3/C4 extras")
     ap.add_argument("--sweep", action="store_true", help="paper-shaped batch sweep (NEXT-3) instead of the headline line")
+    ap.add_argument("--only", default=None, help="run just one leg of `extra` (C1_wdot, C1_energy, C2, C3, C4, C4_energy, "
+                                                 "C4_solve, C4_newton, C4_hybrid) and print it: what the ncu captures under profiles/ run")
     args = ap.parse_args()
-    if args.sweep:
+    if args.only:
+        import torch
+        from paper_2005_11468_b200 import binding, synth
+        torch.cuda.set_device(0)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        print(json.dumps(run_extras(binding, synth, torch, flush, only=args.only, cpu=False)), flush=True)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)
