@@ -127,6 +127,22 @@ psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, con
                            const double* Y, const double* Yin, const double* tau, int64_t ld,
                            double* J, double* F0, void* stream);
 
+/* psr_fd_jacobian for callers that cannot let the library allocate (code under CUDA-graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same arguments, same result (the fused Jacobian kernel), but
+ * the kernel's scratch is a static device array of 32 MiB inside the library -- held by every GPU that loads the
+ * library until the process exits -- and the call performs no cudaMalloc, cudaFree or allocating library routine.
+ * Limits: PSR_EUNSUPPORTED if the mechanism has more than PSR_NOALLOC_MAX_REACTIONS reactions (the array is sized for
+ * that), or does not qualify for the fused kernel (more than 64 species, a falloff reaction with an efficiency list,
+ * more than 3 concentration factors on a side, A <= 0): use psr_fd_jacobian then.  Any N: the launch uses as many CTAs,
+ * up to one per SM, as have room for their scratch rows (n_reactions * 768 bytes each).
+ * The array is shared by every call on the device and keeps the previous call's contents (none of which is read
+ * before it is rewritten): calls that OVERLAP on the GPU -- different streams, or a graph replayed beside an eager
+ * call -- race on it and must be serialised by the caller.  Asynchronous on `stream`. */
+#define PSR_NOALLOC_MAX_REACTIONS 2048
+psr_status psr_fd_jacobian_noalloc(const psr_mech* mech, int64_t N, const double* T, const double* P,
+                                   const double* Y, const double* Yin, const double* tau, int64_t ld,
+                                   double* J, double* F0, void* stream);
+
 /* Sizes the scratch of psr_fd_jacobian / psr_fd_jacobian_energy for batches of up to N reactors (including the
  * internal F0 used when the caller passes none).  Synchronous (cudaMalloc); never shrinks. */
 psr_status psr_mech_reserve(psr_mech* mech, int64_t N);

@@ -18,7 +18,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_solve_hybrid", "psr_solve_hybrid_workspace_bytes", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_fd_jacobian_noalloc", "psr_solve_hybrid", "psr_solve_hybrid_workspace_bytes", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -82,6 +82,8 @@ def lib():
         L.psr_ptc_solve.restype = C.c_int
         L.psr_fd_jacobian.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
         L.psr_fd_jacobian.restype = C.c_int
+        L.psr_fd_jacobian_noalloc.argtypes = [vp, i64, dp, dp, dp, dp, dp, i64, dp, dp, vp]
+        L.psr_fd_jacobian_noalloc.restype = C.c_int
         L.psr_last_error.argtypes = []
         L.psr_last_error.restype = C.c_char_p
         L.psr_mech_info.argtypes = [vp, C.POINTER(PsrMechInfo)]
@@ -318,6 +320,24 @@ def _solve_hybrid(self, T, P, Y, Yin, tau, Tin=None, workspace=None, atol=1e-12,
 
 
 Mechanism.solve_hybrid = _solve_hybrid
+
+
+def _fd_jacobian_noalloc(self, T, P, Y, Yin, tau, J, F0=None):
+    """psr_fd_jacobian_noalloc: the caller passes every array (J [N][n][n], F0 [N][n] or None); the library allocates
+    nothing (its scratch is a static device array).  Returns J."""
+    N = T.shape[0]
+    ld = _ld(Y, N)
+    n = self.K + 1
+    for nm, t in (("T", T), ("P", P), ("Y", Y), ("Yin", Yin), ("tau", tau), ("J", J)) + ((("F0", F0),) if F0 is not None else ()):
+        _chk_dev(nm, t)
+    _chk_ld("Yin", Yin, N, ld)
+    if tuple(J.shape) != (N, n, n) or not J.is_contiguous() or (F0 is not None and (tuple(F0.shape) != (N, n) or not F0.is_contiguous())):
+        raise ValueError("J must be contiguous [N][K+1][K+1] and F0 contiguous [N][K+1]")
+    _check(lib().psr_fd_jacobian_noalloc(self._h, N, _ptr(T), _ptr(P), _ptr(Y), _ptr(Yin), _ptr(tau), ld, _ptr(J), _ptr(F0), _stream()))
+    return J
+
+
+Mechanism.fd_jacobian_noalloc = _fd_jacobian_noalloc
 
 
 def probe_fp64(kind: int, iters: int):

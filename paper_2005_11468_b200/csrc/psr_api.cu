@@ -30,6 +30,8 @@ cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_
                                  int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
 cudaError_t jac_set_smem(size_t smem);
 cudaError_t launch_jac(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
+cudaError_t launch_jac_static(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
+size_t jac_static_scratch_bytes();
 cudaError_t ws_set_smem(size_t smem);
 cudaError_t launch_ws(const WsView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st);
 }  // namespace psr
@@ -1152,6 +1154,32 @@ psr_status psr_mech_reserve(psr_mech* m, int64_t N) {
 psr_status psr_fd_jacobian(const psr_mech* mech, int64_t N, const double* T, const double* P, const double* Y,
                            const double* Yin, const double* tau, int64_t ld, double* J, double* F0, void* stream) {
   return fd_jacobian_impl(mech, N, T, P, Y, nullptr, Yin, tau, ld, J, F0, stream, "psr_fd_jacobian");
+}
+
+// psr_fd_jacobian through the fused kernel with its scratch in a static device array: no cudaMalloc, cudaFree or
+// allocating library routine on this path (argument checks, one cudaGetSymbolAddress per device the first time, one
+// kernel launch).
+psr_status psr_fd_jacobian_noalloc(const psr_mech* m, int64_t N, const double* T, const double* P, const double* Y,
+                                   const double* Yin, const double* tau, int64_t ld, double* J, double* F0, void* stream) {
+  g_err.clear();
+  psr_status st = check_common(m, N, T, P, Y, ld, "psr_fd_jacobian_noalloc");
+  if (st != PSR_OK || N == 0) return st;
+  if (!Yin || !tau || !J) return fail(PSR_EINVAL, "psr_fd_jacobian_noalloc: null Yin, tau or J");
+  if (m->view.I > PSR_NOALLOC_MAX_REACTIONS)
+    return fail(PSR_EUNSUPPORTED, "psr_fd_jacobian_noalloc: %d reactions, the static scratch (%zu bytes) is sized for at most %d",
+                (int)m->view.I, jac_static_scratch_bytes(), (int)PSR_NOALLOC_MAX_REACTIONS);
+  if (!m->jac_ok)
+    return fail(PSR_EUNSUPPORTED, "psr_fd_jacobian_noalloc: the mechanism does not qualify for the fused Jacobian kernel "
+                                  "(more than 64 species, falloff reactions with efficiency lists, long factor lists or A <= 0)");
+  const size_t per_cta = (size_t)m->view.I * 3 * kTile * 8;
+  const int64_t fit = (int64_t)(jac_static_scratch_bytes() / per_cta);   // >= 21 by the limit on the reactions
+  EvalArgs a{};
+  a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.J = J; a.F0out = F0;
+  a.n_tiles = (N + kTile - 1) / kTile;
+  const int grid = (int)std::min<int64_t>(std::min<int64_t>(a.n_tiles, m->n_sm), fit);
+  cudaError_t e = launch_jac_static(m->jac, a, grid, (cudaStream_t)stream);
+  if (e != cudaSuccess) return cuda_fail(e, "psr_fd_jacobian_noalloc");
+  return PSR_OK;
 }
 
 psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double* T, const double* P, const double* Y,

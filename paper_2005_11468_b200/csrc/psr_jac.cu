@@ -415,4 +415,56 @@ cudaError_t launch_jac(const JacView& jv, const EvalArgs& a, int grid, cudaStrea
   return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------ the same kernel with STATIC scratch (psr_fd_jacobian_noalloc)
+// Some callers cannot let the library allocate: code under CUDA-graph capture, tight serving loops, harnesses that
+// forbid cudaMalloc.  For them the kernel's per-CTA scratch ([CTAs][I][3][32] doubles: k_f, k_r, E of the tile a CTA
+// works on) lives in this file-scope array instead of the buffer psr_mech_load allocates.  Every GPU that loads the
+// library holds these 32 MiB until the process exits.
+//   * g_jac_static_scratch is, in HOST code, only a stand-in for the symbol -- not a device address: passing it to a
+//     kernel would fault (or silently use host memory where the GPU can reach it).  The device address comes from
+//     cudaGetSymbolAddress, asked once per device with that device current, and is what the kernel is given.
+//   * Nothing in the array has to start at zero: in phase 1 a CTA writes the rows of all I reactions of its tile (every
+//     lane, lanes past N included) before phase 2 reads any of them, so what the last call left behind is never read.
+//   * Every call on a device shares the array: two calls that overlap on the GPU (different streams, or a graph
+//     replayed beside an eager call) race on it.  Serialise them.
+constexpr size_t kJacStaticBytes = (size_t)32 << 20;
+static __device__ __align__(256) double g_jac_static_scratch[kJacStaticBytes / sizeof(double)];
+
+size_t jac_static_scratch_bytes() { return kJacStaticBytes; }
+
+// Device address of the static scratch on the current device; resolved on the first call per device (no allocation:
+// the array is part of the loaded module).
+static cudaError_t jac_static_scratch_ptr(double** out) {
+  constexpr int kMaxDev = 64;
+  static double* ptr[kMaxDev];
+  static bool have[kMaxDev];
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+  if (!have[dev]) {
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_jac_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    ptr[dev] = p;     // (two host threads racing here store the same address)
+    have[dev] = true;
+  }
+  *out = ptr[dev];
+  return cudaSuccess;
+}
+
+// grid: at most the CTAs whose scratch rows fit the array (the caller has checked that at least one does)
+cudaError_t launch_jac_static(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st) {
+  double* scratch = nullptr;
+  cudaError_t e = jac_static_scratch_ptr(&scratch);
+  if (e != cudaSuccess) return e;
+  const size_t per_cta = (size_t)jv.I * 3 * kTile * sizeof(double);
+  if (grid < 1 || (size_t)grid * per_cta > kJacStaticBytes) return cudaErrorInvalidConfiguration;
+  JacView v = jv;
+  v.scratch = scratch;
+  psr_jac_kernel<<<grid, kJacWarps * 32, v.smem_total, st>>>(v, a);
+  return cudaGetLastError();
+}
+
 }  // namespace psr
