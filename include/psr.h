@@ -233,6 +233,15 @@ psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);
 enum { PSR_OPT_JAC_UNHOISTED = 1, PSR_OPT_FUSED_ONLY = 2, PSR_OPT_JAC_GENERIC = 3 };
 psr_status psr_mech_set_option(psr_mech* mech, int32_t option, int32_t value);
 
+/* Diagnostic of the bounds-checked build (libpsr_b200_check.so: the same sources with -DPSR_CHECK; DESIGN.md 6.7 --
+ * compute-sanitizer is refused on the GPU pool this library is developed on).  In that build the kernels assert, on
+ * the device, every shared-memory offset they take from the mechanism tables and every global output index against
+ * its bound.  Returns the number of failed assertions since the last call and resets it (*first_code, if not NULL:
+ * the code of the first one, see the PSR_CHK sites in csrc/); selftest != 0 first trips one assertion on purpose
+ * (code 999) so that a caller can tell "no failure" from "no checks".  Returns -1 in the product build, which carries
+ * no checks, and -2 on a CUDA error.  Synchronises the device. */
+int32_t psr_check_failures(int32_t selftest, int32_t* first_code);
+
 /* FP64 pipe probes used for the roofline denominator: run `iters` dependent-
  * chain iterations of (kind 0) DFMA, (kind 1) exp, (kind 2) log on every SM and return the device
  * time in milliseconds and the number of operations executed per thread-lane in total.

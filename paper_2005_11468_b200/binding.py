@@ -18,7 +18,7 @@ PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 
 EXPORTS = ("psr_mech_load", "psr_mech_free", "psr_eval_kf_kr", "psr_eval_wdot", "psr_eval_residual",
-           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_fd_jacobian_noalloc", "psr_solve_hybrid", "psr_solve_hybrid_workspace_bytes", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
+           "psr_eval_residual_energy", "psr_fd_jacobian", "psr_fd_jacobian_energy", "psr_lu_solve", "psr_ptc_solve", "psr_last_error", "psr_mech_info", "psr_mech_set_option", "psr_mech_reserve", "psr_fd_jacobian_noalloc", "psr_check_failures", "psr_solve_hybrid", "psr_solve_hybrid_workspace_bytes", "psr_probe_fp64", "psr_probe_exp_values", "psr_version")
 
 _DESC_ARRAYS = (("W", np.float64), ("nasa", np.float64), ("A", np.float64), ("b", np.float64), ("Ea", np.float64),
                 ("rtype", np.uint8), ("reversible", np.uint8), ("reac_ptr", np.int32), ("reac_sp", np.int32),
@@ -92,6 +92,8 @@ def lib():
         L.psr_solve_hybrid_workspace_bytes.restype = C.c_size_t
         L.psr_solve_hybrid.argtypes = [vp, i64, dp, dp, dp, dp, dp, dp, i64, C.POINTER(PsrSolveOpts), vp, C.c_size_t, dp, dp, dp, vp]
         L.psr_solve_hybrid.restype = C.c_int
+        L.psr_check_failures.argtypes = [C.c_int32, C.POINTER(C.c_int32)]
+        L.psr_check_failures.restype = C.c_int32
         L.psr_mech_reserve.argtypes = [vp, i64]
         L.psr_mech_reserve.restype = C.c_int
         L.psr_mech_set_option.argtypes = [vp, C.c_int32, C.c_int32]
@@ -338,6 +340,13 @@ def _fd_jacobian_noalloc(self, T, P, Y, Yin, tau, J, F0=None):
 
 
 Mechanism.fd_jacobian_noalloc = _fd_jacobian_noalloc
+
+
+def check_failures(selftest: bool = False):
+    """psr_check_failures: (count, first_code) of the bounds-checked build; count is -1 in the product build."""
+    code = C.c_int32(0)
+    n = lib().psr_check_failures(1 if selftest else 0, C.byref(code))
+    return int(n), int(code.value)
 
 
 def probe_fp64(kind: int, iters: int):

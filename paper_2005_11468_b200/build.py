@@ -22,26 +22,49 @@ NVCC_FLAGS = [
 ]
 
 
-def needs_build() -> bool:
-    if not LIB.exists():
+LIB_CHECK = PKG / "libpsr_b200_check.so"   # the same sources with -DPSR_CHECK (device-side bounds assertions; tests only)
+
+
+def _stale(lib: Path) -> bool:
+    if not lib.exists():
         return True
-    t = LIB.stat().st_mtime
+    t = lib.stat().st_mtime
     return any(p.stat().st_mtime > t for p in SOURCES + HEADERS)
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
+def needs_build() -> bool:
+    return _stale(LIB)
+
+
+def _cmd(lib: Path, extra):
+    return ["nvcc", *NVCC_FLAGS, *extra, "-o", str(lib), *[str(s) for s in SOURCES]]
+
+
+def _finish(proc, cmd, log_name: str):
+    out, err = proc.communicate()
+    log = (out or "") + (err or "")
+    (PKG / log_name).write_text(" ".join(cmd) + "\n" + log)
+    if proc.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + log[-4000:])
+    return log
+
+
+def build(force: bool = False, verbose: bool = False, check: bool = False) -> Path:
+    """Builds libpsr_b200.so; with check=True also the bounds-checked libpsr_b200_check.so (the two nvcc runs side by side)."""
+    jobs = []
     if force or needs_build():
-        cmd = ["nvcc", *NVCC_FLAGS, "-o", str(LIB), *[str(s) for s in SOURCES]]
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        log = res.stdout + res.stderr
-        (PKG / "build.log").write_text(" ".join(cmd) + "\n" + log)
-        if res.returncode != 0:
-            raise RuntimeError("nvcc failed:\n" + log[-4000:])
+        cmd = _cmd(LIB, [])
+        jobs.append((subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True), cmd, "build.log"))
+    if check and (force or _stale(LIB_CHECK)):
+        cmd = _cmd(LIB_CHECK, ["-DPSR_CHECK"])
+        jobs.append((subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True), cmd, "build_check.log"))
+    for proc, cmd, name in jobs:
+        log = _finish(proc, cmd, name)
         if verbose:
             print(log)
     return LIB
 
 
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose=True)
+    build(force="--force" in sys.argv, verbose=True, check="--check" in sys.argv)
     print(LIB)

@@ -28,6 +28,10 @@ cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_c
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
                                  const int32_t* info, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it, int32_t* status,
                                  int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
+cudaError_t chk_read_kernels(unsigned int* count, unsigned int* first_code);
+cudaError_t chk_read_ws(unsigned int* count, unsigned int* first_code);
+cudaError_t chk_read_jac(unsigned int* count, unsigned int* first_code);
+cudaError_t launch_chk_selftest(cudaStream_t st);
 cudaError_t jac_set_smem(size_t smem);
 cudaError_t launch_jac(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
 cudaError_t launch_jac_static(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
@@ -1301,6 +1305,31 @@ psr_status psr_mech_set_option(psr_mech* m, int32_t option, int32_t value) {
     case PSR_OPT_JAC_GENERIC: m->opt_jac_generic = value != 0; return PSR_OK;
     default: return fail(PSR_EINVAL, "psr_mech_set_option: unknown option %d", (int)option);
   }
+}
+
+int32_t psr_check_failures(int32_t selftest, int32_t* first_code) {
+  g_err.clear();
+  if (first_code) *first_code = 0;
+#ifndef PSR_CHECK
+  (void)selftest;
+  return -1;   // the product build carries no checks
+#else
+  if (selftest) {
+    cudaError_t e = launch_chk_selftest(0);
+    if (e != cudaSuccess) { cuda_fail(e, "psr_check_failures (self-test)"); return -2; }
+  }
+  unsigned int total = 0, first = 0;
+  cudaError_t (*readers[3])(unsigned int*, unsigned int*) = {chk_read_ws, chk_read_jac, chk_read_kernels};
+  for (auto rd : readers) {
+    unsigned int c = 0, code = 0;
+    cudaError_t e = rd(&c, &code);
+    if (e != cudaSuccess) { cuda_fail(e, "psr_check_failures"); return -2; }
+    if (c && !first) first = code;
+    total += c;
+  }
+  if (first_code) *first_code = (int32_t)first;
+  return (int32_t)std::min<unsigned int>(total, 0x7fffffffu);
+#endif
 }
 
 psr_status psr_probe_exp_values(const psr_mech* m, const double* x, double* y, int32_t n) {

@@ -81,6 +81,9 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
   cx.c_lane = smem_u32(Cs) + lane * 8;
   cx.ctot_lane = smem_u32(St + JS_CTOT * kTile) + lane * 8;
   cx.lnctot_lane = smem_u32(St + JS_LNCTOT * kTile) + lane * 8;
+#ifdef PSR_CHECK
+  cx.chk_c_bytes = (uint32_t)(K + 2) * kRowBytes;
+#endif
   double* scr = jv.scratch + (size_t)blockIdx.x * jv.I * 3 * kTile + lane;   // row v of reaction k: scr[(3 k + v) * 32]
   const uint32_t r_lane = smem_u32(AR) + lane * 8;
   const uint32_t d_lane = smem_u32(Dt) + lane * 8;
@@ -144,6 +147,8 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
         // rate-tile rows of a record (its first row and its scratch row ride in the record's korig field):
         //   k_f prod C^nu', k_r prod C^nu''; three-body q = (C_tot + E)(...): C_tot x and E x each of the two
         auto sink = [&](int kl, uint32_t meta, uint32_t korig, int type, double kf, double kr, double pf, double pr, double M) {
+          PSR_CHK((int)(korig & 0xffffu) + (type == RX_THREE_BODY ? 4 : 2) <= jv.rows_max, 301);   // rows of the rate tile
+          PSR_CHK((int)(korig >> 16) < jv.I, 302);                                                // row of the per-CTA scratch
           const uint32_t row = r_lane + (korig & 0xffffu) * (uint32_t)kRowBytes;
           const double Rf = kf * pf, Rr = kr * pr;
           double E = 0.0;
@@ -183,6 +188,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
             uint32_t off;
             asm volatile("ld.shared.u32 %0, [%1];" : "=r"(off) : "r"(dst));
             dst += 4;
+            PSR_CHK(off < (uint32_t)n_cls * (uint32_t)K * kRowBytes && off % kRowBytes == 0, 303);   // a row of the sums tile
             sts64(d_lane + off, lds64(d_lane + off) + acc);
             acc = 0.0;
           };
@@ -205,6 +211,11 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
             b0 = lds64(r_lane + (ob.x & ~3u)), b1 = lds64(r_lane + ob.y), b2 = lds64(r_lane + ob.z), b3 = lds64(r_lane + ob.w);
             ld_group(gs + (uint32_t)(i + 4) * 16u, oa);
             ld_group(gs + (uint32_t)(i + 5) * 16u, ob);
+            {
+              const uint32_t rmax = (uint32_t)(jv.rows_max + 1) * kRowBytes;   // rate tile rows, zero row included
+              PSR_CHK((oa.x & ~3u) < rmax && oa.y < rmax && oa.z < rmax && oa.w < rmax && (ob.x & ~3u) < rmax && ob.y < rmax &&
+                          ob.z < rmax && ob.w < rmax, 304);
+            }
             acc = fma(ta, sgn(c0), acc);
             if (c0 & kGatherLast) flush(acc);
             acc = fma(tb, sgn(c1), acc);
@@ -224,6 +235,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
           Fp[i * kTile + lane] = Fv;
         } else if (valid) {
           if (a.F0out) a.F0out[r * n + 1 + i] = Fv;
+          PSR_CHK((r * n) * n + 1 + i < a.N * (int64_t)n * n, 305);
           a.J[(r * n) * n + 1 + i] = (Fp[i * kTile + lane] - Fv) / hT;   // column 0: T perturbed
         }
       }
@@ -245,6 +257,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
       jn = __shfl_sync(kFullMask, jn, 0);
       if (jn >= K) break;
       const int j = __ldg(jv.col_order + jn);
+      PSR_CHK(j >= 0 && j < K, 306);
       const double yj = ldg_nc(a.Y + (int64_t)j * a.ld + rc);
       const double yp = yj + 1e-8 * fmax(fabs(yj), 1e-10);
       const double h = yp - yj;                    // h_j = fl(x' - x)
@@ -347,6 +360,12 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
             E_c = sr[2 * kTile];
           }
           const uint32_t meta = A[1].w;
+          {   // the record's factor rows (C tile), scatter rows (this warp's [K+1][33] tile) and scratch row
+            const uint32_t cmax = (uint32_t)(K + 2) * kRowBytes, tmax = (uint32_t)(K + 1) * (kJacAccLd * 8);
+            PSR_CHK(A[0].x < cmax && A[0].y < cmax && A[0].z < cmax && A[0].w < cmax && A[1].x < cmax && A[1].y < cmax, 307);
+            PSR_CHK(A[3].x < tmax && A[3].z < tmax && A[4].x < tmax && A[4].z < tmax && A[5].x < tmax && A[5].z < tmax, 308);
+            PSR_CHK((int)A[1].z < jv.I, 309);
+          }
           const int tb = meta & 0xff, nf = (meta >> 8) & 0xff, nr = (meta >> 16) & 0xff, af = meta >> 24;
           const int ar = A[2].x & 0xff;
           const double am1 = __hiloint2double((int)A[2].w, (int)A[2].z);
@@ -395,6 +414,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
       {
         const int n_valid = (int)min((int64_t)kTile, a.N - tile * kTile);
         double* Jc = a.J + ((tile * kTile * n) + 1 + j) * n;   // column 1 + j of the tile's first reactor
+        PSR_CHK(((tile * kTile + n_valid - 1) * n + 1 + j) * n + n <= a.N * (int64_t)n * n, 310);   // the last reactor's column ends inside J
         for (int l = 0; l < n_valid; ++l, Jc += (int64_t)n * n) {
           for (int e = lane; e < n; e += 32)
             Jc[e] = e == 0 ? 0.0 : acc_t[(e - 1) * kJacAccLd + l];   // row 0: F_T = T - T_set does not depend on Y
@@ -405,6 +425,8 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
     __syncthreads();   // the next tile's phase 1 reuses every tile
   }
 }
+
+PSR_CHK_TU_READER(chk_read_jac)
 
 cudaError_t jac_set_smem(size_t smem) {
   return cudaFuncSetAttribute(psr_jac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

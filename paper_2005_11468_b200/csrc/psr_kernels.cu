@@ -364,8 +364,13 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
       for (int i = 0; i < R; ++i) a1[i] = 0.0;
 #pragma unroll 1
+      PSR_CHK(s >= 0 && s < K && g0 <= g1 && g1 <= g2, 407);
       for (uint32_t e = g0; e < g1; ++e) {
         const uint4 o = gent[e];
+        {
+          const uint32_t qmax = (uint32_t)(mv.rc + 1) * (uint32_t)(TR * 8);   // rows of the q tile, zero row included
+          PSR_CHK(o.x < qmax && o.y < qmax && o.z < qmax && o.w < qmax, 408);
+        }
         double v0[R], v1[R], v2[R], v3[R];
         RowIO<R>::ld(q_lane + o.x, v0);
         RowIO<R>::ld(q_lane + o.y, v1);
@@ -382,6 +387,10 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll 1
       for (uint32_t e = g1; e < g2; ++e) {
         const uint4 o = gent[e];
+        {
+          const uint32_t qmax = (uint32_t)(mv.rc + 1) * (uint32_t)(TR * 8);
+          PSR_CHK(o.x < qmax && o.y < qmax && o.z < qmax && o.w < qmax, 409);
+        }
         double v0[R], v1[R], v2[R], v3[R];
         RowIO<R>::ld(q_lane + o.x, v0);
         RowIO<R>::ld(q_lane + o.y, v1);
@@ -407,6 +416,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
       return a.F0out + r_ * n + 1 + s;
     };
     auto ga_finish = [&](int s, int i, int64_t r_, int jsp_, double accv) {
+      PSR_CHK(s >= 0 && s < K && r_ >= 0 && r_ < a.N, 410);   // element (species, r) of the [K][ld] arrays
       const int64_t o = (int64_t)s * a.ld + r_;
       if (!jac) {
         if (a.flags & kOutWdot) a.wdot[o] = accv;
@@ -521,6 +531,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
         // keeps the loop counter and the record addresses in the uniform datapath
         const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
         const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS + 1]);
+        PSR_CHK(kl_begin >= 0 && kl_begin <= kl_end && kl_end <= (int)hdr->n_rx && kl_end <= mv.rc, 401);
         auto exps = [&](auto& ex, auto& ey) {
           constexpr int N = sizeof(ex) / sizeof(double);
           if constexpr (FAST) {
@@ -584,6 +595,10 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
           if constexpr (CLS < kClsLong) {
             double f0[R], f1[R], f2[R], p0[R], p1[R], p2[R];
+            {
+              const uint32_t cmax = (uint32_t)cs_elems * 8u;   // factor rows of the C tile, unit and zero rows included
+              PSR_CHK(ra_.y < cmax && ra_.z < cmax && ra_.w < cmax && rb_.x < cmax && rb_.y < cmax && rb_.z < cmax, 402);
+            }
             RowIO<R>::ld(c_lane + ra_.y, f0);
             RowIO<R>::ld(c_lane + ra_.z, f1);
             RowIO<R>::ld(c_lane + ra_.w, f2);
@@ -607,6 +622,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll 1
             for (int j = 0; j < nr + np; ++j) {
               double cv[R];
+              PSR_CHK((uint32_t)fsp[j] < (uint32_t)(K + 2), 403);
               RowIO<R>::ld(c_lane + (uint32_t)fsp[j] * (uint32_t)(TR * 8), cv);
 #pragma unroll
               for (int i = 0; i < R; ++i) {
@@ -679,8 +695,10 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
 #pragma unroll
             for (int i = 0; i < R; ++i) M[i] = ctot_s[lane * R + i];
             const uint32_t e1 = ax->eff_off + ax->n_eff;
+            PSR_CHK((meta >> kMetaAuxShift) < hdr->n_aux && e1 <= hdr->n_eff, 404);
 #pragma unroll 1
             for (uint32_t e = ax->eff_off; e < e1; ++e) {
+              PSR_CHK(effs[e].off < (uint32_t)cs_elems * 8u, 405);
               double cv[R];
               RowIO<R>::ld(c_lane + effs[e].off, cv);
 #pragma unroll
@@ -820,6 +838,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
               bool valid_;
               state_of(tile, i, r_, jsp_, valid_);
               if (valid_) {
+                PSR_CHK((int64_t)rb_.w < (int64_t)mv.I && r_ < a.N, 406);   // element (reaction, r) of the [I][ldk] outputs
                 const int64_t o = (int64_t)rb_.w * a.ldk + r_;
                 if (a.flags & kOutKf) a.kf[o] = kf[i];
                 if (a.flags & kOutKr) a.kr[o] = (meta & kMetaRev) ? kr[i] : 0.0;
@@ -959,6 +978,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           for (int jj = 0; jj < SPW; ++jj) {
             const int s = sp[jj];
             if (s >= 0) {
+              PSR_CHK(s < K && r[i] >= 0 && r[i] < a.N, 411);
               const int64_t o = (int64_t)s * a.ld + r[i];
               if (a.flags & kOutWdot) a.wdot[o] = acc[jj][i];
               if (wantF) {
@@ -1035,6 +1055,7 @@ __global__ void __launch_bounds__(NW * 32, PSR_MINB(NW)) psr_eval_kernel(const M
           if (v < n_states) {
             const uint32_t rr = (uint32_t)v / (uint32_t)Kp;
             const uint32_t j = (uint32_t)v - rr * (uint32_t)Kp;
+            PSR_CHK(j >= (uint32_t)K || ((int64_t)rr * n + 1 + j) * n + i < a.N * (int64_t)n * n, 412);
             if (j < (uint32_t)K) a.J[((int64_t)rr * n + 1 + j) * n + i] = stg[l * npad + i];
           }
         }
@@ -1113,6 +1134,16 @@ cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, size_t smem_opt
   PSR_SHAPES(PSR_O)
 #undef PSR_O
   return cudaErrorInvalidConfiguration;
+}
+
+// ------------------------------------------------------------------ PSR_CHECK plumbing
+PSR_CHK_TU_READER(chk_read_kernels)
+
+// trips one check on purpose (code 999): "0 failures" must not be able to mean "the checks are compiled out"
+__global__ void chk_selftest_kernel(int one) { PSR_CHK(one != 1, 999); }
+cudaError_t launch_chk_selftest(cudaStream_t st) {
+  chk_selftest_kernel<<<1, 1, 0, st>>>(1);
+  return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------ FP64 pipe probes

@@ -64,5 +64,38 @@ __device__ __forceinline__ void named_bar_sync(int id, int count) {
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// ------------------------------------------------------------------ bounds checks of the -DPSR_CHECK build
+// compute-sanitizer is refused on the GPU pool this library is developed on.  In its place the
+// PSR_CHECK build asserts, on the device, every shared-memory offset the kernels take from the mechanism tables and
+// every global output index against its bound: PSR_CHK(cond, code) counts a failure and keeps the first code (the
+// access still happens: with all checks green nothing is out of range).  In the product build the macro is empty and
+// its arguments are not evaluated.  Each translation unit has its own counter (no relocatable device code);
+// psr_check_failures (psr_api.cu) sums them.
+#ifdef PSR_CHECK
+static __device__ unsigned int g_psr_chk[2];   // failures, first failing code
+#define PSR_CHK(cond, code)                                                       \
+  do {                                                                            \
+    if (!(cond)) {                                                                \
+      if (atomicAdd(&g_psr_chk[0], 1u) == 0u) g_psr_chk[1] = (unsigned)(code);    \
+    }                                                                             \
+  } while (0)
+// host: read and reset this translation unit's counter (synchronises the device)
+static inline cudaError_t psr_chk_read_reset(unsigned int* count, unsigned int* first_code) {
+  unsigned int h[2] = {0u, 0u}, z[2] = {0u, 0u};
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaMemcpyFromSymbol(h, g_psr_chk, sizeof h);
+  if (e == cudaSuccess) e = cudaMemcpyToSymbol(g_psr_chk, z, sizeof z);
+  *count = h[0];
+  *first_code = h[1];
+  return e;
+}
+#define PSR_CHK_TU_READER(name) \
+  cudaError_t name(unsigned int* count, unsigned int* first_code) { return psr_chk_read_reset(count, first_code); }
+#else
+#define PSR_CHK(cond, code) ((void)0)
+#define PSR_CHK_TU_READER(name) \
+  cudaError_t name(unsigned int* count, unsigned int* first_code) { *count = 0u; *first_code = 0u; return cudaSuccess; }
+#endif
+
 }  // namespace psr
 #endif

@@ -25,6 +25,9 @@ struct RxCtx {
   uint32_t lnctot_lane; // this lane's ln C_tot
   ExpTab etab;
   float amax;           // NaN-propagating running max of |high word| of the exp arguments of this lane
+#ifdef PSR_CHECK
+  uint32_t chk_c_bytes; // size of the C tile in bytes, (K + 2) rows: bound of every factor / efficiency offset
+#endif
 };
 
 // One record class of warp w's share of a chunk.  CLS: 0..3 = reaction type in the 3+3 slot form, kClsLong = long
@@ -36,6 +39,7 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
                                              int w, Sink&& sink) {
   const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
   const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS + 1]);
+  PSR_CHK(kl_begin >= 0 && kl_begin <= kl_end && kl_end <= (int)hdr->n_rx, 101);
   auto exps = [&](auto& ex, auto& ey) {
     constexpr int N = sizeof(ex) / sizeof(double);
     if constexpr (FAST) {
@@ -74,6 +78,8 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
 
     // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
     if constexpr (CLS < kClsLong) {
+      PSR_CHK(ra_.y < cx.chk_c_bytes && ra_.z < cx.chk_c_bytes && ra_.w < cx.chk_c_bytes && rb_.x < cx.chk_c_bytes &&
+                  rb_.y < cx.chk_c_bytes && rb_.z < cx.chk_c_bytes && ((ra_.y | ra_.z | ra_.w | rb_.x | rb_.y | rb_.z) % kRowBytes) == 0, 102);
       const double f0 = lds64(cx.c_lane + ra_.y), f1 = lds64(cx.c_lane + ra_.z), f2 = lds64(cx.c_lane + ra_.w);
       const double p0 = lds64(cx.c_lane + rb_.x), p1 = lds64(cx.c_lane + rb_.y), p2 = lds64(cx.c_lane + rb_.z);
       pf = f0 * f1 * f2;
@@ -86,6 +92,7 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
       pr = 1.0;
 #pragma unroll 1
       for (int j = 0; j < nr + np; ++j) {
+        PSR_CHK((uint32_t)fsp[j] * (uint32_t)kRowBytes < cx.chk_c_bytes, 103);
         const double cv = lds64(cx.c_lane + (uint32_t)fsp[j] * (uint32_t)kRowBytes);
         if (j < nr) pf *= cv;
         else pr *= cv;
@@ -121,8 +128,12 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
       const EffEnt* effs = reinterpret_cast<const EffEnt*>(blob + hdr->off_eff);
       double M = lds64(cx.ctot_lane);
       const uint32_t e1 = ax->eff_off + ax->n_eff;
+      PSR_CHK((meta >> kMetaAuxShift) < hdr->n_aux && e1 <= hdr->n_eff, 104);
 #pragma unroll 1
-      for (uint32_t e = ax->eff_off; e < e1; ++e) M = fma(effs[e].am1, lds64(cx.c_lane + effs[e].off), M);
+      for (uint32_t e = ax->eff_off; e < e1; ++e) {
+        PSR_CHK(effs[e].off < cx.chk_c_bytes, 105);
+        M = fma(effs[e].am1, lds64(cx.c_lane + effs[e].off), M);
+      }
       if (type == RX_THREE_BODY) {
         Mout = M;
       } else if (type == RX_LINDEMANN) {

@@ -123,6 +123,9 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     // ================================================================== reaction warps
     RxCtx cx;
     cx.etab = exp_tab_load(mv.exp_tab);
+#ifdef PSR_CHECK
+    cx.chk_c_bytes = (uint32_t)cs_elems * 8u;
+#endif
     mbar_wait(&bars[B_BLOB], 0);
     int64_t tile = blockIdx.x;
     for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += gridDim.x) {
@@ -150,6 +153,8 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
             pr *= M;
           }
           const double q = fma(kf, pf, -(kr * pr));
+          PSR_CHK(kl >= 0 && kl < mv.rc, 201);                               // a row of the q buffer (row rc is the zero row)
+          PSR_CHK(!OUTK || !valid || (int64_t)korig < (int64_t)mv.I, 202);   // a row of the kf / kr / q outputs
           sts64(q_lane + (uint32_t)kl * (uint32_t)kRowBytes, q);
           if constexpr (OUTK) {
             if (valid) {
@@ -297,9 +302,12 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
         uint32_t row_off, pad;
         double W;
         int64_t goff;
+        PSR_CHK(te >= tbl && te < tbl + (uint32_t)mv.spw * (uint32_t)sizeof(SpEnt), 203);   // one flush per owned species
         asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(row_off), "=r"(pad) : "r"(te));
+        PSR_CHK(row_off < (uint32_t)ds_elems * 8u && pad < (uint32_t)ds_elems * 8u, 204);
         if (LAST) {
           asm volatile("ld.shared.v2.b64 {%0, %1}, [%2+16];" : "=l"(goff), "=d"(W) : "r"(te));
+          PSR_CHK(!valid || (goff >= 0 && goff % 8 == 0 && r < a.N && goff / 8 + r < (int64_t)K * a.ld), 205);   // element (species, r) of a [K][ld] output
           if (valid) {
             if (out_w) *reinterpret_cast<double*>(const_cast<char*>(wdot_r) + goff) = acc;
             if (wantF)
@@ -328,6 +336,11 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
         const uint32_t c0 = ca, c1 = cb;
         ca = oa.x;
         cb = ob.x;
+        {   // the groups read ahead (padding groups included) point at rows of the q buffer, zero row included
+          const uint32_t qmax = (uint32_t)q_elems * 8u;
+          PSR_CHK((oa.x & ~3u) < qmax && oa.y < qmax && oa.z < qmax && oa.w < qmax && (ob.x & ~3u) < qmax && ob.y < qmax &&
+                      ob.z < qmax && ob.w < qmax, 206);
+        }
         a0 = lds64(q_lane + (oa.x & ~3u)), a1 = lds64(q_lane + oa.y), a2 = lds64(q_lane + oa.z), a3 = lds64(q_lane + oa.w);
         b0 = lds64(q_lane + (ob.x & ~3u)), b1 = lds64(q_lane + ob.y), b2 = lds64(q_lane + ob.z), b3 = lds64(q_lane + ob.w);
         ld_group(gs + (uint32_t)(i + 4) * 16u, oa);
@@ -377,6 +390,8 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
 
 // once per process: the kernels' dynamic shared-memory limit raised to the device's (mechanisms of different sizes
 // share the kernel instances)
+PSR_CHK_TU_READER(chk_read_ws)
+
 cudaError_t ws_set_smem(size_t smem) {
   cudaError_t e = cudaFuncSetAttribute(psr_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -967,6 +967,68 @@ def test_calls_are_capturable_in_a_cuda_graph_and_honour_the_stream(torch_cuda, 
     assert residual_rel_err(F_g.cpu().numpy(), ref["F"]).max() <= TOL_F
 
 
+# ------------------------------------------------------------------ bounds-checked build (stands in for compute-sanitizer)
+_CHECK_SCRIPT = r"""
+import json, sys
+import numpy as np, torch
+from paper_2005_11468_b200 import binding, build, synth
+build.build(check=True)                       # no-op when libpsr_b200_check.so is newer than the sources
+binding._LIB_PATH = build.LIB_CHECK           # this process loads the -DPSR_CHECK library instead of the product one
+binding._build.needs_build = lambda: False
+dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+out = {"selftest": binding.check_failures(selftest=True)}          # one assertion tripped on purpose
+for cfg, n in (("C0", None), ("C1", 2000), ("C3", 97), ("C2", 70), ("P5", 40)):
+    mech, b = synth.make_config(cfg, n) if n else synth.make_config(cfg)
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y, Yin, tau = (dev(x) for x in (b.T, b.P, b.Y, b.Yin, b.tau))
+    Tin = torch.full_like(T, 400.0)
+    for fused_only in (0, 1):                 # the warp-specialised kernel where it applies, then the general one
+        gm.set_option(binding.OPT_FUSED_ONLY, fused_only)
+        gm.eval_kf_kr(T, P, Y)
+        gm.eval_wdot(T, P, Y, want_q=True)
+        gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+    gm.eval_residual_energy(T, P, Y, Tin, Yin, tau, want_wdot=True)
+    m = min(b.n, 40)
+    a = [x[..., :m].contiguous() for x in (T, P, Y, Yin, tau)]
+    for generic in (0, 1):                    # the fused Jacobian kernel where it applies, then the generic sweep
+        gm.set_option(binding.OPT_JAC_GENERIC, generic)
+        gm.fd_jacobian(*a, want_F0=True)
+    gm.fd_jacobian(*a, Tin=Tin[:m].contiguous())
+    if cfg in ("C0", "C1"):
+        n1 = mech.n_species + 1
+        gm.fd_jacobian_noalloc(*a, J=torch.empty((m, n1, n1), dtype=torch.float64, device="cuda"))
+    torch.cuda.synchronize()
+    out[cfg] = binding.check_failures()
+    gm.close()
+print("RESULT " + json.dumps(out))
+"""
+
+
+def test_bounds_checked_build(torch_cuda):
+    """compute-sanitizer is refused on this GPU pool; this stands in for its memcheck on the indices the
+    kernels take from the mechanism tables.  libpsr_b200_check.so is the same sources with -DPSR_CHECK: every
+    table-derived shared-memory offset (factor rows, q / rate-tile rows, gather entries, flush targets, scatter rows)
+    and every global output index is asserted on the device.  Run in a process of its own (it loads another build of
+    the library) on C0 in full, ragged C1 / C2 / C3 / P5 batches, every evaluation call, both evaluation kernels, both
+    Jacobian paths, the energy row and the no-alloc entry point.  A self-test trips one assertion first: zero failures
+    afterwards means the checks ran and held.  It finds out-of-range indices -- not races, not uninitialised reads."""
+    import subprocess
+    import sys
+    root = Path(__file__).resolve().parent.parent
+    res = subprocess.run([sys.executable, "-c", _CHECK_SCRIPT], cwd=root, capture_output=True, text=True, timeout=900)
+    assert res.returncode == 0, res.stderr[-3000:]
+    line = [l for l in res.stdout.splitlines() if l.startswith("RESULT ")][-1]
+    out = json.loads(line[len("RESULT "):])
+    assert out.pop("selftest") == [1, 999]
+    assert set(out) == {"C0", "C1", "C2", "C3", "P5"}
+    for cfg, (count, code) in out.items():
+        assert (count, code) == (0, 0), (cfg, count, code)
+
+
+def test_product_build_carries_no_checks(binding):
+    assert binding.check_failures() == (-1, 0)
+
+
 # ------------------------------------------------------------------ kernel math
 def test_table_exp_accuracy(torch_cuda, binding):
     """csrc/psr_math.cuh exp_fast against mpmath (50 digits): <= 4e-16 relative over the argument
