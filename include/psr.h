@@ -217,10 +217,16 @@ psr_status psr_solve_hybrid(const psr_mech* mech, int64_t N, double* T, const do
 const char* psr_last_error(void);
 
 /* Introspection: n_species, n_reactions, reactors per tile, warps per CTA, reactions per chunk,
- * number of chunks, dynamic shared memory bytes, CTAs per SM the launch is sized for. */
+ * number of chunks, dynamic shared memory bytes, CTAs per SM the launch is sized for (those six: of the general fused
+ * kernel), then which kernel the evaluation calls and psr_fd_jacobian take for this mechanism. */
 typedef struct {
   int32_t n_species, n_reactions, tile, warps, chunk_reactions, n_chunks, smem_bytes, ctas_per_sm;
   int32_t n_sm, n_falloff, n_third_body, nnz_nu;
+  int32_t eval_kernel;   /* kernel of psr_eval_wdot / _residual / _kf_kr: 0 general fused, 1 warp-specialised (resident
+                            tables), 2 warp-specialised for large mechanisms (streamed parts) */
+  int32_t eval_parts;    /* parts the mechanism is cut into for that kernel */
+  int32_t eval_acc_global; /* kernel 2: running sums of nu^T q in an L2-resident scratch instead of shared memory */
+  int32_t jac_kernel;    /* psr_fd_jacobian: 1 fused Jacobian kernel, 0 generic sweep */
 } psr_mech_info_t;
 psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);
 

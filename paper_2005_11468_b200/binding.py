@@ -33,7 +33,8 @@ class PsrMechDesc(C.Structure):
 
 class PsrMechInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_species", "n_reactions", "tile", "warps", "chunk_reactions", "n_chunks",
-                                         "smem_bytes", "ctas_per_sm", "n_sm", "n_falloff", "n_third_body", "nnz_nu")]
+                                         "smem_bytes", "ctas_per_sm", "n_sm", "n_falloff", "n_third_body", "nnz_nu",
+                                         "eval_kernel", "eval_parts", "eval_acc_global", "jac_kernel")]
 
 
 class PsrSolveOpts(C.Structure):

@@ -13,7 +13,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpsr_b200.so"
-SOURCES = [CSRC / "psr_api.cu", CSRC / "psr_kernels.cu", CSRC / "psr_ws.cu", CSRC / "psr_jac.cu", CSRC / "psr_lu.cu", CSRC / "psr_solve.cu"]
+SOURCES = [CSRC / "psr_api.cu", CSRC / "psr_kernels.cu", CSRC / "psr_ws.cu", CSRC / "psr_wsl.cu", CSRC / "psr_jac.cu", CSRC / "psr_lu.cu", CSRC / "psr_solve.cu"]
 HEADERS = [CSRC / "psr_tables.h", CSRC / "psr_math.cuh", CSRC / "psr_ptx.cuh", CSRC / "psr_rx.cuh", PKG.parent / "include" / "psr.h"]
 
 NVCC_FLAGS = [

@@ -31,6 +31,9 @@ cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_
 cudaError_t chk_read_kernels(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_ws(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_jac(unsigned int* count, unsigned int* first_code);
+cudaError_t chk_read_wsl(unsigned int* count, unsigned int* first_code);
+cudaError_t wsl_set_smem(size_t smem);
+cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st);
 cudaError_t launch_chk_selftest(cudaStream_t st);
 cudaError_t jac_set_smem(size_t smem);
 cudaError_t launch_jac(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
@@ -59,6 +62,11 @@ struct psr_mech {
   bool ws_ok = false;
   unsigned char* d_ws_chunks = nullptr;
   int32_t* d_ws_sp_of = nullptr;
+  WslView wsl{};                // warp-specialised kernel for large mechanisms (psr_wsl.cu), when ws_ok is false (wsl_ok)
+  bool wsl_ok = false;
+  unsigned char* d_wsl_chunks = nullptr;
+  int32_t* d_wsl_sp_of = nullptr;
+  double* d_wsl_acc = nullptr;
   JacView jac{};                // fused finite-difference Jacobian kernel (psr_jac.cu), when the mechanism qualifies (jac_ok)
   bool jac_ok = false;
   unsigned char* d_jac_chunks = nullptr;
@@ -140,8 +148,14 @@ struct JacBuild {                    // extra inputs / outputs when the blobs ar
   int rows_max = 0;                  // out: most rate-tile rows of a part
 };
 
+struct WslBuild {                    // gather streams of the large-mechanism warp-specialised kernel (psr_wsl.cu)
+  const std::vector<int32_t>* sp_of; // ownership [kWslHelpWarps][spw]
+  int spw = 0;
+};
+
 void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out,
-                 const std::vector<int32_t>* ws_sp_of = nullptr, int ws_spw = 0, JacBuild* jb = nullptr) {
+                 const std::vector<int32_t>* ws_sp_of = nullptr, int ws_spw = 0, JacBuild* jb = nullptr,
+                 const WslBuild* wl = nullptr) {
   const uint32_t row_bytes = (uint32_t)kRowBytes;
   const int rc = (I + n_chunks - 1) / n_chunks;
   out.n_chunks = n_chunks;
@@ -304,6 +318,33 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
         gent.insert(gent.end(), 16, jzero);
       }
       gptr.push_back(0);
+    } else if (wl) {
+      // large-mechanism kernel: per helper warp the groups of its species in ownership order ("+" groups, then "-"
+      // groups); a species without a term in this part is left out, except in part 0 whose flushes initialise the
+      // running sums (one all-zero group there).  Every flush reads its target row from the list.
+      gptr.clear();
+      for (int hw = 0; hw < kWslHelpWarps; ++hw) {
+        jac_range[3 * hw] = (uint16_t)(gent.size() / 4);
+        jac_range[3 * hw + 2] = (uint16_t)gptr.size();
+        for (int jj = 0; jj < wl->spw; ++jj) {
+          const int sidx = (*wl->sp_of)[(size_t)hw * wl->spw + jj];
+          if (sidx < 0) break;
+          if (pos[sidx].empty() && neg[sidx].empty() && c != 0) continue;
+          const size_t first = gent.size();
+          add_group(pos[sidx]);
+          const size_t first_neg = gent.size();
+          add_group(neg[sidx]);
+          if (gent.size() == first) gent.insert(gent.end(), 4, zero_off);
+          if (!neg[sidx].empty())
+            for (size_t g = first_neg; g < gent.size(); g += 4) gent[g] |= kGatherNeg;
+          gent[gent.size() - 4] |= kGatherLast;
+          gptr.push_back((uint32_t)sidx * row_bytes);
+        }
+        if ((gent.size() / 4 - jac_range[3 * hw]) % 2) gent.insert(gent.end(), 4, zero_off);
+        jac_range[3 * hw + 1] = (uint16_t)(gent.size() / 4);
+        gent.insert(gent.end(), 16, zero_off);
+        gptr.push_back(gptr.empty() ? 0u : gptr.back());   // read one ahead by the kernel
+      }
     } else if (!ws_sp_of) {
       for (int s = 0; s < K; ++s) {
         gptr[2 * s] = (uint32_t)gent.size();
@@ -348,6 +389,9 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
     if (jb)
       for (int wv = 0; wv < kJacWarps; ++wv)
         for (int t = 0; t < 3; ++t) hdr.wb[kJacWarps + wv][t] = jac_range[3 * wv + t];
+    if (wl)
+      for (int hw = 0; hw < kWslHelpWarps; ++hw)
+        for (int t = 0; t < 3; ++t) hdr.wb[kWslRxWarps + hw][t] = jac_range[3 * hw + t];
     if (jb) jb->rows_max = std::max(jb->rows_max, (int)jrows);
     if (ws_sp_of)
       for (int hw = 0; hw < kWsHelpWarps; ++hw) {
@@ -648,6 +692,56 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     }
   }
 
+  // ---- large mechanisms (psr_wsl.cu): the fewest parts for which one C tile, the running sums, two q buffers, a two-stage
+  // ring of part tables and the per-CTA rows fit one CTA; the sums in shared memory if that is possible at all (larger
+  // parts then), else in an L2-resident scratch
+  BlobSet lbs;
+  WslView lv{};
+  bool wsl_ok = false;
+  std::vector<int32_t> wsl_sp_of;
+  if (!ws_ok) {
+    const int spw_l = (K + kWslHelpWarps - 1) / kWslHelpWarps;
+    const int Kp = (K + 1) & ~1;
+    wsl_sp_of = assign_species(rx, K, I, kWslHelpWarps, spw_l);
+    WslBuild wb;
+    wb.sp_of = &wsl_sp_of;
+    wb.spw = spw_l;
+    for (int acc_global = 0; acc_global < 2 && !wsl_ok; ++acc_global) {
+      for (int n_parts = 2; n_parts <= kWslMaxParts && n_parts <= I && !wsl_ok; ++n_parts) {
+        const int rc_l = (I + n_parts - 1) / n_parts;
+        // (a quick bound before building the blobs: the q buffers alone)
+        if ((size_t)(K + 2) * kRowBytes + (acc_global ? 0 : (size_t)K * kRowBytes) + (size_t)2 * (rc_l + 1) * kRowBytes >
+            (size_t)prop.sharedMemPerBlockOptin)
+          continue;
+        build_blobs(rx, K, I, n_parts, kWslRxWarps, 0.0, lbs, nullptr, 0, nullptr, &wb);
+        size_t o = 0;
+        lv.smem_cs = (uint32_t)o;
+        o += align_up((size_t)(K + 2) * kRowBytes, 128);
+        lv.smem_acc = (uint32_t)o;
+        o += acc_global ? 0 : align_up((size_t)K * kRowBytes, 128);
+        lv.smem_q = (uint32_t)o;
+        o += align_up((size_t)2 * (lbs.rc + 1) * kRowBytes, 128);
+        lv.smem_mech = (uint32_t)o;
+        o += 2 * lbs.stride;
+        lv.smem_misc = (uint32_t)o;
+        o += align_up((size_t)2 * Kp * 8 + (size_t)2 * 8 * kRowBytes + (size_t)2 * 3 * kRowBytes + 10 * 8 +
+                          (size_t)kWslHelpWarps * spw_l * 4, 128);
+        lv.smem_total = (uint32_t)o;
+        if (o <= (size_t)prop.sharedMemPerBlockOptin) {
+          wsl_ok = true;
+          lv.K = K;
+          lv.I = I;
+          lv.n_parts = n_parts;
+          lv.rc = lbs.rc;
+          lv.spw = spw_l;
+          lv.need_lnctot = need_lnctot;
+          lv.acc_global = acc_global;
+          lv.chunk_stride = (uint32_t)lbs.stride;
+        }
+      }
+    }
+  }
+
   // ---- fused Jacobian kernel (psr_jac.cu).  It takes mechanisms whose every rate is k(T, C_tot) x a product of at most
   // 3 + 3 concentrations, x [M] for three-body reactions: no falloff reaction with an efficiency list (its k changes
   // with the composition), no long factor lists, no sign records.  Anything else keeps the generic sweep.
@@ -882,6 +976,26 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     m->jac = jv;
     m->jac_ok = true;
   }
+  if (wsl_ok) {
+    const size_t acc_bytes = lv.acc_global ? (size_t)prop.multiProcessorCount * K * kRowBytes : 256;
+    if ((e = cudaMalloc(&m->d_wsl_chunks, lbs.all.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_wsl_chunks, lbs.all.data(), lbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_wsl_sp_of, 4 * wsl_sp_of.size())) != cudaSuccess ||
+        (e = cudaMemcpy(m->d_wsl_sp_of, wsl_sp_of.data(), 4 * wsl_sp_of.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMalloc(&m->d_wsl_acc, acc_bytes)) != cudaSuccess ||
+        (e = wsl_set_smem((size_t)prop.sharedMemPerBlockOptin)) != cudaSuccess) {
+      cleanup();
+      return cuda_fail(e, "large-mechanism kernel tables");
+    }
+    lv.chunks = m->d_wsl_chunks;
+    lv.sp_of = m->d_wsl_sp_of;
+    lv.acc_g = m->d_wsl_acc;
+    lv.invW = m->d_invW;
+    lv.Wm = m->d_W;
+    lv.exp_tab = m->d_exptab;
+    m->wsl = lv;
+    m->wsl_ok = true;
+  }
   if (ws_ok) {
     if ((e = cudaMalloc(&m->d_ws_chunks, wbs.all.size())) != cudaSuccess ||
         (e = cudaMemcpy(m->d_ws_chunks, wbs.all.data(), wbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
@@ -916,6 +1030,9 @@ void psr_mech_free(psr_mech* m) {
   for (void* q : m->retired) cudaFree(q);
   cudaFree(m->d_ws_chunks);
   cudaFree(m->d_ws_sp_of);
+  cudaFree(m->d_wsl_chunks);
+  cudaFree(m->d_wsl_sp_of);
+  cudaFree(m->d_wsl_acc);
   cudaFree(m->d_jac_chunks);
   cudaFree(m->d_jac_inc);
   cudaFree(m->d_jac_inc_ptr);
@@ -939,6 +1056,10 @@ psr_status psr_mech_info(const psr_mech* m, psr_mech_info_t* info) {
   info->n_falloff = m->n_falloff;
   info->n_third_body = m->n_third_body;
   info->nnz_nu = m->nnz_nu;
+  info->eval_kernel = m->ws_ok ? 1 : m->wsl_ok ? 2 : 0;
+  info->eval_parts = m->ws_ok ? m->ws.n_parts : m->wsl_ok ? m->wsl.n_parts : m->view.n_chunks;
+  info->eval_acc_global = m->wsl_ok ? m->wsl.acc_global : 0;
+  info->jac_kernel = m->jac_ok ? 1 : 0;
   return PSR_OK;
 }
 
@@ -965,6 +1086,15 @@ psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
     const int bulk_ok = al16(a.T) && al16(a.P) && al16(a.Y) && (a.ld % 2 == 0) && (!wantF || (al16(a.Yin) && al16(a.tau)));
     const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
     cudaError_t e = launch_ws(m->ws, a, grid, bulk_ok, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, fn);
+    return PSR_OK;
+  }
+  // the same calls of a mechanism too large for that: the warp-specialised kernel with streamed parts
+  if (m->wsl_ok && !m->opt_fused_only && (a.flags & ~(kOutWdot | kOutF | kOutKf | kOutKr | kOutQ)) == 0) {
+    auto al16 = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; };
+    const int bulk_ok = al16(a.T) && al16(a.P) && al16(a.Y) && (a.ld % 2 == 0) && (!(a.flags & kOutF) || al16(a.tau));
+    const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
+    cudaError_t e = launch_wsl(m->wsl, a, grid, bulk_ok, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, fn);
     return PSR_OK;
   }
@@ -1319,7 +1449,7 @@ int32_t psr_check_failures(int32_t selftest, int32_t* first_code) {
     if (e != cudaSuccess) { cuda_fail(e, "psr_check_failures (self-test)"); return -2; }
   }
   unsigned int total = 0, first = 0;
-  cudaError_t (*readers[3])(unsigned int*, unsigned int*) = {chk_read_ws, chk_read_jac, chk_read_kernels};
+  cudaError_t (*readers[4])(unsigned int*, unsigned int*) = {chk_read_ws, chk_read_wsl, chk_read_jac, chk_read_kernels};
   for (auto rd : readers) {
     unsigned int c = 0, code = 0;
     cudaError_t e = rd(&c, &code);

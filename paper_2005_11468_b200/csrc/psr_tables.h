@@ -127,6 +127,33 @@ struct WsView {
   uint32_t smem_cs, smem_ds, smem_q, smem_acc, smem_mech, smem_misc, smem_total;
 };
 
+// ---- warp-specialised kernel for LARGE mechanisms (psr_wsl.cu): the same roles as psr_ws.cu with what does not fit
+// one CTA's shared memory given up -- a single C tile, no Y - Y_in tile (the epilogue reads Y, Y_in from global
+// memory), the parts streamed through a two-stage ring instead of resident, and the running sums of nu^T q in a
+// shared-memory tile when that fits, else in an L2-resident scratch [CTA][K][32] (acc_global).
+// Gather streams per (part, helper warp) as for psr_ws.cu, except that species without a term in a part are left
+// out (part 0 keeps every owned species: its flushes initialise the sums) and every flush takes its target -- the
+// byte offset of the species' row in a [K][32] tile -- from a list in the blob (gptr area):
+//   wb[kWslRxWarps + hw][0..2] = first group, one past the last group, first entry of the target list.
+constexpr int kWslRxWarps = 11, kWslHelpWarps = 5, kWslWarps = kWslRxWarps + kWslHelpWarps;
+constexpr int kWslMaxParts = 64;
+
+struct WslView {
+  const unsigned char* chunks;  // n_parts blobs, chunk_stride bytes apart
+  const double* invW;
+  const double* Wm;
+  const int32_t* sp_of;         // [kWslHelpWarps][spw] species owned by a helper warp (owned ones first, then -1)
+  const double* exp_tab;
+  double* acc_g;                // acc_global: [CTAs][K][32] running sums; else unused
+  int32_t K, I;
+  int32_t n_parts, rc;
+  int32_t spw;
+  int32_t need_lnctot;
+  int32_t acc_global;
+  uint32_t chunk_stride;
+  uint32_t smem_cs, smem_acc, smem_q, smem_mech, smem_misc, smem_total;
+};
+
 // ---- fused finite-difference Jacobian kernel (psr_jac.cu): lane <-> reactor, one CTA per tile of 32 reactors.
 // Phase 1 evaluates the tile (at T + h_T, then at T) and sums the forward and reverse rates of every reaction
 // into per-species sums BY CONCENTRATION ORDER; phase 2 builds the K species columns from them, warp <-> column.
