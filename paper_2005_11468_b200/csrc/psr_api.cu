@@ -151,6 +151,7 @@ struct JacBuild {                    // extra inputs / outputs when the blobs ar
 struct WslBuild {                    // gather streams of the large-mechanism warp-specialised kernel (psr_wsl.cu)
   const std::vector<int32_t>* sp_of; // ownership [kWslHelpWarps][spw]
   int spw = 0;
+  bool tuples = false;               // running sums in global memory: one (q row | sign, target row) tuple per entry of nu^T
 };
 
 void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out,
@@ -323,7 +324,25 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
       // groups); a species without a term in this part is left out, except in part 0 whose flushes initialise the
       // running sums (one all-zero group there).  Every flush reads its target row from the list.
       gptr.clear();
-      for (int hw = 0; hw < kWslHelpWarps; ++hw) {
+      for (int hw = 0; hw < kWslHelpWarps && wl->tuples; ++hw) {
+        // tuple stream (sums in global memory, added to with red.global: no running sum, no flush): per helper warp, its
+        // species in ownership order, a species' "+" entries then its "-" entries -- a fixed order.  Entry = {byte
+        // offset of the q row | 1 if it is subtracted, byte offset of the species' row}; padded to a multiple of 4
+        // tuples, and 8 more for the kernel's read-ahead, with {zero row of q, spare row K of the sums}.
+        jac_range[3 * hw] = (uint16_t)(gent.size() / 4);   // in 16-byte units = pairs of tuples
+        size_t n_t = 0;
+        for (int jj = 0; jj < wl->spw; ++jj) {
+          const int sidx = (*wl->sp_of)[(size_t)hw * wl->spw + jj];
+          if (sidx < 0) break;
+          for (uint32_t qo : pos[sidx]) { gent.push_back(qo); gent.push_back((uint32_t)sidx * row_bytes); ++n_t; }
+          for (uint32_t qo : neg[sidx]) { gent.push_back(qo | 1u); gent.push_back((uint32_t)sidx * row_bytes); ++n_t; }
+        }
+        for (; n_t % 4; ++n_t) { gent.push_back(zero_off); gent.push_back((uint32_t)K * row_bytes); }
+        jac_range[3 * hw + 1] = (uint16_t)(gent.size() / 4);
+        for (int t = 0; t < 8; ++t) { gent.push_back(zero_off); gent.push_back((uint32_t)K * row_bytes); }
+      }
+      if (wl->tuples) gptr.push_back(0);
+      for (int hw = 0; hw < kWslHelpWarps && !wl->tuples; ++hw) {
         jac_range[3 * hw] = (uint16_t)(gent.size() / 4);
         jac_range[3 * hw + 2] = (uint16_t)gptr.size();
         for (int jj = 0; jj < wl->spw; ++jj) {
@@ -706,8 +725,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     WslBuild wb;
     wb.sp_of = &wsl_sp_of;
     wb.spw = spw_l;
+    // the sums in shared memory only when that leaves room for parts so large that at most 4 are needed (P5: 0.099 ms
+    // against 0.105 with the sums in L2); beyond that the tile's worth of shared memory is better spent on larger
+    // parts (measured: C2 0.522 ms with 8 parts and the sums in L2, 0.538 with 11 parts and the sums in shared memory)
     for (int acc_global = 0; acc_global < 2 && !wsl_ok; ++acc_global) {
-      for (int n_parts = 2; n_parts <= kWslMaxParts && n_parts <= I && !wsl_ok; ++n_parts) {
+      wb.tuples = acc_global != 0;
+      for (int n_parts = 2; n_parts <= (acc_global ? kWslMaxParts : 4) && n_parts <= I && !wsl_ok; ++n_parts) {
         const int rc_l = (I + n_parts - 1) / n_parts;
         // (a quick bound before building the blobs: the q buffers alone)
         if ((size_t)(K + 2) * kRowBytes + (acc_global ? 0 : (size_t)K * kRowBytes) + (size_t)2 * (rc_l + 1) * kRowBytes >
@@ -977,7 +1000,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     m->jac_ok = true;
   }
   if (wsl_ok) {
-    const size_t acc_bytes = lv.acc_global ? (size_t)prop.multiProcessorCount * K * kRowBytes : 256;
+    const size_t acc_bytes = lv.acc_global ? (size_t)prop.multiProcessorCount * (K + 1) * kRowBytes : 256;   // + a spare row
     if ((e = cudaMalloc(&m->d_wsl_chunks, lbs.all.size())) != cudaSuccess ||
         (e = cudaMemcpy(m->d_wsl_chunks, lbs.all.data(), lbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMalloc(&m->d_wsl_sp_of, 4 * wsl_sp_of.size())) != cudaSuccess ||

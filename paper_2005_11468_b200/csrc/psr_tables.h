@@ -135,7 +135,7 @@ struct WsView {
 // out (part 0 keeps every owned species: its flushes initialise the sums) and every flush takes its target -- the
 // byte offset of the species' row in a [K][32] tile -- from a list in the blob (gptr area):
 //   wb[kWslRxWarps + hw][0..2] = first group, one past the last group, first entry of the target list.
-constexpr int kWslRxWarps = 11, kWslHelpWarps = 5, kWslWarps = kWslRxWarps + kWslHelpWarps;
+constexpr int kWslRxWarps = 10, kWslHelpWarps = 6, kWslWarps = kWslRxWarps + kWslHelpWarps;
 constexpr int kWslMaxParts = 64;
 
 struct WslView {

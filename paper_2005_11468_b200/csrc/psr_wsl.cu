@@ -7,13 +7,14 @@
 // pair -- 13 x 500 visits of ~1.5 reactions each at C3, the running sums bouncing through L2 in between: 55 % of
 // its instructions (profiles/r1d_psr_eval_kernel_C3.md).  Here the roles are those of psr_ws.cu:
 //
-//   reaction warps (11)  a3..a7 of their share of a part's records, part after part, tile after tile; q goes to
+//   reaction warps (10)  a3..a7 of their share of a part's records, part after part, tile after tile; q goes to
 //                        one of two q buffers; the part's tables come from a two-stage ring (bulk copies).
-//   helper warps (5)     a8: gather of the q buffer just filled -- flat streams of 4-entry groups that SKIP the
+//   helper warps (6)     a8: gather of the q buffer just filled -- flat streams of 4-entry groups that SKIP the
 //                        species without a term in the part, each flush taking its target row from a list in the
-//                        blob; the running sums live in a shared-memory tile when it fits (C2), else in an
-//                        L2-resident scratch (C3): part 0 stores, later parts add with red.global (one thread owns an
-//                        element: deterministic order, no latency exposed);
+//                        blob; the running sums live in a shared-memory tile when it fits (C2); else (C3) in an
+//                        L2-resident scratch that a flat stream of (q row, species row, sign) tuples adds to with
+//                        red.global -- one per entry of nu^T, no running sum, no flush (one thread owns an element:
+//                        deterministic order, no latency exposed);
 //                        a1: loads and state preparation of the NEXT tile, done ahead of the last part's gather so
 //                        that the reaction warps restart as early as the single C tile allows;
 //                        a9: per-tile epilogue (wdot, F) streaming Y, Y_in and the sums, four rows in flight.
@@ -54,7 +55,7 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
   int n_my = 0;
   while (n_my < mv.spw && my_sp[n_my] >= 0) ++n_my;   // owned species come first, -1 pads the list
   const bool accg = mv.acc_global != 0;
-  char* accg_lane = reinterpret_cast<char*>(mv.acc_g + (size_t)blockIdx.x * K * kTile + lane);   // row s at + s * kRowBytes
+  char* accg_lane = reinterpret_cast<char*>(mv.acc_g + (size_t)blockIdx.x * (K + 1) * kTile + lane);   // row s at + s * kRowBytes; row K: spare
   const uint32_t acc_lane = smem_u32(acc_s) + lane * 8;
 
   // a1: a tile's Y rows (into the C tile), T, P, tau; then W_bar = 1/sum Y_i/W_i, rho = P W_bar/(R T), C_i = rho Y_i/W_i,
@@ -145,14 +146,8 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       asm volatile("ld.shared.u32 %0, [%1];" : "=r"(off) : "r"(dst));
       dst += 4;
       PSR_CHK(off < (uint32_t)K * kRowBytes && off % kRowBytes == 0, 503);   // a row of the [K][32] running sums
-      if (accg) {
-        double* pa = reinterpret_cast<double*>(accg_lane + off);
-        if (FIRST) *pa = acc;
-        else asm volatile("red.global.add.f64 [%0], %1;" ::"l"(pa), "d"(acc) : "memory");
-      } else {
-        const uint32_t addr = acc_lane + off;
-        sts64(addr, FIRST ? acc : lds64(addr) + acc);
-      }
+      const uint32_t addr = acc_lane + off;   // (sums in shared memory; in global memory: gather_tuples)
+      sts64(addr, FIRST ? acc : lds64(addr) + acc);
       acc = 0.0;
     };
     const uint32_t qmax = (uint32_t)q_elems * 8u;
@@ -185,6 +180,38 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
     }
   };
 
+  // a8 with the sums in global memory: the tuple stream of this warp for one part (psr_api.cu build_blobs) -- per entry of
+  // nu^T one q value read from the buffer and one red.global.add to the species' sum, its sign applied on the way; four
+  // tuples per trip, read one trip ahead.  One thread owns an element of the sums and issues its adds in program order,
+  // so the order of the summation is fixed.
+  auto gather_tuples = [&](const unsigned char* blob, const uint32_t q_lane) {
+    const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
+    const uint32_t ts = smem_u32(blob + hdr->off_gent) + (uint32_t)hdr->wb[kWslRxWarps + hw][0] * 16u;
+    const int n_pairs = (int)hdr->wb[kWslRxWarps + hw][1] - (int)hdr->wb[kWslRxWarps + hw][0];   // 16-byte units, even
+    auto ld4 = [&](uint32_t addr, uint4& o) {
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w) : "r"(addr));
+    };
+    auto add = [&](uint32_t qo, uint32_t to) {
+      PSR_CHK((qo & ~1u) < (uint32_t)q_elems * 8u && to <= (uint32_t)K * kRowBytes && to % kRowBytes == 0, 506);
+      const double v = lds64(q_lane + (qo & ~1u));
+      const double sv = __hiloint2double(__double2hiint(v) ^ (int)(qo << 31), __double2loint(v));   // -v if bit 0 is set
+      asm volatile("red.global.add.f64 [%0], %1;" ::"l"(accg_lane + to), "d"(sv) : "memory");
+    };
+    uint4 ta, tb;
+    ld4(ts, ta);
+    ld4(ts + 16, tb);
+#pragma unroll 1
+    for (int i = 0; i < n_pairs; i += 2) {
+      const uint4 ca = ta, cb = tb;
+      ld4(ts + (uint32_t)(i + 2) * 16u, ta);
+      ld4(ts + (uint32_t)(i + 3) * 16u, tb);
+      add(ca.x, ca.y);
+      add(ca.z, ca.w);
+      add(cb.x, cb.y);
+      add(cb.z, cb.w);
+    }
+  };
+
   // a9 (Eq. 2 at steady state) and the wdot store of a tile: F_i = (Y_i - Y_in,i)/tau - wdot_i W_i/rho, eight rows in flight.
   // (A running sum kept in global memory is read past L1: the adds of the later parts were done at L2.)
   auto epilogue = [&](int64_t t, uint32_t lt) {
@@ -212,10 +239,16 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
           if (out_w) a.wdot[o] = tot[u];
           if (wantF) a.F[o] = fma(y[u] - yin[u], invtau, -(tot[u] * (W_s[sp[u]] * invrho)));
         }
+        // sums kept in global memory start the next tile at zero (this thread's own later adds come after this store)
+        if (accg && jj + u < n_my) __stcg(reinterpret_cast<double*>(accg_lane + (size_t)sp[u] * kRowBytes), 0.0);
       }
     }
   };
 
+  if (accg) {   // this warp's rows of the sums (and the spare row) start at zero
+    for (int jj = 0; jj < n_my; ++jj) __stcg(reinterpret_cast<double*>(accg_lane + (size_t)my_sp[jj] * kRowBytes), 0.0);
+    if (hw == 0) __stcg(reinterpret_cast<double*>(accg_lane + (size_t)K * kRowBytes), 0.0);
+  }
   const int64_t stride = gridDim.x;
   int64_t tile = blockIdx.x;
   if (tile < a.n_tiles) load_tile(tile, 0);
@@ -231,7 +264,8 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       }
       const unsigned char* blob = ring + (size_t)qb * mv.chunk_stride;
       const uint32_t q_lane = smem_u32(qh0 + qb * q_elems) + lane * 8;
-      if (p == 0) gather(std::true_type{}, blob, q_lane);
+      if (accg) gather_tuples(blob, q_lane);
+      else if (p == 0) gather(std::true_type{}, blob, q_lane);
       else gather(std::false_type{}, blob, q_lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars[L_EMPTYQ + qb]);
