@@ -36,10 +36,9 @@ struct RxCtx {
 // products of the two sides WITHOUT [M], and [M] (1 for a plain reaction) of record kl.
 template <int CLS, bool FAST, class Sink>
 __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blob, const ChunkHdr* hdr, const RxRec* recs,
-                                             int w, Sink&& sink) {
-  const int kl_begin = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS]);
-  const int kl_end = __reduce_min_sync(kFullMask, (int)hdr->wb[w][CLS + 1]);
+                                             const int kl_begin, const int kl_end, Sink&& sink) {
   PSR_CHK(kl_begin >= 0 && kl_begin <= kl_end && kl_end <= (int)hdr->n_rx, 101);
+  if (kl_begin >= kl_end) return;   // nothing of this class for this warp in this chunk (the rule in small parts)
   auto exps = [&](auto& ex, auto& ey) {
     constexpr int N = sizeof(ex) / sizeof(double);
     if constexpr (FAST) {
@@ -193,11 +192,20 @@ template <bool FAST, class Sink>
 __device__ __forceinline__ void rx_run_chunk(RxCtx& cx, const unsigned char* blob, int w, Sink&& sink) {
   const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
   const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
-  rx_run_class<0, FAST>(cx, blob, hdr, recs, w, sink);
-  rx_run_class<1, FAST>(cx, blob, hdr, recs, w, sink);
-  rx_run_class<2, FAST>(cx, blob, hdr, recs, w, sink);
-  rx_run_class<3, FAST>(cx, blob, hdr, recs, w, sink);
-  rx_run_class<kClsLong, FAST>(cx, blob, hdr, recs, w, sink);
+  // the six class boundaries of this warp are read together, ahead of the loops (read one by one in front of every
+  // class loop they cost a shared-memory round trip each: a quarter of a reaction warp's time when a part holds ten
+  // records per warp, as at 500 species).  The same in every lane: REDUX says so, which keeps loop counters and record
+  // addresses in the uniform datapath.
+  int kb[kClsLong + 2];
+#pragma unroll
+  for (int c = 0; c < kClsLong + 2; ++c) kb[c] = (int)hdr->wb[w][c];
+#pragma unroll
+  for (int c = 0; c < kClsLong + 2; ++c) kb[c] = __reduce_min_sync(kFullMask, kb[c]);
+  rx_run_class<0, FAST>(cx, blob, hdr, recs, kb[0], kb[1], sink);
+  rx_run_class<1, FAST>(cx, blob, hdr, recs, kb[1], kb[2], sink);
+  rx_run_class<2, FAST>(cx, blob, hdr, recs, kb[2], kb[3], sink);
+  rx_run_class<3, FAST>(cx, blob, hdr, recs, kb[3], kb[4], sink);
+  rx_run_class<kClsLong, FAST>(cx, blob, hdr, recs, kb[4], kb[5], sink);
 }
 
 }  // namespace psr
