@@ -438,9 +438,13 @@ def run_extras(binding, synth, torch, flush, only=None, cpu=True):
         instr = algorithmic_fp64_instr(mech.n_species, mech.n_reactions, info["n_third_body"], info["n_falloff"], info["nnz_nu"])
         F, w = torch.empty_like(Y), torch.empty_like(Y)
         ms = _time_call(torch, lambda: gm.eval_residual(T, P, Y, Yin, tau, F=F, wdot=w), flush)
+        prof = ncu_summary(cfg + "_residual")
         out[cfg] = {"call": "psr_eval_residual", "ms": ms, "reactor_evals_per_s": batch.n / (ms * 1e-3),
                     "reaction_evals_per_s": batch.n * mech.n_reactions / (ms * 1e-3),
-                    "alu_frac": instr * batch.n / (ms * 1e-3) / PEAK_INSTR}
+                    "alu_frac": instr * batch.n / (ms * 1e-3) / PEAK_INSTR,
+                    "kernel": {k: info[k] for k in ("eval_kernel", "eval_parts", "eval_acc_global")},
+                    "hbm_algorithmic_bytes": (3 + 4 * mech.n_species) * 8 * batch.n, "dram_bytes_ncu": prof.get("dram_bytes_per_launch"),
+                    "fp64_pipe_util_ncu": prof.get("fp64_pipe_pct"), "ncu_capture": prof.get("capture")}
         if cpu:
             out[cfg]["cpu_oracle"] = _oracle_rates(mech, batch, 2048)
         gm.close()
