@@ -251,7 +251,8 @@ def run_ours(args):
         blocks.append((hin, hout, din, dout))
     h2d = sum(b[0].numel() * 8 for b in blocks)
     d2h = sum(b[1].numel() * 8 for b in blocks)
-    side = [torch.cuda.Stream() for _ in range(3)]
+    # three streams on one handle: allowed for the resident kernel only (psr.h, "Overlap on the GPU")
+    side = [torch.cuda.Stream() for _ in range(3 if info["eval_kernel"] == 1 else 1)]
 
     def e2e_step():
         start = torch.cuda.Event()

@@ -23,6 +23,12 @@
  * Execution: every psr_eval_* / psr_fd_jacobian call enqueues kernels on `stream` (a cudaStream_t
  * cast to void*, NULL = legacy default stream) of the current device and returns without
  * synchronising.  Calls on one psr_mech from several host threads must be serialised by the caller.
+ * Overlap on the GPU: a mechanism handle owns device scratch that some kernels use (the per-CTA rate
+ * constants of the fused Jacobian kernel; the running sums of nu^T q of the large-mechanism evaluation
+ * kernel, psr_mech_info: eval_acc_global = 1; the rate table of the generic Jacobian sweep).  Calls on ONE
+ * handle that may run at the same time on the device -- different streams without an ordering between
+ * them -- therefore race, except psr_eval_wdot / _residual / _kf_kr on a mechanism with eval_kernel = 1
+ * (no scratch).  Order them (one stream, or events), or load the mechanism once per stream.
  *
  * Errors: every call returns a psr_status; on failure nothing was launched and psr_last_error()
  * describes why.  N == 0 is PSR_OK.  Non-finite or negative T/Y are not checked and propagate by
