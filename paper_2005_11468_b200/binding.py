@@ -13,7 +13,7 @@ from . import build as _build
 _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libpsr_b200.so"
 
-OPT_JAC_UNHOISTED, OPT_FUSED_ONLY, OPT_JAC_GENERIC = 1, 2, 3
+OPT_JAC_UNHOISTED, OPT_FUSED_ONLY, OPT_JAC_GENERIC, OPT_NO_TMEM = 1, 2, 3, 4
 PSR_OK, PSR_EINVAL, PSR_EUNSUPPORTED, PSR_ENOMEM, PSR_ECUDA, PSR_EIO = range(6)
 _STATUS = {0: "PSR_OK", 1: "PSR_EINVAL", 2: "PSR_EUNSUPPORTED", 3: "PSR_ENOMEM", 4: "PSR_ECUDA", 5: "PSR_EIO"}
 

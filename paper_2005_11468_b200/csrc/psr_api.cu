@@ -76,6 +76,7 @@ struct psr_mech {
   int32_t* d_jac_col_order = nullptr;
   double* d_jac_scratch = nullptr;
   int opt_fused_only = 0;       // diagnostic (psr_mech_set_option): never take the warp-specialised kernel
+  int opt_no_tmem = 0;          // diagnostic: the resident kernel reads every concentration from shared memory
   int opt_jac_unhoisted = 0;    // diagnostic: every Jacobian column a full evaluation
   int opt_jac_generic = 0;      // diagnostic: psr_fd_jacobian takes the generic three-launch sweep even where the fused kernel applies
   double* d_scratch = nullptr;  // psr_fd_jacobian: rate table [N][I][kRateVals], then F0 when the caller passes none
@@ -707,6 +708,13 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         wv.spw = spw_h;
         wv.need_lnctot = need_lnctot;
         wv.chunk_stride = (uint32_t)wbs.stride;
+        // copies of the two C tiles in tensor memory (512 columns of 32 bits per SM; one CTA per SM)
+        wv.tm_buf = 2 * ((K + 2 + 3) & ~3);
+        wv.tm_cols = 0;
+        if (2 * wv.tm_buf <= 512) {
+          wv.tm_cols = 32;
+          while (wv.tm_cols < 2 * wv.tm_buf) wv.tm_cols *= 2;
+        }
       }
     }
   }
@@ -1108,7 +1116,9 @@ psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
     // whole tiles come by one bulk copy per species row: needs 16-byte aligned rows
     const int bulk_ok = al16(a.T) && al16(a.P) && al16(a.Y) && (a.ld % 2 == 0) && (!wantF || (al16(a.Yin) && al16(a.tau)));
     const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
-    cudaError_t e = launch_ws(m->ws, a, grid, bulk_ok, (cudaStream_t)stream);
+    WsView wv = m->ws;
+    if (m->opt_no_tmem) wv.tm_cols = 0;
+    cudaError_t e = launch_ws(wv, a, grid, bulk_ok, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, fn);
     return PSR_OK;
   }
@@ -1455,6 +1465,7 @@ psr_status psr_mech_set_option(psr_mech* m, int32_t option, int32_t value) {
   switch (option) {
     case PSR_OPT_JAC_UNHOISTED: m->opt_jac_unhoisted = value != 0; return PSR_OK;
     case PSR_OPT_FUSED_ONLY: m->opt_fused_only = value != 0; return PSR_OK;
+    case PSR_OPT_NO_TMEM: m->opt_no_tmem = value != 0; return PSR_OK;
     case PSR_OPT_JAC_GENERIC: m->opt_jac_generic = value != 0; return PSR_OK;
     default: return fail(PSR_EINVAL, "psr_mech_set_option: unknown option %d", (int)option);
   }

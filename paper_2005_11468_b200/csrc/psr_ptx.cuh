@@ -64,6 +64,45 @@ __device__ __forceinline__ void named_bar_sync(int id, int count) {
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// ------------------------------------------------------------------ tensor memory as a per-lane scratchpad
+// TMEM is [128 lanes][512 columns of 32 bits] per SM; warp w of a CTA reaches the 32 lanes of quadrant w % 4, thread
+// l <-> lane 32 (w % 4) + l (.32x32b shape), at a column address that is the same in every thread.  A [row][32 lanes]
+// tile of doubles maps to lane <-> reactor, row r <-> columns 2r, 2r + 1.  Its read path (64 B/clk/SM, 12 clk) is
+// separate from the shared-memory pipe, which is what the reaction loops are short of.
+// Address = (lane << 16) | column.  Whole-warp instructions (.sync.aligned): call them converged.
+__device__ __forceinline__ void tm_alloc(uint32_t* slot_smem, uint32_t ncols) {   // ncols: power of two, 32..512
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot_smem)), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tm_dealloc(uint32_t base, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(ncols) : "memory");
+}
+// four rows (eight columns) of this thread's lane
+__device__ __forceinline__ void tm_st64x4(uint32_t taddr, double v0, double v1, double v2, double v3) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(__double2loint(v0)),
+               "r"(__double2hiint(v0)), "r"(__double2loint(v1)), "r"(__double2hiint(v1)), "r"(__double2loint(v2)),
+               "r"(__double2hiint(v2)), "r"(__double2loint(v3)), "r"(__double2hiint(v3))
+               : "memory");
+}
+// one row of this thread's lane; the registers are valid after tm_wait_ld* only
+struct TmF64 {
+  uint32_t lo, hi;
+  __device__ __forceinline__ double get() const { return __hiloint2double((int)hi, (int)lo); }
+};
+__device__ __forceinline__ void tm_ld64(uint32_t taddr, TmF64& v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(v.lo), "=r"(v.hi) : "r"(taddr));
+}
+// every tcgen05.ld of this thread so far has landed (the registers pass through the statement, so no use of them can
+// be scheduled above it)
+__device__ __forceinline__ void tm_wait_ld4(TmF64& a, TmF64& b, TmF64& c, TmF64& d) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;"
+               : "+r"(a.lo), "+r"(a.hi), "+r"(b.lo), "+r"(b.hi), "+r"(c.lo), "+r"(c.hi), "+r"(d.lo), "+r"(d.hi)::"memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// order this thread's tcgen05 operations against a barrier / mbarrier operation that follows (before) or precedes (after)
+__device__ __forceinline__ void tm_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tm_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
 // ------------------------------------------------------------------ bounds checks of the -DPSR_CHECK build
 // compute-sanitizer is refused on the GPU pool this library is developed on.  In its place the
 // PSR_CHECK build asserts, on the device, every shared-memory offset the kernels take from the mechanism tables and

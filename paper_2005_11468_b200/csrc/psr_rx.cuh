@@ -23,6 +23,7 @@ struct RxCtx {
   uint32_t c_lane;      // this lane's column of row 0 of the C tile (shared-memory address); row K: ones, K+1: zeros
   uint32_t ctot_lane;   // this lane's C_tot, shared-memory address
   uint32_t lnctot_lane; // this lane's ln C_tot
+  uint32_t tm_c;        // MODE & kRxTm: tensor-memory address of row 0 of a copy of the C tile (this warp's quadrant)
   ExpTab etab;
   float amax;           // NaN-propagating running max of |high word| of the exp arguments of this lane
 #ifdef PSR_CHECK
@@ -31,12 +32,17 @@ struct RxCtx {
 };
 
 // One record class of warp w's share of a chunk.  CLS: 0..3 = reaction type in the 3+3 slot form, kClsLong = long
-// factor lists (any type, signs of A).  FAST: table exp, range noted in cx.amax; else the library exp.
+// factor lists (any type, signs of A).  MODE & kRxFast: table exp, range noted in cx.amax; else the library exp.
+// MODE & kRxTm: the first two factors of each side of a 3+3 record come from the copy of the C tile in tensor memory
+// (cx.tm_c) instead of shared memory -- four of a record's six row reads leave the shared-memory pipe; asked for at
+// the top of a trip, waited for at its end.
 // sink(kl, meta, korig, type, kf, kr, pf, pr, M): effective rate constants (falloff applied), the concentration
 // products of the two sides WITHOUT [M], and [M] (1 for a plain reaction) of record kl.
-template <int CLS, bool FAST, class Sink>
+constexpr int kRxFast = 1, kRxTm = 2;
+template <int CLS, int MODE, class Sink>
 __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blob, const ChunkHdr* hdr, const RxRec* recs,
                                              const int kl_begin, const int kl_end, Sink&& sink) {
+  constexpr bool FAST = (MODE & kRxFast) != 0, TM = (MODE & kRxTm) != 0 && CLS < kClsLong;
   PSR_CHK(kl_begin >= 0 && kl_begin <= kl_end && kl_end <= (int)hdr->n_rx, 101);
   if (kl_begin >= kl_end) return;   // nothing of this class for this warp in this chunk (the rule in small parts)
   auto exps = [&](auto& ex, auto& ey) {
@@ -74,15 +80,27 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
     const double pn = fma(fma(fma(rec->d[3], T, rec->d[2]), T, rec->d[1]), T, rec->d[0]);
     const double lnkr = fma(pn, T, fma(rec->e[1], lnT, fma(rec->e[2], invT, rec->e[0])));
     double pf, pr, kf = 0.0, kr = 0.0, Mout = 1.0;
+    TmF64 tf0, tf1, tp0, tp1;
+    (void)tf0, (void)tf1, (void)tp0, (void)tp1;
 
     // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
     if constexpr (CLS < kClsLong) {
       PSR_CHK(ra_.y < cx.chk_c_bytes && ra_.z < cx.chk_c_bytes && ra_.w < cx.chk_c_bytes && rb_.x < cx.chk_c_bytes &&
                   rb_.y < cx.chk_c_bytes && rb_.z < cx.chk_c_bytes && ((ra_.y | ra_.z | ra_.w | rb_.x | rb_.y | rb_.z) % kRowBytes) == 0, 102);
-      const double f0 = lds64(cx.c_lane + ra_.y), f1 = lds64(cx.c_lane + ra_.z), f2 = lds64(cx.c_lane + ra_.w);
-      const double p0 = lds64(cx.c_lane + rb_.x), p1 = lds64(cx.c_lane + rb_.y), p2 = lds64(cx.c_lane + rb_.z);
-      pf = f0 * f1 * f2;
-      pr = p0 * p1 * p2;
+      if constexpr (TM) {
+        // row offsets are multiples of kRowBytes = 256: row r <-> columns 2r, 2r + 1
+        tm_ld64(cx.tm_c + (ra_.y >> 7), tf0);
+        tm_ld64(cx.tm_c + (ra_.z >> 7), tf1);
+        tm_ld64(cx.tm_c + (rb_.x >> 7), tp0);
+        tm_ld64(cx.tm_c + (rb_.y >> 7), tp1);
+        pf = lds64(cx.c_lane + ra_.w);
+        pr = lds64(cx.c_lane + rb_.z);
+      } else {
+        const double f0 = lds64(cx.c_lane + ra_.y), f1 = lds64(cx.c_lane + ra_.z), f2 = lds64(cx.c_lane + ra_.w);
+        const double p0 = lds64(cx.c_lane + rb_.x), p1 = lds64(cx.c_lane + rb_.y), p2 = lds64(cx.c_lane + rb_.z);
+        pf = f0 * f1 * f2;
+        pr = p0 * p1 * p2;
+      }
     } else {
       const uint16_t* fsp = reinterpret_cast<const uint16_t*>(blob + hdr->off_pool) + ra_.y;
       const int nr = (int)((meta >> kMetaNrShift) & 0xF);
@@ -184,11 +202,16 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
         kr = kf * invKc;
       }
     }
+    if constexpr (TM) {
+      tm_wait_ld4(tf0, tf1, tp0, tp1);
+      pf = tf0.get() * tf1.get() * pf;
+      pr = tp0.get() * tp1.get() * pr;
+    }
     sink(kl, meta, rb_.w, type, kf, kr, pf, pr, Mout);
   }
 }
 
-template <bool FAST, class Sink>
+template <int MODE, class Sink>
 __device__ __forceinline__ void rx_run_chunk(RxCtx& cx, const unsigned char* blob, int w, Sink&& sink) {
   const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
   const RxRec* recs = reinterpret_cast<const RxRec*>(blob + sizeof(ChunkHdr));
@@ -201,11 +224,11 @@ __device__ __forceinline__ void rx_run_chunk(RxCtx& cx, const unsigned char* blo
   for (int c = 0; c < kClsLong + 2; ++c) kb[c] = (int)hdr->wb[w][c];
 #pragma unroll
   for (int c = 0; c < kClsLong + 2; ++c) kb[c] = __reduce_min_sync(kFullMask, kb[c]);
-  rx_run_class<0, FAST>(cx, blob, hdr, recs, kb[0], kb[1], sink);
-  rx_run_class<1, FAST>(cx, blob, hdr, recs, kb[1], kb[2], sink);
-  rx_run_class<2, FAST>(cx, blob, hdr, recs, kb[2], kb[3], sink);
-  rx_run_class<3, FAST>(cx, blob, hdr, recs, kb[3], kb[4], sink);
-  rx_run_class<kClsLong, FAST>(cx, blob, hdr, recs, kb[4], kb[5], sink);
+  rx_run_class<0, MODE>(cx, blob, hdr, recs, kb[0], kb[1], sink);
+  rx_run_class<1, MODE>(cx, blob, hdr, recs, kb[1], kb[2], sink);
+  rx_run_class<2, MODE>(cx, blob, hdr, recs, kb[2], kb[3], sink);
+  rx_run_class<3, MODE>(cx, blob, hdr, recs, kb[3], kb[4], sink);
+  rx_run_class<kClsLong, MODE>(cx, blob, hdr, recs, kb[4], kb[5], sink);
 }
 
 }  // namespace psr

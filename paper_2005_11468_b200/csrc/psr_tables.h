@@ -63,9 +63,9 @@ struct __attribute__((aligned(16))) EffEnt {  // 16 bytes
 };
 
 constexpr int kClsLong = 4;      // record classes: 0..3 = PSR_RX_* type in the 3+3 slot form, 4 = long factor lists (any type)
-constexpr int kMaxWarps = 16;
+constexpr int kMaxWarps = 24;
 
-struct __attribute__((aligned(16))) ChunkHdr {  // 240 bytes
+struct __attribute__((aligned(16))) ChunkHdr {  // 336 bytes
   uint32_t n_rx, n_aux, n_eff, rec_base;   // rec_base: mechanism-wide index of the chunk's first record (rate table row)
   uint32_t off_aux, off_eff, off_pool, off_gptr, off_gent;
   uint32_t bytes;         // bytes to copy (multiple of 16)
@@ -73,7 +73,7 @@ struct __attribute__((aligned(16))) ChunkHdr {  // 240 bytes
   // time; a warp's records are contiguous and sorted by class)
   uint16_t wb[kMaxWarps][kClsLong + 2];
 };
-static_assert(sizeof(ChunkHdr) == 240, "ChunkHdr layout");
+static_assert(sizeof(ChunkHdr) == 336, "ChunkHdr layout");
 
 // Gather lists of nu^T (Eq. 4) per chunk: species s adds the q rows gent[gptr[2s] .. gptr[2s+1]) and
 // subtracts gent[gptr[2s+1] .. gptr[2s+2]).  An entry is the byte offset of a row of the q tile;
@@ -103,7 +103,7 @@ struct MechView {
 
 // ---- warp-specialised kernel (psr_ws.cu): 12 reaction warps + 4 helper warps per CTA, the mechanism cut into
 // n_parts resident blobs (same ChunkHdr layout, records dealt to the 12 reaction warps, gather lists per part)
-constexpr int kWsRxWarps = 11, kWsHelpWarps = 5, kWsWarps = kWsRxWarps + kWsHelpWarps;
+constexpr int kWsRxWarps = 13, kWsHelpWarps = 7, kWsWarps = kWsRxWarps + kWsHelpWarps;
 constexpr int kWsStRows = 8;      // per-tile state rows: T, ln T, 1/T, rho, C_tot, ln C_tot, 1/tau, 1/rho
 constexpr int kWsMaxParts = 8;
 // Gather lists of the warp-specialised kernel: one flat stream of 4-entry groups per (part, helper warp), groups
@@ -125,6 +125,8 @@ struct WsView {
   int32_t need_lnctot;
   uint32_t chunk_stride;
   uint32_t smem_cs, smem_ds, smem_q, smem_acc, smem_mech, smem_misc, smem_total;
+  int32_t tm_cols;              // tensor-memory columns to allocate for the copies of the two C tiles (power of two), 0: none
+  int32_t tm_buf;               // columns per tile: 2 per row, rows rounded up to four
 };
 
 // ---- warp-specialised kernel for LARGE mechanisms (psr_wsl.cu): the same roles as psr_ws.cu with what does not fit
@@ -135,7 +137,7 @@ struct WsView {
 // out (part 0 keeps every owned species: its flushes initialise the sums) and every flush takes its target -- the
 // byte offset of the species' row in a [K][32] tile -- from a list in the blob (gptr area):
 //   wb[kWslRxWarps + hw][0..2] = first group, one past the last group, first entry of the target list.
-constexpr int kWslRxWarps = 10, kWslHelpWarps = 6, kWslWarps = kWslRxWarps + kWslHelpWarps;
+constexpr int kWslRxWarps = 12, kWslHelpWarps = 8, kWslWarps = kWslRxWarps + kWslHelpWarps;
 constexpr int kWslMaxParts = 64;
 
 struct WslView {

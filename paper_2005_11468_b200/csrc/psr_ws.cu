@@ -55,7 +55,9 @@ static_assert(sizeof(SpEnt) == 32, "SpEnt layout");
 
 }  // namespace
 
-template <bool OUTK>
+// TM: a copy of each C tile in tensor memory (all four lane quadrants), from which the reaction warps take four of a
+// record's six concentration factors (psr_rx.cuh, kRxTm); mv.tm_cols columns are allocated.
+template <bool OUTK, bool TM>
 __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView mv, const EvalArgs a, const int bulk_ok) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int K = mv.K;
@@ -71,6 +73,7 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
   double* St0 = W_s + Kp;                                          // [2][kWsStRows][32]
   double* tp0 = St0 + 2 * kWsStRows * kTile;                       // [2][3][32]: T, P, tau as loaded
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp0 + 2 * 3 * kTile);
+  uint32_t* tm_slot = reinterpret_cast<uint32_t*>(bars + B_COUNT); // tensor-memory base address (TM)
   int32_t* sp_s = reinterpret_cast<int32_t*>(bars + B_COUNT + 1);  // [helper warps][spw]
   SpEnt* sptab = reinterpret_cast<SpEnt*>(sp_s + ((kWsHelpWarps * mv.spw + 7) & ~7));   // [helper warps][spw]
 
@@ -94,6 +97,7 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     bulk_g2s(smem + mv.smem_mech, mv.chunks, bytes, &bars[B_BLOB]);
   }
   if (w == 0) {
+    if constexpr (TM) tm_alloc(tm_slot, (uint32_t)mv.tm_cols);
     for (int b = 0; b < 2; ++b) {
       Cs0[b * cs_elems + K * kTile + lane] = 1.0;         // unit row: unused factor slots
       Cs0[b * cs_elems + (K + 1) * kTile + lane] = 0.0;   // zero row: product side of an irreversible reaction
@@ -117,7 +121,13 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     sptab[i].goff = (int64_t)s_ * a.ld * 8;
     sptab[i].W = mv.Wm[s_];
   }
+  if constexpr (TM) tm_fence_before_sync();
   __syncthreads();
+  uint32_t tm_quad = 0;   // this warp's quadrant of the allocation, buffer 0; buffer 1 is mv.tm_buf columns further
+  if constexpr (TM) {
+    tm_fence_after_sync();
+    tm_quad = *tm_slot + ((uint32_t)((w & 3) * 32) << 16);
+  }
 
   if (w < kWsRxWarps) {
     // ================================================================== reaction warps
@@ -131,6 +141,10 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += gridDim.x) {
       const int b = lt & 1;
       mbar_wait(&bars[B_FULLC + b], (lt >> 1) & 1);
+      if constexpr (TM) {
+        tm_fence_after_sync();
+        cx.tm_c = tm_quad + (uint32_t)b * (uint32_t)mv.tm_buf;
+      }
       const uint32_t st_lane = smem_u32(St0 + b * kWsStRows * kTile) + lane * 8;
       cx.c_lane = smem_u32(Cs0 + b * cs_elems) + lane * 8;
       cx.ctot_lane = st_lane + ST_CTOT * kRowBytes;
@@ -166,13 +180,14 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
           }
         };
         cx.amax = 0.0f;
-        rx_run_chunk<true>(cx, blob, w, sink);
+        rx_run_chunk<kRxFast | (TM ? kRxTm : 0)>(cx, blob, w, sink);
         // an exp argument out of the table form's range (NaN, Inf, overflow, underflow: never for physical
         // states): this warp repeats its records with the library exp, which keeps IEEE results
-        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<false>(cx, blob, w, sink);
+        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<0>(cx, blob, w, sink);
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[B_FULLQ + qb]);
       }
+      if constexpr (TM) tm_fence_before_sync();   // (every tensor-memory read of the tile has been waited for)
       if (lane == 0) mbar_arrive(&bars[B_EMPTYC + b]);
     }
   } else {
@@ -268,6 +283,23 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
         const double y = Cb[sp * kTile + lane];
         if (wantF) Db[sp * kTile + lane] = y - Db[sp * kTile + lane];
         Cb[sp * kTile + lane] = rho * (y * invW_s[sp]);
+      }
+      if constexpr (TM) {
+        // the finished tile (unit and zero rows included) into tensor memory, once per lane quadrant: four
+        // consecutive warps reach the four quadrants.  Buffer b was released by the reaction warps through empty_C,
+        // which this warp has waited for (issue_loads of this tile).
+        static_assert(kWsHelpWarps >= 4, "four helper warps copy the C tile to the four TMEM quadrants");
+        named_bar_sync(2, kWsHelpWarps * 32);   // every row of the tile is final
+        if (hw < 4) {
+          tm_fence_after_sync();
+          const uint32_t tq = tm_quad + (uint32_t)b * (uint32_t)mv.tm_buf;
+          const int last = K + 1;
+          for (int s4 = 0; s4 <= last; s4 += 4)
+            tm_st64x4(tq + 2u * (uint32_t)s4, Cb[s4 * kTile + lane], Cb[min(s4 + 1, last) * kTile + lane],
+                      Cb[min(s4 + 2, last) * kTile + lane], Cb[min(s4 + 3, last) * kTile + lane]);
+          tm_wait_st();
+          tm_fence_before_sync();
+        }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars[B_FULLC + b]);
@@ -386,6 +418,11 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
       }
     }
   }
+  if constexpr (TM) {
+    tm_fence_before_sync();
+    __syncthreads();   // no warp touches tensor memory any more
+    if (w == 0) tm_dealloc(*tm_slot, (uint32_t)mv.tm_cols);
+  }
 }
 
 // once per process: the kernels' dynamic shared-memory limit raised to the device's (mechanisms of different sizes
@@ -393,14 +430,22 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
 PSR_CHK_TU_READER(chk_read_ws)
 
 cudaError_t ws_set_smem(size_t smem) {
-  cudaError_t e = cudaFuncSetAttribute(psr_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(psr_ws_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_ws_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_ws_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_ws_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   return e;
 }
 
 cudaError_t launch_ws(const WsView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st) {
-  if (a.flags & (kOutKf | kOutKr | kOutQ)) psr_ws_kernel<true><<<grid, kWsWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
-  else psr_ws_kernel<false><<<grid, kWsWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  const bool outk = (a.flags & (kOutKf | kOutKr | kOutQ)) != 0;
+  if (mv.tm_cols > 0) {
+    if (outk) psr_ws_kernel<true, true><<<grid, kWsWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_ws_kernel<false, true><<<grid, kWsWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  } else {
+    if (outk) psr_ws_kernel<true, false><<<grid, kWsWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_ws_kernel<false, false><<<grid, kWsWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  }
   return cudaGetLastError();
 }
 

@@ -386,6 +386,29 @@ def test_C1_full_size_residual_every_reactor(torch_cuda, binding):
     gm.close()
 
 
+@pytest.mark.parametrize("cfg,n", [("C1", 2 * 148 * 32 + 77), ("C0", 333), ("C4", 999)])
+def test_tensor_memory_copy_of_the_tile_changes_no_bit(torch_cuda, binding, cfg, n):
+    """The resident kernel takes four of a record's six concentration factors from a copy of the C tile in tensor
+    memory; PSR_OPT_NO_TMEM reads all six from shared memory.  Same values, same arithmetic: every
+    output agrees to the bit -- over more than two tiles per CTA (both tile buffers reused) and a ragged last tile."""
+    torch = torch_cuda
+    mech, batch = synth.make_config(cfg, n)
+    gm = binding.Mechanism.from_synth(mech)
+    assert gm.info()["eval_kernel"] == 1
+    T, P, Y, Yin, tau = (dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    got = []
+    for no_tmem in (0, 1, 0):
+        gm.set_option(binding.OPT_NO_TMEM, no_tmem)
+        F, w = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+        kf, kr = gm.eval_kf_kr(T, P, Y)
+        got.append([x.cpu().numpy() for x in (F, w, kf, kr)])
+    for a, b in ((0, 1), (0, 2)):
+        for x, y in zip(got[a], got[b]):
+            assert np.array_equal(x, y)
+    assert np.all(np.isfinite(got[0][0]))
+    gm.close()
+
+
 @pytest.mark.parametrize("cfg", ["C2", "C3"])
 def test_large_configs_full_size_every_reactor(torch_cuda, binding, cfg):
     """BASELINE configs 2 and 3 at their full batches through psr_eval_residual (the launches bench.py
