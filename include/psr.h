@@ -241,9 +241,9 @@ psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);
  * column in full instead of reusing the T-only factors of the base state (the two sweeps are bit-identical).
  * PSR_OPT_FUSED_ONLY: psr_eval_wdot / psr_eval_residual / psr_eval_kf_kr take the single fused kernel even
  * where the warp-specialised one applies.  PSR_OPT_JAC_GENERIC: psr_fd_jacobian takes the generic
- * three-launch sweep even where the fused Jacobian kernel applies.  PSR_OPT_NO_TMEM: the resident evaluation kernel
- * (eval_kernel = 1) reads every concentration from shared memory instead of taking part of them from its copy of
- * the tile in tensor memory (bit-identical results).  Not thread-safe against concurrent calls on `mech`. */
+ * three-launch sweep even where the fused Jacobian kernel applies.  PSR_OPT_NO_TMEM: the warp-specialised evaluation
+ * kernels (eval_kernel = 1, 2) read every concentration from shared memory instead of taking the factors of the rate
+ * products from their copy of the tile in tensor memory (bit-identical results).  Not thread-safe against concurrent calls on `mech`. */
 enum { PSR_OPT_JAC_UNHOISTED = 1, PSR_OPT_FUSED_ONLY = 2, PSR_OPT_JAC_GENERIC = 3, PSR_OPT_NO_TMEM = 4 };
 psr_status psr_mech_set_option(psr_mech* mech, int32_t option, int32_t value);
 

@@ -76,7 +76,7 @@ struct psr_mech {
   int32_t* d_jac_col_order = nullptr;
   double* d_jac_scratch = nullptr;
   int opt_fused_only = 0;       // diagnostic (psr_mech_set_option): never take the warp-specialised kernel
-  int opt_no_tmem = 0;          // diagnostic: the resident kernel reads every concentration from shared memory
+  int opt_no_tmem = 0;          // diagnostic: the evaluation kernels read every concentration from shared memory
   int opt_jac_unhoisted = 0;    // diagnostic: every Jacobian column a full evaluation
   int opt_jac_generic = 0;      // diagnostic: psr_fd_jacobian takes the generic three-launch sweep even where the fused kernel applies
   double* d_scratch = nullptr;  // psr_fd_jacobian: rate table [N][I][kRateVals], then F0 when the caller passes none
@@ -755,7 +755,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         lv.smem_mech = (uint32_t)o;
         o += 2 * lbs.stride;
         lv.smem_misc = (uint32_t)o;
-        o += align_up((size_t)2 * Kp * 8 + (size_t)2 * 8 * kRowBytes + (size_t)2 * 3 * kRowBytes + 10 * 8 +
+        o += align_up((size_t)2 * Kp * 8 + (size_t)2 * 8 * kRowBytes + (size_t)2 * 3 * kRowBytes + 12 * 8 +
                           (size_t)kWslHelpWarps * spw_l * 4, 128);
         lv.smem_total = (uint32_t)o;
         if (o <= (size_t)prop.sharedMemPerBlockOptin) {
@@ -768,6 +768,12 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
           lv.need_lnctot = need_lnctot;
           lv.acc_global = acc_global;
           lv.chunk_stride = (uint32_t)lbs.stride;
+          // a copy of the C tile in tensor memory (512 columns of 32 bits per SM, two per row)
+          lv.tm_cols = 0;
+          if (2 * ((K + 2 + 3) & ~3) <= 512) {
+            lv.tm_cols = 32;
+            while (lv.tm_cols < 2 * ((K + 2 + 3) & ~3)) lv.tm_cols *= 2;
+          }
         }
       }
     }
@@ -1127,7 +1133,9 @@ psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
     auto al16 = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; };
     const int bulk_ok = al16(a.T) && al16(a.P) && al16(a.Y) && (a.ld % 2 == 0) && (!(a.flags & kOutF) || al16(a.tau));
     const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
-    cudaError_t e = launch_wsl(m->wsl, a, grid, bulk_ok, (cudaStream_t)stream);
+    WslView lv = m->wsl;
+    if (m->opt_no_tmem) lv.tm_cols = 0;
+    cudaError_t e = launch_wsl(lv, a, grid, bulk_ok, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, fn);
     return PSR_OK;
   }

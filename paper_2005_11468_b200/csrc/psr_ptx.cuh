@@ -94,9 +94,10 @@ __device__ __forceinline__ void tm_ld64(uint32_t taddr, TmF64& v) {
 }
 // every tcgen05.ld of this thread so far has landed (the registers pass through the statement, so no use of them can
 // be scheduled above it)
-__device__ __forceinline__ void tm_wait_ld4(TmF64& a, TmF64& b, TmF64& c, TmF64& d) {
+__device__ __forceinline__ void tm_wait_ld6(TmF64& a, TmF64& b, TmF64& c, TmF64& d, TmF64& e, TmF64& f) {
   asm volatile("tcgen05.wait::ld.sync.aligned;"
-               : "+r"(a.lo), "+r"(a.hi), "+r"(b.lo), "+r"(b.hi), "+r"(c.lo), "+r"(c.hi), "+r"(d.lo), "+r"(d.hi)::"memory");
+               : "+r"(a.lo), "+r"(a.hi), "+r"(b.lo), "+r"(b.hi), "+r"(c.lo), "+r"(c.hi), "+r"(d.lo), "+r"(d.hi), "+r"(e.lo),
+                 "+r"(e.hi), "+r"(f.lo), "+r"(f.hi)::"memory");
 }
 __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 // order this thread's tcgen05 operations against a barrier / mbarrier operation that follows (before) or precedes (after)

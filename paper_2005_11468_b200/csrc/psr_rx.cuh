@@ -33,9 +33,9 @@ struct RxCtx {
 
 // One record class of warp w's share of a chunk.  CLS: 0..3 = reaction type in the 3+3 slot form, kClsLong = long
 // factor lists (any type, signs of A).  MODE & kRxFast: table exp, range noted in cx.amax; else the library exp.
-// MODE & kRxTm: the first two factors of each side of a 3+3 record come from the copy of the C tile in tensor memory
-// (cx.tm_c) instead of shared memory -- four of a record's six row reads leave the shared-memory pipe; asked for at
-// the top of a trip, waited for at its end.
+// MODE & kRxTm: the six factors of a 3+3 record come from the copy of the C tile in tensor memory (cx.tm_c) instead
+// of shared memory -- those row reads leave the shared-memory pipe; asked for at the top of a trip, waited for at
+// its end.  (Efficiency lists and long factor lists, of data-dependent length, still read the shared-memory tile.)
 // sink(kl, meta, korig, type, kf, kr, pf, pr, M): effective rate constants (falloff applied), the concentration
 // products of the two sides WITHOUT [M], and [M] (1 for a plain reaction) of record kl.
 constexpr int kRxFast = 1, kRxTm = 2;
@@ -80,8 +80,8 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
     const double pn = fma(fma(fma(rec->d[3], T, rec->d[2]), T, rec->d[1]), T, rec->d[0]);
     const double lnkr = fma(pn, T, fma(rec->e[1], lnT, fma(rec->e[2], invT, rec->e[0])));
     double pf, pr, kf = 0.0, kr = 0.0, Mout = 1.0;
-    TmF64 tf0, tf1, tp0, tp1;
-    (void)tf0, (void)tf1, (void)tp0, (void)tp1;
+    TmF64 tf0, tf1, tf2, tp0, tp1, tp2;
+    (void)tf0, (void)tf1, (void)tf2, (void)tp0, (void)tp1, (void)tp2;
 
     // concentration products (Eq. 5): integer powers by repetition, unused slots read the unit row
     if constexpr (CLS < kClsLong) {
@@ -93,8 +93,8 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
         tm_ld64(cx.tm_c + (ra_.z >> 7), tf1);
         tm_ld64(cx.tm_c + (rb_.x >> 7), tp0);
         tm_ld64(cx.tm_c + (rb_.y >> 7), tp1);
-        pf = lds64(cx.c_lane + ra_.w);
-        pr = lds64(cx.c_lane + rb_.z);
+        tm_ld64(cx.tm_c + (ra_.w >> 7), tf2);
+        tm_ld64(cx.tm_c + (rb_.z >> 7), tp2);
       } else {
         const double f0 = lds64(cx.c_lane + ra_.y), f1 = lds64(cx.c_lane + ra_.z), f2 = lds64(cx.c_lane + ra_.w);
         const double p0 = lds64(cx.c_lane + rb_.x), p1 = lds64(cx.c_lane + rb_.y), p2 = lds64(cx.c_lane + rb_.z);
@@ -203,9 +203,9 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
       }
     }
     if constexpr (TM) {
-      tm_wait_ld4(tf0, tf1, tp0, tp1);
-      pf = tf0.get() * tf1.get() * pf;
-      pr = tp0.get() * tp1.get() * pr;
+      tm_wait_ld6(tf0, tf1, tf2, tp0, tp1, tp2);
+      pf = tf0.get() * tf1.get() * tf2.get();
+      pr = tp0.get() * tp1.get() * tp2.get();
     }
     sink(kl, meta, rb_.w, type, kf, kr, pf, pr, Mout);
   }

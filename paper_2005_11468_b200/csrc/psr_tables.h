@@ -154,6 +154,7 @@ struct WslView {
   int32_t acc_global;
   uint32_t chunk_stride;
   uint32_t smem_cs, smem_acc, smem_q, smem_mech, smem_misc, smem_total;
+  int32_t tm_cols;              // tensor-memory columns to allocate for the copy of the C tile (power of two), 0: none
 };
 
 // ---- fused finite-difference Jacobian kernel (psr_jac.cu): lane <-> reactor, one CTA per tile of 32 reactors.

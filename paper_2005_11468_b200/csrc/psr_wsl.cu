@@ -41,13 +41,17 @@ namespace psr {
 namespace {
 __device__ constexpr double kRgasL = 8.31446261815324e7;  // erg/mol/K
 constexpr int L_RING = 0, L_FULLC = 2, L_EMPTYC = 3, L_FULLQ = 4, L_EMPTYQ = 6, L_IN = 8, L_COUNT = 10;
+constexpr int L_SLOTS = L_COUNT + 2;   // + the tensor-memory base address (8 bytes used of 16)
 constexpr int LS_T = 0, LS_LNT = 1, LS_INVT = 2, LS_CTOT = 3, LS_LNCTOT = 4, LS_INVTAU = 5, LS_INVRHO = 6, LS_ROWS = 8;
 }  // namespace
 
-// The helper warps' side of psr_wsl_kernel (every thread of warps kWslRxWarps.. calls it).
+// The helper warps' side of psr_wsl_kernel (every thread of warps kWslRxWarps.. calls it).  TM: a finished C tile is
+// also copied to tensor memory, once per lane quadrant (tm_quad: this warp's quadrant of the allocation), as in psr_ws.cu.
+template <bool TM>
 __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArgs& a, double* Cs, double* acc_s, double* qh0,
                                                 unsigned char* ring, const double* invW_s, const double* W_s, double* St0,
-                                                double* tp0, uint64_t* bars, const int32_t* sp_s, uint32_t total_parts, const int bulk_ok) {
+                                                double* tp0, uint64_t* bars, const int32_t* sp_s, uint32_t total_parts, const int bulk_ok,
+                                                const uint32_t tm_quad) {
   const int lane = threadIdx.x & 31, hw = (threadIdx.x >> 5) - kWslRxWarps;
   const int K = mv.K, q_elems = (mv.rc + 1) * kTile;
   const bool wantF = (a.flags & kOutF) != 0, out_w = (a.flags & kOutWdot) != 0;
@@ -124,6 +128,20 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
     for (int jj = 0; jj < n_my; ++jj) {
       const int sp = my_sp[jj];
       Cs[sp * kTile + lane] = rho * (Cs[sp * kTile + lane] * invW_s[sp]);
+    }
+    if constexpr (TM) {
+      // (the reaction warps released the tile through empty_C, which this warp waited for before this call)
+      static_assert(kWslHelpWarps >= 4, "four helper warps copy the C tile to the four TMEM quadrants");
+      named_bar_sync(2, kWslHelpWarps * 32);   // every row of the tile is final
+      if (hw < 4) {
+        tm_fence_after_sync();
+        const int last = K + 1;
+        for (int s4 = 0; s4 <= last; s4 += 4)
+          tm_st64x4(tm_quad + 2u * (uint32_t)s4, Cs[s4 * kTile + lane], Cs[min(s4 + 1, last) * kTile + lane],
+                    Cs[min(s4 + 2, last) * kTile + lane], Cs[min(s4 + 3, last) * kTile + lane]);
+        tm_wait_st();
+        tm_fence_before_sync();
+      }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&bars[L_FULLC]);
@@ -286,7 +304,7 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
   }
 }
 
-template <bool OUTK>
+template <bool OUTK, bool TM>
 __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslView mv, const EvalArgs a, const int bulk_ok) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int K = mv.K;
@@ -301,7 +319,8 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
   double* St0 = W_s + Kp;                                           // [2][LS_ROWS][32]: state rows, by tile parity
   double* tp0 = St0 + 2 * LS_ROWS * kTile;                          // [2][3][32]: T, P, tau as loaded
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp0 + 2 * 3 * kTile);
-  int32_t* sp_s = reinterpret_cast<int32_t*>(bars + L_COUNT);       // [helper warps][spw]
+  uint32_t* tm_slot = reinterpret_cast<uint32_t*>(bars + L_COUNT);  // tensor-memory base address (TM)
+  int32_t* sp_s = reinterpret_cast<int32_t*>(bars + L_SLOTS);       // [helper warps][spw]
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -328,6 +347,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
     }
   }
   if (w == 0) {
+    if constexpr (TM) tm_alloc(tm_slot, (uint32_t)mv.tm_cols);
     Cs[K * kTile + lane] = 1.0;         // unit row: unused factor slots
     Cs[(K + 1) * kTile + lane] = 0.0;   // zero row: product side of an irreversible reaction
     for (int b = 0; b < 2; ++b) qh0[b * q_elems + mv.rc * kTile + lane] = 0.0;   // zero row: padding of the gather streams
@@ -337,19 +357,27 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
     W_s[i] = mv.Wm[i];
   }
   for (int i = threadIdx.x; i < kWslHelpWarps * mv.spw; i += kWslWarps * 32) sp_s[i] = mv.sp_of[i];
+  if constexpr (TM) tm_fence_before_sync();
   __syncthreads();
+  uint32_t tm_quad = 0;   // this warp's quadrant of the copy of the C tile in tensor memory
+  if constexpr (TM) {
+    tm_fence_after_sync();
+    tm_quad = *tm_slot + ((uint32_t)((w & 3) * 32) << 16);
+  }
 
   if (w < kWslRxWarps) {
     // ================================================================== reaction warps
     RxCtx cx;
     cx.etab = exp_tab_load(mv.exp_tab);
     cx.c_lane = smem_u32(Cs) + lane * 8;
+    cx.tm_c = tm_quad;
 #ifdef PSR_CHECK
     cx.chk_c_bytes = (uint32_t)(K + 2) * kRowBytes;
 #endif
     int64_t tile = blockIdx.x;
     for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += gridDim.x) {
       mbar_wait(&bars[L_FULLC], lt & 1);
+      if constexpr (TM) tm_fence_after_sync();
       const uint32_t st_lane = smem_u32(St0 + (lt & 1) * LS_ROWS * kTile) + lane * 8;
       cx.ctot_lane = st_lane + LS_CTOT * kRowBytes;
       cx.lnctot_lane = st_lane + LS_LNCTOT * kRowBytes;
@@ -386,31 +414,45 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
           }
         };
         cx.amax = 0.0f;
-        rx_run_chunk<true>(cx, blob, w, sink);
+        rx_run_chunk<kRxFast | (TM ? kRxTm : 0)>(cx, blob, w, sink);
         // an exp argument out of the table form's range: this warp repeats its records with the library exp
-        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<false>(cx, blob, w, sink);
+        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<0>(cx, blob, w, sink);
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[L_FULLQ + qb]);
       }
+      if constexpr (TM) tm_fence_before_sync();   // (every tensor-memory read of the tile has been waited for)
       if (lane == 0) mbar_arrive(&bars[L_EMPTYC]);
     }
-    return;
+  } else {
+    // ================================================================== helper warps: see above
+    psr_wsl_helpers<TM>(mv, a, Cs, acc_s, qh0, ring, invW_s, W_s, St0, tp0, bars, sp_s, total_parts, bulk_ok, tm_quad);
   }
-  // ==================================================================== helper warps: see below
-  psr_wsl_helpers(mv, a, Cs, acc_s, qh0, ring, invW_s, W_s, St0, tp0, bars, sp_s, total_parts, bulk_ok);
+  if constexpr (TM) {
+    tm_fence_before_sync();
+    __syncthreads();   // no warp touches tensor memory any more
+    if (w == 0) tm_dealloc(*tm_slot, (uint32_t)mv.tm_cols);
+  }
 }
 
 PSR_CHK_TU_READER(chk_read_wsl)
 
 cudaError_t wsl_set_smem(size_t smem) {
-  cudaError_t e = cudaFuncSetAttribute(psr_wsl_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(psr_wsl_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   return e;
 }
 
 cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st) {
-  if (a.flags & (kOutKf | kOutKr | kOutQ)) psr_wsl_kernel<true><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
-  else psr_wsl_kernel<false><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  const bool outk = (a.flags & (kOutKf | kOutKr | kOutQ)) != 0;
+  if (mv.tm_cols > 0) {
+    if (outk) psr_wsl_kernel<true, true><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_wsl_kernel<false, true><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  } else {
+    if (outk) psr_wsl_kernel<true, false><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_wsl_kernel<false, false><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  }
   return cudaGetLastError();
 }
 

@@ -386,15 +386,17 @@ def test_C1_full_size_residual_every_reactor(torch_cuda, binding):
     gm.close()
 
 
-@pytest.mark.parametrize("cfg,n", [("C1", 2 * 148 * 32 + 77), ("C0", 333), ("C4", 999)])
-def test_tensor_memory_copy_of_the_tile_changes_no_bit(torch_cuda, binding, cfg, n):
-    """The resident kernel takes four of a record's six concentration factors from a copy of the C tile in tensor
-    memory; PSR_OPT_NO_TMEM reads all six from shared memory.  Same values, same arithmetic: every
-    output agrees to the bit -- over more than two tiles per CTA (both tile buffers reused) and a ragged last tile."""
+@pytest.mark.parametrize("cfg,n,kernel", [("C1", 2 * 148 * 32 + 77, 1), ("C0", 333, 1), ("C4", 999, 1), ("C2", 2 * 148 * 32 + 5, 2),
+                                          ("C3", 70, 2)])
+def test_tensor_memory_copy_of_the_tile_changes_no_bit(torch_cuda, binding, cfg, n, kernel):
+    """The warp-specialised kernels take the six concentration factors of a 3+3 record from a copy of the C tile in
+    tensor memory; PSR_OPT_NO_TMEM reads them from shared memory.  Same values, same arithmetic: every
+    output agrees to the bit -- over more than two tiles per CTA (tile buffers reused) and a ragged last tile.  (C3:
+    500 species do not fit the 512 columns; the switch changes nothing there.)"""
     torch = torch_cuda
     mech, batch = synth.make_config(cfg, n)
     gm = binding.Mechanism.from_synth(mech)
-    assert gm.info()["eval_kernel"] == 1
+    assert gm.info()["eval_kernel"] == kernel
     T, P, Y, Yin, tau = (dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
     got = []
     for no_tmem in (0, 1, 0):
