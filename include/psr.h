@@ -231,7 +231,8 @@ typedef struct {
   int32_t eval_kernel;   /* kernel of psr_eval_wdot / _residual / _kf_kr: 0 general fused, 1 warp-specialised (resident
                             tables), 2 warp-specialised for large mechanisms (streamed parts) */
   int32_t eval_parts;    /* parts the mechanism is cut into for that kernel */
-  int32_t eval_acc_global; /* kernel 2: running sums of nu^T q in an L2-resident scratch instead of shared memory */
+  int32_t eval_acc_global; /* kernel 2: where the running sums of nu^T q live: 0 shared memory, 1 an L2-resident scratch
+                              of the handle, 2 tensor memory */
   int32_t jac_kernel;    /* psr_fd_jacobian: 1 fused Jacobian kernel, 0 generic sweep */
 } psr_mech_info_t;
 psr_status psr_mech_info(const psr_mech* mech, psr_mech_info_t* info);

@@ -33,7 +33,7 @@ cudaError_t chk_read_ws(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_jac(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_wsl(unsigned int* count, unsigned int* first_code);
 cudaError_t wsl_set_smem(size_t smem);
-cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st);
+cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, int rx_tmem, cudaStream_t st);
 cudaError_t launch_chk_selftest(cudaStream_t st);
 cudaError_t jac_set_smem(size_t smem);
 cudaError_t launch_jac(const JacView& jv, const EvalArgs& a, int grid, cudaStream_t st);
@@ -736,8 +736,17 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     // the sums in shared memory only when that leaves room for parts so large that at most 4 are needed (P5: 0.099 ms
     // against 0.105 with the sums in L2); beyond that the tile's worth of shared memory is better spent on larger
     // parts (measured: C2 0.522 ms with 8 parts and the sums in L2, 0.538 with 11 parts and the sums in shared memory)
-    for (int acc_global = 0; acc_global < 2 && !wsl_ok; ++acc_global) {
-      wb.tuples = acc_global != 0;
+    // Third place for the sums: tensor memory, beside the copy of the C tile (psr_wsl.cu) -- a helper warp's species in
+    // its own lane quadrant, two warps per quadrant -- when both fit the 512 columns (K <= 200).  Parts as large as with
+    // the sums in L2, the group streams of the shared-memory variant, and no red.global traffic through the LSU queue
+    // the reaction warps' shared-memory loads go through.
+    const int tm_tile_cols = 2 * ((K + 2 + 3) & ~3);
+    const int tm_acc_cols = 2 * ((kWslHelpWarps + 3) / 4) * spw_l;
+    const int acc_modes[3] = {0, 2, 1};
+    for (int mi = 0; mi < 3 && !wsl_ok; ++mi) {
+      const int acc_global = acc_modes[mi];
+      if (acc_global == 2 && tm_tile_cols + tm_acc_cols > 512) continue;
+      wb.tuples = acc_global == 1;
       for (int n_parts = 2; n_parts <= (acc_global ? kWslMaxParts : 4) && n_parts <= I && !wsl_ok; ++n_parts) {
         const int rc_l = (I + n_parts - 1) / n_parts;
         // (a quick bound before building the blobs: the q buffers alone)
@@ -756,7 +765,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         o += 2 * lbs.stride;
         lv.smem_misc = (uint32_t)o;
         o += align_up((size_t)2 * Kp * 8 + (size_t)2 * 8 * kRowBytes + (size_t)2 * 3 * kRowBytes + 12 * 8 +
-                          (size_t)kWslHelpWarps * spw_l * 4, 128);
+                          (size_t)kWslHelpWarps * spw_l * 4 + (size_t)K * 2, 128);
         lv.smem_total = (uint32_t)o;
         if (o <= (size_t)prop.sharedMemPerBlockOptin) {
           wsl_ok = true;
@@ -770,9 +779,11 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
           lv.chunk_stride = (uint32_t)lbs.stride;
           // a copy of the C tile in tensor memory (512 columns of 32 bits per SM, two per row)
           lv.tm_cols = 0;
-          if (2 * ((K + 2 + 3) & ~3) <= 512) {
+          lv.tm_acc_col = tm_tile_cols;
+          const int tm_need = tm_tile_cols + (acc_global == 2 ? tm_acc_cols : 0);
+          if (tm_need <= 512) {
             lv.tm_cols = 32;
-            while (lv.tm_cols < 2 * ((K + 2 + 3) & ~3)) lv.tm_cols *= 2;
+            while (lv.tm_cols < tm_need) lv.tm_cols *= 2;
           }
         }
       }
@@ -1014,7 +1025,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     m->jac_ok = true;
   }
   if (wsl_ok) {
-    const size_t acc_bytes = lv.acc_global ? (size_t)prop.multiProcessorCount * (K + 1) * kRowBytes : 256;   // + a spare row
+    const size_t acc_bytes = lv.acc_global == 1 ? (size_t)prop.multiProcessorCount * (K + 1) * kRowBytes : 256;   // + a spare row
     if ((e = cudaMalloc(&m->d_wsl_chunks, lbs.all.size())) != cudaSuccess ||
         (e = cudaMemcpy(m->d_wsl_chunks, lbs.all.data(), lbs.all.size(), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMalloc(&m->d_wsl_sp_of, 4 * wsl_sp_of.size())) != cudaSuccess ||
@@ -1133,9 +1144,7 @@ psr_status run(const psr_mech* m, EvalArgs& a, void* stream, const char* fn) {
     auto al16 = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; };
     const int bulk_ok = al16(a.T) && al16(a.P) && al16(a.Y) && (a.ld % 2 == 0) && (!(a.flags & kOutF) || al16(a.tau));
     const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
-    WslView lv = m->wsl;
-    if (m->opt_no_tmem) lv.tm_cols = 0;
-    cudaError_t e = launch_wsl(lv, a, grid, bulk_ok, (cudaStream_t)stream);
+    cudaError_t e = launch_wsl(m->wsl, a, grid, bulk_ok, m->opt_no_tmem ? 0 : 1, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, fn);
     return PSR_OK;
   }

@@ -84,6 +84,9 @@ __device__ __forceinline__ void tm_st64x4(uint32_t taddr, double v0, double v1, 
                "r"(__double2hiint(v2)), "r"(__double2loint(v3)), "r"(__double2hiint(v3))
                : "memory");
 }
+__device__ __forceinline__ void tm_st64(uint32_t taddr, double v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__double2loint(v)), "r"(__double2hiint(v)) : "memory");
+}
 // one row of this thread's lane; the registers are valid after tm_wait_ld* only
 struct TmF64 {
   uint32_t lo, hi;
@@ -98,6 +101,9 @@ __device__ __forceinline__ void tm_wait_ld6(TmF64& a, TmF64& b, TmF64& c, TmF64&
   asm volatile("tcgen05.wait::ld.sync.aligned;"
                : "+r"(a.lo), "+r"(a.hi), "+r"(b.lo), "+r"(b.hi), "+r"(c.lo), "+r"(c.hi), "+r"(d.lo), "+r"(d.hi), "+r"(e.lo),
                  "+r"(e.hi), "+r"(f.lo), "+r"(f.hi)::"memory");
+}
+__device__ __forceinline__ void tm_wait_ld1(TmF64& a) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(a.lo), "+r"(a.hi)::"memory");
 }
 __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 // order this thread's tcgen05 operations against a barrier / mbarrier operation that follows (before) or precedes (after)

@@ -151,10 +151,12 @@ struct WslView {
   int32_t n_parts, rc;
   int32_t spw;
   int32_t need_lnctot;
-  int32_t acc_global;
+  int32_t acc_global;           // where the running sums of nu^T q live: 0 shared memory, 1 L2-resident scratch (acc_g), 2 tensor memory
   uint32_t chunk_stride;
   uint32_t smem_cs, smem_acc, smem_q, smem_mech, smem_misc, smem_total;
-  int32_t tm_cols;              // tensor-memory columns to allocate for the copy of the C tile (power of two), 0: none
+  int32_t tm_cols;              // tensor-memory columns to allocate (power of two), 0: none
+  int32_t tm_acc_col;           // acc_global == 2: first column of the running sums (after the copy of the C tile);
+                                // helper warp hw, owned species number jj: columns tm_acc_col + 2 ((hw / 4) spw + jj) of its quadrant
 };
 
 // ---- fused finite-difference Jacobian kernel (psr_jac.cu): lane <-> reactor, one CTA per tile of 32 reactors.

@@ -47,18 +47,21 @@ constexpr int LS_T = 0, LS_LNT = 1, LS_INVT = 2, LS_CTOT = 3, LS_LNCTOT = 4, LS_
 
 // The helper warps' side of psr_wsl_kernel (every thread of warps kWslRxWarps.. calls it).  TM: a finished C tile is
 // also copied to tensor memory, once per lane quadrant (tm_quad: this warp's quadrant of the allocation), as in psr_ws.cu.
-template <bool TM>
+template <int TMODE>
 __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArgs& a, double* Cs, double* acc_s, double* qh0,
                                                 unsigned char* ring, const double* invW_s, const double* W_s, double* St0,
                                                 double* tp0, uint64_t* bars, const int32_t* sp_s, uint32_t total_parts, const int bulk_ok,
-                                                const uint32_t tm_quad) {
+                                                const uint32_t tm_quad, const uint16_t* slot_s) {
+  constexpr bool TM = TMODE != 0;   // tensor memory allocated: the copy of the C tile is kept there
   const int lane = threadIdx.x & 31, hw = (threadIdx.x >> 5) - kWslRxWarps;
   const int K = mv.K, q_elems = (mv.rc + 1) * kTile;
   const bool wantF = (a.flags & kOutF) != 0, out_w = (a.flags & kOutWdot) != 0;
   const int32_t* my_sp = sp_s + hw * mv.spw;
   int n_my = 0;
   while (n_my < mv.spw && my_sp[n_my] >= 0) ++n_my;   // owned species come first, -1 pads the list
-  const bool accg = mv.acc_global != 0;
+  const bool accg = mv.acc_global == 1;
+  const bool acct = TM && mv.acc_global == 2;   // the running sums of this warp's species in tensor memory, its own quadrant
+  const uint32_t tm_acc = tm_quad + (uint32_t)mv.tm_acc_col + 2u * (uint32_t)((hw >> 2) * mv.spw);
   char* accg_lane = reinterpret_cast<char*>(mv.acc_g + (size_t)blockIdx.x * (K + 1) * kTile + lane);   // row s at + s * kRowBytes; row K: spare
   const uint32_t acc_lane = smem_u32(acc_s) + lane * 8;
 
@@ -164,12 +167,32 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       asm volatile("ld.shared.u32 %0, [%1];" : "=r"(off) : "r"(dst));
       dst += 4;
       PSR_CHK(off < (uint32_t)K * kRowBytes && off % kRowBytes == 0, 503);   // a row of the [K][32] running sums
+      if constexpr (TM) {
+        if (acct) {
+          // (one flush per species and part: the round trip through tensor memory is not on the stream's critical path)
+          const uint32_t col = tm_acc + 2u * (uint32_t)slot_s[off / kRowBytes];
+          PSR_CHK(slot_s[off / kRowBytes] < mv.spw, 507);
+          if (FIRST) {
+            tm_st64(col, acc);
+          } else {
+            TmF64 t;
+            tm_ld64(col, t);
+            tm_wait_ld1(t);
+            tm_st64(col, t.get() + acc);
+          }
+          acc = 0.0;
+          return;
+        }
+      }
       const uint32_t addr = acc_lane + off;   // (sums in shared memory; in global memory: gather_tuples)
       sts64(addr, FIRST ? acc : lds64(addr) + acc);
       acc = 0.0;
     };
     const uint32_t qmax = (uint32_t)q_elems * 8u;
     (void)qmax;
+    if constexpr (TM) {
+      if (acct && !FIRST) tm_wait_st();   // the sums the previous part stored have landed
+    }
     uint4 oa, ob;
     ld_group(gs, oa);
     ld_group(gs + 16, ob);
@@ -239,13 +262,23 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
     const double* St = St0 + (lt & 1) * LS_ROWS * kTile;
     const double invtau = wantF ? St[LS_INVTAU * kTile + lane] : 0.0, invrho = wantF ? St[LS_INVRHO * kTile + lane] : 0.0;
     constexpr int EU = 8;   // rows in flight
+    if constexpr (TM) {
+      if (acct) tm_wait_st();
+    }
     for (int jj = 0; jj < n_my; jj += EU) {
       double tot[EU], y[EU], yin[EU];
       int sp[EU];
 #pragma unroll
       for (int u = 0; u < EU; ++u) {
         sp[u] = my_sp[min(jj + u, n_my - 1)];
-        tot[u] = accg ? __ldcg(reinterpret_cast<const double*>(accg_lane + (size_t)sp[u] * kRowBytes)) : acc_s[sp[u] * kTile + lane];
+        if (TM && acct) {
+          TmF64 t;
+          tm_ld64(tm_acc + 2u * (uint32_t)min(jj + u, n_my - 1), t);
+          tm_wait_ld1(t);
+          tot[u] = t.get();
+        } else {
+          tot[u] = accg ? __ldcg(reinterpret_cast<const double*>(accg_lane + (size_t)sp[u] * kRowBytes)) : acc_s[sp[u] * kTile + lane];
+        }
         y[u] = wantF ? ldg_nc(a.Y + (int64_t)sp[u] * a.ld + rcl) : 0.0;
         yin[u] = wantF ? ldg_nc(a.Yin + (int64_t)sp[u] * a.ld + rcl) : 0.0;
       }
@@ -304,9 +337,13 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
   }
 }
 
-template <bool OUTK, bool TM>
+// TMODE: 0 no tensor memory; 1 the copy of the C tile there, read by the reaction warps (and the running sums, if
+// mv.acc_global == 2); 2 the same allocation but the reaction warps read shared memory (PSR_OPT_NO_TMEM on a
+// mechanism whose sums live in tensor memory).
+template <bool OUTK, int TMODE>
 __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslView mv, const EvalArgs a, const int bulk_ok) {
   extern __shared__ __align__(128) unsigned char smem[];
+  constexpr bool TM = TMODE != 0, RXTM = TMODE == 1;
   const int K = mv.K;
   const int q_elems = (mv.rc + 1) * kTile;
   double* Cs = reinterpret_cast<double*>(smem + mv.smem_cs);        // [K+2][32]; rows K, K+1: ones, zeros
@@ -321,6 +358,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp0 + 2 * 3 * kTile);
   uint32_t* tm_slot = reinterpret_cast<uint32_t*>(bars + L_COUNT);  // tensor-memory base address (TM)
   int32_t* sp_s = reinterpret_cast<int32_t*>(bars + L_SLOTS);       // [helper warps][spw]
+  uint16_t* slot_s = reinterpret_cast<uint16_t*>(sp_s + kWslHelpWarps * mv.spw);   // [K]: species -> its number in its owner's list
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -356,7 +394,11 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
     invW_s[i] = mv.invW[i];
     W_s[i] = mv.Wm[i];
   }
-  for (int i = threadIdx.x; i < kWslHelpWarps * mv.spw; i += kWslWarps * 32) sp_s[i] = mv.sp_of[i];
+  for (int i = threadIdx.x; i < kWslHelpWarps * mv.spw; i += kWslWarps * 32) {
+    const int sp = mv.sp_of[i];
+    sp_s[i] = sp;
+    if (sp >= 0) slot_s[sp] = (uint16_t)(i % mv.spw);
+  }
   if constexpr (TM) tm_fence_before_sync();
   __syncthreads();
   uint32_t tm_quad = 0;   // this warp's quadrant of the copy of the C tile in tensor memory
@@ -414,7 +456,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
           }
         };
         cx.amax = 0.0f;
-        rx_run_chunk<kRxFast | (TM ? kRxTm : 0)>(cx, blob, w, sink);
+        rx_run_chunk<kRxFast | (RXTM ? kRxTm : 0)>(cx, blob, w, sink);
         // an exp argument out of the table form's range: this warp repeats its records with the library exp
         if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<0>(cx, blob, w, sink);
         __syncwarp();
@@ -425,7 +467,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
     }
   } else {
     // ================================================================== helper warps: see above
-    psr_wsl_helpers<TM>(mv, a, Cs, acc_s, qh0, ring, invW_s, W_s, St0, tp0, bars, sp_s, total_parts, bulk_ok, tm_quad);
+    psr_wsl_helpers<TMODE>(mv, a, Cs, acc_s, qh0, ring, invW_s, W_s, St0, tp0, bars, sp_s, total_parts, bulk_ok, tm_quad, slot_s);
   }
   if constexpr (TM) {
     tm_fence_before_sync();
@@ -437,21 +479,29 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
 PSR_CHK_TU_READER(chk_read_wsl)
 
 cudaError_t wsl_set_smem(size_t smem) {
-  cudaError_t e = cudaFuncSetAttribute(psr_wsl_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(psr_wsl_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  return e;
+  const void* fns[] = {(const void*)psr_wsl_kernel<false, 0>, (const void*)psr_wsl_kernel<true, 0>, (const void*)psr_wsl_kernel<false, 1>,
+                       (const void*)psr_wsl_kernel<true, 1>,  (const void*)psr_wsl_kernel<false, 2>, (const void*)psr_wsl_kernel<true, 2>};
+  for (const void* f : fns) {
+    cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
-cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, cudaStream_t st) {
+// rx_tmem: the reaction warps read the tensor-memory copy of the C tile (0: PSR_OPT_NO_TMEM)
+cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, int rx_tmem, cudaStream_t st) {
   const bool outk = (a.flags & (kOutKf | kOutKr | kOutQ)) != 0;
-  if (mv.tm_cols > 0) {
-    if (outk) psr_wsl_kernel<true, true><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
-    else psr_wsl_kernel<false, true><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+  const int tmode = mv.tm_cols <= 0 ? 0 : rx_tmem ? 1 : mv.acc_global == 2 ? 2 : 0;
+  const int nt = kWslWarps * 32;
+  if (tmode == 1) {
+    if (outk) psr_wsl_kernel<true, 1><<<grid, nt, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_wsl_kernel<false, 1><<<grid, nt, mv.smem_total, st>>>(mv, a, bulk_ok);
+  } else if (tmode == 2) {
+    if (outk) psr_wsl_kernel<true, 2><<<grid, nt, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_wsl_kernel<false, 2><<<grid, nt, mv.smem_total, st>>>(mv, a, bulk_ok);
   } else {
-    if (outk) psr_wsl_kernel<true, false><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
-    else psr_wsl_kernel<false, false><<<grid, kWslWarps * 32, mv.smem_total, st>>>(mv, a, bulk_ok);
+    if (outk) psr_wsl_kernel<true, 0><<<grid, nt, mv.smem_total, st>>>(mv, a, bulk_ok);
+    else psr_wsl_kernel<false, 0><<<grid, nt, mv.smem_total, st>>>(mv, a, bulk_ok);
   }
   return cudaGetLastError();
 }
