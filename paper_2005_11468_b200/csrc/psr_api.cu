@@ -153,6 +153,8 @@ struct WslBuild {                    // gather streams of the large-mechanism wa
   const std::vector<int32_t>* sp_of; // ownership [kWslHelpWarps][spw]
   int spw = 0;
   bool tuples = false;               // running sums in global memory: one (q row | sign, target row) tuple per entry of nu^T
+  bool tm_targets = false;           // tuples whose sums live in tensor memory: target = column offset 2 jj of the species'
+                                     // number jj in its owner's list, bit 1 of the q offset marks a species' last tuple
 };
 
 void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out,
@@ -335,12 +337,21 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
         for (int jj = 0; jj < wl->spw; ++jj) {
           const int sidx = (*wl->sp_of)[(size_t)hw * wl->spw + jj];
           if (sidx < 0) break;
-          for (uint32_t qo : pos[sidx]) { gent.push_back(qo); gent.push_back((uint32_t)sidx * row_bytes); ++n_t; }
-          for (uint32_t qo : neg[sidx]) { gent.push_back(qo | 1u); gent.push_back((uint32_t)sidx * row_bytes); ++n_t; }
+          const uint32_t target = wl->tm_targets ? 2u * (uint32_t)jj : (uint32_t)sidx * row_bytes;
+          size_t n_sp = 0;
+          for (uint32_t qo : pos[sidx]) { gent.push_back(qo); gent.push_back(target); ++n_t; ++n_sp; }
+          for (uint32_t qo : neg[sidx]) { gent.push_back(qo | 1u); gent.push_back(target); ++n_t; ++n_sp; }
+          if (wl->tm_targets) {
+            // the kernel sums a species' tuples in a register and adds the sum to the species' running sum at the tuple
+            // marked last (part 0 stores instead: a species without a term there gets one tuple on the zero row)
+            if (n_sp == 0 && c == 0) { gent.push_back(zero_off); gent.push_back(target); ++n_t; ++n_sp; }
+            if (n_sp) gent[gent.size() - 2] |= 2u;
+          }
         }
-        for (; n_t % 4; ++n_t) { gent.push_back(zero_off); gent.push_back((uint32_t)K * row_bytes); }
+        const uint32_t pad_target = wl->tm_targets ? 0u : (uint32_t)K * row_bytes;
+        for (; n_t % 4; ++n_t) { gent.push_back(zero_off); gent.push_back(pad_target); }
         jac_range[3 * hw + 1] = (uint16_t)(gent.size() / 4);
-        for (int t = 0; t < 8; ++t) { gent.push_back(zero_off); gent.push_back((uint32_t)K * row_bytes); }
+        for (int t = 0; t < 8; ++t) { gent.push_back(zero_off); gent.push_back(pad_target); }
       }
       if (wl->tuples) gptr.push_back(0);
       for (int hw = 0; hw < kWslHelpWarps && !wl->tuples; ++hw) {
@@ -746,7 +757,8 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
     for (int mi = 0; mi < 3 && !wsl_ok; ++mi) {
       const int acc_global = acc_modes[mi];
       if (acc_global == 2 && tm_tile_cols + tm_acc_cols > 512) continue;
-      wb.tuples = acc_global == 1;
+      wb.tuples = acc_global != 0;
+      wb.tm_targets = acc_global == 2;
       for (int n_parts = 2; n_parts <= (acc_global ? kWslMaxParts : 4) && n_parts <= I && !wsl_ok; ++n_parts) {
         const int rc_l = (I + n_parts - 1) / n_parts;
         // (a quick bound before building the blobs: the q buffers alone)
@@ -765,7 +777,7 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         o += 2 * lbs.stride;
         lv.smem_misc = (uint32_t)o;
         o += align_up((size_t)2 * Kp * 8 + (size_t)2 * 8 * kRowBytes + (size_t)2 * 3 * kRowBytes + 12 * 8 +
-                          (size_t)kWslHelpWarps * spw_l * 4 + (size_t)K * 2, 128);
+                          (size_t)kWslHelpWarps * spw_l * 4, 128);
         lv.smem_total = (uint32_t)o;
         if (o <= (size_t)prop.sharedMemPerBlockOptin) {
           wsl_ok = true;

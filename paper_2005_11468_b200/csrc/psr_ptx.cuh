@@ -102,6 +102,10 @@ __device__ __forceinline__ void tm_wait_ld6(TmF64& a, TmF64& b, TmF64& c, TmF64&
                : "+r"(a.lo), "+r"(a.hi), "+r"(b.lo), "+r"(b.hi), "+r"(c.lo), "+r"(c.hi), "+r"(d.lo), "+r"(d.hi), "+r"(e.lo),
                  "+r"(e.hi), "+r"(f.lo), "+r"(f.hi)::"memory");
 }
+__device__ __forceinline__ void tm_wait_ld4(TmF64& a, TmF64& b, TmF64& c, TmF64& d) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;"
+               : "+r"(a.lo), "+r"(a.hi), "+r"(b.lo), "+r"(b.hi), "+r"(c.lo), "+r"(c.hi), "+r"(d.lo), "+r"(d.hi)::"memory");
+}
 __device__ __forceinline__ void tm_wait_ld1(TmF64& a) {
   asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(a.lo), "+r"(a.hi)::"memory");
 }

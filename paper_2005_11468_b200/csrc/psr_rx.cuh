@@ -35,14 +35,15 @@ struct RxCtx {
 // factor lists (any type, signs of A).  MODE & kRxFast: table exp, range noted in cx.amax; else the library exp.
 // MODE & kRxTm: the six factors of a 3+3 record come from the copy of the C tile in tensor memory (cx.tm_c) instead
 // of shared memory -- those row reads leave the shared-memory pipe; asked for at the top of a trip, waited for at
-// its end.  (Efficiency lists and long factor lists, of data-dependent length, still read the shared-memory tile.)
+// its end; efficiency lists come four entries at a time, long factor lists one factor at a time: in this mode the
+// reaction code does not read the shared-memory C tile at all (C_tot and ln C_tot are state rows, not tile rows).
 // sink(kl, meta, korig, type, kf, kr, pf, pr, M): effective rate constants (falloff applied), the concentration
 // products of the two sides WITHOUT [M], and [M] (1 for a plain reaction) of record kl.
 constexpr int kRxFast = 1, kRxTm = 2;
 template <int CLS, int MODE, class Sink>
 __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blob, const ChunkHdr* hdr, const RxRec* recs,
                                              const int kl_begin, const int kl_end, Sink&& sink) {
-  constexpr bool FAST = (MODE & kRxFast) != 0, TM = (MODE & kRxTm) != 0 && CLS < kClsLong;
+  constexpr bool FAST = (MODE & kRxFast) != 0, TMA = (MODE & kRxTm) != 0, TM = TMA && CLS < kClsLong;
   PSR_CHK(kl_begin >= 0 && kl_begin <= kl_end && kl_end <= (int)hdr->n_rx, 101);
   if (kl_begin >= kl_end) return;   // nothing of this class for this warp in this chunk (the rule in small parts)
   auto exps = [&](auto& ex, auto& ey) {
@@ -110,7 +111,15 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
 #pragma unroll 1
       for (int j = 0; j < nr + np; ++j) {
         PSR_CHK((uint32_t)fsp[j] * (uint32_t)kRowBytes < cx.chk_c_bytes, 103);
-        const double cv = lds64(cx.c_lane + (uint32_t)fsp[j] * (uint32_t)kRowBytes);
+        double cv;
+        if constexpr (TMA) {   // (rare records: one factor at a time)
+          TmF64 t;
+          tm_ld64(cx.tm_c + 2u * (uint32_t)fsp[j], t);
+          tm_wait_ld1(t);
+          cv = t.get();
+        } else {
+          cv = lds64(cx.c_lane + (uint32_t)fsp[j] * (uint32_t)kRowBytes);
+        }
         if (j < nr) pf *= cv;
         else pr *= cv;
       }
@@ -146,10 +155,31 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
       double M = lds64(cx.ctot_lane);
       const uint32_t e1 = ax->eff_off + ax->n_eff;
       PSR_CHK((meta >> kMetaAuxShift) < hdr->n_aux && e1 <= hdr->n_eff, 104);
+      if constexpr (TMA) {
+        // the efficiency list four entries at a time from the tensor-memory copy; slots past the end re-read the last
+        // entry and are not added
 #pragma unroll 1
-      for (uint32_t e = ax->eff_off; e < e1; ++e) {
-        PSR_CHK(effs[e].off < cx.chk_c_bytes, 105);
-        M = fma(effs[e].am1, lds64(cx.c_lane + effs[e].off), M);
+        for (uint32_t e = ax->eff_off; e < e1; e += 4) {
+          TmF64 t0, t1, t2, t3;
+          const uint32_t i1 = min(e + 1, e1 - 1), i2 = min(e + 2, e1 - 1), i3 = min(e + 3, e1 - 1);
+          PSR_CHK(effs[e].off < cx.chk_c_bytes && effs[i3].off < cx.chk_c_bytes, 105);
+          tm_ld64(cx.tm_c + (effs[e].off >> 7), t0);
+          tm_ld64(cx.tm_c + (effs[i1].off >> 7), t1);
+          tm_ld64(cx.tm_c + (effs[i2].off >> 7), t2);
+          tm_ld64(cx.tm_c + (effs[i3].off >> 7), t3);
+          const double a0 = effs[e].am1, a1 = effs[i1].am1, a2 = effs[i2].am1, a3 = effs[i3].am1;
+          tm_wait_ld4(t0, t1, t2, t3);
+          M = fma(a0, t0.get(), M);
+          if (e + 1 < e1) M = fma(a1, t1.get(), M);
+          if (e + 2 < e1) M = fma(a2, t2.get(), M);
+          if (e + 3 < e1) M = fma(a3, t3.get(), M);
+        }
+      } else {
+#pragma unroll 1
+        for (uint32_t e = ax->eff_off; e < e1; ++e) {
+          PSR_CHK(effs[e].off < cx.chk_c_bytes, 105);
+          M = fma(effs[e].am1, lds64(cx.c_lane + effs[e].off), M);
+        }
       }
       if (type == RX_THREE_BODY) {
         Mout = M;

@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
         rx_run_chunk<kRxFast | (TM ? kRxTm : 0)>(cx, blob, w, sink);
         // an exp argument out of the table form's range (NaN, Inf, overflow, underflow: never for physical
         // states): this warp repeats its records with the library exp, which keeps IEEE results
-        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<0>(cx, blob, w, sink);
+        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<(TM ? kRxTm : 0)>(cx, blob, w, sink);
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[B_FULLQ + qb]);
       }

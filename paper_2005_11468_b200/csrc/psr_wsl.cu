@@ -51,8 +51,12 @@ template <int TMODE>
 __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArgs& a, double* Cs, double* acc_s, double* qh0,
                                                 unsigned char* ring, const double* invW_s, const double* W_s, double* St0,
                                                 double* tp0, uint64_t* bars, const int32_t* sp_s, uint32_t total_parts, const int bulk_ok,
-                                                const uint32_t tm_quad, const uint16_t* slot_s) {
+                                                const uint32_t tm_quad) {
   constexpr bool TM = TMODE != 0;   // tensor memory allocated: the copy of the C tile is kept there
+  // The reaction warps read only that copy (TMODE 1): the shared-memory tile is then a staging area, and the NEXT tile
+  // is loaded and converted there (stage_tile) while they work on the current one; what is left between two tiles is
+  // the copy into tensor memory (publish_tile).  Otherwise the two run back to back at the tile boundary.
+  constexpr bool EARLY = TMODE == 1;
   const int lane = threadIdx.x & 31, hw = (threadIdx.x >> 5) - kWslRxWarps;
   const int K = mv.K, q_elems = (mv.rc + 1) * kTile;
   const bool wantF = (a.flags & kOutF) != 0, out_w = (a.flags & kOutWdot) != 0;
@@ -67,7 +71,8 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
 
   // a1: a tile's Y rows (into the C tile), T, P, tau; then W_bar = 1/sum Y_i/W_i, rho = P W_bar/(R T), C_i = rho Y_i/W_i,
   // C_tot = rho sum Y_i/W_i and the state rows of the tile.  Every helper warp forms the sum over all species itself.
-  auto load_tile = [&](int64_t t, uint32_t lt) {
+  auto stage_tile = [&](int64_t t, uint32_t lt) {
+    if constexpr (EARLY) named_bar_sync(3, kWslHelpWarps * 32);   // the copy of the previous tile out of Cs is complete
     int64_t r = t * kTile + lane;
     if (r >= a.N) r = a.N - 1;   // lanes past N repeat the last reactor (a valid state, nothing stored)
     double* tb = tp0 + (lt & 1) * 3 * kTile;
@@ -132,10 +137,12 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       const int sp = my_sp[jj];
       Cs[sp * kTile + lane] = rho * (Cs[sp * kTile + lane] * invW_s[sp]);
     }
+  };
+  // (the reaction warps have released the previous tile through empty_C, which this warp has waited for)
+  auto publish_tile = [&]() {
     if constexpr (TM) {
-      // (the reaction warps released the tile through empty_C, which this warp waited for before this call)
       static_assert(kWslHelpWarps >= 4, "four helper warps copy the C tile to the four TMEM quadrants");
-      named_bar_sync(2, kWslHelpWarps * 32);   // every row of the tile is final
+      named_bar_sync(2, kWslHelpWarps * 32);   // every row of the staged tile is final
       if (hw < 4) {
         tm_fence_after_sync();
         const int last = K + 1;
@@ -167,32 +174,12 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       asm volatile("ld.shared.u32 %0, [%1];" : "=r"(off) : "r"(dst));
       dst += 4;
       PSR_CHK(off < (uint32_t)K * kRowBytes && off % kRowBytes == 0, 503);   // a row of the [K][32] running sums
-      if constexpr (TM) {
-        if (acct) {
-          // (one flush per species and part: the round trip through tensor memory is not on the stream's critical path)
-          const uint32_t col = tm_acc + 2u * (uint32_t)slot_s[off / kRowBytes];
-          PSR_CHK(slot_s[off / kRowBytes] < mv.spw, 507);
-          if (FIRST) {
-            tm_st64(col, acc);
-          } else {
-            TmF64 t;
-            tm_ld64(col, t);
-            tm_wait_ld1(t);
-            tm_st64(col, t.get() + acc);
-          }
-          acc = 0.0;
-          return;
-        }
-      }
       const uint32_t addr = acc_lane + off;   // (sums in shared memory; in global memory: gather_tuples)
       sts64(addr, FIRST ? acc : lds64(addr) + acc);
       acc = 0.0;
     };
     const uint32_t qmax = (uint32_t)q_elems * 8u;
     (void)qmax;
-    if constexpr (TM) {
-      if (acct && !FIRST) tm_wait_st();   // the sums the previous part stored have landed
-    }
     uint4 oa, ob;
     ld_group(gs, oa);
     ld_group(gs + 16, ob);
@@ -253,6 +240,60 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
     }
   };
 
+  // a8 with the sums in tensor memory (this warp's species at columns tm_acc + 2 jj of its own lane quadrant): the tuple
+  // stream again -- no padding to groups, which at 4.3 entries per species and part would double the stream -- but a
+  // species' tuples are summed in a register, in stream order, and the tuple marked last adds the sum to the species'
+  // running sum (part 0 stores it).  Tuples are read two trips ahead, q values one trip ahead.
+  auto gather_tuples_tm = [&](auto first_tag, const unsigned char* blob, const uint32_t q_lane) {
+    constexpr bool FIRST = decltype(first_tag)::value;
+    const ChunkHdr* hdr = reinterpret_cast<const ChunkHdr*>(blob);
+    const uint32_t ts = smem_u32(blob + hdr->off_gent) + (uint32_t)hdr->wb[kWslRxWarps + hw][0] * 16u;
+    const int n_pairs = (int)hdr->wb[kWslRxWarps + hw][1] - (int)hdr->wb[kWslRxWarps + hw][0];   // 16-byte units, even
+    auto ld4 = [&](uint32_t addr, uint4& o) {
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w) : "r"(addr));
+    };
+    if (!FIRST) tm_wait_st();   // the sums the previous part stored have landed
+    double acc = 0.0;
+    auto step = [&](uint32_t qo, uint32_t to, double v) {
+      PSR_CHK((qo & ~3u) < (uint32_t)q_elems * 8u && to < 2u * (uint32_t)mv.spw, 507);
+      acc += __hiloint2double(__double2hiint(v) ^ (int)(qo << 31), __double2loint(v));   // -v if bit 0 is set
+      if (qo & 2u) {   // the species' last tuple of this part (the same in every lane)
+        const uint32_t col = tm_acc + to;
+        if (FIRST) {
+          tm_st64(col, acc);
+        } else {
+          TmF64 t;
+          tm_ld64(col, t);
+          tm_wait_ld1(t);
+          tm_st64(col, t.get() + acc);
+        }
+        acc = 0.0;
+      }
+    };
+    uint4 ca, cb, na, nb;
+    ld4(ts, ca);
+    ld4(ts + 16, cb);
+    double v0 = lds64(q_lane + (ca.x & ~3u)), v1 = lds64(q_lane + (ca.z & ~3u)), v2 = lds64(q_lane + (cb.x & ~3u)),
+           v3 = lds64(q_lane + (cb.z & ~3u));
+    ld4(ts + 32, na);
+    ld4(ts + 48, nb);
+#pragma unroll 1
+    for (int i = 0; i < n_pairs; i += 2) {
+      const uint4 a_ = ca, b_ = cb;
+      const double w0 = v0, w1 = v1, w2 = v2, w3 = v3;
+      ca = na;
+      cb = nb;
+      v0 = lds64(q_lane + (ca.x & ~3u)), v1 = lds64(q_lane + (ca.z & ~3u)), v2 = lds64(q_lane + (cb.x & ~3u)),
+      v3 = lds64(q_lane + (cb.z & ~3u));
+      ld4(ts + (uint32_t)(i + 4) * 16u, na);
+      ld4(ts + (uint32_t)(i + 5) * 16u, nb);
+      step(a_.x, a_.y, w0);
+      step(a_.z, a_.w, w1);
+      step(b_.x, b_.y, w2);
+      step(b_.z, b_.w, w3);
+    }
+  };
+
   // a9 (Eq. 2 at steady state) and the wdot store of a tile: F_i = (Y_i - Y_in,i)/tau - wdot_i W_i/rho, eight rows in flight.
   // (A running sum kept in global memory is read past L1: the adds of the later parts were done at L2.)
   auto epilogue = [&](int64_t t, uint32_t lt) {
@@ -302,7 +343,10 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
   }
   const int64_t stride = gridDim.x;
   int64_t tile = blockIdx.x;
-  if (tile < a.n_tiles) load_tile(tile, 0);
+  if (tile < a.n_tiles) {
+    stage_tile(tile, 0);
+    publish_tile();
+  }
   for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += stride) {
     for (int p = 0; p < mv.n_parts; ++p) {
       const uint32_t g = lt * (uint32_t)mv.n_parts + (uint32_t)p, qb = g & 1, u = g >> 1;
@@ -311,12 +355,16 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       if (p == mv.n_parts - 1 && tile + stride < a.n_tiles) {
         // the reaction warps leave the tile now: the next tile's C first, the last part's gather after it
         mbar_wait(&bars[L_EMPTYC], lt & 1);
-        load_tile(tile + stride, lt + 1);
+        if constexpr (!EARLY) stage_tile(tile + stride, lt + 1);
+        publish_tile();
       }
       const unsigned char* blob = ring + (size_t)qb * mv.chunk_stride;
       const uint32_t q_lane = smem_u32(qh0 + qb * q_elems) + lane * 8;
       if (accg) gather_tuples(blob, q_lane);
-      else if (p == 0) gather(std::true_type{}, blob, q_lane);
+      else if (TM && acct) {
+        if (p == 0) gather_tuples_tm(std::true_type{}, blob, q_lane);
+        else gather_tuples_tm(std::false_type{}, blob, q_lane);
+      } else if (p == 0) gather(std::true_type{}, blob, q_lane);
       else gather(std::false_type{}, blob, q_lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars[L_EMPTYQ + qb]);
@@ -331,6 +379,9 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
                    mv.chunk_stride, &bars[L_RING + qb]);
         }
         __syncwarp();
+      }
+      if constexpr (EARLY) {
+        if (p == 0 && tile + stride < a.n_tiles) stage_tile(tile + stride, lt + 1);
       }
     }
     epilogue(tile, lt);
@@ -358,7 +409,6 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
   uint64_t* bars = reinterpret_cast<uint64_t*>(tp0 + 2 * 3 * kTile);
   uint32_t* tm_slot = reinterpret_cast<uint32_t*>(bars + L_COUNT);  // tensor-memory base address (TM)
   int32_t* sp_s = reinterpret_cast<int32_t*>(bars + L_SLOTS);       // [helper warps][spw]
-  uint16_t* slot_s = reinterpret_cast<uint16_t*>(sp_s + kWslHelpWarps * mv.spw);   // [K]: species -> its number in its owner's list
 
   const int lane = threadIdx.x & 31;
   const int w = threadIdx.x >> 5;
@@ -394,11 +444,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
     invW_s[i] = mv.invW[i];
     W_s[i] = mv.Wm[i];
   }
-  for (int i = threadIdx.x; i < kWslHelpWarps * mv.spw; i += kWslWarps * 32) {
-    const int sp = mv.sp_of[i];
-    sp_s[i] = sp;
-    if (sp >= 0) slot_s[sp] = (uint16_t)(i % mv.spw);
-  }
+  for (int i = threadIdx.x; i < kWslHelpWarps * mv.spw; i += kWslWarps * 32) sp_s[i] = mv.sp_of[i];
   if constexpr (TM) tm_fence_before_sync();
   __syncthreads();
   uint32_t tm_quad = 0;   // this warp's quadrant of the copy of the C tile in tensor memory
@@ -458,7 +504,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
         cx.amax = 0.0f;
         rx_run_chunk<kRxFast | (RXTM ? kRxTm : 0)>(cx, blob, w, sink);
         // an exp argument out of the table form's range: this warp repeats its records with the library exp
-        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<0>(cx, blob, w, sink);
+        if (__any_sync(kFullMask, !exp_max_in_range(cx.amax))) rx_run_chunk<(RXTM ? kRxTm : 0)>(cx, blob, w, sink);
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[L_FULLQ + qb]);
       }
@@ -467,7 +513,7 @@ __global__ void __launch_bounds__(kWslWarps * 32, 1) psr_wsl_kernel(const WslVie
     }
   } else {
     // ================================================================== helper warps: see above
-    psr_wsl_helpers<TMODE>(mv, a, Cs, acc_s, qh0, ring, invW_s, W_s, St0, tp0, bars, sp_s, total_parts, bulk_ok, tm_quad, slot_s);
+    psr_wsl_helpers<TMODE>(mv, a, Cs, acc_s, qh0, ring, invW_s, W_s, St0, tp0, bars, sp_s, total_parts, bulk_ok, tm_quad);
   }
   if constexpr (TM) {
     tm_fence_before_sync();
