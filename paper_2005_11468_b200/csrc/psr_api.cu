@@ -154,7 +154,7 @@ struct WslBuild {                    // gather streams of the large-mechanism wa
   int spw = 0;
   bool tuples = false;               // running sums in global memory: one (q row | sign, target row) tuple per entry of nu^T
   bool tm_targets = false;           // tuples whose sums live in tensor memory: target = column offset 2 jj of the species'
-                                     // number jj in its owner's list, bit 1 of the q offset marks a species' last tuple
+                                     // number jj in its owner's list | bit 31: subtract | bit 30: the species' last tuple
 };
 
 void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int nw, double warp0_load, BlobSet& out,
@@ -330,7 +330,7 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
       for (int hw = 0; hw < kWslHelpWarps && wl->tuples; ++hw) {
         // tuple stream (sums in global memory, added to with red.global: no running sum, no flush): per helper warp, its
         // species in ownership order, a species' "+" entries then its "-" entries -- a fixed order.  Entry = {byte
-        // offset of the q row | 1 if it is subtracted, byte offset of the species' row}; padded to a multiple of 4
+        // offset of the q row, byte offset of the species' row | bit 31 if it is subtracted}; padded to a multiple of 4
         // tuples, and 8 more for the kernel's read-ahead, with {zero row of q, spare row K of the sums}.
         jac_range[3 * hw] = (uint16_t)(gent.size() / 4);   // in 16-byte units = pairs of tuples
         size_t n_t = 0;
@@ -339,13 +339,15 @@ void build_blobs(const std::vector<HostRx>& rx, int K, int I, int n_chunks, int 
           if (sidx < 0) break;
           const uint32_t target = wl->tm_targets ? 2u * (uint32_t)jj : (uint32_t)sidx * row_bytes;
           size_t n_sp = 0;
+          // (the target word carries the flags -- bit 31: subtract, bit 30: the species' last tuple of the part, for
+          // tensor-memory targets -- so that the q offset is used as it is)
           for (uint32_t qo : pos[sidx]) { gent.push_back(qo); gent.push_back(target); ++n_t; ++n_sp; }
-          for (uint32_t qo : neg[sidx]) { gent.push_back(qo | 1u); gent.push_back(target); ++n_t; ++n_sp; }
+          for (uint32_t qo : neg[sidx]) { gent.push_back(qo); gent.push_back(target | 0x80000000u); ++n_t; ++n_sp; }
           if (wl->tm_targets) {
             // the kernel sums a species' tuples in a register and adds the sum to the species' running sum at the tuple
             // marked last (part 0 stores instead: a species without a term there gets one tuple on the zero row)
             if (n_sp == 0 && c == 0) { gent.push_back(zero_off); gent.push_back(target); ++n_t; ++n_sp; }
-            if (n_sp) gent[gent.size() - 2] |= 2u;
+            if (n_sp) gent[gent.size() - 1] |= 0x40000000u;
           }
         }
         const uint32_t pad_target = wl->tm_targets ? 0u : (uint32_t)K * row_bytes;

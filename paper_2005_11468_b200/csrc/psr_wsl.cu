@@ -220,10 +220,10 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w) : "r"(addr));
     };
     auto add = [&](uint32_t qo, uint32_t to) {
-      PSR_CHK((qo & ~1u) < (uint32_t)q_elems * 8u && to <= (uint32_t)K * kRowBytes && to % kRowBytes == 0, 506);
-      const double v = lds64(q_lane + (qo & ~1u));
-      const double sv = __hiloint2double(__double2hiint(v) ^ (int)(qo << 31), __double2loint(v));   // -v if bit 0 is set
-      asm volatile("red.global.add.f64 [%0], %1;" ::"l"(accg_lane + to), "d"(sv) : "memory");
+      PSR_CHK(qo < (uint32_t)q_elems * 8u && (to & 0x7fffffffu) <= (uint32_t)K * kRowBytes && to % kRowBytes == 0, 506);
+      const double v = lds64(q_lane + qo);
+      const double sv = __hiloint2double(__double2hiint(v) ^ (int)(to & 0x80000000u), __double2loint(v));   // -v if bit 31 is set
+      asm volatile("red.global.add.f64 [%0], %1;" ::"l"(accg_lane + (to & 0x7fffffffu)), "d"(sv) : "memory");
     };
     uint4 ta, tb;
     ld4(ts, ta);
@@ -255,10 +255,10 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
     if (!FIRST) tm_wait_st();   // the sums the previous part stored have landed
     double acc = 0.0;
     auto step = [&](uint32_t qo, uint32_t to, double v) {
-      PSR_CHK((qo & ~3u) < (uint32_t)q_elems * 8u && to < 2u * (uint32_t)mv.spw, 507);
-      acc += __hiloint2double(__double2hiint(v) ^ (int)(qo << 31), __double2loint(v));   // -v if bit 0 is set
-      if (qo & 2u) {   // the species' last tuple of this part (the same in every lane)
-        const uint32_t col = tm_acc + to;
+      PSR_CHK(qo < (uint32_t)q_elems * 8u && (to & 0xffffu) < 2u * (uint32_t)mv.spw, 507);
+      acc += __hiloint2double(__double2hiint(v) ^ (int)(to & 0x80000000u), __double2loint(v));   // -v if bit 31 is set
+      if (to & 0x40000000u) {   // the species' last tuple of this part (the same in every lane)
+        const uint32_t col = tm_acc + (to & 0xffffu);
         if (FIRST) {
           tm_st64(col, acc);
         } else {
@@ -273,8 +273,7 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
     uint4 ca, cb, na, nb;
     ld4(ts, ca);
     ld4(ts + 16, cb);
-    double v0 = lds64(q_lane + (ca.x & ~3u)), v1 = lds64(q_lane + (ca.z & ~3u)), v2 = lds64(q_lane + (cb.x & ~3u)),
-           v3 = lds64(q_lane + (cb.z & ~3u));
+    double v0 = lds64(q_lane + ca.x), v1 = lds64(q_lane + ca.z), v2 = lds64(q_lane + cb.x), v3 = lds64(q_lane + cb.z);
     ld4(ts + 32, na);
     ld4(ts + 48, nb);
 #pragma unroll 1
@@ -283,8 +282,7 @@ __device__ __forceinline__ void psr_wsl_helpers(const WslView& mv, const EvalArg
       const double w0 = v0, w1 = v1, w2 = v2, w3 = v3;
       ca = na;
       cb = nb;
-      v0 = lds64(q_lane + (ca.x & ~3u)), v1 = lds64(q_lane + (ca.z & ~3u)), v2 = lds64(q_lane + (cb.x & ~3u)),
-      v3 = lds64(q_lane + (cb.z & ~3u));
+      v0 = lds64(q_lane + ca.x), v1 = lds64(q_lane + ca.z), v2 = lds64(q_lane + cb.x), v3 = lds64(q_lane + cb.z);
       ld4(ts + (uint32_t)(i + 4) * 16u, na);
       ld4(ts + (uint32_t)(i + 5) * 16u, nb);
       step(a_.x, a_.y, w0);
