@@ -6,10 +6,10 @@
 // the barriers 0.05 ms, the gather 0.035 ms, the epilogue 0.01 ms, none of it overlapped).  Here the phases
 // are roles of different warps that meet only through mbarriers:
 //
-//   reaction warps (11)  a3..a7: k_f, K_c, k_r, [M], falloff, q of their share of the reactions, tile after
+//   reaction warps (13)  a3..a7: k_f, K_c, k_r, [M], falloff, q of their share of the reactions, tile after
 //                        tile without a CTA barrier; q goes to one of two q buffers (one "part" of the
 //                        mechanism each), concentrations and per-reactor state come from one of two C tiles.
-//   helper warps (5)     a1: TMA bulk loads of the tile after next, state preparation (Wbar, rho, C_i, ln T,
+//   helper warps (7)     a1: TMA bulk loads of the tile after next, state preparation (Wbar, rho, C_i, ln T,
 //                        ln C_tot) of the next tile;  a8: gather of the q buffer the reaction warps have just
 //                        filled (nu^T q, fixed order, partial sums in shared memory between parts);
 //                        a9: residual and stores.
@@ -19,6 +19,10 @@
 //   empty_C[b]   reaction warps are done with the C tile           reaction -> helpers (next loads into it)
 //   full_q[qb]   every reaction warp has written its q rows        reaction -> helpers
 //   empty_q[qb]  the part has been gathered                        helpers  -> reaction warps
+//
+// Tensor memory (K <= 126): four helper warps copy each finished C tile into the four lane quadrants of the SM's
+// tensor memory, and the reaction warps take the six factors of a 3+3 record from there (tcgen05.ld) instead of
+// shared memory, whose data pipe is the busiest unit of this kernel.
 //
 // Same tables (psr_tables.h), same per-reaction arithmetic and the same exp as psr_kernels.cu; the steps are
 // SURVEY.md 8(a) a1..a9 (Eq. 2, 4-9).

@@ -7,17 +7,24 @@
 // pair -- 13 x 500 visits of ~1.5 reactions each at C3, the running sums bouncing through L2 in between: 55 % of
 // its instructions (profiles/r1d_psr_eval_kernel_C3.md).  Here the roles are those of psr_ws.cu:
 //
-//   reaction warps (10)  a3..a7 of their share of a part's records, part after part, tile after tile; q goes to
+//   reaction warps (12)  a3..a7 of their share of a part's records, part after part, tile after tile; q goes to
 //                        one of two q buffers; the part's tables come from a two-stage ring (bulk copies).
-//   helper warps (6)     a8: gather of the q buffer just filled -- flat streams of 4-entry groups that SKIP the
-//                        species without a term in the part, each flush taking its target row from a list in the
-//                        blob; the running sums live in a shared-memory tile when it fits (C2); else (C3) in an
-//                        L2-resident scratch that a flat stream of (q row, species row, sign) tuples adds to with
-//                        red.global -- one per entry of nu^T, no running sum, no flush (one thread owns an element:
-//                        deterministic order, no latency exposed);
-//                        a1: loads and state preparation of the NEXT tile, done ahead of the last part's gather so
-//                        that the reaction warps restart as early as the single C tile allows;
-//                        a9: per-tile epilogue (wdot, F) streaming Y, Y_in and the sums, four rows in flight.
+//   helper warps (8)     a8: gather of the q buffer just filled.  Where the running sums of nu^T q live decides its form
+//                        (WslView::acc_global): 0 -- a shared-memory tile, when that still leaves room for at most four
+//                        parts (P5): flat streams of 4-entry groups that SKIP the species without a term in the part,
+//                        each flush taking its target row from a list in the blob; 2 -- tensor memory, the warp's own
+//                        species in its own lane quadrant (K <= 200: C2): a flat stream of (q row, target | flags)
+//                        tuples, a species' tuples summed in a register and added to its running sum at its last tuple;
+//                        1 -- an L2-resident scratch (C3): the same tuples, each added with red.global (one thread owns
+//                        an element: deterministic order);
+//                        a1: loads and state preparation of the NEXT tile;
+//                        a9: per-tile epilogue (wdot, F) streaming Y, Y_in and the sums, eight rows in flight.
+//
+// Tensor memory (TMODE 1; K <= 250): a copy of the finished C tile in all four lane quadrants, from which the reaction
+// warps read every concentration (psr_rx.cuh, kRxTm) -- the shared-memory tile is then only a staging area, the next tile
+// is loaded and converted there while the current one is evaluated, and between two tiles only the copy into tensor
+// memory remains.  Without it the next tile is prepared ahead of the last part's gather, once the reaction warps have
+// left the single tile.
 //
 //   ring[st]     a part's tables landed (tx bytes)                  helper 0   -> everyone
 //   full_C       C tile + state rows of a tile ready                helpers    -> reaction warps
