@@ -392,8 +392,8 @@ __global__ void __launch_bounds__(kWsWarps * 32, 1) psr_ws_kernel(const WsView m
     int64_t tile = blockIdx.x;
     if (tile < a.n_tiles) issue_loads(tile, 0);
     if (tile + stride < a.n_tiles) issue_loads(tile + stride, 1);
+    if (tile < a.n_tiles) prologue(0);   // (needs no mechanism table: runs while the blobs are still landing)
     mbar_wait(&bars[B_BLOB], 0);
-    if (tile < a.n_tiles) prologue(0);
     for (uint32_t lt = 0; tile < a.n_tiles; ++lt, tile += stride) {
       const int b = lt & 1;
       if (tile + stride < a.n_tiles) prologue(lt + 1);
