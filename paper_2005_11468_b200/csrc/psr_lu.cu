@@ -39,14 +39,24 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
     // pseudo-transient step (psr_ptc_solve): the matrix is J + I/dt, the right-hand side -F
     const double shift = PTC ? 1.0 / dt[r] : 0.0;
     {
-      // column-major stream, 32 consecutive entries per trip, 4 trips in flight; (i, j) tracked without a divide
+      // column-major stream, 32 consecutive entries per trip, kStageU trips in flight (with one warp per system and
+      // nine warps per SM nothing else hides the latency of these loads: at 4 in flight they were 18 % of the samples);
+      // (i, j) tracked without a divide.  The warp's NEXT system is asked into L2 meanwhile.
+      constexpr int kStageU = 24;
+      {
+        const int64_t rn = r + (int64_t)gridDim.x * wpc;
+        if (rn < N) {
+          const char* pn = reinterpret_cast<const char*>(A + (size_t)rn * n * n);
+          for (int o = lane * 128; o < n * n * 8; o += 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(pn + o));
+        }
+      }
       int i = lane, j = 0;
       while (i >= n) { i -= n; ++j; }
-      for (int t = lane; t < n * n; t += 128) {
-        double v[4];
-        int off[4];
+      for (int t = lane; t < n * n; t += 32 * kStageU) {
+        double v[kStageU];
+        int off[kStageU];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < kStageU; ++u) {
           off[u] = j * ld + i;
           v[u] = (t + 32 * u < n * n) ? Ar[t + 32 * u] : 0.0;
           if (PTC && i == j) v[u] += shift;
@@ -54,7 +64,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
           while (i >= n) { i -= n; ++j; }
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+        for (int u = 0; u < kStageU; ++u)
           if (t + 32 * u < n * n) As[off[u]] = v[u];
       }
     }
