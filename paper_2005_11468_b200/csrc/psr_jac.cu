@@ -305,6 +305,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
       issue();
       issue();
       // polynomial part: sum_n (s^(n-1) - 1) D_i^(n)
+#pragma unroll 4
       for (int i = 0; i < K; ++i) {
         double v = 0.0;
 #pragma unroll
@@ -405,6 +406,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
       // tile's row stride of 33 keeps both access directions free of bank conflicts)
       {
         const double invh = 1.0 / h;
+#pragma unroll 4
         for (int i = 0; i < K; ++i) {
           const double d = -(W_s[i] * invrho) * acc_t[i * kJacAccLd + lane];
           acc_t[i * kJacAccLd + lane] = (i == j ? fma(h, invtau, d) : d) * invh;
@@ -415,10 +417,21 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
         const int n_valid = (int)min((int64_t)kTile, a.N - tile * kTile);
         double* Jc = a.J + ((tile * kTile * n) + 1 + j) * n;   // column 1 + j of the tile's first reactor
         PSR_CHK(((tile * kTile + n_valid - 1) * n + 1 + j) * n + n <= a.N * (int64_t)n * n, 310);   // the last reactor's column ends inside J
-        for (int l = 0; l < n_valid; ++l, Jc += (int64_t)n * n) {
-          for (int e = lane; e < n; e += 32)
-            Jc[e] = e == 0 ? 0.0 : acc_t[(e - 1) * kJacAccLd + l];   // row 0: F_T = T - T_set does not depend on Y
+        // four reactors per trip, their values read before the first store (a load the compiler cannot move over a
+        // store through another generic pointer would otherwise wait for it)
+        const int64_t nn = (int64_t)n * n;
+        int l = 0;
+        for (; l + 4 <= n_valid; l += 4, Jc += 4 * nn) {
+          for (int e = lane; e < n; e += 32) {
+            double v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = e == 0 ? 0.0 : acc_t[(e - 1) * kJacAccLd + l + u];   // row 0: F_T = T - T_set does not depend on Y
+#pragma unroll
+            for (int u = 0; u < 4; ++u) Jc[u * nn + e] = v[u];
+          }
         }
+        for (; l < n_valid; ++l, Jc += nn)
+          for (int e = lane; e < n; e += 32) Jc[e] = e == 0 ? 0.0 : acc_t[(e - 1) * kJacAccLd + l];
       }
       __syncwarp();
     }
