@@ -175,10 +175,19 @@ __device__ __forceinline__ void rx_run_class(RxCtx& cx, const unsigned char* blo
           if (e + 3 < e1) M = fma(a3, t3.get(), M);
         }
       } else {
+        // four entries per trip, their loads issued together (one at a time the list is a chain of shared-memory
+        // latencies: 3 % of the C1 kernel's samples); slots past the end re-read the last entry and are not added
 #pragma unroll 1
-        for (uint32_t e = ax->eff_off; e < e1; ++e) {
-          PSR_CHK(effs[e].off < cx.chk_c_bytes, 105);
-          M = fma(effs[e].am1, lds64(cx.c_lane + effs[e].off), M);
+        for (uint32_t e = ax->eff_off; e < e1; e += 4) {
+          const uint32_t i1 = min(e + 1, e1 - 1), i2 = min(e + 2, e1 - 1), i3 = min(e + 3, e1 - 1);
+          PSR_CHK(effs[e].off < cx.chk_c_bytes && effs[i3].off < cx.chk_c_bytes, 105);
+          const double a0 = effs[e].am1, a1 = effs[i1].am1, a2 = effs[i2].am1, a3 = effs[i3].am1;
+          const double c0 = lds64(cx.c_lane + effs[e].off), c1 = lds64(cx.c_lane + effs[i1].off),
+                       c2 = lds64(cx.c_lane + effs[i2].off), c3 = lds64(cx.c_lane + effs[i3].off);
+          M = fma(a0, c0, M);
+          if (e + 1 < e1) M = fma(a1, c1, M);
+          if (e + 2 < e1) M = fma(a2, c2, M);
+          if (e + 3 < e1) M = fma(a3, c3, M);
         }
       }
       if (type == RX_THREE_BODY) {
