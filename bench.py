@@ -516,6 +516,27 @@ def run_extras(binding, synth, torch, flush, only=None, cpu=True):
             out["C4_hybrid"] = {"call": "psr_solve_hybrid", "reactors": nb, "options": kw, "ms": ms_h,
                                 "converged_frac": float((st == 0).float().mean()), "mean_newton": float(nn.float().mean()),
                                 "mean_ptc": float(npt.float().mean()), "ms_per_solve_round": ms_h / kw["max_iter"]}
+            # the restart case: the converged states perturbed by 1 %, same budget of 420 rounds.  Every reactor finishes
+            # within a few Newton iterations; the rounds after the last one are empty launches (finished reactors are
+            # counted on the device), so the budget costs little
+            Tt, Yt = a0[0].clone(), a0[2].clone()
+            st0, _, _ = gm.solve_hybrid(Tt, a0[1], Yt, a0[3], a0[4], workspace=ws, **kw)
+            conv = (st0 == 0).nonzero().flatten()
+            gen = torch.Generator(device="cuda").manual_seed(17)
+            pert = 1.0 + 0.01 * (2.0 * torch.rand((Yt.shape[0], conv.numel()), generator=gen, device="cuda", dtype=torch.float64) - 1.0)
+            a1 = [Tt[conv].contiguous(), a0[1][conv].contiguous(), (Yt[:, conv] * pert).contiguous(), a0[3][:, conv].contiguous(),
+                  a0[4][conv].contiguous()]
+            def restart():
+                return gm.solve_hybrid(a1[0].clone(), a1[1], a1[2].clone(), a1[3], a1[4], workspace=ws, **kw)
+            st1, nn1, np1 = restart()
+            torch.cuda.synchronize()
+            e0.record(torch.cuda.current_stream())
+            st1, nn1, np1 = restart()
+            e1.record(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            out["C4_hybrid"]["restart"] = {"reactors": int(conv.numel()), "start": "converged states x (1 +- 1 %)", "ms": e0.elapsed_time(e1),
+                                           "converged_frac": float((st1 == 0).float().mean()), "mean_newton": float(nn1.float().mean()),
+                                           "mean_ptc": float(np1.float().mean())}
         gm.close()
     return out
 

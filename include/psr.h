@@ -206,8 +206,11 @@ psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F,
  * of each kind performed.  workspace: DEVICE scratch of workspace_bytes >= psr_solve_hybrid_workspace_bytes(mech, 1)
  * bytes; with less than psr_solve_hybrid_workspace_bytes(mech, N) the batch is solved in sub-batches one after the
  * other.  Runs entirely on the device: max_iter rounds of (psr_fd_jacobian, psr_ptc_solve, one bookkeeping kernel)
- * are enqueued on `stream` for every sub-batch, with no host synchronisation (converged reactors are left
- * untouched by the later rounds); capturable in a CUDA graph after psr_mech_reserve(mech, N). */
+ * are enqueued on `stream` for every sub-batch, with no host synchronisation.  Converged reactors are left
+ * untouched by the later rounds and are marked on the device: their linear systems, and the tiles of 32 reactors of
+ * the fused Jacobian kernel that hold only finished reactors, are left out, and once a sub-batch has none left a round
+ * is three empty launches -- max_iter is a budget, not a cost.  Capturable in a CUDA graph after
+ * psr_mech_reserve(mech, N). */
 typedef struct {
   double atol, rtol;
   int32_t max_iter, max_newton, max_ptc, reserved;

@@ -21,13 +21,13 @@ cudaError_t launch_eval(int nw, int spw, int rl, const MechView& mv, const EvalA
 cudaError_t occupancy_eval(int nw, int spw, int rl, size_t smem, size_t smem_optin, int* ctas_per_sm);
 cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream_t st);
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
-                            cudaStream_t st, const double* F, const double* dt);
+                            cudaStream_t st, const double* F, const double* dt, const int32_t* skip_count);
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
 cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
-                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
+                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st);
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
                                  const int32_t* info, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it, int32_t* status,
-                                 int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
+                                 int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st);
 cudaError_t chk_read_kernels(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_ws(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_jac(unsigned int* count, unsigned int* first_code);
@@ -1248,9 +1248,10 @@ size_t jac_scratch_bytes(const psr_mech* m, int64_t N, bool with_F0, int64_t* Nb
 }
 
 // psr_fd_jacobian (Tin == nullptr: row 0 is T - T_set) and psr_fd_jacobian_energy (row 0 is the energy row)
+// skip_dt / skip_count: psr_solve_hybrid's markers of finished reactors (EvalArgs); honoured by the fused kernel only
 psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, const double* P, const double* Y,
                             const double* Tin, const double* Yin, const double* tau, int64_t ld, double* J, double* F0,
-                            void* stream, const char* fn) {
+                            void* stream, const char* fn, const double* skip_dt = nullptr, const int32_t* skip_count = nullptr) {
   g_err.clear();
   psr_status st = check_common(mc, N, T, P, Y, ld, fn);
   if (st != PSR_OK || N == 0) return st;
@@ -1263,6 +1264,8 @@ psr_status fd_jacobian_impl(const psr_mech* mc, int64_t N, const double* T, cons
     EvalArgs a{};
     a.N = N; a.ld = ld; a.T = T; a.P = P; a.Y = Y; a.Yin = Yin; a.tau = tau; a.J = J; a.F0out = F0;
     a.n_tiles = (N + kTile - 1) / kTile;
+    a.skip_dt = skip_dt;
+    a.skip_count = skip_count;
     const int grid = (int)std::min<int64_t>(a.n_tiles, m->n_sm);
     cudaError_t e = launch_jac(m->jac, a, grid, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, fn);
@@ -1391,7 +1394,7 @@ psr_status psr_fd_jacobian_energy(const psr_mech* mech, int64_t N, const double*
 }
 
 static psr_status solve_impl(const char* who, int64_t N, int32_t n, const double* A, double* b, int32_t* info,
-                             const double* F, const double* dt, void* stream) {
+                             const double* F, const double* dt, void* stream, const int32_t* skip_count = nullptr) {
   // SM count and shared-memory limit of the current device, looked up once per device
   static int s_sm[64], s_optin[64];
   int dev = 0;
@@ -1411,7 +1414,7 @@ static psr_status solve_impl(const char* who, int64_t N, int32_t n, const double
     }
   }
   if (n > 168) return fail(PSR_EUNSUPPORTED, "%s: n = %d, the one-warp-per-system kernel takes n <= 168", who, n);
-  e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream, F, dt);
+  e = launch_lu_solve(N, n, A, b, info, n_sm, (size_t)optin, (cudaStream_t)stream, F, dt, skip_count);
   if (e != cudaSuccess) return cuda_fail(e, who);
   return PSR_OK;
 }
@@ -1435,13 +1438,15 @@ psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F,
 }
 
 namespace {
-// workspace of the hybrid solver per reactor: J, F0, dx, the two dt arrays (doubles); info, mode, it (int32)
+// workspace of the hybrid solver per reactor: J, F0, dx, the two dt arrays (doubles); info, mode, it (int32); and once
+// per call the counter of reactors still iterating
 size_t hybrid_bytes_per_reactor(int n) { return ((size_t)n * n + 2 * (size_t)n + 2) * 8 + 3 * 4 + 4; }
+constexpr size_t kHybridFixedBytes = 256;
 }  // namespace
 
 size_t psr_solve_hybrid_workspace_bytes(const psr_mech* m, int64_t N) {
   if (!m || N < 1) return 0;
-  return hybrid_bytes_per_reactor(m->view.K + 1) * (size_t)N + 256;
+  return hybrid_bytes_per_reactor(m->view.K + 1) * (size_t)N + 256 + kHybridFixedBytes;
 }
 
 psr_status psr_solve_hybrid(const psr_mech* m, int64_t N, double* T, const double* P, double* Y, const double* Tin,
@@ -1458,8 +1463,12 @@ psr_status psr_solve_hybrid(const psr_mech* m, int64_t N, double* T, const doubl
   if (n > 168) return fail(PSR_EUNSUPPORTED, "psr_solve_hybrid: %d unknowns, the linear solve takes <= 168", n);
   uintptr_t base = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~(uintptr_t)255;
   const size_t lost = base - reinterpret_cast<uintptr_t>(workspace);
-  if (workspace_bytes <= lost + hybrid_bytes_per_reactor(n)) return fail(PSR_EINVAL, "psr_solve_hybrid: workspace smaller than one reactor needs");
-  const int64_t Nb = std::min<int64_t>(N, (int64_t)((workspace_bytes - lost) / hybrid_bytes_per_reactor(n)));
+  if (workspace_bytes <= lost + kHybridFixedBytes + hybrid_bytes_per_reactor(n))
+    return fail(PSR_EINVAL, "psr_solve_hybrid: workspace smaller than one reactor needs");
+  const int64_t Nb = std::min<int64_t>(std::min<int64_t>(N, (int64_t)1 << 30),
+                                      (int64_t)((workspace_bytes - lost - kHybridFixedBytes) / hybrid_bytes_per_reactor(n)));
+  int32_t* n_active = reinterpret_cast<int32_t*>(base);   // reactors of the block still iterating (device counter)
+  base += kHybridFixedBytes;
   double* J = reinterpret_cast<double*>(base);
   double* F0 = J + (size_t)Nb * n * n;
   double* dx = F0 + (size_t)Nb * n;
@@ -1474,16 +1483,19 @@ psr_status psr_solve_hybrid(const psr_mech* m, int64_t N, double* T, const doubl
     double* Tb = T + r0;
     double* Yb = Y + r0;
     cudaError_t e = launch_hybrid_init(nb, *o, dt_cur, dt_arg, mode, it, status + r0, n_newton ? n_newton + r0 : nullptr,
-                                       n_ptc ? n_ptc + r0 : nullptr, cs);
+                                       n_ptc ? n_ptc + r0 : nullptr, n_active, cs);
     if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (init)");
     for (int iter = 0; iter < o->max_iter; ++iter) {
       // error vector and Jacobian at the current estimates, the (shifted) solve, the per-reactor decisions
-      st = fd_jacobian_impl(m, nb, Tb, P + r0, Yb, Tin ? Tin + r0 : nullptr, Yin + r0, tau + r0, ld, J, F0, stream, "psr_solve_hybrid");
+      // (finished reactors are marked in dt_arg and counted in n_active: their tiles and systems are left out, and a
+      // round after the last one has finished costs three empty launches)
+      st = fd_jacobian_impl(m, nb, Tb, P + r0, Yb, Tin ? Tin + r0 : nullptr, Yin + r0, tau + r0, ld, J, F0, stream, "psr_solve_hybrid",
+                            dt_arg, n_active);
       if (st != PSR_OK) return st;
-      st = solve_impl("psr_solve_hybrid", nb, n, J, dx, info, F0, dt_arg, stream);
+      st = solve_impl("psr_solve_hybrid", nb, n, J, dx, info, F0, dt_arg, stream, n_active);
       if (st != PSR_OK) return st;
       e = launch_hybrid_update(nb, n, ld, *o, Tb, Yb, dx, info, dt_cur, dt_arg, mode, it, status + r0,
-                               n_newton ? n_newton + r0 : nullptr, n_ptc ? n_ptc + r0 : nullptr, cs);
+                               n_newton ? n_newton + r0 : nullptr, n_ptc ? n_ptc + r0 : nullptr, n_active, cs);
       if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (update)");
     }
   }

@@ -62,6 +62,7 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nthr = kJacWarps * 32;
 
+  if (a.skip_count && *a.skip_count == 0) return;   // (hybrid solver: every reactor has finished; uniform in the grid)
   if (threadIdx.x == 0) {
     mbar_init(bar, 1);
     for (int q = 0; q < 2 * kJacWarps; ++q) mbar_init(bar + 2 + q, 1);
@@ -91,6 +92,12 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
   uint32_t n_iss = 0, n_use = 0;   // staging chunks this warp has requested / consumed
 
   for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
+    if (a.skip_dt) {
+      // a tile whose reactors have all finished keeps its (unused) outputs: the same answer in every warp
+      const int64_t rs = tile * kTile + (threadIdx.x & 31);
+      const double d = rs < a.N ? a.skip_dt[rs] : __longlong_as_double(0x7ff8000000000000LL);
+      if (__all_sync(0xffffffffu, d != d)) continue;
+    }
     const int64_t r = tile * kTile + lane;
     const bool valid = r < a.N;
     const int64_t rc = valid ? r : a.N - 1;   // lanes past N repeat the last reactor (a valid state, nothing stored)

@@ -26,7 +26,7 @@ template <int RPL, bool PTC>
 __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const double* __restrict__ A,
                                                        double* __restrict__ b, int32_t* __restrict__ info,
                                                        int sys_doubles, const double* __restrict__ F,
-                                                       const double* __restrict__ dt) {
+                                                       const double* __restrict__ dt, const int32_t* __restrict__ skip_count) {
   extern __shared__ __align__(16) double sm[];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, wpc = blockDim.x >> 5;
   const int ld = n | 1;
@@ -34,7 +34,11 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
   double* bs = As + (size_t)n * ld;            // [n]
   double* dinv = bs + n;                       // [n] reciprocals of the pivots
 
+  // psr_solve_hybrid (skip_count non-null): nothing to do once every reactor has finished, and a finished reactor's
+  // system -- its dt is NaN -- is left out (dx, info unchanged and unused)
+  if (PTC && skip_count && *skip_count == 0) return;
   for (int64_t r = (int64_t)blockIdx.x * wpc + w; r < N; r += (int64_t)gridDim.x * wpc) {
+    if (PTC && skip_count && dt[r] != dt[r]) continue;
     const double* Ar = A + (size_t)r * n * n;
     // pseudo-transient step (psr_ptc_solve): the matrix is J + I/dt, the right-hand side -F
     const double shift = PTC ? 1.0 / dt[r] : 0.0;
@@ -242,7 +246,7 @@ __global__ void __launch_bounds__(128) lu_solve_kernel(int64_t N, int n, const d
 }
 
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
-                            cudaStream_t st, const double* F, const double* dt) {
+                            cudaStream_t st, const double* F, const double* dt, const int32_t* skip_count) {
   const int ld = n | 1;
   const int sys_doubles = n * ld + 2 * n + (n & 1);   // matrix, right-hand side, pivot reciprocals; even
   const size_t per_sys = (size_t)sys_doubles * 8;
@@ -269,7 +273,7 @@ cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_
       if (e != cudaSuccess) return e;                                                                        \
       raised[dt ? 1 : 0] = true;                                                                             \
     }                                                                                                        \
-    kern<<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles, F, dt);                           \
+    kern<<<(int)ctas, wpc * 32, smem, st>>>(N, n, A, b, info, sys_doubles, F, dt, skip_count);               \
     return cudaGetLastError();                                                                               \
   }
   PSR_LU(1) PSR_LU(2) PSR_LU(4) PSR_LU(6)

@@ -15,8 +15,9 @@ constexpr unsigned kAll = 0xffffffffu;
 enum : int32_t { kModeNewton = 0, kModePtc = 1, kModeDone = 2 };
 
 __global__ void hybrid_init_kernel(int64_t nb, psr_solve_opts o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
-                                   int32_t* status, int32_t* n_newton, int32_t* n_ptc) {
+                                   int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active) {
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r == 0) *n_active = (int32_t)nb;   // reactors still iterating (the block is at most 2^31 - 1 reactors: checked by the caller)
   if (r >= nb) return;
   dt_cur[r] = o.dt0;
   dt_arg[r] = INFINITY;   // Newton iteration: the pseudo-transient system without its shift
@@ -34,10 +35,12 @@ __global__ void __launch_bounds__(256) hybrid_update_kernel(int64_t nb, int n, i
                                                             const int32_t* __restrict__ info, double* __restrict__ dt_cur,
                                                             double* __restrict__ dt_arg, int32_t* __restrict__ mode,
                                                             int32_t* __restrict__ it, int32_t* __restrict__ status,
-                                                            int32_t* __restrict__ n_newton, int32_t* __restrict__ n_ptc) {
+                                                            int32_t* __restrict__ n_newton, int32_t* __restrict__ n_ptc,
+                                                            int32_t* __restrict__ n_active) {
   const int lane = threadIdx.x & 31;
   const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (r >= nb) return;
+  if (*reinterpret_cast<volatile int32_t*>(n_active) == 0) return;   // every reactor finished in an earlier round
   const int32_t md = mode[r];
   if (md == kModeDone) return;
   // trial x' = x + dx; admissible when the system solved to a finite dx and every mass fraction stays >= -y_floor
@@ -100,21 +103,24 @@ __global__ void __launch_bounds__(256) hybrid_update_kernel(int64_t nb, int n, i
     mode[r] = new_mode;
     it[r] = k;
     dt_cur[r] = dtc;
-    dt_arg[r] = new_mode == kModePtc ? dtc : INFINITY;
+    // a finished reactor is marked with dt = NaN: the Jacobian and solve launches of the remaining rounds leave it
+    // out (psr_jac.cu: tiles whose reactors have all finished; psr_lu.cu: its system), and n_active counts the rest
+    dt_arg[r] = new_mode == kModeDone ? __longlong_as_double(0x7ff8000000000000LL) : new_mode == kModePtc ? dtc : INFINITY;
+    if (new_mode == kModeDone) atomicSub(n_active, 1);
   }
 }
 
 cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
-                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, cudaStream_t st) {
-  hybrid_init_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(nb, o, dt_cur, dt_arg, mode, it, status, n_newton, n_ptc);
+                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st) {
+  hybrid_init_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(nb, o, dt_cur, dt_arg, mode, it, status, n_newton, n_ptc, n_active);
   return cudaGetLastError();
 }
 
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
                                  const int32_t* info, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it, int32_t* status,
-                                 int32_t* n_newton, int32_t* n_ptc, cudaStream_t st) {
+                                 int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st) {
   hybrid_update_kernel<<<(unsigned)((nb * 32 + 255) / 256), 256, 0, st>>>(nb, n, ld, o, T, Y, dx, info, dt_cur, dt_arg, mode, it,
-                                                                          status, n_newton, n_ptc);
+                                                                          status, n_newton, n_ptc, n_active);
   return cudaGetLastError();
 }
 

@@ -236,6 +236,10 @@ struct EvalArgs {
   double* F0out;          // residual mode: also write [N][K+1] base residual (row 0 = 0)
   uint32_t flags;
   int64_t n_tiles;
+  // psr_solve_hybrid only (null elsewhere): reactors whose skip_dt entry is NaN are finished -- a tile of finished
+  // reactors is left out -- and *skip_count is the number of reactors still active (0: the launch does nothing)
+  const double* skip_dt;
+  const int32_t* skip_count;
 };
 
 }  // namespace psr

@@ -902,6 +902,50 @@ def test_solve_hybrid_on_C4_from_far_and_from_perturbed_converged_states(torch_c
     assert (np.abs(got1["Y"] - ref["Y"][:, conv]) / w)[:, ok].max() <= 1.0     # back at the solution it was perturbed from
 
 
+@pytest.mark.parametrize("generic", [False, True])
+def test_solve_hybrid_rounds_after_convergence_change_nothing(torch_cuda, binding, generic):
+    """Finished reactors are marked on the device (their tiles of the fused Jacobian kernel and their linear systems are
+    left out, and once none is left a round is three empty launches).  So the budget beyond the last reactor's
+    convergence must change no output: 14 rounds and 300 rounds give the same bits -- with sub-batches (the counter is
+    per sub-batch), with a batch in which some reactors never finish, and on both Jacobian paths."""
+    torch = torch_cuda
+    mech, batch = synth.make_config("C4", 160)
+    gm = binding.Mechanism.from_synth(mech)
+    gm.set_option(binding.OPT_JAC_GENERIC, 1 if generic else 0)
+    P, Yin, tau = (dev(torch, x) for x in (batch.P, batch.Yin, batch.tau))
+    kw = dict(SOLVE_KW, max_iter=300)
+    ws = torch.empty(int(binding.lib().psr_solve_hybrid_workspace_bytes(gm._h, 64)), dtype=torch.uint8, device="cuda")   # 3 sub-batches
+    T, Y = dev(torch, batch.T), dev(torch, batch.Y)
+    st, nn, npt = gm.solve_hybrid(T, P, Y, Yin, tau, workspace=ws, **kw)
+    torch.cuda.synchronize()
+    conv = (st == 0).cpu().numpy()
+    assert 0.8 < conv.mean() < 1.0 or conv.all()          # the far start leaves a few reactors unfinished
+    # restart from the finished reactors' solutions, perturbed: every one converges within a few Newton iterations
+    rng = np.random.default_rng(5)
+    idx = np.flatnonzero(conv)
+    Y1 = Y.cpu().numpy()[:, idx] * (1.0 + 0.01 * rng.uniform(-1, 1, (mech.n_species, idx.size)))
+    T1 = T.cpu().numpy()[idx]
+    sub = batch.take(idx)
+    outs = []
+    for max_iter in (14, 300):
+        Tt, Yt = dev(torch, T1), dev(torch, Y1)
+        s1, n1, p1 = gm.solve_hybrid(Tt, dev(torch, sub.P), Yt, dev(torch, sub.Yin), dev(torch, sub.tau), workspace=ws,
+                                     **dict(SOLVE_KW, atol=1e-10, rtol=1e-5, max_iter=max_iter, max_newton=12))
+        torch.cuda.synchronize()
+        outs.append([x.cpu().numpy() for x in (Tt, Yt, s1, n1, p1)])
+    assert (outs[0][2] == 0).all() and outs[0][3].max() <= 12
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b)
+    # and the mixed batch: a budget cut short against the full one agree on every reactor that had finished by then
+    Tt, Yt = dev(torch, batch.T), dev(torch, batch.Y)
+    s2, n2, p2 = gm.solve_hybrid(Tt, P, Yt, Yin, tau, workspace=ws, **dict(SOLVE_KW, max_iter=200))
+    torch.cuda.synchronize()
+    early = (s2 == 0).cpu().numpy()
+    assert early.any() and np.array_equal(Yt.cpu().numpy()[:, early], Y.cpu().numpy()[:, early])
+    assert np.array_equal(n2.cpu().numpy()[early], nn.cpu().numpy()[early]) and np.array_equal(p2.cpu().numpy()[early], npt.cpu().numpy()[early])
+    gm.close()
+
+
 def test_solve_hybrid_adiabatic_and_argument_checks(torch_cuda, binding):
     """Tin given: row 0 of the system is the energy row and T is solved for.  An inert mechanism settles at
     (T_in, Y_in) on the same path as the oracle.  (With chemistry the adiabatic systems of these synthetic mechanisms
