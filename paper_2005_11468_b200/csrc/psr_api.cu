@@ -23,6 +23,13 @@ cudaError_t launch_probe(int kind, int iters, int grid, double* sink, cudaStream
 cudaError_t launch_lu_solve(int64_t N, int n, const double* A, double* b, int32_t* info, int n_sm, size_t smem_optin,
                             cudaStream_t st, const double* F, const double* dt, const int32_t* skip_count);
 cudaError_t launch_exp_values(const double* tab, const double* x, double* y, int n, cudaStream_t st);
+cudaError_t launch_hybrid_gather(int64_t nb, int K, int64_t ld, const double* T, const double* P, const double* Y, const double* Tin,
+                                 const double* Yin, const double* tau, const HybridState& s, const psr_solve_opts& o, int32_t* n_active,
+                                 cudaStream_t st);
+cudaError_t launch_hybrid_compact(int64_t nb, int K, const HybridState& src, const HybridState& dst, int32_t* pos, const int32_t* n_active,
+                                  cudaStream_t st);
+cudaError_t launch_hybrid_scatter(int64_t nb, int K, int64_t ld, const HybridState& s, double* T, double* Y, int32_t* status,
+                                  int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
 cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
                                int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st);
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
@@ -1438,15 +1445,41 @@ psr_status psr_ptc_solve(int64_t N, int32_t n, const double* J, const double* F,
 }
 
 namespace {
-// workspace of the hybrid solver per reactor: J, F0, dx, the two dt arrays (doubles); info, mode, it (int32); and once
-// per call the counter of reactors still iterating
-size_t hybrid_bytes_per_reactor(int n) { return ((size_t)n * n + 2 * (size_t)n + 2) * 8 + 3 * 4 + 4; }
-constexpr size_t kHybridFixedBytes = 256;
+// workspace of the hybrid solver.  Per reactor: J, F0, dx (doubles), info and the partition's destination (int32), and
+// two copies of the sub-batch's state (HybridState: 2 K + 6 double rows, 6 int32 rows) between which the reactors still
+// iterating are moved to the front every kHybridCompactEvery rounds.  Once per call: the counter of active reactors,
+// and the padding of the state rows to a stride of a multiple of 32 reactors.
+constexpr int kHybridCompactEvery = 8;
+size_t hybrid_state_bytes_per_reactor(int n) { return ((size_t)2 * n + 4) * 8 + 6 * 4; }
+size_t hybrid_bytes_per_reactor(int n) { return ((size_t)n * n + 2 * (size_t)n) * 8 + 2 * 4 + 2 * hybrid_state_bytes_per_reactor(n); }
+size_t hybrid_fixed_bytes(int n) { return 256 + 32 * 2 * hybrid_state_bytes_per_reactor(n) + 256; }
+
+// carves a state of row stride ldw out of the workspace: double rows at d (2 K + 6 of them), int32 rows at q (6)
+HybridState hybrid_state_at(double* d, int32_t* q, int K, int64_t ldw, bool adiabatic) {
+  HybridState s{};
+  s.ldw = ldw;
+  s.T = d;
+  s.P = d + ldw;
+  s.tau = d + 2 * ldw;
+  s.Tin = adiabatic ? d + 3 * ldw : nullptr;
+  s.Y = d + 4 * ldw;
+  s.Yin = s.Y + (size_t)K * ldw;
+  s.dt_cur = s.Yin + (size_t)K * ldw;
+  s.dt_arg = s.dt_cur + ldw;
+  s.mode = q;
+  s.it = q + ldw;
+  s.status = q + 2 * ldw;
+  s.nn = q + 3 * ldw;
+  s.np = q + 4 * ldw;
+  s.orig = q + 5 * ldw;
+  return s;
+}
 }  // namespace
 
 size_t psr_solve_hybrid_workspace_bytes(const psr_mech* m, int64_t N) {
   if (!m || N < 1) return 0;
-  return hybrid_bytes_per_reactor(m->view.K + 1) * (size_t)N + 256 + kHybridFixedBytes;
+  const int n = m->view.K + 1;
+  return hybrid_bytes_per_reactor(n) * (size_t)N + hybrid_fixed_bytes(n) + 256;
 }
 
 psr_status psr_solve_hybrid(const psr_mech* m, int64_t N, double* T, const double* P, double* Y, const double* Tin,
@@ -1459,45 +1492,56 @@ psr_status psr_solve_hybrid(const psr_mech* m, int64_t N, double* T, const doubl
   if (!(o->atol >= 0.0) || !(o->rtol >= 0.0) || !(o->atol + o->rtol > 0.0) || o->max_iter < 0 || o->max_newton < 1 || o->max_ptc < 1 ||
       !(o->dt0 > 0.0) || !(o->dt_grow > 0.0) || !(o->dt_shrink > 0.0) || std::isnan(o->y_floor))
     return fail(PSR_EINVAL, "psr_solve_hybrid: options out of range (atol, rtol >= 0 and not both 0; max_iter >= 0; max_newton, max_ptc >= 1; dt0, dt_grow, dt_shrink > 0)");
-  const int n = m->view.K + 1;
+  const int K = m->view.K, n = K + 1;
   if (n > 168) return fail(PSR_EUNSUPPORTED, "psr_solve_hybrid: %d unknowns, the linear solve takes <= 168", n);
   uintptr_t base = (reinterpret_cast<uintptr_t>(workspace) + 255) & ~(uintptr_t)255;
   const size_t lost = base - reinterpret_cast<uintptr_t>(workspace);
-  if (workspace_bytes <= lost + kHybridFixedBytes + hybrid_bytes_per_reactor(n))
+  if (workspace_bytes <= lost + hybrid_fixed_bytes(n) + hybrid_bytes_per_reactor(n))
     return fail(PSR_EINVAL, "psr_solve_hybrid: workspace smaller than one reactor needs");
   const int64_t Nb = std::min<int64_t>(std::min<int64_t>(N, (int64_t)1 << 30),
-                                      (int64_t)((workspace_bytes - lost - kHybridFixedBytes) / hybrid_bytes_per_reactor(n)));
-  int32_t* n_active = reinterpret_cast<int32_t*>(base);   // reactors of the block still iterating (device counter)
-  base += kHybridFixedBytes;
-  double* J = reinterpret_cast<double*>(base);
+                                      (int64_t)((workspace_bytes - lost - hybrid_fixed_bytes(n)) / hybrid_bytes_per_reactor(n)));
+  const int64_t ldw = (Nb + 31) & ~(int64_t)31;
+  int32_t* n_active = reinterpret_cast<int32_t*>(base);   // reactors of the sub-batch still iterating (device counter)
+  double* J = reinterpret_cast<double*>(base + 256);
   double* F0 = J + (size_t)Nb * n * n;
   double* dx = F0 + (size_t)Nb * n;
-  double* dt_cur = dx + (size_t)Nb * n;
-  double* dt_arg = dt_cur + Nb;
-  int32_t* info = reinterpret_cast<int32_t*>(dt_arg + Nb);
-  int32_t* mode = info + Nb;
-  int32_t* it = mode + Nb;
+  double* sd0 = dx + (size_t)Nb * n;                       // double rows of the two states
+  double* sd1 = sd0 + (size_t)(2 * K + 6) * ldw;
+  int32_t* sq0 = reinterpret_cast<int32_t*>(sd1 + (size_t)(2 * K + 6) * ldw);
+  int32_t* sq1 = sq0 + 6 * ldw;
+  int32_t* info = sq1 + 6 * ldw;
+  int32_t* pos = info + Nb;
+  HybridState hs[2] = {hybrid_state_at(sd0, sq0, K, ldw, Tin != nullptr), hybrid_state_at(sd1, sq1, K, ldw, Tin != nullptr)};
   cudaStream_t cs = (cudaStream_t)stream;
   for (int64_t r0 = 0; r0 < N; r0 += Nb) {
     const int64_t nb = std::min(Nb, N - r0);
-    double* Tb = T + r0;
-    double* Yb = Y + r0;
-    cudaError_t e = launch_hybrid_init(nb, *o, dt_cur, dt_arg, mode, it, status + r0, n_newton ? n_newton + r0 : nullptr,
-                                       n_ptc ? n_ptc + r0 : nullptr, n_active, cs);
-    if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (init)");
+    int cur = 0;
+    // the sub-batch's state into the workspace (the caller's P, Y_in, tau are not to be reordered in place)
+    cudaError_t e = launch_hybrid_gather(nb, K, ld, T + r0, P + r0, Y + r0, Tin ? Tin + r0 : nullptr, Yin + r0, tau + r0, hs[cur], *o,
+                                         n_active, cs);
+    if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (gather)");
     for (int iter = 0; iter < o->max_iter; ++iter) {
+      if (iter > 0 && iter % kHybridCompactEvery == 0) {
+        // the reactors still iterating to the front (stable), so that finished ones fill whole tiles and drop out of
+        // the Jacobian kernel; on a fixed schedule: nothing returns to the host
+        e = launch_hybrid_compact(nb, K, hs[cur], hs[cur ^ 1], pos, n_active, cs);
+        if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (compaction)");
+        cur ^= 1;
+      }
+      const HybridState& s = hs[cur];
       // error vector and Jacobian at the current estimates, the (shifted) solve, the per-reactor decisions
       // (finished reactors are marked in dt_arg and counted in n_active: their tiles and systems are left out, and a
-      // round after the last one has finished costs three empty launches)
-      st = fd_jacobian_impl(m, nb, Tb, P + r0, Yb, Tin ? Tin + r0 : nullptr, Yin + r0, tau + r0, ld, J, F0, stream, "psr_solve_hybrid",
-                            dt_arg, n_active);
+      // round after the last one has finished costs a few empty launches)
+      st = fd_jacobian_impl(m, nb, s.T, s.P, s.Y, s.Tin, s.Yin, s.tau, ldw, J, F0, stream, "psr_solve_hybrid", s.dt_arg, n_active);
       if (st != PSR_OK) return st;
-      st = solve_impl("psr_solve_hybrid", nb, n, J, dx, info, F0, dt_arg, stream, n_active);
+      st = solve_impl("psr_solve_hybrid", nb, n, J, dx, info, F0, s.dt_arg, stream, n_active);
       if (st != PSR_OK) return st;
-      e = launch_hybrid_update(nb, n, ld, *o, Tb, Yb, dx, info, dt_cur, dt_arg, mode, it, status + r0,
-                               n_newton ? n_newton + r0 : nullptr, n_ptc ? n_ptc + r0 : nullptr, n_active, cs);
+      e = launch_hybrid_update(nb, n, ldw, *o, s.T, s.Y, dx, info, s.dt_cur, s.dt_arg, s.mode, s.it, s.status, s.nn, s.np, n_active, cs);
       if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (update)");
     }
+    e = launch_hybrid_scatter(nb, K, ld, hs[cur], T + r0, Y + r0, status + r0, n_newton ? n_newton + r0 : nullptr,
+                              n_ptc ? n_ptc + r0 : nullptr, cs);
+    if (e != cudaSuccess) return cuda_fail(e, "psr_solve_hybrid (scatter)");
   }
   return PSR_OK;
 }

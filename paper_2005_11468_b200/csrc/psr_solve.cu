@@ -8,6 +8,7 @@
 #include <stdint.h>
 
 #include "../../include/psr.h"
+#include "psr_tables.h"
 
 namespace psr {
 
@@ -121,6 +122,153 @@ cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_
                                  int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st) {
   hybrid_update_kernel<<<(unsigned)((nb * 32 + 255) / 256), 256, 0, st>>>(nb, n, ld, o, T, Y, dx, info, dt_cur, dt_arg, mode, it,
                                                                           status, n_newton, n_ptc, n_active);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ compaction of the reactors still iterating
+// psr_solve_hybrid works on a copy of the sub-batch's state in its workspace (HybridState, two of them).  Every few
+// rounds the reactors are partitioned -- the ones still iterating first, in their order, the finished ones behind
+// them -- into the other copy: finished reactors then fill whole tiles of 32, which the Jacobian kernel leaves out
+// (psr_jac.cu), so that a round costs what the active reactors cost.  A reactor's arithmetic does not depend on its
+// position, so its path is the same with or without the moves.
+
+// rows of a state: T, P, tau, Tin, Y[0..K), Yin[0..K) (doubles, row stride ldw), then dt_cur, dt_arg, then the integers
+__device__ __forceinline__ double* hs_row(const HybridState& s, int row, int K) {
+  if (row == 0) return s.T;
+  if (row == 1) return s.P;
+  if (row == 2) return s.tau;
+  if (row == 3) return s.Tin;
+  if (row < 4 + K) return s.Y + (int64_t)(row - 4) * s.ldw;
+  if (row < 4 + 2 * K) return s.Yin + (int64_t)(row - 4 - K) * s.ldw;
+  return row == 4 + 2 * K ? s.dt_cur : s.dt_arg;
+}
+
+// the caller's arrays of the sub-batch into a state; bookkeeping initialised (grid.y: rows; the last row: integers)
+__global__ void hybrid_gather_kernel(int64_t nb, int K, int64_t ld, const double* T, const double* P, const double* Y, const double* Tin,
+                                     const double* Yin, const double* tau, HybridState s, psr_solve_opts o, int32_t* n_active) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int row = blockIdx.y;
+  if (row == 0 && r == 0) *n_active = (int32_t)nb;
+  if (r >= nb) return;
+  if (row == 0) s.T[r] = T[r];
+  else if (row == 1) s.P[r] = P[r];
+  else if (row == 2) s.tau[r] = tau[r];
+  else if (row == 3) { if (Tin) s.Tin[r] = Tin[r]; }
+  else if (row < 4 + K) s.Y[(int64_t)(row - 4) * s.ldw + r] = Y[(int64_t)(row - 4) * ld + r];
+  else if (row < 4 + 2 * K) s.Yin[(int64_t)(row - 4 - K) * s.ldw + r] = Yin[(int64_t)(row - 4 - K) * ld + r];
+  else if (row == 4 + 2 * K) {
+    s.dt_cur[r] = o.dt0;
+    s.dt_arg[r] = INFINITY;   // Newton iteration: the pseudo-transient system without its shift
+  } else {
+    s.mode[r] = kModeNewton;
+    s.it[r] = 0;
+    s.status[r] = 1;
+    s.nn[r] = 0;
+    s.np[r] = 0;
+    s.orig[r] = (int32_t)r;
+  }
+}
+
+// destination of every reactor under the stable partition (active first); one CTA walks the sub-batch
+__global__ void __launch_bounds__(1024) hybrid_scan_kernel(int64_t nb, const int32_t* __restrict__ mode, const int32_t* __restrict__ n_active,
+                                                            int32_t* __restrict__ pos) {
+  __shared__ int32_t wsum[32];
+  __shared__ int32_t base_s;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int32_t n_act = *n_active;
+  if (n_act == 0) return;   // nothing iterates any more: the order no longer matters
+  if (threadIdx.x == 0) base_s = 0;
+  __syncthreads();
+  for (int64_t c0 = 0; c0 < nb; c0 += 1024) {
+    const int64_t r = c0 + threadIdx.x;
+    const int f = (r < nb && mode[r] != kModeDone) ? 1 : 0;
+    int v = f;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int u = __shfl_up_sync(kAll, v, d);
+      if (lane >= d) v += u;
+    }
+    if (lane == 31) wsum[w] = v;
+    __syncthreads();
+    if (w == 0) {
+      int t = wsum[lane];
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int u = __shfl_up_sync(kAll, t, d);
+        if (lane >= d) t += u;
+      }
+      wsum[lane] = t;   // inclusive sums of the warps' totals
+    }
+    __syncthreads();
+    const int32_t base = base_s;
+    const int32_t before = base + (w ? wsum[w - 1] : 0) + v - f;   // active reactors in front of r
+    if (r < nb) pos[r] = f ? before : n_act + (int32_t)(r - before);
+    __syncthreads();
+    if (threadIdx.x == 0) base_s = base + wsum[31];
+    __syncthreads();
+  }
+}
+
+__global__ void hybrid_permute_kernel(int64_t nb, int K, HybridState src, HybridState dst, const int32_t* __restrict__ pos,
+                                      const int32_t* __restrict__ n_active) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int row = blockIdx.y;
+  if (r >= nb) return;
+  // (nothing iterates any more: no partition was formed; the copy is still made, in place order, because the host side
+  // swaps the two states on a fixed schedule)
+  const int64_t d = *n_active == 0 ? r : (int64_t)pos[r];
+  if (row < 6 + 2 * K) {
+    if (row == 3 && !src.Tin) return;
+    hs_row(dst, row, K)[d] = hs_row(src, row, K)[r];
+  } else {
+    dst.mode[d] = src.mode[r];
+    dst.it[d] = src.it[r];
+    dst.status[d] = src.status[r];
+    dst.nn[d] = src.nn[r];
+    dst.np[d] = src.np[r];
+    dst.orig[d] = src.orig[r];
+  }
+}
+
+// the state back into the caller's arrays, every reactor at the index it came from
+__global__ void hybrid_scatter_kernel(int64_t nb, int K, int64_t ld, HybridState s, double* T, double* Y, int32_t* status, int32_t* n_newton,
+                                      int32_t* n_ptc) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int row = blockIdx.y;
+  if (r >= nb) return;
+  const int64_t o = s.orig[r];
+  if (row == 0) {
+    T[o] = s.T[r];
+    status[o] = s.status[r];
+    if (n_newton) n_newton[o] = s.nn[r];
+    if (n_ptc) n_ptc[o] = s.np[r];
+  } else {
+    Y[(int64_t)(row - 1) * ld + o] = s.Y[(int64_t)(row - 1) * s.ldw + r];
+  }
+}
+
+cudaError_t launch_hybrid_gather(int64_t nb, int K, int64_t ld, const double* T, const double* P, const double* Y, const double* Tin,
+                                 const double* Yin, const double* tau, const HybridState& s, const psr_solve_opts& o, int32_t* n_active,
+                                 cudaStream_t st) {
+  const dim3 grid((unsigned)((nb + 255) / 256), (unsigned)(2 * K + 6));
+  hybrid_gather_kernel<<<grid, 256, 0, st>>>(nb, K, ld, T, P, Y, Tin, Yin, tau, s, o, n_active);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_hybrid_compact(int64_t nb, int K, const HybridState& src, const HybridState& dst, int32_t* pos, const int32_t* n_active,
+                                  cudaStream_t st) {
+  hybrid_scan_kernel<<<1, 1024, 0, st>>>(nb, src.mode, n_active, pos);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const dim3 grid((unsigned)((nb + 255) / 256), (unsigned)(2 * K + 7));
+  hybrid_permute_kernel<<<grid, 256, 0, st>>>(nb, K, src, dst, pos, n_active);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_hybrid_scatter(int64_t nb, int K, int64_t ld, const HybridState& s, double* T, double* Y, int32_t* status,
+                                  int32_t* n_newton, int32_t* n_ptc, cudaStream_t st) {
+  const dim3 grid((unsigned)((nb + 255) / 256), (unsigned)(K + 1));
+  hybrid_scatter_kernel<<<grid, 256, 0, st>>>(nb, K, ld, s, T, Y, status, n_newton, n_ptc);
   return cudaGetLastError();
 }
 

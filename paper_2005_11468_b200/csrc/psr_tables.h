@@ -242,5 +242,14 @@ struct EvalArgs {
   const int32_t* skip_count;
 };
 
+// ---- psr_solve_hybrid: a sub-batch's state in the workspace (psr_solve.cu); row stride of Y, Yin: ldw
+struct HybridState {
+  double *T, *P, *tau, *Tin;   // [ldw]; Tin: null for the isothermal system
+  double *Y, *Yin;             // [K][ldw]
+  double *dt_cur, *dt_arg;     // [ldw]
+  int32_t *mode, *it, *status, *nn, *np, *orig;   // [ldw]; orig: the reactor's index in the caller's sub-batch
+  int64_t ldw;
+};
+
 }  // namespace psr
 #endif
