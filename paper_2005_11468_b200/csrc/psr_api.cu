@@ -30,8 +30,6 @@ cudaError_t launch_hybrid_compact(int64_t nb, int K, const HybridState& src, con
                                   cudaStream_t st);
 cudaError_t launch_hybrid_scatter(int64_t nb, int K, int64_t ld, const HybridState& s, double* T, double* Y, int32_t* status,
                                   int32_t* n_newton, int32_t* n_ptc, cudaStream_t st);
-cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
-                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st);
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
                                  const int32_t* info, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it, int32_t* status,
                                  int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st);

@@ -15,20 +15,6 @@ namespace psr {
 constexpr unsigned kAll = 0xffffffffu;
 enum : int32_t { kModeNewton = 0, kModePtc = 1, kModeDone = 2 };
 
-__global__ void hybrid_init_kernel(int64_t nb, psr_solve_opts o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
-                                   int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active) {
-  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (r == 0) *n_active = (int32_t)nb;   // reactors still iterating (the block is at most 2^31 - 1 reactors: checked by the caller)
-  if (r >= nb) return;
-  dt_cur[r] = o.dt0;
-  dt_arg[r] = INFINITY;   // Newton iteration: the pseudo-transient system without its shift
-  mode[r] = kModeNewton;
-  it[r] = 0;
-  status[r] = 1;
-  if (n_newton) n_newton[r] = 0;
-  if (n_ptc) n_ptc[r] = 0;
-}
-
 // One step of every reactor's state machine (readings g22-g25), after the solve of
 // (I/dt_arg + J) dx = -F at the current estimate x = (T, Y).
 __global__ void __launch_bounds__(256) hybrid_update_kernel(int64_t nb, int n, int64_t ld, psr_solve_opts o, double* __restrict__ T,
@@ -109,12 +95,6 @@ __global__ void __launch_bounds__(256) hybrid_update_kernel(int64_t nb, int n, i
     dt_arg[r] = new_mode == kModeDone ? __longlong_as_double(0x7ff8000000000000LL) : new_mode == kModePtc ? dtc : INFINITY;
     if (new_mode == kModeDone) atomicSub(n_active, 1);
   }
-}
-
-cudaError_t launch_hybrid_init(int64_t nb, const psr_solve_opts& o, double* dt_cur, double* dt_arg, int32_t* mode, int32_t* it,
-                               int32_t* status, int32_t* n_newton, int32_t* n_ptc, int32_t* n_active, cudaStream_t st) {
-  hybrid_init_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(nb, o, dt_cur, dt_arg, mode, it, status, n_newton, n_ptc, n_active);
-  return cudaGetLastError();
 }
 
 cudaError_t launch_hybrid_update(int64_t nb, int n, int64_t ld, const psr_solve_opts& o, double* T, double* Y, const double* dx,
