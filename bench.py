@@ -497,8 +497,8 @@ def run_extras(binding, synth, torch, flush, only=None, cpu=True):
             out["C4_newton"] = {"call": "psr_fd_jacobian + psr_ptc_solve (one Newton iteration's device work)", "ms": ms_n,
                                 "iterations_per_s": batch.n / (ms_n * 1e-3)}
         if want("C4_hybrid"):
-            # NEXT-4: the whole hybrid solve from the generated (far) states, 2,048 reactors, fixed budget of 420 solves
-            nb = 2048
+            # NEXT-4: the whole hybrid solve from the generated (far) states, the full C4 batch, fixed budget of 420 solves
+            nb = 8192
             a0 = [x[..., :nb].contiguous() for x in (T, P, Y, Yin, tau)]
             kw = dict(atol=1e-12, rtol=1e-7, max_iter=420, max_newton=5, max_ptc=20, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9)
             ws = torch.empty(int(binding.lib().psr_solve_hybrid_workspace_bytes(gm._h, nb)), dtype=torch.uint8, device="cuda")
