@@ -37,6 +37,7 @@ cudaError_t chk_read_kernels(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_ws(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_jac(unsigned int* count, unsigned int* first_code);
 cudaError_t chk_read_wsl(unsigned int* count, unsigned int* first_code);
+cudaError_t chk_read_solve(unsigned int* count, unsigned int* first_code);
 cudaError_t wsl_set_smem(size_t smem);
 cudaError_t launch_wsl(const WslView& mv, const EvalArgs& a, int grid, int bulk_ok, int rx_tmem, cudaStream_t st);
 cudaError_t launch_chk_selftest(cudaStream_t st);
@@ -1568,7 +1569,7 @@ int32_t psr_check_failures(int32_t selftest, int32_t* first_code) {
     if (e != cudaSuccess) { cuda_fail(e, "psr_check_failures (self-test)"); return -2; }
   }
   unsigned int total = 0, first = 0;
-  cudaError_t (*readers[4])(unsigned int*, unsigned int*) = {chk_read_ws, chk_read_wsl, chk_read_jac, chk_read_kernels};
+  cudaError_t (*readers[5])(unsigned int*, unsigned int*) = {chk_read_ws, chk_read_wsl, chk_read_jac, chk_read_kernels, chk_read_solve};
   for (auto rd : readers) {
     unsigned int c = 0, code = 0;
     cudaError_t e = rd(&c, &code);

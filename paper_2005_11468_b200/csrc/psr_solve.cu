@@ -8,6 +8,7 @@
 #include <stdint.h>
 
 #include "../../include/psr.h"
+#include "psr_ptx.cuh"
 #include "psr_tables.h"
 
 namespace psr {
@@ -197,6 +198,7 @@ __global__ void hybrid_permute_kernel(int64_t nb, int K, HybridState src, Hybrid
   // (nothing iterates any more: no partition was formed; the copy is still made, in place order, because the host side
   // swaps the two states on a fixed schedule)
   const int64_t d = *n_active == 0 ? r : (int64_t)pos[r];
+  PSR_CHK(d >= 0 && d < nb, 601);   // the partition's destination is a reactor of the sub-batch
   if (row < 6 + 2 * K) {
     if (row == 3 && !src.Tin) return;
     hs_row(dst, row, K)[d] = hs_row(src, row, K)[r];
@@ -217,6 +219,7 @@ __global__ void hybrid_scatter_kernel(int64_t nb, int K, int64_t ld, HybridState
   const int row = blockIdx.y;
   if (r >= nb) return;
   const int64_t o = s.orig[r];
+  PSR_CHK(o >= 0 && o < nb, 602);   // the index a reactor came from
   if (row == 0) {
     T[o] = s.T[r];
     status[o] = s.status[r];
@@ -226,6 +229,8 @@ __global__ void hybrid_scatter_kernel(int64_t nb, int K, int64_t ld, HybridState
     Y[(int64_t)(row - 1) * ld + o] = s.Y[(int64_t)(row - 1) * s.ldw + r];
   }
 }
+
+PSR_CHK_TU_READER(chk_read_solve)
 
 cudaError_t launch_hybrid_gather(int64_t nb, int K, int64_t ld, const double* T, const double* P, const double* Y, const double* Tin,
                                  const double* Yin, const double* tau, const HybridState& s, const psr_solve_opts& o, int32_t* n_active,

@@ -1066,6 +1066,11 @@ for cfg, n in (("C0", None), ("C1", 2000), ("C3", 97), ("C2", 70), ("P5", 40)):
     if cfg in ("C0", "C1"):
         n1 = mech.n_species + 1
         gm.fd_jacobian_noalloc(*a, J=torch.empty((m, n1, n1), dtype=torch.float64, device="cuda"))
+        # the hybrid solver: 20 rounds, two compactions of the reactors still iterating (the partition's destinations
+        # and the scatter back are checked), in sub-batches
+        ws = torch.empty(int(binding.lib().psr_solve_hybrid_workspace_bytes(gm._h, 24)), dtype=torch.uint8, device="cuda")
+        gm.solve_hybrid(a[0].clone(), a[1], a[2].clone(), a[3], a[4], workspace=ws, atol=1e-10, rtol=1e-6, max_iter=20,
+                        max_newton=4, max_ptc=6, dt0=1e-9, dt_grow=2.0, dt_shrink=0.25, y_floor=1e-9)
     torch.cuda.synchronize()
     out[cfg] = binding.check_failures()
     gm.close()
@@ -1079,7 +1084,8 @@ def test_bounds_checked_build(torch_cuda):
     table-derived shared-memory offset (factor rows, q / rate-tile rows, gather entries, flush targets, scatter rows)
     and every global output index is asserted on the device.  Run in a process of its own (it loads another build of
     the library) on C0 in full, ragged C1 / C2 / C3 / P5 batches, every evaluation call, both evaluation kernels, both
-    Jacobian paths, the energy row and the no-alloc entry point.  A self-test trips one assertion first: zero failures
+    Jacobian paths, the energy row, the no-alloc entry point and the hybrid solver with its compaction.  A self-test
+    trips one assertion first: zero failures
     afterwards means the checks ran and held.  It finds out-of-range indices -- not races, not uninitialised reads."""
     import subprocess
     import sys
