@@ -847,10 +847,13 @@ psr_status psr_mech_load(const psr_mech_desc* d, psr_mech** out) {
         o += align_up((size_t)(K + 2) * kTile * 8, 128);
         jv.smem_d = (uint32_t)o;
         o += align_up((size_t)n_cls * K * kTile * 8, 128);
-        jv.smem_ar = (uint32_t)o;   // phase 1: rate tile (+ zero row) and the F(T + h_T) tile; phase 2: one [K][32] tile per warp
-        o += align_up(std::max((size_t)kJacWarps * (K + 1) * kJacAccLd, ((size_t)jb.rows_max + 1 + K) * kTile) * 8, 128);
-        jv.smem_mech = (uint32_t)o;
-        o += jbs.stride;            // one part at a time
+        // phase 1: rate tile (+ zero row) and the F(T + h_T) tile, then the part being evaluated (one at a time, loaded
+        // again for every tile and pass).  Phase 2 reads neither: its per-warp [K + 1][33] tiles lie over both.
+        jv.smem_ar = (uint32_t)o;
+        const size_t ar1 = align_up(((size_t)jb.rows_max + 1 + K) * kTile * 8, 128);
+        const size_t ar2 = align_up((size_t)kJacWarps * (K + 1) * kJacAccLd * 8, 128);
+        jv.smem_mech = (uint32_t)(o + ar1);
+        o += std::max(ar1 + jbs.stride, ar2);
         jv.smem_misc = (uint32_t)o;
         o += align_up((size_t)2 * Kp * 8 + (size_t)kJacStRows * kTile * 8 + (2 + 2 * kJacWarps) * 8, 128);
         jv.smem_stage = (uint32_t)o;   // per warp: two chunks of kJacStage incidence records

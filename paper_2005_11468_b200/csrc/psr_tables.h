@@ -162,7 +162,7 @@ struct WslView {
 // ---- fused finite-difference Jacobian kernel (psr_jac.cu): lane <-> reactor, one CTA per tile of 32 reactors.
 // Phase 1 evaluates the tile (at T + h_T, then at T) and sums the forward and reverse rates of every reaction
 // into per-species sums BY CONCENTRATION ORDER; phase 2 builds the K species columns from them, warp <-> column.
-constexpr int kJacWarps = 8;
+constexpr int kJacWarps = 10;
 constexpr int kJacMaxOrder = 6;   // highest concentration order of a rate term the kernel takes (else: the generic sweep)
 constexpr int kJacAccLd = 33;     // row stride (doubles) of a warp's phase-2 tile: conflict-free by rows and by columns
 constexpr int kJacStage = 8;       // incidence records per staging chunk of a warp (two chunks in flight)
