@@ -48,8 +48,9 @@ __global__ void __launch_bounds__(kJacWarps * 32, 1) psr_jac_kernel(const JacVie
   double* Cs = reinterpret_cast<double*>(smem + jv.smem_cs);        // [K+2][32]: C_i; rows K, K+1: ones, zeros
   double* Dt = reinterpret_cast<double*>(smem + jv.smem_d);         // [n_cls][K][32]: D_i^(n)
   double* AR = reinterpret_cast<double*>(smem + jv.smem_ar);        // phase 1: rate tile [rows_max+1][32], then Fp [K][32];
-                                                                    // phase 2: [kJacWarps][K][32]
-  unsigned char* blob = smem + jv.smem_mech;                        // the part being evaluated
+                                                                    // phase 2: [kJacWarps][K+1][33], over this region AND the
+                                                                    // blob behind it (phase 2 reads neither: psr_api.cu)
+  unsigned char* blob = smem + jv.smem_mech;                        // the part being evaluated (phase 1; loaded per tile and pass)
   double* invW_s = reinterpret_cast<double*>(smem + jv.smem_misc);  // [Kp]
   const int Kp = (K + 1) & ~1;
   double* W_s = invW_s + Kp;                                        // [Kp]
