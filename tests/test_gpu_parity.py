@@ -91,6 +91,35 @@ def test_configs_ragged_batches(torch_cuda, binding, cfg, n):
     check_against_oracle(mech, batch, got)
 
 
+@pytest.mark.parametrize("K,I,tb,troe,n,expect", [
+    (230, 900, 70, 60, 5 * 148 * 32 // 16 + 19, dict(eval_kernel=2, eval_acc_global=1)),   # tile copy in tensor memory, sums in L2
+    (127, 100, 8, 6, 333, dict(eval_kernel=1)),                                             # resident kernel, K + 2 > 128: no copy
+    (96, 700, 50, 40, 333, dict(eval_kernel=2, eval_acc_global=0)),                        # streamed parts, sums in shared memory
+])
+def test_kernel_variants_between_the_configs(torch_cuda, binding, K, I, tb, troe, n, expect):
+    """The BASELINE configs land on four of the evaluation kernels' variants (resident with the tensor-memory copy: C1;
+    streamed with tile and sums in tensor memory: C2; streamed without tensor memory, sums in L2: C3; sums in shared
+    memory: P5).  Mechanisms sized to take the others, against the oracle like every config, and with the
+    tensor-memory switch off."""
+    torch = torch_cuda
+    mech = synth.make_mechanism(n_species=K, n_reactions=I, n_third_body=tb, n_troe=troe, seed=4242 + K, mmax=3)
+    batch = synth.make_states(K, n, seed=99 + K)
+    gm = binding.Mechanism.from_synth(mech)
+    info = gm.info()
+    for k, v in expect.items():
+        assert info[k] == v, (k, info)
+    gm.close()
+    got = gpu_eval(torch, binding, mech, batch)
+    check_against_oracle(mech, batch, got)
+    gm = binding.Mechanism.from_synth(mech)
+    T, P, Y, Yin, tau = (dev(torch, x) for x in (batch.T, batch.P, batch.Y, batch.Yin, batch.tau))
+    F0, w0 = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+    gm.set_option(binding.OPT_NO_TMEM, 1)
+    F1, w1 = gm.eval_residual(T, P, Y, Yin, tau, want_wdot=True)
+    assert torch.equal(F0, F1) and torch.equal(w0, w1)
+    gm.close()
+
+
 def test_T3_goldens_direct(torch_cuda, binding):
     """The GPU path against the paper-derived T3 values themselves (tests/golden/t3_pins.json)."""
     gold = json.loads((Path(__file__).parent / "golden" / "t3_pins.json").read_text())
